@@ -1,0 +1,159 @@
+"""ctypes loader for the CPU oracle (oracle/qmc_oracle.cpp).
+
+TEST INFRASTRUCTURE: only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+--impl reference leg may import this package.  The product (paper_1811_11720_b200) never does.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "qmc_oracle.cpp")
+_LIB = os.path.join(_HERE, "libqmc_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """g++ -O2 -std=c++17 -ffp-contract=off: no fast-math, no contraction (std::fma is explicit)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", _SRC, "-o", _LIB]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        L = C.CDLL(_LIB)
+        dp, up = C.POINTER(C.c_double), C.POINTER(C.c_uint64)
+        L.oracle_num_threads.restype = C.c_int
+        L.oracle_lattice_points.argtypes = [C.c_uint64, C.c_int, up, dp, C.c_uint64, C.c_uint64, up, dp]
+        L.oracle_transform.argtypes = [C.c_int, C.c_double, dp, dp]
+        L.oracle_fit_map.argtypes = [dp, C.c_double, dp, dp]
+        L.oracle_integrand.argtypes = [C.c_int, dp, C.c_int, C.c_int, dp, dp]
+        L.oracle_shift_sums.argtypes = [C.c_int, dp, C.c_int, C.c_int, C.c_uint64, up, dp, C.c_int, C.c_int, dp,
+                                        C.c_uint64, C.c_uint64, dp]
+        L.oracle_finalize.argtypes = [dp, C.c_int, C.c_int, dp, dp]
+        L.oracle_integrate.argtypes = [C.c_int, dp, C.c_int, C.c_int, C.c_uint64, up, dp, C.c_int, C.c_int, dp, dp, dp, dp]
+        L.oracle_project.argtypes = [C.c_int, dp, C.c_int, C.c_int, C.c_uint64, up, dp, C.c_int, dp]
+        L.oracle_fit_cubic.argtypes = [dp, C.c_int, C.c_int, dp]
+        _lib = L
+    return _lib
+
+
+def _d(a):
+    return None if a is None else a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _u(a):
+    return None if a is None else a.ctypes.data_as(C.POINTER(C.c_uint64))
+
+
+def _f64(a):
+    return None if a is None else np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _u64(a):
+    return np.ascontiguousarray(a, dtype=np.uint64)
+
+
+def num_threads() -> int:
+    return int(lib().oracle_num_threads())
+
+
+def ncomp(family: int) -> int:
+    return 2 if family == 2 else 1
+
+
+def lattice_points(n, z, shift, k0, count):
+    z, shift = _u64(z), _f64(shift)
+    d = len(z)
+    r = np.empty((count, d), dtype=np.uint64)
+    u = np.empty((count, d), dtype=np.float64)
+    st = lib().oracle_lattice_points(int(n), d, _u(z), _d(shift), int(k0), int(count), _u(r), _d(u))
+    assert st == 0
+    return r, u
+
+
+def transform(tr, u):
+    y, w = C.c_double(), C.c_double()
+    st = lib().oracle_transform(int(tr), float(u), C.byref(y), C.byref(w))
+    if st:
+        raise ValueError(f"oracle_transform status {st}")
+    return y.value, w.value
+
+
+def fit_map(a6, y):
+    a6 = _f64(a6)
+    x, dp = C.c_double(), C.c_double()
+    lib().oracle_fit_map(_d(a6), float(y), C.byref(x), C.byref(dp))
+    return x.value, dp.value
+
+
+def integrand(family, params, x):
+    params, x = _f64(params), _f64(x)
+    out = np.zeros(2)
+    st = lib().oracle_integrand(int(family), _d(params), len(params), len(x), _d(x), _d(out))
+    if st:
+        raise ValueError(f"oracle_integrand status {st}")
+    return complex(out[0], out[1]) if family == 2 else float(out[0])
+
+
+def shift_sums(p, k_begin=0, k_end=None):
+    """Raw compensated sums over lattice indices [k_begin, k_end) for problem dict p -> (m, ncomp)."""
+    k_end = p["n"] if k_end is None else k_end
+    nc = ncomp(p["family"])
+    out = np.zeros((p["m"], nc))
+    params, z, sh, fit = _f64(p["params"]), _u64(p["z"]), _f64(p["shifts"]), _f64(p.get("fit_coeffs"))
+    st = lib().oracle_shift_sums(p["family"], _d(params), len(params), p["dim"], p["n"], _u(z), _d(sh), p["m"],
+                                 p["transform"], _d(fit), int(k_begin), int(k_end), _d(out))
+    if st:
+        raise ValueError(f"oracle_shift_sums status {st}")
+    return out
+
+
+def finalize(shift_means):
+    sm = _f64(shift_means)
+    if sm.ndim == 1:
+        sm = sm.reshape(-1, 1)
+    m, nc = sm.shape
+    mean, err = np.zeros(nc), np.zeros(nc)
+    st = lib().oracle_finalize(_d(sm), m, nc, _d(mean), _d(err))
+    if st:
+        raise ValueError(f"oracle_finalize status {st}")
+    return mean, err
+
+
+def integrate(p):
+    """-> (shift_means (m, ncomp), mean (ncomp,), err (ncomp,))"""
+    nc = ncomp(p["family"])
+    sm, mean, err = np.zeros((p["m"], nc)), np.zeros(nc), np.zeros(nc)
+    params, z, sh, fit = _f64(p["params"]), _u64(p["z"]), _f64(p["shifts"]), _f64(p.get("fit_coeffs"))
+    st = lib().oracle_integrate(p["family"], _d(params), len(params), p["dim"], p["n"], _u(z), _d(sh), p["m"],
+                                p["transform"], _d(fit), _d(sm), _d(mean), _d(err))
+    if st:
+        raise ValueError(f"oracle_integrate status {st}")
+    return sm, mean, err
+
+
+def project(p, bins, shift=None):
+    params, z = _f64(p["params"]), _u64(p["z"])
+    shift = _f64(p["shifts"][0] if shift is None else shift)
+    H = np.zeros((p["dim"], bins))
+    st = lib().oracle_project(p["family"], _d(params), len(params), p["dim"], p["n"], _u(z), _d(shift), bins, _d(H))
+    if st:
+        raise ValueError(f"oracle_project status {st}")
+    return H
+
+
+def fit_cubic(hist):
+    H = _f64(hist)
+    d, bins = H.shape
+    out = np.zeros((d, 6))
+    lib().oracle_fit_cubic(_d(H), d, bins, _d(out))
+    return out

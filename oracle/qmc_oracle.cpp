@@ -1,0 +1,351 @@
+// qmc_oracle.cpp -- CPU ORACLE for the rank-1 shifted lattice rule of arXiv:1811.11720.
+//
+// THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and
+// bench.py's cpu_baseline / --impl reference leg may load it.  It shares no code, header, table
+// or constant with the CUDA path under paper_1811_11720_b200/csrc/ and neither includes the other.
+//
+// It is the paper's equations executed literally in fp64 (PAPER.md = /root/reference/PAPER.md,
+// cited as P:L<line>):
+//   O1  r_{k,j} = (k * z_j) mod n with an unsigned __int128 product           Eq. 2
+//   O2  u = wrap(fma(double(r), 1/double(n), Delta_{s,j}))  "{ } = fractional part", P:L100;
+//       the fp64 realisation is DESIGN.md reading C-2
+//   O3  (y, w) = periodizing transform: None (Table A.2), baker Eq. 17 P:L204-L209,
+//       Korobov weight r Eq. 15 P:L189-L193 with phi = int_0^u omega (Eq. 14)
+//   O4  optional fit map x = p(y), w *= p'(y)         Eq. 18-19, order P:L338
+//   O5  v = (prod_j w_j) * f(x)                                           Eq. 12-13
+//   O6  S_s = sum_k v (Neumaier-compensated), Q_s = S_s / n                       Eq. 2
+//   O7  Qbar = (sum_s Q_s) / m                                                    Eq. 2
+//   O8  err = sqrt( sum_s (Q_s - Qbar)^2 / (m (m-1)) ), per component            Eq. 3
+//   O9  projection histogram for the CDF of |f| (Eq. 20) and the cubic fit (C-8)
+// The only liberty taken with Eq. 2 is a loop interchange: the residues of index k do not depend
+// on the shift, so they are formed once per k and reused for all shifts; every per-shift sum still
+// adds its terms in increasing k.  OpenMP runs fixed chunks of 2^16 consecutive k; chunk sums are
+// combined in chunk order, so results do not depend on the thread count.
+//
+// Pins (tests/test_oracle_*.py, all `-m "not gpu"`): Fig. 1 lattice n=55 z=(1,34) P:L108; by-hand
+// lattices n=7 z=(1,3), n=11 z=(1,7) P:L1050; residue permutation property; exact-rational
+// coordinates; Fourier-mode exactness / dual-lattice modes; Eq. 15 normalisation, phi(1)=1,
+// Gauss-Legendre quadrature of omega; closed forms of families 0-2 (Genz 1, 2 P:L709-L713);
+// tensor Gauss-Legendre for the sector family at d<=3; x0*x1*x2 -> 1/8 (Fig. 2);
+// Eq. 3 on hand-made means; projection marginals in closed form; fit recovers an exact cubic.
+// Parity unpinned: nothing (the CBC tool is not part of the oracle).
+//
+// Build: g++ -O2 -std=c++17 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/build.py).
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+typedef unsigned __int128 u128;
+
+enum { FAM_OSC = 0, FAM_PRODPEAK = 1, FAM_CEXP = 2, FAM_SECTOR = 3 };
+enum { TR_NONE = 0, TR_BAKER = 1, TR_KOROBOV = 100 };
+const int MAX_DIM = 64;
+const uint64_t CHUNK = 1ull << 16;
+
+// Neumaier's compensated sum (improved Kahan-Babuska).
+struct Comp {
+    double s = 0.0, c = 0.0;
+    void add(double v) {
+        double t = s + v;
+        if (std::fabs(s) >= std::fabs(v)) c += (s - t) + v; else c += (v - t) + s;
+        s = t;
+    }
+    double value() const { return s + c; }
+};
+
+// O1: exact residue, Eq. 2: i*z mod n.
+inline uint64_t residue(uint64_t k, uint64_t z, uint64_t n) { return (uint64_t)(((u128)k * (u128)z) % (u128)n); }
+
+// O2: fractional part {r/n + Delta}, reading C-2(B): one fused rounding, exact wrap.
+inline double coordinate(uint64_t r, double inv_n, double delta) {
+    double t = std::fma((double)r, inv_n, delta);
+    return t >= 1.0 ? t - 1.0 : t;
+}
+
+double binom(int a, int b) { double v = 1.0; for (int i = 1; i <= b; ++i) v = v * (double)(a - b + i) / (double)i; return v; }
+
+// Korobov weight-r transform, Eq. 15 with r0 = r1 = r:
+//   omega(u) = (2r+1) C(2r,r) u^r (1-u)^r,
+//   phi(u) = int_0^u omega = c_r sum_{i=0}^{r} C(r,i) (-1)^i u^{r+1+i} / (r+1+i)      (Eq. 14)
+// phi is evaluated by Horner for u <= 1/2 and as 1 - phi(1-u) above (symmetric weight).
+struct Korobov {
+    int r; double c; double coef[8];
+    explicit Korobov(int r_) : r(r_) {
+        c = (2.0 * r + 1.0) * binom(2 * r, r);
+        for (int i = 0; i <= r; ++i) coef[i] = c * binom(r, i) * ((i & 1) ? -1.0 : 1.0) / (double)(r + 1 + i);
+    }
+    double phi_low(double u) const {
+        double h = coef[r];
+        for (int i = r - 1; i >= 0; --i) h = h * u + coef[i];
+        double p = 1.0; for (int i = 0; i <= r; ++i) p *= u;     // u^(r+1)
+        return p * h;
+    }
+    double phi(double u) const { return u <= 0.5 ? phi_low(u) : 1.0 - phi_low(1.0 - u); }
+    double omega(double u) const {
+        double p = 1.0; for (int i = 0; i < r; ++i) p *= u * (1.0 - u);
+        return c * p;
+    }
+};
+
+// O3
+inline void transform(int tr, const Korobov* kor, double u, double* y, double* w) {
+    if (tr == TR_NONE) { *y = u; *w = 1.0; }
+    else if (tr == TR_BAKER) { *y = 1.0 - std::fabs(2.0 * u - 1.0); *w = 1.0; }   // Eq. 17
+    else { *y = kor->phi(u); *w = kor->omega(u); }
+}
+
+// O4: Eq. 19 and its derivative; a[0..5] = a_0..a_5, a6 = 1 - a2 - a3 - a4 - a5.
+inline void fit_map(const double* a, double y, double* x, double* dp) {
+    double a6 = 1.0 - a[2] - a[3] - a[4] - a[5];
+    double p = y * (a[4] + y * (a[5] + y * a6));
+    double d = a[4] + y * (2.0 * a[5] + 3.0 * a6 * y);
+    if (a[2] != 0.0) { p += a[2] * y * (a[0] - 1.0) / (a[0] - y); d += a[2] * a[0] * (a[0] - 1.0) / ((a[0] - y) * (a[0] - y)); }
+    if (a[3] != 0.0) { p += a[3] * y * (a[1] - 1.0) / (a[1] - y); d += a[3] * a[1] * (a[1] - 1.0) / ((a[1] - y) * (a[1] - y)); }
+    *x = p; *dp = d;
+}
+
+inline double ipow(double x, int e) { double p = 1.0; for (int i = 0; i < e; ++i) p *= x; return p; }
+
+// Sparse polynomial sum_t c_t prod_j x_j^{e_{t,j}}; exponents stored as doubles.
+double sparse_poly(const double* c, const double* e, int count, int dim, const double* x) {
+    double s = 0.0;
+    for (int t = 0; t < count; ++t) {
+        double mon = c[t];
+        for (int j = 0; j < dim; ++j) mon *= ipow(x[j], (int)e[t * dim + j]);
+        s += mon;
+    }
+    return s;
+}
+
+// O5: the integrand families (layouts: DESIGN.md reading C-7).
+//  0 Genz oscillatory  f = cos(2 pi u0 + sum a_j x_j)
+//  1 Genz product peak f = prod 1/(c_j^-2 + (x_j - w_j)^2)
+//  2 complex           f = exp(i sum a_j x_j) prod (1 + b_j x_j)            BASELINE.json configs[2]
+//  3 sector-like       f = prod x_j^nu_j * U(x)^a / F(x)^b                  BASELINE.json configs[3]
+inline void integrand(int fam, const double* p, int dim, const double* x, double* re, double* im) {
+    *im = 0.0;
+    if (fam == FAM_OSC) {
+        double ph = 2.0 * M_PI * p[0];
+        for (int j = 0; j < dim; ++j) ph += p[1 + j] * x[j];
+        *re = std::cos(ph);
+    } else if (fam == FAM_PRODPEAK) {
+        double f = 1.0;
+        for (int j = 0; j < dim; ++j) { double t = x[j] - p[dim + j]; f *= 1.0 / (1.0 / (p[j] * p[j]) + t * t); }
+        *re = f;
+    } else if (fam == FAM_CEXP) {
+        double ph = 0.0, pr = 1.0;
+        for (int j = 0; j < dim; ++j) { ph += p[j] * x[j]; pr *= 1.0 + p[dim + j] * x[j]; }
+        *re = std::cos(ph) * pr; *im = std::sin(ph) * pr;
+    } else {
+        int a = (int)p[0], b = (int)p[1], nU = (int)p[2], nF = (int)p[3];
+        const double* nu = p + 4;
+        const double* cU = nu + dim; const double* eU = cU + nU;
+        const double* cF = eU + (size_t)nU * dim; const double* eF = cF + nF;
+        double pre = 1.0;
+        for (int j = 0; j < dim; ++j) pre *= ipow(x[j], (int)nu[j]);
+        double U = sparse_poly(cU, eU, nU, dim, x), F = sparse_poly(cF, eF, nF, dim, x);
+        *re = pre * ipow(U, a) / ipow(F, b);
+    }
+}
+
+inline int ncomp_of(int fam) { return fam == FAM_CEXP ? 2 : 1; }
+
+int expected_params(int fam, const double* p, int dim) {
+    if (fam == FAM_OSC) return 1 + dim;
+    if (fam == FAM_PRODPEAK || fam == FAM_CEXP) return 2 * dim;
+    if (fam == FAM_SECTOR) { int nU = (int)p[2], nF = (int)p[3]; return 4 + dim + (nU + nF) * (1 + dim); }
+    return -1;
+}
+
+// One lattice point for one shift: O2-O5.  Returns v = W * f (re, im).
+inline void eval_point(int fam, const double* params, int dim, const uint64_t* r, double inv_n, const double* shift,
+                       int tr, const Korobov* kor, const double* fit, double* re, double* im) {
+    double x[MAX_DIM]; double W = 1.0;
+    for (int j = 0; j < dim; ++j) {
+        double u = coordinate(r[j], inv_n, shift[j]);
+        double y, w; transform(tr, kor, u, &y, &w);
+        if (fit) { double xx, dp; fit_map(fit + 6 * j, y, &xx, &dp); y = xx; w *= dp; }
+        x[j] = y; W *= w;
+    }
+    double fr, fi; integrand(fam, params, dim, x, &fr, &fi);
+    *re = W * fr; *im = W * fi;
+}
+
+}  // namespace
+
+extern "C" {
+
+int oracle_num_threads() {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+// Residues and coordinates of lattice indices k0 .. k0+count-1 for one shift (O1, O2).
+int oracle_lattice_points(uint64_t n, int dim, const uint64_t* z, const double* shift, uint64_t k0, uint64_t count,
+                          uint64_t* out_r, double* out_u) {
+    double inv_n = 1.0 / (double)n;
+    for (uint64_t i = 0; i < count; ++i)
+        for (int j = 0; j < dim; ++j) {
+            uint64_t r = residue(k0 + i, z[j], n);
+            if (out_r) out_r[i * dim + j] = r;
+            if (out_u) out_u[i * dim + j] = coordinate(r, inv_n, shift[j]);
+        }
+    return 0;
+}
+
+// Per-coordinate transform (O3) exposed for the pins.
+int oracle_transform(int tr, double u, double* y, double* w) {
+    if (tr >= TR_KOROBOV + 1 && tr <= TR_KOROBOV + 6) { Korobov k(tr - TR_KOROBOV); transform(tr, &k, u, y, w); return 0; }
+    if (tr == TR_NONE || tr == TR_BAKER) { transform(tr, nullptr, u, y, w); return 0; }
+    return -7;
+}
+
+int oracle_fit_map(const double* a, double y, double* x, double* dp) { fit_map(a, y, x, dp); return 0; }
+
+int oracle_integrand(int fam, const double* params, int n_params, int dim, const double* x, double* out2) {
+    if (fam < 0 || fam > 3 || dim < 1 || dim > MAX_DIM) return -8;
+    if (expected_params(fam, params, dim) != n_params) return -9;
+    integrand(fam, params, dim, x, &out2[0], &out2[1]);
+    return 0;
+}
+
+// Raw sums S_s = sum_{k in [k_begin,k_end)} v_{k,s} (O1-O6 without the 1/n), ncomp per shift
+// interleaved (re, im).  Compensated within 2^16-aligned chunks and across chunks in chunk order.
+int oracle_shift_sums(int fam, const double* params, int n_params, int dim, uint64_t n, const uint64_t* z,
+                      const double* shifts, int m, int tr, const double* fit, uint64_t k_begin, uint64_t k_end,
+                      double* out_sums) {
+    if (fam < 0 || fam > 3) return -8;
+    if (dim < 1 || dim > MAX_DIM) return -2;
+    if (expected_params(fam, params, dim) != n_params) return -9;
+    bool kor_tr = tr >= TR_KOROBOV + 1 && tr <= TR_KOROBOV + 6;
+    if (!(tr == TR_NONE || tr == TR_BAKER || kor_tr)) return -7;
+    if (k_end > n || k_begin > k_end) return -3;
+    Korobov kor(kor_tr ? tr - TR_KOROBOV : 1);
+    const int nc = ncomp_of(fam);
+    const double inv_n = 1.0 / (double)n;
+    const uint64_t c0 = k_begin / CHUNK, c1 = (k_end + CHUNK - 1) / CHUNK;
+    const int64_t nchunks = (int64_t)(c1 - c0);
+    std::vector<double> chunk_sums((size_t)(nchunks > 0 ? nchunks : 0) * m * nc);
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t ci = 0; ci < nchunks; ++ci) {
+        uint64_t ka = (c0 + ci) * CHUNK, kb = ka + CHUNK;
+        if (ka < k_begin) ka = k_begin;
+        if (kb > k_end) kb = k_end;
+        std::vector<Comp> acc((size_t)m * nc);
+        uint64_t r[MAX_DIM];
+        for (uint64_t k = ka; k < kb; ++k) {
+            for (int j = 0; j < dim; ++j) r[j] = residue(k, z[j], n);
+            for (int s = 0; s < m; ++s) {
+                double re, im;
+                eval_point(fam, params, dim, r, inv_n, shifts + (size_t)s * dim, tr, &kor, fit, &re, &im);
+                acc[(size_t)s * nc].add(re);
+                if (nc == 2) acc[(size_t)s * nc + 1].add(im);
+            }
+        }
+        for (int q = 0; q < m * nc; ++q) chunk_sums[(size_t)ci * m * nc + q] = acc[q].value();
+    }
+    for (int q = 0; q < m * nc; ++q) {
+        Comp t;
+        for (int64_t ci = 0; ci < nchunks; ++ci) t.add(chunk_sums[(size_t)ci * m * nc + q]);
+        out_sums[q] = t.value();
+    }
+    return 0;
+}
+
+// O7, O8: Eq. 2 outer mean and Eq. 3, two-pass, per component.
+int oracle_finalize(const double* shift_means, int m, int ncomp, double* out_mean, double* out_err) {
+    if (m < 2) return -6;
+    for (int c = 0; c < ncomp; ++c) {
+        Comp t;
+        for (int s = 0; s < m; ++s) t.add(shift_means[s * ncomp + c]);
+        double mean = t.value() / (double)m;
+        Comp v;
+        for (int s = 0; s < m; ++s) { double d = shift_means[s * ncomp + c] - mean; v.add(d * d); }
+        out_mean[c] = mean;
+        out_err[c] = std::sqrt(v.value() / ((double)m * (double)(m - 1)));
+    }
+    return 0;
+}
+
+// Whole rule: per-shift means Q_s (O6), estimate and error (O7, O8).
+int oracle_integrate(int fam, const double* params, int n_params, int dim, uint64_t n, const uint64_t* z,
+                     const double* shifts, int m, int tr, const double* fit, double* out_shift_means,
+                     double* out_mean, double* out_err) {
+    const int nc = ncomp_of(fam);
+    std::vector<double> sums((size_t)m * 2);
+    int st = oracle_shift_sums(fam, params, n_params, dim, n, z, shifts, m, tr, fit, 0, n, sums.data());
+    if (st) return st;
+    std::vector<double> means((size_t)m * nc);
+    for (int q = 0; q < m * nc; ++q) means[q] = sums[q] / (double)n;
+    if (out_shift_means) std::memcpy(out_shift_means, means.data(), sizeof(double) * m * nc);
+    return oracle_finalize(means.data(), m, nc, out_mean, out_err);
+}
+
+// O9 (reading C-8): transform None, weight 1, one shift; H[j][b] = sum_k |f(x_k)| [floor(B x_{k,j}) = b].
+// |f| is the modulus for the complex family.  Compensated per bin, k increasing.
+int oracle_project(int fam, const double* params, int n_params, int dim, uint64_t n, const uint64_t* z,
+                   const double* shift, int bins, double* out_hist) {
+    if (fam < 0 || fam > 3) return -8;
+    if (dim < 1 || dim > MAX_DIM) return -2;
+    if (expected_params(fam, params, dim) != n_params) return -9;
+    const double inv_n = 1.0 / (double)n;
+    std::vector<Comp> H((size_t)dim * bins);
+    double x[MAX_DIM];
+    for (uint64_t k = 0; k < n; ++k) {
+        for (int j = 0; j < dim; ++j) x[j] = coordinate(residue(k, z[j], n), inv_n, shift[j]);
+        double re, im; integrand(fam, params, dim, x, &re, &im);
+        double a = ncomp_of(fam) == 2 ? std::hypot(re, im) : std::fabs(re);
+        for (int j = 0; j < dim; ++j) {
+            int b = (int)std::floor((double)bins * x[j]);
+            if (b >= bins) b = bins - 1;
+            H[(size_t)j * bins + b].add(a);
+        }
+    }
+    for (size_t q = 0; q < H.size(); ++q) out_hist[q] = H[q].value();
+    return 0;
+}
+
+// Cubic fit of the inverse CDF (reading C-8): with c_b the CDF at the bin edges e_b = b/B,
+// minimise sum_{b=1}^{B-1} (c^3 + a4 (c - c^3) + a5 (c^2 - c^3) - e)^2 (2x2 normal equations);
+// identity if min p' on [0,1] <= 0.05 or the system is singular.  Writes a0..a5 per dimension.
+int oracle_fit_cubic(const double* hist, int dim, int bins, double* fit_coeffs) {
+    for (int j = 0; j < dim; ++j) {
+        const double* H = hist + (size_t)j * bins;
+        Comp tot; for (int b = 0; b < bins; ++b) tot.add(H[b]);
+        double total = tot.value();
+        double a4 = 1.0, a5 = 0.0;
+        if (total > 0.0) {
+            double A11 = 0, A12 = 0, A22 = 0, B1 = 0, B2 = 0;
+            Comp run;
+            for (int b = 1; b < bins; ++b) {
+                run.add(H[b - 1]);
+                double c = run.value() / total, e = (double)b / (double)bins;
+                double c3 = c * c * c, g1 = c - c3, g2 = c * c - c3, t = e - c3;
+                A11 += g1 * g1; A12 += g1 * g2; A22 += g2 * g2; B1 += g1 * t; B2 += g2 * t;
+            }
+            double det = A11 * A22 - A12 * A12;
+            if (std::fabs(det) > 1e-300) {
+                double s4 = (B1 * A22 - B2 * A12) / det, s5 = (A11 * B2 - A12 * B1) / det;
+                double a6 = 1.0 - s4 - s5;
+                // min of p'(y) = s4 + 2 s5 y + 3 a6 y^2 on [0,1]
+                double mn = std::fmin(s4, s4 + 2.0 * s5 + 3.0 * a6);
+                if (a6 != 0.0) { double yv = -s5 / (3.0 * a6); if (yv > 0.0 && yv < 1.0) mn = std::fmin(mn, s4 + yv * (2.0 * s5 + 3.0 * a6 * yv)); }
+                if (mn > 0.05) { a4 = s4; a5 = s5; }
+            }
+        }
+        double* o = fit_coeffs + 6 * j;
+        o[0] = 1.001; o[1] = -0.001; o[2] = 0.0; o[3] = 0.0; o[4] = a4; o[5] = a5;
+    }
+    return 0;
+}
+
+}  // extern "C"

@@ -1,0 +1,346 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (no GPU needed).
+
+Every check compares oracle/ with something that is NOT the oracle: values written out by hand from
+the paper's tiny lattices, exact rational arithmetic, library special functions (scipy betainc,
+quad, leggauss), closed-form integrals, brute-force tensor quadrature.
+"""
+import math
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+import scipy.integrate
+import scipy.special
+
+import oracle
+from paper_1811_11720_b200 import synth
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+K3 = synth.TRANSFORM_KOROBOV + 3
+
+
+# ------------------------------------------------------------------ residues (O1, Eq. 2)
+def test_residues_paper_lattices():
+    for line in open(os.path.join(GOLD, "lattice_small.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        head, vals = line.split(":")
+        n, z2 = (int(v) for v in head.split())
+        want = np.array([int(v) for v in vals.split()], dtype=np.uint64)
+        r, _ = oracle.lattice_points(n, [1, z2], [0.0, 0.0], 0, n)
+        assert np.array_equal(r[:, 0], np.arange(n, dtype=np.uint64))
+        assert np.array_equal(r[:, 1], want)
+
+
+@pytest.mark.parametrize("n", [7, 11, 55, 1021, 65537])
+def test_residues_are_permutations(n):
+    z = [c for c in range(1, n) if math.gcd(c, n) == 1][:: max(1, n // 7)][:6]
+    r, _ = oracle.lattice_points(n, z, [0.0] * len(z), 0, n)
+    for j in range(len(z)):
+        assert np.array_equal(np.sort(r[:, j]), np.arange(n, dtype=np.uint64))
+
+
+def test_residues_large_n_bigint():
+    n = 15173222401                      # the paper's largest lattice, P:L1032 (needs > 64-bit products)
+    z = [1, 6543210987, 15173222400, 9999999967]
+    rng = np.random.default_rng(1)
+    for k0 in [0, 1, n - 5, int(rng.integers(1 << 32, n - 10))]:
+        r, _ = oracle.lattice_points(n, z, [0.0] * 4, k0, 5)
+        for i in range(5):
+            for j in range(4):
+                assert int(r[i, j]) == ((k0 + i) * z[j]) % n
+
+
+# -------------------------------------------------------- coordinates (O2, "{ }" P:L100, reading C-2)
+@pytest.mark.parametrize("n", [55, 65537, 1073741789, 15173222401])
+def test_coordinates_exact_rational(n):
+    rng = np.random.default_rng(n % 1000)
+    z = [1, n // 3 + 1 if math.gcd(n // 3 + 1, n) == 1 else n // 3 + 2, n - 1]
+    shift = rng.random(3)
+    shift[2] = 1.0 - 2.0 ** -53          # largest double below 1
+    cnt = min(200, n)
+    k0 = int(rng.integers(0, n - cnt + 1))
+    r, u = oracle.lattice_points(n, z, shift, k0, cnt)
+    assert np.all(u >= 0.0) and np.all(u < 1.0)
+    for i in range(cnt):
+        for j in range(3):
+            exact = Fraction(int(r[i, j]), n) + Fraction(float(shift[j]))
+            exact -= int(exact)           # fractional part
+            err = abs(Fraction(float(u[i, j])) - exact)
+            err = min(err, 1 - err)       # a value that rounds up to 1.0 wraps to 0.0
+            assert err <= Fraction(1, 2 ** 52)
+
+
+def test_coordinates_d1_mean_closed_form():
+    # z = 1: mean over k of {k/n + D} = (n-1)/(2n) + frac(n D)/n
+    n, D = 1021, 0.3437
+    _, u = oracle.lattice_points(n, [1], [D], 0, n)
+    want = (n - 1) / (2 * n) + ((n * D) % 1.0) / n
+    assert abs(math.fsum(u[:, 0]) / n - want) < 1e-14
+
+
+# ---------------------------------------------------------------------------- transforms (O3)
+@pytest.mark.parametrize("r", [1, 2, 3, 4, 5, 6])
+def test_korobov_normalisation_and_phi(r):
+    # Eq. 15: (2r+1) C(2r,r) = 1 / B(r+1, r+1);  Eq. 14: phi = regularised incomplete beta
+    c = 1.0 / scipy.special.beta(r + 1, r + 1)
+    assert abs(c - (2 * r + 1) * math.comb(2 * r, r)) < 1e-9 * c
+    for u in [0.0, 1e-9, 0.003, 0.1, 0.31, 0.5, 0.5000001, 0.77, 0.999, 1.0 - 2.0 ** -53]:
+        y, w = oracle.transform(synth.TRANSFORM_KOROBOV + r, u)
+        want_y = scipy.special.betainc(r + 1, r + 1, u)
+        assert abs(y - want_y) <= 4e-15 * max(want_y, 1e-300) + 1e-300 or abs(y - want_y) < 1e-16
+        assert abs(w - c * u ** r * (1 - u) ** r) <= 1e-14 * c
+        y2, _ = oracle.transform(synth.TRANSFORM_KOROBOV + r, 1.0 - u)
+        assert abs(y + y2 - 1.0) < 1e-15
+    assert oracle.transform(synth.TRANSFORM_KOROBOV + r, 0.0) == (0.0, 0.0)
+    # phi as the integral of omega (Eq. 14) by Gauss-Legendre, exact for these polynomials
+    xs, ws = np.polynomial.legendre.leggauss(12)
+    for u in [0.2, 0.6, 0.95]:
+        t = 0.5 * u * (xs + 1.0)
+        quad = 0.5 * u * np.sum(ws * np.array([oracle.transform(synth.TRANSFORM_KOROBOV + r, v)[1] for v in t]))
+        assert abs(quad - oracle.transform(synth.TRANSFORM_KOROBOV + r, u)[0]) < 1e-14
+
+
+def test_baker_and_none():
+    # Eq. 17: 2u below 1/2, 2-2u above; weight 1
+    for u, y in [(0.0, 0.0), (0.25, 0.5), (0.5, 1.0), (0.75, 0.5), (0.9, 0.2)]:
+        got = oracle.transform(synth.TRANSFORM_BAKER, u)
+        assert abs(got[0] - y) < 1e-15 and got[1] == 1.0
+        assert oracle.transform(synth.TRANSFORM_NONE, u) == (u, 1.0)
+    with pytest.raises(ValueError):
+        oracle.transform(synth.TRANSFORM_KOROBOV + 7, 0.5)
+
+
+# ------------------------------------------------------------------------------- fit map (O4)
+def test_fit_map_endpoints_and_derivative():
+    for a in [[1.001, -0.001, 0.0, 0.0, 0.6, 0.3], [1.5, -0.4, 0.2, 0.1, 0.3, 0.25], [2.0, -1.0, 0.05, 0.3, 1.0, -0.2]]:
+        assert oracle.fit_map(a, 0.0)[0] == 0.0            # p(0) = 0
+        assert abs(oracle.fit_map(a, 1.0)[0] - 1.0) < 1e-15  # p(1) = 1
+        for y in [0.1, 0.37, 0.8]:
+            h = 1e-6
+            fd = (oracle.fit_map(a, y + h)[0] - oracle.fit_map(a, y - h)[0]) / (2 * h)
+            assert abs(fd - oracle.fit_map(a, y)[1]) < 1e-8
+    # Eq. 19 written out for one point
+    a0, a1, a2, a3, a4, a5 = 1.5, -0.4, 0.2, 0.1, 0.3, 0.25
+    y = 0.3
+    want = a2 * y * (a0 - 1) / (a0 - y) + a3 * y * (a1 - 1) / (a1 - y) + a4 * y + a5 * y ** 2 + (1 - a2 - a3 - a4 - a5) * y ** 3
+    assert abs(oracle.fit_map([a0, a1, a2, a3, a4, a5], y)[0] - want) < 1e-15
+
+
+# --------------------------------------------------------- lattice rule on Fourier modes (O1-O6)
+def _mode_problem(n, z, h, shifts):
+    d = len(z)
+    prm = np.array([2 * math.pi * v for v in h] + [0.0] * d)      # f = exp(2 pi i h.x)
+    return synth.problem(synth.FAMILY_CEXP_POLY, prm, n, z, shifts, synth.TRANSFORM_NONE)
+
+
+def test_rule_exact_on_fourier_modes():
+    n, z = 1021, [1, 374, 147]
+    rng = synth.MT19937_64(7)
+    sh = synth.draw_shifts(rng, 3, 3)
+    # h.z != 0 (mod n): the rule returns 0; h.z == 0: it returns exp(2 pi i h.Delta)
+    for h in [(1, 0, 0), (0, 2, -1), (3, -2, 5), (-7, 1, 1)]:
+        assert sum(a * b for a, b in zip(h, z)) % n != 0
+        sm, _, _ = oracle.integrate(_mode_problem(n, z, h, sh))
+        assert np.max(np.abs(sm)) < 1e-12
+    for h in [(-374, 1, 0), (-147, 0, 1), (n, 0, 0), (0, 0, 0)]:
+        assert sum(a * b for a, b in zip(h, z)) % n == 0
+        sm, _, _ = oracle.integrate(_mode_problem(n, z, h, sh))
+        for s in range(3):
+            ph = 2 * math.pi * math.fsum(a * b for a, b in zip(h, sh[s]))
+            tol = 2 * math.pi * sum(abs(v) for v in h) * 2.0 ** -51 + 1e-13
+            assert abs(sm[s, 0] - math.cos(ph)) < tol and abs(sm[s, 1] - math.sin(ph)) < tol
+
+
+def test_sum_against_fsum_python():
+    # the whole chain in slow exact-ish python: Fractions for the point, math.fsum for the sum
+    n, z = 251, [1, 97, 33]
+    prm = np.array([0.3, 0.9, 0.4, 0.7])
+    sh = synth.draw_shifts(synth.MT19937_64(3), 2, 3)
+    p = synth.problem(synth.FAMILY_GENZ_OSC, prm, n, z, sh, synth.TRANSFORM_NONE)
+    sums = oracle.shift_sums(p)
+    for s in range(2):
+        terms = []
+        for k in range(n):
+            x = [float((Fraction(k * z[j] % n, n) + Fraction(float(sh[s, j]))) % 1) for j in range(3)]
+            terms.append(math.cos(2 * math.pi * prm[0] + math.fsum(prm[1 + j] * x[j] for j in range(3))))
+        assert abs(sums[s, 0] - math.fsum(terms)) < 1e-12
+    # sub-ranges add up to the whole
+    part = oracle.shift_sums(p, 0, 100) + oracle.shift_sums(p, 100, n)
+    assert np.allclose(part, sums, rtol=0, atol=1e-13)
+
+
+# --------------------------------------------------------------- closed forms of the families (O5)
+def closed_osc(prm):
+    u0, a = prm[0], prm[1:]
+    return math.cos(2 * math.pi * u0 + 0.5 * a.sum()) * np.prod(np.sin(a / 2) / (a / 2))
+
+
+def closed_prodpeak(prm):
+    d = len(prm) // 2
+    c, w = prm[:d], prm[d:]
+    return np.prod(c * (np.arctan(c * (1 - w)) + np.arctan(c * w)))
+
+
+def closed_cexp(prm):
+    d = len(prm) // 2
+    out = 1.0 + 0j
+    for a, b in zip(prm[:d], prm[d:]):
+        ia = 1j * a
+        e = np.exp(ia)
+        out *= (e - 1) / ia + b * (e / ia - (e - 1) / ia ** 2)
+    return out
+
+
+def test_closed_cexp_matches_quad():
+    a, b = 1.7, 0.6
+    re = scipy.integrate.quad(lambda x: math.cos(a * x) * (1 + b * x), 0, 1)[0]
+    im = scipy.integrate.quad(lambda x: math.sin(a * x) * (1 + b * x), 0, 1)[0]
+    assert abs(closed_cexp(np.array([a, b])) - complex(re, im)) < 1e-13
+
+
+def _check_vs_exact(p, exact, nsig=6.0, rel=None, floor=1e-14):
+    # floor = relative accuracy of `exact` itself (1e-14 for closed forms, larger for quadrature)
+    sm, mean, err = oracle.integrate(p)
+    val = complex(mean[0], mean[1]) if len(mean) == 2 else mean[0]
+    e = float(np.max(err))
+    assert abs(val - exact) <= nsig * e + floor * abs(exact), (val, exact, e)
+    if rel is not None:
+        assert abs(val - exact) <= rel * abs(exact), (val, exact)
+    return val, e
+
+
+@pytest.mark.parametrize("tr,rel", [(synth.TRANSFORM_NONE, 3e-3), (synth.TRANSFORM_BAKER, 1e-5), (K3, 1e-7),
+                                    (synth.TRANSFORM_KOROBOV + 1, 1e-4), (synth.TRANSFORM_KOROBOV + 2, 1e-6),
+                                    (synth.TRANSFORM_KOROBOV + 5, 1e-6)])
+def test_family0_closed_form_all_transforms(tr, rel):
+    # invariance of the integral under every periodizing transform, Eq. 12
+    n, d = 65537, 4
+    rng = synth.MT19937_64(11)
+    prm = synth.genz_osc(rng, d)
+    p = synth.problem(synth.FAMILY_GENZ_OSC, prm, n, synth.genvec(n, d), synth.draw_shifts(rng, 12, d), tr)
+    _check_vs_exact(p, closed_osc(prm), rel=rel)
+
+
+def test_family1_closed_form():
+    n, d = 65537, 4
+    rng = synth.MT19937_64(12)
+    prm = synth.genz_prodpeak(rng, d)
+    for tr, rel in [(synth.TRANSFORM_BAKER, 1e-4), (K3, 1e-5)]:
+        p = synth.problem(synth.FAMILY_GENZ_PRODPEAK, prm, n, synth.genvec(n, d), synth.draw_shifts(rng, 12, d), tr)
+        _check_vs_exact(p, closed_prodpeak(prm), rel=rel)
+
+
+def test_family2_closed_form():
+    n, d = 65537, 4
+    rng = synth.MT19937_64(13)
+    prm = synth.cexp_poly(rng, d)
+    p = synth.problem(synth.FAMILY_CEXP_POLY, prm, n, synth.genvec(n, d), synth.draw_shifts(rng, 12, d), K3)
+    _check_vs_exact(p, closed_cexp(prm), rel=1e-6)
+
+
+def test_fit_map_leaves_integral_invariant():
+    # Eq. 18 with arbitrary valid coefficients, composed as x = p(phi(u))
+    n, d = 65537, 4
+    rng = synth.MT19937_64(14)
+    prm = synth.genz_osc(rng, d)
+    sh = synth.draw_shifts(rng, 12, d)
+    fit = synth.cubic_fit_coeffs(d, 0.6, 0.3)
+    fit[1] = [1.4, -0.3, 0.15, 0.1, 0.5, 0.2]            # full Eq. 19 in one dimension
+    p = synth.problem(synth.FAMILY_GENZ_OSC, prm, n, synth.genvec(n, d), sh, K3, fit_coeffs=fit)
+    _check_vs_exact(p, closed_osc(prm), rel=1e-6)
+
+
+def test_minimal_example_one_eighth():
+    # Fig. 2: f = x0 x1 x2, Korobov-3 -> 1/8; here as a degenerate sector integrand
+    d, n = 3, 8191
+    prm = np.array([1, 2, 1, 1, 1, 1, 1, 1.0, 0, 0, 0, 1.0, 0, 0, 0], dtype=np.float64)   # U = F = 1, nu = (1,1,1)
+    rng = synth.MT19937_64(15)
+    p = synth.problem(synth.FAMILY_SECTOR, prm, n, synth.korobov_form_vector(n, d, 1487), synth.draw_shifts(rng, 32, d), K3)
+    _check_vs_exact(p, 0.125, rel=1e-6)
+
+
+def _sector_numpy(prm, d, X):
+    """Independent vectorised evaluation of prod x^nu U^a / F^b on points X (N, d)."""
+    a, b, nU, nF = (int(v) for v in prm[:4])
+    nu = prm[4:4 + d]
+    o = 4 + d
+    cU, eU = prm[o:o + nU], prm[o + nU:o + nU + nU * d].reshape(nU, d)
+    o += nU * (1 + d)
+    cF, eF = prm[o:o + nF], prm[o + nF:o + nF + nF * d].reshape(nF, d)
+    U = sum(cU[t] * np.prod(X ** eU[t], axis=1) for t in range(nU))
+    F = sum(cF[t] * np.prod(X ** eF[t], axis=1) for t in range(nF))
+    return np.prod(X ** nu, axis=1) * U ** a / F ** b
+
+
+@pytest.mark.parametrize("d,seed", [(2, 21), (3, 22), (3, 23)])
+def test_family3_tensor_gauss_legendre(d, seed):
+    rng = synth.MT19937_64(seed)
+    prm = synth.sector(rng, d)
+    xs, ws = np.polynomial.legendre.leggauss(24)
+    xs, ws = 0.5 * (xs + 1), 0.5 * ws
+    grids = np.meshgrid(*([xs] * d), indexing="ij")
+    X = np.stack([g.ravel() for g in grids], axis=1)
+    Wt = np.prod(np.stack([g.ravel() for g in np.meshgrid(*([ws] * d), indexing="ij")], axis=1), axis=1)
+    exact = float(np.sum(Wt * _sector_numpy(prm, d, X)))
+    n = 65537
+    p = synth.problem(synth.FAMILY_SECTOR, prm, n, synth.genvec(n, 4)[:d], synth.draw_shifts(rng, 12, d), K3)
+    _check_vs_exact(p, exact, rel=1e-7, floor=1e-11)      # 24-node Gauss-Legendre is good to ~1e-12
+    # pointwise: oracle integrand vs the numpy restatement
+    pts = np.array([[rng.uniform() for _ in range(d)] for _ in range(5)])
+    for x, want in zip(pts, _sector_numpy(prm, d, pts)):
+        assert abs(oracle.integrand(synth.FAMILY_SECTOR, prm, x) - want) <= 1e-14 * abs(want)
+
+
+def test_integrand_param_count_checked():
+    with pytest.raises(ValueError):
+        oracle.integrand(synth.FAMILY_GENZ_OSC, [0.1, 0.2], [0.5, 0.5])
+
+
+# ------------------------------------------------------------------------- Eq. 3 (O7, O8)
+@pytest.mark.parametrize("m", [2, 10, 33])
+def test_error_estimate_hand_made(m):
+    mean, err = oracle.finalize(np.arange(1, m + 1, dtype=np.float64))
+    assert abs(mean[0] - (m + 1) / 2) < 1e-15 * m
+    assert abs(err[0] - math.sqrt((m + 1) / 12.0)) < 1e-15 * m
+    # complex: components separately
+    q = np.stack([np.arange(1, m + 1.0), 5.0 - 2.0 * np.arange(1, m + 1.0)], axis=1)
+    mean, err = oracle.finalize(q)
+    assert abs(mean[1] - (5.0 - (m + 1))) < 1e-13 and abs(err[1] - 2 * math.sqrt((m + 1) / 12.0)) < 1e-14 * m
+    with pytest.raises(ValueError):
+        oracle.finalize(np.array([1.0]))
+
+
+# ------------------------------------------------------------- projection and cubic fit (O9)
+def test_projection_marginals_product_peak():
+    n, d, B = 65537, 3, 16
+    rng = synth.MT19937_64(31)
+    prm = synth.genz_prodpeak(rng, d)
+    p = synth.problem(synth.FAMILY_GENZ_PRODPEAK, prm, n, synth.genvec(n, 4)[:d], synth.draw_shifts(rng, 1, d), synth.TRANSFORM_NONE)
+    H = oracle.project(p, B)
+    tot = oracle.shift_sums(p)[0, 0]                   # f > 0: sum |f| = sum f
+    c, w = prm[:d], prm[d:]
+    for j in range(d):
+        assert abs(H[j].sum() - tot) < 1e-12 * tot
+        edges = np.arange(B + 1) / B
+        cdf = np.arctan(c[j] * (edges - w[j]))
+        want = np.diff(cdf) / (cdf[-1] - cdf[0])
+        assert np.max(np.abs(H[j] / tot - want)) < 2e-3
+
+
+def test_fit_recovers_exact_cubic():
+    B, a4, a5 = 256, 0.55, 0.35
+    a6 = 1 - a4 - a5
+    edges = np.arange(B + 1) / B
+    cdf = np.array([0.0] + [min(r.real for r in np.roots([a6, a5, a4, -e]) if abs(r.imag) < 1e-12 and -1e-12 <= r.real <= 1 + 1e-12)
+                            for e in edges[1:]])
+    H = np.stack([np.diff(cdf), np.full(B, 1.0 / B)])
+    out = oracle.fit_cubic(H)
+    assert abs(out[0, 4] - a4) < 1e-9 and abs(out[0, 5] - a5) < 1e-9
+    assert abs(out[1, 4] - 1.0) < 1e-12 and abs(out[1, 5]) < 1e-12      # flat marginal -> identity
+    assert np.all(out[:, 2:4] == 0.0)
+    # a non-monotone least-squares solution falls back to the identity
+    H2 = np.zeros((1, B)); H2[0, 0] = 1.0
+    out2 = oracle.fit_cubic(H2)
+    assert out2[0, 4] == 1.0 and out2[0, 5] == 0.0
