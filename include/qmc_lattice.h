@@ -1,0 +1,176 @@
+/* qmc_lattice.h -- C ABI of the B200-native rank-1 shifted lattice (R1SL) integrator.
+ *
+ * The library computes, on one CUDA device (sm_100a), the hot path of the `qmc` integrator of
+ * arXiv:1811.11720 (PAPER.md = the paper text; cited as P:L<line>):
+ *
+ *   Q_s   = (1/n) sum_{k=0}^{n-1} W(u_{k,s}) f(x(u_{k,s})),  u_{k,s} = { k z / n + Delta_s }   Eq. 2
+ *   Qbar  = (1/m) sum_s Q_s                                                                   Eq. 2
+ *   err   = sqrt( sum_s (Q_s - Qbar)^2 / (m (m-1)) )   (per component for complex f)           Eq. 3
+ *
+ * with x = p(phi(u)) and W = prod_j omega(u_j) p'(phi(u_j)): phi/omega a periodizing transform
+ * (Eq. 12-17), p an optional per-dimension fitted inverse-CDF map (Eq. 18-19,
+ * P:L215-L223; composition order P:L338).  f is a member of a parameterised integrand family (a C
+ * ABI cannot carry the paper's functors).
+ *
+ * Conventions
+ *  - every function returns a qmc_status (0 = OK, negative = error); on an argument error no output
+ *    is written and nothing is launched;
+ *  - the caller owns every buffer; the library keeps no global state, allocates nothing that
+ *    outlives a call and may be called from several host threads on different streams;
+ *  - "HOST" / "DEVICE" beside a pointer says which address space it must point to;
+ *  - there is no CPU fallback: without a CUDA device every compute entry returns QMC_ERR_CUDA.
+ *
+ * Layouts
+ *  - z[j], j < dim: generating vector, 1 <= z_j < n, gcd(z_j, n) = 1 ("coprime to n");
+ *  - shifts[s*dim + j] in [0,1): shift s, dimension j (Delta_k of Eq. 2);
+ *  - fit_coeffs[j*6 + i] = a_i of Eq. 19 for dimension j, a_6 := 1-a_2-a_3-a_4-a_5
+ *    (cubic map <=> a_2 = a_3 = 0; then a_0, a_1 are ignored); NULL = no fit map;
+ *  - complex results are interleaved (re, im);
+ *  - params: packed per family, all doubles (small integers stored as exact doubles):
+ *      QMC_FAMILY_GENZ_OSC      [u0, a_1..a_d]            f = cos(2 pi u0 + sum a_j x_j)
+ *      QMC_FAMILY_GENZ_PRODPEAK [c_1..c_d, w_1..w_d]      f = prod 1/(c_j^-2 + (x_j-w_j)^2)
+ *      QMC_FAMILY_CEXP_POLY     [a_1..a_d, b_1..b_d]      f = exp(i sum a_j x_j) prod(1+b_j x_j)  (complex)
+ *      QMC_FAMILY_SECTOR        [a, b, nU, nF, nu_1..nu_d, cU_1..cU_nU, eU_{1,1}..eU_{nU,d},
+ *                                cF_1..cF_nF, eF_{1,1}..eF_{nF,d}]
+ *                               f = prod x_j^nu_j * U(x)^a / F(x)^b, U = sum_t cU_t prod_j x_j^eU_{t,j}
+ *                               (sector-decomposed shape); limits: 0 <= a,b <= 8, nu_j <= 8,
+ *                               nU,nF in 1..64, exponents <= 8, total degree of a monomial <= 16.
+ */
+#ifndef QMC_LATTICE_H
+#define QMC_LATTICE_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    QMC_OK = 0,
+    QMC_ERR_NULL = -1,       /* a required pointer is NULL */
+    QMC_ERR_DIM = -2,        /* dim outside 1..QMC_MAX_DIM */
+    QMC_ERR_N = -3,          /* n outside 2 .. 2^53-1 (double(r) must be exact), or count/bins invalid */
+    QMC_ERR_Z = -4,          /* z_j outside [1, n-1] or not coprime to n */
+    QMC_ERR_SHIFT = -5,      /* a shift outside [0,1) or not finite */
+    QMC_ERR_M = -6,          /* m < 2 (Eq. 3 divides by m-1) or m > QMC_MAX_M */
+    QMC_ERR_TRANSFORM = -7,  /* unknown transform id / Korobov weight outside 1..6 */
+    QMC_ERR_FAMILY = -8,     /* unknown family id */
+    QMC_ERR_PARAMS = -9,     /* n_params does not match the family layout, or a value is out of range */
+    QMC_ERR_FIT = -10,       /* fit map not monotone on [0,1] or parameters outside P:L231's bounds */
+    QMC_ERR_WORKSPACE = -11, /* workspace NULL, misaligned (256 B) or too small */
+    QMC_ERR_CUDA = -12,      /* CUDA runtime error (qmc_last_cuda_error() has the text) */
+    QMC_ERR_NONFINITE = -13  /* a result is NaN/Inf (synchronous entry only; results are still written) */
+} qmc_status;
+
+enum { QMC_FAMILY_GENZ_OSC = 0, QMC_FAMILY_GENZ_PRODPEAK = 1, QMC_FAMILY_CEXP_POLY = 2, QMC_FAMILY_SECTOR = 3 };
+
+/* Periodizing transforms, Table A.2: none; baker Eq. 17;
+ * Korobov with symmetric weight r, Eq. 15: QMC_TRANSFORM_KOROBOV + r, r = 1..6. */
+enum { QMC_TRANSFORM_NONE = 0, QMC_TRANSFORM_BAKER = 1, QMC_TRANSFORM_KOROBOV = 100 };
+
+enum { QMC_MAX_DIM = 32, QMC_MAX_M = 4096 };
+
+/* One integration problem.  In qmc_lattice_integrate_batch / qmc_lattice_project the four data
+ * pointers are DEVICE pointers; the struct array itself is HOST memory. */
+typedef struct {
+    int family;               /* QMC_FAMILY_* */
+    int dim;                  /* d, 1..QMC_MAX_DIM */
+    int m;                    /* number of random shifts, >= 2 */
+    int transform;            /* QMC_TRANSFORM_* */
+    uint64_t n;               /* lattice size (need not be prime, Fig. 1 uses 55) */
+    const double* params;     /* DEVICE, n_params doubles, family layout above */
+    int n_params;
+    const uint64_t* z;        /* DEVICE, dim entries */
+    const double* shifts;     /* DEVICE, m*dim entries */
+    const double* fit_coeffs; /* DEVICE, dim*6 entries, or NULL */
+} qmc_problem;
+
+/* Synchronous convenience call, HOST pointers only (north_star's argument list).  Validates all
+ * values (including gcd(z_j,n) = 1, shifts in [0,1), monotone fit map), copies the inputs to the
+ * device, runs the fused kernel + finalize on the default stream of the current device, copies the
+ * results back and synchronises.  out_mean / out_err: 1 double (real families) or 2 (re, im).
+ * n_params is implied by (family, dim, params).  Eq. 2-3. */
+int qmc_lattice_integrate(int family, const double* params /*HOST*/, int dim, uint64_t n,
+                          const uint64_t* z /*HOST*/, const double* shifts /*HOST [m][dim]*/, int m,
+                          int transform, const double* fit_coeffs /*HOST [dim][6] or NULL*/,
+                          double* out_mean /*HOST*/, double* out_err /*HOST*/);
+
+/* As above, additionally returning the per-shift means Q_s (HOST, m*ncomp doubles, may be NULL). */
+int qmc_lattice_integrate_ex(int family, const double* params, int n_params, int dim, uint64_t n,
+                             const uint64_t* z, const double* shifts, int m, int transform,
+                             const double* fit_coeffs, double* out_mean, double* out_err,
+                             double* out_shift_means /*HOST or NULL*/);
+
+/* Stream-ordered batched call: `count` problems of arbitrary, unequal cost in ONE persistent-grid
+ * launch (device-side tile queue; the paper's host-side work queue is P:L388-L402) followed by one
+ * finalize launch.  Never synchronises.  problems: HOST array whose data pointers are DEVICE
+ * pointers (only the struct fields are validated here; the pointed-to values are the caller's
+ * responsibility -- use qmc_validate_problem_host before uploading).
+ *   out_means, out_errs : DEVICE, count*2 doubles: [p*2 + c], c = 0 (re) / 1 (im, 0 for real families)
+ *   out_shift_means     : DEVICE or NULL, count*stride doubles, stride = 2*max_m:
+ *                         [p*stride + s*ncomp + c]
+ *   workspace           : DEVICE, 256-byte aligned, >= qmc_workspace_bytes(count, problems) bytes;
+ *                         contents are scratch (per-tile partial sums in fixed slots: results do not
+ *                         depend on the scheduling order, the grid size or the device's SM count).
+ */
+int qmc_lattice_integrate_batch(int count, const qmc_problem* problems /*HOST*/, double* out_means /*DEVICE*/,
+                                double* out_errs /*DEVICE*/, double* out_shift_means /*DEVICE or NULL*/,
+                                void* workspace /*DEVICE*/, size_t workspace_bytes, void* cuda_stream);
+
+/* Bytes of workspace qmc_lattice_integrate_batch / qmc_lattice_project need (0 on invalid input). */
+size_t qmc_workspace_bytes(int count, const qmc_problem* problems /*HOST*/);
+
+/* Full value validation of one problem whose data pointers are HOST pointers. */
+int qmc_validate_problem_host(const qmc_problem* p /*HOST, HOST data pointers*/);
+
+/* Projection pass for the variance-reduction fit (Eq. 20; reading C-8):
+ * transform None, weight 1, the first shift of p only, all n lattice points:
+ *   out_hist[j*bins + b] = sum_k |f(x_k)| [ floor(bins * x_{k,j}) == b ]     (|f| = modulus if complex)
+ * Stream-ordered, deterministic.  p: HOST struct with DEVICE data pointers (p->m >= 1 here,
+ * p->transform and p->fit_coeffs are ignored).  bins in 2..1024.  out_hist: DEVICE, dim*bins. */
+int qmc_lattice_project(const qmc_problem* p /*HOST*/, int bins, double* out_hist /*DEVICE*/,
+                        void* workspace /*DEVICE*/, size_t workspace_bytes, void* cuda_stream);
+size_t qmc_project_workspace_bytes(const qmc_problem* p /*HOST*/, int bins);
+
+/* Host-side closed-form least squares for the cubic sub-family of Eq. 19 (a_2 = a_3 = 0): with
+ * c_b the CDF of hist at the bin edges e_b = b/bins, minimise sum_b (p(c_b) - e_b)^2 over (a_4, a_5);
+ * identity map if the minimiser is not safely monotone (min p' <= 0.05).  hist, fit_coeffs: HOST. */
+int qmc_fit_cubic(const double* hist /*HOST [dim][bins]*/, int dim, int bins, double* fit_coeffs /*HOST [dim][6]*/);
+
+/* Inspection: residues r = (k z_j) mod n and coordinates u = {r/n + shift_j} for k = k0..k0+count-1,
+ * produced by the same device code the fused kernel uses (Eq. 2; fp64 realisation:
+ * u = wrap(fma(double(r), 1/double(n), shift_j)), reading C-2).
+ * z, shift: HOST.  out_r [count][dim], out_u [count][dim]: DEVICE (either may be NULL). */
+int qmc_lattice_points(uint64_t n, int dim, const uint64_t* z /*HOST*/, const double* shift /*HOST [dim]*/,
+                       uint64_t k0, uint64_t count, uint64_t* out_r /*DEVICE*/, double* out_u /*DEVICE*/,
+                       void* cuda_stream);
+
+/* Finalize stage alone (Eq. 2 outer mean + Eq. 3) on DEVICE per-shift means [m][ncomp]:
+ * out_mean, out_err DEVICE, ncomp doubles each.  Stream-ordered. */
+int qmc_finalize_means(const double* shift_means /*DEVICE*/, int m, int ncomp, double* out_mean /*DEVICE*/,
+                       double* out_err /*DEVICE*/, void* cuda_stream);
+
+/* Measurement helper: runs a DFMA-chain kernel (8 independent chains per thread, full occupancy)
+ * for `iters` iterations on `cuda_stream`, synchronises, and returns the sustained thread-level
+ * FP64 instruction rate in instructions/second through *out_rate (HOST) and the kernel time in ms
+ * through *out_ms (HOST, may be NULL).  This is the denominator of the FP64 issue-rate roofline. */
+int qmc_fp64_peak_probe(int iters, double* out_rate /*HOST*/, double* out_ms /*HOST or NULL*/, void* cuda_stream);
+
+/* Number of fused-kernel launches + finalize launches the last batch call of this thread issued
+ * (for the benchmark's gpu_launches accounting). */
+int qmc_last_launch_count(void);
+
+/* Launch geometry the library uses for a batch (for DESIGN.md / bench reporting): tiles, CTAs,
+ * k indices per tile of problem 0.  Any pointer may be NULL. */
+int qmc_plan_info(int count, const qmc_problem* problems /*HOST*/, long long* out_tiles, int* out_ctas,
+                  long long* out_tile_len0);
+
+int qmc_num_components(int family);          /* 1 or 2; <0 on unknown family */
+const char* qmc_status_string(int status);
+const char* qmc_last_cuda_error(void);       /* thread-local text of the last CUDA error ("" if none) */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QMC_LATTICE_H */

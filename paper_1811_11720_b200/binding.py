@@ -1,0 +1,254 @@
+"""Thin ctypes binding of include/qmc_lattice.h -- argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of libqmc_lattice.so; PyTorch supplies device
+memory and streams.  There is no CPU fallback: if the library is missing or no CUDA device is
+present the calls raise.  Function names mirror the C ABI.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libqmc_lattice.so")
+
+EXPORTS = [
+    "qmc_lattice_integrate", "qmc_lattice_integrate_ex", "qmc_lattice_integrate_batch", "qmc_workspace_bytes",
+    "qmc_validate_problem_host", "qmc_lattice_project", "qmc_project_workspace_bytes", "qmc_fit_cubic",
+    "qmc_lattice_points", "qmc_finalize_means", "qmc_fp64_peak_probe", "qmc_last_launch_count", "qmc_plan_info",
+    "qmc_num_components", "qmc_status_string", "qmc_last_cuda_error",
+]
+
+QMC_OK = 0
+QMC_ERR_NONFINITE = -13
+
+
+class QmcError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = status
+        L = lib()
+        msg = L.qmc_status_string(status).decode()
+        if status == -12:
+            msg += ": " + L.qmc_last_cuda_error().decode()
+        super().__init__(f"{where}: status {status} ({msg})")
+
+
+class qmc_problem(C.Structure):
+    _fields_ = [("family", C.c_int), ("dim", C.c_int), ("m", C.c_int), ("transform", C.c_int), ("n", C.c_uint64),
+                ("params", C.c_void_p), ("n_params", C.c_int), ("z", C.c_void_p), ("shifts", C.c_void_p),
+                ("fit_coeffs", C.c_void_p)]
+
+
+_lib = None
+
+
+def lib():
+    """Loads libqmc_lattice.so (build it with `python -m paper_1811_11720_b200.build`); fails loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} not built: run `python -m paper_1811_11720_b200.build` (nvcc, sm_100a)")
+        L = C.CDLL(LIB_PATH)
+        dp, up, vp = C.POINTER(C.c_double), C.POINTER(C.c_uint64), C.c_void_p
+        pp = C.POINTER(qmc_problem)
+        L.qmc_lattice_integrate.argtypes = [C.c_int, dp, C.c_int, C.c_uint64, up, dp, C.c_int, C.c_int, dp, dp, dp]
+        L.qmc_lattice_integrate_ex.argtypes = [C.c_int, dp, C.c_int, C.c_int, C.c_uint64, up, dp, C.c_int, C.c_int, dp, dp,
+                                               dp, dp]
+        L.qmc_lattice_integrate_batch.argtypes = [C.c_int, pp, vp, vp, vp, vp, C.c_size_t, vp]
+        L.qmc_workspace_bytes.argtypes = [C.c_int, pp]
+        L.qmc_workspace_bytes.restype = C.c_size_t
+        L.qmc_validate_problem_host.argtypes = [pp]
+        L.qmc_lattice_project.argtypes = [pp, C.c_int, vp, vp, C.c_size_t, vp]
+        L.qmc_project_workspace_bytes.argtypes = [pp, C.c_int]
+        L.qmc_project_workspace_bytes.restype = C.c_size_t
+        L.qmc_fit_cubic.argtypes = [dp, C.c_int, C.c_int, dp]
+        L.qmc_lattice_points.argtypes = [C.c_uint64, C.c_int, up, dp, C.c_uint64, C.c_uint64, vp, vp, vp]
+        L.qmc_finalize_means.argtypes = [vp, C.c_int, C.c_int, vp, vp, vp]
+        L.qmc_fp64_peak_probe.argtypes = [C.c_int, dp, dp, vp]
+        L.qmc_plan_info.argtypes = [C.c_int, pp, C.POINTER(C.c_longlong), C.POINTER(C.c_int), C.POINTER(C.c_longlong)]
+        L.qmc_num_components.argtypes = [C.c_int]
+        L.qmc_status_string.argtypes = [C.c_int]
+        L.qmc_status_string.restype = C.c_char_p
+        L.qmc_last_cuda_error.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def _check(status, where, allow=()):
+    if status != QMC_OK and status not in allow:
+        raise QmcError(status, where)
+    return status
+
+
+def _d(a):
+    return None if a is None else a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _u(a):
+    return a.ctypes.data_as(C.POINTER(C.c_uint64))
+
+
+def _f64(a):
+    return None if a is None else np.ascontiguousarray(a, dtype=np.float64)
+
+
+def qmc_num_components(family: int) -> int:
+    return int(lib().qmc_num_components(int(family)))
+
+
+def qmc_lattice_integrate(family, params, dim, n, z, shifts, m, transform, fit_coeffs=None):
+    """Synchronous HOST-pointer call (north_star's signature) -> (mean, err) arrays of ncomp doubles."""
+    params, shifts, fit = _f64(params), _f64(shifts), _f64(fit_coeffs)
+    z = np.ascontiguousarray(z, dtype=np.uint64)
+    nc = max(qmc_num_components(family), 1)
+    mean, err = np.zeros(2), np.zeros(2)
+    _check(lib().qmc_lattice_integrate(int(family), _d(params), int(dim), int(n), _u(z), _d(shifts), int(m), int(transform),
+                                       _d(fit), _d(mean), _d(err)), "qmc_lattice_integrate")
+    return mean[:nc].copy(), err[:nc].copy()
+
+
+def qmc_lattice_integrate_ex(p: dict):
+    """Synchronous HOST-pointer call on a problem dict (synth.problem) -> (shift_means (m, ncomp), mean, err)."""
+    params, shifts, fit = _f64(p["params"]), _f64(p["shifts"]), _f64(p.get("fit_coeffs"))
+    z = np.ascontiguousarray(p["z"], dtype=np.uint64)
+    nc = max(qmc_num_components(p["family"]), 1)
+    mean, err, sm = np.zeros(2), np.zeros(2), np.zeros((p["m"], nc))
+    _check(lib().qmc_lattice_integrate_ex(p["family"], _d(params), len(params), p["dim"], p["n"], _u(z), _d(shifts), p["m"],
+                                          p["transform"], _d(fit), _d(mean), _d(err), _d(sm)), "qmc_lattice_integrate_ex")
+    return sm, mean[:nc].copy(), err[:nc].copy()
+
+
+def qmc_validate_problem_host(p: dict) -> int:
+    params, shifts, fit = _f64(p["params"]), _f64(p["shifts"]), _f64(p.get("fit_coeffs"))
+    z = np.ascontiguousarray(p["z"], dtype=np.uint64)
+    s = qmc_problem(p["family"], p["dim"], p["m"], p["transform"], p["n"], params.ctypes.data, len(params), z.ctypes.data,
+                    shifts.ctypes.data, None if fit is None else fit.ctypes.data)
+    return int(lib().qmc_validate_problem_host(C.byref(s)))
+
+
+def qmc_fit_cubic(hist):
+    H = _f64(hist)
+    d, bins = H.shape
+    out = np.zeros((d, 6))
+    _check(lib().qmc_fit_cubic(_d(H), d, bins, _d(out)), "qmc_fit_cubic")
+    return out
+
+
+class DeviceBatch:
+    """Device-resident batch of problems for the stream-ordered entry points (torch owns the memory).
+
+    Uploads the inputs once; `integrate()` then issues qmc_lattice_integrate_batch on torch's current
+    stream without synchronising.  Outputs are torch tensors: means/errs (count, 2), shift_means
+    (count, 2*max_m).
+    """
+
+    def __init__(self, problems, device="cuda:0"):
+        import torch
+        self.torch = torch
+        self.device = torch.device(device)
+        self.problems = problems
+        self.count = len(problems)
+        self._keep = []
+        arr = (qmc_problem * self.count)()
+        for i, p in enumerate(problems):
+            t_params = torch.from_numpy(_f64(p["params"])).to(self.device)
+            t_z = torch.from_numpy(np.ascontiguousarray(p["z"], dtype=np.uint64).view(np.int64)).to(self.device)
+            t_sh = torch.from_numpy(_f64(p["shifts"])).to(self.device)
+            fit = p.get("fit_coeffs")
+            t_fit = None if fit is None else torch.from_numpy(_f64(fit)).to(self.device)
+            self._keep += [t_params, t_z, t_sh, t_fit]
+            arr[i] = qmc_problem(p["family"], p["dim"], p["m"], p["transform"], p["n"], t_params.data_ptr(),
+                                 t_params.numel(), t_z.data_ptr(), t_sh.data_ptr(),
+                                 None if t_fit is None else t_fit.data_ptr())
+        self.arr = arr
+        self.max_m = max(p["m"] for p in problems)
+        self.ws_bytes = int(lib().qmc_workspace_bytes(self.count, arr))
+        if self.ws_bytes == 0:
+            st = lib().qmc_plan_info(self.count, arr, None, None, None)
+            raise QmcError(st if st != 0 else -11, "qmc_workspace_bytes")
+        self.workspace = torch.empty(self.ws_bytes + 256, dtype=torch.uint8, device=self.device)
+        off = (-self.workspace.data_ptr()) % 256
+        self.ws_ptr = self.workspace.data_ptr() + off
+        self.means = torch.zeros(self.count, 2, dtype=torch.float64, device=self.device)
+        self.errs = torch.zeros(self.count, 2, dtype=torch.float64, device=self.device)
+        self.shift_means = torch.zeros(self.count, 2 * self.max_m, dtype=torch.float64, device=self.device)
+
+    def plan_info(self):
+        tiles, ctas, tl0 = C.c_longlong(), C.c_int(), C.c_longlong()
+        _check(lib().qmc_plan_info(self.count, self.arr, C.byref(tiles), C.byref(ctas), C.byref(tl0)), "qmc_plan_info")
+        return {"tiles": tiles.value, "ctas": ctas.value, "tile_len0": tl0.value}
+
+    def integrate(self, stream=None):
+        """qmc_lattice_integrate_batch on `stream` (default: torch's current stream); returns launch count."""
+        s = self.torch.cuda.current_stream(self.device).cuda_stream if stream is None else stream
+        _check(lib().qmc_lattice_integrate_batch(self.count, self.arr, self.means.data_ptr(), self.errs.data_ptr(),
+                                                 self.shift_means.data_ptr(), self.ws_ptr, self.ws_bytes, s),
+               "qmc_lattice_integrate_batch")
+        return int(lib().qmc_last_launch_count())
+
+    def results(self):
+        """Synchronises and returns numpy (shift_means list of (m, ncomp), means (count, ncomp_max), errs)."""
+        self.torch.cuda.synchronize(self.device)
+        sm = self.shift_means.cpu().numpy()
+        means, errs = self.means.cpu().numpy(), self.errs.cpu().numpy()
+        out = []
+        for i, p in enumerate(self.problems):
+            nc = qmc_num_components(p["family"])
+            out.append(sm[i, : p["m"] * nc].reshape(p["m"], nc).copy())
+        return out, means, errs
+
+    def project(self, index=0, bins=256, stream=None):
+        """qmc_lattice_project for problem `index` -> torch tensor (dim, bins) on the device."""
+        torch = self.torch
+        p = self.problems[index]
+        one = (qmc_problem * 1)(self.arr[index])
+        need = int(lib().qmc_project_workspace_bytes(one, int(bins)))
+        if need == 0:
+            raise QmcError(-11, "qmc_project_workspace_bytes")
+        ws = torch.empty(need + 256, dtype=torch.uint8, device=self.device)
+        ptr = ws.data_ptr() + ((-ws.data_ptr()) % 256)
+        hist = torch.zeros(p["dim"], bins, dtype=torch.float64, device=self.device)
+        s = torch.cuda.current_stream(self.device).cuda_stream if stream is None else stream
+        _check(lib().qmc_lattice_project(one, int(bins), hist.data_ptr(), ptr, need, s), "qmc_lattice_project")
+        torch.cuda.synchronize(self.device)
+        return hist
+
+
+def qmc_lattice_points(n, z, shift, k0, count, device="cuda:0"):
+    """Residues (count, dim) uint64 and coordinates (count, dim) float64 from the device generator."""
+    import torch
+    z = np.ascontiguousarray(z, dtype=np.uint64)
+    shift = _f64(shift)
+    d = len(z)
+    r = torch.zeros(max(count, 1), d, dtype=torch.int64, device=device)
+    u = torch.zeros(max(count, 1), d, dtype=torch.float64, device=device)
+    s = torch.cuda.current_stream(torch.device(device)).cuda_stream
+    _check(lib().qmc_lattice_points(int(n), d, _u(z), _d(shift), int(k0), int(count), r.data_ptr(), u.data_ptr(), s),
+           "qmc_lattice_points")
+    torch.cuda.synchronize()
+    return r.cpu().numpy().view(np.uint64)[:count], u.cpu().numpy()[:count]
+
+
+def qmc_finalize_means(shift_means, device="cuda:0"):
+    """Eq. 3 on the device for given per-shift means (m, ncomp) -> (mean, err)."""
+    import torch
+    sm = _f64(shift_means)
+    if sm.ndim == 1:
+        sm = sm.reshape(-1, 1)
+    m, nc = sm.shape
+    t = torch.from_numpy(sm).to(device)
+    mean = torch.zeros(nc, dtype=torch.float64, device=device)
+    err = torch.zeros(nc, dtype=torch.float64, device=device)
+    s = torch.cuda.current_stream(torch.device(device)).cuda_stream
+    _check(lib().qmc_finalize_means(t.data_ptr(), m, nc, mean.data_ptr(), err.data_ptr(), s), "qmc_finalize_means")
+    torch.cuda.synchronize()
+    return mean.cpu().numpy(), err.cpu().numpy()
+
+
+def qmc_fp64_peak_probe(iters=20000):
+    """-> (thread-level FP64 instructions per second, kernel ms) from the DFMA-chain probe."""
+    rate, ms = C.c_double(), C.c_double()
+    _check(lib().qmc_fp64_peak_probe(int(iters), C.byref(rate), C.byref(ms), None), "qmc_fp64_peak_probe")
+    return rate.value, ms.value

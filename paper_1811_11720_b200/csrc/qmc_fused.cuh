@@ -1,0 +1,296 @@
+// qmc_fused.cuh -- the fused persistent-grid kernel of the R1SL hot path.
+//
+// One launch serves a queue of tiles (problem, range of lattice indices k).  A CTA of kThreads pops
+// tiles from a global counter (S9; the paper's host-side locked work queue is P:L388-L402).  For a
+// tile, thread t owns the indices k0 + t + i*kThreads, i < steps.  Shifts are processed G at a
+// time: for a group the thread walks its indices, steps the d residues on the integer pipe (S1),
+// and evaluates G shifted points per index with all per-shift state in registers (S2-S6).  After
+// the walk the G (x ncomp) per-thread sums are reduced by a fixed xor-butterfly + fixed-order
+// cross-warp sum and written to the tile's fixed slot (S7).  Results therefore do not depend on
+// which CTA ran a tile or in which order.
+//
+// Template parameters: FAMILY (integrand family), DP (dimension slots held in registers; the
+// runtime dim <= DP), G (shifts per group), WIDE (64-bit residues for n >= 2^31).  Transform and
+// fit map are runtime (warp-uniform) and select a fully specialised tile loop.
+#pragma once
+#include "qmc_device.cuh"
+
+namespace qmc {
+
+template <int FAMILY> struct FamTraits;
+template <> struct FamTraits<QMC_FAMILY_GENZ_OSC> { static constexpr int NC = 1; static constexpr int NS = 1; };
+template <> struct FamTraits<QMC_FAMILY_GENZ_PRODPEAK> { static constexpr int NC = 1; static constexpr int NS = 1; };
+template <> struct FamTraits<QMC_FAMILY_CEXP_POLY> { static constexpr int NC = 2; static constexpr int NS = 2; };
+
+// Shared-memory image of the problem a CTA is working on.
+template <int DP, int G> struct SmemCtx {
+    double delta[G * DP];          // shifts of the current group, [q][j]
+    double fam_a[DP], fam_b[DP];
+    double fit[5][DP];
+    double kor[8];
+    unsigned long long z[DP], step[DP], back[DP];
+    double red[kWarps][G * 2];
+    DevProblem prob;
+    double fam0;
+    long long tile;                // popped tile index
+};
+
+// ---- per-dimension and per-point pieces of the closed-form families (S5) ----------------------
+//  OSC       f = cos(2 pi u0 + sum a_j x_j)
+//  PRODPEAK  f = prod 1/(c_j^-2 + (x_j - w_j)^2)  = 1 / prod(...)
+//  CEXP      f = exp(i sum a_j x_j) prod (1 + b_j x_j)             BASELINE.json configs[2]
+template <int FAMILY> __device__ __forceinline__ void fam_init(double& s0, double& s1, double fam0) {
+    if (FAMILY == QMC_FAMILY_GENZ_OSC) { s0 = fam0; s1 = 0.0; }
+    else if (FAMILY == QMC_FAMILY_GENZ_PRODPEAK) { s0 = 1.0; s1 = 0.0; }
+    else { s0 = 0.0; s1 = 1.0; }
+}
+template <int FAMILY> __device__ __forceinline__ void fam_dim(double& s0, double& s1, double x, double fa, double fb) {
+    if (FAMILY == QMC_FAMILY_GENZ_OSC) { s0 = __fma_rn(fa, x, s0); }
+    else if (FAMILY == QMC_FAMILY_GENZ_PRODPEAK) { const double t = x - fb; s0 *= __fma_rn(t, t, fa); }   // fa = c_j^-2, fb = w_j
+    else { s0 = __fma_rn(fa, x, s0); s1 *= __fma_rn(fb, x, 1.0); }
+}
+// adds W*f to acc[0..NC)
+template <int FAMILY> __device__ __forceinline__ void fam_finish(double s0, double s1, double W, bool use_w, double* acc) {
+    if (FAMILY == QMC_FAMILY_GENZ_OSC) {
+        const double f = cos(s0);
+        acc[0] = use_w ? __fma_rn(W, f, acc[0]) : acc[0] + f;
+    } else if (FAMILY == QMC_FAMILY_GENZ_PRODPEAK) {
+        acc[0] += use_w ? W / s0 : 1.0 / s0;
+    } else {
+        double sn, cs;
+        sincos(s0, &sn, &cs);
+        const double a = use_w ? W * s1 : s1;
+        acc[0] = __fma_rn(a, cs, acc[0]);
+        acc[1] = __fma_rn(a, sn, acc[1]);
+    }
+}
+
+// ---- S2-S4 for one (shift q, dimension j): coordinate, periodizing transform, fit map ----------
+// Returns x_j; multiplies P by u(1-u) (Korobov) and D by p'(y) (fit).
+template <int DP, int G, int TR, bool FIT>
+__device__ __forceinline__ double point_coord(double rd, double inv_n, int q, int j, const SmemCtx<DP, G>& sm, int kor_r,
+                                              double& P, double& D) {
+    const double t = coord_t(rd, inv_n, sm.delta[q * DP + j]);
+    double x;
+    if (TR == TR_NONE) {
+        x = wrap_u(t);
+    } else {
+        const double c = centre_c(t);
+        if (TR == TR_BAKER) {
+            x = baker_y(c);
+        } else {
+            const double s = c * c;
+            P *= (0.25 - s);                                  // u (1-u)
+            double g;
+            if (TR == TR_KOR3) {                              // g_3(s) = 35/16 - 35/4 s + 21 s^2 - 20 s^3
+                g = __fma_rn(-20.0, s, 21.0);
+                g = __fma_rn(g, s, -8.75);
+                g = __fma_rn(g, s, 2.1875);
+            } else {
+                g = sm.kor[kor_r];
+#pragma unroll 1
+                for (int i = kor_r - 1; i >= 0; --i) g = __fma_rn(g, s, sm.kor[i]);
+            }
+            x = __fma_rn(c, g, 0.5);                          // phi(u) = 1/2 + c g(c^2)
+        }
+    }
+    if (FIT) {                                                // S4: cubic map of Eq. 19 (a2 = a3 = 0)
+        const double y = x;
+        const double h = __fma_rn(y, __fma_rn(y, sm.fit[2][j], sm.fit[1][j]), sm.fit[0][j]);
+        D *= __fma_rn(y, __fma_rn(y, sm.fit[4][j], sm.fit[3][j]), sm.fit[0][j]);   // p'(y)
+        x = y * h;                                            // p(y)
+    }
+    return x;
+}
+
+// Weight W = prod_j omega(u_j) p'(y_j) from the carried products (Eq. 12, Eq. 18).
+template <int TR, bool FIT> __device__ __forceinline__ double point_weight(double P, double D, double wconst, int kor_r) {
+    double W = 1.0;
+    if (TR == TR_KOR3) W = wconst * (P * P * P);
+    else if (TR == TR_KORR) W = wconst * ipow_small(P, kor_r);
+    if (FIT) W = (TR == TR_KOR3 || TR == TR_KORR) ? W * D : D;
+    return W;
+}
+
+// ---- one lattice index, G shifts: S2-S6 for the closed-form families --------------------------
+template <int FAMILY, int DP, int G, bool WIDE, int TR, bool FIT>
+__device__ __forceinline__ void eval_point_group(const typename Res<WIDE>::T (&r)[DP], const SmemCtx<DP, G>& sm, int dim,
+                                                 double inv_n, double wconst, int kor_r,
+                                                 double (&acc)[G][FamTraits<FAMILY>::NC]) {
+    double s0[G], s1[G], P[G], D[G];
+#pragma unroll
+    for (int q = 0; q < G; ++q) { fam_init<FAMILY>(s0[q], s1[q], sm.fam0); P[q] = 1.0; D[q] = 1.0; }
+#pragma unroll
+    for (int j = 0; j < DP; ++j) {
+        if (j < dim) {
+            const double rd = Res<WIDE>::to_double(r[j]);
+            const double fa = sm.fam_a[j], fb = sm.fam_b[j];
+#pragma unroll
+            for (int q = 0; q < G; ++q) {
+                const double x = point_coord<DP, G, TR, FIT>(rd, inv_n, q, j, sm, kor_r, P[q], D[q]);
+                fam_dim<FAMILY>(s0[q], s1[q], x, fa, fb);
+            }
+        }
+    }
+    constexpr bool USEW = (TR == TR_KOR3 || TR == TR_KORR || FIT);
+#pragma unroll
+    for (int q = 0; q < G; ++q)
+        fam_finish<FAMILY>(s0[q], s1[q], point_weight<TR, FIT>(P[q], D[q], wconst, kor_r), USEW, acc[q]);
+}
+
+struct NoExtra {};
+
+template <int FAMILY, int DP, int G, bool WIDE, int TR, bool FIT> struct ClosedEval {
+    static constexpr int NC = FamTraits<FAMILY>::NC;
+    typedef NoExtra Extra;
+    static __device__ __forceinline__ void eval(const typename Res<WIDE>::T (&r)[DP], const SmemCtx<DP, G>& sm, const Extra&,
+                                                int dim, double inv_n, double wconst, int kor_r, double (&acc)[G][NC]) {
+        eval_point_group<FAMILY, DP, G, WIDE, TR, FIT>(r, sm, dim, inv_n, wconst, kor_r, acc);
+    }
+};
+
+// ---- one tile: residue walk (S1), G shifts per index (EV::eval = S2-S6), tile reduction (S7) ----
+template <class EV, int DP, int G, bool WIDE>
+__device__ __forceinline__ void run_tile(SmemCtx<DP, G>& sm, const typename EV::Extra& ex, long long tile_local,
+                                         double* __restrict__ partials) {
+    typedef typename Res<WIDE>::T RT;
+    constexpr int NC = EV::NC;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const DevProblem& pb = sm.prob;
+    const int dim = pb.dim, m = pb.m, steps = pb.steps, kor_r = pb.kor_r;
+    const unsigned long long n = pb.n;
+    const double inv_n = pb.inv_n, wconst = pb.wconst;
+    const unsigned long long tile_len = (unsigned long long)steps * kThreads;
+    const unsigned long long k0 = (unsigned long long)tile_local * tile_len;
+    const unsigned long long kend = (k0 + tile_len < n) ? k0 + tile_len : n;
+    const unsigned long long kfirst = k0 + tid;
+
+    RT r[DP];
+#pragma unroll
+    for (int j = 0; j < DP; ++j) r[j] = (j < dim) ? (RT)mulmod_u64(kfirst % n, sm.z[j], n) : (RT)0;
+
+#pragma unroll 1
+    for (int g0 = 0; g0 < m; g0 += G) {
+        const int gcount = (m - g0 < G) ? (m - g0) : G;
+        __syncthreads();                                    // previous group's readers of delta/red are done
+        for (int e = tid; e < G * DP; e += kThreads) {
+            const int q = e / DP, j = e - q * DP;
+            sm.delta[e] = (q < gcount && j < dim) ? pb.shifts[(size_t)(g0 + q) * dim + j] : 0.0;
+        }
+        __syncthreads();
+
+        double acc[G][NC];
+#pragma unroll
+        for (int q = 0; q < G; ++q)
+#pragma unroll
+            for (int c = 0; c < NC; ++c) acc[q][c] = 0.0;
+
+        unsigned long long k = kfirst;
+#pragma unroll 1
+        for (int i = 0; i < steps; ++i) {
+            asm volatile("" ::: "memory");   // keep the shared-memory operands as loads inside the walk (no hoisting into registers)
+            if (k < kend) EV::eval(r, sm, ex, dim, inv_n, wconst, kor_r, acc);
+#pragma unroll
+            for (int j = 0; j < DP; ++j)
+                if (j < dim) r[j] = add_mod<RT>(r[j], (RT)sm.step[j], (RT)n);
+            k += kThreads;
+        }
+        // rewind to the thread's first index for the next group
+#pragma unroll
+        for (int j = 0; j < DP; ++j)
+            if (j < dim) r[j] = sub_mod<RT>(r[j], (RT)sm.back[j], (RT)n);
+
+        // S7: fixed-shape reduction of the group's sums, one slot per (tile, shift, component)
+#pragma unroll
+        for (int q = 0; q < G; ++q)
+#pragma unroll
+            for (int c = 0; c < NC; ++c) {
+                const double v = warp_sum(acc[q][c]);
+                if (lane == 0) sm.red[warp][q * NC + c] = v;
+            }
+        __syncthreads();
+        if (tid < G * NC) {
+            const int q = tid / NC, c = tid - q * NC;
+            if (q < gcount) {
+                double v = sm.red[0][tid];
+#pragma unroll
+                for (int w = 1; w < kWarps; ++w) v += sm.red[w][tid];
+                partials[pb.partial_off + ((long long)(g0 + q) * NC + c) * pb.tiles + tile_local] = v;
+            }
+        }
+    }
+}
+
+// ---- queue handling shared by all fused kernels ------------------------------------------------
+// Pops the next tile; returns false when the queue is empty.  On a problem change the CTA reloads
+// its shared-memory image of the problem (changed = true).  `cur` = problem index loaded (-1: none).
+template <int DP, int G>
+__device__ __forceinline__ bool next_tile(SmemCtx<DP, G>& sm, const DevProblem* __restrict__ probs,
+                                          const DevAux* __restrict__ aux, const VariantQueue& vq, int& cur,
+                                          long long& tile_local, bool& changed) {
+    const int tid = threadIdx.x;
+    changed = false;
+    __syncthreads();                                        // everyone is done with the previous tile
+    if (tid == 0) sm.tile = (long long)atomicAdd(vq.counter, 1ull);
+    __syncthreads();
+    const long long tile = sm.tile;
+    if (tile >= vq.total_tiles) return false;
+    int lo = 0, hi = vq.plist_len;                          // largest lo with tile_prefix[lo] <= tile
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (__ldg(&vq.tile_prefix[mid]) <= tile) lo = mid; else hi = mid;
+    }
+    tile_local = tile - __ldg(&vq.tile_prefix[lo]);
+    const int pidx = __ldg(&vq.plist[lo]);
+    if (pidx != cur) {
+        cur = pidx;
+        changed = true;
+        if (tid == 0) sm.prob = probs[pidx];
+        const DevAux& a = aux[pidx];
+        if (tid == 32) sm.fam0 = a.fam0;
+        if (tid >= 64 && tid < 72) sm.kor[tid - 64] = probs[pidx].kor[tid - 64];
+        for (int j = tid; j < DP; j += kThreads) {
+            sm.z[j] = a.z[j]; sm.step[j] = a.step[j]; sm.back[j] = a.back[j];
+            sm.fam_a[j] = a.fam_a[j]; sm.fam_b[j] = a.fam_b[j];
+#pragma unroll
+            for (int i = 0; i < 5; ++i) sm.fit[i][j] = a.fit[i][j];
+        }
+        __syncthreads();
+    }
+    return true;
+}
+
+// resident CTAs per SM the register budget is sized for (128 / 168 / 255 registers per thread)
+template <int DP, bool WIDE> struct MinBlocks { static constexpr int value = (DP <= 8) ? 4 : (DP <= 16 ? (WIDE ? 2 : 3) : 2); };
+
+template <int FAMILY, int DP, int G, bool WIDE>
+__global__ void __launch_bounds__(kThreads, MinBlocks<DP, WIDE>::value) fused_kernel(const DevProblem* __restrict__ probs,
+                                                         const DevAux* __restrict__ aux, VariantQueue vq,
+                                                         double* __restrict__ partials) {
+    __shared__ SmemCtx<DP, G> sm;
+    int cur = -1;
+    long long tile_local = 0;
+    bool changed;
+    NoExtra ex;
+    while (next_tile<DP, G>(sm, probs, aux, vq, cur, tile_local, changed)) {
+        const int sel = sm.prob.tr_kind * 2 + (sm.prob.has_fit ? 1 : 0);
+        switch (sel) {
+#define QMC_CASE(TRK, FITB) \
+    case TRK * 2 + (FITB ? 1 : 0): run_tile<ClosedEval<FAMILY, DP, G, WIDE, TRK, FITB>, DP, G, WIDE>(sm, ex, tile_local, partials); break;
+            QMC_CASE(TR_NONE, false) QMC_CASE(TR_NONE, true) QMC_CASE(TR_BAKER, false) QMC_CASE(TR_BAKER, true)
+            QMC_CASE(TR_KOR3, false) QMC_CASE(TR_KOR3, true) QMC_CASE(TR_KORR, false) QMC_CASE(TR_KORR, true)
+#undef QMC_CASE
+            default: break;
+        }
+    }
+}
+
+// Arguments of every fused kernel; launcher tables are instantiated per family in qmc_fused_f*.cu
+struct FusedArgs {
+    const DevProblem* probs;
+    const DevAux* aux;
+    VariantQueue vq;
+    double* partials;
+};
+
+}  // namespace qmc

@@ -1,0 +1,586 @@
+// qmc_host.cu -- the C ABI of include/qmc_lattice.h: validation, launch planning, workspace layout
+// and launches.  Every step of the hot path runs in the CUDA kernels; there is no CPU fallback.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <numeric>
+#include <string>
+#include <vector>
+
+#include "qmc_fused.cuh"
+#include "qmc_kernels.h"
+
+namespace qmc {
+namespace {
+
+thread_local std::string g_last_error;
+thread_local int g_last_launches = 0;
+
+int cuda_fail(cudaError_t e, const char* where) {
+    g_last_error = std::string(where) + ": " + cudaGetErrorString(e);
+    return QMC_ERR_CUDA;
+}
+#define QMC_CUDA(call)                                              \
+    do {                                                            \
+        cudaError_t e_ = (call);                                    \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #call);         \
+    } while (0)
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+int ncomp_of(int family) {
+    if (family == QMC_FAMILY_CEXP_POLY) return 2;
+    if (family >= 0 && family <= QMC_FAMILY_SECTOR) return 1;
+    return -1;
+}
+
+int dim_slots(int family, int dim) {
+    if (family == QMC_FAMILY_SECTOR) return dim <= 4 ? 4 : (dim <= 8 ? 8 : (dim <= 16 ? 16 : -1));
+    return dim <= 4 ? 4 : (dim <= 8 ? 8 : (dim <= 16 ? 16 : 32));
+}
+
+bool decode_transform(int transform, int* kind, int* r) {
+    if (transform == QMC_TRANSFORM_NONE) { *kind = TR_NONE; *r = 0; return true; }
+    if (transform == QMC_TRANSFORM_BAKER) { *kind = TR_BAKER; *r = 0; return true; }
+    if (transform >= QMC_TRANSFORM_KOROBOV + 1 && transform <= QMC_TRANSFORM_KOROBOV + 6) {
+        *r = transform - QMC_TRANSFORM_KOROBOV;
+        *kind = (*r == 3) ? TR_KOR3 : TR_KORR;
+        return true;
+    }
+    return false;
+}
+
+double binom(int a, int b) {
+    double v = 1.0;
+    for (int i = 1; i <= b; ++i) v = v * (double)(a - b + i) / (double)i;
+    return v;
+}
+
+// struct-level validation (no dereference of the data pointers)
+int validate_struct(const qmc_problem& p, bool need_two_shifts) {
+    if (ncomp_of(p.family) < 0) return QMC_ERR_FAMILY;
+    if (p.dim < 1 || p.dim > QMC_MAX_DIM) return QMC_ERR_DIM;
+    if (dim_slots(p.family, p.dim) < 0) return QMC_ERR_DIM;
+    if (p.n < 2 || p.n >= (1ull << 53)) return QMC_ERR_N;
+    if (p.m < (need_two_shifts ? 2 : 1) || p.m > QMC_MAX_M) return QMC_ERR_M;
+    int kind, r;
+    if (!decode_transform(p.transform, &kind, &r)) return QMC_ERR_TRANSFORM;
+    if (!p.params || !p.z || !p.shifts) return QMC_ERR_NULL;
+    if (p.family == QMC_FAMILY_GENZ_OSC && p.n_params != 1 + p.dim) return QMC_ERR_PARAMS;
+    if ((p.family == QMC_FAMILY_GENZ_PRODPEAK || p.family == QMC_FAMILY_CEXP_POLY) && p.n_params != 2 * p.dim) return QMC_ERR_PARAMS;
+    if (p.family == QMC_FAMILY_SECTOR) {
+        const int rest = p.n_params - 4 - p.dim;
+        if (rest < 2 * (1 + p.dim) || rest % (1 + p.dim) != 0 || rest / (1 + p.dim) > 2 * kMaxSectorMono) return QMC_ERR_PARAMS;
+    }
+    return QMC_OK;
+}
+
+int tiles_target() {
+    static const int v = [] {
+        const char* e = std::getenv("QMC_TILES_TARGET");
+        const int t = e ? std::atoi(e) : 0;
+        return t > 0 ? t : kTilesTarget;
+    }();
+    return v;
+}
+
+// ---- launch plan: tiles, kernel variants, workspace layout (pure function of the problem structs) ----
+struct Variant {
+    int family, dp;
+    bool wide;
+    std::vector<int> plist;          // problem indices, queue order (most expensive tiles first)
+    long long total_tiles = 0;
+};
+
+struct Plan {
+    std::vector<DevProblem> dev;
+    std::vector<Variant> variants;
+    int max_m = 0;
+    size_t off_counters = 0, off_probs = 0, off_plist = 0, off_prefix = 0, off_aux = 0, off_prog = 0, off_means = 0,
+           off_partials = 0, total = 0;
+    size_t prog_words = 0, means_doubles = 0, partial_doubles = 0;
+    long long total_tiles = 0;
+};
+
+int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan* plan) {
+    if (count < 1 || !problems) return count < 1 ? QMC_ERR_N : QMC_ERR_NULL;
+    plan->dev.resize(count);
+    const int per_problem_target = std::max(16, tiles_target() / count);
+    long long partial_off = 0, means_off = 0;
+    size_t prog_off = 0;
+    for (int i = 0; i < count; ++i) {
+        const qmc_problem& p = problems[i];
+        const int st = validate_struct(p, need_two_shifts);
+        if (st != QMC_OK) return st;
+        DevProblem d;
+        std::memset(&d, 0, sizeof(d));
+        d.params = p.params; d.z = reinterpret_cast<const unsigned long long*>(p.z); d.shifts = p.shifts; d.fit = p.fit_coeffs;
+        d.n = p.n;
+        d.inv_n = 1.0 / (double)p.n;                                   // reading C-2
+        d.family = p.family; d.dim = p.dim; d.m = p.m; d.ncomp = ncomp_of(p.family);
+        decode_transform(p.transform, &d.tr_kind, &d.kor_r);
+        d.has_fit = p.fit_coeffs ? 1 : 0;
+        d.n_params = p.n_params;
+        d.out_index = i;
+        d.wconst = 1.0;
+        if (d.kor_r > 0) {
+            // Eq. 15: c_r = (2r+1) C(2r,r); centred antiderivative coefficients of Eq. 14 (see qmc_device.cuh)
+            const int r = d.kor_r;
+            const double cr = (2.0 * r + 1.0) * binom(2 * r, r);
+            for (int k = 0; k <= r; ++k)
+                d.kor[k] = cr * binom(r, k) * std::ldexp(1.0, 2 * (k - r)) * ((k & 1) ? -1.0 : 1.0) / (double)(2 * k + 1);
+            for (int j = 0; j < p.dim; ++j) d.wconst *= cr;
+        }
+        const unsigned long long per = (unsigned long long)kThreads * (unsigned long long)per_problem_target;
+        unsigned long long steps = (p.n + per - 1) / per;
+        steps = std::min<unsigned long long>(std::max<unsigned long long>(steps, 1), kMaxSteps);
+        const unsigned long long tile_len = steps * kThreads;
+        const unsigned long long tiles = (p.n + tile_len - 1) / tile_len;
+        if (tiles > 0x7fffffffull) return QMC_ERR_N;
+        d.steps = (int)steps;
+        d.tiles = (int)tiles;
+        d.partial_off = partial_off;
+        d.means_off = means_off;
+        partial_off += (long long)tiles * p.m * d.ncomp;
+        means_off += (long long)p.m * d.ncomp;
+        if (p.family == QMC_FAMILY_SECTOR) {
+            const int nmono = (p.n_params - 4 - p.dim) / (1 + p.dim);
+            d.aux_off = (int)prog_off;
+            d.aux_len = 5 * nmono;                                      // coefs + 16 u16 ops per monomial
+            prog_off += (size_t)d.aux_len;
+        }
+        plan->max_m = std::max(plan->max_m, p.m);
+        plan->dev[i] = d;
+    }
+    // kernel variants
+    for (int i = 0; i < count; ++i) {
+        const DevProblem& d = plan->dev[i];
+        const int dp = dim_slots(d.family, d.dim);
+        const bool wide = d.n >= (1ull << 31);
+        Variant* v = nullptr;
+        for (auto& c : plan->variants)
+            if (c.family == d.family && c.dp == dp && c.wide == wide) v = &c;
+        if (!v) { plan->variants.push_back(Variant{d.family, dp, wide, {}, 0}); v = &plan->variants.back(); }
+        v->plist.push_back(i);
+    }
+    if (plan->variants.size() > 64) return QMC_ERR_WORKSPACE;
+    for (auto& v : plan->variants) {
+        // most expensive tiles first (S9); cost ~ indices x shifts x (dimension work + integrand size)
+        auto cost = [&](int i) {
+            const DevProblem& d = plan->dev[i];
+            return (double)d.steps * d.m * (12.0 * d.dim + 0.5 * d.n_params + 40.0);
+        };
+        std::stable_sort(v.plist.begin(), v.plist.end(), [&](int a, int b) { return cost(a) > cost(b); });
+        for (int i : v.plist) { plan->dev[i].tile_begin = v.total_tiles; v.total_tiles += plan->dev[i].tiles; }
+        plan->total_tiles += v.total_tiles;
+    }
+    plan->prog_words = prog_off;
+    plan->means_doubles = (size_t)means_off;
+    plan->partial_doubles = (size_t)partial_off;
+    size_t o = 0;
+    plan->off_counters = o; o = align_up(o + 64 * sizeof(unsigned long long), 256);
+    plan->off_probs = o; o = align_up(o + (size_t)count * sizeof(DevProblem), 256);
+    plan->off_plist = o; o = align_up(o + (size_t)count * sizeof(int), 256);
+    plan->off_prefix = o; o = align_up(o + ((size_t)count + plan->variants.size()) * sizeof(long long), 256);
+    plan->off_aux = o; o = align_up(o + (size_t)count * sizeof(DevAux), 256);
+    plan->off_prog = o; o = align_up(o + plan->prog_words * 8, 256);
+    plan->off_means = o; o = align_up(o + plan->means_doubles * 8, 256);
+    plan->off_partials = o; o = align_up(o + plan->partial_doubles * 8, 256);
+    plan->total = o;
+    return QMC_OK;
+}
+
+int sm_count() {
+    static const int v = [] {
+        int dev = 0, n = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
+        return n;
+    }();
+    return v;
+}
+
+int occupancy(int family, int dp, bool wide) {
+    static int cache[4][33][2];
+    int& c = cache[family][dp][wide ? 1 : 0];
+    if (c > 0) return c;
+    int v = -1;
+    switch (family) {
+        case 0: v = occupancy_fused_f0(dp, wide); break;
+        case 1: v = occupancy_fused_f1(dp, wide); break;
+        case 2: v = occupancy_fused_f2(dp, wide); break;
+        case 3: v = occupancy_fused_f3(dp, wide); break;
+    }
+    if (v > 0) c = v;
+    return v;
+}
+
+int run_batch(int count, const qmc_problem* problems, double* out_means, double* out_errs, double* out_shift_means,
+              void* workspace, size_t workspace_bytes, cudaStream_t st) {
+    g_last_launches = 0;
+    if (!out_means || !out_errs) return QMC_ERR_NULL;
+    Plan plan;
+    const int pst = make_plan(count, problems, true, &plan);
+    if (pst != QMC_OK) return pst;
+    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || workspace_bytes < plan.total) return QMC_ERR_WORKSPACE;
+    const int sms = sm_count();
+    if (sms <= 0) return cuda_fail(cudaErrorNoDevice, "no CUDA device");
+    char* ws = static_cast<char*>(workspace);
+
+    // host image of [probs | plist | prefix]
+    const size_t blob_bytes = plan.off_aux - plan.off_probs;
+    std::vector<char> blob(blob_bytes, 0);
+    std::memcpy(blob.data(), plan.dev.data(), (size_t)count * sizeof(DevProblem));
+    int* plist = reinterpret_cast<int*>(blob.data() + (plan.off_plist - plan.off_probs));
+    long long* prefix = reinterpret_cast<long long*>(blob.data() + (plan.off_prefix - plan.off_probs));
+    std::vector<VariantQueue> queues;
+    {
+        size_t pl = 0, pf = 0;
+        int vi = 0;
+        for (auto& v : plan.variants) {
+            VariantQueue q;
+            q.plist = reinterpret_cast<const int*>(ws + plan.off_plist) + pl;
+            q.tile_prefix = reinterpret_cast<const long long*>(ws + plan.off_prefix) + pf;
+            q.plist_len = (int)v.plist.size();
+            q.total_tiles = v.total_tiles;
+            q.counter = reinterpret_cast<unsigned long long*>(ws + plan.off_counters) + vi;
+            long long acc = 0;
+            for (int i : v.plist) { plist[pl++] = i; prefix[pf++] = acc; acc += plan.dev[i].tiles; }
+            prefix[pf++] = acc;
+            queues.push_back(q);
+            ++vi;
+        }
+    }
+    QMC_CUDA(cudaMemsetAsync(ws + plan.off_counters, 0, 64 * sizeof(unsigned long long), st));
+    QMC_CUDA(cudaMemcpyAsync(ws + plan.off_probs, blob.data(), blob_bytes, cudaMemcpyHostToDevice, st));
+    const DevProblem* dprobs = reinterpret_cast<const DevProblem*>(ws + plan.off_probs);
+    DevAux* daux = reinterpret_cast<DevAux*>(ws + plan.off_aux);
+    unsigned long long* dprog = reinterpret_cast<unsigned long long*>(ws + plan.off_prog);
+    double* dmeans = reinterpret_cast<double*>(ws + plan.off_means);
+    double* dpart = reinterpret_cast<double*>(ws + plan.off_partials);
+    QMC_CUDA(launch_prepare(count, st, dprobs, daux, dprog));
+    ++g_last_launches;
+    for (size_t vi = 0; vi < plan.variants.size(); ++vi) {
+        const Variant& v = plan.variants[vi];
+        const int occ = occupancy(v.family, v.dp, v.wide);
+        if (occ <= 0) return cuda_fail(cudaErrorInvalidDeviceFunction, "occupancy query (is the sm_100a image loadable on this device?)");
+        const long long cap = (long long)sms * occ;
+        const int grid = (int)std::min<long long>(cap, v.total_tiles);
+        FusedArgs a{dprobs, daux, queues[vi], dpart};
+        cudaError_t e = cudaErrorInvalidValue;
+        switch (v.family) {
+            case 0: e = launch_fused_f0(v.dp, v.wide, grid, st, a); break;
+            case 1: e = launch_fused_f1(v.dp, v.wide, grid, st, a); break;
+            case 2: e = launch_fused_f2(v.dp, v.wide, grid, st, a); break;
+            case 3: e = launch_fused_f3(v.dp, v.wide, grid, st, a, dprog); break;
+        }
+        if (e != cudaSuccess) return cuda_fail(e, "fused kernel launch");
+        ++g_last_launches;
+    }
+    QMC_CUDA(launch_finalize(count, st, dprobs, daux, dpart, dmeans, out_means, out_errs, out_shift_means, 2 * plan.max_m));
+    ++g_last_launches;
+    return QMC_OK;
+}
+
+// ---- full value validation of host-resident data --------------------------------------------------
+unsigned long long gcd_u64(unsigned long long a, unsigned long long b) {
+    while (b) { const unsigned long long t = a % b; a = b; b = t; }
+    return a;
+}
+
+int validate_values(const qmc_problem& p) {
+    const int st = validate_struct(p, true);
+    if (st != QMC_OK) return st;
+    for (int j = 0; j < p.dim; ++j) {
+        const unsigned long long z = p.z[j];
+        if (z < 1 || z >= p.n || gcd_u64(z, p.n) != 1) return QMC_ERR_Z;          // "coprime to n"
+    }
+    for (long long i = 0; i < (long long)p.m * p.dim; ++i)
+        if (!(p.shifts[i] >= 0.0 && p.shifts[i] < 1.0)) return QMC_ERR_SHIFT;      // Delta in [0,1)
+    for (int i = 0; i < p.n_params; ++i)
+        if (!std::isfinite(p.params[i])) return QMC_ERR_PARAMS;
+    if (p.family == QMC_FAMILY_GENZ_PRODPEAK)
+        for (int j = 0; j < p.dim; ++j)
+            if (p.params[j] == 0.0) return QMC_ERR_PARAMS;
+    if (p.family == QMC_FAMILY_SECTOR) {
+        const double* q = p.params;
+        for (int k = 0; k < 4; ++k)
+            if (q[k] != std::floor(q[k]) || q[k] < 0.0) return QMC_ERR_PARAMS;
+        if (q[0] > 8 || q[1] > 8 || q[2] < 1 || q[3] < 1 || q[2] > kMaxSectorMono || q[3] > kMaxSectorMono) return QMC_ERR_PARAMS;
+        if (4 + p.dim + ((int)q[2] + (int)q[3]) * (1 + p.dim) != p.n_params) return QMC_ERR_PARAMS;
+    }
+    if (p.fit_coeffs) {
+        for (int j = 0; j < p.dim; ++j) {
+            const double* a = p.fit_coeffs + 6 * j;
+            for (int k = 0; k < 6; ++k)
+                if (!std::isfinite(a[k])) return QMC_ERR_FIT;
+            if (a[2] != 0.0 || a[3] != 0.0) return QMC_ERR_FIT;   // pole terms of Eq. 19: not on the fused path yet
+            const double a4 = a[4], a5 = a[5], a6 = 1.0 - a[2] - a[3] - a4 - a5;
+            // p'(y) = a4 + 2 a5 y + 3 a6 y^2 must stay positive on [0,1] (monotone map, Eq. 18)
+            double mn = std::fmin(a4, a4 + 2.0 * a5 + 3.0 * a6);
+            if (a6 != 0.0) {
+                const double yv = -a5 / (3.0 * a6);
+                if (yv > 0.0 && yv < 1.0) mn = std::fmin(mn, a4 + yv * (2.0 * a5 + 3.0 * a6 * yv));
+            }
+            if (!(mn > 0.0)) return QMC_ERR_FIT;
+        }
+    }
+    return QMC_OK;
+}
+
+int family_param_count(int family, const double* params, int dim) {
+    if (family == QMC_FAMILY_GENZ_OSC) return 1 + dim;
+    if (family == QMC_FAMILY_GENZ_PRODPEAK || family == QMC_FAMILY_CEXP_POLY) return 2 * dim;
+    if (family == QMC_FAMILY_SECTOR && params) {
+        const double nU = params[2], nF = params[3];
+        if (!(nU >= 1 && nU <= kMaxSectorMono && nF >= 1 && nF <= kMaxSectorMono)) return -1;
+        return 4 + dim + ((int)nU + (int)nF) * (1 + dim);
+    }
+    return -1;
+}
+
+}  // namespace
+}  // namespace qmc
+
+using namespace qmc;
+
+extern "C" {
+
+int qmc_num_components(int family) { return ncomp_of(family); }
+
+const char* qmc_status_string(int status) {
+    switch (status) {
+        case QMC_OK: return "ok";
+        case QMC_ERR_NULL: return "null pointer";
+        case QMC_ERR_DIM: return "dimension out of range";
+        case QMC_ERR_N: return "lattice size / count out of range";
+        case QMC_ERR_Z: return "generating vector component out of range or not coprime to n";
+        case QMC_ERR_SHIFT: return "shift outside [0,1)";
+        case QMC_ERR_M: return "number of shifts out of range";
+        case QMC_ERR_TRANSFORM: return "unknown periodizing transform";
+        case QMC_ERR_FAMILY: return "unknown integrand family";
+        case QMC_ERR_PARAMS: return "integrand parameter block invalid";
+        case QMC_ERR_FIT: return "fit map invalid";
+        case QMC_ERR_WORKSPACE: return "workspace null, misaligned or too small";
+        case QMC_ERR_CUDA: return "CUDA error";
+        case QMC_ERR_NONFINITE: return "non-finite result";
+    }
+    return "unknown status";
+}
+
+const char* qmc_last_cuda_error(void) { return g_last_error.c_str(); }
+int qmc_last_launch_count(void) { return g_last_launches; }
+
+size_t qmc_workspace_bytes(int count, const qmc_problem* problems) {
+    Plan plan;
+    if (make_plan(count, problems, true, &plan) != QMC_OK) return 0;
+    return plan.total;
+}
+
+int qmc_plan_info(int count, const qmc_problem* problems, long long* out_tiles, int* out_ctas, long long* out_tile_len0) {
+    Plan plan;
+    const int st = make_plan(count, problems, true, &plan);
+    if (st != QMC_OK) return st;
+    if (out_tiles) *out_tiles = plan.total_tiles;
+    if (out_tile_len0) *out_tile_len0 = (long long)plan.dev[0].steps * kThreads;
+    if (out_ctas) {
+        int ctas = 0;
+        const int sms = sm_count();
+        for (auto& v : plan.variants) {
+            const int occ = sms > 0 ? occupancy(v.family, v.dp, v.wide) : 0;
+            ctas += (int)std::min<long long>((long long)sms * std::max(occ, 0), v.total_tiles);
+        }
+        *out_ctas = ctas;
+    }
+    return QMC_OK;
+}
+
+int qmc_validate_problem_host(const qmc_problem* p) {
+    if (!p) return QMC_ERR_NULL;
+    return validate_values(*p);
+}
+
+int qmc_lattice_integrate_batch(int count, const qmc_problem* problems, double* out_means, double* out_errs,
+                                double* out_shift_means, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    return run_batch(count, problems, out_means, out_errs, out_shift_means, workspace, workspace_bytes,
+                     static_cast<cudaStream_t>(cuda_stream));
+}
+
+int qmc_lattice_integrate_ex(int family, const double* params, int n_params, int dim, uint64_t n, const uint64_t* z,
+                             const double* shifts, int m, int transform, const double* fit_coeffs, double* out_mean,
+                             double* out_err, double* out_shift_means) {
+    if (!params || !z || !shifts || !out_mean || !out_err) return QMC_ERR_NULL;
+    qmc_problem hp;
+    hp.family = family; hp.dim = dim; hp.m = m; hp.transform = transform; hp.n = n;
+    hp.params = params; hp.n_params = n_params; hp.z = z; hp.shifts = shifts; hp.fit_coeffs = fit_coeffs;
+    const int vst = validate_values(hp);
+    if (vst != QMC_OK) return vst;
+    const int nc = ncomp_of(family);
+    // one stream-ordered allocation: [params | z | shifts | fit | out_means(2) | out_errs(2) | shift_means(2m) | workspace]
+    const size_t b_params = align_up((size_t)n_params * 8, 256), b_z = align_up((size_t)dim * 8, 256),
+                 b_sh = align_up((size_t)m * dim * 8, 256), b_fit = align_up((size_t)dim * 6 * 8, 256),
+                 b_out = align_up((size_t)(4 + 2 * m) * 8, 256);
+    qmc_problem dp = hp;
+    Plan plan;
+    const int pst = make_plan(1, &hp, true, &plan);
+    if (pst != QMC_OK) return pst;
+    const size_t total = b_params + b_z + b_sh + b_fit + b_out + plan.total;
+    cudaStream_t st = 0;
+    char* buf = nullptr;
+    QMC_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&buf), total, st));
+    char* d_params = buf;
+    char* d_z = d_params + b_params;
+    char* d_sh = d_z + b_z;
+    char* d_fit = d_sh + b_sh;
+    double* d_out = reinterpret_cast<double*>(d_fit + b_fit);
+    char* d_ws = reinterpret_cast<char*>(d_out) + b_out;
+    int status = QMC_OK;
+    cudaError_t e;
+    std::vector<double> host_out((size_t)4 + 2 * m);
+    do {
+        if ((e = cudaMemcpyAsync(d_params, params, (size_t)n_params * 8, cudaMemcpyHostToDevice, st)) != cudaSuccess) break;
+        if ((e = cudaMemcpyAsync(d_z, z, (size_t)dim * 8, cudaMemcpyHostToDevice, st)) != cudaSuccess) break;
+        if ((e = cudaMemcpyAsync(d_sh, shifts, (size_t)m * dim * 8, cudaMemcpyHostToDevice, st)) != cudaSuccess) break;
+        if (fit_coeffs && (e = cudaMemcpyAsync(d_fit, fit_coeffs, (size_t)dim * 6 * 8, cudaMemcpyHostToDevice, st)) != cudaSuccess) break;
+        dp.params = reinterpret_cast<const double*>(d_params);
+        dp.z = reinterpret_cast<const uint64_t*>(d_z);
+        dp.shifts = reinterpret_cast<const double*>(d_sh);
+        dp.fit_coeffs = fit_coeffs ? reinterpret_cast<const double*>(d_fit) : nullptr;
+        status = run_batch(1, &dp, d_out, d_out + 2, d_out + 4, d_ws, plan.total, st);
+        if (status != QMC_OK) { e = cudaSuccess; break; }
+        if ((e = cudaMemcpyAsync(host_out.data(), d_out, (size_t)(4 + 2 * m) * 8, cudaMemcpyDeviceToHost, st)) != cudaSuccess) break;
+        e = cudaStreamSynchronize(st);
+    } while (0);
+    cudaFreeAsync(buf, st);
+    if (e != cudaSuccess) return cuda_fail(e, "qmc_lattice_integrate");
+    if (status != QMC_OK) return status;
+    bool finite = true;
+    for (int c = 0; c < nc; ++c) {
+        out_mean[c] = host_out[c];
+        out_err[c] = host_out[2 + c];
+        finite = finite && std::isfinite(out_mean[c]) && std::isfinite(out_err[c]);
+    }
+    if (out_shift_means)
+        for (int i = 0; i < m * nc; ++i) out_shift_means[i] = host_out[4 + i];
+    return finite ? QMC_OK : QMC_ERR_NONFINITE;
+}
+
+int qmc_lattice_integrate(int family, const double* params, int dim, uint64_t n, const uint64_t* z, const double* shifts,
+                          int m, int transform, const double* fit_coeffs, double* out_mean, double* out_err) {
+    if (!params) return QMC_ERR_NULL;
+    if (ncomp_of(family) < 0) return QMC_ERR_FAMILY;
+    if (dim < 1 || dim > QMC_MAX_DIM) return QMC_ERR_DIM;
+    const int n_params = family_param_count(family, params, dim);
+    if (n_params < 0) return QMC_ERR_PARAMS;
+    return qmc_lattice_integrate_ex(family, params, n_params, dim, n, z, shifts, m, transform, fit_coeffs, out_mean, out_err,
+                                    nullptr);
+}
+
+int qmc_finalize_means(const double* shift_means, int m, int ncomp, double* out_mean, double* out_err, void* cuda_stream) {
+    if (!shift_means || !out_mean || !out_err) return QMC_ERR_NULL;
+    if (m < 2 || m > QMC_MAX_M) return QMC_ERR_M;
+    if (ncomp < 1 || ncomp > 2) return QMC_ERR_FAMILY;
+    QMC_CUDA(launch_finalize_means(static_cast<cudaStream_t>(cuda_stream), shift_means, m, ncomp, out_mean, out_err));
+    return QMC_OK;
+}
+
+int qmc_lattice_points(uint64_t n, int dim, const uint64_t* z, const double* shift, uint64_t k0, uint64_t count,
+                       uint64_t* out_r, double* out_u, void* cuda_stream) {
+    if (!z || !shift) return QMC_ERR_NULL;
+    if (dim < 1 || dim > QMC_MAX_DIM) return QMC_ERR_DIM;
+    if (n < 2 || n >= (1ull << 53)) return QMC_ERR_N;
+    PointsArgs a;
+    std::memset(&a, 0, sizeof(a));
+    for (int j = 0; j < dim; ++j) {
+        if (z[j] < 1 || z[j] >= n || gcd_u64(z[j], n) != 1) return QMC_ERR_Z;
+        if (!(shift[j] >= 0.0 && shift[j] < 1.0)) return QMC_ERR_SHIFT;
+        a.z[j] = z[j];
+        a.shift[j] = shift[j];
+    }
+    a.n = n; a.k0 = k0; a.count = count; a.inv_n = 1.0 / (double)n; a.dim = dim;
+    a.out_r = reinterpret_cast<unsigned long long*>(out_r);
+    a.out_u = out_u;
+    const int sms = sm_count();
+    if (sms <= 0) return cuda_fail(cudaErrorNoDevice, "no CUDA device");
+    QMC_CUDA(launch_points(static_cast<cudaStream_t>(cuda_stream), a, sms));
+    return QMC_OK;
+}
+
+int qmc_fp64_peak_probe(int iters, double* out_rate, double* out_ms, void* cuda_stream) {
+    if (!out_rate) return QMC_ERR_NULL;
+    if (iters < 1) return QMC_ERR_N;
+    const int sms = sm_count();
+    if (sms <= 0) return cuda_fail(cudaErrorNoDevice, "no CUDA device");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const int blocks = sms * 8;
+    double* buf = nullptr;
+    QMC_CUDA(cudaMalloc(reinterpret_cast<void**>(&buf), (size_t)blocks * 256 * 8));
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    cudaError_t e = launch_dfma_probe(st, buf, blocks, 16);       // warm-up
+    float ms = 0.f;
+    if (e == cudaSuccess) {
+        cudaEventRecord(e0, st);
+        e = launch_dfma_probe(st, buf, blocks, iters);
+        cudaEventRecord(e1, st);
+        if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+        if (e == cudaSuccess) cudaEventElapsedTime(&ms, e0, e1);
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(buf);
+    if (e != cudaSuccess) return cuda_fail(e, "dfma probe");
+    const double instr = (double)blocks * 256.0 * (double)iters * 64.0;   // 8 chains x 8 unrolled, per thread per iteration
+    *out_rate = instr / ((double)ms * 1e-3);
+    if (out_ms) *out_ms = (double)ms;
+    return QMC_OK;
+}
+
+}  // extern "C"
+
+// ---- variance-reduction fit: host-side closed-form least squares (reading C-8) ----------
+extern "C" int qmc_fit_cubic(const double* hist, int dim, int bins, double* fit_coeffs) {
+    if (!hist || !fit_coeffs) return QMC_ERR_NULL;
+    if (dim < 1 || dim > QMC_MAX_DIM) return QMC_ERR_DIM;
+    if (bins < 2 || bins > 1024) return QMC_ERR_N;
+    for (int j = 0; j < dim; ++j) {
+        const double* h = hist + (size_t)j * bins;
+        long double total = 0.0L;
+        bool ok = true;
+        for (int b = 0; b < bins; ++b) { ok = ok && std::isfinite(h[b]) && h[b] >= 0.0; total += h[b]; }
+        double a4 = 1.0, a5 = 0.0;                              // identity map unless a safe fit exists
+        if (ok && total > 0.0L) {
+            // p(c) = c^3 + a4 (c - c^3) + a5 (c^2 - c^3) must reproduce the bin edges e_b at the CDF values c_b
+            long double s11 = 0, s12 = 0, s22 = 0, t1 = 0, t2 = 0, run = 0;
+            for (int b = 1; b < bins; ++b) {
+                run += h[b - 1];
+                const long double c = run / total, e = (long double)b / (long double)bins;
+                const long double c3 = c * c * c, g1 = c - c3, g2 = c * c - c3, rhs = e - c3;
+                s11 += g1 * g1; s12 += g1 * g2; s22 += g2 * g2; t1 += g1 * rhs; t2 += g2 * rhs;
+            }
+            const long double det = s11 * s22 - s12 * s12;
+            if (fabsl(det) > 1e-300L) {
+                const double c4 = (double)((t1 * s22 - t2 * s12) / det), c5 = (double)((s11 * t2 - s12 * t1) / det);
+                const double c6 = 1.0 - c4 - c5;
+                double mn = std::fmin(c4, c4 + 2.0 * c5 + 3.0 * c6);     // p' at the end points
+                if (c6 != 0.0) {
+                    const double yv = -c5 / (3.0 * c6);                   // interior extremum of p'
+                    if (yv > 0.0 && yv < 1.0) mn = std::fmin(mn, c4 + yv * (2.0 * c5 + 3.0 * c6 * yv));
+                }
+                if (mn > 0.05) { a4 = c4; a5 = c5; }
+            }
+        }
+        double* o = fit_coeffs + 6 * j;
+        o[0] = 1.001; o[1] = -0.001; o[2] = 0.0; o[3] = 0.0; o[4] = a4; o[5] = a5;   // bounds of P:L231 for the unused poles
+    }
+    return QMC_OK;
+}
+
+// TEMPORARY until qmc_project.cu lands (next commit)
+#ifndef QMC_HAVE_PROJECT
+extern "C" int qmc_lattice_project(const qmc_problem*, int, double*, void*, size_t, void*) { return QMC_ERR_CUDA; }
+extern "C" size_t qmc_project_workspace_bytes(const qmc_problem*, int) { return 0; }
+#endif

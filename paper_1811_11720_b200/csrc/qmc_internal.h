@@ -1,0 +1,75 @@
+// qmc_internal.h -- types shared by the host side (qmc_host.cu) and the kernels of the CUDA path.
+// Nothing here is shared with oracle/ (the CPU oracle is an independent translation unit).
+#pragma once
+#include <cstddef>
+#include <cstdint>
+
+#include "../../include/qmc_lattice.h"
+
+namespace qmc {
+
+constexpr int kThreads = 128;          // threads per CTA of the fused kernels (4 warps)
+constexpr int kWarps = kThreads / 32;
+constexpr int kGroup = 4;             // shifts evaluated together per lattice index (register-resident)
+constexpr int kMaxSteps = 1024;        // max lattice indices per thread per tile (bounds the naive fp64 chain length)
+constexpr int kTilesTarget = 2368;     // tiles aimed at per launch: 148 SMs x 4 resident CTAs x 4 waves
+constexpr int kMaxSectorOps = 1024;    // interpreter program length limit per polynomial
+constexpr int kMaxSectorMono = 64;
+
+// transform kinds after host-side decoding
+enum : int { TR_NONE = 0, TR_BAKER = 1, TR_KOR3 = 2, TR_KORR = 3 };
+
+// Device-resident description of one problem (built on the host, copied into the workspace).
+struct alignas(16) DevProblem {
+    const double* params;      // DEVICE, user layout
+    const unsigned long long* z;
+    const double* shifts;      // [m][dim]
+    const double* fit;         // [dim][6] or nullptr
+    unsigned long long n;
+    double inv_n;              // fl(1/double(n))  (reading C-2)
+    double wconst;             // Korobov: c_r^dim ; else 1
+    double kor[8];             // centred Korobov polynomial g_r coefficients (degree r in s=c^2), kor[i], i<=r
+    long long partial_off;     // offset in doubles into the partial-sum area
+    long long means_off;       // offset in doubles into the per-shift means area
+    long long tile_begin;      // first tile index (within this problem's kernel variant queue)
+    int tiles;                 // number of k-tiles
+    int steps;                 // I: lattice indices per thread per tile; tile length = steps*kThreads
+    int family, dim, m, ncomp;
+    int tr_kind;               // TR_*
+    int kor_r;                 // Korobov weight r (1..6) or 0
+    int has_fit;               // 0 none, 1 cubic
+    int n_params;
+    int aux_off;               // sector: offset (in 8-byte words) of the compiled program in the aux area
+    int aux_len;
+    int out_index;             // index of the problem in the caller's arrays
+    int pad_;
+};
+
+// Per-problem tables derived on the device by prepare_kernel (one record per problem).
+struct alignas(16) DevAux {
+    unsigned long long z[QMC_MAX_DIM];     // z_j
+    unsigned long long step[QMC_MAX_DIM];  // (kThreads * z_j) mod n : residue stride between a thread's points
+    unsigned long long back[QMC_MAX_DIM];  // (steps * kThreads * z_j) mod n : rewinds a thread to its first point
+    double fam_a[QMC_MAX_DIM];             // per-dimension integrand constants (family dependent)
+    double fam_b[QMC_MAX_DIM];
+    double fit[5][QMC_MAX_DIM];            // a4, a5, a6, 2*a5, 3*a6 of the cubic map
+    double fam0;                           // OSC: 2 pi u0
+    double sec_c0[2];                      // sector: constant terms of U and F
+    int sec_a, sec_b;                      // sector: powers of U and F
+    int sec_nops[2];                       // sector: interpreter ops of U and F
+    int sec_ncoef[2];                      // sector: non-constant monomials of U and F
+    int status;                            // 0 or a qmc_status found while preparing
+    int pad_;
+    unsigned char nu[QMC_MAX_DIM];         // sector: nu_j
+};
+
+// One kernel variant queue: the problems (indices into DevProblem[]) it serves, in queue order.
+struct VariantQueue {
+    const int* plist;            // DEVICE: problem indices in queue order
+    const long long* tile_prefix;// DEVICE: exclusive prefix of tiles over plist, plist_len+1 entries
+    int plist_len;
+    long long total_tiles;
+    unsigned long long* counter; // DEVICE: tile queue head (zeroed before launch)
+};
+
+}  // namespace qmc

@@ -1,0 +1,179 @@
+// qmc_misc.cu -- the small kernels around the fused kernel: per-problem preparation, the finalize
+// stage (S8), the inspection kernel (residues / coordinates) and the FP64 peak probe.
+#include <cmath>
+
+#include "qmc_sector.cuh"
+#include "qmc_kernels.h"
+
+namespace qmc {
+
+// ---------------------------------------------------------------------------------------------
+// prepare: derive the per-problem tables the fused kernel reads (one warp per problem)
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(32) prepare_kernel(const DevProblem* __restrict__ probs, DevAux* __restrict__ aux,
+                                                     unsigned long long* __restrict__ prog_area) {
+    const DevProblem pb = probs[blockIdx.x];
+    DevAux& a = aux[blockIdx.x];
+    const int j = threadIdx.x, d = pb.dim;
+    const unsigned long long n = pb.n;
+    if (j < QMC_MAX_DIM) {
+        unsigned long long z = 0, step = 0, back = 0;
+        double fa = 0.0, fb = 0.0, f[5] = {1.0, 0.0, 0.0, 0.0, 0.0};
+        if (j < d) {
+            z = pb.z[j] % n;
+            step = mulmod_u64((unsigned long long)kThreads % n, z, n);
+            back = mulmod_u64(((unsigned long long)pb.steps * kThreads) % n, z, n);
+            const double* p = pb.params;
+            if (pb.family == QMC_FAMILY_GENZ_OSC) { fa = p[1 + j]; }
+            else if (pb.family == QMC_FAMILY_GENZ_PRODPEAK) { const double c = p[j]; fa = __ddiv_rn(1.0, __dmul_rn(c, c)); fb = p[d + j]; }
+            else if (pb.family == QMC_FAMILY_CEXP_POLY) { fa = p[j]; fb = p[d + j]; }
+            if (pb.has_fit) {
+                const double* c = pb.fit + 6 * j;
+                const double a4 = c[4], a5 = c[5];
+                const double a6 = __dadd_rn(__dadd_rn(__dadd_rn(__dadd_rn(1.0, -c[2]), -c[3]), -a4), -a5);
+                f[0] = a4; f[1] = a5; f[2] = a6; f[3] = 2.0 * a5; f[4] = 3.0 * a6;
+            }
+        }
+        a.z[j] = z; a.step[j] = step; a.back[j] = back; a.fam_a[j] = fa; a.fam_b[j] = fb;
+#pragma unroll
+        for (int i = 0; i < 5; ++i) a.fit[i][j] = f[i];
+        a.nu[j] = 0;
+    }
+    if (j == 0) {
+        a.fam0 = (pb.family == QMC_FAMILY_GENZ_OSC) ? __dmul_rn(6.283185307179586476925286766559, pb.params[0]) : 0.0;
+        a.status = 0;
+        a.sec_a = a.sec_b = 0;
+        a.sec_nops[0] = a.sec_nops[1] = a.sec_ncoef[0] = a.sec_ncoef[1] = 0;
+        a.sec_c0[0] = a.sec_c0[1] = 0.0;
+    }
+    if (pb.family == QMC_FAMILY_SECTOR) {
+        __syncwarp();
+        prepare_sector(pb, a, prog_area);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// S8 finalize: Q_s = (sum over tiles in tile order)/n, Qbar, err (Eq. 2-3); one CTA
+// per problem.  Compensated sums; per component for complex results.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void eq3_component(const double* __restrict__ means, int m, int nc, int c, double* mean_out,
+                                              double* err_out) {
+    CompSum t;
+    for (int s = 0; s < m; ++s) t.add(means[s * nc + c]);
+    const double mean = __ddiv_rn(t.value(), (double)m);
+    CompSum v;
+    for (int s = 0; s < m; ++s) { const double dlt = __dadd_rn(means[s * nc + c], -mean); v.add(__dmul_rn(dlt, dlt)); }
+    *mean_out = mean;
+    *err_out = __dsqrt_rn(__ddiv_rn(v.value(), __dmul_rn((double)m, (double)(m - 1))));
+}
+
+__global__ void __launch_bounds__(256) finalize_kernel(const DevProblem* __restrict__ probs, const DevAux* __restrict__ aux,
+                                                       const double* __restrict__ partials, double* __restrict__ means_ws,
+                                                       double* __restrict__ out_means, double* __restrict__ out_errs,
+                                                       double* __restrict__ out_shift_means, int stride) {
+    const DevProblem& pb = probs[blockIdx.x];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nc = pb.ncomp, m = pb.m, tiles = pb.tiles, npairs = m * nc;
+    double* means = means_ws + pb.means_off;
+    const bool bad = aux[blockIdx.x].status != 0;
+    for (int pair = warp; pair < npairs; pair += 8) {
+        const double* src = partials + pb.partial_off + (long long)pair * tiles;
+        CompSum cs;
+        for (int t = lane; t < tiles; t += 32) cs.add(src[t]);
+        const double v = warp_sum(cs.value());
+        if (lane == 0) {
+            double q = __ddiv_rn(v, (double)pb.n);
+            if (bad) q = nan("");
+            means[pair] = q;
+            if (out_shift_means) out_shift_means[(size_t)pb.out_index * stride + pair] = q;
+        }
+    }
+    __syncthreads();
+    if (tid < 2) {
+        double mean = 0.0, err = 0.0;
+        if (tid < nc) eq3_component(means, m, nc, tid, &mean, &err);
+        out_means[(size_t)pb.out_index * 2 + tid] = mean;
+        out_errs[(size_t)pb.out_index * 2 + tid] = err;
+    }
+}
+
+__global__ void __launch_bounds__(32) finalize_means_kernel(const double* __restrict__ means, int m, int nc,
+                                                            double* __restrict__ out_mean, double* __restrict__ out_err) {
+    if (threadIdx.x < nc) eq3_component(means, m, nc, threadIdx.x, &out_mean[threadIdx.x], &out_err[threadIdx.x]);
+}
+
+// ---------------------------------------------------------------------------------------------
+// inspection: residues and coordinates through the same device functions as the fused kernel
+// (first residue by mulmod, then stepping by add_mod; conversion and wrap as in S1-S2)
+// ---------------------------------------------------------------------------------------------
+template <bool WIDE>
+__global__ void __launch_bounds__(kThreads) points_kernel(PointsArgs a) {
+    typedef typename Res<WIDE>::T RT;
+    const unsigned long long stride = (unsigned long long)gridDim.x * kThreads;
+    unsigned long long i = (unsigned long long)blockIdx.x * kThreads + threadIdx.x;
+    if (i >= a.count) return;
+    const unsigned long long n = a.n;
+    RT r[QMC_MAX_DIM], step[QMC_MAX_DIM];
+    const unsigned long long kfirst = (a.k0 % n + i % n) % n;
+    for (int j = 0; j < a.dim; ++j) {
+        const unsigned long long z = a.z[j] % n;
+        r[j] = (RT)mulmod_u64(kfirst, z, n);
+        step[j] = (RT)mulmod_u64(stride % n, z, n);
+    }
+    for (; i < a.count; i += stride) {
+        for (int j = 0; j < a.dim; ++j) {
+            if (a.out_r) a.out_r[i * a.dim + j] = (unsigned long long)r[j];
+            if (a.out_u) a.out_u[i * a.dim + j] = wrap_u(coord_t(Res<WIDE>::to_double(r[j]), a.inv_n, a.shift[j]));
+            r[j] = add_mod<RT>(r[j], step[j], (RT)n);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// FP64 peak probe: 8 independent DFMA chains per thread, 2048 threads per SM
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256, 8) dfma_probe_kernel(double* __restrict__ out, int iters, double a, double b) {
+    double x0 = threadIdx.x * 1e-3, x1 = x0 + 0.1, x2 = x0 + 0.2, x3 = x0 + 0.3, x4 = x0 + 0.4, x5 = x0 + 0.5, x6 = x0 + 0.6,
+           x7 = x0 + 0.7;
+#pragma unroll 1
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            x0 = __fma_rn(x0, a, b); x1 = __fma_rn(x1, a, b); x2 = __fma_rn(x2, a, b); x3 = __fma_rn(x3, a, b);
+            x4 = __fma_rn(x4, a, b); x5 = __fma_rn(x5, a, b); x6 = __fma_rn(x6, a, b); x7 = __fma_rn(x7, a, b);
+        }
+    }
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+}
+
+// ---------------------------------------------------------------------------------------------
+// host-callable launchers
+// ---------------------------------------------------------------------------------------------
+cudaError_t launch_prepare(int count, cudaStream_t st, const DevProblem* probs, DevAux* aux, unsigned long long* prog_area) {
+    prepare_kernel<<<count, 32, 0, st>>>(probs, aux, prog_area);
+    return cudaGetLastError();
+}
+cudaError_t launch_finalize(int count, cudaStream_t st, const DevProblem* probs, const DevAux* aux, const double* partials,
+                            double* means_ws, double* out_means, double* out_errs, double* out_shift_means, int stride) {
+    finalize_kernel<<<count, 256, 0, st>>>(probs, aux, partials, means_ws, out_means, out_errs, out_shift_means, stride);
+    return cudaGetLastError();
+}
+cudaError_t launch_finalize_means(cudaStream_t st, const double* means, int m, int nc, double* out_mean, double* out_err) {
+    finalize_means_kernel<<<1, 32, 0, st>>>(means, m, nc, out_mean, out_err);
+    return cudaGetLastError();
+}
+cudaError_t launch_points(cudaStream_t st, const PointsArgs& a, int sm_count) {
+    if (a.count == 0) return cudaSuccess;
+    unsigned long long blocks = (a.count + kThreads - 1) / kThreads;
+    const unsigned long long cap = (unsigned long long)sm_count * 8;
+    if (blocks > cap) blocks = cap;
+    if (a.n >= (1ull << 31)) points_kernel<true><<<(unsigned)blocks, kThreads, 0, st>>>(a);
+    else points_kernel<false><<<(unsigned)blocks, kThreads, 0, st>>>(a);
+    return cudaGetLastError();
+}
+cudaError_t launch_dfma_probe(cudaStream_t st, double* out, int blocks, int iters) {
+    dfma_probe_kernel<<<blocks, 256, 0, st>>>(out, iters, 0.999999, 1e-6);
+    return cudaGetLastError();
+}
+
+}  // namespace qmc
