@@ -1,0 +1,370 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the rank-1 shifted lattice hot path on B200 (BASELINE.json metric:
+fp64 lattice-point integrand evaluations per second, and the fraction of the FP64 issue-rate roofline).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--main-only]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+A "step" is one pass of the whole hot path (prepare, fused persistent kernel,
+finalize) over one batch of synthetic input through the C ABI (qmc_lattice_integrate_batch).  The headline
+workload is BASELINE.json configs[1]; configs[0], [2], [3], [4] are timed too and reported under "others".
+Inputs are seeded and synthetic (paper_1811_11720_b200.synth).
+
+Multi-GPU: the path has no exchange step: every rank integrates its own
+independent problems (same shapes, rank-specific seeds); weak scaling; the only communication is the
+MAX-reduction of the measured time.  `--impl reference` times the CPU oracle (oracle/) on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1811_11720_b200 import synth  # noqa: E402
+
+METRIC = "fp64 lattice-point integrand evaluations per second"
+UNIT = "evals/s"
+MAIN_CONFIG = 1
+
+# Algorithmic FP64-pipe instructions per integrand evaluation (thread level; FMA, MUL, ADD each count 1),
+# derived in DESIGN.md "Roofline" from the method itself: per dimension coordinate (1 FMA) + wrap/centre
+# (1 ADD) + transform + fit map + integrand term, plus per-evaluation weight, transcendental / divide and
+# accumulate.  These are the numerators of roofline.achieved; the executed counts are in profiles/.
+ALG_FP64_PER_EVAL = {
+    0: 4 * (2 + 6 + 1) + 3 + 38 + 1,          # d=4 osc, Korobov-3
+    1: 8 * (2 + 1 + 3) + 10 + 1,              # d=8 product peak, baker, one divide
+    2: 12 * (2 + 6 + 2) + 3 + 62 + 1 + 2,     # d=12 complex, Korobov-3, sincos
+    3: 6 * (2 + 6) + 3 + 70 + 6 + 10 + 1,     # d=6 sector (mean 70 monomial-degree steps), Korobov-3, divide
+    4: 16 * (2 + 6 + 5 + 1) + 4 + 38 + 1,     # d=16 osc, Korobov-3 + cubic map
+}
+FP64_LANES_PER_SM = 64                        # B200 (sm_100): 64 FP64 FMA lanes per SM -> nominal peak
+
+
+def workload_name(c):
+    d, n, m = synth.CONFIG_SHAPES[c]
+    return {0: f"configs[0] d=4 Genz oscillatory, n={n}, m={m}, Korobov r=3",
+            1: f"configs[1] d=8 Genz product peak, n={n}, m={m}, baker",
+            2: f"configs[2] d=12 complex exp*poly, n={n}, m={m}, Korobov r=3",
+            3: f"configs[3] 256 sector-like integrands d=6, n={n}, m={m}, Korobov r=3",
+            4: f"configs[4] d=16 Genz oscillatory + cubic ICDF fit map, n={n}, m={m}, Korobov r=3"}[c]
+
+
+def evals_of(problems):
+    return float(sum(p["n"] * p["m"] for p in problems))
+
+
+def rank_problems(c, rank):
+    """Problems of BASELINE.json configs[c] for `rank`: rank 0 gets exactly the seeded config; other ranks
+    get the same shapes with rank-specific shifts (independent problems -> no data-path collective)."""
+    probs = synth.config(c)
+    if rank == 0:
+        return probs
+    out = []
+    for i, p in enumerate(probs):
+        rng = synth.MT19937_64(synth.CONFIG_SEED + 7919 * rank + 104729 * c + i)
+        out.append(dict(p, shifts=synth.draw_shifts(rng, p["m"], p["dim"]), name=f"{p['name']}.rank{rank}"))
+    return out
+
+
+def aggregate(per_rank_evals, max_seconds):
+    """whole-job throughput: all ranks' evaluations over the slowest rank's time"""
+    return float(sum(per_rank_evals)) / max_seconds
+
+
+# ----------------------------------------------------------------------------------------------------
+# clocks sampling during the timed region (NVML; nvidia-smi fallback)
+# ----------------------------------------------------------------------------------------------------
+class ClockSampler:
+    REASONS = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown",
+               0x10: "sync_boost", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x100: "display_clock_setting"}
+
+    def __init__(self, index):
+        self.samples, self.stop_flag, self.thread, self.h, self.sm_max = [], False, None, None, None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.sm_max = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _loop(self):
+        nv = self.nv
+        while not self.stop_flag:
+            try:
+                self.samples.append((time.perf_counter(), nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM),
+                                     nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0,
+                                     nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                                     if hasattr(nv, "nvmlDeviceGetCurrentClocksEventReasons")
+                                     else nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)))
+            except Exception:
+                pass
+            time.sleep(0.01)
+
+    def start(self):
+        if self.nv is not None:
+            self.thread = threading.Thread(target=self._loop, daemon=True)
+            self.thread.start()
+
+    def stop(self):
+        self.stop_flag = True
+        if self.thread is not None:
+            self.thread.join()
+
+    def summary(self, windows):
+        """median SM clock over the samples that fall inside the timed windows [(t0, t1), ...]"""
+        inside = [s for s in self.samples if any(a <= s[0] <= b for a, b in windows)] or self.samples
+        if not inside:
+            return {"sm_mhz": None, "sm_max_mhz": self.sm_max, "reasons": [], "samples": 0}
+        mask = 0
+        for s in inside:
+            mask |= int(s[3])
+        reasons = [name for bit, name in self.REASONS.items() if mask & bit and name != "gpu_idle"]
+        return {"sm_mhz": float(statistics.median(s[1] for s in inside)), "sm_max_mhz": self.sm_max,
+                "power_w_max": max(s[2] for s in inside), "reasons": reasons, "samples": len(inside)}
+
+
+# ----------------------------------------------------------------------------------------------------
+# GPU arm
+# ----------------------------------------------------------------------------------------------------
+class L2Flusher:
+    """writes a buffer larger than the 126 MB L2 between timed iterations (outside the timed events)"""
+
+    def __init__(self, torch, device):
+        self.buf = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=device)
+
+    def __call__(self):
+        self.buf.fill_(1)
+
+
+def time_steps(torch, binding, batch, steps, warmup, flush):
+    """-> (per-step ms list (CUDA events on the launching stream), fused-kernel ms list, launches per step)"""
+    stream = torch.cuda.current_stream()
+    for _ in range(warmup):
+        flush()
+        batch.integrate()
+    torch.cuda.synchronize()
+    step_ms, fused_ms, launches = [], [], 0
+    for _ in range(steps):
+        flush()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        launches = batch.integrate()
+        e1.record(stream)
+        e1.synchronize()
+        step_ms.append(e0.elapsed_time(e1))
+        fused_ms.append(binding.qmc_profile_last_fused_ms())
+    return step_ms, fused_ms, launches
+
+
+def config4_with_device_fit(binding, probs):
+    """configs[4]: fit coefficients from the DEVICE projection pass + the library's host fit (no oracle)."""
+    p = probs[0]
+    proj = dict(p, n=synth.CONFIG4_NFIT, z=synth.genvec(synth.CONFIG4_NFIT, p["dim"]), transform=synth.TRANSFORM_NONE)
+    H = binding.DeviceBatch([proj]).project(0, synth.PROJECTION_BINS).cpu().numpy()
+    return [dict(p, fit_coeffs=binding.qmc_fit_cubic(H))]
+
+
+def e2e_host_api(binding, probs, reps):
+    """The same metric through the synchronous HOST-pointer C-ABI call (qmc_lattice_integrate_ex): device
+    allocation, host->device copies of the inputs, the kernels, the device->host copy of the results and the
+    synchronisation are all inside the timed region (host wall clock around a blocking call)."""
+    h2d = d2h = 0
+    for p in probs:
+        h2d += p["params"].nbytes + p["z"].nbytes + p["shifts"].nbytes + (0 if p.get("fit_coeffs") is None else p["fit_coeffs"].nbytes)
+        d2h += (4 + 2 * p["m"]) * 8
+    for p in probs[:2]:
+        binding.qmc_lattice_integrate_ex(p)                 # warm-up (module load, pools)
+    t0 = time.perf_counter()
+    for _ in range(reps):
+        for p in probs:
+            binding.qmc_lattice_integrate_ex(p)
+    dt = (time.perf_counter() - t0) / reps
+    return dt, h2d, d2h
+
+
+def run_ours(args):
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product has no CPU fallback (use --impl reference for the oracle)")
+    from paper_1811_11720_b200 import binding
+    binding.lib()                                           # fails loudly if libqmc_lattice.so is missing
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    device = f"cuda:{local}"
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(device))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    binding.qmc_profile_enable(True)
+    flush = L2Flusher(torch, device)
+    sampler = ClockSampler(local)
+    sampler.start()
+
+    # FP64 issue-rate peak, measured in this process right before the timed runs (thread-level DFMA / s)
+    binding.qmc_fp64_peak_probe(2000)
+    peak_rate, peak_ms = binding.qmc_fp64_peak_probe(60000)
+    sm_count = torch.cuda.get_device_properties(local).multi_processor_count
+
+    def measure(c, steps, warmup):
+        probs = rank_problems(c, rank)
+        if c == 4:
+            probs = config4_with_device_fit(binding, probs)
+        batch = binding.DeviceBatch(probs, device=device)
+        barrier()
+        w0 = time.perf_counter()
+        step_ms, fused_ms, launches = time_steps(torch, binding, batch, steps, warmup, flush)
+        barrier()
+        w1 = time.perf_counter()
+        total_s = max_over_ranks(sum(step_ms) * 1e-3)
+        ev = evals_of(probs)
+        fused_avg_s = statistics.fmean(fused_ms) * 1e-3
+        alg = ALG_FP64_PER_EVAL[c]
+        achieved = alg * ev / fused_avg_s
+        sms, means, errs = batch.results()
+        rec = {"workload": workload_name(c), "value": aggregate([ev * steps] * world, total_s), "unit": UNIT,
+               "ms_per_step": total_s / steps * 1e3, "ms_per_step_best": min(step_ms), "steps": steps, "warmup": warmup,
+               "evals_per_step_per_gpu": ev, "fused_kernel_ms": fused_avg_s * 1e3,
+               "fused_kernel_share_of_step": fused_avg_s * 1e3 * steps / sum(step_ms),
+               "gpu_launches_per_step": launches, "plan": batch.plan_info(),
+               "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": peak_rate / 1e12, "unit": "Tinst/s (thread-level FP64 instructions)",
+                            "frac": achieved / peak_rate, "traffic": None, "alg_fp64_inst_per_eval": alg,
+                            "peak_source": "qmc_fp64_peak_probe (DFMA chains) measured in this run",
+                            "peak_nominal": sm_count * FP64_LANES_PER_SM * 1.965e9 / 1e12},
+               "result_mean": [float(v) for v in means[0]], "result_err": [float(v) for v in errs[0]]}
+        return rec, probs, (w0, w1)
+
+    windows = []
+    main, main_probs, w = measure(MAIN_CONFIG, args.steps, args.warmup)
+    windows.append(w)
+    others = []
+    if not args.main_only:
+        for c, (k, wu) in {0: (50, 5), 2: (5, 3), 3: (3, 3), 4: (2, 3)}.items():
+            rec, _, w = measure(c, k, wu)
+            windows.append(w)
+            others.append(rec)
+
+    # end-to-end through the HOST-pointer entry (rank-local; max over ranks)
+    barrier()
+    e2e_reps = max(5, min(args.steps, 50))
+    e2e_s, h2d, d2h = e2e_host_api(binding, main_probs, e2e_reps)
+    e2e_s = max_over_ranks(e2e_s)
+    sampler.stop()
+    clocks = sampler.summary(windows)
+
+    out = {"metric": METRIC, "value": main["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic",
+           "config": {"workload": main["workload"], "evals_per_step_per_gpu": main["evals_per_step_per_gpu"],
+                      "l2": "256 MiB buffer written between timed iterations (inputs are KB-sized and stay resident)",
+                      "parallelism": f"replicas x{world} (independent problems per rank, no data-path collective)",
+                      "plan": main["plan"]},
+           "e2e": {"value": aggregate([main["evals_per_step_per_gpu"]] * world, e2e_s), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                   "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3,
+                   "api": "qmc_lattice_integrate_ex (HOST pointers; alloc + H2D + kernels + D2H + sync inside the timed call)"},
+           "gpu_launches": main["gpu_launches_per_step"] * args.steps,
+           "roofline": main["roofline"], "fused_kernel_ms": main["fused_kernel_ms"],
+           "fused_kernel_share_of_step": main["fused_kernel_share_of_step"],
+           "fp64_peak_probe": {"thread_inst_per_s": peak_rate, "ms": peak_ms, "sm_count": sm_count,
+                               "implied_clock_mhz_at_64_lanes": peak_rate / (sm_count * FP64_LANES_PER_SM) / 1e6},
+           "clocks": clocks, "others": others}
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        out["cpu_baseline"] = cpu_baseline(MAIN_CONFIG, reps=3)
+    if rank == 0:
+        print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+# ----------------------------------------------------------------------------------------------------
+# CPU oracle arm (reported baseline; never tuned)
+# ----------------------------------------------------------------------------------------------------
+def cpu_baseline(c, reps):
+    import oracle
+    probs = synth.config(c)
+    t0 = time.perf_counter()
+    for _ in range(reps):
+        for p in probs:
+            oracle.integrate(p)
+    dt = (time.perf_counter() - t0) / reps
+    return {"value": evals_of(probs) / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"the full {workload_name(c)} ({evals_of(probs):.3g} evaluations), {reps} repetitions, OpenMP over 2^16-index chunks",
+            "seconds_per_pass": dt}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    probs = synth.config(MAIN_CONFIG)
+    ev = evals_of(probs)
+    for _ in range(min(args.warmup, 1)):
+        oracle.integrate(probs[0])
+    times = []
+    for _ in range(args.steps):
+        t0 = time.perf_counter()
+        for p in probs:
+            oracle.integrate(p)
+        times.append(time.perf_counter() - t0)
+    total = sum(times)
+    value = ev * args.steps / total
+    sample = f"each step = the full {workload_name(MAIN_CONFIG)} ({ev:.3g} evaluations) on the host cores"
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+                      "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": total / args.steps * 1e3,
+                      "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                      "config": {"workload": workload_name(MAIN_CONFIG), "evals_per_step_per_gpu": ev},
+                      "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
+                      "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                      "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--main-only", action="store_true", help="time configs[1] only (skip the 'others' list)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        if args.steps > 40:
+            args.steps = 40                                 # bounded: a step is ~1 s of host time
+        run_reference(args)
+    else:
+        if args.warmup < 3:
+            args.warmup = 3
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

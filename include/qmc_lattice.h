@@ -161,6 +161,13 @@ int qmc_fp64_peak_probe(int iters, double* out_rate /*HOST*/, double* out_ms /*H
  * (for the benchmark's gpu_launches accounting). */
 int qmc_last_launch_count(void);
 
+/* Measurement helper: with profiling enabled (per host thread), qmc_lattice_integrate_batch brackets its
+ * fused-kernel launches (not prepare / finalize) with CUDA events on the caller's stream;
+ * qmc_profile_last_fused_ms synchronises on the closing event of the LAST batch call of this thread and
+ * returns the device time of the fused kernels in milliseconds (QMC_ERR_N if nothing was recorded). */
+int qmc_profile_enable(int on);
+int qmc_profile_last_fused_ms(double* out_ms /*HOST*/);
+
 /* Launch geometry the library uses for a batch (for DESIGN.md / bench reporting): tiles, CTAs,
  * k indices per tile of problem 0.  Any pointer may be NULL. */
 int qmc_plan_info(int count, const qmc_problem* problems /*HOST*/, long long* out_tiles, int* out_ctas,

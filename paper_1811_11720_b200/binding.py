@@ -18,6 +18,7 @@ EXPORTS = [
     "qmc_lattice_integrate", "qmc_lattice_integrate_ex", "qmc_lattice_integrate_batch", "qmc_workspace_bytes",
     "qmc_validate_problem_host", "qmc_lattice_project", "qmc_project_workspace_bytes", "qmc_fit_cubic",
     "qmc_lattice_points", "qmc_finalize_means", "qmc_fp64_peak_probe", "qmc_last_launch_count", "qmc_plan_info",
+    "qmc_profile_enable", "qmc_profile_last_fused_ms",
     "qmc_num_components", "qmc_status_string", "qmc_last_cuda_error",
 ]
 
@@ -69,6 +70,8 @@ def lib():
         L.qmc_fp64_peak_probe.argtypes = [C.c_int, dp, dp, vp]
         L.qmc_plan_info.argtypes = [C.c_int, pp, C.POINTER(C.c_longlong), C.POINTER(C.c_int), C.POINTER(C.c_longlong)]
         L.qmc_num_components.argtypes = [C.c_int]
+        L.qmc_profile_enable.argtypes = [C.c_int]
+        L.qmc_profile_last_fused_ms.argtypes = [dp]
         L.qmc_status_string.argtypes = [C.c_int]
         L.qmc_status_string.restype = C.c_char_p
         L.qmc_last_cuda_error.restype = C.c_char_p
@@ -252,3 +255,15 @@ def qmc_fp64_peak_probe(iters=20000):
     rate, ms = C.c_double(), C.c_double()
     _check(lib().qmc_fp64_peak_probe(int(iters), C.byref(rate), C.byref(ms), None), "qmc_fp64_peak_probe")
     return rate.value, ms.value
+
+
+def qmc_profile_enable(on=True):
+    """Bracket the fused-kernel launches of later batch calls (this host thread) with CUDA events."""
+    _check(lib().qmc_profile_enable(1 if on else 0), "qmc_profile_enable")
+
+
+def qmc_profile_last_fused_ms():
+    """Device time (ms) of the fused kernels of the last batch call; synchronises on its closing event."""
+    ms = C.c_double()
+    _check(lib().qmc_profile_last_fused_ms(C.byref(ms)), "qmc_profile_last_fused_ms")
+    return ms.value

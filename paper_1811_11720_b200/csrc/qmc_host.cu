@@ -17,11 +17,18 @@ namespace {
 
 thread_local std::string g_last_error;
 thread_local int g_last_launches = 0;
+thread_local bool g_profile = false;                 // qmc_profile_enable
+thread_local cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
+thread_local bool g_ev_valid = false;
 
 int cuda_fail(cudaError_t e, const char* where) {
     g_last_error = std::string(where) + ": " + cudaGetErrorString(e);
     return QMC_ERR_CUDA;
 }
+}  // namespace
+// shared with the other translation units (qmc_kernels.h): records the text for qmc_last_cuda_error()
+int report_cuda_error(cudaError_t e, const char* where) { return cuda_fail(e, where); }
+namespace {
 #define QMC_CUDA(call)                                              \
     do {                                                            \
         cudaError_t e_ = (call);                                    \
@@ -84,6 +91,12 @@ int tiles_target() {
         return t > 0 ? t : kTilesTarget;
     }();
     return v;
+}
+
+// test knob: run small lattices through the 64-bit-residue kernels (they are otherwise reached only for n >= 2^31)
+bool force_wide() {
+    const char* e = std::getenv("QMC_FORCE_WIDE");
+    return e && e[0] == '1';
 }
 
 // ---- launch plan: tiles, kernel variants, workspace layout (pure function of the problem structs) ----
@@ -158,7 +171,7 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
     for (int i = 0; i < count; ++i) {
         const DevProblem& d = plan->dev[i];
         const int dp = dim_slots(d.family, d.dim);
-        const bool wide = d.n >= (1ull << 31);
+        const bool wide = d.n >= (1ull << 31) || force_wide();
         Variant* v = nullptr;
         for (auto& c : plan->variants)
             if (c.family == d.family && c.dp == dp && c.wide == wide) v = &c;
@@ -262,6 +275,11 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
     double* dpart = reinterpret_cast<double*>(ws + plan.off_partials);
     QMC_CUDA(launch_prepare(count, st, dprobs, daux, dprog));
     ++g_last_launches;
+    g_ev_valid = false;
+    if (g_profile) {
+        if (!g_ev0) { QMC_CUDA(cudaEventCreate(&g_ev0)); QMC_CUDA(cudaEventCreate(&g_ev1)); }
+        QMC_CUDA(cudaEventRecord(g_ev0, st));
+    }
     for (size_t vi = 0; vi < plan.variants.size(); ++vi) {
         const Variant& v = plan.variants[vi];
         const int occ = occupancy(v.family, v.dp, v.wide);
@@ -279,6 +297,7 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
         if (e != cudaSuccess) return cuda_fail(e, "fused kernel launch");
         ++g_last_launches;
     }
+    if (g_profile) { QMC_CUDA(cudaEventRecord(g_ev1, st)); g_ev_valid = true; }
     QMC_CUDA(launch_finalize(count, st, dprobs, daux, dpart, dmeans, out_means, out_errs, out_shift_means, 2 * plan.max_m));
     ++g_last_launches;
     return QMC_OK;
@@ -372,6 +391,18 @@ const char* qmc_status_string(int status) {
 
 const char* qmc_last_cuda_error(void) { return g_last_error.c_str(); }
 int qmc_last_launch_count(void) { return g_last_launches; }
+
+int qmc_profile_enable(int on) { g_profile = on != 0; return QMC_OK; }
+
+int qmc_profile_last_fused_ms(double* out_ms) {
+    if (!out_ms) return QMC_ERR_NULL;
+    if (!g_ev_valid) return QMC_ERR_N;
+    QMC_CUDA(cudaEventSynchronize(g_ev1));
+    float ms = 0.f;
+    QMC_CUDA(cudaEventElapsedTime(&ms, g_ev0, g_ev1));
+    *out_ms = (double)ms;
+    return QMC_OK;
+}
 
 size_t qmc_workspace_bytes(int count, const qmc_problem* problems) {
     Plan plan;
@@ -578,9 +609,3 @@ extern "C" int qmc_fit_cubic(const double* hist, int dim, int bins, double* fit_
     }
     return QMC_OK;
 }
-
-// TEMPORARY until qmc_project.cu lands (next commit)
-#ifndef QMC_HAVE_PROJECT
-extern "C" int qmc_lattice_project(const qmc_problem*, int, double*, void*, size_t, void*) { return QMC_ERR_CUDA; }
-extern "C" size_t qmc_project_workspace_bytes(const qmc_problem*, int) { return 0; }
-#endif

@@ -18,6 +18,9 @@ struct PointsArgs {
     double* out_u;
 };
 
+// records a CUDA error for qmc_last_cuda_error() and returns QMC_ERR_CUDA (qmc_host.cu)
+int report_cuda_error(cudaError_t e, const char* where);
+
 cudaError_t launch_prepare(int count, cudaStream_t st, const DevProblem* probs, DevAux* aux, unsigned long long* prog_area);
 cudaError_t launch_finalize(int count, cudaStream_t st, const DevProblem* probs, const DevAux* aux, const double* partials,
                             double* means_ws, double* out_means, double* out_errs, double* out_shift_means, int stride);

@@ -1,0 +1,224 @@
+// qmc_project.cu -- S10, the projection pass that feeds the variance-reduction fit
+// (Eq. 20; the paper's `evaluate`, keeps all n samples on the host and
+// sorts them per dimension, P:L958-L960 -- here replaced by a device histogram, C-8):
+//
+//     H[j][b] = sum_k |f(x_k)| [ floor(B x_{k,j}) == b ],   x_k = { k z / n + Delta_0 },
+//
+// transform None, weight 1, first shift only, all n lattice points.
+//
+// Determinism: a tile is a fixed range of lattice indices; inside a tile every warp owns a private
+// shared-memory histogram and adds its points in a fixed order (index step by step; within a step
+// the lanes that hit the same bin are summed in lane order by the lowest lane, found with
+// __match_any_sync -- no floating-point atomics anywhere).  Warp histograms are merged in warp
+// order, tile histograms in tile order (compensated) by project_merge_kernel.  The result does not
+// depend on the grid size, the SM count or the scheduling order.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+
+#include "qmc_device.cuh"
+#include "qmc_kernels.h"
+
+namespace qmc {
+namespace {
+
+constexpr int kProjTilesTarget = 592;       // 148 SMs x 4: fixed, so the tiling is a function of n only
+constexpr int kProjSmemBudget = 200 * 1024; // bytes of warp-private histograms per CTA
+
+struct ProjArgs {
+    const double* params;
+    const unsigned long long* z;
+    const double* shift;        // first shift, dim entries
+    unsigned long long n;
+    double inv_n;
+    int family, dim, n_params, bins;
+    int steps;                  // lattice indices per thread per tile
+    int tiles;
+    int dchunk;                 // dimensions histogrammed per CTA
+    int nchunks;
+    double* tile_hist;          // [tile][dim][bins]
+    double* out_hist;           // [dim][bins]
+};
+
+// |f(x)| for the four families, straight from the caller's parameter block (layouts: qmc_lattice.h).
+__device__ double abs_integrand(const ProjArgs& a, const double* x) {
+    const double* p = a.params;
+    const int d = a.dim;
+    if (a.family == QMC_FAMILY_GENZ_OSC) {
+        double ph = __dmul_rn(6.283185307179586476925286766559, p[0]);
+        for (int j = 0; j < d; ++j) ph = __fma_rn(p[1 + j], x[j], ph);
+        return fabs(cos(ph));
+    }
+    if (a.family == QMC_FAMILY_GENZ_PRODPEAK) {
+        double den = 1.0;
+        for (int j = 0; j < d; ++j) {
+            const double c = p[j], t = x[j] - p[d + j];
+            den *= __fma_rn(t, t, 1.0 / (c * c));
+        }
+        return fabs(1.0 / den);
+    }
+    if (a.family == QMC_FAMILY_CEXP_POLY) {                                  // |exp(i phase)| = 1
+        double pr = 1.0;
+        for (int j = 0; j < d; ++j) pr *= __fma_rn(p[d + j], x[j], 1.0);
+        return fabs(pr);
+    }
+    const int pa = (int)p[0], pb = (int)p[1], nU = (int)p[2], nF = (int)p[3];
+    double pre = 1.0;
+    for (int j = 0; j < d; ++j) pre *= ipow_small(x[j], (int)p[4 + j]);
+    const double* base = p + 4 + d;
+    double poly[2];
+    const int cnt[2] = {nU, nF};
+    for (int w = 0; w < 2; ++w) {
+        const double* c = base;
+        const double* e = base + cnt[w];
+        double s = 0.0;
+        for (int t = 0; t < cnt[w]; ++t) {
+            double mon = c[t];
+            for (int j = 0; j < d; ++j) mon *= ipow_small(x[j], (int)e[t * d + j]);
+            s += mon;
+        }
+        poly[w] = s;
+        base += cnt[w] * (1 + d);
+    }
+    return fabs(pre * ipow_small(poly[0], pa) / ipow_small(poly[1], pb));
+}
+
+template <bool WIDE>
+__global__ void __launch_bounds__(kThreads) project_kernel(ProjArgs a) {
+    typedef typename Res<WIDE>::T RT;
+    extern __shared__ double hist[];                    // [warp][dchunk][bins]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tile = blockIdx.x / a.nchunks, chunk = blockIdx.x - tile * a.nchunks;
+    const int j0 = chunk * a.dchunk, j1 = min(a.dim, j0 + a.dchunk);
+    const int hsize = a.dchunk * a.bins;
+    for (int i = tid; i < kWarps * hsize; i += kThreads) hist[i] = 0.0;
+    __syncthreads();
+    double* mine = hist + warp * hsize;
+
+    const unsigned long long n = a.n;
+    const unsigned long long tile_len = (unsigned long long)a.steps * kThreads;
+    const unsigned long long k0 = (unsigned long long)tile * tile_len;
+    const unsigned long long kend = (k0 + tile_len < n) ? k0 + tile_len : n;
+    RT r[QMC_MAX_DIM], step[QMC_MAX_DIM];
+    double x[QMC_MAX_DIM];
+    for (int j = 0; j < a.dim; ++j) {
+        const unsigned long long z = a.z[j] % n;
+        r[j] = (RT)mulmod_u64((k0 + tid) % n, z, n);
+        step[j] = (RT)mulmod_u64((unsigned long long)kThreads % n, z, n);
+    }
+    unsigned long long k = k0 + tid;
+    for (int i = 0; i < a.steps; ++i, k += kThreads) {
+        const bool live = k < kend;
+        double v = 0.0;
+        if (live) {
+            for (int j = 0; j < a.dim; ++j) x[j] = wrap_u(coord_t(Res<WIDE>::to_double(r[j]), a.inv_n, a.shift[j]));
+            v = abs_integrand(a, x);
+        }
+        for (int j = j0; j < j1; ++j) {
+            int b = -1 - lane;                                        // dead lanes: unique keys, never added
+            if (live) {
+                b = (int)floor((double)a.bins * x[j]);
+                if (b >= a.bins) b = a.bins - 1;
+            }
+            unsigned peers = __match_any_sync(0xffffffffu, b);
+            const bool leader = (__ffs(peers) - 1) == lane;
+            double sum = v;
+            unsigned rem = peers & (peers - 1);                       // peers above the leader, lane order
+            while (__any_sync(0xffffffffu, leader && rem != 0u)) {
+                const int src = (leader && rem) ? (__ffs(rem) - 1) : lane;
+                const double pv = __shfl_sync(0xffffffffu, v, src);
+                if (leader && rem) { sum += pv; rem &= rem - 1; }
+            }
+            if (live && leader) mine[(j - j0) * a.bins + b] += sum;    // bins of one step are distinct per leader
+            __syncwarp();
+        }
+        for (int j = 0; j < a.dim; ++j) r[j] = add_mod<RT>(r[j], step[j], (RT)n);
+    }
+    __syncthreads();
+    // merge the warp histograms in warp order and publish the tile's histogram
+    for (int i = tid; i < (j1 - j0) * a.bins; i += kThreads) {
+        double s = hist[i];
+#pragma unroll
+        for (int w = 1; w < kWarps; ++w) s += hist[w * hsize + i];
+        a.tile_hist[((size_t)tile * a.dim + j0) * a.bins + i] = s;
+    }
+}
+
+__global__ void __launch_bounds__(256) project_merge_kernel(ProjArgs a) {
+    const int cells = a.dim * a.bins;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < cells; i += gridDim.x * blockDim.x) {
+        CompSum cs;
+        for (int t = 0; t < a.tiles; ++t) cs.add(a.tile_hist[(size_t)t * cells + i]);
+        a.out_hist[i] = cs.value();
+    }
+}
+
+int plan_project(const qmc_problem* p, int bins, ProjArgs* a) {
+    if (!p) return QMC_ERR_NULL;
+    if (p->family < 0 || p->family > QMC_FAMILY_SECTOR) return QMC_ERR_FAMILY;
+    if (p->dim < 1 || p->dim > QMC_MAX_DIM) return QMC_ERR_DIM;
+    if (p->n < 2 || p->n >= (1ull << 53)) return QMC_ERR_N;
+    if (bins < 2 || bins > 1024) return QMC_ERR_N;
+    if (p->m < 1) return QMC_ERR_M;
+    if (!p->params || !p->z || !p->shifts) return QMC_ERR_NULL;
+    if (p->family == QMC_FAMILY_GENZ_OSC && p->n_params != 1 + p->dim) return QMC_ERR_PARAMS;
+    if ((p->family == QMC_FAMILY_GENZ_PRODPEAK || p->family == QMC_FAMILY_CEXP_POLY) && p->n_params != 2 * p->dim) return QMC_ERR_PARAMS;
+    if (p->family == QMC_FAMILY_SECTOR && p->n_params < 4 + p->dim + 2 * (1 + p->dim)) return QMC_ERR_PARAMS;
+    std::memset(a, 0, sizeof(*a));
+    a->params = p->params;
+    a->z = reinterpret_cast<const unsigned long long*>(p->z);
+    a->shift = p->shifts;
+    a->n = p->n;
+    a->inv_n = 1.0 / (double)p->n;                                    // reading C-2
+    a->family = p->family; a->dim = p->dim; a->n_params = p->n_params; a->bins = bins;
+    const unsigned long long per = (unsigned long long)kThreads * kProjTilesTarget;
+    const unsigned long long steps = std::max<unsigned long long>(1, (p->n + per - 1) / per);
+    if (steps > 0x7fffffffull) return QMC_ERR_N;
+    a->steps = (int)steps;
+    a->tiles = (int)((p->n + steps * kThreads - 1) / (steps * kThreads));
+    a->dchunk = std::max(1, std::min(p->dim, kProjSmemBudget / (kWarps * bins * 8)));
+    a->nchunks = (p->dim + a->dchunk - 1) / a->dchunk;
+    return QMC_OK;
+}
+
+}  // namespace
+}  // namespace qmc
+
+using namespace qmc;
+
+extern "C" size_t qmc_project_workspace_bytes(const qmc_problem* p, int bins) {
+    ProjArgs a;
+    if (plan_project(p, bins, &a) != QMC_OK) return 0;
+    return ((size_t)a.tiles * a.dim * bins * 8 + 255) / 256 * 256;
+}
+
+extern "C" int qmc_lattice_project(const qmc_problem* p, int bins, double* out_hist, void* workspace, size_t workspace_bytes,
+                                   void* cuda_stream) {
+    ProjArgs a;
+    const int st = plan_project(p, bins, &a);
+    if (st != QMC_OK) return st;
+    if (!out_hist) return QMC_ERR_NULL;
+    const size_t need = ((size_t)a.tiles * a.dim * bins * 8 + 255) / 256 * 256;
+    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || workspace_bytes < need) return QMC_ERR_WORKSPACE;
+    a.tile_hist = static_cast<double*>(workspace);
+    a.out_hist = out_hist;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    const size_t smem = (size_t)kWarps * a.dchunk * bins * 8;
+    const bool wide = p->n >= (1ull << 31);
+    cudaError_t e;
+    if (wide) {
+        e = cudaFuncSetAttribute(project_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) project_kernel<true><<<a.tiles * a.nchunks, kThreads, smem, stream>>>(a);
+    } else {
+        e = cudaFuncSetAttribute(project_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) project_kernel<false><<<a.tiles * a.nchunks, kThreads, smem, stream>>>(a);
+    }
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e == cudaSuccess) {
+        const int cells = a.dim * bins;
+        project_merge_kernel<<<(cells + 255) / 256, 256, 0, stream>>>(a);
+        e = cudaGetLastError();
+    }
+    if (e != cudaSuccess) return report_cuda_error(e, "qmc_lattice_project");
+    return QMC_OK;
+}

@@ -1,0 +1,172 @@
+"""CPU-side checks of the C-ABI boundary (no compute launches): the library loads, exports every symbol
+include/qmc_lattice.h declares, validates arguments as the header states, and its host-only pieces
+(launch plan, cubic fit) behave.  Runs with -m "not gpu"."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1811_11720_b200 import binding, synth
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+K3 = synth.TRANSFORM_KOROBOV + 3
+
+
+@pytest.fixture(scope="module")
+def L():
+    from paper_1811_11720_b200 import build
+    build.build()
+    return binding.lib()
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "qmc_lattice.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(qmc_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_every_declared_symbol_is_exported(L):
+    names = _declared_symbols()
+    assert len(names) >= 16
+    for name in names:
+        assert hasattr(L, name), f"{name} declared in include/qmc_lattice.h but not exported"
+    assert sorted(binding.EXPORTS) == names
+
+
+def test_status_strings_and_components(L):
+    assert L.qmc_status_string(0) == b"ok"
+    for st in range(-13, 0):
+        assert L.qmc_status_string(st) not in (b"ok", b"unknown status")
+    assert [L.qmc_num_components(f) for f in range(4)] == [1, 1, 2, 1]
+    assert L.qmc_num_components(9) < 0
+
+
+def _cfg0():
+    return synth.config(0)[0]
+
+
+def test_validate_problem_host_accepts_all_configs():
+    for c in range(5):
+        n_over = None if c < 4 else 1048573           # config 4's CBC vector is large; same code path
+        for p in synth.config(c, n_override=n_over, count_override=4 if c == 3 else None):
+            assert binding.qmc_validate_problem_host(p) == 0, p["name"]
+
+
+@pytest.mark.parametrize("mutate,status", [
+    (lambda p: p.update(dim=0), -2),
+    (lambda p: p.update(n=1), -3),
+    (lambda p: p.update(n=1 << 53), -3),
+    (lambda p: p["z"].__setitem__(1, 0), -4),
+    (lambda p: p["z"].__setitem__(1, 65537), -4),
+    (lambda p: p["shifts"].__setitem__((0, 0), 1.0), -5),
+    (lambda p: p["shifts"].__setitem__((1, 2), -1e-9), -5),
+    (lambda p: p["shifts"].__setitem__((1, 2), float("nan")), -5),
+    (lambda p: p.update(m=1), -6),
+    (lambda p: p.update(transform=107), -7),
+    (lambda p: p.update(transform=2), -7),
+    (lambda p: p.update(family=7), -8),
+    (lambda p: p.update(params=p["params"][:-1]), -9),
+    (lambda p: p.update(fit_coeffs=synth.cubic_fit_coeffs(4, a4=-0.2, a5=0.3)), -10),
+    (lambda p: p.update(fit_coeffs=synth.cubic_fit_coeffs(4, a4=2.0, a5=-5.0)), -10),
+])
+def test_validate_problem_host_rejects(mutate, status):
+    p = _cfg0()
+    p = dict(p, z=p["z"].copy(), shifts=p["shifts"].copy(), params=p["params"].copy())
+    mutate(p)
+    assert binding.qmc_validate_problem_host(p) == status
+
+
+def test_z_must_be_coprime_to_n():
+    """'integers coprime to n'; n itself need not be prime (Fig. 1 uses 55, L108)."""
+    p = _cfg0()
+    p = dict(p, n=55, z=np.array([1, 34, 13, 21], dtype=np.uint64))
+    assert binding.qmc_validate_problem_host(p) == 0
+    p["z"][2] = 15                                        # gcd(15, 55) = 5
+    assert binding.qmc_validate_problem_host(p) == -4
+
+
+def test_synchronous_entry_rejects_before_touching_the_device(L):
+    """Argument errors are reported without any launch, so this works without a GPU."""
+    p = _cfg0()
+    with pytest.raises(binding.QmcError) as e:
+        binding.qmc_lattice_integrate(p["family"], p["params"], p["dim"], p["n"], p["z"], p["shifts"], 1, p["transform"])
+    assert e.value.status == -6
+    with pytest.raises(binding.QmcError) as e:
+        binding.qmc_lattice_integrate(9, p["params"], p["dim"], p["n"], p["z"], p["shifts"], p["m"], p["transform"])
+    assert e.value.status == -8
+
+
+def _host_struct(p):
+    keep = [np.ascontiguousarray(p["params"]), np.ascontiguousarray(p["z"]), np.ascontiguousarray(p["shifts"])]
+    s = binding.qmc_problem(p["family"], p["dim"], p["m"], p["transform"], p["n"], keep[0].ctypes.data, len(keep[0]),
+                            keep[1].ctypes.data, keep[2].ctypes.data, None)
+    return s, keep
+
+
+def test_plan_is_a_pure_function_of_the_problem(L):
+    """Tiles and workspace size depend on the problem structs only (not on the device): the fixed
+    result slots are what makes the reduction deterministic."""
+    for c in (0, 1, 2):
+        p = synth.config(c)[0]
+        s, keep = _host_struct(p)
+        arr = (binding.qmc_problem * 1)(s)
+        tiles, tl0 = C.c_longlong(), C.c_longlong()
+        assert L.qmc_plan_info(1, arr, C.byref(tiles), None, C.byref(tl0)) == 0
+        assert tiles.value * tl0.value >= p["n"] > (tiles.value - 1) * tl0.value
+        assert tl0.value % 128 == 0
+        ws = L.qmc_workspace_bytes(1, arr)
+        assert ws >= tiles.value * p["m"] * oracle.ncomp(p["family"]) * 8
+        assert ws == L.qmc_workspace_bytes(1, arr)
+    bad = (binding.qmc_problem * 1)(binding.qmc_problem(0, 0, 2, 0, 7, None, 0, None, None, None))
+    assert L.qmc_workspace_bytes(1, bad) == 0
+    assert L.qmc_plan_info(1, bad, None, None, None) == -2
+
+
+def test_fit_cubic_matches_oracle_and_recovers_a_cubic():
+    """qmc_fit_cubic is host code of the product; the oracle's fit is independent code (reading C-8)."""
+    rng = np.random.default_rng(7)
+    bins, d = 256, 5
+    H = np.empty((d, bins))
+    edges = np.arange(bins + 1) / bins
+    truth = []
+    for j in range(d):
+        a4, a5 = 0.5 + 0.4 * rng.random(), 0.6 * rng.random() - 0.1
+        a6 = 1 - a4 - a5
+        pinv = lambda y: y * (a4 + y * (a5 + y * a6))          # p = CDF^-1, so CDF(e) = p^-1(e)
+        ys = np.linspace(0, 1, 200001)
+        cdf = np.interp(edges, pinv(ys), ys)
+        H[j] = np.diff(cdf)
+        truth.append((a4, a5))
+    got = binding.qmc_fit_cubic(H)
+    ref = oracle.fit_cubic(H)
+    np.testing.assert_allclose(got, ref, rtol=0, atol=1e-10)
+    for j, (a4, a5) in enumerate(truth):
+        assert abs(got[j, 4] - a4) < 1e-6 and abs(got[j, 5] - a5) < 1e-6
+        assert got[j, 2] == 0.0 and got[j, 3] == 0.0
+    flat = binding.qmc_fit_cubic(np.ones((2, 64)))
+    np.testing.assert_allclose(flat[:, 4:], [[1.0, 0.0], [1.0, 0.0]], atol=1e-12)
+    spike = np.zeros((1, 64)); spike[0, 3] = 1.0              # not fittable by a monotone cubic -> identity
+    assert binding.qmc_fit_cubic(spike)[0, 4:].tolist() == [1.0, 0.0]
+
+
+def test_product_never_imports_the_oracle():
+    """The product path must not route through oracle/ (or any CPU fallback)."""
+    pkg = os.path.join(ROOT, "paper_1811_11720_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h", ".inc")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", text, flags=re.M), f
+                assert "qmc_oracle" not in text and "libqmc_oracle" not in text, f
+    otext = open(os.path.join(ROOT, "oracle", "qmc_oracle.cpp")).read()
+    assert "#include \"" not in otext                         # the oracle includes no project header
+
+
+def test_missing_library_fails_loudly(monkeypatch):
+    monkeypatch.setattr(binding, "_lib", None)
+    monkeypatch.setattr(binding, "LIB_PATH", "/nonexistent/libqmc_lattice.so")
+    with pytest.raises(ImportError):
+        binding.lib()
