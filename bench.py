@@ -268,6 +268,8 @@ def run_ours(args):
     others = []
     if not args.main_only:
         for c, (k, wu) in {0: (50, 5), 2: (5, 3), 3: (3, 3), 4: (2, 3)}.items():
+            if args.others is not None and c not in args.others:
+                continue
             rec, _, w = measure(c, k, wu)
             windows.append(w)
             others.append(rec)
@@ -355,6 +357,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--main-only", action="store_true", help="time configs[1] only (skip the 'others' list)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--others", type=lambda v: [int(x) for x in v.split(",") if x != ""], default=None,
+                    help="comma-separated subset of configs 0,2,3,4 to time besides configs[1] (default: all)")
     args = ap.parse_args()
     if args.impl == "reference":
         if args.steps > 40:
