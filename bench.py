@@ -63,10 +63,25 @@ def evals_of(problems):
     return float(sum(p["n"] * p["m"] for p in problems))
 
 
+SHRINK = 1        # --shrink S (profiling runs only): 1/S of the work of every config, same kernels and tile shapes
+
+
+def shrunk_config(c):
+    if SHRINK <= 1:
+        return synth.config(c)
+    if c == 3:
+        return synth.config(3, count_override=max(1, 256 // SHRINK))
+    from paper_1811_11720_b200 import cbc
+    n = synth.CONFIG_SHAPES[c][1] // SHRINK
+    while not cbc.is_prime(n):
+        n -= 1
+    return synth.config(c, n_override=n)
+
+
 def rank_problems(c, rank):
     """Problems of BASELINE.json configs[c] for `rank`: rank 0 gets exactly the seeded config; other ranks
     get the same shapes with rank-specific shifts (independent problems -> no data-path collective)."""
-    probs = synth.config(c)
+    probs = shrunk_config(c)
     if rank == 0:
         return probs
     out = []
@@ -250,7 +265,7 @@ def run_ours(args):
         alg = ALG_FP64_PER_EVAL[c]
         achieved = alg * ev / fused_avg_s
         sms, means, errs = batch.results()
-        rec = {"workload": workload_name(c), "value": aggregate([ev * steps] * world, total_s), "unit": UNIT,
+        rec = {"workload": workload_name(c) + (f" [SHRUNK x1/{SHRINK} for profiling: not a bench value]" if SHRINK > 1 else ""), "value": aggregate([ev * steps] * world, total_s), "unit": UNIT,
                "ms_per_step": total_s / steps * 1e3, "ms_per_step_best": min(step_ms), "steps": steps, "warmup": warmup,
                "evals_per_step_per_gpu": ev, "fused_kernel_ms": fused_avg_s * 1e3,
                "fused_kernel_share_of_step": fused_avg_s * 1e3 * steps / sum(step_ms),
@@ -263,12 +278,12 @@ def run_ours(args):
         return rec, probs, (w0, w1)
 
     windows = []
-    main, main_probs, w = measure(MAIN_CONFIG, args.steps, args.warmup)
+    main, main_probs, w = measure(args.main, args.steps, args.warmup)
     windows.append(w)
     others = []
     if not args.main_only:
-        for c, (k, wu) in {0: (50, 5), 2: (5, 3), 3: (3, 3), 4: (2, 3)}.items():
-            if args.others is not None and c not in args.others:
+        for c, (k, wu) in {0: (50, 5), 1: (50, 5), 2: (5, 3), 3: (3, 3), 4: (2, 3)}.items():
+            if c == args.main or (args.others is not None and c not in args.others):
                 continue
             rec, _, w = measure(c, k, wu)
             windows.append(w)
@@ -299,7 +314,7 @@ def run_ours(args):
                                "implied_clock_mhz_at_64_lanes": peak_rate / (sm_count * FP64_LANES_PER_SM) / 1e6},
            "clocks": clocks, "others": others}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        out["cpu_baseline"] = cpu_baseline(MAIN_CONFIG, reps=3)
+        out["cpu_baseline"] = cpu_baseline(args.main, reps=3)
     if rank == 0:
         print(json.dumps(out))
     if dist is not None:
@@ -311,7 +326,7 @@ def run_ours(args):
 # ----------------------------------------------------------------------------------------------------
 def cpu_baseline(c, reps):
     import oracle
-    probs = synth.config(c)
+    probs = shrunk_config(c)
     t0 = time.perf_counter()
     for _ in range(reps):
         for p in probs:
@@ -357,9 +372,15 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--main-only", action="store_true", help="time configs[1] only (skip the 'others' list)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--shrink", type=int, default=1,
+                    help="profiling only: run 1/S of every config's work (fewer sectors / a smaller prime n)")
+    ap.add_argument("--main", type=int, default=MAIN_CONFIG, choices=[0, 1, 2, 3, 4],
+                    help="config reported as the headline line (default configs[1]; others are for profiling runs)")
     ap.add_argument("--others", type=lambda v: [int(x) for x in v.split(",") if x != ""], default=None,
                     help="comma-separated subset of configs 0,2,3,4 to time besides configs[1] (default: all)")
     args = ap.parse_args()
+    global SHRINK
+    SHRINK = max(1, args.shrink)
     if args.impl == "reference":
         if args.steps > 40:
             args.steps = 40                                 # bounded: a step is ~1 s of host time

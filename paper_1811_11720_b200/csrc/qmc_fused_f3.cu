@@ -4,38 +4,39 @@
 
 namespace qmc {
 
-template <int DP, int G, bool WIDE> static cudaError_t launch_one(int grid, cudaStream_t st, const FusedArgs& a,
-                                                                  const unsigned long long* prog) {
-    fused_sector_kernel<DP, G, WIDE><<<grid, kThreads, 0, st>>>(a.probs, a.aux, a.vq, a.partials, prog);
+template <int DP, bool WIDE> static cudaError_t launch_one(int grid, cudaStream_t st, const FusedArgs& a,
+                                                           const unsigned long long* prog) {
+    fused_sector_kernel<DP, SectorGroup<DP>::value, WIDE><<<grid, kThreads, 0, st>>>(a.probs, a.aux, a.vq, a.partials, prog);
     return cudaGetLastError();
 }
-template <int DP, int G, bool WIDE> static int occ_one() {
+template <int DP, bool WIDE> static int occ_one() {
     int nb = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fused_sector_kernel<DP, G, WIDE>, kThreads, 0) != cudaSuccess) return -1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fused_sector_kernel<DP, SectorGroup<DP>::value, WIDE>, kThreads, 0) !=
+        cudaSuccess)
+        return -1;
     return nb;
 }
 
-cudaError_t launch_fused_f3(int dp, bool wide, int grid, cudaStream_t st, const FusedArgs& a, const unsigned long long* prog) {
-    switch (dp * 2 + (wide ? 1 : 0)) {
-        case 4 * 2: return launch_one<4, kGroup, false>(grid, st, a, prog);
-        case 4 * 2 + 1: return launch_one<4, kGroup, true>(grid, st, a, prog);
-        case 8 * 2: return launch_one<8, kGroup, false>(grid, st, a, prog);
-        case 8 * 2 + 1: return launch_one<8, kGroup, true>(grid, st, a, prog);
-        case 16 * 2: return launch_one<16, 2, false>(grid, st, a, prog);
-        case 16 * 2 + 1: return launch_one<16, 2, true>(grid, st, a, prog);
+#define QMC_F3_TABLE(FN, ...)                                    \
+    switch (dp * 2 + (wide ? 1 : 0)) {                            \
+        case 4 * 2: return FN<4, false>(__VA_ARGS__);             \
+        case 4 * 2 + 1: return FN<4, true>(__VA_ARGS__);          \
+        case 6 * 2: return FN<6, false>(__VA_ARGS__);             \
+        case 6 * 2 + 1: return FN<6, true>(__VA_ARGS__);          \
+        case 8 * 2: return FN<8, false>(__VA_ARGS__);             \
+        case 8 * 2 + 1: return FN<8, true>(__VA_ARGS__);          \
+        case 16 * 2: return FN<16, false>(__VA_ARGS__);           \
+        case 16 * 2 + 1: return FN<16, true>(__VA_ARGS__);        \
     }
+
+cudaError_t launch_fused_f3(int dp, bool wide, int grid, cudaStream_t st, const FusedArgs& a, const unsigned long long* prog) {
+    QMC_F3_TABLE(launch_one, grid, st, a, prog)
     return cudaErrorInvalidValue;
 }
 int occupancy_fused_f3(int dp, bool wide) {
-    switch (dp * 2 + (wide ? 1 : 0)) {
-        case 4 * 2: return occ_one<4, kGroup, false>();
-        case 4 * 2 + 1: return occ_one<4, kGroup, true>();
-        case 8 * 2: return occ_one<8, kGroup, false>();
-        case 8 * 2 + 1: return occ_one<8, kGroup, true>();
-        case 16 * 2: return occ_one<16, 2, false>();
-        case 16 * 2 + 1: return occ_one<16, 2, true>();
-    }
+    QMC_F3_TABLE(occ_one)
     return -1;
 }
+int group_fused_f3(int dp) { return dp <= 8 ? SectorGroup<8>::value : SectorGroup<16>::value; }
 
 }  // namespace qmc

@@ -44,7 +44,7 @@ int ncomp_of(int family) {
 }
 
 int dim_slots(int family, int dim) {
-    if (family == QMC_FAMILY_SECTOR) return dim <= 4 ? 4 : (dim <= 8 ? 8 : (dim <= 16 ? 16 : -1));
+    if (family == QMC_FAMILY_SECTOR) return dim <= 4 ? 4 : (dim <= 6 ? 6 : (dim <= 8 ? 8 : (dim <= 16 ? 16 : -1)));
     return dim <= 4 ? 4 : (dim <= 8 ? 8 : (dim <= 16 ? 16 : 32));
 }
 
@@ -161,7 +161,7 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
         if (p.family == QMC_FAMILY_SECTOR) {
             const int nmono = (p.n_params - 4 - p.dim) / (1 + p.dim);
             d.aux_off = (int)prog_off;
-            d.aux_len = 5 * nmono;                                      // coefs + 16 u16 ops per monomial
+            d.aux_len = 3 * nmono + 1;                                  // coefs + 16 one-byte steps per monomial + end-of-U / padding
             prog_off += (size_t)d.aux_len;
         }
         plan->max_m = std::max(plan->max_m, p.m);

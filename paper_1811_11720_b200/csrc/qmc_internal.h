@@ -56,8 +56,8 @@ struct alignas(16) DevAux {
     double fam0;                           // OSC: 2 pi u0
     double sec_c0[2];                      // sector: constant terms of U and F
     int sec_a, sec_b;                      // sector: powers of U and F
-    int sec_nops[2];                       // sector: interpreter ops of U and F
-    int sec_ncoef[2];                      // sector: non-constant monomials of U and F
+    int sec_nops[2];                       // sector: [0] = 32-bit step words of the program (U, end-of-U, F)
+    int sec_ncoef[2];                      // sector: [0] = coefficients of the program
     int status;                            // 0 or a qmc_status found while preparing
     int pad_;
     unsigned char nu[QMC_MAX_DIM];         // sector: nu_j

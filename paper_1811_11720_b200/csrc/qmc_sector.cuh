@@ -6,33 +6,41 @@
 // so the parameter block is compiled ON THE DEVICE (prepare_sector) into a tiny straight-line
 // program that the fused kernel interprets with warp-uniform control flow.  One program step is
 // one fp64 instruction per point:
-//     step = (variable j, FIRST, LAST, coefficient index)
-//     FIRST & LAST : sum  = fma(coef, x_j, sum)        (degree-1 monomial)
+//     step = one byte: 4 + 4*(variable j) + 2*FIRST + LAST     (0 = no-op, 1 = end of U, 2 = end of program)
+//     FIRST & LAST : sum  = fma(coef, x_j, sum)        (degree-1 monomial; coef = next coefficient)
 //     FIRST        : mon  = coef * x_j
 //     LAST         : sum  = fma(mon, x_j, sum)
 //     otherwise    : mon *= x_j
 // so a polynomial costs sum_t deg(t) fp64 instructions per point, with no separate additions.
-// The decode cost of a step (load, extract, indexed branch) is shared by the G points a thread
-// evaluates together.
+// Steps are dispatched by one indexed branch each (PTX brx.idx, threaded code: every case fetches
+// the next step and the next coefficient before its own fp64 work); the decode cost of a step is
+// shared by the G points a thread evaluates together, which is why this family runs G = 8 shifts
+// per lattice index where the registers allow it.  U and F are one instruction stream (the
+// end-of-U step parks the sum and restarts it with F's constant).
 #pragma once
 #include "qmc_fused.cuh"
 
 namespace qmc {
 
 constexpr int kSecMaxCoef = 128;     // non-constant monomials of U and F together
+constexpr int kSecMaxWords = kMaxSectorOps / 4;
+
+// step codes (one byte each): 0 = no-op, 1 = end of U, 2 = end of program, 4 + 4*j + 2*FIRST + LAST otherwise
+enum : int { SEC_NOP = 0, SEC_ENDU = 1, SEC_END = 2, SEC_BASE = 4 };
 
 struct SectorSmem {
-    double coefs[kSecMaxCoef];
-    unsigned short ops[kMaxSectorOps];
-    double c0[2];
-    int nops[2], ncoef[2];
+    double coefs[kSecMaxCoef];       // coefficients of the non-constant monomials, in step order
+    unsigned int words[kSecMaxWords];// step bytes: U's steps, SEC_ENDU, F's steps, SEC_END (copied word-wise)
+    double c0[2];                    // constant terms of U and F
+    int nwords, ncoef;
     int a, b;
     int nu[QMC_MAX_DIM];
 };
 
 // ---- device-side compiler: params -> program (one thread; a few hundred steps at most) ---------
-// program area of a problem (8-byte words at prog_area + aux_off): coefs[ncoefU + ncoefF], then
-// the u16 ops of U followed by those of F.
+// program area of a problem (8-byte words at prog_area + aux_off): coefs[nU + nF] (upper bound),
+// then the step bytes.  DevAux: sec_nops[0] = number of 32-bit step words, sec_ncoef[0] = number
+// of coefficients.
 __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned long long* prog_area) {
     if (threadIdx.x != 0) return;
     const int d = pb.dim;
@@ -55,15 +63,14 @@ __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned 
     }
     double* coefs = reinterpret_cast<double*>(prog_area + pb.aux_off);
     const int max_coef = cnt[0] + cnt[1];
-    unsigned short* ops = reinterpret_cast<unsigned short*>(prog_area + pb.aux_off + max_coef);
-    const int max_ops = (pb.aux_len - max_coef) * 4;
-    int nops_total = 0, ncoef_total = 0;
+    unsigned char* ops = reinterpret_cast<unsigned char*>(prog_area + pb.aux_off + max_coef);
+    const int max_ops = min((pb.aux_len - max_coef) * 8, kMaxSectorOps) - 4;   // room for SEC_ENDU, SEC_END and padding
+    int nops = 0, ncoef = 0;
     const double* base = p + 4 + d;
     for (int pol = 0; pol < 2; ++pol) {
         const double* c = base;
         const double* e = base + cnt[pol];
         double c0 = 0.0;
-        int nops = 0, ncoef = 0;
         for (int t = 0; t < cnt[pol]; ++t) {
             int deg = 0;
             for (int j = 0; j < d; ++j) {
@@ -73,97 +80,91 @@ __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned 
             }
             if (deg > 16 || status) { status = QMC_ERR_PARAMS; continue; }
             if (deg == 0) { c0 += c[t]; continue; }
-            if (ncoef_total + ncoef >= kSecMaxCoef || nops_total + nops + deg > kMaxSectorOps ||
-                nops_total + nops + deg > max_ops) { status = QMC_ERR_PARAMS; continue; }
-            coefs[ncoef_total + ncoef] = c[t];
+            if (ncoef >= kSecMaxCoef - 1 || nops + deg > max_ops) { status = QMC_ERR_PARAMS; continue; }
+            coefs[ncoef++] = c[t];
             int seen = 0;
             for (int j = 0; j < d; ++j) {
                 const int ej = (int)e[t * d + j];
                 for (int r = 0; r < ej; ++r) {
                     const int first = (seen == 0), last = (seen == deg - 1);
-                    ops[nops_total + nops] = (unsigned short)((j * 4 + first * 2 + last) | (ncoef << 8));
-                    ++nops; ++seen;
+                    ops[nops++] = (unsigned char)(SEC_BASE + j * 4 + first * 2 + last);
+                    ++seen;
                 }
             }
-            ++ncoef;
         }
         a.sec_c0[pol] = c0;
-        a.sec_nops[pol] = nops;
-        a.sec_ncoef[pol] = ncoef;
-        nops_total += nops;
-        ncoef_total += ncoef;
+        if (!status) ops[nops++] = (unsigned char)(pol == 0 ? SEC_ENDU : SEC_END);
         base += cnt[pol] * (1 + d);
     }
+    if (!status) while (nops & 3) ops[nops++] = (unsigned char)SEC_NOP;
+    a.sec_nops[0] = status ? 0 : nops / 4;
+    a.sec_nops[1] = 0;
+    a.sec_ncoef[0] = status ? 0 : ncoef;
+    a.sec_ncoef[1] = 0;
     a.status = status;
 }
 
-// ---- interpreter: one polynomial for G points --------------------------------------------------
-#define QMC_SEC_CASE(J)                                                                                         \
-    case 4 * (J) + 0:                                                                                           \
-        _Pragma("unroll") for (int q = 0; q < G; ++q) mon[q] *= x[q][(J) < DP ? (J) : 0];                       \
-        break;                                                                                                  \
-    case 4 * (J) + 1:                                                                                           \
-        _Pragma("unroll") for (int q = 0; q < G; ++q) sum[q] = __fma_rn(mon[q], x[q][(J) < DP ? (J) : 0], sum[q]); \
-        break;                                                                                                  \
-    case 4 * (J) + 2:                                                                                           \
-        _Pragma("unroll") for (int q = 0; q < G; ++q) mon[q] = cf * x[q][(J) < DP ? (J) : 0];                   \
-        break;                                                                                                  \
-    case 4 * (J) + 3:                                                                                           \
-        _Pragma("unroll") for (int q = 0; q < G; ++q) sum[q] = __fma_rn(cf, x[q][(J) < DP ? (J) : 0], sum[q]);  \
-        break;
+// ---- interpreter: U and F for G points (threaded code in inline PTX, see gen_sector_interp.py) ------
+#include "qmc_sector_interp.inc"
 
-template <int DP, int G>
-__device__ __forceinline__ void sector_poly(const double (&x)[G][DP], const unsigned short* __restrict__ ops, int nops,
-                                            const double* __restrict__ coefs, double c0, double (&sum)[G]) {
-    double mon[G];
+// S2-S4 for the G points of one lattice index: x[q][j] and the weight W[q] (Eq. 12, Eq. 18)
+template <int DP, int G, bool WIDE, int TR, bool FIT>
+__device__ __forceinline__ void sector_coords(const typename Res<WIDE>::T (&r)[DP], const SmemCtx<DP, G>& sm, int dim,
+                                              double inv_n, double wconst, int kor_r, double (&x)[G][DP], double (&W)[G]) {
+    double P[G], D[G];
 #pragma unroll
-    for (int q = 0; q < G; ++q) { sum[q] = c0; mon[q] = 0.0; }
-#pragma unroll 1
-    for (int i = 0; i < nops; ++i) {
-        const unsigned op = ops[i];
-        const double cf = coefs[op >> 8];
-        switch (op & 0xffu) {
-            QMC_SEC_CASE(0) QMC_SEC_CASE(1) QMC_SEC_CASE(2) QMC_SEC_CASE(3)
-            QMC_SEC_CASE(4) QMC_SEC_CASE(5) QMC_SEC_CASE(6) QMC_SEC_CASE(7)
-            QMC_SEC_CASE(8) QMC_SEC_CASE(9) QMC_SEC_CASE(10) QMC_SEC_CASE(11)
-            QMC_SEC_CASE(12) QMC_SEC_CASE(13) QMC_SEC_CASE(14) QMC_SEC_CASE(15)
-            default: break;
+    for (int q = 0; q < G; ++q) { P[q] = 1.0; D[q] = 1.0; }
+#pragma unroll
+    for (int j = 0; j < DP; ++j) {
+        if (j < dim) {
+            const double rd = Res<WIDE>::to_double(r[j]);
+#pragma unroll
+            for (int q = 0; q < G; ++q) x[q][j] = point_coord<DP, G, TR, FIT>(rd, inv_n, q, j, sm, kor_r, P[q], D[q]);
+        } else {
+#pragma unroll
+            for (int q = 0; q < G; ++q) x[q][j] = 1.0;
         }
     }
+#pragma unroll
+    for (int q = 0; q < G; ++q) W[q] = point_weight<TR, FIT>(P[q], D[q], wconst, kor_r);
 }
-#undef QMC_SEC_CASE
 
-template <int DP, int G, bool WIDE, int TR, bool FIT> struct SectorEval {
+// Transform and fit map are selected per point by a warp-uniform switch, so that the interpreter
+// below exists once per kernel (not once per transform variant).
+template <int DP, int G, bool WIDE> struct SectorEval {
     static constexpr int NC = 1;
     typedef SectorSmem Extra;
     static __device__ __forceinline__ void eval(const typename Res<WIDE>::T (&r)[DP], const SmemCtx<DP, G>& sm,
                                                 const SectorSmem& ex, int dim, double inv_n, double wconst, int kor_r,
                                                 double (&acc)[G][1]) {
-        double x[G][DP], P[G], D[G], pre[G];
+        double x[G][DP], num[G];
+        switch (sm.prob.tr_kind * 2 + (sm.prob.has_fit ? 1 : 0)) {
+#define QMC_CASE(TRK, FITB) \
+    case TRK * 2 + (FITB ? 1 : 0): sector_coords<DP, G, WIDE, TRK, FITB>(r, sm, dim, inv_n, wconst, kor_r, x, num); break;
+            QMC_CASE(TR_NONE, false) QMC_CASE(TR_NONE, true) QMC_CASE(TR_BAKER, false) QMC_CASE(TR_BAKER, true)
+            QMC_CASE(TR_KOR3, false) QMC_CASE(TR_KOR3, true) QMC_CASE(TR_KORR, false)
+#undef QMC_CASE
+            default: sector_coords<DP, G, WIDE, TR_KORR, true>(r, sm, dim, inv_n, wconst, kor_r, x, num); break;
+        }
+        double U[G], F[G];
 #pragma unroll
-        for (int q = 0; q < G; ++q) { P[q] = 1.0; D[q] = 1.0; pre[q] = 1.0; }
+        for (int q = 0; q < G; ++q) { U[q] = 0.0; F[q] = ex.c0[0]; }
+        sector_interp<DP, G>(x, (unsigned)__cvta_generic_to_shared(ex.words), (unsigned)__cvta_generic_to_shared(ex.coefs),
+                             ex.c0[1], U, F);
+        // num = W prod_j x_j^nu_j U^a, den = F^b   (small integer powers by repeated multiplication)
 #pragma unroll
         for (int j = 0; j < DP; ++j) {
             if (j < dim) {
-                const double rd = Res<WIDE>::to_double(r[j]);
-#pragma unroll
-                for (int q = 0; q < G; ++q) x[q][j] = point_coord<DP, G, TR, FIT>(rd, inv_n, q, j, sm, kor_r, P[q], D[q]);
                 const int nu = ex.nu[j];
 #pragma unroll 1
                 for (int e = 0; e < nu; ++e)
 #pragma unroll
-                    for (int q = 0; q < G; ++q) pre[q] *= x[q][j];
-            } else {
-#pragma unroll
-                for (int q = 0; q < G; ++q) x[q][j] = 1.0;
+                    for (int q = 0; q < G; ++q) num[q] *= x[q][j];
             }
         }
-        double U[G], F[G];
-        sector_poly<DP, G>(x, ex.ops, ex.nops[0], ex.coefs, ex.c0[0], U);
-        sector_poly<DP, G>(x, ex.ops + ex.nops[0], ex.nops[1], ex.coefs + ex.ncoef[0], ex.c0[1], F);
-        double num[G], den[G];
+        double den[G];
 #pragma unroll
-        for (int q = 0; q < G; ++q) { num[q] = pre[q]; den[q] = 1.0; }
+        for (int q = 0; q < G; ++q) den[q] = 1.0;
 #pragma unroll 1
         for (int e = 0; e < ex.a; ++e)
 #pragma unroll
@@ -172,20 +173,19 @@ template <int DP, int G, bool WIDE, int TR, bool FIT> struct SectorEval {
         for (int e = 0; e < ex.b; ++e)
 #pragma unroll
             for (int q = 0; q < G; ++q) den[q] *= F[q];
-        constexpr bool USEW = (TR == TR_KOR3 || TR == TR_KORR || FIT);
 #pragma unroll
-        for (int q = 0; q < G; ++q) {
-            const double w = USEW ? point_weight<TR, FIT>(P[q], D[q], wconst, kor_r) * num[q] : num[q];
-            acc[q][0] += w / den[q];
-        }
+        for (int q = 0; q < G; ++q) acc[q][0] += num[q] / den[q];
     }
 };
 
+// shifts per group and resident CTAs per SM by dimension-slot count (x[G][DP] lives in registers)
+template <int DP> struct SectorGroup { static constexpr int value = (DP <= 8) ? 8 : 4; };
+template <int DP, int G> struct SectorMinBlocks { static constexpr int value = (G * DP > 32 || G >= 8) ? 2 : 3; };
+
 template <int DP, int G, bool WIDE>
-__global__ void __launch_bounds__(kThreads, 3) fused_sector_kernel(const DevProblem* __restrict__ probs,
-                                                                   const DevAux* __restrict__ aux, VariantQueue vq,
-                                                                   double* __restrict__ partials,
-                                                                   const unsigned long long* __restrict__ prog_area) {
+__global__ void __launch_bounds__(kThreads, SectorMinBlocks<DP, G>::value)
+fused_sector_kernel(const DevProblem* __restrict__ probs, const DevAux* __restrict__ aux, VariantQueue vq,
+                    double* __restrict__ partials, const unsigned long long* __restrict__ prog_area) {
     __shared__ SmemCtx<DP, G> sm;
     __shared__ SectorSmem ex;
     int cur = -1;
@@ -196,30 +196,21 @@ __global__ void __launch_bounds__(kThreads, 3) fused_sector_kernel(const DevProb
             const int tid = threadIdx.x;
             const DevAux& a = aux[cur];
             const DevProblem& pb = sm.prob;
-            const int ncoef = a.sec_ncoef[0] + a.sec_ncoef[1], nops = a.sec_nops[0] + a.sec_nops[1];
+            const int ncoef = a.sec_ncoef[0], nwords = a.sec_nops[0];
             const int max_coef = (pb.n_params - 4 - pb.dim) / (1 + pb.dim);
             const double* coefs = reinterpret_cast<const double*>(prog_area + pb.aux_off);
-            const unsigned short* ops = reinterpret_cast<const unsigned short*>(prog_area + pb.aux_off + max_coef);
+            const unsigned int* words = reinterpret_cast<const unsigned int*>(prog_area + pb.aux_off + max_coef);
             for (int i = tid; i < ncoef; i += kThreads) ex.coefs[i] = coefs[i];
-            for (int i = tid; i < nops; i += kThreads) ex.ops[i] = ops[i];
+            for (int i = tid; i < nwords; i += kThreads) ex.words[i] = words[i];
             if (tid < QMC_MAX_DIM) ex.nu[tid] = a.nu[tid];
             if (tid == 32) {
                 ex.c0[0] = a.sec_c0[0]; ex.c0[1] = a.sec_c0[1];
-                ex.nops[0] = a.sec_nops[0]; ex.nops[1] = a.sec_nops[1];
-                ex.ncoef[0] = a.sec_ncoef[0]; ex.ncoef[1] = a.sec_ncoef[1];
+                ex.nwords = nwords; ex.ncoef = ncoef;
                 ex.a = a.sec_a; ex.b = a.sec_b;
             }
             __syncthreads();
         }
-        const int sel = sm.prob.tr_kind * 2 + (sm.prob.has_fit ? 1 : 0);
-        switch (sel) {
-#define QMC_CASE(TRK, FITB) \
-    case TRK * 2 + (FITB ? 1 : 0): run_tile<SectorEval<DP, G, WIDE, TRK, FITB>, DP, G, WIDE>(sm, ex, tile_local, partials); break;
-            QMC_CASE(TR_NONE, false) QMC_CASE(TR_NONE, true) QMC_CASE(TR_BAKER, false) QMC_CASE(TR_BAKER, true)
-            QMC_CASE(TR_KOR3, false) QMC_CASE(TR_KOR3, true) QMC_CASE(TR_KORR, false) QMC_CASE(TR_KORR, true)
-#undef QMC_CASE
-            default: break;
-        }
+        run_tile<SectorEval<DP, G, WIDE>, DP, G, WIDE>(sm, ex, tile_local, partials);
     }
 }
 
