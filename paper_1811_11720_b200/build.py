@@ -18,15 +18,24 @@ SOURCES = ["qmc_host.cu", "qmc_misc.cu", "qmc_project.cu", "qmc_fused_f0.cu", "q
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
 
 
-def _deps():
-    return [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cuh", ".h", ".inc"))] + \
-           [os.path.join(os.path.dirname(HERE), "include", "qmc_lattice.h")]
+def _deps(path, seen=None):
+    """the files `path` includes with #include "...", recursively (paths relative to the including file)"""
+    seen = set() if seen is None else seen
+    with open(path) as f:
+        for line in f:
+            line = line.strip()
+            if line.startswith("#include \""):
+                inc = os.path.normpath(os.path.join(os.path.dirname(path), line.split('"')[1]))
+                if inc not in seen and os.path.exists(inc):
+                    seen.add(inc)
+                    _deps(inc, seen)
+    return seen
 
 
 def _compile(src: str, force: bool) -> str:
     obj = os.path.join(OBJ, src.replace(".cu", ".o"))
     path = os.path.join(CSRC, src)
-    newest = max(os.path.getmtime(p) for p in [path] + _deps())
+    newest = max(os.path.getmtime(p) for p in [path, *_deps(path)])
     if force or not os.path.exists(obj) or os.path.getmtime(obj) < newest:
         subprocess.run(["nvcc", *NVCC_FLAGS, "-c", path, "-o", obj], check=True)
     return obj

@@ -12,27 +12,44 @@
 // Template parameters: FAMILY (integrand family), DP (dimension slots held in registers; the
 // runtime dim <= DP), G (shifts per group), WIDE (64-bit residues for n >= 2^31).  Transform and
 // fit map are runtime (warp-uniform) and select a fully specialised tile loop.
+//
+// Dimension slots j >= dim are PADDED, not branched around: z_j = 0 and Delta_j = 1/2 pin the slot
+// to u = 1/2 (centred coordinate c = 0), the family constants of the slot make its factor exactly
+// 1 (or its phase contribution exactly 0), the fit map of the slot is the identity, and a Korobov
+// slot contributes u(1-u) = 1/4 to the weight product, which the host compensates in wconst by
+// the exact factor 4^r per slot.  The per-point code is therefore one branch-free block and the
+// results are bit-identical to skipping the slots.
 #pragma once
+#include <cstddef>
+
 #include "qmc_device.cuh"
 
 namespace qmc {
 
 template <int FAMILY> struct FamTraits;
-template <> struct FamTraits<QMC_FAMILY_GENZ_OSC> { static constexpr int NC = 1; static constexpr int NS = 1; };
-template <> struct FamTraits<QMC_FAMILY_GENZ_PRODPEAK> { static constexpr int NC = 1; static constexpr int NS = 1; };
-template <> struct FamTraits<QMC_FAMILY_CEXP_POLY> { static constexpr int NC = 2; static constexpr int NS = 2; };
+template <> struct FamTraits<QMC_FAMILY_GENZ_OSC> { static constexpr int NC = 1; };
+template <> struct FamTraits<QMC_FAMILY_GENZ_PRODPEAK> { static constexpr int NC = 1; };
+template <> struct FamTraits<QMC_FAMILY_CEXP_POLY> { static constexpr int NC = 2; };
 
-// Shared-memory image of the problem a CTA is working on.
-template <int DP, int G> struct SmemCtx {
-    double delta[G * DP];          // shifts of the current group, [q][j]
-    double fam_a[DP], fam_b[DP];
-    double fit[5][DP];
-    double kor[8];
-    unsigned long long z[DP], step[DP], back[DP];
+// Shared-memory image of the problem a CTA is working on.  The double arrays at the front are the
+// operands of the inner loop; they are read with ld.shared at sbase + compile-time offsets.
+template <int DP, int G> struct alignas(16) SmemCtx {
+    double delta[DP * G];          // [j][q]  shifts of the current group (1/2 in padded slots)
+    double fam[DP * 2];            // [j] = (fam_a, fam_b)
+    double fit[DP * 6];            // [j] = (a4, a5, a6, 2 a5, 3 a6, -)  cubic map of Eq. 19
+    double kor[8];                 // centred Korobov polynomial g_r
+    unsigned long long step[DP], back[DP], z[DP];
     double red[kWarps][G * 2];
     DevProblem prob;
     double fam0;
     long long tile;                // popped tile index
+};
+template <int DP, int G> struct SmemOff {
+    static constexpr unsigned delta = 0;
+    static constexpr unsigned fam = delta + DP * G * 8;
+    static constexpr unsigned fit = fam + DP * 2 * 8;
+    static constexpr unsigned kor = fit + DP * 6 * 8;
+    static constexpr unsigned step = kor + 8 * 8;
 };
 
 // ---- per-dimension and per-point pieces of the closed-form families (S5) ----------------------
@@ -55,7 +72,8 @@ template <int FAMILY> __device__ __forceinline__ void fam_finish(double s0, doub
         const double f = cos(s0);
         acc[0] = use_w ? __fma_rn(W, f, acc[0]) : acc[0] + f;
     } else if (FAMILY == QMC_FAMILY_GENZ_PRODPEAK) {
-        acc[0] += use_w ? W / s0 : 1.0 / s0;
+        const double f = rcp_nr(s0);
+        acc[0] = use_w ? __fma_rn(W, f, acc[0]) : acc[0] + f;
     } else {
         double sn, cs;
         sincos(s0, &sn, &cs);
@@ -66,11 +84,13 @@ template <int FAMILY> __device__ __forceinline__ void fam_finish(double s0, doub
 }
 
 // ---- S2-S4 for one (shift q, dimension j): coordinate, periodizing transform, fit map ----------
+struct FitC { double f0, f1, f2, f3, f4; };       // a4, a5, a6, 2 a5, 3 a6 of one dimension
+
 // Returns x_j; multiplies P by u(1-u) (Korobov) and D by p'(y) (fit).
-template <int DP, int G, int TR, bool FIT>
-__device__ __forceinline__ double point_coord(double rd, double inv_n, int q, int j, const SmemCtx<DP, G>& sm, int kor_r,
-                                              double& P, double& D) {
-    const double t = coord_t(rd, inv_n, sm.delta[q * DP + j]);
+template <int TR, bool FIT>
+__device__ __forceinline__ double point_coord(double rd, double inv_n, double delta, const FitC& fc, unsigned kor_addr,
+                                              int kor_r, double& P, double& D) {
+    const double t = coord_t(rd, inv_n, delta);
     double x;
     if (TR == TR_NONE) {
         x = wrap_u(t);
@@ -87,17 +107,17 @@ __device__ __forceinline__ double point_coord(double rd, double inv_n, int q, in
                 g = __fma_rn(g, s, -8.75);
                 g = __fma_rn(g, s, 2.1875);
             } else {
-                g = sm.kor[kor_r];
+                g = lds_f64(kor_addr + 8u * (unsigned)kor_r);
 #pragma unroll 1
-                for (int i = kor_r - 1; i >= 0; --i) g = __fma_rn(g, s, sm.kor[i]);
+                for (int i = kor_r - 1; i >= 0; --i) g = __fma_rn(g, s, lds_f64(kor_addr + 8u * (unsigned)i));
             }
             x = __fma_rn(c, g, 0.5);                          // phi(u) = 1/2 + c g(c^2)
         }
     }
     if (FIT) {                                                // S4: cubic map of Eq. 19 (a2 = a3 = 0)
         const double y = x;
-        const double h = __fma_rn(y, __fma_rn(y, sm.fit[2][j], sm.fit[1][j]), sm.fit[0][j]);
-        D *= __fma_rn(y, __fma_rn(y, sm.fit[4][j], sm.fit[3][j]), sm.fit[0][j]);   // p'(y)
+        const double h = __fma_rn(y, __fma_rn(y, fc.f2, fc.f1), fc.f0);
+        D *= __fma_rn(y, __fma_rn(y, fc.f4, fc.f3), fc.f0);   // p'(y)
         x = y * h;                                            // p(y)
     }
     return x;
@@ -112,30 +132,55 @@ template <int TR, bool FIT> __device__ __forceinline__ double point_weight(doubl
     return W;
 }
 
+// operands of dimension slot j: family constants, fit constants, the G shifts of the group
+template <int DP, int G, bool FIT>
+__device__ __forceinline__ void load_slot(unsigned sbase, int j, double& fa, double& fb, FitC& fc, double (&dl)[G]) {
+    typedef SmemOff<DP, G> O;
+    lds_f64x2(sbase + O::fam + 16u * j, fa, fb);
+    if (FIT) {
+        lds_f64x2(sbase + O::fit + 48u * j, fc.f0, fc.f1);
+        lds_f64x2(sbase + O::fit + 48u * j + 16u, fc.f2, fc.f3);
+        fc.f4 = lds_f64(sbase + O::fit + 48u * j + 32u);
+    }
+    if (G % 2 == 0) {
+#pragma unroll
+        for (int q = 0; q < G; q += 2) lds_f64x2(sbase + O::delta + 8u * (j * G + q), dl[q], dl[q + 1 < G ? q + 1 : q]);
+    } else {
+#pragma unroll
+        for (int q = 0; q < G; ++q) dl[q] = lds_f64(sbase + O::delta + 8u * (j * G + q));
+    }
+}
+
 // ---- one lattice index, G shifts: S2-S6 for the closed-form families --------------------------
+struct EvalCtx {            // per-tile constants held in registers
+    unsigned sbase;         // shared address of the CTA's SmemCtx
+    double inv_n, wconst, fam0;
+    int kor_r;
+    int sel;                // tr_kind * 2 + has_fit
+};
+
 template <int FAMILY, int DP, int G, bool WIDE, int TR, bool FIT>
-__device__ __forceinline__ void eval_point_group(const typename Res<WIDE>::T (&r)[DP], const SmemCtx<DP, G>& sm, int dim,
-                                                 double inv_n, double wconst, int kor_r,
+__device__ __forceinline__ void eval_point_group(const typename Res<WIDE>::T (&r)[DP], const EvalCtx& cx,
                                                  double (&acc)[G][FamTraits<FAMILY>::NC]) {
     double s0[G], s1[G], P[G], D[G];
 #pragma unroll
-    for (int q = 0; q < G; ++q) { fam_init<FAMILY>(s0[q], s1[q], sm.fam0); P[q] = 1.0; D[q] = 1.0; }
+    for (int q = 0; q < G; ++q) { fam_init<FAMILY>(s0[q], s1[q], cx.fam0); P[q] = 1.0; D[q] = 1.0; }
 #pragma unroll
     for (int j = 0; j < DP; ++j) {
-        if (j < dim) {
-            const double rd = Res<WIDE>::to_double(r[j]);
-            const double fa = sm.fam_a[j], fb = sm.fam_b[j];
+        const double rd = Res<WIDE>::to_double(r[j]);
+        double fa, fb, dl[G];
+        FitC fc;
+        load_slot<DP, G, FIT>(cx.sbase, j, fa, fb, fc, dl);
 #pragma unroll
-            for (int q = 0; q < G; ++q) {
-                const double x = point_coord<DP, G, TR, FIT>(rd, inv_n, q, j, sm, kor_r, P[q], D[q]);
-                fam_dim<FAMILY>(s0[q], s1[q], x, fa, fb);
-            }
+        for (int q = 0; q < G; ++q) {
+            const double x = point_coord<TR, FIT>(rd, cx.inv_n, dl[q], fc, cx.sbase + SmemOff<DP, G>::kor, cx.kor_r, P[q], D[q]);
+            fam_dim<FAMILY>(s0[q], s1[q], x, fa, fb);
         }
     }
     constexpr bool USEW = (TR == TR_KOR3 || TR == TR_KORR || FIT);
 #pragma unroll
     for (int q = 0; q < G; ++q)
-        fam_finish<FAMILY>(s0[q], s1[q], point_weight<TR, FIT>(P[q], D[q], wconst, kor_r), USEW, acc[q]);
+        fam_finish<FAMILY>(s0[q], s1[q], point_weight<TR, FIT>(P[q], D[q], cx.wconst, cx.kor_r), USEW, acc[q]);
 }
 
 struct NoExtra {};
@@ -143,39 +188,51 @@ struct NoExtra {};
 template <int FAMILY, int DP, int G, bool WIDE, int TR, bool FIT> struct ClosedEval {
     static constexpr int NC = FamTraits<FAMILY>::NC;
     typedef NoExtra Extra;
-    static __device__ __forceinline__ void eval(const typename Res<WIDE>::T (&r)[DP], const SmemCtx<DP, G>& sm, const Extra&,
-                                                int dim, double inv_n, double wconst, int kor_r, double (&acc)[G][NC]) {
-        eval_point_group<FAMILY, DP, G, WIDE, TR, FIT>(r, sm, dim, inv_n, wconst, kor_r, acc);
+    static __device__ __forceinline__ void eval(const typename Res<WIDE>::T (&r)[DP], const SmemCtx<DP, G>&, const Extra&,
+                                                const EvalCtx& cx, double (&acc)[G][NC]) {
+        eval_point_group<FAMILY, DP, G, WIDE, TR, FIT>(r, cx, acc);
     }
 };
 
 // ---- one tile: residue walk (S1), G shifts per index (EV::eval = S2-S6), tile reduction (S7) ----
 template <class EV, int DP, int G, bool WIDE>
-__device__ __forceinline__ void run_tile(SmemCtx<DP, G>& sm, const typename EV::Extra& ex, long long tile_local,
+__device__ __forceinline__ void run_tile(SmemCtx<DP, G>& sm, unsigned sbase, const typename EV::Extra& ex, long long tile_local,
                                          double* __restrict__ partials) {
     typedef typename Res<WIDE>::T RT;
     constexpr int NC = EV::NC;
+    // residue strides live in registers while they are few; otherwise they are re-read from shared memory
+    constexpr bool STEP_IN_REGS = DP * (WIDE ? 2 : 1) <= 16;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const DevProblem& pb = sm.prob;
-    const int dim = pb.dim, m = pb.m, steps = pb.steps, kor_r = pb.kor_r;
+    const int dim = pb.dim, m = pb.m, steps = pb.steps;
     const unsigned long long n = pb.n;
-    const double inv_n = pb.inv_n, wconst = pb.wconst;
+    EvalCtx cx;
+    cx.sbase = sbase; cx.inv_n = pb.inv_n; cx.wconst = pb.wconst; cx.fam0 = sm.fam0; cx.kor_r = pb.kor_r;
+    cx.sel = pb.tr_kind * 2 + (pb.has_fit ? 1 : 0);
+    typedef SmemCtx<DP, G> Ctx;
+    typedef SmemOff<DP, G> Off;
+    static_assert(offsetof(Ctx, fam) == Off::fam && offsetof(Ctx, fit) == Off::fit && offsetof(Ctx, kor) == Off::kor &&
+                  offsetof(Ctx, step) == Off::step, "SmemOff must mirror SmemCtx");
     const unsigned long long tile_len = (unsigned long long)steps * kThreads;
     const unsigned long long k0 = (unsigned long long)tile_local * tile_len;
     const unsigned long long kend = (k0 + tile_len < n) ? k0 + tile_len : n;
     const unsigned long long kfirst = k0 + tid;
+    const int live_steps = kfirst < kend ? (int)((kend - kfirst + kThreads - 1) / kThreads) : 0;   // indices this thread owns
 
-    RT r[DP];
+    RT r[DP], stp[STEP_IN_REGS ? DP : 1];
 #pragma unroll
-    for (int j = 0; j < DP; ++j) r[j] = (j < dim) ? (RT)mulmod_u64(kfirst % n, sm.z[j], n) : (RT)0;
+    for (int j = 0; j < DP; ++j) {
+        r[j] = (RT)mulmod_u64(kfirst % n, sm.z[j], n);          // padded slots: z = 0 -> r = 0
+        if (STEP_IN_REGS) stp[j] = (RT)sm.step[j];
+    }
 
 #pragma unroll 1
     for (int g0 = 0; g0 < m; g0 += G) {
         const int gcount = (m - g0 < G) ? (m - g0) : G;
         __syncthreads();                                    // previous group's readers of delta/red are done
         for (int e = tid; e < G * DP; e += kThreads) {
-            const int q = e / DP, j = e - q * DP;
-            sm.delta[e] = (q < gcount && j < dim) ? pb.shifts[(size_t)(g0 + q) * dim + j] : 0.0;
+            const int j = e / G, q = e - j * G;
+            sm.delta[e] = (q < gcount && j < dim) ? pb.shifts[(size_t)(g0 + q) * dim + j] : 0.5;
         }
         __syncthreads();
 
@@ -185,20 +242,24 @@ __device__ __forceinline__ void run_tile(SmemCtx<DP, G>& sm, const typename EV::
 #pragma unroll
             for (int c = 0; c < NC; ++c) acc[q][c] = 0.0;
 
-        unsigned long long k = kfirst;
 #pragma unroll 1
-        for (int i = 0; i < steps; ++i) {
-            asm volatile("" ::: "memory");   // keep the shared-memory operands as loads inside the walk (no hoisting into registers)
-            if (k < kend) EV::eval(r, sm, ex, dim, inv_n, wconst, kor_r, acc);
+        for (int i = 0; i < live_steps; ++i) {
+            EV::eval(r, sm, ex, cx, acc);
 #pragma unroll
             for (int j = 0; j < DP; ++j)
-                if (j < dim) r[j] = add_mod<RT>(r[j], (RT)sm.step[j], (RT)n);
-            k += kThreads;
+                r[j] = add_mod<RT>(r[j], STEP_IN_REGS ? stp[STEP_IN_REGS ? j : 0] : (RT)lds_u64(sbase + SmemOff<DP, G>::step + 8u * j), (RT)n);
         }
-        // rewind to the thread's first index for the next group
+        // rewind to the thread's first index for the next group: live_steps * kThreads * z_j, via the full-tile rewind
+        // when the thread walked the whole tile, else by recomputing the first residue
+        if (g0 + G < m) {
+            if (live_steps == steps) {
 #pragma unroll
-        for (int j = 0; j < DP; ++j)
-            if (j < dim) r[j] = sub_mod<RT>(r[j], (RT)sm.back[j], (RT)n);
+                for (int j = 0; j < DP; ++j) r[j] = sub_mod<RT>(r[j], (RT)sm.back[j], (RT)n);
+            } else {
+#pragma unroll
+                for (int j = 0; j < DP; ++j) r[j] = (RT)mulmod_u64(kfirst % n, sm.z[j], n);
+            }
+        }
 
         // S7: fixed-shape reduction of the group's sums, one slot per (tile, shift, component)
 #pragma unroll
@@ -249,11 +310,12 @@ __device__ __forceinline__ bool next_tile(SmemCtx<DP, G>& sm, const DevProblem* 
         const DevAux& a = aux[pidx];
         if (tid == 32) sm.fam0 = a.fam0;
         if (tid >= 64 && tid < 72) sm.kor[tid - 64] = probs[pidx].kor[tid - 64];
-        for (int j = tid; j < DP; j += kThreads) {
+        for (int j = tid; j < DP; j += kThreads) {          // slots j >= dim hold the padding values (prepare_kernel)
             sm.z[j] = a.z[j]; sm.step[j] = a.step[j]; sm.back[j] = a.back[j];
-            sm.fam_a[j] = a.fam_a[j]; sm.fam_b[j] = a.fam_b[j];
+            sm.fam[2 * j] = a.fam_a[j]; sm.fam[2 * j + 1] = a.fam_b[j];
 #pragma unroll
-            for (int i = 0; i < 5; ++i) sm.fit[i][j] = a.fit[i][j];
+            for (int i = 0; i < 5; ++i) sm.fit[6 * j + i] = a.fit[i][j];
+            sm.fit[6 * j + 5] = 0.0;
         }
         __syncthreads();
     }
@@ -268,6 +330,7 @@ __global__ void __launch_bounds__(kThreads, MinBlocks<DP, WIDE>::value) fused_ke
                                                          const DevAux* __restrict__ aux, VariantQueue vq,
                                                          double* __restrict__ partials) {
     __shared__ SmemCtx<DP, G> sm;
+    const unsigned sbase = (unsigned)__cvta_generic_to_shared(&sm);
     int cur = -1;
     long long tile_local = 0;
     bool changed;
@@ -276,7 +339,7 @@ __global__ void __launch_bounds__(kThreads, MinBlocks<DP, WIDE>::value) fused_ke
         const int sel = sm.prob.tr_kind * 2 + (sm.prob.has_fit ? 1 : 0);
         switch (sel) {
 #define QMC_CASE(TRK, FITB) \
-    case TRK * 2 + (FITB ? 1 : 0): run_tile<ClosedEval<FAMILY, DP, G, WIDE, TRK, FITB>, DP, G, WIDE>(sm, ex, tile_local, partials); break;
+    case TRK * 2 + (FITB ? 1 : 0): run_tile<ClosedEval<FAMILY, DP, G, WIDE, TRK, FITB>, DP, G, WIDE>(sm, sbase, ex, tile_local, partials); break;
             QMC_CASE(TR_NONE, false) QMC_CASE(TR_NONE, true) QMC_CASE(TR_BAKER, false) QMC_CASE(TR_BAKER, true)
             QMC_CASE(TR_KOR3, false) QMC_CASE(TR_KOR3, true) QMC_CASE(TR_KORR, false) QMC_CASE(TR_KORR, true)
 #undef QMC_CASE

@@ -145,6 +145,8 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
             for (int k = 0; k <= r; ++k)
                 d.kor[k] = cr * binom(r, k) * std::ldexp(1.0, 2 * (k - r)) * ((k & 1) ? -1.0 : 1.0) / (double)(2 * k + 1);
             for (int j = 0; j < p.dim; ++j) d.wconst *= cr;
+            // padded dimension slots contribute u(1-u) = 1/4 each to the weight product (qmc_fused.cuh): exact compensation
+            d.wconst = std::ldexp(d.wconst, 2 * r * (dim_slots(p.family, p.dim) - p.dim));
         }
         const unsigned long long per = (unsigned long long)kThreads * (unsigned long long)per_problem_target;
         unsigned long long steps = (p.n + per - 1) / per;

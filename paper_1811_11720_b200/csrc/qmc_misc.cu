@@ -34,6 +34,11 @@ __global__ void __launch_bounds__(32) prepare_kernel(const DevProblem* __restric
                 f[0] = a4; f[1] = a5; f[2] = a6; f[3] = 2.0 * a5; f[4] = 3.0 * a6;
             }
         }
+        if (j >= d && pb.family == QMC_FAMILY_GENZ_PRODPEAK) {
+            // padded slot (qmc_fused.cuh): the coordinate is pinned to u = 1/2, i.e. x = 1 (baker) or 1/2; factor (x-fb)^2 + fa = 1
+            fa = 1.0;
+            fb = (pb.tr_kind == TR_BAKER) ? 1.0 : 0.5;
+        }
         a.z[j] = z; a.step[j] = step; a.back[j] = back; a.fam_a[j] = fa; a.fam_b[j] = fb;
 #pragma unroll
         for (int i = 0; i < 5; ++i) a.fit[i][j] = f[i];

@@ -25,25 +25,37 @@ namespace qmc {
 constexpr int kSecMaxCoef = 128;     // non-constant monomials of U and F together
 constexpr int kSecMaxWords = kMaxSectorOps / 4;
 
-// step codes (one byte each): 0 = no-op, 1 = end of U, 2 = end of program, 4 + 4*j + 2*FIRST + LAST otherwise
+// step codes (one byte each): 0 = no-op, 1 = end of U, 2 = end of program, 4 + 4*j + 2*FIRST + LAST (single
+// variable); with DP <= 8 dimension slots also 4 + 4*DP + 2*pair(a,b) + FULL, a <= b: the first two variables of a
+// monomial in one step (mon = coef x_a; FULL ? sum = fma(mon, x_b, sum) : mon *= x_b), pair(a,b) = a DP - a(a-1)/2 + b - a
 enum : int { SEC_NOP = 0, SEC_ENDU = 1, SEC_END = 2, SEC_BASE = 4 };
 
-struct SectorSmem {
+struct alignas(16) SectorSmem {
     double coefs[kSecMaxCoef];       // coefficients of the non-constant monomials, in step order
     unsigned int words[kSecMaxWords];// step bytes: U's steps, SEC_ENDU, F's steps, SEC_END (copied word-wise)
     double c0[2];                    // constant terms of U and F
-    int nwords, ncoef;
-    int a, b;
-    int nu[QMC_MAX_DIM];
+    unsigned long long nu_packed;    // nu_j in 4 bits each
+    int a, b;                        // powers of U and F
 };
+struct SectorOff {                   // byte offsets of the fields above (read with ld.shared in the inner loop)
+    static constexpr unsigned coefs = 0, words = kSecMaxCoef * 8, c0 = words + kSecMaxWords * 4, nu = c0 + 16, ab = nu + 8;
+};
+
+static_assert(offsetof(SectorSmem, words) == SectorOff::words && offsetof(SectorSmem, c0) == SectorOff::c0 &&
+              offsetof(SectorSmem, nu_packed) == SectorOff::nu && offsetof(SectorSmem, a) == SectorOff::ab, "SectorOff must mirror SectorSmem");
 
 // ---- device-side compiler: params -> program (one thread; a few hundred steps at most) ---------
 // program area of a problem (8-byte words at prog_area + aux_off): coefs[nU + nF] (upper bound),
 // then the step bytes.  DevAux: sec_nops[0] = number of 32-bit step words, sec_ncoef[0] = number
 // of coefficients.
+__host__ __device__ inline bool sector_has_pairs(int dp) { return dp <= 0; }   // all step codes must fit one byte
+__host__ __device__ inline int sector_dim_slots(int dim) { return dim <= 4 ? 4 : (dim <= 6 ? 6 : (dim <= 8 ? 8 : (dim <= 16 ? 16 : -1))); }
+
 __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned long long* prog_area) {
     if (threadIdx.x != 0) return;
     const int d = pb.dim;
+    const int dp = sector_dim_slots(d);
+    const bool pairs = sector_has_pairs(dp);
     const double* p = pb.params;
     int status = 0;
     const double av = p[0], bv = p[1], nUv = p[2], nFv = p[3];
@@ -64,7 +76,7 @@ __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned 
     double* coefs = reinterpret_cast<double*>(prog_area + pb.aux_off);
     const int max_coef = cnt[0] + cnt[1];
     unsigned char* ops = reinterpret_cast<unsigned char*>(prog_area + pb.aux_off + max_coef);
-    const int max_ops = min((pb.aux_len - max_coef) * 8, kMaxSectorOps) - 4;   // room for SEC_ENDU, SEC_END and padding
+    const int max_ops = min((pb.aux_len - max_coef) * 8, kMaxSectorOps) - 8;   // room for SEC_ENDU, SEC_END and 3+ bytes of read-ahead padding
     int nops = 0, ncoef = 0;
     const double* base = p + 4 + d;
     for (int pol = 0; pol < 2; ++pol) {
@@ -82,12 +94,17 @@ __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned 
             if (deg == 0) { c0 += c[t]; continue; }
             if (ncoef >= kSecMaxCoef - 1 || nops + deg > max_ops) { status = QMC_ERR_PARAMS; continue; }
             coefs[ncoef++] = c[t];
-            int seen = 0;
+            int seen = 0, va = -1;
             for (int j = 0; j < d; ++j) {
                 const int ej = (int)e[t * d + j];
                 for (int r = 0; r < ej; ++r) {
                     const int first = (seen == 0), last = (seen == deg - 1);
-                    ops[nops++] = (unsigned char)(SEC_BASE + j * 4 + first * 2 + last);
+                    if (pairs && deg >= 2 && seen < 2) {        // the first two variables a <= b go into one pair step
+                        if (seen == 0) va = j;
+                        else ops[nops++] = (unsigned char)(SEC_BASE + 4 * dp + 2 * (va * dp - va * (va - 1) / 2 + (j - va)) + last);
+                    } else {
+                        ops[nops++] = (unsigned char)(SEC_BASE + j * 4 + first * 2 + last);
+                    }
                     ++seen;
                 }
             }
@@ -109,72 +126,72 @@ __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned 
 
 // S2-S4 for the G points of one lattice index: x[q][j] and the weight W[q] (Eq. 12, Eq. 18)
 template <int DP, int G, bool WIDE, int TR, bool FIT>
-__device__ __forceinline__ void sector_coords(const typename Res<WIDE>::T (&r)[DP], const SmemCtx<DP, G>& sm, int dim,
-                                              double inv_n, double wconst, int kor_r, double (&x)[G][DP], double (&W)[G]) {
+__device__ __forceinline__ void sector_coords(const typename Res<WIDE>::T (&r)[DP], const EvalCtx& cx, double (&x)[G][DP],
+                                              double (&W)[G]) {
     double P[G], D[G];
 #pragma unroll
     for (int q = 0; q < G; ++q) { P[q] = 1.0; D[q] = 1.0; }
 #pragma unroll
     for (int j = 0; j < DP; ++j) {
-        if (j < dim) {
-            const double rd = Res<WIDE>::to_double(r[j]);
+        const double rd = Res<WIDE>::to_double(r[j]);
+        double fa, fb, dl[G];
+        FitC fc;
+        load_slot<DP, G, FIT>(cx.sbase, j, fa, fb, fc, dl);
 #pragma unroll
-            for (int q = 0; q < G; ++q) x[q][j] = point_coord<DP, G, TR, FIT>(rd, inv_n, q, j, sm, kor_r, P[q], D[q]);
-        } else {
-#pragma unroll
-            for (int q = 0; q < G; ++q) x[q][j] = 1.0;
-        }
+        for (int q = 0; q < G; ++q)
+            x[q][j] = point_coord<TR, FIT>(rd, cx.inv_n, dl[q], fc, cx.sbase + SmemOff<DP, G>::kor, cx.kor_r, P[q], D[q]);
     }
 #pragma unroll
-    for (int q = 0; q < G; ++q) W[q] = point_weight<TR, FIT>(P[q], D[q], wconst, kor_r);
+    for (int q = 0; q < G; ++q) W[q] = point_weight<TR, FIT>(P[q], D[q], cx.wconst, cx.kor_r);
 }
 
 // Transform and fit map are selected per point by a warp-uniform switch, so that the interpreter
-// below exists once per kernel (not once per transform variant).
+// exists once per kernel (not once per transform variant).
 template <int DP, int G, bool WIDE> struct SectorEval {
     static constexpr int NC = 1;
-    typedef SectorSmem Extra;
-    static __device__ __forceinline__ void eval(const typename Res<WIDE>::T (&r)[DP], const SmemCtx<DP, G>& sm,
-                                                const SectorSmem& ex, int dim, double inv_n, double wconst, int kor_r,
-                                                double (&acc)[G][1]) {
+    typedef unsigned Extra;                                  // shared address of the CTA's SectorSmem
+    static __device__ __forceinline__ void eval(const typename Res<WIDE>::T (&r)[DP], const SmemCtx<DP, G>&, const unsigned& exbase,
+                                                const EvalCtx& cx, double (&acc)[G][1]) {
         double x[G][DP], num[G];
-        switch (sm.prob.tr_kind * 2 + (sm.prob.has_fit ? 1 : 0)) {
+        switch (cx.sel) {
 #define QMC_CASE(TRK, FITB) \
-    case TRK * 2 + (FITB ? 1 : 0): sector_coords<DP, G, WIDE, TRK, FITB>(r, sm, dim, inv_n, wconst, kor_r, x, num); break;
+    case TRK * 2 + (FITB ? 1 : 0): sector_coords<DP, G, WIDE, TRK, FITB>(r, cx, x, num); break;
             QMC_CASE(TR_NONE, false) QMC_CASE(TR_NONE, true) QMC_CASE(TR_BAKER, false) QMC_CASE(TR_BAKER, true)
             QMC_CASE(TR_KOR3, false) QMC_CASE(TR_KOR3, true) QMC_CASE(TR_KORR, false)
 #undef QMC_CASE
-            default: sector_coords<DP, G, WIDE, TR_KORR, true>(r, sm, dim, inv_n, wconst, kor_r, x, num); break;
+            default: sector_coords<DP, G, WIDE, TR_KORR, true>(r, cx, x, num); break;
         }
+        double c0u, c0f;
+        lds_f64x2(exbase + SectorOff::c0, c0u, c0f);
         double U[G], F[G];
 #pragma unroll
-        for (int q = 0; q < G; ++q) { U[q] = 0.0; F[q] = ex.c0[0]; }
-        sector_interp<DP, G>(x, (unsigned)__cvta_generic_to_shared(ex.words), (unsigned)__cvta_generic_to_shared(ex.coefs),
-                             ex.c0[1], U, F);
+        for (int q = 0; q < G; ++q) { U[q] = 0.0; F[q] = c0u; }
+        sector_interp<DP, G>(x, exbase + SectorOff::words, exbase + SectorOff::coefs, c0f, U, F);
         // num = W prod_j x_j^nu_j U^a, den = F^b   (small integer powers by repeated multiplication)
+        const unsigned long long nup = lds_u64(exbase + SectorOff::nu);
+        const unsigned long long ab = lds_u64(exbase + SectorOff::ab);
+        const int pa = (int)(unsigned)ab, pb = (int)(ab >> 32);
 #pragma unroll
         for (int j = 0; j < DP; ++j) {
-            if (j < dim) {
-                const int nu = ex.nu[j];
+            const int nu = (int)((nup >> (4 * j)) & 15ull);
 #pragma unroll 1
-                for (int e = 0; e < nu; ++e)
+            for (int e = 0; e < nu; ++e)
 #pragma unroll
-                    for (int q = 0; q < G; ++q) num[q] *= x[q][j];
-            }
+                for (int q = 0; q < G; ++q) num[q] *= x[q][j];
         }
         double den[G];
 #pragma unroll
         for (int q = 0; q < G; ++q) den[q] = 1.0;
 #pragma unroll 1
-        for (int e = 0; e < ex.a; ++e)
+        for (int e = 0; e < pa; ++e)
 #pragma unroll
             for (int q = 0; q < G; ++q) num[q] *= U[q];
 #pragma unroll 1
-        for (int e = 0; e < ex.b; ++e)
+        for (int e = 0; e < pb; ++e)
 #pragma unroll
             for (int q = 0; q < G; ++q) den[q] *= F[q];
 #pragma unroll
-        for (int q = 0; q < G; ++q) acc[q][0] += num[q] / den[q];
+        for (int q = 0; q < G; ++q) acc[q][0] = __fma_rn(num[q], rcp_nr(den[q]), acc[q][0]);
     }
 };
 
@@ -188,6 +205,7 @@ fused_sector_kernel(const DevProblem* __restrict__ probs, const DevAux* __restri
                     double* __restrict__ partials, const unsigned long long* __restrict__ prog_area) {
     __shared__ SmemCtx<DP, G> sm;
     __shared__ SectorSmem ex;
+    const unsigned sbase = (unsigned)__cvta_generic_to_shared(&sm), exbase = (unsigned)__cvta_generic_to_shared(&ex);
     int cur = -1;
     long long tile_local = 0;
     bool changed;
@@ -200,17 +218,18 @@ fused_sector_kernel(const DevProblem* __restrict__ probs, const DevAux* __restri
             const int max_coef = (pb.n_params - 4 - pb.dim) / (1 + pb.dim);
             const double* coefs = reinterpret_cast<const double*>(prog_area + pb.aux_off);
             const unsigned int* words = reinterpret_cast<const unsigned int*>(prog_area + pb.aux_off + max_coef);
-            for (int i = tid; i < ncoef; i += kThreads) ex.coefs[i] = coefs[i];
+            for (int i = tid; i <= ncoef && i < kSecMaxCoef; i += kThreads) ex.coefs[i] = i < ncoef ? coefs[i] : 0.0;
             for (int i = tid; i < nwords; i += kThreads) ex.words[i] = words[i];
-            if (tid < QMC_MAX_DIM) ex.nu[tid] = a.nu[tid];
             if (tid == 32) {
                 ex.c0[0] = a.sec_c0[0]; ex.c0[1] = a.sec_c0[1];
-                ex.nwords = nwords; ex.ncoef = ncoef;
                 ex.a = a.sec_a; ex.b = a.sec_b;
+                unsigned long long nup = 0;
+                for (int j = 0; j < 16; ++j) nup |= (unsigned long long)(a.nu[j] & 15) << (4 * j);
+                ex.nu_packed = nup;
             }
             __syncthreads();
         }
-        run_tile<SectorEval<DP, G, WIDE>, DP, G, WIDE>(sm, ex, tile_local, partials);
+        run_tile<SectorEval<DP, G, WIDE>, DP, G, WIDE>(sm, sbase, exbase, tile_local, partials);
     }
 }
 
