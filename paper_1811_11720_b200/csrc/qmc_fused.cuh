@@ -34,19 +34,20 @@ template <> struct FamTraits<QMC_FAMILY_CEXP_POLY> { static constexpr int NC = 2
 // Shared-memory image of the problem a CTA is working on.  The double arrays at the front are the
 // operands of the inner loop; they are read with ld.shared at sbase + compile-time offsets.
 template <int DP, int G> struct alignas(16) SmemCtx {
-    double delta[DP * G];          // [j][q]  shifts of the current group (1/2 in padded slots)
+    double delta[(DP * G > kDeltaCache) ? DP * G : kDeltaCache];   // [group][j][q] shifts (1/2 in padded slots): all groups of
+                                   // the problem when they fit, else only the current group
     double fam[DP * 2];            // [j] = (fam_a, fam_b)
     double fit[DP * 6];            // [j] = (a4, a5, a6, 2 a5, 3 a6, -)  cubic map of Eq. 19
     double kor[8];                 // centred Korobov polynomial g_r
     unsigned long long step[DP], back[DP], z[DP];
-    double red[kWarps][G * 2];
+    double red[2][kWarps][G * 2];  // double-buffered by group parity
     DevProblem prob;
     double fam0;
     long long tile;                // popped tile index
 };
 template <int DP, int G> struct SmemOff {
     static constexpr unsigned delta = 0;
-    static constexpr unsigned fam = delta + DP * G * 8;
+    static constexpr unsigned fam = delta + ((DP * G > kDeltaCache) ? DP * G : kDeltaCache) * 8;
     static constexpr unsigned fit = fam + DP * 2 * 8;
     static constexpr unsigned kor = fit + DP * 6 * 8;
     static constexpr unsigned step = kor + 8 * 8;
@@ -134,7 +135,7 @@ template <int TR, bool FIT> __device__ __forceinline__ double point_weight(doubl
 
 // operands of dimension slot j: family constants, fit constants, the G shifts of the group
 template <int DP, int G, bool FIT>
-__device__ __forceinline__ void load_slot(unsigned sbase, int j, double& fa, double& fb, FitC& fc, double (&dl)[G]) {
+__device__ __forceinline__ void load_slot(unsigned sbase, unsigned delta, int j, double& fa, double& fb, FitC& fc, double (&dl)[G]) {
     typedef SmemOff<DP, G> O;
     lds_f64x2(sbase + O::fam + 16u * j, fa, fb);
     if (FIT) {
@@ -144,16 +145,17 @@ __device__ __forceinline__ void load_slot(unsigned sbase, int j, double& fa, dou
     }
     if (G % 2 == 0) {
 #pragma unroll
-        for (int q = 0; q < G; q += 2) lds_f64x2(sbase + O::delta + 8u * (j * G + q), dl[q], dl[q + 1 < G ? q + 1 : q]);
+        for (int q = 0; q < G; q += 2) lds_f64x2(delta + 8u * (j * G + q), dl[q], dl[q + 1 < G ? q + 1 : q]);
     } else {
 #pragma unroll
-        for (int q = 0; q < G; ++q) dl[q] = lds_f64(sbase + O::delta + 8u * (j * G + q));
+        for (int q = 0; q < G; ++q) dl[q] = lds_f64(delta + 8u * (j * G + q));
     }
 }
 
 // ---- one lattice index, G shifts: S2-S6 for the closed-form families --------------------------
 struct EvalCtx {            // per-tile constants held in registers
     unsigned sbase;         // shared address of the CTA's SmemCtx
+    unsigned delta;         // shared address of the current group's shifts
     double inv_n, wconst, fam0;
     int kor_r;
     int sel;                // tr_kind * 2 + has_fit
@@ -170,7 +172,7 @@ __device__ __forceinline__ void eval_point_group(const typename Res<WIDE>::T (&r
         const double rd = Res<WIDE>::to_double(r[j]);
         double fa, fb, dl[G];
         FitC fc;
-        load_slot<DP, G, FIT>(cx.sbase, j, fa, fb, fc, dl);
+        load_slot<DP, G, FIT>(cx.sbase, cx.delta, j, fa, fb, fc, dl);
 #pragma unroll
         for (int q = 0; q < G; ++q) {
             const double x = point_coord<TR, FIT>(rd, cx.inv_n, dl[q], fc, cx.sbase + SmemOff<DP, G>::kor, cx.kor_r, P[q], D[q]);
@@ -197,7 +199,7 @@ template <int FAMILY, int DP, int G, bool WIDE, int TR, bool FIT> struct ClosedE
 // ---- one tile: residue walk (S1), G shifts per index (EV::eval = S2-S6), tile reduction (S7) ----
 template <class EV, int DP, int G, bool WIDE>
 __device__ __forceinline__ void run_tile(SmemCtx<DP, G>& sm, unsigned sbase, const typename EV::Extra& ex, long long tile_local,
-                                         double* __restrict__ partials) {
+                                         bool changed, double* __restrict__ partials) {
     typedef typename Res<WIDE>::T RT;
     constexpr int NC = EV::NC;
     // residue strides live in registers while they are few; otherwise they are re-read from shared memory
@@ -213,7 +215,7 @@ __device__ __forceinline__ void run_tile(SmemCtx<DP, G>& sm, unsigned sbase, con
     typedef SmemOff<DP, G> Off;
     static_assert(offsetof(Ctx, fam) == Off::fam && offsetof(Ctx, fit) == Off::fit && offsetof(Ctx, kor) == Off::kor &&
                   offsetof(Ctx, step) == Off::step, "SmemOff must mirror SmemCtx");
-    const unsigned long long tile_len = (unsigned long long)steps * kThreads;
+    const unsigned long long tile_len = (unsigned long long)pb.tile_len;
     const unsigned long long k0 = (unsigned long long)tile_local * tile_len;
     const unsigned long long kend = (k0 + tile_len < n) ? k0 + tile_len : n;
     const unsigned long long kfirst = k0 + tid;
@@ -226,15 +228,29 @@ __device__ __forceinline__ void run_tile(SmemCtx<DP, G>& sm, unsigned sbase, con
         if (STEP_IN_REGS) stp[j] = (RT)sm.step[j];
     }
 
-#pragma unroll 1
-    for (int g0 = 0; g0 < m; g0 += G) {
-        const int gcount = (m - g0 < G) ? (m - g0) : G;
-        __syncthreads();                                    // previous group's readers of delta/red are done
-        for (int e = tid; e < G * DP; e += kThreads) {
-            const int j = e / G, q = e - j * G;
-            sm.delta[e] = (q < gcount && j < dim) ? pb.shifts[(size_t)(g0 + q) * dim + j] : 0.5;
+    // shifts: staged once per problem for all groups when they fit the shared-memory cache, else per group
+    const int ngroups = (m + G - 1) / G;
+    const bool cached = ngroups * (DP * G) <= (int)(sizeof(sm.delta) / sizeof(double));
+    if (cached && changed) {
+        for (int e = tid; e < ngroups * G * DP; e += kThreads) {
+            const int g = e / (G * DP), rest = e - g * (G * DP), j = rest / G, s = g * G + (rest - j * G);
+            sm.delta[e] = (s < m && j < dim) ? pb.shifts[(size_t)s * dim + j] : 0.5;
         }
         __syncthreads();
+    }
+
+#pragma unroll 1
+    for (int g0 = 0, gi = 0; g0 < m; g0 += G, ++gi) {
+        const int gcount = (m - g0 < G) ? (m - g0) : G;
+        if (!cached) {
+            __syncthreads();                                // previous group's readers of delta are done
+            for (int e = tid; e < G * DP; e += kThreads) {
+                const int j = e / G, q = e - j * G;
+                sm.delta[e] = (q < gcount && j < dim) ? pb.shifts[(size_t)(g0 + q) * dim + j] : 0.5;
+            }
+            __syncthreads();
+        }
+        cx.delta = sbase + SmemOff<DP, G>::delta + (cached ? 8u * (unsigned)(gi * (G * DP)) : 0u);
 
         double acc[G][NC];
 #pragma unroll
@@ -249,12 +265,16 @@ __device__ __forceinline__ void run_tile(SmemCtx<DP, G>& sm, unsigned sbase, con
             for (int j = 0; j < DP; ++j)
                 r[j] = add_mod<RT>(r[j], STEP_IN_REGS ? stp[STEP_IN_REGS ? j : 0] : (RT)lds_u64(sbase + SmemOff<DP, G>::step + 8u * j), (RT)n);
         }
-        // rewind to the thread's first index for the next group: live_steps * kThreads * z_j, via the full-tile rewind
-        // when the thread walked the whole tile, else by recomputing the first residue
+        // rewind to the thread's first index for the next group: back = steps * kThreads * z_j rewinds a full walk; a
+        // thread one index short (ragged tile length) takes one step forward after it; anything else recomputes
         if (g0 + G < m) {
-            if (live_steps == steps) {
+            if (live_steps + 1 >= steps) {
 #pragma unroll
-                for (int j = 0; j < DP; ++j) r[j] = sub_mod<RT>(r[j], (RT)sm.back[j], (RT)n);
+                for (int j = 0; j < DP; ++j) {
+                    RT v = sub_mod<RT>(r[j], (RT)sm.back[j], (RT)n);
+                    if (live_steps != steps) v = add_mod<RT>(v, (RT)sm.step[j], (RT)n);
+                    r[j] = v;
+                }
             } else {
 #pragma unroll
                 for (int j = 0; j < DP; ++j) r[j] = (RT)mulmod_u64(kfirst % n, sm.z[j], n);
@@ -267,15 +287,15 @@ __device__ __forceinline__ void run_tile(SmemCtx<DP, G>& sm, unsigned sbase, con
 #pragma unroll
             for (int c = 0; c < NC; ++c) {
                 const double v = warp_sum(acc[q][c]);
-                if (lane == 0) sm.red[warp][q * NC + c] = v;
+                if (lane == 0) sm.red[gi & 1][warp][q * NC + c] = v;
             }
-        __syncthreads();
+        __syncthreads();                                    // one barrier per group: red is double-buffered by group parity
         if (tid < G * NC) {
             const int q = tid / NC, c = tid - q * NC;
             if (q < gcount) {
-                double v = sm.red[0][tid];
+                double v = sm.red[gi & 1][0][tid];
 #pragma unroll
-                for (int w = 1; w < kWarps; ++w) v += sm.red[w][tid];
+                for (int w = 1; w < kWarps; ++w) v += sm.red[gi & 1][w][tid];
                 partials[pb.partial_off + ((long long)(g0 + q) * NC + c) * pb.tiles + tile_local] = v;
             }
         }
@@ -323,7 +343,7 @@ __device__ __forceinline__ bool next_tile(SmemCtx<DP, G>& sm, const DevProblem* 
 }
 
 // resident CTAs per SM the register budget is sized for (128 / 168 / 255 registers per thread)
-template <int DP, bool WIDE> struct MinBlocks { static constexpr int value = (DP <= 8) ? 4 : (DP <= 16 ? (WIDE ? 2 : 3) : 2); };
+template <int DP, bool WIDE> struct MinBlocks { static constexpr int value = min_blocks_closed(DP, WIDE); };
 
 template <int FAMILY, int DP, int G, bool WIDE>
 __global__ void __launch_bounds__(kThreads, MinBlocks<DP, WIDE>::value) fused_kernel(const DevProblem* __restrict__ probs,
@@ -339,7 +359,7 @@ __global__ void __launch_bounds__(kThreads, MinBlocks<DP, WIDE>::value) fused_ke
         const int sel = sm.prob.tr_kind * 2 + (sm.prob.has_fit ? 1 : 0);
         switch (sel) {
 #define QMC_CASE(TRK, FITB) \
-    case TRK * 2 + (FITB ? 1 : 0): run_tile<ClosedEval<FAMILY, DP, G, WIDE, TRK, FITB>, DP, G, WIDE>(sm, sbase, ex, tile_local, partials); break;
+    case TRK * 2 + (FITB ? 1 : 0): run_tile<ClosedEval<FAMILY, DP, G, WIDE, TRK, FITB>, DP, G, WIDE>(sm, sbase, ex, tile_local, changed, partials); break;
             QMC_CASE(TR_NONE, false) QMC_CASE(TR_NONE, true) QMC_CASE(TR_BAKER, false) QMC_CASE(TR_BAKER, true)
             QMC_CASE(TR_KOR3, false) QMC_CASE(TR_KOR3, true) QMC_CASE(TR_KORR, false) QMC_CASE(TR_KORR, true)
 #undef QMC_CASE

@@ -88,7 +88,7 @@ int tiles_target() {
     static const int v = [] {
         const char* e = std::getenv("QMC_TILES_TARGET");
         const int t = e ? std::atoi(e) : 0;
-        return t > 0 ? t : kTilesTarget;
+        return t > 0 ? t : 0;
     }();
     return v;
 }
@@ -120,8 +120,7 @@ struct Plan {
 int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan* plan) {
     if (count < 1 || !problems) return count < 1 ? QMC_ERR_N : QMC_ERR_NULL;
     plan->dev.resize(count);
-    const int per_problem_target = std::max(16, tiles_target() / count);
-    long long partial_off = 0, means_off = 0;
+    long long means_off = 0;
     size_t prog_off = 0;
     for (int i = 0; i < count; ++i) {
         const qmc_problem& p = problems[i];
@@ -148,24 +147,14 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
             // padded dimension slots contribute u(1-u) = 1/4 each to the weight product (qmc_fused.cuh): exact compensation
             d.wconst = std::ldexp(d.wconst, 2 * r * (dim_slots(p.family, p.dim) - p.dim));
         }
-        const unsigned long long per = (unsigned long long)kThreads * (unsigned long long)per_problem_target;
-        unsigned long long steps = (p.n + per - 1) / per;
-        steps = std::min<unsigned long long>(std::max<unsigned long long>(steps, 1), kMaxSteps);
-        const unsigned long long tile_len = steps * kThreads;
-        const unsigned long long tiles = (p.n + tile_len - 1) / tile_len;
-        if (tiles > 0x7fffffffull) return QMC_ERR_N;
-        d.steps = (int)steps;
-        d.tiles = (int)tiles;
-        d.partial_off = partial_off;
-        d.means_off = means_off;
-        partial_off += (long long)tiles * p.m * d.ncomp;
-        means_off += (long long)p.m * d.ncomp;
         if (p.family == QMC_FAMILY_SECTOR) {
             const int nmono = (p.n_params - 4 - p.dim) / (1 + p.dim);
             d.aux_off = (int)prog_off;
             d.aux_len = 3 * nmono + 1;                                  // coefs + 16 one-byte steps per monomial + end-of-U / padding
             prog_off += (size_t)d.aux_len;
         }
+        d.means_off = means_off;
+        means_off += (long long)p.m * d.ncomp;
         plan->max_m = std::max(plan->max_m, p.m);
         plan->dev[i] = d;
     }
@@ -181,11 +170,37 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
         v->plist.push_back(i);
     }
     if (plan->variants.size() > 64) return QMC_ERR_WORKSPACE;
+    // tiling (S9): per kernel variant aim at kWaves x (resident CTAs of a B200) tiles, shared among the variant's problems
+    // in proportion to their cost; a tile is at least one index per thread and at most kMaxSteps (bounds the fp64 chains)
+    for (auto& v : plan->variants) {
+        const int resident = kPlanSMs * (v.family == QMC_FAMILY_SECTOR ? min_blocks_sector(v.dp) : min_blocks_closed(v.dp, v.wide));
+        const int env = tiles_target();
+        const double target = env > 0 ? env : resident * (v.plist.size() == 1 ? kWavesSingle : kWavesBatch);
+        double total_cost = 0.0;
+        for (int i : v.plist) total_cost += (double)plan->dev[i].n * plan->dev[i].m * (12.0 * plan->dev[i].dim + 0.5 * plan->dev[i].n_params + 40.0);
+        for (int i : v.plist) {
+            DevProblem& d = plan->dev[i];
+            const double cost = (double)d.n * d.m * (12.0 * d.dim + 0.5 * d.n_params + 40.0);
+            const double want = std::max(1.0, std::floor(target * cost / total_cost));
+            unsigned long long tile_len = (unsigned long long)std::ceil((double)d.n / want);
+            tile_len = std::min<unsigned long long>(std::max<unsigned long long>(tile_len, kThreads), (unsigned long long)kMaxSteps * kThreads);
+            const unsigned long long tiles = (d.n + tile_len - 1) / tile_len;
+            if (tiles > 0x7fffffffull) return QMC_ERR_N;
+            d.tile_len = (long long)tile_len;
+            d.steps = (int)((tile_len + kThreads - 1) / kThreads);
+            d.tiles = (int)tiles;
+        }
+    }
+    long long partial_off = 0;
+    for (int i = 0; i < count; ++i) {
+        plan->dev[i].partial_off = partial_off;
+        partial_off += (long long)plan->dev[i].tiles * plan->dev[i].m * plan->dev[i].ncomp;
+    }
     for (auto& v : plan->variants) {
         // most expensive tiles first (S9); cost ~ indices x shifts x (dimension work + integrand size)
         auto cost = [&](int i) {
             const DevProblem& d = plan->dev[i];
-            return (double)d.steps * d.m * (12.0 * d.dim + 0.5 * d.n_params + 40.0);
+            return (double)d.tile_len * d.m * (12.0 * d.dim + 0.5 * d.n_params + 40.0);
         };
         std::stable_sort(v.plist.begin(), v.plist.end(), [&](int a, int b) { return cost(a) > cost(b); });
         for (int i : v.plist) { plan->dev[i].tile_begin = v.total_tiles; v.total_tiles += plan->dev[i].tiles; }
@@ -417,7 +432,7 @@ int qmc_plan_info(int count, const qmc_problem* problems, long long* out_tiles, 
     const int st = make_plan(count, problems, true, &plan);
     if (st != QMC_OK) return st;
     if (out_tiles) *out_tiles = plan.total_tiles;
-    if (out_tile_len0) *out_tile_len0 = (long long)plan.dev[0].steps * kThreads;
+    if (out_tile_len0) *out_tile_len0 = plan.dev[0].tile_len;
     if (out_ctas) {
         int ctas = 0;
         const int sms = sm_count();

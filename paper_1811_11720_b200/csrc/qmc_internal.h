@@ -12,7 +12,16 @@ constexpr int kThreads = 128;          // threads per CTA of the fused kernels (
 constexpr int kWarps = kThreads / 32;
 constexpr int kGroup = 4;             // shifts evaluated together per lattice index (register-resident)
 constexpr int kMaxSteps = 1024;        // max lattice indices per thread per tile (bounds the naive fp64 chain length)
-constexpr int kTilesTarget = 2368;     // tiles aimed at per launch: 148 SMs x 4 resident CTAs x 4 waves
+constexpr int kPlanSMs = 148;          // the tiling is planned for a B200 (a pure function of the problem structs: results
+                                       // are bit-identical on any device, only the balance is tuned for 148 SMs)
+constexpr int kWavesSingle = 2;        // tiles per resident CTA when a kernel variant serves one problem (equal-cost tiles)
+constexpr int kWavesBatch = 8;         // ... and when it serves a batch of unequal problems (dynamic balance)
+
+// resident CTAs per SM each fused kernel is register-budgeted for (its __launch_bounds__ minimum)
+constexpr int min_blocks_closed(int dp, bool wide) { return dp <= 8 ? 4 : (dp <= 16 ? (wide ? 2 : 3) : 2); }
+constexpr int sector_group(int dp) { return dp <= 8 ? 8 : 4; }                       // shifts per group, sector family
+constexpr int min_blocks_sector(int dp) { return dp <= 6 ? 3 : 2; }
+constexpr int kDeltaCache = 768;       // doubles of shared memory per CTA that cache the shifts of all groups of a problem
 constexpr int kMaxSectorOps = 1024;    // interpreter program length limit per polynomial
 constexpr int kMaxSectorMono = 64;
 
@@ -32,6 +41,7 @@ struct alignas(16) DevProblem {
     long long partial_off;     // offset in doubles into the partial-sum area
     long long means_off;       // offset in doubles into the per-shift means area
     long long tile_begin;      // first tile index (within this problem's kernel variant queue)
+    long long tile_len;        // lattice indices per tile (the last tile is shorter); steps = ceil(tile_len / kThreads)
     int tiles;                 // number of k-tiles
     int steps;                 // I: lattice indices per thread per tile; tile length = steps*kThreads
     int family, dim, m, ncomp;

@@ -136,7 +136,7 @@ __device__ __forceinline__ void sector_coords(const typename Res<WIDE>::T (&r)[D
         const double rd = Res<WIDE>::to_double(r[j]);
         double fa, fb, dl[G];
         FitC fc;
-        load_slot<DP, G, FIT>(cx.sbase, j, fa, fb, fc, dl);
+        load_slot<DP, G, FIT>(cx.sbase, cx.delta, j, fa, fb, fc, dl);
 #pragma unroll
         for (int q = 0; q < G; ++q)
             x[q][j] = point_coord<TR, FIT>(rd, cx.inv_n, dl[q], fc, cx.sbase + SmemOff<DP, G>::kor, cx.kor_r, P[q], D[q]);
@@ -196,8 +196,8 @@ template <int DP, int G, bool WIDE> struct SectorEval {
 };
 
 // shifts per group and resident CTAs per SM by dimension-slot count (x[G][DP] lives in registers)
-template <int DP> struct SectorGroup { static constexpr int value = (DP <= 8) ? 8 : 4; };
-template <int DP, int G> struct SectorMinBlocks { static constexpr int value = (G * DP > 32 || G >= 8) ? 2 : 3; };
+template <int DP> struct SectorGroup { static constexpr int value = sector_group(DP); };
+template <int DP, int G> struct SectorMinBlocks { static constexpr int value = min_blocks_sector(DP); };
 
 template <int DP, int G, bool WIDE>
 __global__ void __launch_bounds__(kThreads, SectorMinBlocks<DP, G>::value)
@@ -229,7 +229,7 @@ fused_sector_kernel(const DevProblem* __restrict__ probs, const DevAux* __restri
             }
             __syncthreads();
         }
-        run_tile<SectorEval<DP, G, WIDE>, DP, G, WIDE>(sm, sbase, exbase, tile_local, partials);
+        run_tile<SectorEval<DP, G, WIDE>, DP, G, WIDE>(sm, sbase, exbase, tile_local, changed, partials);
     }
 }
 
