@@ -43,10 +43,14 @@ int ncomp_of(int family) {
     return -1;
 }
 
-int dim_slots(int family, int dim) {
-    if (family == QMC_FAMILY_SECTOR) return dim <= 4 ? 4 : (dim <= 6 ? 6 : (dim <= 8 ? 8 : (dim <= 16 ? 16 : -1)));
-    return dim <= 4 ? 4 : (dim <= 8 ? 8 : (dim <= 16 ? 16 : 32));
+// dimension slots of the kernel variant that serves (family, dim, residue width); slots beyond dim are padded
+int dim_slots(int family, int dim, bool wide) {
+    if (family == QMC_FAMILY_SECTOR) return dim <= 4 ? 4 : (dim <= 6 ? 6 : (dim <= 8 ? 8 : (dim <= 16 ? 16 : -1)));   // = sector_dim_slots (qmc_sector.cuh)
+    if (wide) return dim <= 8 ? 8 : (dim <= 16 ? 16 : 32);
+    return dim <= 4 ? 4 : (dim <= 6 ? 6 : (dim <= 8 ? 8 : (dim <= 12 ? 12 : (dim <= 16 ? 16 : 32))));
 }
+bool force_wide();
+bool is_wide(unsigned long long n) { return n >= (1ull << 31) || force_wide(); }
 
 bool decode_transform(int transform, int* kind, int* r) {
     if (transform == QMC_TRANSFORM_NONE) { *kind = TR_NONE; *r = 0; return true; }
@@ -69,7 +73,7 @@ double binom(int a, int b) {
 int validate_struct(const qmc_problem& p, bool need_two_shifts) {
     if (ncomp_of(p.family) < 0) return QMC_ERR_FAMILY;
     if (p.dim < 1 || p.dim > QMC_MAX_DIM) return QMC_ERR_DIM;
-    if (dim_slots(p.family, p.dim) < 0) return QMC_ERR_DIM;
+    if (dim_slots(p.family, p.dim, false) < 0) return QMC_ERR_DIM;
     if (p.n < 2 || p.n >= (1ull << 53)) return QMC_ERR_N;
     if (p.m < (need_two_shifts ? 2 : 1) || p.m > QMC_MAX_M) return QMC_ERR_M;
     int kind, r;
@@ -145,7 +149,7 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
                 d.kor[k] = cr * binom(r, k) * std::ldexp(1.0, 2 * (k - r)) * ((k & 1) ? -1.0 : 1.0) / (double)(2 * k + 1);
             for (int j = 0; j < p.dim; ++j) d.wconst *= cr;
             // padded dimension slots contribute u(1-u) = 1/4 each to the weight product (qmc_fused.cuh): exact compensation
-            d.wconst = std::ldexp(d.wconst, 2 * r * (dim_slots(p.family, p.dim) - p.dim));
+            d.wconst = std::ldexp(d.wconst, 2 * r * (dim_slots(p.family, p.dim, is_wide(p.n)) - p.dim));
         }
         if (p.family == QMC_FAMILY_SECTOR) {
             const int nmono = (p.n_params - 4 - p.dim) / (1 + p.dim);
@@ -161,8 +165,8 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
     // kernel variants
     for (int i = 0; i < count; ++i) {
         const DevProblem& d = plan->dev[i];
-        const int dp = dim_slots(d.family, d.dim);
-        const bool wide = d.n >= (1ull << 31) || force_wide();
+        const bool wide = is_wide(d.n);
+        const int dp = dim_slots(d.family, d.dim, wide);
         Variant* v = nullptr;
         for (auto& c : plan->variants)
             if (c.family == d.family && c.dp == dp && c.wide == wide) v = &c;

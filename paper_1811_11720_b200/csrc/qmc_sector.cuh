@@ -58,6 +58,16 @@ __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned 
     const bool pairs = sector_has_pairs(dp);
     const double* p = pb.params;
     int status = 0;
+    // A rejected parameter block must still leave a program the interpreter can run to its end (the problem's
+    // results are then replaced by NaN in the finalize stage): end-of-U, end, read-ahead padding.
+    {
+        const int slots = (pb.n_params - 4 - d) / (1 + d);
+        unsigned char* stub = reinterpret_cast<unsigned char*>(prog_area + pb.aux_off + slots);
+        stub[0] = (unsigned char)SEC_ENDU; stub[1] = (unsigned char)SEC_END;
+        for (int i = 2; i < 8; ++i) stub[i] = (unsigned char)SEC_NOP;
+        a.sec_nops[0] = 2; a.sec_nops[1] = 0; a.sec_ncoef[0] = 0; a.sec_ncoef[1] = 0;
+        a.sec_c0[0] = a.sec_c0[1] = 1.0;
+    }
     const double av = p[0], bv = p[1], nUv = p[2], nFv = p[3];
     if (!(av >= 0.0 && av <= 8.0 && bv >= 0.0 && bv <= 8.0 && nUv >= 1.0 && nUv <= kMaxSectorMono && nFv >= 1.0 &&
           nFv <= kMaxSectorMono) ||
@@ -114,10 +124,14 @@ __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned 
         base += cnt[pol] * (1 + d);
     }
     if (!status) while (nops & 3) ops[nops++] = (unsigned char)SEC_NOP;
-    a.sec_nops[0] = status ? 0 : nops / 4;
-    a.sec_nops[1] = 0;
-    a.sec_ncoef[0] = status ? 0 : ncoef;
-    a.sec_ncoef[1] = 0;
+    if (!status) {
+        a.sec_nops[0] = nops / 4;
+        a.sec_ncoef[0] = ncoef;
+    } else {                                           // restore the stub (the loop above may have overwritten it)
+        ops[0] = (unsigned char)SEC_ENDU; ops[1] = (unsigned char)SEC_END;
+        for (int i = 2; i < 8; ++i) ops[i] = (unsigned char)SEC_NOP;
+        a.sec_c0[0] = a.sec_c0[1] = 1.0;
+    }
     a.status = status;
 }
 

@@ -137,11 +137,11 @@ def test_means_all_transforms(fam, tr):
     check_against_oracle(probs)
 
 
-@pytest.mark.parametrize("fam,d", [(0, 1), (0, 4), (0, 9), (0, 16), (0, 17), (0, 32), (1, 2), (1, 8), (1, 13), (1, 24),
-                                   (2, 1), (2, 4), (2, 12), (2, 16), (2, 29), (3, 1), (3, 3), (3, 6), (3, 8), (3, 11),
-                                   (3, 16)])
+@pytest.mark.parametrize("fam,d", [(0, 1), (0, 4), (0, 6), (0, 9), (0, 12), (0, 16), (0, 17), (0, 32), (1, 2), (1, 5), (1, 8),
+                                   (1, 11), (1, 13), (1, 24), (2, 1), (2, 4), (2, 6), (2, 10), (2, 12), (2, 16), (2, 29),
+                                   (3, 1), (3, 3), (3, 5), (3, 6), (3, 8), (3, 11), (3, 16)])
 def test_means_all_dimension_slots(fam, d):
-    """every register-slot count (4, 8, 16, 32) and ragged dims inside a slot count; several tiles + ragged tail"""
+    """every register-slot count (4, 6, 8, 12, 16, 32) and dims that leave padded slots; several tiles + ragged tail"""
     n = 65537 if d <= 16 else 8191
     tr = K + 3 if fam != 1 else BAKER
     a_hi = 1.0 if d <= 16 else 0.3
