@@ -302,40 +302,104 @@ __device__ __forceinline__ void run_tile(SmemCtx<DP, G>& sm, unsigned sbase, con
     }
 }
 
-// ---- queue handling shared by all fused kernels ------------------------------------------------
-// Pops the next tile; returns false when the queue is empty.  On a problem change the CTA reloads
-// its shared-memory image of the problem (changed = true).  `cur` = problem index loaded (-1: none).
-template <int DP, int G>
-__device__ __forceinline__ bool next_tile(SmemCtx<DP, G>& sm, const DevProblem* __restrict__ probs,
-                                          const DevAux* __restrict__ aux, const VariantQueue& vq, int& cur,
-                                          long long& tile_local, bool& changed) {
+// ---- S0: per-slot constants of a problem, derived from the caller's arrays ------------------------
+// z mod n, the residue stride between a thread's points (kThreads z_j mod n), the rewind of a full walk, the family
+// constants and the cubic-map constants of dimension slot j.  Slots j >= dim get the padding values (file header).
+struct SlotConst {
+    unsigned long long z, step, back;
+    double fa, fb, f[5];
+};
+__device__ __forceinline__ SlotConst derive_slot(const DevProblem& pb, int j) {
+    SlotConst s;
+    s.z = 0; s.step = 0; s.back = 0; s.fa = 0.0; s.fb = 0.0;
+    s.f[0] = 1.0; s.f[1] = s.f[2] = s.f[3] = s.f[4] = 0.0;
+    const int d = pb.dim;
+    const unsigned long long n = pb.n;
+    if (j < d) {
+        s.z = pb.z[j] % n;
+        s.step = mulmod_u64((unsigned long long)kThreads % n, s.z, n);
+        s.back = mulmod_u64(((unsigned long long)pb.steps * kThreads) % n, s.z, n);
+        const double* p = pb.params;
+        if (pb.family == QMC_FAMILY_GENZ_OSC) { s.fa = p[1 + j]; }
+        else if (pb.family == QMC_FAMILY_GENZ_PRODPEAK) { const double c = p[j]; s.fa = __ddiv_rn(1.0, __dmul_rn(c, c)); s.fb = p[d + j]; }
+        else if (pb.family == QMC_FAMILY_CEXP_POLY) { s.fa = p[j]; s.fb = p[d + j]; }
+        if (pb.has_fit) {
+            const double* c = pb.fit + 6 * j;
+            const double a4 = c[4], a5 = c[5];
+            const double a6 = __dadd_rn(__dadd_rn(__dadd_rn(__dadd_rn(1.0, -c[2]), -c[3]), -a4), -a5);
+            s.f[0] = a4; s.f[1] = a5; s.f[2] = a6; s.f[3] = 2.0 * a5; s.f[4] = 3.0 * a6;
+        }
+    } else if (pb.family == QMC_FAMILY_GENZ_PRODPEAK) {
+        // padded slot: the coordinate is pinned to u = 1/2, i.e. x = 1 (baker) or 1/2; factor (x - fb)^2 + fa = 1
+        s.fa = 1.0;
+        s.fb = (pb.tr_kind == TR_BAKER) ? 1.0 : 0.5;
+    }
+    return s;
+}
+__device__ __forceinline__ double derive_fam0(const DevProblem& pb) {
+    return (pb.family == QMC_FAMILY_GENZ_OSC) ? __dmul_rn(6.283185307179586476925286766559, pb.params[0]) : 0.0;
+}
+
+// ---- tile source shared by all fused kernels ---------------------------------------------------
+// Next tile of this CTA; returns false when there is none.  On a problem change the CTA rebuilds its
+// shared-memory image of the problem (changed = true): closed-form families derive the slot constants
+// themselves (S0), the sector family reads what prepare_kernel left in DevAux.
+// `cur` = problem index loaded (-1: none), `iter` = tiles this CTA has taken (single mode).
+template <int DP, int G, bool SECTOR>
+__device__ __forceinline__ bool next_tile(SmemCtx<DP, G>& sm, const FusedLaunch& L, int& cur, int& iter, long long& tile_local,
+                                          bool& changed) {
     const int tid = threadIdx.x;
     changed = false;
     __syncthreads();                                        // everyone is done with the previous tile
-    if (tid == 0) sm.tile = (long long)atomicAdd(vq.counter, 1ull);
-    __syncthreads();
-    const long long tile = sm.tile;
-    if (tile >= vq.total_tiles) return false;
-    int lo = 0, hi = vq.plist_len;                          // largest lo with tile_prefix[lo] <= tile
-    while (hi - lo > 1) {
-        const int mid = (lo + hi) >> 1;
-        if (__ldg(&vq.tile_prefix[mid]) <= tile) lo = mid; else hi = mid;
+    int pidx = 0;
+    if (L.single && L.vq.counter == nullptr) {              // at most one tile per CTA: no queue needed
+        tile_local = (long long)blockIdx.x + (long long)iter * gridDim.x;
+        ++iter;
+        if (tile_local >= L.one.tiles) return false;
+    } else if (L.single) {
+        if (tid == 0) sm.tile = (long long)atomicAdd(L.vq.counter, 1ull);
+        __syncthreads();
+        tile_local = sm.tile;
+        if (tile_local >= L.one.tiles) return false;
+    } else {
+        if (tid == 0) sm.tile = (long long)atomicAdd(L.vq.counter, 1ull);
+        __syncthreads();
+        const long long tile = sm.tile;
+        if (tile >= L.vq.total_tiles) return false;
+        int lo = 0, hi = L.vq.plist_len;                    // largest lo with tile_prefix[lo] <= tile
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (__ldg(&L.vq.tile_prefix[mid]) <= tile) lo = mid; else hi = mid;
+        }
+        tile_local = tile - __ldg(&L.vq.tile_prefix[lo]);
+        pidx = __ldg(&L.vq.plist[lo]);
     }
-    tile_local = tile - __ldg(&vq.tile_prefix[lo]);
-    const int pidx = __ldg(&vq.plist[lo]);
     if (pidx != cur) {
         cur = pidx;
         changed = true;
-        if (tid == 0) sm.prob = probs[pidx];
-        const DevAux& a = aux[pidx];
-        if (tid == 32) sm.fam0 = a.fam0;
-        if (tid >= 64 && tid < 72) sm.kor[tid - 64] = probs[pidx].kor[tid - 64];
-        for (int j = tid; j < DP; j += kThreads) {          // slots j >= dim hold the padding values (prepare_kernel)
-            sm.z[j] = a.z[j]; sm.step[j] = a.step[j]; sm.back[j] = a.back[j];
-            sm.fam[2 * j] = a.fam_a[j]; sm.fam[2 * j + 1] = a.fam_b[j];
+        const DevProblem& src = L.single ? L.one : L.probs[pidx];
+        if (tid == 0) sm.prob = src;
+        if (tid >= 64 && tid < 72) sm.kor[tid - 64] = src.kor[tid - 64];
+        if (SECTOR) {
+            const DevAux& a = L.aux[pidx];
+            if (tid == 32) sm.fam0 = a.fam0;
+            for (int j = tid; j < DP; j += kThreads) {      // slots j >= dim hold the padding values
+                sm.z[j] = a.z[j]; sm.step[j] = a.step[j]; sm.back[j] = a.back[j];
+                sm.fam[2 * j] = a.fam_a[j]; sm.fam[2 * j + 1] = a.fam_b[j];
 #pragma unroll
-            for (int i = 0; i < 5; ++i) sm.fit[6 * j + i] = a.fit[i][j];
-            sm.fit[6 * j + 5] = 0.0;
+                for (int i = 0; i < 5; ++i) sm.fit[6 * j + i] = a.fit[i][j];
+                sm.fit[6 * j + 5] = 0.0;
+            }
+        } else {
+            if (tid == 32) sm.fam0 = derive_fam0(src);
+            for (int j = tid; j < DP; j += kThreads) {
+                const SlotConst s = derive_slot(src, j);
+                sm.z[j] = s.z; sm.step[j] = s.step; sm.back[j] = s.back;
+                sm.fam[2 * j] = s.fa; sm.fam[2 * j + 1] = s.fb;
+#pragma unroll
+                for (int i = 0; i < 5; ++i) sm.fit[6 * j + i] = s.f[i];
+                sm.fit[6 * j + 5] = 0.0;
+            }
         }
         __syncthreads();
     }
@@ -346,20 +410,18 @@ __device__ __forceinline__ bool next_tile(SmemCtx<DP, G>& sm, const DevProblem* 
 template <int DP, bool WIDE> struct MinBlocks { static constexpr int value = min_blocks_closed(DP, WIDE); };
 
 template <int FAMILY, int DP, int G, bool WIDE>
-__global__ void __launch_bounds__(kThreads, MinBlocks<DP, WIDE>::value) fused_kernel(const DevProblem* __restrict__ probs,
-                                                         const DevAux* __restrict__ aux, VariantQueue vq,
-                                                         double* __restrict__ partials) {
+__global__ void __launch_bounds__(kThreads, MinBlocks<DP, WIDE>::value) fused_kernel(const __grid_constant__ FusedLaunch L) {
     __shared__ SmemCtx<DP, G> sm;
     const unsigned sbase = (unsigned)__cvta_generic_to_shared(&sm);
-    int cur = -1;
+    int cur = -1, iter = 0;
     long long tile_local = 0;
     bool changed;
     NoExtra ex;
-    while (next_tile<DP, G>(sm, probs, aux, vq, cur, tile_local, changed)) {
+    while (next_tile<DP, G, false>(sm, L, cur, iter, tile_local, changed)) {
         const int sel = sm.prob.tr_kind * 2 + (sm.prob.has_fit ? 1 : 0);
         switch (sel) {
 #define QMC_CASE(TRK, FITB) \
-    case TRK * 2 + (FITB ? 1 : 0): run_tile<ClosedEval<FAMILY, DP, G, WIDE, TRK, FITB>, DP, G, WIDE>(sm, sbase, ex, tile_local, changed, partials); break;
+    case TRK * 2 + (FITB ? 1 : 0): run_tile<ClosedEval<FAMILY, DP, G, WIDE, TRK, FITB>, DP, G, WIDE>(sm, sbase, ex, tile_local, changed, L.partials); break;
             QMC_CASE(TR_NONE, false) QMC_CASE(TR_NONE, true) QMC_CASE(TR_BAKER, false) QMC_CASE(TR_BAKER, true)
             QMC_CASE(TR_KOR3, false) QMC_CASE(TR_KOR3, true) QMC_CASE(TR_KORR, false) QMC_CASE(TR_KORR, true)
 #undef QMC_CASE
@@ -367,13 +429,5 @@ __global__ void __launch_bounds__(kThreads, MinBlocks<DP, WIDE>::value) fused_ke
         }
     }
 }
-
-// Arguments of every fused kernel; launcher tables are instantiated per family in qmc_fused_f*.cu
-struct FusedArgs {
-    const DevProblem* probs;
-    const DevAux* aux;
-    VariantQueue vq;
-    double* partials;
-};
 
 }  // namespace qmc

@@ -4,9 +4,8 @@
 
 namespace qmc {
 
-template <int DP, bool WIDE> static cudaError_t launch_one(int grid, cudaStream_t st, const FusedArgs& a,
-                                                           const unsigned long long* prog) {
-    fused_sector_kernel<DP, SectorGroup<DP>::value, WIDE><<<grid, kThreads, 0, st>>>(a.probs, a.aux, a.vq, a.partials, prog);
+template <int DP, bool WIDE> static cudaError_t launch_one(int grid, cudaStream_t st, const FusedLaunch& a) {
+    fused_sector_kernel<DP, SectorGroup<DP>::value, WIDE><<<grid, kThreads, 0, st>>>(a);
     return cudaGetLastError();
 }
 template <int DP, bool WIDE> static int occ_one() {
@@ -29,8 +28,8 @@ template <int DP, bool WIDE> static int occ_one() {
         case 16 * 2 + 1: return FN<16, true>(__VA_ARGS__);        \
     }
 
-cudaError_t launch_fused_f3(int dp, bool wide, int grid, cudaStream_t st, const FusedArgs& a, const unsigned long long* prog) {
-    QMC_F3_TABLE(launch_one, grid, st, a, prog)
+cudaError_t launch_fused_f3(int dp, bool wide, int grid, cudaStream_t st, const FusedLaunch& a) {
+    QMC_F3_TABLE(launch_one, grid, st, a)
     return cudaErrorInvalidValue;
 }
 int occupancy_fused_f3(int dp, bool wide) {

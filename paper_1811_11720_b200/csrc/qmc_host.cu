@@ -263,18 +263,33 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
     if (sms <= 0) return cuda_fail(cudaErrorNoDevice, "no CUDA device");
     char* ws = static_cast<char*>(workspace);
 
-    // host image of [probs | plist | prefix]
-    const size_t blob_bytes = plan.off_aux - plan.off_probs;
-    std::vector<char> blob(blob_bytes, 0);
-    std::memcpy(blob.data(), plan.dev.data(), (size_t)count * sizeof(DevProblem));
-    int* plist = reinterpret_cast<int*>(blob.data() + (plan.off_plist - plan.off_probs));
-    long long* prefix = reinterpret_cast<long long*>(blob.data() + (plan.off_prefix - plan.off_probs));
-    std::vector<VariantQueue> queues;
-    {
+    const DevProblem* dprobs = reinterpret_cast<const DevProblem*>(ws + plan.off_probs);
+    DevAux* daux = reinterpret_cast<DevAux*>(ws + plan.off_aux);
+    unsigned long long* dprog = reinterpret_cast<unsigned long long*>(ws + plan.off_prog);
+    double* dmeans = reinterpret_cast<double*>(ws + plan.off_means);
+    double* dpart = reinterpret_cast<double*>(ws + plan.off_partials);
+    bool any_sector = false;
+    for (const DevProblem& d : plan.dev) any_sector = any_sector || d.family == QMC_FAMILY_SECTOR;
+    // single mode: one closed-form problem travels in the kernel parameter; nothing is uploaded, reset or prepared
+    const bool single = count == 1 && !any_sector;
+    FusedLaunch base;
+    std::memset(&base, 0, sizeof(base));
+    base.probs = dprobs; base.aux = daux; base.prog = dprog; base.partials = dpart;
+    base.single = single ? 1 : 0;
+    if (single) base.one = plan.dev[0];
+
+    std::vector<VariantQueue> queues(plan.variants.size());
+    if (!single) {
+        // host image of [queue heads (zero) | probs | plist | prefix]: one upload resets the queues too
+        const size_t blob_bytes = plan.off_aux - plan.off_counters;
+        std::vector<char> blob(blob_bytes, 0);
+        std::memcpy(blob.data() + (plan.off_probs - plan.off_counters), plan.dev.data(), (size_t)count * sizeof(DevProblem));
+        int* plist = reinterpret_cast<int*>(blob.data() + (plan.off_plist - plan.off_counters));
+        long long* prefix = reinterpret_cast<long long*>(blob.data() + (plan.off_prefix - plan.off_counters));
         size_t pl = 0, pf = 0;
         int vi = 0;
         for (auto& v : plan.variants) {
-            VariantQueue q;
+            VariantQueue& q = queues[vi];
             q.plist = reinterpret_cast<const int*>(ws + plan.off_plist) + pl;
             q.tile_prefix = reinterpret_cast<const long long*>(ws + plan.off_prefix) + pf;
             q.plist_len = (int)v.plist.size();
@@ -283,19 +298,23 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
             long long acc = 0;
             for (int i : v.plist) { plist[pl++] = i; prefix[pf++] = acc; acc += plan.dev[i].tiles; }
             prefix[pf++] = acc;
-            queues.push_back(q);
             ++vi;
         }
+        QMC_CUDA(cudaMemcpyAsync(ws + plan.off_counters, blob.data(), blob_bytes, cudaMemcpyHostToDevice, st));
+        if (any_sector) {                                   // S0 for the sector family: tables + device-side program compiler
+            QMC_CUDA(launch_prepare(count, st, dprobs, daux, dprog));
+            ++g_last_launches;
+        }
+    } else {
+        std::memset(&queues[0], 0, sizeof(VariantQueue));
+        queues[0].total_tiles = plan.variants[0].total_tiles;
+        const Variant& v0 = plan.variants[0];
+        if (v0.total_tiles > (long long)sms * std::max(1, occupancy(v0.family, v0.dp, v0.wide))) {
+            // more tiles than resident CTAs: dynamic queue (one 8-byte reset); otherwise every CTA owns one tile
+            queues[0].counter = reinterpret_cast<unsigned long long*>(ws + plan.off_counters);
+            QMC_CUDA(cudaMemsetAsync(queues[0].counter, 0, sizeof(unsigned long long), st));
+        }
     }
-    QMC_CUDA(cudaMemsetAsync(ws + plan.off_counters, 0, 64 * sizeof(unsigned long long), st));
-    QMC_CUDA(cudaMemcpyAsync(ws + plan.off_probs, blob.data(), blob_bytes, cudaMemcpyHostToDevice, st));
-    const DevProblem* dprobs = reinterpret_cast<const DevProblem*>(ws + plan.off_probs);
-    DevAux* daux = reinterpret_cast<DevAux*>(ws + plan.off_aux);
-    unsigned long long* dprog = reinterpret_cast<unsigned long long*>(ws + plan.off_prog);
-    double* dmeans = reinterpret_cast<double*>(ws + plan.off_means);
-    double* dpart = reinterpret_cast<double*>(ws + plan.off_partials);
-    QMC_CUDA(launch_prepare(count, st, dprobs, daux, dprog));
-    ++g_last_launches;
     g_ev_valid = false;
     if (g_profile) {
         if (!g_ev0) { QMC_CUDA(cudaEventCreate(&g_ev0)); QMC_CUDA(cudaEventCreate(&g_ev1)); }
@@ -307,19 +326,20 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
         if (occ <= 0) return cuda_fail(cudaErrorInvalidDeviceFunction, "occupancy query (is the sm_100a image loadable on this device?)");
         const long long cap = (long long)sms * occ;
         const int grid = (int)std::min<long long>(cap, v.total_tiles);
-        FusedArgs a{dprobs, daux, queues[vi], dpart};
+        FusedLaunch a = base;
+        a.vq = queues[vi];
         cudaError_t e = cudaErrorInvalidValue;
         switch (v.family) {
             case 0: e = launch_fused_f0(v.dp, v.wide, grid, st, a); break;
             case 1: e = launch_fused_f1(v.dp, v.wide, grid, st, a); break;
             case 2: e = launch_fused_f2(v.dp, v.wide, grid, st, a); break;
-            case 3: e = launch_fused_f3(v.dp, v.wide, grid, st, a, dprog); break;
+            case 3: e = launch_fused_f3(v.dp, v.wide, grid, st, a); break;
         }
         if (e != cudaSuccess) return cuda_fail(e, "fused kernel launch");
         ++g_last_launches;
     }
     if (g_profile) { QMC_CUDA(cudaEventRecord(g_ev1, st)); g_ev_valid = true; }
-    QMC_CUDA(launch_finalize(count, st, dprobs, daux, dpart, dmeans, out_means, out_errs, out_shift_means, 2 * plan.max_m));
+    QMC_CUDA(launch_finalize(count, st, base, dmeans, out_means, out_errs, out_shift_means, 2 * plan.max_m));
     ++g_last_launches;
     return QMC_OK;
 }

@@ -82,4 +82,19 @@ struct VariantQueue {
     unsigned long long* counter; // DEVICE: tile queue head (zeroed before launch)
 };
 
+// Kernel parameter of every fused kernel and of the finalize kernel (passed by value).  Queue mode: the problems
+// live in the workspace and CTAs pop tiles from vq.counter.  Single mode (one closed-form problem): the problem
+// travels in the parameter itself, so the call needs no workspace upload and no prepare launch; when there are no
+// more tiles than resident CTAs every CTA owns tile blockIdx.x and the queue (vq.counter == nullptr) is not used.  Result slots are per tile in both modes.
+struct FusedLaunch {
+    const DevProblem* probs;
+    const DevAux* aux;                    // sector family only
+    const unsigned long long* prog;       // sector family only
+    double* partials;
+    VariantQueue vq;
+    int single;
+    int pad_;
+    DevProblem one;
+};
+
 }  // namespace qmc

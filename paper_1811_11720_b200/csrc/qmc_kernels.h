@@ -6,7 +6,6 @@
 
 namespace qmc {
 
-struct FusedArgs;
 
 struct PointsArgs {
     unsigned long long n, k0, count;
@@ -22,17 +21,17 @@ struct PointsArgs {
 int report_cuda_error(cudaError_t e, const char* where);
 
 cudaError_t launch_prepare(int count, cudaStream_t st, const DevProblem* probs, DevAux* aux, unsigned long long* prog_area);
-cudaError_t launch_finalize(int count, cudaStream_t st, const DevProblem* probs, const DevAux* aux, const double* partials,
-                            double* means_ws, double* out_means, double* out_errs, double* out_shift_means, int stride);
+cudaError_t launch_finalize(int count, cudaStream_t st, const FusedLaunch& a, double* means_ws, double* out_means, double* out_errs,
+                            double* out_shift_means, int stride);
 cudaError_t launch_finalize_means(cudaStream_t st, const double* means, int m, int nc, double* out_mean, double* out_err);
 cudaError_t launch_points(cudaStream_t st, const PointsArgs& a, int sm_count);
 cudaError_t launch_dfma_probe(cudaStream_t st, double* out, int blocks, int iters);
 
 // fused kernels, one translation unit per family
-cudaError_t launch_fused_f0(int dp, bool wide, int grid, cudaStream_t st, const FusedArgs& a);
-cudaError_t launch_fused_f1(int dp, bool wide, int grid, cudaStream_t st, const FusedArgs& a);
-cudaError_t launch_fused_f2(int dp, bool wide, int grid, cudaStream_t st, const FusedArgs& a);
-cudaError_t launch_fused_f3(int dp, bool wide, int grid, cudaStream_t st, const FusedArgs& a, const unsigned long long* prog);
+cudaError_t launch_fused_f0(int dp, bool wide, int grid, cudaStream_t st, const FusedLaunch& a);
+cudaError_t launch_fused_f1(int dp, bool wide, int grid, cudaStream_t st, const FusedLaunch& a);
+cudaError_t launch_fused_f2(int dp, bool wide, int grid, cudaStream_t st, const FusedLaunch& a);
+cudaError_t launch_fused_f3(int dp, bool wide, int grid, cudaStream_t st, const FusedLaunch& a);
 int occupancy_fused_f0(int dp, bool wide);
 int occupancy_fused_f1(int dp, bool wide);
 int occupancy_fused_f2(int dp, bool wide);

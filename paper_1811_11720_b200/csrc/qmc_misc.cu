@@ -13,39 +13,18 @@ namespace qmc {
 __global__ void __launch_bounds__(32) prepare_kernel(const DevProblem* __restrict__ probs, DevAux* __restrict__ aux,
                                                      unsigned long long* __restrict__ prog_area) {
     const DevProblem pb = probs[blockIdx.x];
+    if (pb.family != QMC_FAMILY_SECTOR) return;             // closed-form families derive their tables inside the fused kernel
     DevAux& a = aux[blockIdx.x];
-    const int j = threadIdx.x, d = pb.dim;
-    const unsigned long long n = pb.n;
+    const int j = threadIdx.x;
     if (j < QMC_MAX_DIM) {
-        unsigned long long z = 0, step = 0, back = 0;
-        double fa = 0.0, fb = 0.0, f[5] = {1.0, 0.0, 0.0, 0.0, 0.0};
-        if (j < d) {
-            z = pb.z[j] % n;
-            step = mulmod_u64((unsigned long long)kThreads % n, z, n);
-            back = mulmod_u64(((unsigned long long)pb.steps * kThreads) % n, z, n);
-            const double* p = pb.params;
-            if (pb.family == QMC_FAMILY_GENZ_OSC) { fa = p[1 + j]; }
-            else if (pb.family == QMC_FAMILY_GENZ_PRODPEAK) { const double c = p[j]; fa = __ddiv_rn(1.0, __dmul_rn(c, c)); fb = p[d + j]; }
-            else if (pb.family == QMC_FAMILY_CEXP_POLY) { fa = p[j]; fb = p[d + j]; }
-            if (pb.has_fit) {
-                const double* c = pb.fit + 6 * j;
-                const double a4 = c[4], a5 = c[5];
-                const double a6 = __dadd_rn(__dadd_rn(__dadd_rn(__dadd_rn(1.0, -c[2]), -c[3]), -a4), -a5);
-                f[0] = a4; f[1] = a5; f[2] = a6; f[3] = 2.0 * a5; f[4] = 3.0 * a6;
-            }
-        }
-        if (j >= d && pb.family == QMC_FAMILY_GENZ_PRODPEAK) {
-            // padded slot (qmc_fused.cuh): the coordinate is pinned to u = 1/2, i.e. x = 1 (baker) or 1/2; factor (x-fb)^2 + fa = 1
-            fa = 1.0;
-            fb = (pb.tr_kind == TR_BAKER) ? 1.0 : 0.5;
-        }
-        a.z[j] = z; a.step[j] = step; a.back[j] = back; a.fam_a[j] = fa; a.fam_b[j] = fb;
+        const SlotConst s = derive_slot(pb, j);
+        a.z[j] = s.z; a.step[j] = s.step; a.back[j] = s.back; a.fam_a[j] = s.fa; a.fam_b[j] = s.fb;
 #pragma unroll
-        for (int i = 0; i < 5; ++i) a.fit[i][j] = f[i];
+        for (int i = 0; i < 5; ++i) a.fit[i][j] = s.f[i];
         a.nu[j] = 0;
     }
     if (j == 0) {
-        a.fam0 = (pb.family == QMC_FAMILY_GENZ_OSC) ? __dmul_rn(6.283185307179586476925286766559, pb.params[0]) : 0.0;
+        a.fam0 = derive_fam0(pb);
         a.status = 0;
         a.sec_a = a.sec_b = 0;
         a.sec_nops[0] = a.sec_nops[1] = a.sec_ncoef[0] = a.sec_ncoef[1] = 0;
@@ -72,16 +51,17 @@ __device__ __forceinline__ void eq3_component(const double* __restrict__ means, 
     *err_out = __dsqrt_rn(__ddiv_rn(v.value(), __dmul_rn((double)m, (double)(m - 1))));
 }
 
-__global__ void __launch_bounds__(256) finalize_kernel(const DevProblem* __restrict__ probs, const DevAux* __restrict__ aux,
-                                                       const double* __restrict__ partials, double* __restrict__ means_ws,
-                                                       double* __restrict__ out_means, double* __restrict__ out_errs,
-                                                       double* __restrict__ out_shift_means, int stride) {
-    const DevProblem& pb = probs[blockIdx.x];
+constexpr int kFinalizeThreads = 1024;
+__global__ void __launch_bounds__(kFinalizeThreads) finalize_kernel(const __grid_constant__ FusedLaunch L, double* __restrict__ means_ws,
+                                                                    double* __restrict__ out_means, double* __restrict__ out_errs,
+                                                                    double* __restrict__ out_shift_means, int stride) {
+    const DevProblem& pb = L.single ? L.one : L.probs[blockIdx.x];
+    const double* __restrict__ partials = L.partials;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nc = pb.ncomp, m = pb.m, tiles = pb.tiles, npairs = m * nc;
     double* means = means_ws + pb.means_off;
-    const bool bad = aux[blockIdx.x].status != 0;
-    for (int pair = warp; pair < npairs; pair += 8) {
+    const bool bad = pb.family == QMC_FAMILY_SECTOR && L.aux[blockIdx.x].status != 0;
+    for (int pair = warp; pair < npairs; pair += kFinalizeThreads / 32) {
         const double* src = partials + pb.partial_off + (long long)pair * tiles;
         CompSum cs;
         for (int t = lane; t < tiles; t += 32) cs.add(src[t]);
@@ -158,9 +138,9 @@ cudaError_t launch_prepare(int count, cudaStream_t st, const DevProblem* probs, 
     prepare_kernel<<<count, 32, 0, st>>>(probs, aux, prog_area);
     return cudaGetLastError();
 }
-cudaError_t launch_finalize(int count, cudaStream_t st, const DevProblem* probs, const DevAux* aux, const double* partials,
-                            double* means_ws, double* out_means, double* out_errs, double* out_shift_means, int stride) {
-    finalize_kernel<<<count, 256, 0, st>>>(probs, aux, partials, means_ws, out_means, out_errs, out_shift_means, stride);
+cudaError_t launch_finalize(int count, cudaStream_t st, const FusedLaunch& a, double* means_ws, double* out_means, double* out_errs,
+                            double* out_shift_means, int stride) {
+    finalize_kernel<<<count, kFinalizeThreads, 0, st>>>(a, means_ws, out_means, out_errs, out_shift_means, stride);
     return cudaGetLastError();
 }
 cudaError_t launch_finalize_means(cudaStream_t st, const double* means, int m, int nc, double* out_mean, double* out_err) {

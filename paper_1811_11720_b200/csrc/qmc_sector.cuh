@@ -214,16 +214,17 @@ template <int DP> struct SectorGroup { static constexpr int value = sector_group
 template <int DP, int G> struct SectorMinBlocks { static constexpr int value = min_blocks_sector(DP); };
 
 template <int DP, int G, bool WIDE>
-__global__ void __launch_bounds__(kThreads, SectorMinBlocks<DP, G>::value)
-fused_sector_kernel(const DevProblem* __restrict__ probs, const DevAux* __restrict__ aux, VariantQueue vq,
-                    double* __restrict__ partials, const unsigned long long* __restrict__ prog_area) {
+__global__ void __launch_bounds__(kThreads, SectorMinBlocks<DP, G>::value) fused_sector_kernel(const __grid_constant__ FusedLaunch L) {
+    const DevAux* __restrict__ aux = L.aux;
+    const unsigned long long* __restrict__ prog_area = L.prog;
+    double* __restrict__ partials = L.partials;
     __shared__ SmemCtx<DP, G> sm;
     __shared__ SectorSmem ex;
     const unsigned sbase = (unsigned)__cvta_generic_to_shared(&sm), exbase = (unsigned)__cvta_generic_to_shared(&ex);
-    int cur = -1;
+    int cur = -1, iter = 0;
     long long tile_local = 0;
     bool changed;
-    while (next_tile<DP, G>(sm, probs, aux, vq, cur, tile_local, changed)) {
+    while (next_tile<DP, G, true>(sm, L, cur, iter, tile_local, changed)) {
         if (changed) {
             const int tid = threadIdx.x;
             const DevAux& a = aux[cur];
