@@ -39,7 +39,7 @@ MAIN_CONFIG = 1
 # Algorithmic FP64-pipe instructions per integrand evaluation (thread level; FMA, MUL, ADD each count 1), derived in
 # DESIGN.md section 5 from the method itself.  Per dimension: coordinate (1 FMA) + wrap/centre (1 ADD) = 2; transform: none 0,
 # baker 1, Korobov-3 7 (c^2, 1/4 - c^2, weight product, 3-term Horner, phi); cubic fit map 6; integrand term: oscillatory 1,
-# product peak 3, complex exp*poly 3.  Per evaluation: Korobov weight 3 (+1 with the fit Jacobian); cos 14 / sincos 25
+# product peak 3, complex exp*poly 3.  Per evaluation: Korobov weight 3 (+1 with the fit Jacobian); cos 14 / sincos 21
 # (executed counts of the libdevice fast paths); reciprocal 5; accumulate 1 per component (+1 for the complex amplitude).
 # Sector family: sum of monomial degrees of U and F (mean 44.44 over the 256 seeded sectors) + prefactor (mean 3.04) +
 # powers (a: mean 1.51, b-1: mean 1.50) + weight*numerator 1.  These are the numerators of roofline.achieved; the EXECUTED
@@ -47,7 +47,7 @@ MAIN_CONFIG = 1
 ALG_FP64_PER_EVAL = {
     0: 4 * (2 + 7 + 1) + 3 + 14 + 1,                                  # 58   d=4 osc, Korobov-3
     1: 8 * (2 + 1 + 3) + 5 + 1,                                       # 54   d=8 product peak, baker
-    2: 12 * (2 + 7 + 3) + 3 + 25 + 1 + 2,                             # 175  d=12 complex, Korobov-3
+    2: 12 * (2 + 7 + 3) + 3 + 21 + 1 + 2,                             # 171  d=12 complex, Korobov-3
     3: 6 * (2 + 7) + 3 + 44.44 + 3.04 + 1.51 + 1.50 + 1 + 5 + 1,      # 114.5 d=6 sector, Korobov-3
     4: 16 * (2 + 7 + 6 + 1) + 4 + 14 + 1,                             # 275  d=16 osc, Korobov-3 + cubic map
 }
