@@ -10,7 +10,8 @@ latency bound).  PTX `brx.idx` gives one indexed branch per step; every case end
 (threaded code) and loads the next step code and the next coefficient before its fp64 work, so the
 shared-memory latency hides behind the G fp64 instructions of the step.
 
-Step codes (qmc_sector.cuh): 0 = no-op, 1 = end of U, 2 = end of program, 4 + 4*j + 2*FIRST + LAST.
+Step codes (qmc_sector.cuh): 0 = no-op, 1 = end of U, 2 = end of program, 3 = dense linear form
+(sum += sum_j c_j x_j with DP coefficients from the stream), 4 + 4*j + 2*FIRST + LAST:
     FIRST & LAST : sum  = fma(coef, x_j, sum)
     FIRST        : mon  = coef * x_j
     LAST         : sum  = fma(mon, x_j, sum)
@@ -43,10 +44,10 @@ def gen(dp, g):
     L = []
     a = L.append
     a("{")
-    a(".reg .f64 " + ", ".join(f"m{q}" for q in range(g)) + ", cf, cfn;")
+    a(".reg .f64 " + ", ".join(f"m{q}" for q in range(g)) + ", cf, cfn, " + ", ".join(f"l{j}" for j in range(1, dp)) + ";")
     a(".reg .u32 pc, pk, tgt, " + ", ".join(f"c{t}" for t in range(max(SETS, 2))) + ";")
     for t in range(SETS):
-        labels = [f"T{t}_NOP", f"T{t}_ENDU", "LEND", f"T{t}_NOP"] + [f"T{t}_S{j}_{k}" for j in range(dp) for k in range(4)]
+        labels = [f"T{t}_NOP", f"T{t}_ENDU", "LEND", f"T{t}_LIN"] + [f"T{t}_S{j}_{k}" for j in range(dp) for k in range(4)]
         labels += [f"T{t}_P{p}_{q}_{full}" for (p, q) in pairs for full in range(2)]
         a(f"ts{t}: .branchtargets " + ", ".join(labels) + ";")
     for q in range(g):
@@ -58,21 +59,21 @@ def gen(dp, g):
         a("ld.shared.u8 tgt, [pc];")
         a("ld.shared.u8 c0, [pc+1];")
         a("ld.shared.u8 c1, [pc+2];")
-        a("brx.idx tgt, ts0;")
+        a("brx.idx.uni tgt, ts0;")
     else:
         for t in range(SETS):
             a(f"ld.shared.u8 c{t}, [pc+{t}];")
-        a("brx.idx c0, ts0;")
+        a("brx.idx.uni c0, ts0;")
     for t in range(SETS):
         # case of step i in table t = i mod SETS: register c_t held code[i]; it is reloaded with code[i+SETS] and the
         # step leaves through c_{t+1} (loaded SETS-1 steps ago) into the next table
         nt = (t + 1) % SETS
         fetch = [f"ld.shared.u8 c{t}, [pc+{SETS}];", "add.u32 pc, pc, 1;"]
-        leave = f"brx.idx c{nt}, ts{nt};"
+        leave = f"brx.idx.uni c{nt}, ts{nt};"
         if SETS == 1:
             # one table: c0 = code[i+1] (arrived), c1 = code[i+2] (in flight); the target of step i+1 is known at entry
             fetch = ["mov.u32 tgt, c0;", "mov.u32 c0, c1;", "ld.shared.u8 c1, [pc+3];", "add.u32 pc, pc, 1;"]
-            leave = "brx.idx tgt, ts0;"
+            leave = "brx.idx.uni tgt, ts0;"
         coef = ["mov.f64 cf, cfn;", "ld.shared.f64 cfn, [pk+8];", "add.u32 pk, pk, 8;"]
         a(f"T{t}_NOP:")
         L.extend(fetch)
@@ -82,6 +83,18 @@ def gen(dp, g):
         for q in range(g):
             a(f"mov.f64 {u(q)}, {s(q)};")
             a(f"mov.f64 {s(q)}, {c0f};")
+        a(leave)
+        # dense linear form: DP coefficients from the stream (the first one is the prefetched cfn)
+        a(f"T{t}_LIN:")
+        L.extend(fetch)
+        a("mov.f64 cf, cfn;")
+        for j in range(1, dp):
+            a(f"ld.shared.f64 l{j}, [pk+{8 * j}];")
+        a(f"ld.shared.f64 cfn, [pk+{8 * dp}];")
+        a(f"add.u32 pk, pk, {8 * dp};")
+        for j in range(dp):
+            for q in range(g):
+                a(f"fma.rn.f64 {s(q)}, {'cf' if j == 0 else f'l{j}'}, {x(q, j)}, {s(q)};")
         a(leave)
         for j in range(dp):
             for k in range(4):
@@ -133,7 +146,7 @@ template <> __device__ __forceinline__ void sector_interp<{dp}, {g}>(const doubl
 def main():
     here = os.path.dirname(os.path.abspath(__file__))
     out = ["// GENERATED by gen_sector_interp.py -- do not edit.  Threaded-code interpreter of the sector family",
-           "// (inline PTX, one brx.idx per step); included by qmc_sector.cuh inside namespace qmc.",
+           "// (inline PTX, one brx.idx.uni per step); included by qmc_sector.cuh inside namespace qmc.",
            "// sum[] must hold U's constant term on entry; on return U[q] = U(x_q), sum[q] = F(x_q).",
            "template <int DP, int G> __device__ __forceinline__ void sector_interp(const double (&x)[G][DP], unsigned steps_addr,",
            "                                                                       unsigned coefs_addr, double c0f, double (&U)[G],",

@@ -154,7 +154,7 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
         if (p.family == QMC_FAMILY_SECTOR) {
             const int nmono = (p.n_params - 4 - p.dim) / (1 + p.dim);
             d.aux_off = (int)prog_off;
-            d.aux_len = 3 * nmono + 1;                                  // coefs + 16 one-byte steps per monomial + end-of-U / padding
+            d.aux_len = sector_coef_slots(nmono) + 2 * nmono + 1;       // coefs + 16 one-byte steps per monomial + end-of-U / padding
             prog_off += (size_t)d.aux_len;
         }
         d.means_off = means_off;

@@ -24,6 +24,8 @@ constexpr int min_blocks_sector(int dp) { return dp <= 6 ? 3 : 2; }
 constexpr int kDeltaCache = 768;       // doubles of shared memory per CTA that cache the shifts of all groups of a problem
 constexpr int kMaxSectorOps = 1024;    // interpreter program length limit per polynomial
 constexpr int kMaxSectorMono = 64;
+constexpr int kSectorLinSlots = 32;    // extra coefficient slots of a sector program: one dense linear form (<= 16 entries) per polynomial
+__host__ __device__ constexpr int sector_coef_slots(int nmono) { return nmono + kSectorLinSlots; }   // coefficient region of a program, in doubles
 
 // transform kinds after host-side decoding
 enum : int { TR_NONE = 0, TR_BAKER = 1, TR_KOR3 = 2, TR_KORR = 3 };

@@ -22,13 +22,14 @@
 
 namespace qmc {
 
-constexpr int kSecMaxCoef = 128;     // non-constant monomials of U and F together
+constexpr int kSecMaxCoef = 192;     // coefficient stream of a program: non-constant monomials of U and F + two dense linear forms
 constexpr int kSecMaxWords = kMaxSectorOps / 4;
 
-// step codes (one byte each): 0 = no-op, 1 = end of U, 2 = end of program, 4 + 4*j + 2*FIRST + LAST (single
+// step codes (one byte each): 0 = no-op, 1 = end of U, 2 = end of program, 3 = dense linear form (sum += sum_j c_j x_j over
+// all DP slots, DP coefficients from the stream: the degree-1 monomials of a polynomial in ONE step), 4 + 4*j + 2*FIRST + LAST (single
 // variable); with DP <= 8 dimension slots also 4 + 4*DP + 2*pair(a,b) + FULL, a <= b: the first two variables of a
 // monomial in one step (mon = coef x_a; FULL ? sum = fma(mon, x_b, sum) : mon *= x_b), pair(a,b) = a DP - a(a-1)/2 + b - a
-enum : int { SEC_NOP = 0, SEC_ENDU = 1, SEC_END = 2, SEC_BASE = 4 };
+enum : int { SEC_NOP = 0, SEC_ENDU = 1, SEC_END = 2, SEC_LIN = 3, SEC_BASE = 4 };
 
 struct alignas(16) SectorSmem {
     double coefs[kSecMaxCoef];       // coefficients of the non-constant monomials, in step order
@@ -61,7 +62,7 @@ __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned 
     // A rejected parameter block must still leave a program the interpreter can run to its end (the problem's
     // results are then replaced by NaN in the finalize stage): end-of-U, end, read-ahead padding.
     {
-        const int slots = (pb.n_params - 4 - d) / (1 + d);
+        const int slots = sector_coef_slots((pb.n_params - 4 - d) / (1 + d));
         unsigned char* stub = reinterpret_cast<unsigned char*>(prog_area + pb.aux_off + slots);
         stub[0] = (unsigned char)SEC_ENDU; stub[1] = (unsigned char)SEC_END;
         for (int i = 2; i < 8; ++i) stub[i] = (unsigned char)SEC_NOP;
@@ -84,7 +85,7 @@ __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned 
         a.nu[j] = (unsigned char)(int)v;
     }
     double* coefs = reinterpret_cast<double*>(prog_area + pb.aux_off);
-    const int max_coef = cnt[0] + cnt[1];
+    const int max_coef = sector_coef_slots(cnt[0] + cnt[1]);
     unsigned char* ops = reinterpret_cast<unsigned char*>(prog_area + pb.aux_off + max_coef);
     const int max_ops = min((pb.aux_len - max_coef) * 8, kMaxSectorOps) - 8;   // room for SEC_ENDU, SEC_END and 3+ bytes of read-ahead padding
     int nops = 0, ncoef = 0;
@@ -93,6 +94,24 @@ __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned 
         const double* c = base;
         const double* e = base + cnt[pol];
         double c0 = 0.0;
+        // the degree-1 monomials of the polynomial become one dense linear-form step when there are at least two
+        int nlin = 0;
+        for (int t = 0; t < cnt[pol]; ++t) {
+            int deg = 0;
+            for (int j = 0; j < d; ++j) deg += (int)e[t * d + j];
+            nlin += (deg == 1);
+        }
+        const bool lin = nlin >= 2 && ncoef + dp < kSecMaxCoef - 1 && nops + 1 <= max_ops;
+        if (lin) {
+            for (int j = 0; j < dp; ++j) coefs[ncoef + j] = 0.0;
+            for (int t = 0; t < cnt[pol]; ++t) {
+                int deg = 0, var = 0;
+                for (int j = 0; j < d; ++j) { const int ej = (int)e[t * d + j]; deg += ej; if (ej) var = j; }
+                if (deg == 1) coefs[ncoef + var] += c[t];
+            }
+            ncoef += dp;
+            ops[nops++] = (unsigned char)SEC_LIN;
+        }
         for (int t = 0; t < cnt[pol]; ++t) {
             int deg = 0;
             for (int j = 0; j < d; ++j) {
@@ -102,6 +121,7 @@ __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned 
             }
             if (deg > 16 || status) { status = QMC_ERR_PARAMS; continue; }
             if (deg == 0) { c0 += c[t]; continue; }
+            if (deg == 1 && lin) continue;
             if (ncoef >= kSecMaxCoef - 1 || nops + deg > max_ops) { status = QMC_ERR_PARAMS; continue; }
             coefs[ncoef++] = c[t];
             int seen = 0, va = -1;
@@ -230,7 +250,7 @@ __global__ void __launch_bounds__(kThreads, SectorMinBlocks<DP, G>::value) fused
             const DevAux& a = aux[cur];
             const DevProblem& pb = sm.prob;
             const int ncoef = a.sec_ncoef[0], nwords = a.sec_nops[0];
-            const int max_coef = (pb.n_params - 4 - pb.dim) / (1 + pb.dim);
+            const int max_coef = sector_coef_slots((pb.n_params - 4 - pb.dim) / (1 + pb.dim));
             const double* coefs = reinterpret_cast<const double*>(prog_area + pb.aux_off);
             const unsigned int* words = reinterpret_cast<const unsigned int*>(prog_area + pb.aux_off + max_coef);
             for (int i = tid; i <= ncoef && i < kSecMaxCoef; i += kThreads) ex.coefs[i] = i < ncoef ? coefs[i] : 0.0;
