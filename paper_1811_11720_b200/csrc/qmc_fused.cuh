@@ -96,10 +96,10 @@ __device__ __forceinline__ double point_coord(double rd, double inv_n, double de
     if (TR == TR_NONE) {
         x = wrap_u(t);
     } else {
-        const double c = centre_c(t);
         if (TR == TR_BAKER) {
-            x = baker_y(c);
+            x = 1.0 - fabs(baker_w(t));                       // Eq. 17: the tent map is even about u = 1/2, no wrap decision needed
         } else {
+            const double c = centre_c(t);
             const double s = c * c;
             P *= (0.25 - s);                                  // u (1-u)
             double g;
@@ -175,8 +175,14 @@ __device__ __forceinline__ void eval_point_group(const typename Res<WIDE>::T (&r
         load_slot<DP, G, FIT>(cx.sbase, cx.delta, j, fa, fb, fc, dl);
 #pragma unroll
         for (int q = 0; q < G; ++q) {
-            const double x = point_coord<TR, FIT>(rd, cx.inv_n, dl[q], fc, cx.sbase + SmemOff<DP, G>::kor, cx.kor_r, P[q], D[q]);
-            fam_dim<FAMILY>(s0[q], s1[q], x, fa, fb);
+            if (FAMILY == QMC_FAMILY_GENZ_PRODPEAK && TR == TR_BAKER && !FIT) {
+                // x - w_j = (1 - w_j) - |w| with the slot constant fb = 1 - w_j (derive_slot): the baker map folds into the factor
+                const double dd = fb - fabs(baker_w(coord_t(rd, cx.inv_n, dl[q])));
+                s0[q] *= __fma_rn(dd, dd, fa);
+            } else {
+                const double x = point_coord<TR, FIT>(rd, cx.inv_n, dl[q], fc, cx.sbase + SmemOff<DP, G>::kor, cx.kor_r, P[q], D[q]);
+                fam_dim<FAMILY>(s0[q], s1[q], x, fa, fb);
+            }
         }
     }
     constexpr bool USEW = (TR == TR_KOR3 || TR == TR_KORR || FIT);
@@ -334,6 +340,8 @@ __device__ __forceinline__ SlotConst derive_slot(const DevProblem& pb, int j) {
         s.fa = 1.0;
         s.fb = (pb.tr_kind == TR_BAKER) ? 1.0 : 0.5;
     }
+    // product peak under the baker map without fit: the fused kernel wants 1 - w_j (eval_point_group)
+    if (pb.family == QMC_FAMILY_GENZ_PRODPEAK && pb.tr_kind == TR_BAKER && !pb.has_fit) s.fb = __dadd_rn(1.0, -s.fb);
     return s;
 }
 __device__ __forceinline__ double derive_fam0(const DevProblem& pb) {
