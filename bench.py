@@ -214,6 +214,38 @@ def e2e_host_api(binding, probs, reps):
     return dt, h2d, d2h
 
 
+def closed_form(c, prm):
+    """exact integrals of the closed-form configs (Genz families 1, 2: PAPER.md L709-L713; complex exp*poly): analysis only"""
+    d = synth.CONFIG_SHAPES[c][0]
+    if c in (0, 4):
+        a = prm[1:]
+        return complex(np.cos(2 * np.pi * prm[0] + 0.5 * a.sum()) * np.prod(np.sin(a / 2) / (a / 2)))
+    if c == 1:
+        cc, w = prm[:d], prm[d:]
+        return complex(np.prod(cc * (np.arctan(cc * (1 - w)) + np.arctan(cc * w))))
+    a, b = prm[:d].astype(complex), prm[d:]
+    e = np.exp(1j * a)
+    return complex(np.prod((e - 1) / (1j * a) + b * (e / (1j * a) - (e - 1) / (1j * a) ** 2)))
+
+
+def time_to_target(binding, c, probs, epsrel=1e-8):
+    """BASELINE metric part 3: wall time of the paper's iteration (qmc_integrate) to an ESTIMATED relative
+    error of 1e-8 on the committed lattice ladder, shifts and parameters of configs[c]; earlier lattices are discarded (L357)."""
+    p = probs[0]
+    ln, lz = synth.ladder(p["dim"], p["n"])
+    kw = dict(min_n=1000, min_m=p["m"], epsrel=epsrel, epsabs=0.0, maxeval=2 ** 62, fit_coeffs=p.get("fit_coeffs"))
+    binding.qmc_integrate(p["family"], p["params"], p["dim"], p["transform"], ln[:1], lz[:1], p["shifts"], **kw)   # warm-up
+    t0 = time.perf_counter()
+    res, st = binding.qmc_integrate(p["family"], p["params"], p["dim"], p["transform"], ln, lz, p["shifts"], **kw)
+    dt = time.perf_counter() - t0
+    exact = closed_form(c, p["params"])
+    est = complex(*res["integral"]) if len(res["integral"]) == 2 else complex(res["integral"][0])
+    return {"workload": workload_name(c), "target_rel_err": epsrel, "reached": st == 0, "seconds": dt, "n": res["n"], "m": res["m"],
+            "iterations": res["iterations"], "evaluations": res["evaluations"],
+            "estimated_rel_err": float(max(res["error"]) / abs(est)), "true_rel_err": abs(est - exact) / abs(exact),
+            "ladder": [int(v) for v in ln]}
+
+
 def run_ours(args):
     import torch
     if not torch.cuda.is_available():
@@ -293,6 +325,16 @@ def run_ours(args):
             windows.append(w)
             others.append(rec)
 
+    ttt = []
+    if rank == 0 and world == 1 and not args.main_only:
+        for c in (0, 1, 2, 4):
+            if args.others is not None and c not in args.others and c != args.main:
+                continue
+            probs = rank_problems(c, 0)
+            if c == 4:
+                probs = config4_with_device_fit(binding, probs)
+            ttt.append(time_to_target(binding, c, probs))
+
     # end-to-end through the HOST-pointer entry (rank-local; max over ranks)
     barrier()
     e2e_reps = max(5, min(args.steps, 50))
@@ -316,7 +358,7 @@ def run_ours(args):
            "fused_kernel_share_of_step": main["fused_kernel_share_of_step"],
            "fp64_peak_probe": {"thread_inst_per_s": peak_rate, "ms": peak_ms, "sm_count": sm_count,
                                "implied_clock_mhz_at_64_lanes": peak_rate / (sm_count * FP64_LANES_PER_SM) / 1e6},
-           "clocks": clocks, "others": others}
+           "clocks": clocks, "others": others, "time_to_rel_err_1e-8": ttt}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(args.main, reps=3)
     if rank == 0:

@@ -151,6 +151,33 @@ int qmc_lattice_points(uint64_t n, int dim, const uint64_t* z /*HOST*/, const do
 int qmc_finalize_means(const double* shift_means /*DEVICE*/, int m, int ncomp, double* out_mean /*DEVICE*/,
                        double* out_err /*DEVICE*/, void* cuda_stream);
 
+/* The paper's `integrate` iteration (section 3.3.1; fields P:L887-L920; result P:L988-L995) around the
+ * fused hot path: sample min_m shifted copies of the smallest ladder lattice with n >= min_n; if the error goal
+ *     err <= max(epsabs, epsrel * |E|)                                  (per component for complex)
+ * is not met, DISCARD the result and take a larger lattice; stop when the goal is met or `maxeval`
+ * evaluations have been spent; when the ladder is exhausted keep the largest lattice and add shifts
+ * (Monte Carlo scaling) up to max_m.  The paper does not say how the next lattice is chosen (DESIGN.md reading
+ * C-14): the smallest ladder n >= n * max(2, err / goal) (assumes >= 1/n error scaling), limited to what `maxeval` still
+ * allows.  All pointers HOST; synchronous; allocates device memory for the duration of the call only.
+ *   ladder_n[i] ascending, ladder_z[i*dim + j] the generating vector of lattice i (an INPUT: P:L940-L942)
+ *   shifts[max_m][dim]: the first m rows are used for a lattice sampled with m shifts
+ *   errormode: 0 = all components, 1 = largest component (ignored for real families)
+ * Returns QMC_OK when the goal was met, QMC_ERR_MAXEVAL (result still written) when it was not. */
+typedef struct {
+    double integral[2];       /* estimate (re, im); im = 0 for real families */
+    double error[2];          /* error estimate per component (Eq. 3) */
+    uint64_t n;               /* size of the last (largest) lattice used */
+    int m;                    /* shifts of that lattice */
+    int iterations;           /* lattices sampled + shift extensions */
+    uint64_t evaluations;     /* integrand evaluations over all iterations */
+} qmc_result;
+enum { QMC_ERR_MAXEVAL = -14 };
+int qmc_integrate(int family, const double* params /*HOST*/, int n_params, int dim, int transform,
+                  const double* fit_coeffs /*HOST or NULL*/, int n_lattices, const uint64_t* ladder_n /*HOST*/,
+                  const uint64_t* ladder_z /*HOST [n_lattices][dim]*/, const double* shifts /*HOST [max_m][dim]*/,
+                  uint64_t min_n, int min_m, int max_m, double epsrel, double epsabs, uint64_t maxeval, int errormode,
+                  qmc_result* out /*HOST*/);
+
 /* Measurement helper: runs a DFMA-chain kernel (8 independent chains per thread, full occupancy)
  * for `iters` iterations on `cuda_stream`, synchronises, and returns the sustained thread-level
  * FP64 instruction rate in instructions/second through *out_rate (HOST) and the kernel time in ms

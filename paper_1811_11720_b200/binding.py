@@ -19,11 +19,12 @@ EXPORTS = [
     "qmc_validate_problem_host", "qmc_lattice_project", "qmc_project_workspace_bytes", "qmc_fit_cubic",
     "qmc_lattice_points", "qmc_finalize_means", "qmc_fp64_peak_probe", "qmc_last_launch_count", "qmc_plan_info",
     "qmc_profile_enable", "qmc_profile_last_fused_ms",
-    "qmc_num_components", "qmc_status_string", "qmc_last_cuda_error",
+    "qmc_num_components", "qmc_status_string", "qmc_last_cuda_error", "qmc_integrate",
 ]
 
 QMC_OK = 0
 QMC_ERR_NONFINITE = -13
+QMC_ERR_MAXEVAL = -14
 
 
 class QmcError(RuntimeError):
@@ -40,6 +41,11 @@ class qmc_problem(C.Structure):
     _fields_ = [("family", C.c_int), ("dim", C.c_int), ("m", C.c_int), ("transform", C.c_int), ("n", C.c_uint64),
                 ("params", C.c_void_p), ("n_params", C.c_int), ("z", C.c_void_p), ("shifts", C.c_void_p),
                 ("fit_coeffs", C.c_void_p)]
+
+
+class qmc_result(C.Structure):
+    _fields_ = [("integral", C.c_double * 2), ("error", C.c_double * 2), ("n", C.c_uint64), ("m", C.c_int),
+                ("iterations", C.c_int), ("evaluations", C.c_uint64)]
 
 
 _lib = None
@@ -72,6 +78,8 @@ def lib():
         L.qmc_num_components.argtypes = [C.c_int]
         L.qmc_profile_enable.argtypes = [C.c_int]
         L.qmc_profile_last_fused_ms.argtypes = [dp]
+        L.qmc_integrate.argtypes = [C.c_int, dp, C.c_int, C.c_int, C.c_int, dp, C.c_int, up, up, dp, C.c_uint64, C.c_int, C.c_int,
+                                    C.c_double, C.c_double, C.c_uint64, C.c_int, C.POINTER(qmc_result)]
         L.qmc_status_string.argtypes = [C.c_int]
         L.qmc_status_string.restype = C.c_char_p
         L.qmc_last_cuda_error.restype = C.c_char_p
@@ -121,6 +129,22 @@ def qmc_lattice_integrate_ex(p: dict):
     _check(lib().qmc_lattice_integrate_ex(p["family"], _d(params), len(params), p["dim"], p["n"], _u(z), _d(shifts), p["m"],
                                           p["transform"], _d(fit), _d(mean), _d(err), _d(sm)), "qmc_lattice_integrate_ex")
     return sm, mean[:nc].copy(), err[:nc].copy()
+
+
+def qmc_integrate(family, params, dim, transform, ladder_n, ladder_z, shifts, min_n=8191, min_m=32, epsrel=0.01, epsabs=1e-7,
+                  maxeval=1000000, errormode=0, fit_coeffs=None):
+    """The paper's `integrate` iteration (defaults: PAPER.md L887-L905) -> (dict result, status); status is QMC_OK when the
+    error goal was met and QMC_ERR_MAXEVAL when maxeval / the ladder / the shifts ran out (the last result is returned)."""
+    params, shifts, fit = _f64(params), _f64(shifts), _f64(fit_coeffs)
+    ln = np.ascontiguousarray(ladder_n, dtype=np.uint64)
+    lz = np.ascontiguousarray(ladder_z, dtype=np.uint64).reshape(len(ln), int(dim))
+    nc = max(qmc_num_components(family), 1)
+    res = qmc_result()
+    st = _check(lib().qmc_integrate(int(family), _d(params), len(params), int(dim), int(transform), _d(fit), len(ln), _u(ln), _u(lz),
+                                    _d(shifts), int(min_n), int(min_m), int(shifts.shape[0]), float(epsrel), float(epsabs),
+                                    int(maxeval), int(errormode), C.byref(res)), "qmc_integrate", allow=(QMC_ERR_MAXEVAL,))
+    return {"integral": np.array(res.integral[:nc]), "error": np.array(res.error[:nc]), "n": int(res.n), "m": int(res.m),
+            "iterations": int(res.iterations), "evaluations": int(res.evaluations)}, st
 
 
 def qmc_validate_problem_host(p: dict) -> int:

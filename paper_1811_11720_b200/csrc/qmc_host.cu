@@ -426,6 +426,7 @@ const char* qmc_status_string(int status) {
         case QMC_ERR_WORKSPACE: return "workspace null, misaligned or too small";
         case QMC_ERR_CUDA: return "CUDA error";
         case QMC_ERR_NONFINITE: return "non-finite result";
+        case QMC_ERR_MAXEVAL: return "error goal not reached within maxeval / the available lattices and shifts";
     }
     return "unknown status";
 }

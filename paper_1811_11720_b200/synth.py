@@ -75,6 +75,16 @@ def genvec(n: int, d: int):
     return np.array(table[key]["z"], dtype=np.uint64)
 
 
+def ladder(d: int, n_max: int, n_min: int = 1021):
+    """The committed lattice ladder for dimension d: largest primes below 2^10, 2^12, ... plus the configs' own sizes, with
+    their CBC vectors (ascending n, n_min <= n <= n_max) -> (ladder_n (L,), ladder_z (L, d)).  Stand-in for the paper's
+    generating-vector tables (PAPER.md, Table A.1), which are not available."""
+    with open(_DATA) as f:
+        table = json.load(f)
+    ns = sorted(v["n"] for v in table.values() if v["d"] == d and n_min <= v["n"] <= n_max)
+    return (np.array(ns, dtype=np.uint64), np.array([table[f"{n}:{d}"]["z"] for n in ns], dtype=np.uint64).reshape(len(ns), d))
+
+
 def korobov_form_vector(n: int, d: int, a: int):
     """z = (1, a, a^2, ...) mod n: any valid z exercises the same code path (used by tests)."""
     z, cur = [], 1
