@@ -10,7 +10,7 @@
 //   O2  u = wrap(fma(double(r), 1/double(n), Delta_{s,j}))  "{ } = fractional part", P:L100;
 //       the fp64 realisation is DESIGN.md reading C-2
 //   O3  (y, w) = periodizing transform: None (Table A.2), baker Eq. 17 P:L204-L209,
-//       Korobov weight r Eq. 15 P:L189-L193 with phi = int_0^u omega (Eq. 14)
+//       Korobov weights (r0, r1) Eq. 15 P:L189-L193 and Sidi weight r Eq. 16, phi = int_0^u omega (Eq. 14)
 //   O4  optional fit map x = p(y), w *= p'(y)         Eq. 18-19, order P:L338
 //   O5  v = (prod_j w_j) * f(x)                                           Eq. 12-13
 //   O6  S_s = sum_k v (Neumaier-compensated), Q_s = S_s / n                       Eq. 2
@@ -44,7 +44,8 @@ namespace {
 typedef unsigned __int128 u128;
 
 enum { FAM_OSC = 0, FAM_PRODPEAK = 1, FAM_CEXP = 2, FAM_SECTOR = 3 };
-enum { TR_NONE = 0, TR_BAKER = 1, TR_KOROBOV = 100 };
+// transform ids: Table A.2.  Korobov<r> = 100 + r; Sidi<r> = 200 + r; Korobov<r0,r1> = 1000 + 16 r0 + r1.
+enum { TR_NONE = 0, TR_BAKER = 1, TR_KOROBOV = 100, TR_SIDI = 200, TR_KOROBOV_ASYM = 1000 };
 const int MAX_DIM = 64;
 const uint64_t CHUNK = 1ull << 16;
 
@@ -70,34 +71,79 @@ inline double coordinate(uint64_t r, double inv_n, double delta) {
 
 double binom(int a, int b) { double v = 1.0; for (int i = 1; i <= b; ++i) v = v * (double)(a - b + i) / (double)i; return v; }
 
-// Korobov weight-r transform, Eq. 15 with r0 = r1 = r:
-//   omega(u) = (2r+1) C(2r,r) u^r (1-u)^r,
-//   phi(u) = int_0^u omega = c_r sum_{i=0}^{r} C(r,i) (-1)^i u^{r+1+i} / (r+1+i)      (Eq. 14)
-// phi is evaluated by Horner for u <= 1/2 and as 1 - phi(1-u) above (symmetric weight).
+// Korobov transform, Eq. 15, weights (r0, r1):
+//   omega(u) = (r0+r1+1) C(r0+r1,r0) u^r0 (1-u)^r1,
+//   phi(u) = int_0^u omega = c sum_{i=0}^{r1} C(r1,i) (-1)^i u^{r0+1+i} / (r0+1+i)      (Eq. 14, binomial expansion)
+// phi is evaluated by Horner for u <= 1/2 and as 1 - phi_{r1,r0}(1-u) above (int_u^1 omega_{r0,r1} = int_0^{1-u} omega_{r1,r0}).
 struct Korobov {
-    int r; double c; double coef[8];
-    explicit Korobov(int r_) : r(r_) {
-        c = (2.0 * r + 1.0) * binom(2 * r, r);
-        for (int i = 0; i <= r; ++i) coef[i] = c * binom(r, i) * ((i & 1) ? -1.0 : 1.0) / (double)(r + 1 + i);
+    int r0, r1; double c; double lo[8], hi[8];
+    explicit Korobov(int r) : Korobov(r, r) {}
+    Korobov(int r0_, int r1_) : r0(r0_), r1(r1_) {
+        c = (double)(r0 + r1 + 1) * binom(r0 + r1, r0);
+        for (int i = 0; i <= r1; ++i) lo[i] = c * binom(r1, i) * ((i & 1) ? -1.0 : 1.0) / (double)(r0 + 1 + i);
+        for (int i = 0; i <= r0; ++i) hi[i] = c * binom(r0, i) * ((i & 1) ? -1.0 : 1.0) / (double)(r1 + 1 + i);
     }
-    double phi_low(double u) const {
-        double h = coef[r];
-        for (int i = r - 1; i >= 0; --i) h = h * u + coef[i];
-        double p = 1.0; for (int i = 0; i <= r; ++i) p *= u;     // u^(r+1)
+    static double series(const double* coef, int deg, int lead, double u) {   // u^(lead+1) * Horner(coef[0..deg], u)
+        double h = coef[deg];
+        for (int i = deg - 1; i >= 0; --i) h = h * u + coef[i];
+        double p = 1.0; for (int i = 0; i <= lead; ++i) p *= u;
         return p * h;
     }
-    double phi(double u) const { return u <= 0.5 ? phi_low(u) : 1.0 - phi_low(1.0 - u); }
+    double phi(double u) const { return u <= 0.5 ? series(lo, r1, r0, u) : 1.0 - series(hi, r0, r1, 1.0 - u); }
     double omega(double u) const {
-        double p = 1.0; for (int i = 0; i < r; ++i) p *= u * (1.0 - u);
+        double p = 1.0;
+        for (int i = 0; i < r0; ++i) p *= u;
+        for (int i = 0; i < r1; ++i) p *= 1.0 - u;
         return c * p;
     }
 };
 
+// Sidi transform of weight r, Eq. 16: omega(u) = K_r sin^r(pi u), K_r = pi/2^r Gamma(r+1)/Gamma((r+1)/2)^2;
+// phi = int_0^u omega written out per r (s = sin pi u, c = cos pi u):
+//   r=1  (1-c)/2                         r=2  u - sin(2 pi u)/(2 pi)
+//   r=3  (2 - 3c + c^3)/4                r=4  u - 2 sin(2 pi u)/(3 pi) + sin(4 pi u)/(12 pi)
+//   r=5  1/2 - 15c/16 + 5c^3/8 - 3c^5/16 r=6  u - 3 sin(2 pi u)/(4 pi) + 3 sin(4 pi u)/(20 pi) - sin(6 pi u)/(60 pi)
+struct Sidi {
+    int r; double K;
+    explicit Sidi(int r_) : r(r_) { double g = std::tgamma(0.5 * (r + 1)); K = M_PI / std::ldexp(1.0, r) * std::tgamma(r + 1.0) / (g * g); }
+    double omega(double u) const { double s = std::sin(M_PI * u), p = 1.0; for (int i = 0; i < r; ++i) p *= s; return K * p; }
+    double phi(double u) const {
+        const double t = M_PI * u, c = std::cos(t);
+        switch (r) {
+            case 1: return 0.5 * (1.0 - c);
+            case 2: return u - std::sin(2.0 * t) / (2.0 * M_PI);
+            case 3: return 0.25 * (2.0 - 3.0 * c + c * c * c);
+            case 4: return u - 2.0 * std::sin(2.0 * t) / (3.0 * M_PI) + std::sin(4.0 * t) / (12.0 * M_PI);
+            case 5: return 0.5 - 15.0 * c / 16.0 + 5.0 * c * c * c / 8.0 - 3.0 * c * c * c * c * c / 16.0;
+            default: return u - 3.0 * std::sin(2.0 * t) / (4.0 * M_PI) + 3.0 * std::sin(4.0 * t) / (20.0 * M_PI) - std::sin(6.0 * t) / (60.0 * M_PI);
+        }
+    }
+};
+
+// decoded transform of a call
+struct Transform {
+    int kind;                 // 0 none, 1 baker, 2 Korobov (any weights), 3 Sidi
+    Korobov kor; Sidi sidi;
+    Transform() : kind(0), kor(1), sidi(1) {}
+};
+inline bool decode_transform(int tr, Transform* t) {
+    if (tr == TR_NONE) { t->kind = 0; return true; }
+    if (tr == TR_BAKER) { t->kind = 1; return true; }
+    if (tr >= TR_KOROBOV + 1 && tr <= TR_KOROBOV + 6) { t->kind = 2; t->kor = Korobov(tr - TR_KOROBOV); return true; }
+    if (tr >= TR_SIDI + 1 && tr <= TR_SIDI + 6) { t->kind = 3; t->sidi = Sidi(tr - TR_SIDI); return true; }
+    if (tr >= TR_KOROBOV_ASYM) {
+        const int r0 = (tr - TR_KOROBOV_ASYM) / 16, r1 = (tr - TR_KOROBOV_ASYM) % 16;
+        if (r0 >= 1 && r0 <= 6 && r1 >= 1 && r1 <= 6) { t->kind = 2; t->kor = Korobov(r0, r1); return true; }
+    }
+    return false;
+}
+
 // O3
-inline void transform(int tr, const Korobov* kor, double u, double* y, double* w) {
-    if (tr == TR_NONE) { *y = u; *w = 1.0; }
-    else if (tr == TR_BAKER) { *y = 1.0 - std::fabs(2.0 * u - 1.0); *w = 1.0; }   // Eq. 17
-    else { *y = kor->phi(u); *w = kor->omega(u); }
+inline void transform(const Transform& tr, double u, double* y, double* w) {
+    if (tr.kind == 0) { *y = u; *w = 1.0; }
+    else if (tr.kind == 1) { *y = 1.0 - std::fabs(2.0 * u - 1.0); *w = 1.0; }     // Eq. 17
+    else if (tr.kind == 2) { *y = tr.kor.phi(u); *w = tr.kor.omega(u); }          // Eq. 15
+    else { *y = tr.sidi.phi(u); *w = tr.sidi.omega(u); }                          // Eq. 16
 }
 
 // O4: Eq. 19 and its derivative; a[0..5] = a_0..a_5, a6 = 1 - a2 - a3 - a4 - a5.
@@ -165,11 +211,11 @@ int expected_params(int fam, const double* p, int dim) {
 
 // One lattice point for one shift: O2-O5.  Returns v = W * f (re, im).
 inline void eval_point(int fam, const double* params, int dim, const uint64_t* r, double inv_n, const double* shift,
-                       int tr, const Korobov* kor, const double* fit, double* re, double* im) {
+                       const Transform& tr, const double* fit, double* re, double* im) {
     double x[MAX_DIM]; double W = 1.0;
     for (int j = 0; j < dim; ++j) {
         double u = coordinate(r[j], inv_n, shift[j]);
-        double y, w; transform(tr, kor, u, &y, &w);
+        double y, w; transform(tr, u, &y, &w);
         if (fit) { double xx, dp; fit_map(fit + 6 * j, y, &xx, &dp); y = xx; w *= dp; }
         x[j] = y; W *= w;
     }
@@ -204,9 +250,10 @@ int oracle_lattice_points(uint64_t n, int dim, const uint64_t* z, const double* 
 
 // Per-coordinate transform (O3) exposed for the pins.
 int oracle_transform(int tr, double u, double* y, double* w) {
-    if (tr >= TR_KOROBOV + 1 && tr <= TR_KOROBOV + 6) { Korobov k(tr - TR_KOROBOV); transform(tr, &k, u, y, w); return 0; }
-    if (tr == TR_NONE || tr == TR_BAKER) { transform(tr, nullptr, u, y, w); return 0; }
-    return -7;
+    Transform t;
+    if (!decode_transform(tr, &t)) return -7;
+    transform(t, u, y, w);
+    return 0;
 }
 
 int oracle_fit_map(const double* a, double y, double* x, double* dp) { fit_map(a, y, x, dp); return 0; }
@@ -226,10 +273,9 @@ int oracle_shift_sums(int fam, const double* params, int n_params, int dim, uint
     if (fam < 0 || fam > 3) return -8;
     if (dim < 1 || dim > MAX_DIM) return -2;
     if (expected_params(fam, params, dim) != n_params) return -9;
-    bool kor_tr = tr >= TR_KOROBOV + 1 && tr <= TR_KOROBOV + 6;
-    if (!(tr == TR_NONE || tr == TR_BAKER || kor_tr)) return -7;
+    Transform trf;
+    if (!decode_transform(tr, &trf)) return -7;
     if (k_end > n || k_begin > k_end) return -3;
-    Korobov kor(kor_tr ? tr - TR_KOROBOV : 1);
     const int nc = ncomp_of(fam);
     const double inv_n = 1.0 / (double)n;
     const uint64_t c0 = k_begin / CHUNK, c1 = (k_end + CHUNK - 1) / CHUNK;
@@ -246,7 +292,7 @@ int oracle_shift_sums(int fam, const double* params, int n_params, int dim, uint
             for (int j = 0; j < dim; ++j) r[j] = residue(k, z[j], n);
             for (int s = 0; s < m; ++s) {
                 double re, im;
-                eval_point(fam, params, dim, r, inv_n, shifts + (size_t)s * dim, tr, &kor, fit, &re, &im);
+                eval_point(fam, params, dim, r, inv_n, shifts + (size_t)s * dim, trf, fit, &re, &im);
                 acc[(size_t)s * nc].add(re);
                 if (nc == 2) acc[(size_t)s * nc + 1].add(im);
             }
