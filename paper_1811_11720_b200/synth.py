@@ -19,6 +19,8 @@ import numpy as np
 
 FAMILY_GENZ_OSC, FAMILY_GENZ_PRODPEAK, FAMILY_CEXP_POLY, FAMILY_SECTOR = 0, 1, 2, 3
 TRANSFORM_NONE, TRANSFORM_BAKER, TRANSFORM_KOROBOV = 0, 1, 100      # Korobov weight r = 100 + r
+TRANSFORM_SIDI = 200                                                # Sidi weight r = 200 + r
+TRANSFORM_KOROBOV_ASYM = 1000                                       # Korobov weights (r0, r1) = 1000 + 16 r0 + r1
 
 _DATA = os.path.join(os.path.dirname(os.path.abspath(__file__)), "data", "genvecs.json")
 

@@ -102,6 +102,61 @@ def test_korobov_normalisation_and_phi(r):
         assert abs(quad - oracle.transform(synth.TRANSFORM_KOROBOV + r, u)[0]) < 1e-14
 
 
+@pytest.mark.parametrize("r0,r1", [(1, 2), (2, 1), (3, 1), (1, 4), (5, 3), (2, 6), (6, 6), (4, 4)])
+def test_korobov_asymmetric_is_the_incomplete_beta(r0, r1):
+    # Eq. 15: omega = u^r0 (1-u)^r1 / B(r0+1, r1+1); Eq. 14: phi = I_u(r0+1, r1+1); Korobov<5,3> is the paper's example
+    tr = synth.TRANSFORM_KOROBOV_ASYM + 16 * r0 + r1
+    c = 1.0 / scipy.special.beta(r0 + 1, r1 + 1)
+    assert abs(c - (r0 + r1 + 1) * math.comb(r0 + r1, r0)) < 1e-9 * c
+    for u in [0.0, 1e-7, 0.02, 0.3, 0.5, 0.50001, 0.8, 0.9999, 1.0 - 2.0 ** -53]:
+        y, w = oracle.transform(tr, u)
+        want = scipy.special.betainc(r0 + 1, r1 + 1, u)
+        assert abs(y - want) <= 8e-15 * want + 1e-300 or abs(y - want) < 2e-16
+        assert abs(w - c * u ** r0 * (1 - u) ** r1) <= 1e-14 * c
+        ym, _ = oracle.transform(synth.TRANSFORM_KOROBOV_ASYM + 16 * r1 + r0, 1.0 - u)   # mirror symmetry
+        assert abs(y + ym - 1.0) < 1e-15
+    if r0 == r1:                                            # the symmetric id is the same transform
+        for u in [0.1, 0.5, 0.9]:
+            assert oracle.transform(tr, u) == oracle.transform(synth.TRANSFORM_KOROBOV + r0, u)
+    for bad in (synth.TRANSFORM_KOROBOV_ASYM + 16 * 0 + 3, synth.TRANSFORM_KOROBOV_ASYM + 16 * 7 + 1, synth.TRANSFORM_KOROBOV_ASYM + 16 * 2 + 9):
+        with pytest.raises(ValueError):
+            oracle.transform(bad, 0.5)
+
+
+@pytest.mark.parametrize("r", [1, 2, 3, 4, 5, 6])
+def test_sidi_normalisation_and_phi(r):
+    # Eq. 16: omega = K_r sin^r(pi u), K_r = pi/2^r Gamma(r+1)/Gamma((r+1)/2)^2 = 1 / int_0^1 sin^r(pi t) dt
+    tr = synth.TRANSFORM_SIDI + r
+    K = math.pi / 2 ** r * math.gamma(r + 1) / math.gamma((r + 1) / 2) ** 2
+    assert abs(K - {1: math.pi / 2, 2: 2.0, 3: 3 * math.pi / 4, 4: 8 / 3, 5: 15 * math.pi / 16, 6: 16 / 5}[r]) < 1e-14 * K
+    norm, _ = scipy.integrate.quad(lambda t: math.sin(math.pi * t) ** r, 0.0, 1.0, epsabs=1e-13, epsrel=1e-13)
+    assert abs(K * norm - 1.0) < 1e-13
+    assert oracle.transform(tr, 0.0)[0] == 0.0 and abs(oracle.transform(tr, 0.0)[1]) < 1e-15
+    assert abs(oracle.transform(tr, 1.0 - 2.0 ** -53)[0] - 1.0) < 1e-15
+    assert abs(oracle.transform(tr, 0.5)[0] - 0.5) < 1e-15 and abs(oracle.transform(tr, 0.5)[1] - K) < 1e-14 * K
+    xs, ws = np.polynomial.legendre.leggauss(40)
+    for u in [0.003, 0.2, 0.45, 0.6, 0.95, 0.999]:
+        y, w = oracle.transform(tr, u)
+        assert abs(w - K * math.sin(math.pi * u) ** r) <= 1e-14 * K
+        t = 0.5 * u * (xs + 1.0)                             # phi = int_0^u omega (Eq. 14) by Gauss-Legendre
+        quad = 0.5 * u * np.sum(ws * K * np.sin(np.pi * t) ** r)
+        assert abs(quad - y) < 1e-14
+        y2, _ = oracle.transform(tr, 1.0 - u)
+        assert abs(y + y2 - 1.0) < 2e-15
+    with pytest.raises(ValueError):
+        oracle.transform(synth.TRANSFORM_SIDI + 7, 0.5)
+
+
+@pytest.mark.parametrize("tr,rel", [(synth.TRANSFORM_SIDI + 2, 3e-6), (synth.TRANSFORM_SIDI + 3, 3e-7),
+                                    (synth.TRANSFORM_KOROBOV_ASYM + 16 * 3 + 2, 1e-5), (synth.TRANSFORM_KOROBOV_ASYM + 16 * 1 + 4, 1e-3)])
+def test_new_transforms_leave_the_integral_invariant(tr, rel):
+    """Eq. 12: the transformed rule still integrates f; closed form of Genz oscillatory"""
+    rng = synth.MT19937_64(2024)
+    prm = synth.genz_osc(rng, 4)
+    p = synth.problem(0, prm, 8191, synth.genvec(65537, 4) % 8191, synth.draw_shifts(rng, 8, 4), tr)
+    _check_vs_exact(p, closed_osc(prm), rel=rel)
+
+
 def test_baker_and_none():
     # Eq. 17 (P:L206): 2u below 1/2, 2-2u above; weight 1 (P:L209)
     for u, y in [(0.0, 0.0), (0.25, 0.5), (0.5, 1.0), (0.75, 0.5), (0.9, 0.2)]:
