@@ -66,8 +66,11 @@ typedef enum {
 enum { QMC_FAMILY_GENZ_OSC = 0, QMC_FAMILY_GENZ_PRODPEAK = 1, QMC_FAMILY_CEXP_POLY = 2, QMC_FAMILY_SECTOR = 3 };
 
 /* Periodizing transforms, Table A.2: none; baker Eq. 17;
- * Korobov with symmetric weight r, Eq. 15: QMC_TRANSFORM_KOROBOV + r, r = 1..6. */
-enum { QMC_TRANSFORM_NONE = 0, QMC_TRANSFORM_BAKER = 1, QMC_TRANSFORM_KOROBOV = 100 };
+ * Korobov with symmetric weight r, Eq. 15: QMC_TRANSFORM_KOROBOV + r, r = 1..6;
+ * Sidi with weight r, Eq. 16: QMC_TRANSFORM_SIDI + r, r = 1..6;
+ * Korobov with weights (r0, r1), Eq. 15: QMC_TRANSFORM_KOROBOV_ASYM + 16 r0 + r1, r0, r1 = 1..6 (Korobov<5,3>). */
+enum { QMC_TRANSFORM_NONE = 0, QMC_TRANSFORM_BAKER = 1, QMC_TRANSFORM_KOROBOV = 100, QMC_TRANSFORM_SIDI = 200,
+       QMC_TRANSFORM_KOROBOV_ASYM = 1000 };
 
 enum { QMC_MAX_DIM = 32, QMC_MAX_M = 4096 };
 

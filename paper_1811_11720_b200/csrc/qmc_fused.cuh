@@ -38,7 +38,7 @@ template <int DP, int G> struct alignas(16) SmemCtx {
                                    // the problem when they fit, else only the current group
     double fam[DP * 2];            // [j] = (fam_a, fam_b)
     double fit[DP * 6];            // [j] = (a4, a5, a6, 2 a5, 3 a6, -)  cubic map of Eq. 19
-    double kor[8];                 // centred Korobov polynomial g_r
+    double kor[16];                // transform tables (DevProblem::kor)
     unsigned long long step[DP], back[DP], z[DP];
     double red[2][kWarps][G * 2];  // double-buffered by group parity
     DevProblem prob;
@@ -50,7 +50,7 @@ template <int DP, int G> struct SmemOff {
     static constexpr unsigned fam = delta + ((DP * G > kDeltaCache) ? DP * G : kDeltaCache) * 8;
     static constexpr unsigned fit = fam + DP * 2 * 8;
     static constexpr unsigned kor = fit + DP * 6 * 8;
-    static constexpr unsigned step = kor + 8 * 8;
+    static constexpr unsigned step = kor + 16 * 8;
 };
 
 // ---- per-dimension and per-point pieces of the closed-form families (S5) ----------------------
@@ -87,6 +87,52 @@ template <int FAMILY> __device__ __forceinline__ void fam_finish(double s0, doub
 // ---- S2-S4 for one (shift q, dimension j): coordinate, periodizing transform, fit map ----------
 struct FitC { double f0, f1, f2, f3, f4; };       // a4, a5, a6, 2 a5, 3 a6 of one dimension
 
+// The generic weight transforms (Table A.2), selected per coordinate by the warp-uniform code
+// gen = kind | r0 << 4 | r1 << 8; P is multiplied by omega(u) / normalisation (the constant is in wconst).
+//   GEN_KOROBOV_SYM   Eq. 15, r0 = r1 = r: phi = 1/2 + c g_r(c^2), omega ~ (1/4 - c^2)^r
+//   GEN_KOROBOV_ASYM  Eq. 15, r0 != r1: phi(u) = u^(r0+1) A(u) below 1/2, 1 - v^(r1+1) B(v), v = 1 - u, above
+//                     (int_u^1 omega_{r0,r1} = int_0^{1-u} omega_{r1,r0}); tables zero padded to degree 6
+//   GEN_SIDI          Eq. 16: omega ~ sin^r(pi u), phi = (K_r / pi) I_r(pi u) with the reduction
+//                     I_n = ((n-1) I_{n-2} - sin^(n-1) cos) / n, I_0 = theta, I_1 = 1 - cos
+__device__ __forceinline__ double generic_transform(double t, unsigned kor_addr, int gen, double& P) {
+    const int kind = gen & 15, r0 = (gen >> 4) & 15, r1 = (gen >> 8) & 15;
+    if (kind == GEN_KOROBOV_SYM) {
+        const double c = centre_c(t);
+        const double s = c * c;
+        P *= ipow_small(0.25 - s, r0);
+        double g = lds_f64(kor_addr + 8u * (unsigned)r0);
+#pragma unroll 1
+        for (int i = r0 - 1; i >= 0; --i) g = __fma_rn(g, s, lds_f64(kor_addr + 8u * (unsigned)i));
+        return __fma_rn(c, g, 0.5);
+    }
+    const double u = wrap_u(t);
+    if (kind == GEN_KOROBOV_ASYM) {
+        const double um = 1.0 - u;
+        const bool low = u <= 0.5;
+        const double v = low ? u : um;
+        const unsigned tab = kor_addr + (low ? 0u : 64u);
+        double h = lds_f64(tab + 48u);
+#pragma unroll 1
+        for (int i = 5; i >= 0; --i) h = __fma_rn(h, v, lds_f64(tab + 8u * (unsigned)i));
+        const double ph = ipow_small(v, (low ? r0 : r1) + 1) * h;
+        P *= ipow_small(u, r0) * ipow_small(um, r1);
+        return low ? ph : 1.0 - ph;
+    }
+    double s, c;
+    sincospi(u, &s, &c);
+    const bool even = (r0 & 1) == 0;
+    double I = even ? 3.141592653589793238462643383279 * u : 1.0 - c;
+    double sp = even ? s : s * s;                             // sin^(n-1) for the first reduction step
+    const double s2 = s * s;
+#pragma unroll 1
+    for (int n = even ? 2 : 3; n <= r0; n += 2) {
+        I = __ddiv_rn(__fma_rn((double)(n - 1), I, -(sp * c)), (double)n);
+        sp *= s2;
+    }
+    P *= ipow_small(s, r0);
+    return lds_f64(kor_addr) * I;
+}
+
 // Returns x_j; multiplies P by u(1-u) (Korobov) and D by p'(y) (fit).
 template <int TR, bool FIT>
 __device__ __forceinline__ double point_coord(double rd, double inv_n, double delta, const FitC& fc, unsigned kor_addr,
@@ -98,21 +144,16 @@ __device__ __forceinline__ double point_coord(double rd, double inv_n, double de
     } else {
         if (TR == TR_BAKER) {
             x = 1.0 - fabs(baker_w(t));                       // Eq. 17: the tent map is even about u = 1/2, no wrap decision needed
-        } else {
+        } else if (TR == TR_KOR3) {
             const double c = centre_c(t);
             const double s = c * c;
             P *= (0.25 - s);                                  // u (1-u)
-            double g;
-            if (TR == TR_KOR3) {                              // g_3(s) = 35/16 - 35/4 s + 21 s^2 - 20 s^3
-                g = __fma_rn(-20.0, s, 21.0);
-                g = __fma_rn(g, s, -8.75);
-                g = __fma_rn(g, s, 2.1875);
-            } else {
-                g = lds_f64(kor_addr + 8u * (unsigned)kor_r);
-#pragma unroll 1
-                for (int i = kor_r - 1; i >= 0; --i) g = __fma_rn(g, s, lds_f64(kor_addr + 8u * (unsigned)i));
-            }
+            double g = __fma_rn(-20.0, s, 21.0);              // g_3(s) = 35/16 - 35/4 s + 21 s^2 - 20 s^3
+            g = __fma_rn(g, s, -8.75);
+            g = __fma_rn(g, s, 2.1875);
             x = __fma_rn(c, g, 0.5);                          // phi(u) = 1/2 + c g(c^2)
+        } else {
+            x = generic_transform(t, kor_addr, kor_r, P);
         }
     }
     if (FIT) {                                                // S4: cubic map of Eq. 19 (a2 = a3 = 0)
@@ -128,7 +169,7 @@ __device__ __forceinline__ double point_coord(double rd, double inv_n, double de
 template <int TR, bool FIT> __device__ __forceinline__ double point_weight(double P, double D, double wconst, int kor_r) {
     double W = 1.0;
     if (TR == TR_KOR3) W = wconst * (P * P * P);
-    else if (TR == TR_KORR) W = wconst * ipow_small(P, kor_r);
+    else if (TR == TR_KORR) W = wconst * P;                  // generic transforms carry the full weight product
     if (FIT) W = (TR == TR_KOR3 || TR == TR_KORR) ? W * D : D;
     return W;
 }
@@ -157,7 +198,7 @@ struct EvalCtx {            // per-tile constants held in registers
     unsigned sbase;         // shared address of the CTA's SmemCtx
     unsigned delta;         // shared address of the current group's shifts
     double inv_n, wconst, fam0;
-    int kor_r;
+    int kor_r;              // generic weight transforms: DevProblem::gen
     int sel;                // tr_kind * 2 + has_fit
 };
 
@@ -215,7 +256,7 @@ __device__ __forceinline__ void run_tile(SmemCtx<DP, G>& sm, unsigned sbase, con
     const int dim = pb.dim, m = pb.m, steps = pb.steps;
     const unsigned long long n = pb.n;
     EvalCtx cx;
-    cx.sbase = sbase; cx.inv_n = pb.inv_n; cx.wconst = pb.wconst; cx.fam0 = sm.fam0; cx.kor_r = pb.kor_r;
+    cx.sbase = sbase; cx.inv_n = pb.inv_n; cx.wconst = pb.wconst; cx.fam0 = sm.fam0; cx.kor_r = pb.gen;
     cx.sel = pb.tr_kind * 2 + (pb.has_fit ? 1 : 0);
     typedef SmemCtx<DP, G> Ctx;
     typedef SmemOff<DP, G> Off;
@@ -387,7 +428,7 @@ __device__ __forceinline__ bool next_tile(SmemCtx<DP, G>& sm, const FusedLaunch&
         changed = true;
         const DevProblem& src = L.single ? L.one : L.probs[pidx];
         if (tid == 0) sm.prob = src;
-        if (tid >= 64 && tid < 72) sm.kor[tid - 64] = src.kor[tid - 64];
+        if (tid >= 64 && tid < 80) sm.kor[tid - 64] = src.kor[tid - 64];
         if (SECTOR) {
             const DevAux& a = L.aux[pidx];
             if (tid == 32) sm.fam0 = a.fam0;
@@ -410,6 +451,15 @@ __device__ __forceinline__ bool next_tile(SmemCtx<DP, G>& sm, const FusedLaunch&
             }
         }
         __syncthreads();
+        // product peak under a generic weight transform: a padded slot must see x - fb = 0, and phi(1/2) is not 1/2 for
+        // asymmetric weights -- take it from the same device function the point block calls (bit-identical)
+        if (!SECTOR && src.family == QMC_FAMILY_GENZ_PRODPEAK && src.tr_kind == TR_KORR && src.dim < DP) {
+            if (tid >= src.dim && tid < DP) {
+                double Pdummy = 1.0;
+                sm.fam[2 * tid + 1] = generic_transform(0.5, (unsigned)__cvta_generic_to_shared(&sm) + SmemOff<DP, G>::kor, src.gen, Pdummy);
+            }
+            __syncthreads();
+        }
     }
     return true;
 }

@@ -52,15 +52,34 @@ int dim_slots(int family, int dim, bool wide) {
 bool force_wide();
 bool is_wide(unsigned long long n) { return n >= (1ull << 31) || force_wide(); }
 
-bool decode_transform(int transform, int* kind, int* r) {
-    if (transform == QMC_TRANSFORM_NONE) { *kind = TR_NONE; *r = 0; return true; }
-    if (transform == QMC_TRANSFORM_BAKER) { *kind = TR_BAKER; *r = 0; return true; }
-    if (transform >= QMC_TRANSFORM_KOROBOV + 1 && transform <= QMC_TRANSFORM_KOROBOV + 6) {
+// transform id -> tile-loop kind, symmetric Korobov weight r (0 if none) and the generic-transform code
+// gen = GEN_* | r0 << 4 | r1 << 8 (Table A.2)
+bool decode_transform(int transform, int* kind, int* r, int* gen = nullptr) {
+    int g = 0;
+    bool ok = false;
+    *r = 0;
+    if (transform == QMC_TRANSFORM_NONE) { *kind = TR_NONE; ok = true; }
+    else if (transform == QMC_TRANSFORM_BAKER) { *kind = TR_BAKER; ok = true; }
+    else if (transform >= QMC_TRANSFORM_KOROBOV + 1 && transform <= QMC_TRANSFORM_KOROBOV + 6) {
         *r = transform - QMC_TRANSFORM_KOROBOV;
         *kind = (*r == 3) ? TR_KOR3 : TR_KORR;
-        return true;
+        g = GEN_KOROBOV_SYM | (*r << 4) | (*r << 8);
+        ok = true;
+    } else if (transform >= QMC_TRANSFORM_SIDI + 1 && transform <= QMC_TRANSFORM_SIDI + 6) {
+        *kind = TR_KORR;
+        g = GEN_SIDI | ((transform - QMC_TRANSFORM_SIDI) << 4);
+        ok = true;
+    } else if (transform >= QMC_TRANSFORM_KOROBOV_ASYM) {
+        const int r0 = (transform - QMC_TRANSFORM_KOROBOV_ASYM) / 16, r1 = (transform - QMC_TRANSFORM_KOROBOV_ASYM) % 16;
+        if (r0 >= 1 && r0 <= 6 && r1 >= 1 && r1 <= 6) {
+            if (r0 == r1) return decode_transform(QMC_TRANSFORM_KOROBOV + r0, kind, r, gen);
+            *kind = TR_KORR;
+            g = GEN_KOROBOV_ASYM | (r0 << 4) | (r1 << 8);
+            ok = true;
+        }
     }
-    return false;
+    if (gen) *gen = (ok && *kind == TR_KORR) ? g : 0;
+    return ok;
 }
 
 double binom(int a, int b) {
@@ -136,11 +155,12 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
         d.n = p.n;
         d.inv_n = 1.0 / (double)p.n;                                   // reading C-2
         d.family = p.family; d.dim = p.dim; d.m = p.m; d.ncomp = ncomp_of(p.family);
-        decode_transform(p.transform, &d.tr_kind, &d.kor_r);
+        decode_transform(p.transform, &d.tr_kind, &d.kor_r, &d.gen);
         d.has_fit = p.fit_coeffs ? 1 : 0;
         d.n_params = p.n_params;
         d.out_index = i;
         d.wconst = 1.0;
+        const int npad = dim_slots(p.family, p.dim, is_wide(p.n)) - p.dim;   // padded dimension slots sit at u = 1/2 (qmc_fused.cuh)
         if (d.kor_r > 0) {
             // Eq. 15: c_r = (2r+1) C(2r,r); centred antiderivative coefficients of Eq. 14 (see qmc_device.cuh)
             const int r = d.kor_r;
@@ -148,8 +168,22 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
             for (int k = 0; k <= r; ++k)
                 d.kor[k] = cr * binom(r, k) * std::ldexp(1.0, 2 * (k - r)) * ((k & 1) ? -1.0 : 1.0) / (double)(2 * k + 1);
             for (int j = 0; j < p.dim; ++j) d.wconst *= cr;
-            // padded dimension slots contribute u(1-u) = 1/4 each to the weight product (qmc_fused.cuh): exact compensation
-            d.wconst = std::ldexp(d.wconst, 2 * r * (dim_slots(p.family, p.dim, is_wide(p.n)) - p.dim));
+            d.wconst = std::ldexp(d.wconst, 2 * r * npad);               // a padded slot contributes (1/4)^r: exact compensation
+        } else if ((d.gen & 15) == GEN_KOROBOV_ASYM) {
+            // Eq. 15 with r0 != r1: c = (r0+r1+1) C(r0+r1,r0); phi(u) = c sum_i C(r1,i)(-1)^i u^(r0+1+i)/(r0+1+i) (Eq. 14)
+            const int r0 = (d.gen >> 4) & 15, r1 = (d.gen >> 8) & 15;
+            const double c = (double)(r0 + r1 + 1) * binom(r0 + r1, r0);
+            for (int k = 0; k <= r1; ++k) d.kor[k] = c * binom(r1, k) * ((k & 1) ? -1.0 : 1.0) / (double)(r0 + 1 + k);
+            for (int k = 0; k <= r0; ++k) d.kor[8 + k] = c * binom(r0, k) * ((k & 1) ? -1.0 : 1.0) / (double)(r1 + 1 + k);
+            for (int j = 0; j < p.dim; ++j) d.wconst *= c;
+            d.wconst = std::ldexp(d.wconst, (r0 + r1) * npad);           // a padded slot contributes (1/2)^(r0+r1)
+        } else if ((d.gen & 15) == GEN_SIDI && d.gen) {
+            // Eq. 16: K_r = pi / 2^r Gamma(r+1) / Gamma((r+1)/2)^2; a padded slot has sin(pi/2)^r = 1
+            const int r = (d.gen >> 4) & 15;
+            const double gh = std::tgamma(0.5 * (r + 1));
+            const double K = 3.141592653589793238462643383279 / std::ldexp(1.0, r) * std::tgamma(r + 1.0) / (gh * gh);
+            d.kor[0] = K / 3.141592653589793238462643383279;
+            for (int j = 0; j < p.dim; ++j) d.wconst *= K;
         }
         if (p.family == QMC_FAMILY_SECTOR) {
             const int nmono = (p.n_params - 4 - p.dim) / (1 + p.dim);

@@ -28,7 +28,9 @@ constexpr int kSectorLinSlots = 32;    // extra coefficient slots of a sector pr
 __host__ __device__ constexpr int sector_coef_slots(int nmono) { return nmono + kSectorLinSlots; }   // coefficient region of a program, in doubles
 
 // transform kinds after host-side decoding
-enum : int { TR_NONE = 0, TR_BAKER = 1, TR_KOR3 = 2, TR_KORR = 3 };
+enum : int { TR_NONE = 0, TR_BAKER = 1, TR_KOR3 = 2, TR_KORR = 3 };   // TR_KORR = the generic weight transforms, see GEN_*
+// generic weight transforms (one tile loop, selected per coordinate by DevProblem::gen = kind | r0 << 4 | r1 << 8):
+enum : int { GEN_KOROBOV_SYM = 0, GEN_KOROBOV_ASYM = 1, GEN_SIDI = 2 };
 
 // Device-resident description of one problem (built on the host, copied into the workspace).
 struct alignas(16) DevProblem {
@@ -39,7 +41,9 @@ struct alignas(16) DevProblem {
     unsigned long long n;
     double inv_n;              // fl(1/double(n))  (reading C-2)
     double wconst;             // Korobov: c_r^dim ; else 1
-    double kor[8];             // centred Korobov polynomial g_r coefficients (degree r in s=c^2), kor[i], i<=r
+    double kor[16];            // transform tables: symmetric Korobov: centred polynomial g_r, kor[i], i <= r (degree r in c^2);
+                               // asymmetric Korobov: kor[0..7] = phi series below 1/2, kor[8..15] = mirrored series above
+                               // (zero padded to degree 6); Sidi: kor[0] = K_r / pi
     long long partial_off;     // offset in doubles into the partial-sum area
     long long means_off;       // offset in doubles into the per-shift means area
     long long tile_begin;      // first tile index (within this problem's kernel variant queue)
@@ -48,13 +52,13 @@ struct alignas(16) DevProblem {
     int steps;                 // I: lattice indices per thread per tile; tile length = steps*kThreads
     int family, dim, m, ncomp;
     int tr_kind;               // TR_*
-    int kor_r;                 // Korobov weight r (1..6) or 0
+    int kor_r;                 // symmetric Korobov weight r (1..6) or 0
     int has_fit;               // 0 none, 1 cubic
     int n_params;
     int aux_off;               // sector: offset (in 8-byte words) of the compiled program in the aux area
     int aux_len;
     int out_index;             // index of the problem in the caller's arrays
-    int pad_;
+    int gen;                   // generic weight transform: GEN_* | r0 << 4 | r1 << 8 (0 otherwise)
 };
 
 // Per-problem tables derived on the device by prepare_kernel (one record per problem).

@@ -128,8 +128,12 @@ def test_points_empty_window():
 # ------------------------------------------------------------------------------------------------
 # S1-S8: per-shift means, estimate and error for every family x transform x fit
 # ------------------------------------------------------------------------------------------------
+SIDI, KA = synth.TRANSFORM_SIDI, synth.TRANSFORM_KOROBOV_ASYM
+
+
 @pytest.mark.parametrize("fam", [0, 1, 2, 3])
-@pytest.mark.parametrize("tr", [NONE, BAKER, K + 1, K + 2, K + 3, K + 4, K + 5, K + 6])
+@pytest.mark.parametrize("tr", [NONE, BAKER, K + 1, K + 2, K + 3, K + 4, K + 5, K + 6, SIDI + 1, SIDI + 2, SIDI + 3, SIDI + 4, SIDI + 5,
+                                SIDI + 6, KA + 16 * 2 + 1, KA + 16 * 5 + 3, KA + 16 * 1 + 4, KA + 16 * 3 + 6, KA + 16 * 4 + 4])
 def test_means_all_transforms(fam, tr):
     d = {0: 5, 1: 3, 2: 7, 3: 6}[fam]
     probs = [make(fam, d, 8191, 6, tr, 300 + 10 * fam + tr % 97, fit=False),
