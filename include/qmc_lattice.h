@@ -24,7 +24,8 @@
  *  - z[j], j < dim: generating vector, 1 <= z_j < n, gcd(z_j, n) = 1 ("coprime to n");
  *  - shifts[s*dim + j] in [0,1): shift s, dimension j (Delta_k of Eq. 2);
  *  - fit_coeffs[j*6 + i] = a_i of Eq. 19 for dimension j, a_6 := 1-a_2-a_3-a_4-a_5
- *    (cubic map <=> a_2 = a_3 = 0; then a_0, a_1 are ignored); NULL = no fit map;
+ *    (cubic map <=> a_2 = a_3 = 0; then a_0, a_1 are ignored; with pole terms a_0 >= 1.001, a_1 <= -0.001, a_2, a_3 >= 0,
+ *    P:L231); the map must be increasing on [0,1]; NULL = no fit map;
  *  - complex results are interleaved (re, im);
  *  - params: packed per family, all doubles (small integers stored as exact doubles):
  *      QMC_FAMILY_GENZ_OSC      [u0, a_1..a_d]            f = cos(2 pi u0 + sum a_j x_j)

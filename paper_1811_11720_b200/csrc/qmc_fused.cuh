@@ -37,19 +37,20 @@ template <int DP, int G> struct alignas(16) SmemCtx {
     double delta[(DP * G > kDeltaCache) ? DP * G : kDeltaCache];   // [group][j][q] shifts (1/2 in padded slots): all groups of
                                    // the problem when they fit, else only the current group
     double fam[DP * 2];            // [j] = (fam_a, fam_b)
-    double fit[DP * 6];            // [j] = (a4, a5, a6, 2 a5, 3 a6, -)  cubic map of Eq. 19
+    double fit[DP * 10];           // [j] = (a4, a5, a6, 2 a5, 3 a6, -, a0, a2 (a0-1), a1, a3 (a1-1))  fit map of Eq. 19
     double kor[16];                // transform tables (DevProblem::kor)
     unsigned long long step[DP], back[DP], z[DP];
     double red[2][kWarps][G * 2];  // double-buffered by group parity
     DevProblem prob;
     double fam0;
     long long tile;                // popped tile index
+    int fit_full;                  // the fit map of the problem has pole terms (a2 or a3 non-zero in some dimension)
 };
 template <int DP, int G> struct SmemOff {
     static constexpr unsigned delta = 0;
     static constexpr unsigned fam = delta + ((DP * G > kDeltaCache) ? DP * G : kDeltaCache) * 8;
     static constexpr unsigned fit = fam + DP * 2 * 8;
-    static constexpr unsigned kor = fit + DP * 6 * 8;
+    static constexpr unsigned kor = fit + DP * 10 * 8;
     static constexpr unsigned step = kor + 16 * 8;
 };
 
@@ -85,7 +86,11 @@ template <int FAMILY> __device__ __forceinline__ void fam_finish(double s0, doub
 }
 
 // ---- S2-S4 for one (shift q, dimension j): coordinate, periodizing transform, fit map ----------
-struct FitC { double f0, f1, f2, f3, f4; };       // a4, a5, a6, 2 a5, 3 a6 of one dimension
+struct FitC {                                     // fit map of one dimension (Eq. 19)
+    double f0, f1, f2, f3, f4;                    // a4, a5, a6, 2 a5, 3 a6: cubic part and its derivative
+    double a0, k2, a1, k3;                        // poles: a0, a2 (a0 - 1), a1, a3 (a1 - 1)
+    bool full;                                    // warp-uniform: the problem has pole terms
+};
 
 // The generic weight transforms (Table A.2), selected per coordinate by the warp-uniform code
 // gen = kind | r0 << 4 | r1 << 8; P is multiplied by omega(u) / normalisation (the constant is in wconst).
@@ -156,11 +161,19 @@ __device__ __forceinline__ double point_coord(double rd, double inv_n, double de
             x = generic_transform(t, kor_addr, kor_r, P);
         }
     }
-    if (FIT) {                                                // S4: cubic map of Eq. 19 (a2 = a3 = 0)
+    if (FIT) {                                                // S4: fit map of Eq. 19
         const double y = x;
         const double h = __fma_rn(y, __fma_rn(y, fc.f2, fc.f1), fc.f0);
-        D *= __fma_rn(y, __fma_rn(y, fc.f4, fc.f3), fc.f0);   // p'(y)
-        x = y * h;                                            // p(y)
+        double dp = __fma_rn(y, __fma_rn(y, fc.f4, fc.f3), fc.f0);   // cubic part of p'(y)
+        x = y * h;                                            // cubic part of p(y)
+        if (fc.full) {
+            // pole terms a2 y (a0-1)/(a0-y) + a3 y (a1-1)/(a1-y); derivatives a2 a0 (a0-1)/(a0-y)^2 + a3 a1 (a1-1)/(a1-y)^2
+            const double q0 = rcp_nr(fc.a0 - y), q1 = rcp_nr(fc.a1 - y);     // a0 >= 1.001, a1 <= -0.001: never 0
+            const double e0 = fc.k2 * q0, e1 = fc.k3 * q1;
+            x = __fma_rn(y, e0, __fma_rn(y, e1, x));
+            dp = __fma_rn(fc.a0 * e0, q0, __fma_rn(fc.a1 * e1, q1, dp));
+        }
+        D *= dp;
     }
     return x;
 }
@@ -176,13 +189,19 @@ template <int TR, bool FIT> __device__ __forceinline__ double point_weight(doubl
 
 // operands of dimension slot j: family constants, fit constants, the G shifts of the group
 template <int DP, int G, bool FIT>
-__device__ __forceinline__ void load_slot(unsigned sbase, unsigned delta, int j, double& fa, double& fb, FitC& fc, double (&dl)[G]) {
+__device__ __forceinline__ void load_slot(unsigned sbase, unsigned delta, int j, bool fit_full, double& fa, double& fb, FitC& fc,
+                                          double (&dl)[G]) {
     typedef SmemOff<DP, G> O;
     lds_f64x2(sbase + O::fam + 16u * j, fa, fb);
+    fc.full = FIT && fit_full;
     if (FIT) {
-        lds_f64x2(sbase + O::fit + 48u * j, fc.f0, fc.f1);
-        lds_f64x2(sbase + O::fit + 48u * j + 16u, fc.f2, fc.f3);
-        fc.f4 = lds_f64(sbase + O::fit + 48u * j + 32u);
+        lds_f64x2(sbase + O::fit + 80u * j, fc.f0, fc.f1);
+        lds_f64x2(sbase + O::fit + 80u * j + 16u, fc.f2, fc.f3);
+        fc.f4 = lds_f64(sbase + O::fit + 80u * j + 32u);
+        if (fit_full) {
+            lds_f64x2(sbase + O::fit + 80u * j + 48u, fc.a0, fc.k2);
+            lds_f64x2(sbase + O::fit + 80u * j + 64u, fc.a1, fc.k3);
+        }
     }
     if (G % 2 == 0) {
 #pragma unroll
@@ -200,6 +219,7 @@ struct EvalCtx {            // per-tile constants held in registers
     double inv_n, wconst, fam0;
     int kor_r;              // generic weight transforms: DevProblem::gen
     int sel;                // tr_kind * 2 + has_fit
+    int fit_full;           // the fit map has pole terms
 };
 
 template <int FAMILY, int DP, int G, bool WIDE, int TR, bool FIT>
@@ -213,7 +233,7 @@ __device__ __forceinline__ void eval_point_group(const typename Res<WIDE>::T (&r
         const double rd = Res<WIDE>::to_double(r[j]);
         double fa, fb, dl[G];
         FitC fc;
-        load_slot<DP, G, FIT>(cx.sbase, cx.delta, j, fa, fb, fc, dl);
+        load_slot<DP, G, FIT>(cx.sbase, cx.delta, j, cx.fit_full != 0, fa, fb, fc, dl);
 #pragma unroll
         for (int q = 0; q < G; ++q) {
             if (FAMILY == QMC_FAMILY_GENZ_PRODPEAK && TR == TR_BAKER && !FIT) {
@@ -258,6 +278,7 @@ __device__ __forceinline__ void run_tile(SmemCtx<DP, G>& sm, unsigned sbase, con
     EvalCtx cx;
     cx.sbase = sbase; cx.inv_n = pb.inv_n; cx.wconst = pb.wconst; cx.fam0 = sm.fam0; cx.kor_r = pb.gen;
     cx.sel = pb.tr_kind * 2 + (pb.has_fit ? 1 : 0);
+    cx.fit_full = sm.fit_full;
     typedef SmemCtx<DP, G> Ctx;
     typedef SmemOff<DP, G> Off;
     static_assert(offsetof(Ctx, fam) == Off::fam && offsetof(Ctx, fit) == Off::fit && offsetof(Ctx, kor) == Off::kor &&
@@ -354,12 +375,13 @@ __device__ __forceinline__ void run_tile(SmemCtx<DP, G>& sm, unsigned sbase, con
 // constants and the cubic-map constants of dimension slot j.  Slots j >= dim get the padding values (file header).
 struct SlotConst {
     unsigned long long z, step, back;
-    double fa, fb, f[5];
+    double fa, fb, f[9];
 };
 __device__ __forceinline__ SlotConst derive_slot(const DevProblem& pb, int j) {
     SlotConst s;
     s.z = 0; s.step = 0; s.back = 0; s.fa = 0.0; s.fb = 0.0;
     s.f[0] = 1.0; s.f[1] = s.f[2] = s.f[3] = s.f[4] = 0.0;
+    s.f[5] = 2.0; s.f[6] = 0.0; s.f[7] = -1.0; s.f[8] = 0.0;       // no pole terms (identity map in padded slots)
     const int d = pb.dim;
     const unsigned long long n = pb.n;
     if (j < d) {
@@ -375,6 +397,7 @@ __device__ __forceinline__ SlotConst derive_slot(const DevProblem& pb, int j) {
             const double a4 = c[4], a5 = c[5];
             const double a6 = __dadd_rn(__dadd_rn(__dadd_rn(__dadd_rn(1.0, -c[2]), -c[3]), -a4), -a5);
             s.f[0] = a4; s.f[1] = a5; s.f[2] = a6; s.f[3] = 2.0 * a5; s.f[4] = 3.0 * a6;
+            s.f[5] = c[0]; s.f[6] = __dmul_rn(c[2], __dadd_rn(c[0], -1.0)); s.f[7] = c[1]; s.f[8] = __dmul_rn(c[3], __dadd_rn(c[1], -1.0));
         }
     } else if (pb.family == QMC_FAMILY_GENZ_PRODPEAK) {
         // padded slot: the coordinate is pinned to u = 1/2, i.e. x = 1 (baker) or 1/2; factor (x - fb)^2 + fa = 1
@@ -384,6 +407,12 @@ __device__ __forceinline__ SlotConst derive_slot(const DevProblem& pb, int j) {
     // product peak under the baker map without fit: the fused kernel wants 1 - w_j (eval_point_group)
     if (pb.family == QMC_FAMILY_GENZ_PRODPEAK && pb.tr_kind == TR_BAKER && !pb.has_fit) s.fb = __dadd_rn(1.0, -s.fb);
     return s;
+}
+__device__ __forceinline__ int fit_has_poles(const DevProblem& pb) {       // a2 or a3 non-zero in some dimension (Eq. 19)
+    int any = 0;
+    if (pb.has_fit)
+        for (int j = 0; j < pb.dim; ++j) any |= (pb.fit[6 * j + 2] != 0.0 || pb.fit[6 * j + 3] != 0.0) ? 1 : 0;
+    return any;
 }
 __device__ __forceinline__ double derive_fam0(const DevProblem& pb) {
     return (pb.family == QMC_FAMILY_GENZ_OSC) ? __dmul_rn(6.283185307179586476925286766559, pb.params[0]) : 0.0;
@@ -432,22 +461,28 @@ __device__ __forceinline__ bool next_tile(SmemCtx<DP, G>& sm, const FusedLaunch&
         if (SECTOR) {
             const DevAux& a = L.aux[pidx];
             if (tid == 32) sm.fam0 = a.fam0;
+            if (tid == 96) sm.fit_full = a.fit_full;
             for (int j = tid; j < DP; j += kThreads) {      // slots j >= dim hold the padding values
                 sm.z[j] = a.z[j]; sm.step[j] = a.step[j]; sm.back[j] = a.back[j];
                 sm.fam[2 * j] = a.fam_a[j]; sm.fam[2 * j + 1] = a.fam_b[j];
 #pragma unroll
-                for (int i = 0; i < 5; ++i) sm.fit[6 * j + i] = a.fit[i][j];
-                sm.fit[6 * j + 5] = 0.0;
+                for (int i = 0; i < 5; ++i) sm.fit[10 * j + i] = a.fit[i][j];
+                sm.fit[10 * j + 5] = 0.0;
+#pragma unroll
+                for (int i = 5; i < 9; ++i) sm.fit[10 * j + 1 + i] = a.fit[i][j];
             }
         } else {
             if (tid == 32) sm.fam0 = derive_fam0(src);
+            if (tid == 96) sm.fit_full = fit_has_poles(src);
             for (int j = tid; j < DP; j += kThreads) {
                 const SlotConst s = derive_slot(src, j);
                 sm.z[j] = s.z; sm.step[j] = s.step; sm.back[j] = s.back;
                 sm.fam[2 * j] = s.fa; sm.fam[2 * j + 1] = s.fb;
 #pragma unroll
-                for (int i = 0; i < 5; ++i) sm.fit[6 * j + i] = s.f[i];
-                sm.fit[6 * j + 5] = 0.0;
+                for (int i = 0; i < 5; ++i) sm.fit[10 * j + i] = s.f[i];
+                sm.fit[10 * j + 5] = 0.0;
+#pragma unroll
+                for (int i = 5; i < 9; ++i) sm.fit[10 * j + 1 + i] = s.f[i];
             }
         }
         __syncthreads();

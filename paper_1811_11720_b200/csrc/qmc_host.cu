@@ -410,15 +410,25 @@ int validate_values(const qmc_problem& p) {
             const double* a = p.fit_coeffs + 6 * j;
             for (int k = 0; k < 6; ++k)
                 if (!std::isfinite(a[k])) return QMC_ERR_FIT;
-            if (a[2] != 0.0 || a[3] != 0.0) return QMC_ERR_FIT;   // pole terms of Eq. 19: not on the fused path yet
             const double a4 = a[4], a5 = a[5], a6 = 1.0 - a[2] - a[3] - a4 - a5;
-            // p'(y) = a4 + 2 a5 y + 3 a6 y^2 must stay positive on [0,1] (monotone map, Eq. 18)
-            double mn = std::fmin(a4, a4 + 2.0 * a5 + 3.0 * a6);
-            if (a6 != 0.0) {
-                const double yv = -a5 / (3.0 * a6);
-                if (yv > 0.0 && yv < 1.0) mn = std::fmin(mn, a4 + yv * (2.0 * a5 + 3.0 * a6 * yv));
+            if (a[2] == 0.0 && a[3] == 0.0) {
+                // cubic map: p'(y) = a4 + 2 a5 y + 3 a6 y^2 must stay positive on [0,1] (monotone map, Eq. 18)
+                double mn = std::fmin(a4, a4 + 2.0 * a5 + 3.0 * a6);
+                if (a6 != 0.0) {
+                    const double yv = -a5 / (3.0 * a6);
+                    if (yv > 0.0 && yv < 1.0) mn = std::fmin(mn, a4 + yv * (2.0 * a5 + 3.0 * a6 * yv));
+                }
+                if (!(mn > 0.0)) return QMC_ERR_FIT;
+            } else {
+                // pole terms: the bounds of P:L231 keep the poles outside [0,1]; monotonicity is checked on a fine grid
+                if (!(a[0] >= 1.001) || !(a[1] <= -0.001) || !(a[2] >= 0.0) || !(a[3] >= 0.0)) return QMC_ERR_FIT;
+                for (int i = 0; i <= 1024; ++i) {
+                    const double y = (double)i / 1024.0;
+                    const double dp = a[2] * a[0] * (a[0] - 1.0) / ((a[0] - y) * (a[0] - y)) + a[3] * a[1] * (a[1] - 1.0) / ((a[1] - y) * (a[1] - y)) +
+                                      a4 + y * (2.0 * a5 + 3.0 * a6 * y);
+                    if (!(dp > 0.0)) return QMC_ERR_FIT;
+                }
             }
-            if (!(mn > 0.0)) return QMC_ERR_FIT;
         }
     }
     return QMC_OK;

@@ -53,7 +53,7 @@ struct alignas(16) DevProblem {
     int family, dim, m, ncomp;
     int tr_kind;               // TR_*
     int kor_r;                 // symmetric Korobov weight r (1..6) or 0
-    int has_fit;               // 0 none, 1 cubic
+    int has_fit;               // 0 none, 1 fit map of Eq. 19 (cubic, or with pole terms: decided on the device from a2, a3)
     int n_params;
     int aux_off;               // sector: offset (in 8-byte words) of the compiled program in the aux area
     int aux_len;
@@ -68,14 +68,14 @@ struct alignas(16) DevAux {
     unsigned long long back[QMC_MAX_DIM];  // (steps * kThreads * z_j) mod n : rewinds a thread to its first point
     double fam_a[QMC_MAX_DIM];             // per-dimension integrand constants (family dependent)
     double fam_b[QMC_MAX_DIM];
-    double fit[5][QMC_MAX_DIM];            // a4, a5, a6, 2*a5, 3*a6 of the cubic map
+    double fit[9][QMC_MAX_DIM];            // a4, a5, a6, 2*a5, 3*a6 of the cubic part; a0, a2 (a0-1), a1, a3 (a1-1) of the poles
     double fam0;                           // OSC: 2 pi u0
     double sec_c0[2];                      // sector: constant terms of U and F
     int sec_a, sec_b;                      // sector: powers of U and F
     int sec_nops[2];                       // sector: [0] = 32-bit step words of the program (U, end-of-U, F)
     int sec_ncoef[2];                      // sector: [0] = coefficients of the program
     int status;                            // 0 or a qmc_status found while preparing
-    int pad_;
+    int fit_full;                          // 1 if any dimension of the fit map has a pole term (a2 or a3 non-zero)
     unsigned char nu[QMC_MAX_DIM];         // sector: nu_j
 };
 

@@ -20,11 +20,12 @@ __global__ void __launch_bounds__(32) prepare_kernel(const DevProblem* __restric
         const SlotConst s = derive_slot(pb, j);
         a.z[j] = s.z; a.step[j] = s.step; a.back[j] = s.back; a.fam_a[j] = s.fa; a.fam_b[j] = s.fb;
 #pragma unroll
-        for (int i = 0; i < 5; ++i) a.fit[i][j] = s.f[i];
+        for (int i = 0; i < 9; ++i) a.fit[i][j] = s.f[i];
         a.nu[j] = 0;
     }
     if (j == 0) {
         a.fam0 = derive_fam0(pb);
+        a.fit_full = fit_has_poles(pb);
         a.status = 0;
         a.sec_a = a.sec_b = 0;
         a.sec_nops[0] = a.sec_nops[1] = a.sec_ncoef[0] = a.sec_ncoef[1] = 0;

@@ -170,7 +170,7 @@ __device__ __forceinline__ void sector_coords(const typename Res<WIDE>::T (&r)[D
         const double rd = Res<WIDE>::to_double(r[j]);
         double fa, fb, dl[G];
         FitC fc;
-        load_slot<DP, G, FIT>(cx.sbase, cx.delta, j, fa, fb, fc, dl);
+        load_slot<DP, G, FIT>(cx.sbase, cx.delta, j, cx.fit_full != 0, fa, fb, fc, dl);
 #pragma unroll
         for (int q = 0; q < G; ++q)
             x[q][j] = point_coord<TR, FIT>(rd, cx.inv_n, dl[q], fc, cx.sbase + SmemOff<DP, G>::kor, cx.kor_r, P[q], D[q]);

@@ -74,6 +74,10 @@ def test_validate_problem_host_accepts_all_configs():
     (lambda p: p.update(params=p["params"][:-1]), -9),
     (lambda p: p.update(fit_coeffs=synth.cubic_fit_coeffs(4, a4=-0.2, a5=0.3)), -10),
     (lambda p: p.update(fit_coeffs=synth.cubic_fit_coeffs(4, a4=2.0, a5=-5.0)), -10),
+    (lambda p: p.update(fit_coeffs=np.array([[1.0005, -0.5, 0.1, 0.0, 0.6, 0.2]] * 4)), -10),   # a0 below 1.001
+    (lambda p: p.update(fit_coeffs=np.array([[1.5, 0.2, 0.0, 0.1, 0.6, 0.2]] * 4)), -10),       # a1 above -0.001
+    (lambda p: p.update(fit_coeffs=np.array([[1.5, -0.5, -0.1, 0.0, 0.6, 0.2]] * 4)), -10),     # a2 negative
+    (lambda p: p.update(fit_coeffs=np.array([[1.5, -0.5, 0.05, 0.05, 3.0, -6.0]] * 4)), -10),   # not increasing
 ])
 def test_validate_problem_host_rejects(mutate, status):
     p = _cfg0()

@@ -84,9 +84,13 @@ def make(fam, d, n, m, tr, seed, fit=False, z=None, a_hi=1.0):
     if z is None:
         z = synth.korobov_form_vector(n, d, 1 + n // 3)
     fc = None
-    if fit:
+    if fit == "full":
+        # Eq. 19 with pole terms inside the bounds of PAPER.md L231; every third dimension stays a pure cubic
+        fc = np.array([[1.001 + 0.5 * rng.uniform(), -0.001 - 0.5 * rng.uniform(), 0.25 * rng.uniform() * (j % 3 != 2),
+                        0.25 * rng.uniform() * (j % 3 != 2), 0.45 + 0.3 * rng.uniform(), 0.2 * rng.uniform() - 0.05] for j in range(d)])
+    elif fit:
         fc = np.array([[1.001, -0.001, 0.0, 0.0, 0.45 + 0.5 * rng.uniform(), 0.5 * rng.uniform() - 0.1] for _ in range(d)])
-    return synth.problem(fam, prm, n, z, sh, tr, fc, name=f"f{fam}.d{d}.n{n}.m{m}.tr{tr}.fit{int(fit)}")
+    return synth.problem(fam, prm, n, z, sh, tr, fc, name=f"f{fam}.d{d}.n{n}.m{m}.tr{tr}.fit{fit if isinstance(fit, str) else int(fit)}")
 
 
 # ------------------------------------------------------------------------------------------------
@@ -139,6 +143,16 @@ def test_means_all_transforms(fam, tr):
     probs = [make(fam, d, 8191, 6, tr, 300 + 10 * fam + tr % 97, fit=False),
              make(fam, d, 8191, 6, tr, 400 + 10 * fam + tr % 97, fit=True)]
     check_against_oracle(probs)
+
+
+@pytest.mark.parametrize("fam,d", [(0, 3), (0, 16), (1, 8), (2, 5), (2, 12), (3, 6), (3, 9)])
+@pytest.mark.parametrize("tr", [NONE, BAKER, K + 3, K + 2, SIDI + 2])
+def test_means_full_fit_map(fam, d, tr):
+    """the complete fit function of Eq. 19: two pole terms + cubic, Jacobian p'(y) (row f-2)"""
+    p = make(fam, d, 8191, 5, tr, 2100 + 17 * fam + d + tr % 89, fit="full", a_hi=0.6)
+    assert binding.qmc_validate_problem_host(p) == 0
+    assert np.any(p["fit_coeffs"][:, 2] > 0) or d < 2
+    check_against_oracle([p, make(fam, d, 8191, 5, tr, 2200 + d, fit=True, a_hi=0.6)])      # a pole-free problem in the same launch
 
 
 @pytest.mark.parametrize("fam,d", [(0, 1), (0, 4), (0, 6), (0, 9), (0, 12), (0, 16), (0, 17), (0, 32), (1, 2), (1, 5), (1, 8),
