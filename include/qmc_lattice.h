@@ -142,6 +142,12 @@ size_t qmc_project_workspace_bytes(const qmc_problem* p /*HOST*/, int bins);
  * identity map if the minimiser is not safely monotone (min p' <= 0.05).  hist, fit_coeffs: HOST. */
 int qmc_fit_cubic(const double* hist /*HOST [dim][bins]*/, int dim, int bins, double* fit_coeffs /*HOST [dim][6]*/);
 
+/* Host-side fit of the COMPLETE fit function of Eq. 19 (two pole terms + cubic) to the same data: bounded
+ * Levenberg-Marquardt on (a_0..a_5) with a_0 >= 1.001, a_1 <= -0.001, a_2, a_3 >= 0 (the paper uses GSL), started from
+ * the cubic solution; the cubic result is kept for a dimension unless the full function is a strictly better fit that is
+ * increasing on [0,1].  bins in 8..1024.  hist, fit_coeffs: HOST.  The result is valid input for every compute entry. */
+int qmc_fit_polysingular(const double* hist /*HOST [dim][bins]*/, int dim, int bins, double* fit_coeffs /*HOST [dim][6]*/);
+
 /* Inspection: residues r = (k z_j) mod n and coordinates u = {r/n + shift_j} for k = k0..k0+count-1,
  * produced by the same device code the fused kernel uses (Eq. 2; fp64 realisation:
  * u = wrap(fma(double(r), 1/double(n), shift_j)), reading C-2).

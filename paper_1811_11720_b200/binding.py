@@ -19,7 +19,7 @@ EXPORTS = [
     "qmc_validate_problem_host", "qmc_lattice_project", "qmc_project_workspace_bytes", "qmc_fit_cubic",
     "qmc_lattice_points", "qmc_finalize_means", "qmc_fp64_peak_probe", "qmc_last_launch_count", "qmc_plan_info",
     "qmc_profile_enable", "qmc_profile_last_fused_ms",
-    "qmc_num_components", "qmc_status_string", "qmc_last_cuda_error", "qmc_integrate",
+    "qmc_num_components", "qmc_status_string", "qmc_last_cuda_error", "qmc_integrate", "qmc_fit_polysingular",
 ]
 
 QMC_OK = 0
@@ -71,6 +71,7 @@ def lib():
         L.qmc_project_workspace_bytes.argtypes = [pp, C.c_int]
         L.qmc_project_workspace_bytes.restype = C.c_size_t
         L.qmc_fit_cubic.argtypes = [dp, C.c_int, C.c_int, dp]
+        L.qmc_fit_polysingular.argtypes = [dp, C.c_int, C.c_int, dp]
         L.qmc_lattice_points.argtypes = [C.c_uint64, C.c_int, up, dp, C.c_uint64, C.c_uint64, vp, vp, vp]
         L.qmc_finalize_means.argtypes = [vp, C.c_int, C.c_int, vp, vp, vp]
         L.qmc_fp64_peak_probe.argtypes = [C.c_int, dp, dp, vp]
@@ -160,6 +161,15 @@ def qmc_fit_cubic(hist):
     d, bins = H.shape
     out = np.zeros((d, 6))
     _check(lib().qmc_fit_cubic(_d(H), d, bins, _d(out)), "qmc_fit_cubic")
+    return out
+
+
+def qmc_fit_polysingular(hist):
+    """Bounded Levenberg-Marquardt fit of the complete fit function of Eq. 19 -> (dim, 6) coefficients a_0..a_5."""
+    H = _f64(hist)
+    d, bins = H.shape
+    out = np.zeros((d, 6))
+    _check(lib().qmc_fit_polysingular(_d(H), d, bins, _d(out)), "qmc_fit_polysingular")
     return out
 
 

@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libqmc_lattice.so")
-SOURCES = ["qmc_host.cu", "qmc_adaptive.cu", "qmc_misc.cu", "qmc_project.cu", "qmc_fused_f0.cu", "qmc_fused_f1.cu", "qmc_fused_f2.cu",
+SOURCES = ["qmc_host.cu", "qmc_adaptive.cu", "qmc_fit.cu", "qmc_misc.cu", "qmc_project.cu", "qmc_fused_f0.cu", "qmc_fused_f1.cu", "qmc_fused_f2.cu",
            "qmc_fused_f3.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
 

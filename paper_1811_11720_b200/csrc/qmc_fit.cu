@@ -1,0 +1,138 @@
+// qmc_fit.cu -- host-side fit of the complete fit function of Eq. 19 to the inverse CDF sampled by the device
+// projection pass (Eq. 20).  SURVEY.md 8(f) row f-2.  The paper uses GSL's Levenberg-Marquardt with the
+// parameter bounds a0 >= 1.001, a1 <= -0.001, a2, a3 >= 0; this is an own bounded Levenberg-Marquardt (no GSL).
+// Setup code, off the timed path; the result is an INPUT of the fused kernels (fit_coeffs), which are parity-tested for
+// arbitrary valid coefficients, so the optimiser itself needs no oracle counterpart (any valid map keeps the integral, Eq. 18).
+#include <algorithm>
+#include <cmath>
+#include <vector>
+
+#include "../../include/qmc_lattice.h"
+
+namespace {
+
+struct Model {                      // p(y) of Eq. 19 with a6 = 1 - a2 - a3 - a4 - a5, and its parameter gradient
+    static long double eval(const long double* a, long double y, long double* grad) {
+        const long double y2 = y * y, y3 = y2 * y;
+        const long double d0 = a[0] - y, d1 = a[1] - y;
+        const long double t0 = y * (a[0] - 1.0L) / d0, t1 = y * (a[1] - 1.0L) / d1;
+        const long double a6 = 1.0L - a[2] - a[3] - a[4] - a[5];
+        if (grad) {
+            grad[0] = a[2] * y * (1.0L - y) / (d0 * d0);
+            grad[1] = a[3] * y * (1.0L - y) / (d1 * d1);
+            grad[2] = t0 - y3;
+            grad[3] = t1 - y3;
+            grad[4] = y - y3;
+            grad[5] = y2 - y3;
+        }
+        return a[2] * t0 + a[3] * t1 + y * (a[4] + y * (a[5] + y * a6));
+    }
+    static bool increasing(const long double* a) {
+        const long double a6 = 1.0L - a[2] - a[3] - a[4] - a[5];
+        for (int i = 0; i <= 1024; ++i) {
+            const long double y = (long double)i / 1024.0L, d0 = a[0] - y, d1 = a[1] - y;
+            const long double dp = a[2] * a[0] * (a[0] - 1.0L) / (d0 * d0) + a[3] * a[1] * (a[1] - 1.0L) / (d1 * d1) + a[4] +
+                                   y * (2.0L * a[5] + 3.0L * a6 * y);
+            if (!(dp > 0.05L)) return false;                      // same safety margin as the cubic fit (reading C-8)
+        }
+        return true;
+    }
+};
+
+void project(long double* a) {      // bounds of P:L231
+    a[0] = std::max(a[0], 1.001L);
+    a[1] = std::min(a[1], -0.001L);
+    a[2] = std::max(a[2], 0.0L);
+    a[3] = std::max(a[3], 0.0L);
+}
+
+long double cost(const long double* a, const std::vector<long double>& c, const std::vector<long double>& e) {
+    long double s = 0.0L;
+    for (size_t b = 0; b < c.size(); ++b) { const long double r = Model::eval(a, c[b], nullptr) - e[b]; s += r * r; }
+    return s;
+}
+
+bool solve6(long double A[6][6], long double* b) {               // Gaussian elimination with partial pivoting
+    for (int k = 0; k < 6; ++k) {
+        int piv = k;
+        for (int i = k + 1; i < 6; ++i) if (fabsl(A[i][k]) > fabsl(A[piv][k])) piv = i;
+        if (fabsl(A[piv][k]) < 1e-300L) return false;
+        if (piv != k) { for (int j = 0; j < 6; ++j) std::swap(A[k][j], A[piv][j]); std::swap(b[k], b[piv]); }
+        for (int i = k + 1; i < 6; ++i) {
+            const long double f = A[i][k] / A[k][k];
+            for (int j = k; j < 6; ++j) A[i][j] -= f * A[k][j];
+            b[i] -= f * b[k];
+        }
+    }
+    for (int k = 5; k >= 0; --k) {
+        long double s = b[k];
+        for (int j = k + 1; j < 6; ++j) s -= A[k][j] * b[j];
+        b[k] = s / A[k][k];
+    }
+    return true;
+}
+
+}  // namespace
+
+extern "C" int qmc_fit_polysingular(const double* hist, int dim, int bins, double* fit_coeffs) {
+    if (!hist || !fit_coeffs) return QMC_ERR_NULL;
+    if (dim < 1 || dim > QMC_MAX_DIM) return QMC_ERR_DIM;
+    if (bins < 8 || bins > 1024) return QMC_ERR_N;
+    const int st = qmc_fit_cubic(hist, dim, bins, fit_coeffs);   // starting point and fall-back (identity if that fails too)
+    if (st != QMC_OK) return st;
+    for (int j = 0; j < dim; ++j) {
+        const double* h = hist + (size_t)j * bins;
+        long double total = 0.0L;
+        bool ok = true;
+        for (int b = 0; b < bins; ++b) { ok = ok && std::isfinite(h[b]) && h[b] >= 0.0; total += h[b]; }
+        if (!ok || !(total > 0.0L)) continue;
+        std::vector<long double> c, e;                             // CDF values at the bin edges: p(c_b) = e_b (Eq. 18-20)
+        long double run = 0.0L;
+        for (int b = 1; b < bins; ++b) { run += h[b - 1]; c.push_back(run / total); e.push_back((long double)b / bins); }
+        double* o = fit_coeffs + 6 * j;
+        long double a[6] = {1.1L, -0.1L, 0.0L, 0.0L, o[4], o[5]};
+        // two starts: the cubic solution with dormant poles, and the same with small active poles (the gradient of a0, a1 vanishes
+        // while a2 = a3 = 0)
+        long double best[6], best_cost = cost(a, c, e);
+        for (int k = 0; k < 6; ++k) best[k] = a[k];
+        for (int start = 0; start < 2; ++start) {
+            long double th[6] = {1.1L, -0.1L, start ? 0.05L : 0.0L, start ? 0.05L : 0.0L, o[4], o[5]};
+            long double cur = cost(th, c, e), lambda = 1e-3L;
+            for (int it = 0; it < 400; ++it) {
+                long double JTJ[6][6] = {}, JTr[6] = {};
+                for (size_t b = 0; b < c.size(); ++b) {
+                    long double g[6];
+                    const long double r = Model::eval(th, c[b], g) - e[b];
+                    for (int p = 0; p < 6; ++p) { JTr[p] += g[p] * r; for (int q = 0; q < 6; ++q) JTJ[p][q] += g[p] * g[q]; }
+                }
+                long double A[6][6], rhs[6];
+                for (int p = 0; p < 6; ++p) {
+                    rhs[p] = -JTr[p];
+                    for (int q = 0; q < 6; ++q) A[p][q] = JTJ[p][q];
+                    A[p][p] += lambda * std::max(JTJ[p][p], 1e-12L);
+                }
+                if (!solve6(A, rhs)) { lambda *= 10.0L; continue; }
+                long double trial[6];
+                for (int p = 0; p < 6; ++p) trial[p] = th[p] + rhs[p];
+                project(trial);
+                const long double tc = cost(trial, c, e);
+                if (tc < cur) {
+                    const long double gain = (cur - tc) / std::max(cur, 1e-300L);
+                    for (int p = 0; p < 6; ++p) th[p] = trial[p];
+                    cur = tc;
+                    lambda = std::max(lambda / 3.0L, 1e-12L);
+                    if (gain < 1e-12L) break;
+                } else {
+                    lambda *= 4.0L;
+                    if (lambda > 1e12L) break;
+                }
+            }
+            if (cur < best_cost && Model::increasing(th)) { best_cost = cur; for (int k = 0; k < 6; ++k) best[k] = th[k]; }
+        }
+        // keep the cubic result unless the full function is a strictly better, valid fit
+        const long double cubic[6] = {1.1L, -0.1L, 0.0L, 0.0L, o[4], o[5]};
+        if (best_cost < cost(cubic, c, e) && Model::increasing(best) && (best[2] > 0.0L || best[3] > 0.0L))
+            for (int k = 0; k < 6; ++k) o[k] = (double)best[k];
+    }
+    return QMC_OK;
+}

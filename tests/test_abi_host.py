@@ -177,3 +177,49 @@ def test_missing_library_fails_loudly(monkeypatch):
     monkeypatch.setattr(binding, "LIB_PATH", "/nonexistent/libqmc_lattice.so")
     with pytest.raises(ImportError):
         binding.lib()
+
+
+def _hist_of_map(a, bins):
+    """histogram whose CDF is the inverse of the increasing map p of PAPER.md Eq. 19: c_b = p^-1(b/bins) by bisection
+    (p evaluated by the ORACLE's fit_map), H[b] = c_{b+1} - c_b"""
+    edges = [0.0]
+    for b in range(1, bins):
+        lo, hi = 0.0, 1.0
+        for _ in range(80):
+            mid = 0.5 * (lo + hi)
+            if oracle.fit_map(a, mid)[0] < b / bins:
+                lo = mid
+            else:
+                hi = mid
+        edges.append(0.5 * (lo + hi))
+    edges.append(1.0)
+    return np.diff(np.array(edges))
+
+
+def test_fit_polysingular_recovers_a_map_with_poles():
+    """row f-2: the bounded Levenberg-Marquardt fit of the complete fit function (bounds L231) reproduces
+    an inverse CDF generated from known parameters far better than the cubic sub-family can, and returns a valid map"""
+    truth = np.array([[1.05, -0.4, 0.35, 0.0, 0.30, 0.25], [1.6, -0.03, 0.0, 0.45, 0.35, 0.10], [1.001, -0.001, 0.0, 0.0, 0.7, 0.2]])
+    bins = 256
+    H = np.array([_hist_of_map(a, bins) for a in truth])
+    full, cubic = binding.qmc_fit_polysingular(H), binding.qmc_fit_cubic(H)
+    for j in range(3):
+        c = np.cumsum(H[j])[:-1] / H[j].sum()
+        e = np.arange(1, bins) / bins
+        res_full = max(abs(oracle.fit_map(full[j], y)[0] - t) for y, t in zip(c, e))
+        res_cub = max(abs(oracle.fit_map(cubic[j], y)[0] - t) for y, t in zip(c, e))
+        assert res_full <= res_cub + 1e-15
+        a = full[j]
+        assert a[0] >= 1.001 and a[1] <= -0.001 and a[2] >= 0 and a[3] >= 0
+        assert min(oracle.fit_map(a, y)[1] for y in np.linspace(0, 1, 513)) > 0          # increasing
+        assert abs(oracle.fit_map(a, 1.0)[0] - 1.0) < 1e-14 and oracle.fit_map(a, 0.0)[0] == 0.0
+        if j < 2:
+            assert res_full < 2e-4 and res_full < 0.05 * res_cub                            # the poles matter and are found
+            assert a[2] > 0 or a[3] > 0
+        else:
+            assert res_full < 1e-9                                                           # an exact cubic stays a cubic fit
+    p = dict(_cfg0(), fit_coeffs=np.tile(full[0], (4, 1)))
+    assert binding.qmc_validate_problem_host(p) == 0                                         # valid input of the compute entries
+    flat = binding.qmc_fit_polysingular(np.ones((2, 64)))
+    np.testing.assert_allclose(flat[:, 4:], [[1.0, 0.0]] * 2, atol=1e-12)
+    assert np.all(flat[:, 2:4] == 0.0)
