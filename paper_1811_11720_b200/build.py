@@ -13,8 +13,11 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libqmc_lattice.so")
-SOURCES = ["qmc_host.cu", "qmc_adaptive.cu", "qmc_fit.cu", "qmc_misc.cu", "qmc_project.cu", "qmc_fused_f0.cu", "qmc_fused_f1.cu", "qmc_fused_f2.cu",
-           "qmc_fused_f3.cu"]
+# (source, extra nvcc defines, object name): the closed-form fused kernels are one source compiled per (family, part)
+SOURCES = [("qmc_host.cu", [], "qmc_host.o"), ("qmc_adaptive.cu", [], "qmc_adaptive.o"), ("qmc_fit.cu", [], "qmc_fit.o"),
+           ("qmc_misc.cu", [], "qmc_misc.o"), ("qmc_project.cu", [], "qmc_project.o"), ("qmc_fused_f3.cu", [], "qmc_fused_f3.o")]
+SOURCES += [("qmc_fused_closed.cu", [f"-DQMC_FAM={f}", f"-DQMC_PART={q}"], f"qmc_fused_closed_f{f}_p{q}.o")
+            for q in (4, 3, 2, 1, 0) for f in (2, 1, 0)]       # the slowest parts first
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
 
 
@@ -32,20 +35,21 @@ def _deps(path, seen=None):
     return seen
 
 
-def _compile(src: str, force: bool) -> str:
-    obj = os.path.join(OBJ, src.replace(".cu", ".o"))
+def _compile(job, force: bool) -> str:
+    src, defines, objname = job
+    obj = os.path.join(OBJ, objname)
     path = os.path.join(CSRC, src)
     newest = max(os.path.getmtime(p) for p in [path, *_deps(path)])
     if force or not os.path.exists(obj) or os.path.getmtime(obj) < newest:
-        subprocess.run(["nvcc", *NVCC_FLAGS, "-c", path, "-o", obj], check=True)
+        subprocess.run(["nvcc", *NVCC_FLAGS, *defines, "-c", path, "-o", obj], check=True)
     return obj
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
-    srcs = [s for s in SOURCES if os.path.exists(os.path.join(CSRC, s))]
-    with concurrent.futures.ThreadPoolExecutor(max_workers=min(8, len(srcs))) as ex:
-        objs = list(ex.map(lambda s: _compile(s, force), srcs))
+    jobs = [j for j in SOURCES if os.path.exists(os.path.join(CSRC, j[0]))]
+    with concurrent.futures.ThreadPoolExecutor(max_workers=min(os.cpu_count() or 4, len(jobs))) as ex:
+        objs = list(ex.map(lambda j: _compile(j, force), jobs))
     if force or not os.path.exists(LIB) or os.path.getmtime(LIB) < max(os.path.getmtime(o) for o in objs):
         subprocess.run(["nvcc", "-shared", "-o", LIB, *objs, "-gencode", "arch=compute_100a,code=sm_100a", "-lcudart"],
                        check=True)

@@ -88,8 +88,7 @@ template <int FAMILY> __device__ __forceinline__ void fam_finish(double s0, doub
 // ---- S2-S4 for one (shift q, dimension j): coordinate, periodizing transform, fit map ----------
 struct FitC {                                     // fit map of one dimension (Eq. 19)
     double f0, f1, f2, f3, f4;                    // a4, a5, a6, 2 a5, 3 a6: cubic part and its derivative
-    double a0, k2, a1, k3;                        // poles: a0, a2 (a0 - 1), a1, a3 (a1 - 1)
-    bool full;                                    // warp-uniform: the problem has pole terms
+    double a0, k2, a1, k3;                        // poles: a0, a2 (a0 - 1), a1, a3 (a1 - 1)   (fit mode 2 only)
 };
 
 // The generic weight transforms (Table A.2), selected per coordinate by the warp-uniform code
@@ -138,8 +137,18 @@ __device__ __forceinline__ double generic_transform(double t, unsigned kor_addr,
     return lds_f64(kor_addr) * I;
 }
 
+// Pole terms of the fit function (Eq. 19): adds a2 y (a0-1)/(a0-y) + a3 y (a1-1)/(a1-y) to p and
+// a2 a0 (a0-1)/(a0-y)^2 + a3 a1 (a1-1)/(a1-y)^2 to p'; k2 = a2 (a0-1), k3 = a3 (a1-1).  a0 >= 1.001 and a1 <= -0.001
+// keep the denominators away from 0 on [0,1].  Only the fit-mode-2 tile loops contain it.
+__device__ __forceinline__ void fit_poles(double y, double a0, double k2, double a1, double k3, double& p, double& dp) {
+    const double q0 = rcp_nr(a0 - y), q1 = rcp_nr(a1 - y);
+    const double e0 = k2 * q0, e1 = k3 * q1;
+    p = __fma_rn(y, e0, __fma_rn(y, e1, p));
+    dp = __fma_rn(a0 * e0, q0, __fma_rn(a1 * e1, q1, dp));
+}
+
 // Returns x_j; multiplies P by u(1-u) (Korobov) and D by p'(y) (fit).
-template <int TR, bool FIT>
+template <int TR, int FIT>
 __device__ __forceinline__ double point_coord(double rd, double inv_n, double delta, const FitC& fc, unsigned kor_addr,
                                               int kor_r, double& P, double& D) {
     const double t = coord_t(rd, inv_n, delta);
@@ -166,20 +175,14 @@ __device__ __forceinline__ double point_coord(double rd, double inv_n, double de
         const double h = __fma_rn(y, __fma_rn(y, fc.f2, fc.f1), fc.f0);
         double dp = __fma_rn(y, __fma_rn(y, fc.f4, fc.f3), fc.f0);   // cubic part of p'(y)
         x = y * h;                                            // cubic part of p(y)
-        if (fc.full) {
-            // pole terms a2 y (a0-1)/(a0-y) + a3 y (a1-1)/(a1-y); derivatives a2 a0 (a0-1)/(a0-y)^2 + a3 a1 (a1-1)/(a1-y)^2
-            const double q0 = rcp_nr(fc.a0 - y), q1 = rcp_nr(fc.a1 - y);     // a0 >= 1.001, a1 <= -0.001: never 0
-            const double e0 = fc.k2 * q0, e1 = fc.k3 * q1;
-            x = __fma_rn(y, e0, __fma_rn(y, e1, x));
-            dp = __fma_rn(fc.a0 * e0, q0, __fma_rn(fc.a1 * e1, q1, dp));
-        }
+        if (FIT == 2) fit_poles(y, fc.a0, fc.k2, fc.a1, fc.k3, x, dp);
         D *= dp;
     }
     return x;
 }
 
 // Weight W = prod_j omega(u_j) p'(y_j) from the carried products (Eq. 12, Eq. 18).
-template <int TR, bool FIT> __device__ __forceinline__ double point_weight(double P, double D, double wconst, int kor_r) {
+template <int TR, int FIT> __device__ __forceinline__ double point_weight(double P, double D, double wconst, int kor_r) {
     double W = 1.0;
     if (TR == TR_KOR3) W = wconst * (P * P * P);
     else if (TR == TR_KORR) W = wconst * P;                  // generic transforms carry the full weight product
@@ -188,17 +191,15 @@ template <int TR, bool FIT> __device__ __forceinline__ double point_weight(doubl
 }
 
 // operands of dimension slot j: family constants, fit constants, the G shifts of the group
-template <int DP, int G, bool FIT>
-__device__ __forceinline__ void load_slot(unsigned sbase, unsigned delta, int j, bool fit_full, double& fa, double& fb, FitC& fc,
-                                          double (&dl)[G]) {
+template <int DP, int G, int FIT>
+__device__ __forceinline__ void load_slot(unsigned sbase, unsigned delta, int j, double& fa, double& fb, FitC& fc, double (&dl)[G]) {
     typedef SmemOff<DP, G> O;
     lds_f64x2(sbase + O::fam + 16u * j, fa, fb);
-    fc.full = FIT && fit_full;
     if (FIT) {
         lds_f64x2(sbase + O::fit + 80u * j, fc.f0, fc.f1);
         lds_f64x2(sbase + O::fit + 80u * j + 16u, fc.f2, fc.f3);
         fc.f4 = lds_f64(sbase + O::fit + 80u * j + 32u);
-        if (fit_full) {
+        if (FIT == 2) {
             lds_f64x2(sbase + O::fit + 80u * j + 48u, fc.a0, fc.k2);
             lds_f64x2(sbase + O::fit + 80u * j + 64u, fc.a1, fc.k3);
         }
@@ -218,11 +219,10 @@ struct EvalCtx {            // per-tile constants held in registers
     unsigned delta;         // shared address of the current group's shifts
     double inv_n, wconst, fam0;
     int kor_r;              // generic weight transforms: DevProblem::gen
-    int sel;                // tr_kind * 2 + has_fit
-    int fit_full;           // the fit map has pole terms
+    int sel;                // tr_kind * 3 + fit mode (0 none, 1 cubic, 2 cubic + pole terms)
 };
 
-template <int FAMILY, int DP, int G, bool WIDE, int TR, bool FIT>
+template <int FAMILY, int DP, int G, bool WIDE, int TR, int FIT>
 __device__ __forceinline__ void eval_point_group(const typename Res<WIDE>::T (&r)[DP], const EvalCtx& cx,
                                                  double (&acc)[G][FamTraits<FAMILY>::NC]) {
     double s0[G], s1[G], P[G], D[G];
@@ -233,7 +233,7 @@ __device__ __forceinline__ void eval_point_group(const typename Res<WIDE>::T (&r
         const double rd = Res<WIDE>::to_double(r[j]);
         double fa, fb, dl[G];
         FitC fc;
-        load_slot<DP, G, FIT>(cx.sbase, cx.delta, j, cx.fit_full != 0, fa, fb, fc, dl);
+        load_slot<DP, G, FIT>(cx.sbase, cx.delta, j, fa, fb, fc, dl);
 #pragma unroll
         for (int q = 0; q < G; ++q) {
             if (FAMILY == QMC_FAMILY_GENZ_PRODPEAK && TR == TR_BAKER && !FIT) {
@@ -246,7 +246,7 @@ __device__ __forceinline__ void eval_point_group(const typename Res<WIDE>::T (&r
             }
         }
     }
-    constexpr bool USEW = (TR == TR_KOR3 || TR == TR_KORR || FIT);
+    constexpr bool USEW = (TR == TR_KOR3 || TR == TR_KORR || FIT != 0);
 #pragma unroll
     for (int q = 0; q < G; ++q)
         fam_finish<FAMILY>(s0[q], s1[q], point_weight<TR, FIT>(P[q], D[q], cx.wconst, cx.kor_r), USEW, acc[q]);
@@ -254,7 +254,7 @@ __device__ __forceinline__ void eval_point_group(const typename Res<WIDE>::T (&r
 
 struct NoExtra {};
 
-template <int FAMILY, int DP, int G, bool WIDE, int TR, bool FIT> struct ClosedEval {
+template <int FAMILY, int DP, int G, bool WIDE, int TR, int FIT> struct ClosedEval {
     static constexpr int NC = FamTraits<FAMILY>::NC;
     typedef NoExtra Extra;
     static __device__ __forceinline__ void eval(const typename Res<WIDE>::T (&r)[DP], const SmemCtx<DP, G>&, const Extra&,
@@ -277,8 +277,7 @@ __device__ __forceinline__ void run_tile(SmemCtx<DP, G>& sm, unsigned sbase, con
     const unsigned long long n = pb.n;
     EvalCtx cx;
     cx.sbase = sbase; cx.inv_n = pb.inv_n; cx.wconst = pb.wconst; cx.fam0 = sm.fam0; cx.kor_r = pb.gen;
-    cx.sel = pb.tr_kind * 2 + (pb.has_fit ? 1 : 0);
-    cx.fit_full = sm.fit_full;
+    cx.sel = pb.tr_kind * 3 + (pb.has_fit ? 1 + sm.fit_full : 0);
     typedef SmemCtx<DP, G> Ctx;
     typedef SmemOff<DP, G> Off;
     static_assert(offsetof(Ctx, fam) == Off::fam && offsetof(Ctx, fit) == Off::fit && offsetof(Ctx, kor) == Off::kor &&
@@ -368,6 +367,13 @@ __device__ __forceinline__ void run_tile(SmemCtx<DP, G>& sm, unsigned sbase, con
             }
         }
     }
+}
+
+// the same tile loop as a real (not inlined) call: used for the correctness paths so that their register needs stay theirs
+template <class EV, int DP, int G, bool WIDE>
+__device__ __noinline__ void run_tile_call(SmemCtx<DP, G>& sm, unsigned sbase, const typename EV::Extra& ex, long long tile_local,
+                                           bool changed, double* __restrict__ partials) {
+    run_tile<EV, DP, G, WIDE>(sm, sbase, ex, tile_local, changed, partials);
 }
 
 // ---- S0: per-slot constants of a problem, derived from the caller's arrays ------------------------
@@ -511,13 +517,19 @@ __global__ void __launch_bounds__(kThreads, MinBlocks<DP, WIDE>::value) fused_ke
     bool changed;
     NoExtra ex;
     while (next_tile<DP, G, false>(sm, L, cur, iter, tile_local, changed)) {
-        const int sel = sm.prob.tr_kind * 2 + (sm.prob.has_fit ? 1 : 0);
+        // tile loop = (transform kind) x (fit mode 0 none / 1 cubic / 2 cubic + poles, decided on the device).  The
+        // specialised loops are inlined; the generic weight transforms and the pole-term fit are real calls, so they
+        // cost the specialised loops no registers.
+        const int sel = sm.prob.tr_kind * 3 + (sm.prob.has_fit ? 1 + sm.fit_full : 0);
         switch (sel) {
-#define QMC_CASE(TRK, FITB) \
-    case TRK * 2 + (FITB ? 1 : 0): run_tile<ClosedEval<FAMILY, DP, G, WIDE, TRK, FITB>, DP, G, WIDE>(sm, sbase, ex, tile_local, changed, L.partials); break;
-            QMC_CASE(TR_NONE, false) QMC_CASE(TR_NONE, true) QMC_CASE(TR_BAKER, false) QMC_CASE(TR_BAKER, true)
-            QMC_CASE(TR_KOR3, false) QMC_CASE(TR_KOR3, true) QMC_CASE(TR_KORR, false) QMC_CASE(TR_KORR, true)
-#undef QMC_CASE
+#define QMC_FAST(TRK, FITM) \
+    case TRK * 3 + FITM: run_tile<ClosedEval<FAMILY, DP, G, WIDE, TRK, FITM>, DP, G, WIDE>(sm, sbase, ex, tile_local, changed, L.partials); break;
+#define QMC_SLOW(TRK, FITM) \
+    case TRK * 3 + FITM: run_tile_call<ClosedEval<FAMILY, DP, G, WIDE, TRK, FITM>, DP, G, WIDE>(sm, sbase, ex, tile_local, changed, L.partials); break;
+            QMC_FAST(TR_NONE, 0) QMC_FAST(TR_NONE, 1) QMC_FAST(TR_BAKER, 0) QMC_FAST(TR_BAKER, 1) QMC_FAST(TR_KOR3, 0) QMC_FAST(TR_KOR3, 1)
+            QMC_SLOW(TR_NONE, 2) QMC_SLOW(TR_BAKER, 2) QMC_SLOW(TR_KOR3, 2) QMC_SLOW(TR_KORR, 0) QMC_SLOW(TR_KORR, 1) QMC_SLOW(TR_KORR, 2)
+#undef QMC_FAST
+#undef QMC_SLOW
             default: break;
         }
     }

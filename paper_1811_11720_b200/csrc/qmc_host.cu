@@ -270,15 +270,40 @@ int sm_count() {
     return v;
 }
 
+// closed-form families: the kernel variants live in five parts per family (qmc_fused_closed.inc); try each
+#define QMC_TRY_PARTS(FAM, PREFIX, FAIL, ...)                                                             \
+    {                                                                                                    \
+        auto r0 = PREFIX##FAM##_0(__VA_ARGS__); if (r0 != FAIL) return r0;                               \
+        auto r1 = PREFIX##FAM##_1(__VA_ARGS__); if (r1 != FAIL) return r1;                               \
+        auto r2 = PREFIX##FAM##_2(__VA_ARGS__); if (r2 != FAIL) return r2;                               \
+        auto r3 = PREFIX##FAM##_3(__VA_ARGS__); if (r3 != FAIL) return r3;                               \
+        return PREFIX##FAM##_4(__VA_ARGS__);                                                             \
+    }
+cudaError_t launch_closed(int family, int dp, bool wide, int grid, cudaStream_t st, const FusedLaunch& a) {
+    switch (family) {
+        case 0: QMC_TRY_PARTS(0, launch_fused_part_, cudaErrorInvalidValue, dp, wide, grid, st, a)
+        case 1: QMC_TRY_PARTS(1, launch_fused_part_, cudaErrorInvalidValue, dp, wide, grid, st, a)
+        case 2: QMC_TRY_PARTS(2, launch_fused_part_, cudaErrorInvalidValue, dp, wide, grid, st, a)
+    }
+    return cudaErrorInvalidValue;
+}
+int occupancy_closed(int family, int dp, bool wide) {
+    switch (family) {
+        case 0: QMC_TRY_PARTS(0, occupancy_fused_part_, -1, dp, wide)
+        case 1: QMC_TRY_PARTS(1, occupancy_fused_part_, -1, dp, wide)
+        case 2: QMC_TRY_PARTS(2, occupancy_fused_part_, -1, dp, wide)
+    }
+    return -1;
+}
+#undef QMC_TRY_PARTS
+
 int occupancy(int family, int dp, bool wide) {
     static int cache[4][33][2];
     int& c = cache[family][dp][wide ? 1 : 0];
     if (c > 0) return c;
     int v = -1;
     switch (family) {
-        case 0: v = occupancy_fused_f0(dp, wide); break;
-        case 1: v = occupancy_fused_f1(dp, wide); break;
-        case 2: v = occupancy_fused_f2(dp, wide); break;
+        case 0: case 1: case 2: v = occupancy_closed(family, dp, wide); break;
         case 3: v = occupancy_fused_f3(dp, wide); break;
     }
     if (v > 0) c = v;
@@ -364,9 +389,7 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
         a.vq = queues[vi];
         cudaError_t e = cudaErrorInvalidValue;
         switch (v.family) {
-            case 0: e = launch_fused_f0(v.dp, v.wide, grid, st, a); break;
-            case 1: e = launch_fused_f1(v.dp, v.wide, grid, st, a); break;
-            case 2: e = launch_fused_f2(v.dp, v.wide, grid, st, a); break;
+            case 0: case 1: case 2: e = launch_closed(v.family, v.dp, v.wide, grid, st, a); break;
             case 3: e = launch_fused_f3(v.dp, v.wide, grid, st, a); break;
         }
         if (e != cudaSuccess) return cuda_fail(e, "fused kernel launch");

@@ -27,14 +27,15 @@ cudaError_t launch_finalize_means(cudaStream_t st, const double* means, int m, i
 cudaError_t launch_points(cudaStream_t st, const PointsArgs& a, int sm_count);
 cudaError_t launch_dfma_probe(cudaStream_t st, double* out, int blocks, int iters);
 
-// fused kernels, one translation unit per family
-cudaError_t launch_fused_f0(int dp, bool wide, int grid, cudaStream_t st, const FusedLaunch& a);
-cudaError_t launch_fused_f1(int dp, bool wide, int grid, cudaStream_t st, const FusedLaunch& a);
-cudaError_t launch_fused_f2(int dp, bool wide, int grid, cudaStream_t st, const FusedLaunch& a);
+// fused kernels: closed-form families 0-2 in parts (qmc_fused_closed.inc), the sector family in qmc_fused_f3.cu
+#define QMC_DECLARE_PART(FAM, PART)                                                                                         \
+    cudaError_t launch_fused_part_##FAM##_##PART(int dp, bool wide, int grid, cudaStream_t st, const FusedLaunch& a); \
+    int occupancy_fused_part_##FAM##_##PART(int dp, bool wide);
+#define QMC_DECLARE_FAMILY(FAM) QMC_DECLARE_PART(FAM, 0) QMC_DECLARE_PART(FAM, 1) QMC_DECLARE_PART(FAM, 2) QMC_DECLARE_PART(FAM, 3) QMC_DECLARE_PART(FAM, 4)
+QMC_DECLARE_FAMILY(0) QMC_DECLARE_FAMILY(1) QMC_DECLARE_FAMILY(2)
+#undef QMC_DECLARE_FAMILY
+#undef QMC_DECLARE_PART
 cudaError_t launch_fused_f3(int dp, bool wide, int grid, cudaStream_t st, const FusedLaunch& a);
-int occupancy_fused_f0(int dp, bool wide);
-int occupancy_fused_f1(int dp, bool wide);
-int occupancy_fused_f2(int dp, bool wide);
 int occupancy_fused_f3(int dp, bool wide);
 
 }  // namespace qmc

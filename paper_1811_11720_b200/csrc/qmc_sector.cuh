@@ -159,7 +159,7 @@ __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned 
 #include "qmc_sector_interp.inc"
 
 // S2-S4 for the G points of one lattice index: x[q][j] and the weight W[q] (Eq. 12, Eq. 18)
-template <int DP, int G, bool WIDE, int TR, bool FIT>
+template <int DP, int G, bool WIDE, int TR, int FIT>
 __device__ __forceinline__ void sector_coords(const typename Res<WIDE>::T (&r)[DP], const EvalCtx& cx, double (&x)[G][DP],
                                               double (&W)[G]) {
     double P[G], D[G];
@@ -170,7 +170,7 @@ __device__ __forceinline__ void sector_coords(const typename Res<WIDE>::T (&r)[D
         const double rd = Res<WIDE>::to_double(r[j]);
         double fa, fb, dl[G];
         FitC fc;
-        load_slot<DP, G, FIT>(cx.sbase, cx.delta, j, cx.fit_full != 0, fa, fb, fc, dl);
+        load_slot<DP, G, FIT>(cx.sbase, cx.delta, j, fa, fb, fc, dl);
 #pragma unroll
         for (int q = 0; q < G; ++q)
             x[q][j] = point_coord<TR, FIT>(rd, cx.inv_n, dl[q], fc, cx.sbase + SmemOff<DP, G>::kor, cx.kor_r, P[q], D[q]);
@@ -179,22 +179,30 @@ __device__ __forceinline__ void sector_coords(const typename Res<WIDE>::T (&r)[D
     for (int q = 0; q < G; ++q) W[q] = point_weight<TR, FIT>(P[q], D[q], cx.wconst, cx.kor_r);
 }
 
-// Transform and fit map are selected per point by a warp-uniform switch, so that the interpreter
-// exists once per kernel (not once per transform variant).
-template <int DP, int G, bool WIDE> struct SectorEval {
+// Transform and fit map are selected per point by a warp-uniform switch, so that the interpreter exists once per
+// tile loop.  SLOW = false: the specialised transforms without fit map (inlined tile loop of the kernel); SLOW = true:
+// every other combination (generic weight transforms, fit maps), reached through a real call (run_tile_call).
+template <int DP, int G, bool WIDE, bool SLOW> struct SectorEval {
     static constexpr int NC = 1;
     typedef unsigned Extra;                                  // shared address of the CTA's SectorSmem
     static __device__ __forceinline__ void eval(const typename Res<WIDE>::T (&r)[DP], const SmemCtx<DP, G>&, const unsigned& exbase,
                                                 const EvalCtx& cx, double (&acc)[G][1]) {
         double x[G][DP], num[G];
-        switch (cx.sel) {
-#define QMC_CASE(TRK, FITB) \
-    case TRK * 2 + (FITB ? 1 : 0): sector_coords<DP, G, WIDE, TRK, FITB>(r, cx, x, num); break;
-            QMC_CASE(TR_NONE, false) QMC_CASE(TR_NONE, true) QMC_CASE(TR_BAKER, false) QMC_CASE(TR_BAKER, true)
-            QMC_CASE(TR_KOR3, false) QMC_CASE(TR_KOR3, true) QMC_CASE(TR_KORR, false)
-#undef QMC_CASE
-            default: sector_coords<DP, G, WIDE, TR_KORR, true>(r, cx, x, num); break;
+#define QMC_CASE(TRK, FITM) \
+    case TRK * 3 + FITM: sector_coords<DP, G, WIDE, TRK, FITM>(r, cx, x, num); break;
+        if (!SLOW) {
+            switch (cx.sel) {
+                QMC_CASE(TR_NONE, 0) QMC_CASE(TR_BAKER, 0)
+                default: sector_coords<DP, G, WIDE, TR_KOR3, 0>(r, cx, x, num); break;
+            }
+        } else {
+            switch (cx.sel) {
+                QMC_CASE(TR_NONE, 1) QMC_CASE(TR_NONE, 2) QMC_CASE(TR_BAKER, 1) QMC_CASE(TR_BAKER, 2) QMC_CASE(TR_KOR3, 1)
+                QMC_CASE(TR_KOR3, 2) QMC_CASE(TR_KORR, 0) QMC_CASE(TR_KORR, 1)
+                default: sector_coords<DP, G, WIDE, TR_KORR, 2>(r, cx, x, num); break;
+            }
         }
+#undef QMC_CASE
         double c0u, c0f;
         lds_f64x2(exbase + SectorOff::c0, c0u, c0f);
         double U[G], F[G];
@@ -264,7 +272,9 @@ __global__ void __launch_bounds__(kThreads, SectorMinBlocks<DP, G>::value) fused
             }
             __syncthreads();
         }
-        run_tile<SectorEval<DP, G, WIDE>, DP, G, WIDE>(sm, sbase, exbase, tile_local, changed, partials);
+        const bool fast = !sm.prob.has_fit && sm.prob.tr_kind != TR_KORR;
+        if (fast) run_tile<SectorEval<DP, G, WIDE, false>, DP, G, WIDE>(sm, sbase, exbase, tile_local, changed, partials);
+        else run_tile_call<SectorEval<DP, G, WIDE, true>, DP, G, WIDE>(sm, sbase, exbase, tile_local, changed, partials);
     }
 }
 

@@ -370,6 +370,29 @@ def test_config4_projection_and_fit():
             assert stored.tobytes() == fit_or.tobytes()
 
 
+def test_projection_to_full_fit_to_integration():
+    """row f-2 end to end: device projection pass (Eq. 20) -> qmc_fit_polysingular (Eq. 19, bounds PAPER.md L231) -> fused
+    integration with the fitted map; the fitted coefficients are an input of both sides, so parity holds at the usual bars,
+    and for this peaked integrand the fitted map reduces the error estimate (the purpose of section 2.4)"""
+    d, n = 3, 16381
+    rng = synth.MT19937_64(31337)
+    prm = np.array([9.0, 7.0, 8.0] + [0.02, 0.97, 0.03])                               # narrow peaks at the boundary
+    sh = synth.draw_shifts(rng, 8, d)
+    z = synth.korobov_form_vector(n, d, 1 + n // 3)
+    base = synth.problem(1, prm, n, z, sh, BAKER, name="peaked")
+    H = binding.DeviceBatch([dict(base, transform=NONE)]).project(0, 256).cpu().numpy()
+    fit = binding.qmc_fit_polysingular(H)
+    assert np.any(fit[:, 2:4] > 0)                          # the pole terms are used for this integrand
+    fitted = dict(base, fit_coeffs=fit, name="peaked.fitted")
+    assert binding.qmc_validate_problem_host(fitted) == 0
+    sms, means, errs = check_against_oracle([base, fitted])
+    cc, w = prm[:d], prm[d:]
+    exact = np.prod(cc * (np.arctan(cc * (1 - w)) + np.arctan(cc * w)))                # Genz product peak, PAPER.md L712-L713
+    for i in range(2):
+        assert abs(means[i, 0] - exact) <= 6 * errs[i, 0]
+    assert errs[1, 0] < 0.2 * errs[0, 0]                    # (the CPU experiment behind this test saw a factor 40)
+
+
 # ------------------------------------------------------------------------------------------------
 # boundary behaviour on the device
 # ------------------------------------------------------------------------------------------------
