@@ -43,7 +43,8 @@ namespace {
 
 typedef unsigned __int128 u128;
 
-enum { FAM_OSC = 0, FAM_PRODPEAK = 1, FAM_CEXP = 2, FAM_SECTOR = 3 };
+enum { FAM_OSC = 0, FAM_PRODPEAK = 1, FAM_CEXP = 2, FAM_SECTOR = 3, FAM_CORNER = 4, FAM_GAUSS = 5, FAM_C0 = 6, FAM_DISC = 7 };
+const int FAM_LAST = FAM_DISC;
 // transform ids: Table A.2.  Korobov<r> = 100 + r; Sidi<r> = 200 + r; Korobov<r0,r1> = 1000 + 16 r0 + r1.
 enum { TR_NONE = 0, TR_BAKER = 1, TR_KOROBOV = 100, TR_SIDI = 200, TR_KOROBOV_ASYM = 1000 };
 const int MAX_DIM = 64;
@@ -174,6 +175,10 @@ double sparse_poly(const double* c, const double* e, int count, int dim, const d
 //  1 Genz product peak f = prod 1/(c_j^-2 + (x_j - w_j)^2)
 //  2 complex           f = exp(i sum a_j x_j) prod (1 + b_j x_j)            BASELINE.json configs[2]
 //  3 sector-like       f = prod x_j^nu_j * U(x)^a / F(x)^b                  BASELINE.json configs[3]
+//  4 Genz corner peak  f = (1 + sum c_j x_j)^-(d+1)             [c]
+//  5 Genz Gaussian     f = exp(-sum c_j^2 (x_j - w_j)^2)        [c, w]
+//  6 Genz C^0          f = exp(-sum c_j |x_j - w_j|)            [c, w]
+//  7 Genz discontinuous f = 0 if x_1 > w_1 or x_2 > w_2, else exp(sum c_j x_j)   [c, w_1, w_2]
 inline void integrand(int fam, const double* p, int dim, const double* x, double* re, double* im) {
     *im = 0.0;
     if (fam == FAM_OSC) {
@@ -188,6 +193,23 @@ inline void integrand(int fam, const double* p, int dim, const double* x, double
         double ph = 0.0, pr = 1.0;
         for (int j = 0; j < dim; ++j) { ph += p[j] * x[j]; pr *= 1.0 + p[dim + j] * x[j]; }
         *re = std::cos(ph) * pr; *im = std::sin(ph) * pr;
+    } else if (fam == FAM_CORNER) {
+        double b = 1.0;
+        for (int j = 0; j < dim; ++j) b += p[j] * x[j];
+        *re = 1.0 / ipow(b, dim + 1);
+    } else if (fam == FAM_GAUSS) {
+        double e = 0.0;
+        for (int j = 0; j < dim; ++j) { double t = x[j] - p[dim + j]; e += p[j] * p[j] * t * t; }
+        *re = std::exp(-e);
+    } else if (fam == FAM_C0) {
+        double e = 0.0;
+        for (int j = 0; j < dim; ++j) e += p[j] * std::fabs(x[j] - p[dim + j]);
+        *re = std::exp(-e);
+    } else if (fam == FAM_DISC) {
+        bool zero = false;
+        double e = 0.0;
+        for (int j = 0; j < dim; ++j) { e += p[j] * x[j]; if (j < 2 && x[j] > p[dim + j]) zero = true; }
+        *re = zero ? 0.0 : std::exp(e);
     } else {
         int a = (int)p[0], b = (int)p[1], nU = (int)p[2], nF = (int)p[3];
         const double* nu = p + 4;
@@ -206,6 +228,9 @@ int expected_params(int fam, const double* p, int dim) {
     if (fam == FAM_OSC) return 1 + dim;
     if (fam == FAM_PRODPEAK || fam == FAM_CEXP) return 2 * dim;
     if (fam == FAM_SECTOR) { int nU = (int)p[2], nF = (int)p[3]; return 4 + dim + (nU + nF) * (1 + dim); }
+    if (fam == FAM_CORNER) return dim;
+    if (fam == FAM_GAUSS || fam == FAM_C0) return 2 * dim;
+    if (fam == FAM_DISC) return dim + (dim < 2 ? dim : 2);
     return -1;
 }
 
@@ -259,7 +284,7 @@ int oracle_transform(int tr, double u, double* y, double* w) {
 int oracle_fit_map(const double* a, double y, double* x, double* dp) { fit_map(a, y, x, dp); return 0; }
 
 int oracle_integrand(int fam, const double* params, int n_params, int dim, const double* x, double* out2) {
-    if (fam < 0 || fam > 3 || dim < 1 || dim > MAX_DIM) return -8;
+    if (fam < 0 || fam > FAM_LAST || dim < 1 || dim > MAX_DIM) return -8;
     if (expected_params(fam, params, dim) != n_params) return -9;
     integrand(fam, params, dim, x, &out2[0], &out2[1]);
     return 0;
@@ -270,7 +295,7 @@ int oracle_integrand(int fam, const double* params, int n_params, int dim, const
 int oracle_shift_sums(int fam, const double* params, int n_params, int dim, uint64_t n, const uint64_t* z,
                       const double* shifts, int m, int tr, const double* fit, uint64_t k_begin, uint64_t k_end,
                       double* out_sums) {
-    if (fam < 0 || fam > 3) return -8;
+    if (fam < 0 || fam > FAM_LAST) return -8;
     if (dim < 1 || dim > MAX_DIM) return -2;
     if (expected_params(fam, params, dim) != n_params) return -9;
     Transform trf;
@@ -340,7 +365,7 @@ int oracle_integrate(int fam, const double* params, int n_params, int dim, uint6
 // |f| is the modulus for the complex family.  Compensated per bin, k increasing.
 int oracle_project(int fam, const double* params, int n_params, int dim, uint64_t n, const uint64_t* z,
                    const double* shift, int bins, double* out_hist) {
-    if (fam < 0 || fam > 3) return -8;
+    if (fam < 0 || fam > FAM_LAST) return -8;
     if (dim < 1 || dim > MAX_DIM) return -2;
     if (expected_params(fam, params, dim) != n_params) return -9;
     const double inv_n = 1.0 / (double)n;

@@ -18,6 +18,10 @@ import os
 import numpy as np
 
 FAMILY_GENZ_OSC, FAMILY_GENZ_PRODPEAK, FAMILY_CEXP_POLY, FAMILY_SECTOR = 0, 1, 2, 3
+FAMILY_GENZ_CORNER, FAMILY_GENZ_GAUSSIAN, FAMILY_GENZ_C0, FAMILY_GENZ_DISCONT = 4, 5, 6, 7
+# integrand difficulties ||c||_1 of the paper's Genz protocol, families 1..6
+GENZ_DIFFICULTY = {FAMILY_GENZ_OSC: 6.0, FAMILY_GENZ_PRODPEAK: 18.0, FAMILY_GENZ_CORNER: 2.2, FAMILY_GENZ_GAUSSIAN: 15.2,
+                   FAMILY_GENZ_C0: 16.1, FAMILY_GENZ_DISCONT: 16.4}
 TRANSFORM_NONE, TRANSFORM_BAKER, TRANSFORM_KOROBOV = 0, 1, 100      # Korobov weight r = 100 + r
 TRANSFORM_SIDI = 200                                                # Sidi weight r = 200 + r
 TRANSFORM_KOROBOV_ASYM = 1000                                       # Korobov weights (r0, r1) = 1000 + 16 r0 + r1
@@ -110,6 +114,21 @@ def genz_prodpeak(rng, d):
     c = [rng.uniform_range(1.0, 5.0) for _ in range(d)]
     w = [rng.uniform() for _ in range(d)]
     return np.array(c + w, dtype=np.float64)
+
+
+def genz_protocol(rng, family, d):
+    """Parameters of one Genz test integral as in the paper's protocol: w_i ~ U[0,1), c_i > 0 random and
+    rescaled to the family's difficulty ||c||_1; packed in the family's layout (include/qmc_lattice.h)."""
+    c = np.array([rng.uniform() + 1e-3 for _ in range(d)])
+    c *= GENZ_DIFFICULTY[family] / c.sum()
+    w = np.array([rng.uniform() for _ in range(d)])
+    if family == FAMILY_GENZ_OSC:
+        return np.concatenate([[w[0]], c])
+    if family == FAMILY_GENZ_CORNER:
+        return c.copy()
+    if family == FAMILY_GENZ_DISCONT:
+        return np.concatenate([c, w[:min(d, 2)]])
+    return np.concatenate([c, w])
 
 
 def cexp_poly(rng, d):

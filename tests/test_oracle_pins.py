@@ -295,6 +295,63 @@ def test_family2_closed_form():
     _check_vs_exact(p, closed_cexp(prm), rel=1e-6)
 
 
+def closed_genz(fam, prm, d):
+    """analytic integrals of Genz families 3-6 over the unit cube"""
+    c = prm[:d]
+    if fam == synth.FAMILY_GENZ_CORNER:                     # inclusion-exclusion over the corners
+        tot = 0.0
+        for mask in range(1 << d):
+            sel = [j for j in range(d) if mask >> j & 1]
+            tot += (-1.0) ** len(sel) / (1.0 + sum(c[j] for j in sel))
+        return tot / (math.factorial(d) * np.prod(c))
+    if fam == synth.FAMILY_GENZ_GAUSSIAN:
+        w = prm[d:]
+        return float(np.prod(np.sqrt(np.pi) / (2 * c) * (scipy.special.erf(c * (1 - w)) + scipy.special.erf(c * w))))
+    if fam == synth.FAMILY_GENZ_C0:
+        w = prm[d:]
+        return float(np.prod((2.0 - np.exp(-c * w) - np.exp(-c * (1 - w))) / c))
+    b = np.ones(d)
+    b[:min(d, 2)] = prm[d:]
+    return float(np.prod(np.expm1(c * b) / c))
+
+
+@pytest.mark.parametrize("fam", [4, 5, 6, 7])
+def test_genz_families_3_to_6_pointwise_and_closed_form(fam):
+    rng = synth.MT19937_64(600 + fam)
+    d = 4
+    prm = synth.genz_protocol(rng, fam, d)
+    # pointwise against the definitions (PAPER.md L714-L722)
+    for _ in range(20):
+        x = np.array([rng.uniform() for _ in range(d)])
+        c = prm[:d]
+        if fam == 4:
+            want = (1.0 + c @ x) ** -(d + 1)
+        elif fam == 5:
+            want = math.exp(-np.sum(c ** 2 * (x - prm[d:]) ** 2))
+        elif fam == 6:
+            want = math.exp(-np.sum(c * np.abs(x - prm[d:])))
+        else:
+            want = 0.0 if (x[0] > prm[d] or x[1] > prm[d + 1]) else math.exp(c @ x)
+        assert abs(oracle.integrand(fam, prm, x) - want) <= 1e-14 * max(abs(want), 1e-300)
+    # the rule integrates them: closed form inside the error bar (baker copes with the kinks of families 5, 6)
+    n = 65521
+    tr = synth.TRANSFORM_KOROBOV + 3 if fam in (4, 5) else synth.TRANSFORM_BAKER
+    p = synth.problem(fam, prm, n, synth.genvec(n, 4), synth.draw_shifts(rng, 8, d), tr)
+    _check_vs_exact(p, closed_genz(fam, prm, d), nsig=6.0, rel={4: 1e-8, 5: 1e-6, 6: 1e-4, 7: 2e-2}[fam])
+    with pytest.raises(ValueError):
+        oracle.integrand(fam, prm[:-1], np.zeros(d))
+
+
+def test_corner_peak_closed_form_against_nested_quadrature():
+    # the inclusion-exclusion formula itself, checked by tensor Gauss-Legendre at d = 3
+    c = np.array([0.9, 0.4, 0.7])
+    xs, ws = np.polynomial.legendre.leggauss(24)
+    xs, ws = 0.5 * (xs + 1), 0.5 * ws
+    X = np.stack(np.meshgrid(xs, xs, xs, indexing="ij"), -1)
+    quad = np.sum(np.einsum("i,j,k->ijk", ws, ws, ws) * (1.0 + X @ c) ** -4.0)
+    assert abs(quad - closed_genz(4, c, 3)) < 1e-13
+
+
 def test_fit_map_leaves_integral_invariant():
     # Eq. 18 (P:L217) with arbitrary valid coefficients, composed as x = p(phi(u)) (P:L338)
     n, d = 65537, 4
