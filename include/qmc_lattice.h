@@ -31,6 +31,11 @@
  *      QMC_FAMILY_GENZ_OSC      [u0, a_1..a_d]            f = cos(2 pi u0 + sum a_j x_j)
  *      QMC_FAMILY_GENZ_PRODPEAK [c_1..c_d, w_1..w_d]      f = prod 1/(c_j^-2 + (x_j-w_j)^2)
  *      QMC_FAMILY_CEXP_POLY     [a_1..a_d, b_1..b_d]      f = exp(i sum a_j x_j) prod(1+b_j x_j)  (complex)
+ *      QMC_FAMILY_GENZ_CORNER   [c_1..c_d]                f = (1 + sum c_j x_j)^-(d+1)
+ *      QMC_FAMILY_GENZ_GAUSSIAN [c_1..c_d, w_1..w_d]      f = exp(-sum c_j^2 (x_j-w_j)^2)
+ *      QMC_FAMILY_GENZ_C0       [c_1..c_d, w_1..w_d]      f = exp(-sum c_j |x_j-w_j|)
+ *      QMC_FAMILY_GENZ_DISCONT  [c_1..c_d, w_1, w_2]      f = 0 if x_1 > w_1 or x_2 > w_2, else exp(sum c_j x_j)
+ *                               (d = 1: [c_1, w_1])
  *      QMC_FAMILY_SECTOR        [a, b, nU, nF, nu_1..nu_d, cU_1..cU_nU, eU_{1,1}..eU_{nU,d},
  *                                cF_1..cF_nF, eF_{1,1}..eF_{nF,d}]
  *                               f = prod x_j^nu_j * U(x)^a / F(x)^b, U = sum_t cU_t prod_j x_j^eU_{t,j}
@@ -64,7 +69,9 @@ typedef enum {
     QMC_ERR_NONFINITE = -13  /* a result is NaN/Inf (synchronous entry only; results are still written) */
 } qmc_status;
 
-enum { QMC_FAMILY_GENZ_OSC = 0, QMC_FAMILY_GENZ_PRODPEAK = 1, QMC_FAMILY_CEXP_POLY = 2, QMC_FAMILY_SECTOR = 3 };
+enum { QMC_FAMILY_GENZ_OSC = 0, QMC_FAMILY_GENZ_PRODPEAK = 1, QMC_FAMILY_CEXP_POLY = 2, QMC_FAMILY_SECTOR = 3,
+       /* the remaining functions of Genz' test suite: */
+       QMC_FAMILY_GENZ_CORNER = 4, QMC_FAMILY_GENZ_GAUSSIAN = 5, QMC_FAMILY_GENZ_C0 = 6, QMC_FAMILY_GENZ_DISCONT = 7 };
 
 /* Periodizing transforms, Table A.2: none; baker Eq. 17;
  * Korobov with symmetric weight r, Eq. 15: QMC_TRANSFORM_KOROBOV + r, r = 1..6;

@@ -30,6 +30,7 @@ template <int FAMILY> struct FamTraits;
 template <> struct FamTraits<QMC_FAMILY_GENZ_OSC> { static constexpr int NC = 1; };
 template <> struct FamTraits<QMC_FAMILY_GENZ_PRODPEAK> { static constexpr int NC = 1; };
 template <> struct FamTraits<QMC_FAMILY_CEXP_POLY> { static constexpr int NC = 2; };
+template <> struct FamTraits<kKernelFamilyGenzMisc> { static constexpr int NC = 1; };
 
 // Shared-memory image of the problem a CTA is working on.  The double arrays at the front are the
 // operands of the inner loop; they are read with ld.shared at sbase + compile-time offsets.
@@ -58,18 +59,36 @@ template <int DP, int G> struct SmemOff {
 //  OSC       f = cos(2 pi u0 + sum a_j x_j)
 //  PRODPEAK  f = prod 1/(c_j^-2 + (x_j - w_j)^2)  = 1 / prod(...)
 //  CEXP      f = exp(i sum a_j x_j) prod (1 + b_j x_j)             BASELINE.json configs[2]
+//  kernel family 4 (runtime sub-kind = public family id), s0 = the sum below, s1 = 1 once the integrand is cut to 0:
+//    CORNER    f = (1 + sum c_j x_j)^-(d+1)                        P:L714-L715   fa = c_j
+//    GAUSSIAN  f = exp(-sum c_j^2 (x_j - w_j)^2)                   P:L716-L717   fa = -c_j^2, fb = w_j
+//    C0        f = exp(-sum c_j |x_j - w_j|)                       P:L718-L720   fa = -c_j,   fb = w_j
+//    DISCONT   f = 0 if x_1 > w_1 or x_2 > w_2 else exp(sum c_j x_j)  P:L721-L722   fa = c_j, fb = w_j (j < 2), +inf beyond
 template <int FAMILY> __device__ __forceinline__ void fam_init(double& s0, double& s1, double fam0) {
     if (FAMILY == QMC_FAMILY_GENZ_OSC) { s0 = fam0; s1 = 0.0; }
     else if (FAMILY == QMC_FAMILY_GENZ_PRODPEAK) { s0 = 1.0; s1 = 0.0; }
+    else if (FAMILY == kKernelFamilyGenzMisc) { s0 = 0.0; s1 = 0.0; }
     else { s0 = 0.0; s1 = 1.0; }
 }
-template <int FAMILY> __device__ __forceinline__ void fam_dim(double& s0, double& s1, double x, double fa, double fb) {
+template <int FAMILY> __device__ __forceinline__ void fam_dim(double& s0, double& s1, double x, double fa, double fb, int kind) {
     if (FAMILY == QMC_FAMILY_GENZ_OSC) { s0 = __fma_rn(fa, x, s0); }
     else if (FAMILY == QMC_FAMILY_GENZ_PRODPEAK) { const double t = x - fb; s0 *= __fma_rn(t, t, fa); }   // fa = c_j^-2, fb = w_j
+    else if (FAMILY == kKernelFamilyGenzMisc) {
+        if (kind == QMC_FAMILY_GENZ_GAUSSIAN) { const double t = x - fb; s0 = __fma_rn(fa * t, t, s0); }
+        else if (kind == QMC_FAMILY_GENZ_C0) { s0 = __fma_rn(fa, fabs(x - fb), s0); }
+        else { s0 = __fma_rn(fa, x, s0); if (x > fb) s1 = 1.0; }          // corner peak (fb = +inf) and discontinuous
+    }
     else { s0 = __fma_rn(fa, x, s0); s1 *= __fma_rn(fb, x, 1.0); }
 }
-// adds W*f to acc[0..NC)
-template <int FAMILY> __device__ __forceinline__ void fam_finish(double s0, double s1, double W, bool use_w, double* acc) {
+// adds W*f to acc[0..NC); kind / pw: sub-kind and exponent d + 1 of kernel family 4
+template <int FAMILY> __device__ __forceinline__ void fam_finish(double s0, double s1, double W, bool use_w, double* acc, int kind, int pw) {
+    if (FAMILY == kKernelFamilyGenzMisc) {
+        double f;
+        if (kind == QMC_FAMILY_GENZ_CORNER) f = rcp_nr(ipow_small(1.0 + s0, pw));
+        else f = (s1 != 0.0) ? 0.0 : exp(s0);
+        acc[0] = use_w ? __fma_rn(W, f, acc[0]) : acc[0] + f;
+        return;
+    }
     if (FAMILY == QMC_FAMILY_GENZ_OSC) {
         const double f = cos(s0);
         acc[0] = use_w ? __fma_rn(W, f, acc[0]) : acc[0] + f;
@@ -220,6 +239,7 @@ struct EvalCtx {            // per-tile constants held in registers
     double inv_n, wconst, fam0;
     int kor_r;              // generic weight transforms: DevProblem::gen
     int sel;                // tr_kind * 3 + fit mode (0 none, 1 cubic, 2 cubic + pole terms)
+    int fam_kind, fam_pow;  // kernel family 4: public family id and the corner-peak exponent d + 1
 };
 
 template <int FAMILY, int DP, int G, bool WIDE, int TR, int FIT>
@@ -242,14 +262,14 @@ __device__ __forceinline__ void eval_point_group(const typename Res<WIDE>::T (&r
                 s0[q] *= __fma_rn(dd, dd, fa);
             } else {
                 const double x = point_coord<TR, FIT>(rd, cx.inv_n, dl[q], fc, cx.sbase + SmemOff<DP, G>::kor, cx.kor_r, P[q], D[q]);
-                fam_dim<FAMILY>(s0[q], s1[q], x, fa, fb);
+                fam_dim<FAMILY>(s0[q], s1[q], x, fa, fb, cx.fam_kind);
             }
         }
     }
     constexpr bool USEW = (TR == TR_KOR3 || TR == TR_KORR || FIT != 0);
 #pragma unroll
     for (int q = 0; q < G; ++q)
-        fam_finish<FAMILY>(s0[q], s1[q], point_weight<TR, FIT>(P[q], D[q], cx.wconst, cx.kor_r), USEW, acc[q]);
+        fam_finish<FAMILY>(s0[q], s1[q], point_weight<TR, FIT>(P[q], D[q], cx.wconst, cx.kor_r), USEW, acc[q], cx.fam_kind, cx.fam_pow);
 }
 
 struct NoExtra {};
@@ -278,6 +298,7 @@ __device__ __forceinline__ void run_tile(SmemCtx<DP, G>& sm, unsigned sbase, con
     EvalCtx cx;
     cx.sbase = sbase; cx.inv_n = pb.inv_n; cx.wconst = pb.wconst; cx.fam0 = sm.fam0; cx.kor_r = pb.gen;
     cx.sel = pb.tr_kind * 3 + (pb.has_fit ? 1 + sm.fit_full : 0);
+    cx.fam_kind = pb.family; cx.fam_pow = pb.dim + 1;
     typedef SmemCtx<DP, G> Ctx;
     typedef SmemOff<DP, G> Off;
     static_assert(offsetof(Ctx, fam) == Off::fam && offsetof(Ctx, fit) == Off::fit && offsetof(Ctx, kor) == Off::kor &&
@@ -398,6 +419,10 @@ __device__ __forceinline__ SlotConst derive_slot(const DevProblem& pb, int j) {
         if (pb.family == QMC_FAMILY_GENZ_OSC) { s.fa = p[1 + j]; }
         else if (pb.family == QMC_FAMILY_GENZ_PRODPEAK) { const double c = p[j]; s.fa = __ddiv_rn(1.0, __dmul_rn(c, c)); s.fb = p[d + j]; }
         else if (pb.family == QMC_FAMILY_CEXP_POLY) { s.fa = p[j]; s.fb = p[d + j]; }
+        else if (pb.family == QMC_FAMILY_GENZ_CORNER) { s.fa = p[j]; s.fb = __longlong_as_double(0x7ff0000000000000ll); }
+        else if (pb.family == QMC_FAMILY_GENZ_GAUSSIAN) { s.fa = -__dmul_rn(p[j], p[j]); s.fb = p[d + j]; }
+        else if (pb.family == QMC_FAMILY_GENZ_C0) { s.fa = -p[j]; s.fb = p[d + j]; }
+        else if (pb.family == QMC_FAMILY_GENZ_DISCONT) { s.fa = p[j]; s.fb = j < 2 ? p[d + j] : __longlong_as_double(0x7ff0000000000000ll); }
         if (pb.has_fit) {
             const double* c = pb.fit + 6 * j;
             const double a4 = c[4], a5 = c[5];
@@ -405,6 +430,8 @@ __device__ __forceinline__ SlotConst derive_slot(const DevProblem& pb, int j) {
             s.f[0] = a4; s.f[1] = a5; s.f[2] = a6; s.f[3] = 2.0 * a5; s.f[4] = 3.0 * a6;
             s.f[5] = c[0]; s.f[6] = __dmul_rn(c[2], __dadd_rn(c[0], -1.0)); s.f[7] = c[1]; s.f[8] = __dmul_rn(c[3], __dadd_rn(c[1], -1.0));
         }
+    } else if (pb.family == QMC_FAMILY_GENZ_CORNER || pb.family == QMC_FAMILY_GENZ_DISCONT) {
+        s.fb = __longlong_as_double(0x7ff0000000000000ll);      // padded slot: fa = 0 adds nothing, x > +inf never cuts
     } else if (pb.family == QMC_FAMILY_GENZ_PRODPEAK) {
         // padded slot: the coordinate is pinned to u = 1/2, i.e. x = 1 (baker) or 1/2; factor (x - fb)^2 + fa = 1
         s.fa = 1.0;

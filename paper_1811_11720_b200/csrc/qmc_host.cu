@@ -39,7 +39,7 @@ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 int ncomp_of(int family) {
     if (family == QMC_FAMILY_CEXP_POLY) return 2;
-    if (family >= 0 && family <= QMC_FAMILY_SECTOR) return 1;
+    if (family >= 0 && family <= QMC_FAMILY_GENZ_DISCONT) return 1;
     return -1;
 }
 
@@ -100,6 +100,9 @@ int validate_struct(const qmc_problem& p, bool need_two_shifts) {
     if (!p.params || !p.z || !p.shifts) return QMC_ERR_NULL;
     if (p.family == QMC_FAMILY_GENZ_OSC && p.n_params != 1 + p.dim) return QMC_ERR_PARAMS;
     if ((p.family == QMC_FAMILY_GENZ_PRODPEAK || p.family == QMC_FAMILY_CEXP_POLY) && p.n_params != 2 * p.dim) return QMC_ERR_PARAMS;
+    if (p.family == QMC_FAMILY_GENZ_CORNER && p.n_params != p.dim) return QMC_ERR_PARAMS;
+    if ((p.family == QMC_FAMILY_GENZ_GAUSSIAN || p.family == QMC_FAMILY_GENZ_C0) && p.n_params != 2 * p.dim) return QMC_ERR_PARAMS;
+    if (p.family == QMC_FAMILY_GENZ_DISCONT && p.n_params != p.dim + std::min(p.dim, 2)) return QMC_ERR_PARAMS;
     if (p.family == QMC_FAMILY_SECTOR) {
         const int rest = p.n_params - 4 - p.dim;
         if (rest < 2 * (1 + p.dim) || rest % (1 + p.dim) != 0 || rest / (1 + p.dim) > 2 * kMaxSectorMono) return QMC_ERR_PARAMS;
@@ -124,7 +127,7 @@ bool force_wide() {
 
 // ---- launch plan: tiles, kernel variants, workspace layout (pure function of the problem structs) ----
 struct Variant {
-    int family, dp;
+    int family, dp;                  // kernel family (kernel_family(public id)), dimension slots
     bool wide;
     std::vector<int> plist;          // problem indices, queue order (most expensive tiles first)
     long long total_tiles = 0;
@@ -203,8 +206,8 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
         const int dp = dim_slots(d.family, d.dim, wide);
         Variant* v = nullptr;
         for (auto& c : plan->variants)
-            if (c.family == d.family && c.dp == dp && c.wide == wide) v = &c;
-        if (!v) { plan->variants.push_back(Variant{d.family, dp, wide, {}, 0}); v = &plan->variants.back(); }
+            if (c.family == kernel_family(d.family) && c.dp == dp && c.wide == wide) v = &c;
+        if (!v) { plan->variants.push_back(Variant{kernel_family(d.family), dp, wide, {}, 0}); v = &plan->variants.back(); }
         v->plist.push_back(i);
     }
     if (plan->variants.size() > 64) return QMC_ERR_WORKSPACE;
@@ -284,6 +287,7 @@ cudaError_t launch_closed(int family, int dp, bool wide, int grid, cudaStream_t 
         case 0: QMC_TRY_PARTS(0, launch_fused_part_, cudaErrorInvalidValue, dp, wide, grid, st, a)
         case 1: QMC_TRY_PARTS(1, launch_fused_part_, cudaErrorInvalidValue, dp, wide, grid, st, a)
         case 2: QMC_TRY_PARTS(2, launch_fused_part_, cudaErrorInvalidValue, dp, wide, grid, st, a)
+        case 4: QMC_TRY_PARTS(4, launch_fused_part_, cudaErrorInvalidValue, dp, wide, grid, st, a)
     }
     return cudaErrorInvalidValue;
 }
@@ -292,18 +296,19 @@ int occupancy_closed(int family, int dp, bool wide) {
         case 0: QMC_TRY_PARTS(0, occupancy_fused_part_, -1, dp, wide)
         case 1: QMC_TRY_PARTS(1, occupancy_fused_part_, -1, dp, wide)
         case 2: QMC_TRY_PARTS(2, occupancy_fused_part_, -1, dp, wide)
+        case 4: QMC_TRY_PARTS(4, occupancy_fused_part_, -1, dp, wide)
     }
     return -1;
 }
 #undef QMC_TRY_PARTS
 
 int occupancy(int family, int dp, bool wide) {
-    static int cache[4][33][2];
+    static int cache[5][33][2];
     int& c = cache[family][dp][wide ? 1 : 0];
     if (c > 0) return c;
     int v = -1;
     switch (family) {
-        case 0: case 1: case 2: v = occupancy_closed(family, dp, wide); break;
+        case 0: case 1: case 2: case 4: v = occupancy_closed(family, dp, wide); break;
         case 3: v = occupancy_fused_f3(dp, wide); break;
     }
     if (v > 0) c = v;
@@ -389,7 +394,7 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
         a.vq = queues[vi];
         cudaError_t e = cudaErrorInvalidValue;
         switch (v.family) {
-            case 0: case 1: case 2: e = launch_closed(v.family, v.dp, v.wide, grid, st, a); break;
+            case 0: case 1: case 2: case 4: e = launch_closed(v.family, v.dp, v.wide, grid, st, a); break;
             case 3: e = launch_fused_f3(v.dp, v.wide, grid, st, a); break;
         }
         if (e != cudaSuccess) return cuda_fail(e, "fused kernel launch");
@@ -460,6 +465,9 @@ int validate_values(const qmc_problem& p) {
 int family_param_count(int family, const double* params, int dim) {
     if (family == QMC_FAMILY_GENZ_OSC) return 1 + dim;
     if (family == QMC_FAMILY_GENZ_PRODPEAK || family == QMC_FAMILY_CEXP_POLY) return 2 * dim;
+    if (family == QMC_FAMILY_GENZ_CORNER) return dim;
+    if (family == QMC_FAMILY_GENZ_GAUSSIAN || family == QMC_FAMILY_GENZ_C0) return 2 * dim;
+    if (family == QMC_FAMILY_GENZ_DISCONT) return dim + std::min(dim, 2);
     if (family == QMC_FAMILY_SECTOR && params) {
         const double nU = params[2], nF = params[3];
         if (!(nU >= 1 && nU <= kMaxSectorMono && nF >= 1 && nF <= kMaxSectorMono)) return -1;

@@ -27,6 +27,10 @@ constexpr int kMaxSectorMono = 64;
 constexpr int kSectorLinSlots = 32;    // extra coefficient slots of a sector program: one dense linear form (<= 16 entries) per polynomial
 __host__ __device__ constexpr int sector_coef_slots(int nmono) { return nmono + kSectorLinSlots; }   // coefficient region of a program, in doubles
 
+// kernel family of a public family id: the four remaining Genz functions share one fused kernel (runtime sub-kind)
+constexpr int kKernelFamilyGenzMisc = 4;
+__host__ __device__ constexpr int kernel_family(int family) { return family <= QMC_FAMILY_SECTOR ? family : kKernelFamilyGenzMisc; }
+
 // transform kinds after host-side decoding
 enum : int { TR_NONE = 0, TR_BAKER = 1, TR_KOR3 = 2, TR_KORR = 3 };   // TR_KORR = the generic weight transforms, see GEN_*
 // generic weight transforms (one tile loop, selected per coordinate by DevProblem::gen = kind | r0 << 4 | r1 << 8):

@@ -62,6 +62,25 @@ __device__ double abs_integrand(const ProjArgs& a, const double* x) {
         for (int j = 0; j < d; ++j) pr *= __fma_rn(p[d + j], x[j], 1.0);
         return fabs(pr);
     }
+    if (a.family == QMC_FAMILY_GENZ_CORNER) {
+        double b = 1.0;
+        for (int j = 0; j < d; ++j) b = __fma_rn(p[j], x[j], b);
+        return fabs(1.0 / ipow_small(b, d + 1));
+    }
+    if (a.family == QMC_FAMILY_GENZ_GAUSSIAN || a.family == QMC_FAMILY_GENZ_C0) {
+        double e = 0.0;
+        for (int j = 0; j < d; ++j) {
+            const double t = x[j] - p[d + j];
+            e += (a.family == QMC_FAMILY_GENZ_GAUSSIAN) ? p[j] * p[j] * t * t : p[j] * fabs(t);
+        }
+        return exp(-e);
+    }
+    if (a.family == QMC_FAMILY_GENZ_DISCONT) {
+        double e = 0.0;
+        bool zero = false;
+        for (int j = 0; j < d; ++j) { e = __fma_rn(p[j], x[j], e); zero = zero || (j < 2 && x[j] > p[d + j]); }
+        return zero ? 0.0 : exp(e);
+    }
     const int pa = (int)p[0], pb = (int)p[1], nU = (int)p[2], nF = (int)p[3];
     double pre = 1.0;
     for (int j = 0; j < d; ++j) pre *= ipow_small(x[j], (int)p[4 + j]);
@@ -155,7 +174,7 @@ __global__ void __launch_bounds__(256) project_merge_kernel(ProjArgs a) {
 
 int plan_project(const qmc_problem* p, int bins, ProjArgs* a) {
     if (!p) return QMC_ERR_NULL;
-    if (p->family < 0 || p->family > QMC_FAMILY_SECTOR) return QMC_ERR_FAMILY;
+    if (p->family < 0 || p->family > QMC_FAMILY_GENZ_DISCONT) return QMC_ERR_FAMILY;
     if (p->dim < 1 || p->dim > QMC_MAX_DIM) return QMC_ERR_DIM;
     if (p->n < 2 || p->n >= (1ull << 53)) return QMC_ERR_N;
     if (bins < 2 || bins > 1024) return QMC_ERR_N;
@@ -163,6 +182,9 @@ int plan_project(const qmc_problem* p, int bins, ProjArgs* a) {
     if (!p->params || !p->z || !p->shifts) return QMC_ERR_NULL;
     if (p->family == QMC_FAMILY_GENZ_OSC && p->n_params != 1 + p->dim) return QMC_ERR_PARAMS;
     if ((p->family == QMC_FAMILY_GENZ_PRODPEAK || p->family == QMC_FAMILY_CEXP_POLY) && p->n_params != 2 * p->dim) return QMC_ERR_PARAMS;
+    if (p->family == QMC_FAMILY_GENZ_CORNER && p->n_params != p->dim) return QMC_ERR_PARAMS;
+    if ((p->family == QMC_FAMILY_GENZ_GAUSSIAN || p->family == QMC_FAMILY_GENZ_C0) && p->n_params != 2 * p->dim) return QMC_ERR_PARAMS;
+    if (p->family == QMC_FAMILY_GENZ_DISCONT && p->n_params != p->dim + (p->dim < 2 ? p->dim : 2)) return QMC_ERR_PARAMS;
     if (p->family == QMC_FAMILY_SECTOR && p->n_params < 4 + p->dim + 2 * (1 + p->dim)) return QMC_ERR_PARAMS;
     std::memset(a, 0, sizeof(*a));
     a->params = p->params;

@@ -78,6 +78,8 @@ def make(fam, d, n, m, tr, seed, fit=False, z=None, a_hi=1.0):
         prm = synth.genz_prodpeak(rng, d)
     elif fam == 2:
         prm = synth.cexp_poly(rng, d)
+    elif fam >= 4:
+        prm = synth.genz_protocol(rng, fam, d)               # Genz families 3-6 at the paper's difficulties
     else:
         prm = synth.sector(rng, d)
     sh = synth.draw_shifts(rng, m, d)
@@ -143,6 +145,21 @@ def test_means_all_transforms(fam, tr):
     probs = [make(fam, d, 8191, 6, tr, 300 + 10 * fam + tr % 97, fit=False),
              make(fam, d, 8191, 6, tr, 400 + 10 * fam + tr % 97, fit=True)]
     check_against_oracle(probs)
+
+
+@pytest.mark.parametrize("fam", [4, 5, 6, 7])
+@pytest.mark.parametrize("tr", [NONE, BAKER, K + 3, K + 1, SIDI + 2, KA + 16 * 2 + 1])
+def test_genz_families_3_to_6(fam, tr):
+    """corner peak, Gaussian, C^0, discontinuous (row f-4): every transform kind, with and without fit map"""
+    d = {4: 5, 5: 8, 6: 10, 7: 5}[fam]                       # the dimensions of the paper's protocol (L728)
+    check_against_oracle([make(fam, d, 8191, 6, tr, 3100 + 13 * fam + tr % 83), make(fam, d, 8191, 6, tr, 3200 + 13 * fam + tr % 83, fit=True),
+                          make(fam, d, 8191, 5, tr, 3300 + fam, fit="full")])
+
+
+@pytest.mark.parametrize("fam,d", [(4, 1), (4, 12), (4, 17), (5, 2), (5, 16), (6, 3), (6, 32), (7, 1), (7, 2), (7, 9), (7, 24)])
+def test_genz_families_3_to_6_dimension_slots(fam, d):
+    n = 65537 if d <= 16 else 8191
+    check_against_oracle([make(fam, d, n, 5, K + 3 if fam in (4, 5) else BAKER, 3400 + 31 * fam + d)])
 
 
 @pytest.mark.parametrize("fam,d", [(0, 3), (0, 16), (1, 8), (2, 5), (2, 12), (3, 6), (3, 9)])
@@ -339,6 +356,7 @@ def test_config4_full_size_vs_stored_oracle():
 # S10: projection pass and fit (Eq. 20; reading C-8)
 # ------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("fam,d,n,bins", [(0, 16, 65537, 256), (1, 8, 65537, 256), (2, 12, 16381, 64), (3, 6, 16381, 256),
+                                          (4, 5, 8191, 128), (5, 8, 8191, 128), (6, 10, 8191, 256), (7, 5, 8191, 64),
                                           (1, 5, 8191, 1024), (0, 32, 4099, 1024), (1, 2, 127, 2)])
 def test_projection_histogram(fam, d, n, bins):
     p = make(fam, d, n, 2, NONE, 1500 + fam + d)
