@@ -228,6 +228,65 @@ def closed_form(c, prm):
     return complex(np.prod((e - 1) / (1j * a) + b * (e / (1j * a) - (e - 1) / (1j * a) ** 2)))
 
 
+def genz_exact(fam, prm, d):
+    """analytic integrals of the six Genz functions over the unit cube: analysis only"""
+    from math import factorial
+    from scipy.special import erf
+    if fam == synth.FAMILY_GENZ_OSC:
+        a = prm[1:]
+        return float(np.cos(2 * np.pi * prm[0] + 0.5 * a.sum()) * np.prod(np.sin(a / 2) / (a / 2)))
+    c = prm[:d]
+    if fam == synth.FAMILY_GENZ_PRODPEAK:
+        w = prm[d:]
+        return float(np.prod(c * (np.arctan(c * (1 - w)) + np.arctan(c * w))))
+    if fam == synth.FAMILY_GENZ_CORNER:
+        tot = 0.0
+        for mask in range(1 << d):
+            sel = [j for j in range(d) if mask >> j & 1]
+            tot += (-1.0) ** len(sel) / (1.0 + sum(c[j] for j in sel))
+        return tot / (factorial(d) * np.prod(c))
+    if fam == synth.FAMILY_GENZ_GAUSSIAN:
+        w = prm[d:]
+        return float(np.prod(np.sqrt(np.pi) / (2 * c) * (erf(c * (1 - w)) + erf(c * w))))
+    if fam == synth.FAMILY_GENZ_C0:
+        w = prm[d:]
+        return float(np.prod((2.0 - np.exp(-c * w) - np.exp(-c * (1 - w))) / c))
+    b = np.ones(d)
+    b[:min(d, 2)] = prm[d:]
+    return float(np.prod(np.expm1(c * b) / c))
+
+
+def genz_table(binding, transform, dims=(5, 8, 10), sets=10, m=32, epsrel=1e-8, maxeval=7 * 10 ** 8):
+    """The protocol of the paper's Table 1 / Table 2: per family and dimension, `sets` random parameter
+    sets at the family's difficulty, eps_rel = 1e-8, at most 7e8 samples, 32 shifts; average correct digits
+    (against the analytic result) and seconds per integration through qmc_integrate on the committed lattice ladder."""
+    fams = [synth.FAMILY_GENZ_OSC, synth.FAMILY_GENZ_PRODPEAK, synth.FAMILY_GENZ_CORNER, synth.FAMILY_GENZ_GAUSSIAN,
+            synth.FAMILY_GENZ_C0, synth.FAMILY_GENZ_DISCONT]
+    rows = []
+    for fi, fam in enumerate(fams):
+        for d in dims:
+            ln, lz = synth.ladder(d, 16777213)
+            rng = synth.MT19937_64(1811117400 + 100 * fi + d)
+            digits, secs, evals = [], [], []
+            for k in range(sets + 1):                       # set 0 is the warm-up
+                prm = synth.genz_protocol(rng, fam, d)
+                sh = synth.draw_shifts(rng, m, d)
+                t0 = time.perf_counter()
+                res, st = binding.qmc_integrate(fam, prm, d, transform, ln, lz, sh, min_n=1000, min_m=m, epsrel=epsrel, epsabs=0.0,
+                                                maxeval=maxeval)
+                dt = time.perf_counter() - t0
+                if k == 0:
+                    continue
+                exact = genz_exact(fam, prm, d)
+                rel = abs(res["integral"][0] - exact) / abs(exact)
+                digits.append(-np.log10(max(rel, 1e-16)))
+                secs.append(dt)
+                evals.append(res["evaluations"])
+            rows.append({"family": fi + 1, "d": d, "digits": float(np.mean(digits)), "seconds": float(np.mean(secs)),
+                         "evaluations": float(np.mean(evals))})
+    return rows
+
+
 def time_to_target(binding, c, probs, epsrel=1e-8):
     """BASELINE metric part 3: wall time of the paper's iteration (qmc_integrate) to an ESTIMATED relative
     error of 1e-8 on the committed lattice ladder, shifts and parameters of configs[c]; earlier lattices are discarded (L357)."""
@@ -274,6 +333,14 @@ def run_ours(args):
         t = torch.tensor([x], dtype=torch.float64, device=device)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         return float(t.item())
+
+    if args.genz_table:
+        out = {"genz_protocol": {"korobov3": genz_table(binding, synth.TRANSFORM_KOROBOV + 3),
+                                 "baker_d10": genz_table(binding, synth.TRANSFORM_BAKER, dims=(10,))},
+               "note": "PAPER.md Table 1 / Table 2 protocol on one B200; averages over 10 seeded parameter sets"}
+        if rank == 0:
+            print(json.dumps(out))
+        return
 
     binding.qmc_profile_enable(True)
     flush = L2Flusher(torch, device)
@@ -418,6 +485,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--main-only", action="store_true", help="time configs[1] only (skip the 'others' list)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--genz-table", action="store_true",
+                    help="run the Genz protocol of the paper's Table 1 / Table 2 through qmc_integrate instead of the throughput bench")
     ap.add_argument("--shrink", type=int, default=1,
                     help="profiling only: run 1/S of every config's work (fewer sectors / a smaller prime n)")
     ap.add_argument("--main", type=int, default=MAIN_CONFIG, choices=[0, 1, 2, 3, 4],
