@@ -108,6 +108,7 @@ template <int FAMILY> __device__ __forceinline__ void fam_finish(double s0, doub
 struct FitC {                                     // fit map of one dimension (Eq. 19)
     double f0, f1, f2, f3, f4;                    // a4, a5, a6, 2 a5, 3 a6: cubic part and its derivative
     double a0, k2, a1, k3;                        // poles: a0, a2 (a0 - 1), a1, a3 (a1 - 1)   (fit mode 2 only)
+    int mode;                                     // generic tile loop (FIT_RT): fit mode of the problem, warp-uniform
 };
 
 // The generic weight transforms (Table A.2), selected per coordinate by the warp-uniform code
@@ -119,6 +120,8 @@ struct FitC {                                     // fit map of one dimension (E
 //                     I_n = ((n-1) I_{n-2} - sin^(n-1) cos) / n, I_0 = theta, I_1 = 1 - cos
 __device__ __forceinline__ double generic_transform(double t, unsigned kor_addr, int gen, double& P) {
     const int kind = gen & 15, r0 = (gen >> 4) & 15, r1 = (gen >> 8) & 15;
+    if (kind == GEN_NONE) return wrap_u(t);
+    if (kind == GEN_BAKER) return 1.0 - fabs(baker_w(t));
     if (kind == GEN_KOROBOV_SYM) {
         const double c = centre_c(t);
         const double s = c * c;
@@ -189,12 +192,13 @@ __device__ __forceinline__ double point_coord(double rd, double inv_n, double de
             x = generic_transform(t, kor_addr, kor_r, P);
         }
     }
-    if (FIT) {                                                // S4: fit map of Eq. 19
+    const int mode = (FIT == FIT_RT) ? fc.mode : FIT;
+    if (FIT && mode) {                                        // S4: fit map of Eq. 19
         const double y = x;
         const double h = __fma_rn(y, __fma_rn(y, fc.f2, fc.f1), fc.f0);
         double dp = __fma_rn(y, __fma_rn(y, fc.f4, fc.f3), fc.f0);   // cubic part of p'(y)
         x = y * h;                                            // cubic part of p(y)
-        if (FIT == 2) fit_poles(y, fc.a0, fc.k2, fc.a1, fc.k3, x, dp);
+        if (mode == 2) fit_poles(y, fc.a0, fc.k2, fc.a1, fc.k3, x, dp);
         D *= dp;
     }
     return x;
@@ -211,14 +215,17 @@ template <int TR, int FIT> __device__ __forceinline__ double point_weight(double
 
 // operands of dimension slot j: family constants, fit constants, the G shifts of the group
 template <int DP, int G, int FIT>
-__device__ __forceinline__ void load_slot(unsigned sbase, unsigned delta, int j, double& fa, double& fb, FitC& fc, double (&dl)[G]) {
+__device__ __forceinline__ void load_slot(unsigned sbase, unsigned delta, int j, int fit_mode, double& fa, double& fb, FitC& fc,
+                                          double (&dl)[G]) {
     typedef SmemOff<DP, G> O;
     lds_f64x2(sbase + O::fam + 16u * j, fa, fb);
-    if (FIT) {
+    const int mode = (FIT == FIT_RT) ? fit_mode : FIT;
+    fc.mode = mode;
+    if (FIT && mode) {
         lds_f64x2(sbase + O::fit + 80u * j, fc.f0, fc.f1);
         lds_f64x2(sbase + O::fit + 80u * j + 16u, fc.f2, fc.f3);
         fc.f4 = lds_f64(sbase + O::fit + 80u * j + 32u);
-        if (FIT == 2) {
+        if (mode == 2) {
             lds_f64x2(sbase + O::fit + 80u * j + 48u, fc.a0, fc.k2);
             lds_f64x2(sbase + O::fit + 80u * j + 64u, fc.a1, fc.k3);
         }
@@ -238,7 +245,8 @@ struct EvalCtx {            // per-tile constants held in registers
     unsigned delta;         // shared address of the current group's shifts
     double inv_n, wconst, fam0;
     int kor_r;              // generic weight transforms: DevProblem::gen
-    int sel;                // tr_kind * 3 + fit mode (0 none, 1 cubic, 2 cubic + pole terms)
+    int fit_mode;           // 0 none, 1 cubic, 2 cubic + pole terms (decided on the device from a2, a3)
+    int sel;                // specialised tile loop: tr_kind * 2 + fit_mode, or -1 for the generic loop
     int fam_kind, fam_pow;  // kernel family 4: public family id and the corner-peak exponent d + 1
 };
 
@@ -253,7 +261,7 @@ __device__ __forceinline__ void eval_point_group(const typename Res<WIDE>::T (&r
         const double rd = Res<WIDE>::to_double(r[j]);
         double fa, fb, dl[G];
         FitC fc;
-        load_slot<DP, G, FIT>(cx.sbase, cx.delta, j, fa, fb, fc, dl);
+        load_slot<DP, G, FIT>(cx.sbase, cx.delta, j, cx.fit_mode, fa, fb, fc, dl);
 #pragma unroll
         for (int q = 0; q < G; ++q) {
             if (FAMILY == QMC_FAMILY_GENZ_PRODPEAK && TR == TR_BAKER && !FIT) {
@@ -297,7 +305,8 @@ __device__ __forceinline__ void run_tile(SmemCtx<DP, G>& sm, unsigned sbase, con
     const unsigned long long n = pb.n;
     EvalCtx cx;
     cx.sbase = sbase; cx.inv_n = pb.inv_n; cx.wconst = pb.wconst; cx.fam0 = sm.fam0; cx.kor_r = pb.gen;
-    cx.sel = pb.tr_kind * 3 + (pb.has_fit ? 1 + sm.fit_full : 0);
+    cx.fit_mode = pb.has_fit ? 1 + sm.fit_full : 0;
+    cx.sel = (pb.tr_kind != TR_KORR && cx.fit_mode <= 1) ? pb.tr_kind * 2 + cx.fit_mode : -1;
     cx.fam_kind = pb.family; cx.fam_pow = pb.dim + 1;
     typedef SmemCtx<DP, G> Ctx;
     typedef SmemOff<DP, G> Off;
@@ -519,9 +528,10 @@ __device__ __forceinline__ bool next_tile(SmemCtx<DP, G>& sm, const FusedLaunch&
             }
         }
         __syncthreads();
-        // product peak under a generic weight transform: a padded slot must see x - fb = 0, and phi(1/2) is not 1/2 for
-        // asymmetric weights -- take it from the same device function the point block calls (bit-identical)
-        if (!SECTOR && src.family == QMC_FAMILY_GENZ_PRODPEAK && src.tr_kind == TR_KORR && src.dim < DP) {
+        // product peak: a padded slot must see x - fb = 0, and phi(1/2) is not 1/2 for asymmetric weights -- take it from
+        // the device function of the generic loop (for none / baker / Korobov it returns exactly 1/2, 1, 1/2 as the
+        // specialised loops do); the folded baker path keeps its own constant (derive_slot)
+        if (!SECTOR && src.family == QMC_FAMILY_GENZ_PRODPEAK && src.dim < DP && !(src.tr_kind == TR_BAKER && !src.has_fit)) {
             if (tid >= src.dim && tid < DP) {
                 double Pdummy = 1.0;
                 sm.fam[2 * tid + 1] = generic_transform(0.5, (unsigned)__cvta_generic_to_shared(&sm) + SmemOff<DP, G>::kor, src.gen, Pdummy);
@@ -544,20 +554,17 @@ __global__ void __launch_bounds__(kThreads, MinBlocks<DP, WIDE>::value) fused_ke
     bool changed;
     NoExtra ex;
     while (next_tile<DP, G, false>(sm, L, cur, iter, tile_local, changed)) {
-        // tile loop = (transform kind) x (fit mode 0 none / 1 cubic / 2 cubic + poles, decided on the device).  The
-        // specialised loops are inlined; the generic weight transforms and the pole-term fit are real calls, so they
-        // cost the specialised loops no registers.
-        const int sel = sm.prob.tr_kind * 3 + (sm.prob.has_fit ? 1 + sm.fit_full : 0);
+        // six specialised tile loops (none / baker / Korobov-3 x no fit / cubic fit) are inlined; every other combination
+        // (generic weight transforms, pole-term fit) runs the generic loop through a real call, so that it costs the
+        // specialised loops no registers
+        const int fit_mode = sm.prob.has_fit ? 1 + sm.fit_full : 0;
+        const int sel = (sm.prob.tr_kind != TR_KORR && fit_mode <= 1) ? sm.prob.tr_kind * 2 + fit_mode : -1;
         switch (sel) {
 #define QMC_FAST(TRK, FITM) \
-    case TRK * 3 + FITM: run_tile<ClosedEval<FAMILY, DP, G, WIDE, TRK, FITM>, DP, G, WIDE>(sm, sbase, ex, tile_local, changed, L.partials); break;
-#define QMC_SLOW(TRK, FITM) \
-    case TRK * 3 + FITM: run_tile_call<ClosedEval<FAMILY, DP, G, WIDE, TRK, FITM>, DP, G, WIDE>(sm, sbase, ex, tile_local, changed, L.partials); break;
+    case TRK * 2 + FITM: run_tile<ClosedEval<FAMILY, DP, G, WIDE, TRK, FITM>, DP, G, WIDE>(sm, sbase, ex, tile_local, changed, L.partials); break;
             QMC_FAST(TR_NONE, 0) QMC_FAST(TR_NONE, 1) QMC_FAST(TR_BAKER, 0) QMC_FAST(TR_BAKER, 1) QMC_FAST(TR_KOR3, 0) QMC_FAST(TR_KOR3, 1)
-            QMC_SLOW(TR_NONE, 2) QMC_SLOW(TR_BAKER, 2) QMC_SLOW(TR_KOR3, 2) QMC_SLOW(TR_KORR, 0) QMC_SLOW(TR_KORR, 1) QMC_SLOW(TR_KORR, 2)
 #undef QMC_FAST
-#undef QMC_SLOW
-            default: break;
+            default: run_tile_call<ClosedEval<FAMILY, DP, G, WIDE, TR_KORR, FIT_RT>, DP, G, WIDE>(sm, sbase, ex, tile_local, changed, L.partials); break;
         }
     }
 }

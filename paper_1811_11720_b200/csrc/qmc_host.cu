@@ -51,6 +51,9 @@ int dim_slots(int family, int dim, bool wide) {
 }
 bool force_wide();
 bool is_wide(unsigned long long n) { return n >= (1ull << 31) || force_wide(); }
+// residue width of the kernel variant: 64-bit for n >= 2^31, and for the 32-slot closed-form kernels (dim > 16), which
+// exist only with wide residues
+bool variant_wide(int family, int dim, unsigned long long n) { return is_wide(n) || (family != QMC_FAMILY_SECTOR && dim > 16); }
 
 // transform id -> tile-loop kind, symmetric Korobov weight r (0 if none) and the generic-transform code
 // gen = GEN_* | r0 << 4 | r1 << 8 (Table A.2)
@@ -58,8 +61,8 @@ bool decode_transform(int transform, int* kind, int* r, int* gen = nullptr) {
     int g = 0;
     bool ok = false;
     *r = 0;
-    if (transform == QMC_TRANSFORM_NONE) { *kind = TR_NONE; ok = true; }
-    else if (transform == QMC_TRANSFORM_BAKER) { *kind = TR_BAKER; ok = true; }
+    if (transform == QMC_TRANSFORM_NONE) { *kind = TR_NONE; g = GEN_NONE; ok = true; }
+    else if (transform == QMC_TRANSFORM_BAKER) { *kind = TR_BAKER; g = GEN_BAKER; ok = true; }
     else if (transform >= QMC_TRANSFORM_KOROBOV + 1 && transform <= QMC_TRANSFORM_KOROBOV + 6) {
         *r = transform - QMC_TRANSFORM_KOROBOV;
         *kind = (*r == 3) ? TR_KOR3 : TR_KORR;
@@ -78,7 +81,7 @@ bool decode_transform(int transform, int* kind, int* r, int* gen = nullptr) {
             ok = true;
         }
     }
-    if (gen) *gen = (ok && *kind == TR_KORR) ? g : 0;
+    if (gen) *gen = ok ? g : 0;
     return ok;
 }
 
@@ -163,7 +166,7 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
         d.n_params = p.n_params;
         d.out_index = i;
         d.wconst = 1.0;
-        const int npad = dim_slots(p.family, p.dim, is_wide(p.n)) - p.dim;   // padded dimension slots sit at u = 1/2 (qmc_fused.cuh)
+        const int npad = dim_slots(p.family, p.dim, variant_wide(p.family, p.dim, p.n)) - p.dim;   // padded dimension slots sit at u = 1/2 (qmc_fused.cuh)
         if (d.kor_r > 0) {
             // Eq. 15: c_r = (2r+1) C(2r,r); centred antiderivative coefficients of Eq. 14 (see qmc_device.cuh)
             const int r = d.kor_r;
@@ -202,7 +205,7 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
     // kernel variants
     for (int i = 0; i < count; ++i) {
         const DevProblem& d = plan->dev[i];
-        const bool wide = is_wide(d.n);
+        const bool wide = variant_wide(d.family, d.dim, d.n);
         const int dp = dim_slots(d.family, d.dim, wide);
         Variant* v = nullptr;
         for (auto& c : plan->variants)
@@ -273,14 +276,13 @@ int sm_count() {
     return v;
 }
 
-// closed-form families: the kernel variants live in five parts per family (qmc_fused_closed.inc); try each
+// closed-form families: the kernel variants live in four parts per family (qmc_fused_closed.inc); try each
 #define QMC_TRY_PARTS(FAM, PREFIX, FAIL, ...)                                                             \
     {                                                                                                    \
         auto r0 = PREFIX##FAM##_0(__VA_ARGS__); if (r0 != FAIL) return r0;                               \
         auto r1 = PREFIX##FAM##_1(__VA_ARGS__); if (r1 != FAIL) return r1;                               \
         auto r2 = PREFIX##FAM##_2(__VA_ARGS__); if (r2 != FAIL) return r2;                               \
-        auto r3 = PREFIX##FAM##_3(__VA_ARGS__); if (r3 != FAIL) return r3;                               \
-        return PREFIX##FAM##_4(__VA_ARGS__);                                                             \
+        return PREFIX##FAM##_3(__VA_ARGS__);                                                             \
     }
 cudaError_t launch_closed(int family, int dp, bool wide, int grid, cudaStream_t st, const FusedLaunch& a) {
     switch (family) {

@@ -32,9 +32,11 @@ constexpr int kKernelFamilyGenzMisc = 4;
 __host__ __device__ constexpr int kernel_family(int family) { return family <= QMC_FAMILY_SECTOR ? family : kKernelFamilyGenzMisc; }
 
 // transform kinds after host-side decoding
-enum : int { TR_NONE = 0, TR_BAKER = 1, TR_KOR3 = 2, TR_KORR = 3 };   // TR_KORR = the generic weight transforms, see GEN_*
-// generic weight transforms (one tile loop, selected per coordinate by DevProblem::gen = kind | r0 << 4 | r1 << 8):
-enum : int { GEN_KOROBOV_SYM = 0, GEN_KOROBOV_ASYM = 1, GEN_SIDI = 2 };
+enum : int { TR_NONE = 0, TR_BAKER = 1, TR_KOR3 = 2, TR_KORR = 3 };   // TR_KORR = the generic tile loop, see GEN_*
+// The generic tile loop serves every transform (selected per coordinate by DevProblem::gen = kind | r0 << 4 | r1 << 8)
+// and every fit mode at run time; the specialised loops are none / baker / Korobov-3 x (no fit, cubic fit).
+enum : int { GEN_KOROBOV_SYM = 0, GEN_KOROBOV_ASYM = 1, GEN_SIDI = 2, GEN_NONE = 3, GEN_BAKER = 4 };
+constexpr int FIT_RT = 3;              // template value "fit mode decided at run time" (0 none, 1 cubic, 2 cubic + poles)
 
 // Device-resident description of one problem (built on the host, copied into the workspace).
 struct alignas(16) DevProblem {
@@ -62,7 +64,7 @@ struct alignas(16) DevProblem {
     int aux_off;               // sector: offset (in 8-byte words) of the compiled program in the aux area
     int aux_len;
     int out_index;             // index of the problem in the caller's arrays
-    int gen;                   // generic weight transform: GEN_* | r0 << 4 | r1 << 8 (0 otherwise)
+    int gen;                   // the transform for the generic tile loop: GEN_* | r0 << 4 | r1 << 8
 };
 
 // Per-problem tables derived on the device by prepare_kernel (one record per problem).

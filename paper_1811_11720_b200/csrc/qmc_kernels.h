@@ -31,7 +31,7 @@ cudaError_t launch_dfma_probe(cudaStream_t st, double* out, int blocks, int iter
 #define QMC_DECLARE_PART(FAM, PART)                                                                                         \
     cudaError_t launch_fused_part_##FAM##_##PART(int dp, bool wide, int grid, cudaStream_t st, const FusedLaunch& a); \
     int occupancy_fused_part_##FAM##_##PART(int dp, bool wide);
-#define QMC_DECLARE_FAMILY(FAM) QMC_DECLARE_PART(FAM, 0) QMC_DECLARE_PART(FAM, 1) QMC_DECLARE_PART(FAM, 2) QMC_DECLARE_PART(FAM, 3) QMC_DECLARE_PART(FAM, 4)
+#define QMC_DECLARE_FAMILY(FAM) QMC_DECLARE_PART(FAM, 0) QMC_DECLARE_PART(FAM, 1) QMC_DECLARE_PART(FAM, 2) QMC_DECLARE_PART(FAM, 3)
 QMC_DECLARE_FAMILY(0) QMC_DECLARE_FAMILY(1) QMC_DECLARE_FAMILY(2) QMC_DECLARE_FAMILY(4)
 #undef QMC_DECLARE_FAMILY
 #undef QMC_DECLARE_PART

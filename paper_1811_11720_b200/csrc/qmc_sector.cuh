@@ -37,13 +37,15 @@ struct alignas(16) SectorSmem {
     double c0[2];                    // constant terms of U and F
     unsigned long long nu_packed;    // nu_j in 4 bits each
     int a, b;                        // powers of U and F
+    double wpark[8 * kThreads];      // [q][thread]: the G weights of a thread, parked while the interpreter runs (registers)
 };
 struct SectorOff {                   // byte offsets of the fields above (read with ld.shared in the inner loop)
-    static constexpr unsigned coefs = 0, words = kSecMaxCoef * 8, c0 = words + kSecMaxWords * 4, nu = c0 + 16, ab = nu + 8;
+    static constexpr unsigned coefs = 0, words = kSecMaxCoef * 8, c0 = words + kSecMaxWords * 4, nu = c0 + 16, ab = nu + 8, wpark = ab + 8;
 };
 
 static_assert(offsetof(SectorSmem, words) == SectorOff::words && offsetof(SectorSmem, c0) == SectorOff::c0 &&
-              offsetof(SectorSmem, nu_packed) == SectorOff::nu && offsetof(SectorSmem, a) == SectorOff::ab, "SectorOff must mirror SectorSmem");
+              offsetof(SectorSmem, nu_packed) == SectorOff::nu && offsetof(SectorSmem, a) == SectorOff::ab &&
+              offsetof(SectorSmem, wpark) == SectorOff::wpark, "SectorOff must mirror SectorSmem");
 
 // ---- device-side compiler: params -> program (one thread; a few hundred steps at most) ---------
 // program area of a problem (8-byte words at prog_area + aux_off): coefs[nU + nF] (upper bound),
@@ -170,7 +172,7 @@ __device__ __forceinline__ void sector_coords(const typename Res<WIDE>::T (&r)[D
         const double rd = Res<WIDE>::to_double(r[j]);
         double fa, fb, dl[G];
         FitC fc;
-        load_slot<DP, G, FIT>(cx.sbase, cx.delta, j, fa, fb, fc, dl);
+        load_slot<DP, G, FIT>(cx.sbase, cx.delta, j, cx.fit_mode, fa, fb, fc, dl);
 #pragma unroll
         for (int q = 0; q < G; ++q)
             x[q][j] = point_coord<TR, FIT>(rd, cx.inv_n, dl[q], fc, cx.sbase + SmemOff<DP, G>::kor, cx.kor_r, P[q], D[q]);
@@ -181,34 +183,34 @@ __device__ __forceinline__ void sector_coords(const typename Res<WIDE>::T (&r)[D
 
 // Transform and fit map are selected per point by a warp-uniform switch, so that the interpreter exists once per
 // tile loop.  SLOW = false: the specialised transforms without fit map (inlined tile loop of the kernel); SLOW = true:
-// every other combination (generic weight transforms, fit maps), reached through a real call (run_tile_call).
+// the generic coordinate block (any transform, any fit mode at run time), reached through a real call (run_tile_call).
 template <int DP, int G, bool WIDE, bool SLOW> struct SectorEval {
     static constexpr int NC = 1;
     typedef unsigned Extra;                                  // shared address of the CTA's SectorSmem
     static __device__ __forceinline__ void eval(const typename Res<WIDE>::T (&r)[DP], const SmemCtx<DP, G>&, const unsigned& exbase,
                                                 const EvalCtx& cx, double (&acc)[G][1]) {
         double x[G][DP], num[G];
-#define QMC_CASE(TRK, FITM) \
-    case TRK * 3 + FITM: sector_coords<DP, G, WIDE, TRK, FITM>(r, cx, x, num); break;
         if (!SLOW) {
             switch (cx.sel) {
-                QMC_CASE(TR_NONE, 0) QMC_CASE(TR_BAKER, 0)
+                case TR_NONE * 2: sector_coords<DP, G, WIDE, TR_NONE, 0>(r, cx, x, num); break;
+                case TR_BAKER * 2: sector_coords<DP, G, WIDE, TR_BAKER, 0>(r, cx, x, num); break;
                 default: sector_coords<DP, G, WIDE, TR_KOR3, 0>(r, cx, x, num); break;
             }
         } else {
-            switch (cx.sel) {
-                QMC_CASE(TR_NONE, 1) QMC_CASE(TR_NONE, 2) QMC_CASE(TR_BAKER, 1) QMC_CASE(TR_BAKER, 2) QMC_CASE(TR_KOR3, 1)
-                QMC_CASE(TR_KOR3, 2) QMC_CASE(TR_KORR, 0) QMC_CASE(TR_KORR, 1)
-                default: sector_coords<DP, G, WIDE, TR_KORR, 2>(r, cx, x, num); break;
-            }
+            sector_coords<DP, G, WIDE, TR_KORR, FIT_RT>(r, cx, x, num);
         }
-#undef QMC_CASE
+        // the weights are not needed until the interpreter is done: park them in shared memory ([q][thread], conflict free)
+        const unsigned park = exbase + SectorOff::wpark + 8u * threadIdx.x;
+#pragma unroll
+        for (int q = 0; q < G; ++q) sts_f64(park + 8u * kThreads * q, num[q]);
         double c0u, c0f;
         lds_f64x2(exbase + SectorOff::c0, c0u, c0f);
         double U[G], F[G];
 #pragma unroll
         for (int q = 0; q < G; ++q) { U[q] = 0.0; F[q] = c0u; }
         sector_interp<DP, G>(x, exbase + SectorOff::words, exbase + SectorOff::coefs, c0f, U, F);
+#pragma unroll
+        for (int q = 0; q < G; ++q) num[q] = lds_f64(park + 8u * kThreads * q);
         // num = W prod_j x_j^nu_j U^a, den = F^b   (small integer powers by repeated multiplication)
         const unsigned long long nup = lds_u64(exbase + SectorOff::nu);
         const unsigned long long ab = lds_u64(exbase + SectorOff::ab);
