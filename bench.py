@@ -51,6 +51,9 @@ ALG_FP64_PER_EVAL = {
     3: 6 * (2 + 7) + 3 + 44.44 + 3.04 + 1.51 + 1.50 + 1 + 5 + 1,      # 114.5 d=6 sector, Korobov-3
     4: 16 * (2 + 7 + 6 + 1) + 4 + 14 + 1,                             # 275  d=16 osc, Korobov-3 + cubic map
 }
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused kernel at full size, from the committed
+# `ncu --set full` capture profiles/r07_fused_full.md (configs[3], [4] were captured at 1/8 size: no full-size figure)
+PROFILED_DRAM_BYTES_PER_LAUNCH = {1: 70656, 2: 141312}
 FP64_LANES_PER_SM = 64                        # B200 (sm_100): 64 FP64 FMA lanes per SM -> nominal peak
 
 
@@ -374,7 +377,9 @@ def run_ours(args):
                "fused_kernel_share_of_step": fused_avg_s * 1e3 * steps / sum(step_ms),
                "gpu_launches_per_step": launches, "plan": batch.plan_info(),
                "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": peak_rate / 1e12, "unit": "Tinst/s (thread-level FP64 instructions)",
-                            "frac": achieved / peak_rate, "traffic": None, "alg_fp64_inst_per_eval": alg,
+                            "frac": achieved / peak_rate, "traffic": PROFILED_DRAM_BYTES_PER_LAUNCH.get(c) if SHRINK == 1 else None,
+                            "traffic_unit": "bytes per launch (ncu, profiles/r07_fused_full.md); the path is ALU bound, inputs are KBs",
+                            "alg_fp64_inst_per_eval": alg,
                             "peak_source": "qmc_fp64_peak_probe (DFMA chains) measured in this run",
                             "peak_nominal": sm_count * FP64_LANES_PER_SM * 1.965e9 / 1e12},
                "result_mean": [float(v) for v in means[0]], "result_err": [float(v) for v in errs[0]]}
