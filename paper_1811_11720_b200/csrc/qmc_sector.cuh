@@ -182,7 +182,8 @@ __device__ __forceinline__ void sector_coords(const typename Res<WIDE>::T (&r)[D
 }
 
 // Transform and fit map are selected per point by a warp-uniform switch, so that the interpreter exists once per
-// tile loop.  SLOW = false: the specialised transforms without fit map (inlined tile loop of the kernel); SLOW = true:
+// tile loop.  SLOW = false: Korobov-3 without fit map, the paper's default for loop integrals, as the only
+// inlined tile loop of the kernel (a smaller kernel body measurably helps the interpreter: DESIGN.md section 5); SLOW = true:
 // the generic coordinate block (any transform, any fit mode at run time), reached through a real call (run_tile_call).
 template <int DP, int G, bool WIDE, bool SLOW> struct SectorEval {
     static constexpr int NC = 1;
@@ -191,11 +192,7 @@ template <int DP, int G, bool WIDE, bool SLOW> struct SectorEval {
                                                 const EvalCtx& cx, double (&acc)[G][1]) {
         double x[G][DP], num[G];
         if (!SLOW) {
-            switch (cx.sel) {
-                case TR_NONE * 2: sector_coords<DP, G, WIDE, TR_NONE, 0>(r, cx, x, num); break;
-                case TR_BAKER * 2: sector_coords<DP, G, WIDE, TR_BAKER, 0>(r, cx, x, num); break;
-                default: sector_coords<DP, G, WIDE, TR_KOR3, 0>(r, cx, x, num); break;
-            }
+            sector_coords<DP, G, WIDE, TR_KOR3, 0>(r, cx, x, num);
         } else {
             sector_coords<DP, G, WIDE, TR_KORR, FIT_RT>(r, cx, x, num);
         }
@@ -274,7 +271,7 @@ __global__ void __launch_bounds__(kThreads, SectorMinBlocks<DP, G>::value) fused
             }
             __syncthreads();
         }
-        const bool fast = !sm.prob.has_fit && sm.prob.tr_kind != TR_KORR;
+        const bool fast = !sm.prob.has_fit && sm.prob.tr_kind == TR_KOR3;
         if (fast) run_tile<SectorEval<DP, G, WIDE, false>, DP, G, WIDE>(sm, sbase, exbase, tile_local, changed, partials);
         else run_tile_call<SectorEval<DP, G, WIDE, true>, DP, G, WIDE>(sm, sbase, exbase, tile_local, changed, partials);
     }
