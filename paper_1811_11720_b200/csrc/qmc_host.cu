@@ -589,11 +589,15 @@ int qmc_lattice_integrate_ex(int family, const double* params, int n_params, int
     int status = QMC_OK;
     cudaError_t e;
     std::vector<double> host_out((size_t)4 + 2 * m);
+    // the inputs travel in ONE host-to-device copy: [params | z | shifts | fit] packed with the device layout
+    const size_t b_in = b_params + b_z + b_sh + (fit_coeffs ? (size_t)dim * 6 * 8 : 0);
+    std::vector<char> host_in(b_in);
+    std::memcpy(host_in.data(), params, (size_t)n_params * 8);
+    std::memcpy(host_in.data() + b_params, z, (size_t)dim * 8);
+    std::memcpy(host_in.data() + b_params + b_z, shifts, (size_t)m * dim * 8);
+    if (fit_coeffs) std::memcpy(host_in.data() + b_params + b_z + b_sh, fit_coeffs, (size_t)dim * 6 * 8);
     do {
-        if ((e = cudaMemcpyAsync(d_params, params, (size_t)n_params * 8, cudaMemcpyHostToDevice, st)) != cudaSuccess) break;
-        if ((e = cudaMemcpyAsync(d_z, z, (size_t)dim * 8, cudaMemcpyHostToDevice, st)) != cudaSuccess) break;
-        if ((e = cudaMemcpyAsync(d_sh, shifts, (size_t)m * dim * 8, cudaMemcpyHostToDevice, st)) != cudaSuccess) break;
-        if (fit_coeffs && (e = cudaMemcpyAsync(d_fit, fit_coeffs, (size_t)dim * 6 * 8, cudaMemcpyHostToDevice, st)) != cudaSuccess) break;
+        if ((e = cudaMemcpyAsync(buf, host_in.data(), b_in, cudaMemcpyHostToDevice, st)) != cudaSuccess) break;
         dp.params = reinterpret_cast<const double*>(d_params);
         dp.z = reinterpret_cast<const uint64_t*>(d_z);
         dp.shifts = reinterpret_cast<const double*>(d_sh);

@@ -213,6 +213,28 @@ def test_wide_residue_path(monkeypatch):
     assert_means(sms[0], sm_or, p["name"])
 
 
+def test_paper_largest_lattice_full_size():
+    """n = 15173222401 > 2^33, the largest lattice the paper ships: 64-bit residues and the 128-bit first
+    product of every thread, at full size.  The oracle cannot afford 3e10 evaluations, but in one dimension the residues
+    k z mod n are a permutation of 0..n-1 for any z coprime to n, so with the trivial transform the rule is the equispaced
+    sum  (1/n) sum_j cos(phi + a (j + theta)/n),  theta = frac(n Delta),  a geometric series with the closed form
+    sin(a/2) / (n sin(a/(2n))) * cos(phi + a (theta - 1/2)/n + a/2): an exact value (to rounding) that any wrong or
+    repeated residue would miss."""
+    from fractions import Fraction
+    n, m = 15173222401, 2
+    prm = np.array([0.3125, 1.75])                            # u0, a
+    sh = np.array([[0.6180339887498949], [0.1415926535897932]])
+    z = np.array([5546223817], dtype=np.uint64)               # any z coprime to n
+    assert np.gcd(int(z[0]), n) == 1
+    p = synth.problem(0, prm, n, z, sh, NONE, name="paper.nmax.d1")
+    sms, means, errs = run_gpu([p])
+    phi, a = 2 * np.pi * prm[0], prm[1]
+    for s_, delta in enumerate(sh[:, 0]):
+        theta = float((Fraction(delta) * n) % 1)              # exact: Delta is a dyadic rational
+        want = np.sin(a / 2) / (n * np.sin(a / (2 * n))) * np.cos(phi + a * (theta - 0.5) / n + a / 2)
+        assert abs(sms[0][s_, 0] - want) <= 1e-13 * abs(want), (sms[0][s_, 0], want)
+
+
 def test_mixed_batch_one_call():
     """problems of different family, dimension, n, m, transform in one stream-ordered call (S9)"""
     probs = [make(0, 4, 65537, 10, K + 3, 1), make(1, 8, 8191, 5, BAKER, 2), make(2, 12, 4099, 7, K + 3, 3),

@@ -208,6 +208,22 @@ def test_rule_exact_on_fourier_modes():
             assert abs(sm[s, 0] - math.cos(ph)) < tol and abs(sm[s, 1] - math.sin(ph)) < tol
 
 
+@pytest.mark.parametrize("n,z", [(65537, 25016), (1048573, 32373), (55, 34)])
+def test_one_dimensional_rule_is_a_geometric_series(n, z):
+    """d = 1, transform None: k z mod n runs through 0..n-1 (z coprime to n), so Eq. 2 is the equispaced sum
+    (1/n) sum_j cos(phi + a (j + theta)/n), theta = frac(n Delta) = sin(a/2) / (n sin(a/(2n))) cos(phi + a (theta - 1/2)/n + a/2):
+    an exact value of the whole rule (residues, coordinates, integrand, compensated sum) to rounding"""
+    prm = np.array([0.3125, 1.75])
+    sh = np.array([[0.6180339887498949], [0.1415926535897932], [0.0]])
+    p = synth.problem(0, prm, n, np.array([z], dtype=np.uint64), sh, synth.TRANSFORM_NONE)
+    sm, mean, err = oracle.integrate(p)
+    phi, a = 2 * np.pi * prm[0], prm[1]
+    for s_, delta in enumerate(sh[:, 0]):
+        theta = float((Fraction(delta) * n) % 1)
+        want = np.sin(a / 2) / (n * np.sin(a / (2 * n))) * np.cos(phi + a * (theta - 0.5) / n + a / 2)
+        assert abs(sm[s_, 0] - want) <= 2e-15 * abs(want)
+
+
 def test_sum_against_fsum_python():
     # the whole chain in slow exact-ish python: Fractions for the point, math.fsum for the sum
     n, z = 251, [1, 97, 33]
