@@ -22,13 +22,15 @@
 // adds its terms in increasing k.  OpenMP runs fixed chunks of 2^16 consecutive k; chunk sums are
 // combined in chunk order, so results do not depend on the thread count.
 //
-// Pins (tests/test_oracle_*.py, all `-m "not gpu"`): Fig. 1 lattice n=55 z=(1,34) P:L108; by-hand
-// lattices n=7 z=(1,3), n=11 z=(1,7) P:L1050; residue permutation property; exact-rational
-// coordinates; Fourier-mode exactness / dual-lattice modes; Eq. 15 normalisation, phi(1)=1,
-// Gauss-Legendre quadrature of omega; closed forms of families 0-2 (Genz 1, 2 P:L709-L713);
-// tensor Gauss-Legendre for the sector family at d<=3; x0*x1*x2 -> 1/8 (Fig. 2);
-// Eq. 3 on hand-made means; projection marginals in closed form; fit recovers an exact cubic.
-// Parity unpinned: nothing (the CBC tool is not part of the oracle).
+// Pins (tests/test_oracle_pins.py, all `-m "not gpu"`; table in DESIGN.md section 6): Fig. 1 lattice n=55 z=(1,34) P:L108;
+// by-hand lattices n=7 z=(1,3), n=11 z=(1,7) P:L1050; residue permutation property; exact-rational coordinates;
+// Fourier-mode exactness / dual-lattice modes; the one-dimensional rule as an exact geometric series; Eq. 15 normalisation
+// and phi = regularised incomplete beta (symmetric and asymmetric weights); Eq. 16 constants and Gauss-Legendre
+// quadrature of the Sidi weight; closed forms of families 0-2 and 4-7 (Genz 1-6); tensor Gauss-Legendre for
+// the sector family at d<=3; x0*x1*x2 -> 1/8 (Fig. 2); Eq. 3 on hand-made means; projection marginals in
+// closed form; fit recovers an exact cubic.
+// Parity unpinned: nothing in this file (the CBC tool and the Levenberg-Marquardt fit of the product are not part of the
+// oracle).
 //
 // Build: g++ -O2 -std=c++17 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/build.py).
 #include <cmath>
