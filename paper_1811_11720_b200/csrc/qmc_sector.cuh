@@ -26,9 +26,7 @@ constexpr int kSecMaxCoef = 192;     // coefficient stream of a program: non-con
 constexpr int kSecMaxWords = kMaxSectorOps / 4;
 
 // step codes (one byte each): 0 = no-op, 1 = end of U, 2 = end of program, 3 = dense linear form (sum += sum_j c_j x_j over
-// all DP slots, DP coefficients from the stream: the degree-1 monomials of a polynomial in ONE step), 4 + 4*j + 2*FIRST + LAST (single
-// variable); with DP <= 8 dimension slots also 4 + 4*DP + 2*pair(a,b) + FULL, a <= b: the first two variables of a
-// monomial in one step (mon = coef x_a; FULL ? sum = fma(mon, x_b, sum) : mon *= x_b), pair(a,b) = a DP - a(a-1)/2 + b - a
+// all DP slots, DP coefficients from the stream: the degree-1 monomials of a polynomial in ONE step), 4 + 4*j + 2*FIRST + LAST
 enum : int { SEC_NOP = 0, SEC_ENDU = 1, SEC_END = 2, SEC_LIN = 3, SEC_BASE = 4 };
 
 struct alignas(16) SectorSmem {
@@ -51,14 +49,12 @@ static_assert(offsetof(SectorSmem, words) == SectorOff::words && offsetof(Sector
 // program area of a problem (8-byte words at prog_area + aux_off): coefs[nU + nF] (upper bound),
 // then the step bytes.  DevAux: sec_nops[0] = number of 32-bit step words, sec_ncoef[0] = number
 // of coefficients.
-__host__ __device__ inline bool sector_has_pairs(int dp) { return dp <= 0; }   // all step codes must fit one byte
 __host__ __device__ inline int sector_dim_slots(int dim) { return dim <= 4 ? 4 : (dim <= 6 ? 6 : (dim <= 8 ? 8 : (dim <= 16 ? 16 : -1))); }
 
 __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned long long* prog_area) {
     if (threadIdx.x != 0) return;
     const int d = pb.dim;
     const int dp = sector_dim_slots(d);
-    const bool pairs = sector_has_pairs(dp);
     const double* p = pb.params;
     int status = 0;
     // A rejected parameter block must still leave a program the interpreter can run to its end (the problem's
@@ -126,17 +122,12 @@ __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned 
             if (deg == 1 && lin) continue;
             if (ncoef >= kSecMaxCoef - 1 || nops + deg > max_ops) { status = QMC_ERR_PARAMS; continue; }
             coefs[ncoef++] = c[t];
-            int seen = 0, va = -1;
+            int seen = 0;
             for (int j = 0; j < d; ++j) {
                 const int ej = (int)e[t * d + j];
                 for (int r = 0; r < ej; ++r) {
                     const int first = (seen == 0), last = (seen == deg - 1);
-                    if (pairs && deg >= 2 && seen < 2) {        // the first two variables a <= b go into one pair step
-                        if (seen == 0) va = j;
-                        else ops[nops++] = (unsigned char)(SEC_BASE + 4 * dp + 2 * (va * dp - va * (va - 1) / 2 + (j - va)) + last);
-                    } else {
-                        ops[nops++] = (unsigned char)(SEC_BASE + j * 4 + first * 2 + last);
-                    }
+                    ops[nops++] = (unsigned char)(SEC_BASE + j * 4 + first * 2 + last);
                     ++seen;
                 }
             }
