@@ -18,7 +18,7 @@ constexpr int kWavesSingle = 2;        // tiles per resident CTA when a kernel v
 constexpr int kWavesBatch = 8;         // ... and when it serves a batch of unequal problems (dynamic balance)
 
 // resident CTAs per SM each fused kernel is register-budgeted for (its __launch_bounds__ minimum)
-constexpr int min_blocks_closed(int dp, bool wide) { return dp <= 8 ? 4 : (dp <= 16 ? (wide ? 2 : 3) : 2); }
+constexpr int min_blocks_closed(int dp, bool wide) { return (dp <= 8 || (dp <= 12 && !wide)) ? 4 : (dp <= 16 ? (wide ? 2 : 3) : 2); }
 constexpr int sector_group(int dp) { return dp <= 8 ? 8 : 4; }                       // shifts per group, sector family
 constexpr int min_blocks_sector(int dp) { return dp <= 6 ? 3 : 2; }
 constexpr int kDeltaCache = 768;       // doubles of shared memory per CTA that cache the shifts of all groups of a problem
