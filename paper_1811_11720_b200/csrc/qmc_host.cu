@@ -219,7 +219,15 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
     for (auto& v : plan->variants) {
         const int resident = kPlanSMs * (v.family == QMC_FAMILY_SECTOR ? min_blocks_sector(v.dp) : min_blocks_closed(v.dp, v.wide));
         const int env = tiles_target();
-        const double target = env > 0 ? env : resident * (v.plist.size() == 1 ? kWavesSingle : kWavesBatch);
+        // one problem: equal tiles, 2 per resident CTA (the queue evens out SM speed differences over a long kernel) -- or
+        // exactly 1 when the whole kernel is short (< kShortEvalsPerCta evaluations per CTA: per-tile overhead and the
+        // queue reset matter more than balance); a batch of unequal problems: 8 per resident CTA
+        int waves = kWavesBatch;
+        if (v.plist.size() == 1) {
+            const DevProblem& d0 = plan->dev[v.plist[0]];
+            waves = ((double)d0.n * d0.m < (double)kShortEvalsPerCta * resident) ? 1 : kWavesSingle;
+        }
+        const double target = env > 0 ? env : resident * waves;
         double total_cost = 0.0;
         for (int i : v.plist) total_cost += (double)plan->dev[i].n * plan->dev[i].m * (12.0 * plan->dev[i].dim + 0.5 * plan->dev[i].n_params + 40.0);
         for (int i : v.plist) {

@@ -15,6 +15,7 @@ constexpr int kMaxSteps = 1024;        // max lattice indices per thread per til
 constexpr int kPlanSMs = 148;          // the tiling is planned for a B200 (a pure function of the problem structs: results
                                        // are bit-identical on any device, only the balance is tuned for 148 SMs)
 constexpr int kWavesSingle = 2;        // tiles per resident CTA when a kernel variant serves one problem (equal-cost tiles)
+constexpr int kShortEvalsPerCta = 200000;   // below this many evaluations per resident CTA a single problem gets 1 tile per CTA
 constexpr int kWavesBatch = 8;         // ... and when it serves a batch of unequal problems (dynamic balance)
 
 // resident CTAs per SM each fused kernel is register-budgeted for (its __launch_bounds__ minimum)
