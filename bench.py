@@ -52,8 +52,8 @@ ALG_FP64_PER_EVAL = {
     4: 16 * (2 + 7 + 6 + 1) + 4 + 14 + 1,                             # 275  d=16 osc, Korobov-3 + cubic map
 }
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused kernel at full size, from the committed
-# `ncu --set full` capture profiles/r07_fused_full.md (configs[3], [4] were captured at 1/8 size: no full-size figure)
-PROFILED_DRAM_BYTES_PER_LAUNCH = {1: 70656, 2: 141312}
+# `ncu --set full` capture profiles/r08_fused_full.md (configs[3], [4] were captured at 1/8 size: no full-size figure)
+PROFILED_DRAM_BYTES_PER_LAUNCH = {1: 70400, 2: 122368}
 FP64_LANES_PER_SM = 64                        # B200 (sm_100): 64 FP64 FMA lanes per SM -> nominal peak
 
 
@@ -398,7 +398,7 @@ def run_ours(args):
                "gpu_launches_per_step": launches, "plan": batch.plan_info(),
                "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": peak_rate / 1e12, "unit": "Tinst/s (thread-level FP64 instructions)",
                             "frac": achieved / peak_rate, "traffic": PROFILED_DRAM_BYTES_PER_LAUNCH.get(c) if SHRINK == 1 else None,
-                            "traffic_unit": "bytes per launch (ncu, profiles/r07_fused_full.md); the path is ALU bound, inputs are KBs",
+                            "traffic_unit": "bytes per launch (ncu, profiles/r08_fused_full.md); the path is ALU bound, inputs are KBs",
                             "alg_fp64_inst_per_eval": alg,
                             "peak_source": "qmc_fp64_peak_probe (DFMA chains) measured in this run",
                             "peak_nominal": sm_count * FP64_LANES_PER_SM * 1.965e9 / 1e12},
@@ -416,6 +416,29 @@ def run_ours(args):
             rec, _, w = measure(c, k, wu)
             windows.append(w)
             others.append(rec)
+
+    # the same step replayed from a CUDA graph (single-problem calls are capturable): launch overhead of small problems
+    graphs = []
+    if rank == 0 and world == 1 and not args.main_only:
+        for c in (0, 1):
+            if args.others is not None and c not in args.others and c != args.main:
+                continue
+            batch = binding.DeviceBatch(rank_problems(c, 0), device=device)
+            g = batch.capture()
+            for _ in range(5):
+                g.replay()
+            torch.cuda.synchronize()
+            reps = 200
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(reps):
+                g.replay()
+            e1.record()
+            e1.synchronize()
+            ms = e0.elapsed_time(e1) / reps
+            graphs.append({"workload": workload_name(c), "ms_per_step_graph_replay": ms, "value": evals_of(batch.problems) / (ms * 1e-3),
+                           "note": "back-to-back replays, no L2 flush in between (inputs are KBs)"})
+        binding.qmc_profile_enable(True)
 
     ttt = []
     if rank == 0 and world == 1 and not args.main_only:
@@ -450,7 +473,7 @@ def run_ours(args):
            "fused_kernel_share_of_step": main["fused_kernel_share_of_step"],
            "fp64_peak_probe": {"thread_inst_per_s": peak_rate, "ms": peak_ms, "sm_count": sm_count,
                                "implied_clock_mhz_at_64_lanes": peak_rate / (sm_count * FP64_LANES_PER_SM) / 1e6},
-           "clocks": clocks, "others": others, "time_to_rel_err_1e-8": ttt}
+           "clocks": clocks, "others": others, "time_to_rel_err_1e-8": ttt, "cuda_graph": graphs}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(args.main, reps=3)
     if rank == 0:

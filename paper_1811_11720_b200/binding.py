@@ -225,6 +225,19 @@ class DeviceBatch:
                "qmc_lattice_integrate_batch")
         return int(lib().qmc_last_launch_count())
 
+    def capture(self):
+        """Captures one integrate() call in a CUDA graph and returns the torch.cuda.CUDAGraph (call .replay()).  A call for
+        ONE closed-form problem is two kernel launches plus at most one 8-byte memset, all stream-ordered and capturable; a
+        batch call uploads its plan from pageable host memory and cannot be captured (the library then returns QMC_ERR_CUDA)."""
+        torch = self.torch
+        qmc_profile_enable(False)                          # event records do not belong in a graph
+        self.integrate()                                    # warm-up outside the capture (module load, occupancy cache)
+        torch.cuda.synchronize(self.device)
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            self.integrate()
+        return graph
+
     def results(self):
         """Synchronises and returns numpy (shift_means list of (m, ncomp), means (count, ncomp_max), errs)."""
         self.torch.cuda.synchronize(self.device)

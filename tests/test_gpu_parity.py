@@ -253,6 +253,20 @@ def test_determinism_bitwise():
     assert a[1].tobytes() == b[1].tobytes() and a[2].tobytes() == b[2].tobytes()
 
 
+def test_cuda_graph_replay_is_bitwise_the_direct_call():
+    """a single-problem call is stream-ordered and capturable: graph replays reproduce the direct call bit for bit"""
+    p = make(2, 12, 65537, 8, K + 3, 4711)
+    direct = run_gpu([p])
+    batch = binding.DeviceBatch([p])
+    graph = batch.capture()
+    batch.means.zero_(); batch.errs.zero_(); batch.shift_means.zero_()
+    for _ in range(3):
+        graph.replay()
+    sms, means, errs = batch.results()
+    assert sms[0].tobytes() == direct[0][0].tobytes()
+    assert means.tobytes() == direct[1].tobytes() and errs.tobytes() == direct[2].tobytes()
+
+
 def test_minimal_example_one_eighth():
     """Fig. 2: f = x0 x1 x2, Korobov weight 3 -> 1/8, through the synchronous HOST entry."""
     d = 3
