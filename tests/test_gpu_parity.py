@@ -197,6 +197,13 @@ def test_means_shift_counts(m):
     check_against_oracle([make(1, 4, 8191, m, BAKER, 1200 + m), make(2, 5, 8191, m, K + 3, 1300 + m)])
 
 
+@pytest.mark.parametrize("fam,d,m", [(0, 20, 40), (1, 4, 301), (2, 12, 70), (3, 6, 130), (3, 16, 50)])
+def test_means_many_shifts_uncached(fam, d, m):
+    """more shifts than the shared-memory shift cache holds (768 doubles per CTA): the per-group staging path"""
+    n = 2053 if m > 100 else 8191
+    check_against_oracle([make(fam, d, n, m, K + 3 if fam != 1 else BAKER, 5100 + d + m, a_hi=0.4)])
+
+
 def test_wide_residue_path(monkeypatch):
     """n >= 2^31 uses 64-bit residue registers; n >= 2^32 needs the 128-bit product (the
     paper ships n = 15173222401).  The oracle can only afford one cheap full run above 2^31, so the 64-bit
