@@ -204,6 +204,27 @@ def test_means_many_shifts_uncached(fam, d, m):
     check_against_oracle([make(fam, d, n, m, K + 3 if fam != 1 else BAKER, 5100 + d + m, a_hi=0.4)])
 
 
+def test_maximum_shift_count():
+    """m = QMC_MAX_M = 4096 shifts (include/qmc_lattice.h): 1024 groups, 8192 rows in the finalize stage for the complex family"""
+    check_against_oracle([make(2, 2, 127, 4096, K + 3, 61), make(0, 3, 257, 4096, BAKER, 62)])
+
+
+def test_large_mixed_batch_of_all_families():
+    """300 small problems of all eight families, mixed transforms / fit modes / sizes in ONE call: every kernel variant's
+    queue, the cost-sorted tile lists and the binary search of the tile prefix"""
+    rng = synth.MT19937_64(9001)
+    trs = [NONE, BAKER, K + 3, K + 1, SIDI + 3, KA + 16 * 2 + 3]
+    probs = []
+    for i in range(300):
+        fam = i % 8
+        d = 1 + rng.next_u64() % (6 if fam == 3 else 9)
+        n = [127, 509, 1021, 2053, 4099][rng.next_u64() % 5]
+        m = 2 + rng.next_u64() % 9
+        fit = [False, True, "full"][rng.next_u64() % 3] if i % 5 == 0 else False
+        probs.append(make(fam, int(d), n, int(m), trs[rng.next_u64() % len(trs)], 9100 + i, fit=fit, a_hi=0.5))
+    check_against_oracle(probs)
+
+
 def test_wide_residue_path(monkeypatch):
     """n >= 2^31 uses 64-bit residue registers; n >= 2^32 needs the 128-bit product (the
     paper ships n = 15173222401).  The oracle can only afford one cheap full run above 2^31, so the 64-bit
