@@ -177,11 +177,13 @@ double sparse_poly(const double* c, const double* e, int count, int dim, const d
 //  1 Genz product peak f = prod 1/(c_j^-2 + (x_j - w_j)^2)
 //  2 complex           f = exp(i sum a_j x_j) prod (1 + b_j x_j)            BASELINE.json configs[2]
 //  3 sector-like       f = prod x_j^nu_j * U(x)^a / F(x)^b                  BASELINE.json configs[3]
+//    with the optional trailing block [lu, lf, p]: f * (lu log U + lf log F)^p, the shape of the order-eps^p term of
+//    U^(a + lu eps) / F^(b - lf eps) that sector decomposition integrates (reading C-15)
 //  4 Genz corner peak  f = (1 + sum c_j x_j)^-(d+1)             [c]
 //  5 Genz Gaussian     f = exp(-sum c_j^2 (x_j - w_j)^2)        [c, w]
 //  6 Genz C^0          f = exp(-sum c_j |x_j - w_j|)            [c, w]
 //  7 Genz discontinuous f = 0 if x_1 > w_1 or x_2 > w_2, else exp(sum c_j x_j)   [c, w_1, w_2]
-inline void integrand(int fam, const double* p, int dim, const double* x, double* re, double* im) {
+inline void integrand(int fam, const double* p, int n_params, int dim, const double* x, double* re, double* im) {
     *im = 0.0;
     if (fam == FAM_OSC) {
         double ph = 2.0 * M_PI * p[0];
@@ -221,15 +223,26 @@ inline void integrand(int fam, const double* p, int dim, const double* x, double
         for (int j = 0; j < dim; ++j) pre *= ipow(x[j], (int)nu[j]);
         double U = sparse_poly(cU, eU, nU, dim, x), F = sparse_poly(cF, eF, nF, dim, x);
         *re = pre * ipow(U, a) / ipow(F, b);
+        if (n_params == 4 + dim + (nU + nF) * (1 + dim) + 3) {           // trailing [lu, lf, p]
+            const double* t = p + n_params - 3;
+            *re *= ipow(t[0] * std::log(U) + t[1] * std::log(F), (int)t[2]);
+        }
     }
 }
 
 inline int ncomp_of(int fam) { return fam == FAM_CEXP ? 2 : 1; }
 
-int expected_params(int fam, const double* p, int dim) {
+int expected_params(int fam, const double* p, int n_params, int dim) {
     if (fam == FAM_OSC) return 1 + dim;
     if (fam == FAM_PRODPEAK || fam == FAM_CEXP) return 2 * dim;
-    if (fam == FAM_SECTOR) { int nU = (int)p[2], nF = (int)p[3]; return 4 + dim + (nU + nF) * (1 + dim); }
+    if (fam == FAM_SECTOR) {
+        int nU = (int)p[2], nF = (int)p[3], base = 4 + dim + (nU + nF) * (1 + dim);
+        if (n_params == base + 3) {                                        // trailing [lu, lf, p], p a small positive integer
+            const double pw = p[base + 2];
+            return (pw >= 1.0 && pw <= 4.0 && pw == std::floor(pw)) ? n_params : -1;
+        }
+        return base;
+    }
     if (fam == FAM_CORNER) return dim;
     if (fam == FAM_GAUSS || fam == FAM_C0) return 2 * dim;
     if (fam == FAM_DISC) return dim + (dim < 2 ? dim : 2);
@@ -237,7 +250,7 @@ int expected_params(int fam, const double* p, int dim) {
 }
 
 // One lattice point for one shift: O2-O5.  Returns v = W * f (re, im).
-inline void eval_point(int fam, const double* params, int dim, const uint64_t* r, double inv_n, const double* shift,
+inline void eval_point(int fam, const double* params, int n_params, int dim, const uint64_t* r, double inv_n, const double* shift,
                        const Transform& tr, const double* fit, double* re, double* im) {
     double x[MAX_DIM]; double W = 1.0;
     for (int j = 0; j < dim; ++j) {
@@ -246,7 +259,7 @@ inline void eval_point(int fam, const double* params, int dim, const uint64_t* r
         if (fit) { double xx, dp; fit_map(fit + 6 * j, y, &xx, &dp); y = xx; w *= dp; }
         x[j] = y; W *= w;
     }
-    double fr, fi; integrand(fam, params, dim, x, &fr, &fi);
+    double fr, fi; integrand(fam, params, n_params, dim, x, &fr, &fi);
     *re = W * fr; *im = W * fi;
 }
 
@@ -287,8 +300,8 @@ int oracle_fit_map(const double* a, double y, double* x, double* dp) { fit_map(a
 
 int oracle_integrand(int fam, const double* params, int n_params, int dim, const double* x, double* out2) {
     if (fam < 0 || fam > FAM_LAST || dim < 1 || dim > MAX_DIM) return -8;
-    if (expected_params(fam, params, dim) != n_params) return -9;
-    integrand(fam, params, dim, x, &out2[0], &out2[1]);
+    if (expected_params(fam, params, n_params, dim) != n_params) return -9;
+    integrand(fam, params, n_params, dim, x, &out2[0], &out2[1]);
     return 0;
 }
 
@@ -299,7 +312,7 @@ int oracle_shift_sums(int fam, const double* params, int n_params, int dim, uint
                       double* out_sums) {
     if (fam < 0 || fam > FAM_LAST) return -8;
     if (dim < 1 || dim > MAX_DIM) return -2;
-    if (expected_params(fam, params, dim) != n_params) return -9;
+    if (expected_params(fam, params, n_params, dim) != n_params) return -9;
     Transform trf;
     if (!decode_transform(tr, &trf)) return -7;
     if (k_end > n || k_begin > k_end) return -3;
@@ -319,7 +332,7 @@ int oracle_shift_sums(int fam, const double* params, int n_params, int dim, uint
             for (int j = 0; j < dim; ++j) r[j] = residue(k, z[j], n);
             for (int s = 0; s < m; ++s) {
                 double re, im;
-                eval_point(fam, params, dim, r, inv_n, shifts + (size_t)s * dim, trf, fit, &re, &im);
+                eval_point(fam, params, n_params, dim, r, inv_n, shifts + (size_t)s * dim, trf, fit, &re, &im);
                 acc[(size_t)s * nc].add(re);
                 if (nc == 2) acc[(size_t)s * nc + 1].add(im);
             }
@@ -369,13 +382,13 @@ int oracle_project(int fam, const double* params, int n_params, int dim, uint64_
                    const double* shift, int bins, double* out_hist) {
     if (fam < 0 || fam > FAM_LAST) return -8;
     if (dim < 1 || dim > MAX_DIM) return -2;
-    if (expected_params(fam, params, dim) != n_params) return -9;
+    if (expected_params(fam, params, n_params, dim) != n_params) return -9;
     const double inv_n = 1.0 / (double)n;
     std::vector<Comp> H((size_t)dim * bins);
     double x[MAX_DIM];
     for (uint64_t k = 0; k < n; ++k) {
         for (int j = 0; j < dim; ++j) x[j] = coordinate(residue(k, z[j], n), inv_n, shift[j]);
-        double re, im; integrand(fam, params, dim, x, &re, &im);
+        double re, im; integrand(fam, params, n_params, dim, x, &re, &im);
         double a = ncomp_of(fam) == 2 ? std::hypot(re, im) : std::fabs(re);
         for (int j = 0; j < dim; ++j) {
             int b = (int)std::floor((double)bins * x[j]);

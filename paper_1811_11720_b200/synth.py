@@ -173,6 +173,16 @@ def sector(rng, d, deg_u=2, deg_f=3, n_lo=6, n_span=15):
     return np.array(out, dtype=np.float64)
 
 
+def sector_log(rng, d, **kw):
+    """Sector-like integrand with the trailing block [lu, lf, p]: f * (lu log U + lf log F)^p, the shape of the
+    order-eps^p term of U^(a + lu eps) / F^(b - lf eps).  lu in [0.5, 2), lf in [-3, -1), p in 1..3."""
+    prm = sector(rng, d, **kw)
+    lu = rng.uniform_range(0.5, 2.0)
+    lf = rng.uniform_range(-3.0, -1.0)
+    pw = 1 + rng.next_u64() % 3
+    return np.concatenate([prm, np.array([lu, lf, float(pw)])])
+
+
 def problem(family, params, n, z, shifts, transform, fit_coeffs=None, name=""):
     shifts = np.ascontiguousarray(shifts, dtype=np.float64)
     return {"name": name, "family": int(family), "params": np.ascontiguousarray(params, dtype=np.float64),

@@ -421,6 +421,72 @@ def test_family3_tensor_gauss_legendre(d, seed):
         assert abs(oracle.integrand(synth.FAMILY_SECTOR, prm, x) - want) <= 1e-14 * abs(want)
 
 
+# --- log factors of the sector family (trailing [lu, lf, p], reading C-15) ---
+def _one_dim_log_problem(prm, n=65537, seed=31):
+    rng = synth.MT19937_64(seed)
+    return synth.problem(synth.FAMILY_SECTOR, np.array(prm, dtype=np.float64), n, np.array([1], dtype=np.uint64),
+                         synth.draw_shifts(rng, 8, 1), K3)
+
+
+def test_sector_log_closed_forms_one_dimension():
+    L2 = math.log(2.0)
+    # U = 1 + x, F = 1, a = b = 0:  int log(1+x) = 2 ln 2 - 1;  int log^2(1+x) = 2 ln^2 2 - 4 ln 2 + 2
+    base = [0, 0, 2, 1, 0, 1.0, 1.0, 0, 1, 1.0, 0]
+    _check_vs_exact(_one_dim_log_problem(base + [1.0, 0.0, 1]), 2 * L2 - 1, rel=1e-9)
+    _check_vs_exact(_one_dim_log_problem(base + [1.0, 0.0, 2]), 2 * L2 * L2 - 4 * L2 + 2, rel=1e-9)
+    # coefficient lu scales the term; lf multiplies log F = log 1 = 0 here
+    _check_vs_exact(_one_dim_log_problem(base + [-2.5, 7.0, 1]), -2.5 * (2 * L2 - 1), rel=1e-9)
+    # U = 1, F = 1 + x, b = 1: int log(1+x)/(1+x) = ln^2 2 / 2 (lf picks F, lu picks U = 1)
+    base = [0, 1, 1, 2, 0, 1.0, 0, 1.0, 1.0, 0, 1]
+    _check_vs_exact(_one_dim_log_problem(base + [9.0, 1.0, 1]), 0.5 * L2 * L2, rel=1e-9)
+    # U = 1 + x, a = 1, F = 2 (constant): int (1+x)/2 * (log(1+x) - log 2) = [ (1+x)^2 (2 log(1+x) - 1) / 8 ]_0^1 - 3 ln 2 / 4
+    base = [1, 1, 2, 1, 0, 1.0, 1.0, 0, 1, 2.0, 0]
+    exact = (4 * (2 * L2 - 1) / 8 + 1 / 8) - 0.75 * L2
+    _check_vs_exact(_one_dim_log_problem(base + [1.0, -1.0, 1]), exact, rel=1e-9)
+
+
+@pytest.mark.parametrize("d,seed", [(2, 41), (3, 42), (6, 43)])
+def test_sector_log_is_the_epsilon_derivative(d, seed):
+    """f L^p is the p-th eps-derivative at 0 of prod x^nu U^(a + lu eps) F^(-b + lf eps): checked pointwise against real
+    powers (numpy, central differences in extended steps), which involve no logarithm of the oracle's."""
+    rng = synth.MT19937_64(seed)
+    prm = synth.sector_log(rng, d)
+    lu, lf, pw = prm[-3], prm[-2], int(prm[-1])
+    base = prm[:-3]
+    a, b, nU, nF = (int(v) for v in base[:4])
+    o = 4 + d
+    cU, eU = base[o:o + nU], base[o + nU:o + nU + nU * d].reshape(nU, d)
+    o += nU * (1 + d)
+    cF, eF = base[o:o + nF], base[o + nF:o + nF + nF * d].reshape(nF, d)
+    X = np.array([[rng.uniform() for _ in range(d)] for _ in range(6)])
+    U = np.array([sum(cU[t] * np.prod(x ** eU[t]) for t in range(nU)) for x in X]).astype(np.longdouble)
+    F = np.array([sum(cF[t] * np.prod(x ** eF[t]) for t in range(nF)) for x in X]).astype(np.longdouble)
+    pre = np.prod(X ** base[4:4 + d], axis=1).astype(np.longdouble)
+
+    def g(eps):
+        eps = np.longdouble(eps)
+        return pre * U ** (a + np.longdouble(lu) * eps) * F ** (-b + np.longdouble(lf) * eps)
+
+    h = 2e-3 if pw > 1 else 1e-4
+    # central differences, O(h^2) error removed by one Richardson step
+    def deriv(h):
+        if pw == 1:
+            return (g(h) - g(-h)) / (2 * h)
+        if pw == 2:
+            return (g(h) - 2 * g(0) + g(-h)) / (h * h)
+        return (g(2 * h) - 2 * g(h) + 2 * g(-h) - g(-2 * h)) / (2 * h ** 3)
+    want = (4 * deriv(h / 2) - deriv(h)) / 3
+    # the difference quotient is accurate relative to the size of its terms, not to a result that nearly cancels
+    scale = np.asarray(g(0) * (abs(lu) * np.abs(np.log(U)) + abs(lf) * np.abs(np.log(F))) ** pw, dtype=np.float64)
+    for x, w, sc in zip(X, want, scale):
+        got = oracle.integrand(synth.FAMILY_SECTOR, prm, x)
+        assert abs(got - float(w)) <= 2e-6 * sc, (got, float(w), sc)
+    # and p is only accepted as an integer in 1..4
+    bad = prm.copy(); bad[-1] = 0.0
+    with pytest.raises(ValueError):
+        oracle.integrand(synth.FAMILY_SECTOR, bad, X[0])
+
+
 def test_integrand_param_count_checked():
     with pytest.raises(ValueError):
         oracle.integrand(synth.FAMILY_GENZ_OSC, [0.1, 0.2], [0.5, 0.5])
