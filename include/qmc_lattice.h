@@ -41,6 +41,12 @@
  *                               f = prod x_j^nu_j * U(x)^a / F(x)^b, U = sum_t cU_t prod_j x_j^eU_{t,j}
  *                               (sector-decomposed shape); limits: 0 <= a,b <= 8, nu_j <= 8,
  *                               nU,nF in 1..64, exponents <= 8, total degree of a monomial <= 16.
+ *                               Optional trailing block [lu, lf, p] (n_params = the above + 3):
+ *                               f * (lu log U + lf log F)^p, p an integer in 1..4 -- the shape of the order-eps^p
+ *                               term of U^(a + lu eps) / F^(b - lf eps) in the eps-expansion of a sector;
+ *                               U, F > 0 is the caller's responsibility (a non-positive value gives NaN results).
+ *                               Entry points that take n_params accept it; qmc_lattice_integrate, which derives
+ *                               n_params from (family, dim, params), reads the block without it.
  */
 #ifndef QMC_LATTICE_H
 #define QMC_LATTICE_H

@@ -27,7 +27,8 @@
 // Fourier-mode exactness / dual-lattice modes; the one-dimensional rule as an exact geometric series; Eq. 15 normalisation
 // and phi = regularised incomplete beta (symmetric and asymmetric weights); Eq. 16 constants and Gauss-Legendre
 // quadrature of the Sidi weight; closed forms of families 0-2 and 4-7 (Genz 1-6); tensor Gauss-Legendre for
-// the sector family at d<=3; x0*x1*x2 -> 1/8 (Fig. 2); Eq. 3 on hand-made means; projection marginals in
+// the sector family at d<=3; x0*x1*x2 -> 1/8 (Fig. 2); log factors of the sector family by one-dimensional
+// closed forms and the eps-derivative identity; Eq. 3 on hand-made means; projection marginals in
 // closed form; fit recovers an exact cubic.
 // Parity unpinned: nothing in this file (the CBC tool and the Levenberg-Marquardt fit of the product are not part of the
 // oracle).

@@ -108,7 +108,8 @@ int validate_struct(const qmc_problem& p, bool need_two_shifts) {
     if (p.family == QMC_FAMILY_GENZ_DISCONT && p.n_params != p.dim + std::min(p.dim, 2)) return QMC_ERR_PARAMS;
     if (p.family == QMC_FAMILY_SECTOR) {
         const int rest = p.n_params - 4 - p.dim;
-        if (rest < 2 * (1 + p.dim) || rest % (1 + p.dim) != 0 || rest / (1 + p.dim) > 2 * kMaxSectorMono) return QMC_ERR_PARAMS;
+        const bool plain = rest % (1 + p.dim) == 0, with_log = rest >= 3 && (rest - 3) % (1 + p.dim) == 0;   // optional trailing [lu, lf, p]
+        if (rest < 2 * (1 + p.dim) || !(plain || with_log) || rest / (1 + p.dim) > 2 * kMaxSectorMono) return QMC_ERR_PARAMS;
     }
     return QMC_OK;
 }
@@ -441,7 +442,10 @@ int validate_values(const qmc_problem& p) {
         for (int k = 0; k < 4; ++k)
             if (q[k] != std::floor(q[k]) || q[k] < 0.0) return QMC_ERR_PARAMS;
         if (q[0] > 8 || q[1] > 8 || q[2] < 1 || q[3] < 1 || q[2] > kMaxSectorMono || q[3] > kMaxSectorMono) return QMC_ERR_PARAMS;
-        if (4 + p.dim + ((int)q[2] + (int)q[3]) * (1 + p.dim) != p.n_params) return QMC_ERR_PARAMS;
+        const int base = 4 + p.dim + ((int)q[2] + (int)q[3]) * (1 + p.dim);
+        if (p.n_params == base + 3) {                                            // log factor: p an integer in 1..4
+            if (!(q[base + 2] >= 1.0 && q[base + 2] <= 4.0) || q[base + 2] != std::floor(q[base + 2])) return QMC_ERR_PARAMS;
+        } else if (p.n_params != base) return QMC_ERR_PARAMS;
     }
     if (p.fit_coeffs) {
         for (int j = 0; j < p.dim; ++j) {

@@ -78,7 +78,9 @@ struct alignas(16) DevAux {
     double fit[9][QMC_MAX_DIM];            // a4, a5, a6, 2*a5, 3*a6 of the cubic part; a0, a2 (a0-1), a1, a3 (a1-1) of the poles
     double fam0;                           // OSC: 2 pi u0
     double sec_c0[2];                      // sector: constant terms of U and F
+    double sec_log[2];                     // sector: lu, lf of the optional log factor (lu log U + lf log F)^p
     int sec_a, sec_b;                      // sector: powers of U and F
+    int sec_logp, sec_pad_;                // sector: p of the log factor, 0 = none
     int sec_nops[2];                       // sector: [0] = 32-bit step words of the program (U, end-of-U, F)
     int sec_ncoef[2];                      // sector: [0] = coefficients of the program
     int status;                            // 0 or a qmc_status found while preparing

@@ -28,6 +28,7 @@ __global__ void __launch_bounds__(32) prepare_kernel(const DevProblem* __restric
         a.fit_full = fit_has_poles(pb);
         a.status = 0;
         a.sec_a = a.sec_b = 0;
+        a.sec_logp = 0; a.sec_log[0] = a.sec_log[1] = 0.0;
         a.sec_nops[0] = a.sec_nops[1] = a.sec_ncoef[0] = a.sec_ncoef[1] = 0;
         a.sec_c0[0] = a.sec_c0[1] = 0.0;
     }

@@ -99,7 +99,12 @@ __device__ double abs_integrand(const ProjArgs& a, const double* x) {
         poly[w] = s;
         base += cnt[w] * (1 + d);
     }
-    return fabs(pre * ipow_small(poly[0], pa) / ipow_small(poly[1], pb));
+    double f = pre * ipow_small(poly[0], pa) / ipow_small(poly[1], pb);
+    if (a.n_params == 4 + d + (nU + nF) * (1 + d) + 3) {                     // trailing [lu, lf, p]: log factors of the sector family
+        const double* t = p + a.n_params - 3;
+        f *= ipow_small(t[0] * log(poly[0]) + t[1] * log(poly[1]), (int)t[2]);
+    }
+    return fabs(f);
 }
 
 template <bool WIDE>

@@ -35,14 +35,17 @@ struct alignas(16) SectorSmem {
     double c0[2];                    // constant terms of U and F
     unsigned long long nu_packed;    // nu_j in 4 bits each
     int a, b;                        // powers of U and F
+    double lg[2];                    // lu, lf of the log factor
+    int logp, pad_;                  // its power p (0 = no log factor)
     double wpark[8 * kThreads];      // [q][thread]: the G weights of a thread, parked while the interpreter runs (registers)
 };
 struct SectorOff {                   // byte offsets of the fields above (read with ld.shared in the inner loop)
-    static constexpr unsigned coefs = 0, words = kSecMaxCoef * 8, c0 = words + kSecMaxWords * 4, nu = c0 + 16, ab = nu + 8, wpark = ab + 8;
+    static constexpr unsigned coefs = 0, words = kSecMaxCoef * 8, c0 = words + kSecMaxWords * 4, nu = c0 + 16, ab = nu + 8, lg = ab + 8, logp = lg + 16, wpark = logp + 8;
 };
 
 static_assert(offsetof(SectorSmem, words) == SectorOff::words && offsetof(SectorSmem, c0) == SectorOff::c0 &&
               offsetof(SectorSmem, nu_packed) == SectorOff::nu && offsetof(SectorSmem, a) == SectorOff::ab &&
+              offsetof(SectorSmem, lg) == SectorOff::lg && offsetof(SectorSmem, logp) == SectorOff::logp &&
               offsetof(SectorSmem, wpark) == SectorOff::wpark, "SectorOff must mirror SectorSmem");
 
 // ---- device-side compiler: params -> program (one thread; a few hundred steps at most) ---------
@@ -75,7 +78,12 @@ __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned 
         return;
     }
     const int cnt[2] = {(int)nUv, (int)nFv};
-    if (4 + d + (cnt[0] + cnt[1]) * (1 + d) != pb.n_params) { a.status = QMC_ERR_PARAMS; return; }
+    const int n_base = 4 + d + (cnt[0] + cnt[1]) * (1 + d);
+    if (pb.n_params == n_base + 3) {                   // trailing [lu, lf, p]: f (lu log U + lf log F)^p, p in 1..4
+        const double pw = p[n_base + 2];
+        if (!(pw >= 1.0 && pw <= 4.0) || pw != floor(pw)) { a.status = QMC_ERR_PARAMS; return; }
+        a.sec_log[0] = p[n_base]; a.sec_log[1] = p[n_base + 1]; a.sec_logp = (int)pw;
+    } else if (pb.n_params != n_base) { a.status = QMC_ERR_PARAMS; return; }
     a.sec_a = (int)av; a.sec_b = (int)bv;
     for (int j = 0; j < d; ++j) {
         const double v = p[4 + j];
@@ -83,7 +91,7 @@ __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned 
         a.nu[j] = (unsigned char)(int)v;
     }
     double* coefs = reinterpret_cast<double*>(prog_area + pb.aux_off);
-    const int max_coef = sector_coef_slots(cnt[0] + cnt[1]);
+    const int max_coef = sector_coef_slots((pb.n_params - 4 - d) / (1 + d));   // the same upper bound as the host plan and the kernel
     unsigned char* ops = reinterpret_cast<unsigned char*>(prog_area + pb.aux_off + max_coef);
     const int max_ops = min((pb.aux_len - max_coef) * 8, kMaxSectorOps) - 8;   // room for SEC_ENDU, SEC_END and 3+ bytes of read-ahead padding
     int nops = 0, ncoef = 0;
@@ -172,6 +180,15 @@ __device__ __forceinline__ void sector_coords(const typename Res<WIDE>::T (&r)[D
     for (int q = 0; q < G; ++q) W[q] = point_weight<TR, FIT>(P[q], D[q], cx.wconst, cx.kor_r);
 }
 
+// (lu log U + lf log F)^p, p in 1..4 (the eps-expansion of U^(a + lu eps) / F^(b - lf eps)).
+// Kept out of line: the kernels are tuned for the plain sector integrand and only pay a predicated-off call for this.
+static __device__ __noinline__ double sector_log_factor(double U, double F, double lu, double lf, int p) {
+    const double L = __dadd_rn(__dmul_rn(lu, log(U)), __dmul_rn(lf, log(F)));
+    double r = L;
+    for (int e = 1; e < p; ++e) r = __dmul_rn(r, L);
+    return r;
+}
+
 // Transform and fit map are selected per point by a warp-uniform switch, so that the interpreter exists once per
 // tile loop.  SLOW = false: Korobov-3 without fit map, the paper's default for loop integrals, as the only
 // inlined tile loop of the kernel (a smaller kernel body measurably helps the interpreter: DESIGN.md section 5); SLOW = true:
@@ -210,6 +227,13 @@ template <int DP, int G, bool WIDE, bool SLOW> struct SectorEval {
             for (int e = 0; e < nu; ++e)
 #pragma unroll
                 for (int q = 0; q < G; ++q) num[q] *= x[q][j];
+        }
+        // optional log factor (lu log U + lf log F)^p of an eps-expansion term: a cold, warp-uniform branch through a real call
+        const int lp = (int)(unsigned)lds_u64(exbase + SectorOff::logp);
+        if (lp) {
+            const double lu = lds_f64(exbase + SectorOff::lg), lf = lds_f64(exbase + SectorOff::lg + 8u);
+#pragma unroll
+            for (int q = 0; q < G; ++q) num[q] *= sector_log_factor(U[q], F[q], lu, lf, lp);
         }
         double den[G];
 #pragma unroll
@@ -256,6 +280,7 @@ __global__ void __launch_bounds__(kThreads, SectorMinBlocks<DP, G>::value) fused
             if (tid == 32) {
                 ex.c0[0] = a.sec_c0[0]; ex.c0[1] = a.sec_c0[1];
                 ex.a = a.sec_a; ex.b = a.sec_b;
+                ex.lg[0] = a.sec_log[0]; ex.lg[1] = a.sec_log[1]; ex.logp = a.sec_logp; ex.pad_ = 0;
                 unsigned long long nup = 0;
                 for (int j = 0; j < 16; ++j) nup |= (unsigned long long)(a.nu[j] & 15) << (4 * j);
                 ex.nu_packed = nup;

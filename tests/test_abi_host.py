@@ -87,6 +87,25 @@ def test_validate_problem_host_rejects(mutate, status):
     assert binding.qmc_validate_problem_host(p) == status
 
 
+@pytest.mark.parametrize("d", [1, 2, 3, 6])
+def test_validate_sector_log_block(d):
+    """The sector block takes an optional trailing [lu, lf, p] (p an integer in 1..4); d = 2 is the case where three more
+    doubles could be mistaken for one more monomial."""
+    rng = synth.MT19937_64(90 + d)
+    prm = synth.sector_log(rng, d)
+    n = 1021
+    p = synth.problem(synth.FAMILY_SECTOR, prm, n, synth.korobov_form_vector(n, d, 341), synth.draw_shifts(rng, 4, d),
+                      synth.TRANSFORM_KOROBOV + 3)
+    assert binding.qmc_validate_problem_host(p) == 0
+    assert binding.qmc_validate_problem_host(dict(p, params=prm[:-3])) == 0               # the plain block
+    for bad_p in (0.0, 5.0, 1.5, -1.0):
+        q = prm.copy(); q[-1] = bad_p
+        assert binding.qmc_validate_problem_host(dict(p, params=q)) == -9
+    for cut in (1, 2):
+        assert binding.qmc_validate_problem_host(dict(p, params=prm[:-cut])) == -9
+    assert binding.qmc_validate_problem_host(dict(p, params=np.concatenate([prm, [1.0]]))) == -9
+
+
 def test_z_must_be_coprime_to_n():
     """'integers coprime to n'; n itself need not be prime (Fig. 1 uses 55, L108)."""
     p = _cfg0()

@@ -497,6 +497,60 @@ def test_workspace_errors():
     assert abs(b.means.cpu().numpy()[0, 0] - mean_or[0]) <= 1e-13 * abs(mean_or[0])
 
 
+# ------------------------------------------------------------------------------------------------
+# log factors of the sector family: f (lu log U + lf log F)^p (reading C-15)
+# ------------------------------------------------------------------------------------------------
+def make_log(d, n, m, tr, seed, fit=False, pw=None):
+    p = make(3, d, n, m, tr, seed, fit=fit)
+    rng = synth.MT19937_64(seed)
+    prm = synth.sector_log(rng, d)                            # the same leading block as make() draws + [lu, lf, p]
+    assert np.array_equal(prm[:-3], p["params"])
+    if pw is not None:
+        prm[-1] = float(pw)
+    return dict(p, params=prm, name=p["name"] + f".log{int(prm[-1])}")
+
+
+@pytest.mark.parametrize("d", [1, 3, 4, 6, 8, 9, 16])
+@pytest.mark.parametrize("tr,fit", [(K + 3, False), (K + 3, True), (NONE, False), (BAKER, "full"), (SIDI + 2, False), (KA + 16 * 2 + 1, True)])
+def test_sector_log_factor_means(d, tr, fit):
+    probs = [make_log(d, 8191, 6, tr, 2600 + d, fit=fit, pw=pw) for pw in (1, 2, 3, 4)]
+    check_against_oracle(probs)
+
+
+def test_sector_log_factor_in_a_mixed_batch_and_tails():
+    """plain and log sectors of several sizes share one launch; the log factor of one problem never leaks into the next"""
+    probs = []
+    for i, n in enumerate([127, 1021, 4099, 65537, 262147]):
+        probs.append(make(3, 6, n, 5, K + 3, 2700 + i))
+        probs.append(make_log(6, n, 5, K + 3, 2700 + i))
+        probs.append(make(3, 6, n, 5, K + 3, 2750 + i))
+    sms, _, _ = check_against_oracle(probs)
+    assert not np.array_equal(sms[0], sms[1])
+
+
+def test_sector_log_factor_many_shifts():
+    check_against_oracle([make_log(6, 4099, 130, K + 3, 2800), make_log(16, 4099, 50, K + 3, 2801, fit=True)])
+
+
+def test_sector_log_factor_projection():
+    p = make_log(6, 16381, 2, NONE, 2810)
+    H_or = oracle.project(p, 128)
+    H = binding.DeviceBatch([p]).project(0, 128).cpu().numpy()
+    np.testing.assert_allclose(H, H_or, rtol=1e-12, atol=0)
+    H_plain = oracle.project(dict(p, params=p["params"][:-3]), 128)
+    assert not np.allclose(H_or, H_plain)
+
+
+def test_sector_log_factor_bad_power_yields_nan():
+    good = make_log(3, 1021, 3, K + 3, 2820)
+    bad = dict(good, params=good["params"].copy(), name="bad")
+    bad["params"][-1] = 5.0                                  # p outside 1..4
+    sms, _, _ = run_gpu([good, bad])
+    sm_or, _, _ = oracle.integrate(good)
+    assert_means(sms[0], sm_or, "good")
+    assert np.all(np.isnan(sms[1]))
+
+
 def test_bad_sector_block_yields_nan_not_garbage():
     """a parameter block the device-side compiler rejects (exponent > 8) poisons that problem's results only"""
     good = make(3, 3, 1021, 3, K + 3, 11)
