@@ -91,6 +91,27 @@ def test_complex_error_modes(errormode):
     assert np.all(np.abs(E - mean_or) <= 1e-13 * np.hypot(*mean_or))
 
 
+def test_sector_with_log_factor_through_the_iteration():
+    """an eps-expansion term of a sector (trailing [lu, lf, p] block, reading C-15) through qmc_integrate: the
+    result equals the oracle's at the lattice the iteration stops on"""
+    d = 6
+    rng = synth.MT19937_64(5150)
+    prm = synth.sector_log(rng, d)
+    sh = synth.draw_shifts(rng, 16, d)
+    ln, lz = synth.ladder(d, 262139)
+    res, st = binding.qmc_integrate(synth.FAMILY_SECTOR, prm, d, K + 3, ln, lz, sh, min_n=1000, min_m=16, epsrel=1e-6, epsabs=0.0,
+                                    maxeval=10**9)
+    assert st == 0 and res["m"] == 16 and res["error"][0] <= 1e-6 * abs(res["integral"][0])
+    p = synth.problem(synth.FAMILY_SECTOR, prm, int(ln[0]), lz[0], sh, K + 3)
+    sm_or, mean_or, err_or = _oracle_at(p, res, ln, lz)
+    assert abs(res["integral"][0] - mean_or[0]) <= 1e-13 * abs(mean_or[0])
+    assert abs(res["error"][0] - err_or[0]) <= 1e-12 * err_or[0] + 1e-13 * np.max(np.abs(sm_or)) / np.sqrt(15.0)
+    # without the block the same call integrates a different function
+    res0, st0 = binding.qmc_integrate(synth.FAMILY_SECTOR, prm[:-3], d, K + 3, ln, lz, sh, min_n=1000, min_m=16, epsrel=1e-6,
+                                      epsabs=0.0, maxeval=10**9)
+    assert st0 == 0 and abs(res0["integral"][0] - res["integral"][0]) > 1e-3 * abs(res0["integral"][0])
+
+
 def test_argument_errors():
     p = _problem(0, 10)
     ln, lz = synth.ladder(4, 65537)
