@@ -37,7 +37,8 @@ struct alignas(16) SectorSmem {
     int a, b;                        // powers of U and F
     double lg[2];                    // lu, lf of the log factor
     int logp, pad_;                  // its power p (0 = no log factor)
-    double wpark[8 * kThreads];      // [q][thread]: the G weights of a thread, parked while the interpreter runs (registers)
+    double wpark[16 * kThreads];     // [q][thread]: the G weights of a thread, parked while the interpreter runs (registers);
+                                     // with a log factor afterwards U in [0, 8), F in [8, 16) for sector_log_factors
 };
 struct SectorOff {                   // byte offsets of the fields above (read with ld.shared in the inner loop)
     static constexpr unsigned coefs = 0, words = kSecMaxCoef * 8, c0 = words + kSecMaxWords * 4, nu = c0 + 16, ab = nu + 8, lg = ab + 8, logp = lg + 16, wpark = logp + 8;
@@ -181,12 +182,62 @@ __device__ __forceinline__ void sector_coords(const typename Res<WIDE>::T (&r)[D
 }
 
 // (lu log U + lf log F)^p, p in 1..4 (the eps-expansion of U^(a + lu eps) / F^(b - lf eps)).
-// Kept out of line: the kernels are tuned for the plain sector integrand and only pay a predicated-off call for this.
-static __device__ __noinline__ double sector_log_factor(double U, double F, double lu, double lf, int p) {
-    const double L = __dadd_rn(__dmul_rn(lu, log(U)), __dmul_rn(lf, log(F)));
-    double r = L;
-    for (int e = 1; e < p; ++e) r = __dmul_rn(r, L);
-    return r;
+// The kernels are tuned for the plain sector integrand and only pay a never-taken warp-uniform branch for this (C-15).
+// log x for the log factor.  Normal positive x (every sane U, F): x = 2^e m with m in (sqrt(1/2), sqrt(2)], log m = 2 atanh(s),
+// s = (m - 1)/(m + 1), |s| <= 0.1716, by the Taylor series 2s (1 + z/3 + z^2/5 + ... + z^11/23), z = s^2 (truncation 6e-19
+// relative), the quotient corrected to 1 ulp, e log 2 added as a two-term sum; measured <= 2 ulp against long double on
+// 2e7 arguments in [e^-20, e^20] and relatively accurate towards x = 1.  Anything else (x <= 0, subnormal, inf, NaN) takes
+// the library routine (sector_log_factors).
+// Series coefficients 1/23 .. 1/3, sqrt 2 and the two halves of log 2 come from the constant bank as direct DFMA operands (as
+// immediates every one of them cost two uniform moves per use).
+static __constant__ double kLogC[14] = {1.0 / 23.0, 1.0 / 21.0, 1.0 / 19.0, 1.0 / 17.0, 1.0 / 15.0, 1.0 / 13.0, 1.0 / 11.0, 1.0 / 9.0,
+                                        1.0 / 7.0, 1.0 / 5.0, 1.0 / 3.0, 1.4142135623730951, 0.6931471805599453, 2.3190468138462996e-17};
+// The series itself is branch-free (its result is meaningless unless log_arg_is_normal_positive(x)), so that the chains of
+// several logarithms share a basic block and overlap: with 3 warps per scheduler the path is bound by FP64 latency.
+static __device__ __forceinline__ bool log_arg_is_normal_positive(double x) {
+    const int hi = __double2hiint(x);
+    return hi >= 0x00100000 && hi < 0x7ff00000;
+}
+static __device__ __forceinline__ double log_normal_positive(double x) {
+    const int hi = __double2hiint(x);
+    int e = (hi >> 20) - 1023;
+    double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(x));
+    const bool big = m > kLogC[11];
+    m = big ? __dmul_rn(m, 0.5) : m;
+    e += big;
+    const double f = __dadd_rn(m, -1.0), den = __dadd_rn(m, 1.0);
+    const double r = rcp_nr(den);
+    double sq = __dmul_rn(f, r);
+    sq = __fma_rn(__fma_rn(-sq, den, f), r, sq);
+    const double z = __dmul_rn(sq, sq);
+    double p = kLogC[0];
+#pragma unroll
+    for (int i = 1; i <= 10; ++i) p = __fma_rn(p, z, kLogC[i]);
+    const double t = __dadd_rn(sq, sq);
+    const double lm = __fma_rn(__dmul_rn(t, z), p, t);
+    const double ed = (double)e;
+    return __fma_rn(ed, kLogC[12], __fma_rn(ed, kLogC[13], lm));   // log 2 = hi + lo
+}
+
+// Once per lattice index: the caller parks U[q] at park + 8 kThreads q and F[q] at park + 8 kThreads (8 + q) (its own
+// column of SectorSmem::wpark) and reads the factors back from the U slots.
+static __device__ __forceinline__ void sector_log_factors(unsigned park, int g, double lu, double lf, int p) {
+#pragma unroll 1
+    for (int q = 0; q < g; q += 2) {                     // g is 4 or 8: two points = four independent logarithms per pass
+        const unsigned at = park + 8u * kThreads * q;
+        const double U0 = lds_f64(at), F0 = lds_f64(at + 64u * kThreads);
+        const double U1 = lds_f64(at + 8u * kThreads), F1 = lds_f64(at + 72u * kThreads);
+        double a0 = log_normal_positive(U0), b0 = log_normal_positive(F0), a1 = log_normal_positive(U1), b1 = log_normal_positive(F1);
+        if (!(log_arg_is_normal_positive(U0) && log_arg_is_normal_positive(F0) && log_arg_is_normal_positive(U1) &&
+              log_arg_is_normal_positive(F1))) {
+            a0 = log(U0); b0 = log(F0); a1 = log(U1); b1 = log(F1);
+        }
+        const double L0 = __dadd_rn(__dmul_rn(lu, a0), __dmul_rn(lf, b0)), L1 = __dadd_rn(__dmul_rn(lu, a1), __dmul_rn(lf, b1));
+        double r0 = L0, r1 = L1;
+        for (int e = 1; e < p; ++e) { r0 = __dmul_rn(r0, L0); r1 = __dmul_rn(r1, L1); }
+        sts_f64(at, r0);
+        sts_f64(at + 8u * kThreads, r1);
+    }
 }
 
 // Transform and fit map are selected per point by a warp-uniform switch, so that the interpreter exists once per
@@ -228,12 +279,15 @@ template <int DP, int G, bool WIDE, bool SLOW> struct SectorEval {
 #pragma unroll
                 for (int q = 0; q < G; ++q) num[q] *= x[q][j];
         }
-        // optional log factor (lu log U + lf log F)^p of an eps-expansion term: a cold, warp-uniform branch through a real call
+        // optional log factor (lu log U + lf log F)^p of an eps-expansion term: a cold, warp-uniform branch
         const int lp = (int)(unsigned)lds_u64(exbase + SectorOff::logp);
         if (lp) {
             const double lu = lds_f64(exbase + SectorOff::lg), lf = lds_f64(exbase + SectorOff::lg + 8u);
 #pragma unroll
-            for (int q = 0; q < G; ++q) num[q] *= sector_log_factor(U[q], F[q], lu, lf, lp);
+            for (int q = 0; q < G; ++q) { sts_f64(park + 8u * kThreads * q, U[q]); sts_f64(park + 8u * kThreads * (8 + q), F[q]); }
+            sector_log_factors(park, G, lu, lf, lp);
+#pragma unroll
+            for (int q = 0; q < G; ++q) num[q] *= lds_f64(park + 8u * kThreads * q);
         }
         double den[G];
 #pragma unroll
