@@ -541,6 +541,28 @@ def test_sector_log_factor_projection():
     assert not np.allclose(H_or, H_plain)
 
 
+def test_sector_log_factor_arguments_outside_the_series():
+    """the kernel's own logarithm serves normal positive arguments; a subnormal U takes the library routine (same bar), and a
+    negative U gives NaN on both sides (include/qmc_lattice.h: U, F > 0 is the caller's responsibility)"""
+    n, d = 1021, 2
+    rng = synth.MT19937_64(2830)
+    z, sh = synth.korobov_form_vector(n, d, 341), synth.draw_shifts(rng, 4, d)
+
+    def prob(cU0, name):
+        # U = cU0 (constant), F = 2 + x0 + 0.5 x1, a = 0, b = 1, nu = (1, 0); log factor (log U + 0.5 log F)^2
+        prm = [0, 1, 1, 3, 1, 0, cU0, 0, 0, 2.0, 1.0, 0.5, 0, 0, 1, 0, 0, 1, 1.0, 0.5, 2]
+        return synth.problem(3, np.array(prm, dtype=np.float64), n, z, sh, K + 3, name=name)
+
+    probs = [prob(1e-310, "subnormal U"), prob(3.0, "normal U"), prob(-1.0, "negative U")]
+    sms, means, errs = run_gpu(probs)
+    for i in (0, 1):
+        sm_or, _, err_or = oracle.integrate(probs[i])
+        assert np.all(np.isfinite(sm_or))
+        assert_means(sms[i], sm_or, probs[i]["name"])
+        assert_err(errs[i, :1], err_or, sm_or, probs[i]["name"])
+    assert np.all(np.isnan(oracle.integrate(probs[2])[0])) and np.all(np.isnan(sms[2]))
+
+
 def test_sector_log_factor_bad_power_yields_nan():
     good = make_log(3, 1021, 3, K + 3, 2820)
     bad = dict(good, params=good["params"].copy(), name="bad")
