@@ -73,7 +73,23 @@ def evals_of(problems):
 SHRINK = 1        # --shrink S (profiling runs only): 1/S of the work of every config, same kernels and tile shapes
 
 
+SECTOR_LOG = False    # --sector-log: configs[3]'s sectors with the log factors of an eps-expansion term (reading C-15)
+# per evaluation on top of configs[3]: 2 logarithms (26 FP64 each: DESIGN.md section 9) + combination 3 + power (mean p - 1 = 1) + product 1
+ALG_FP64_SECTOR_LOG_EXTRA = 2 * 26 + 3 + 1 + 1
+
+
+def with_log_factors(probs):
+    out = []
+    for i, p in enumerate(probs):
+        rng = synth.MT19937_64(synth.SECTOR_SEED + 5000 + i)
+        tail = np.array([rng.uniform_range(0.5, 2.0), rng.uniform_range(-3.0, -1.0), float(1 + rng.next_u64() % 3)])
+        out.append(dict(p, params=np.concatenate([p["params"], tail]), name=p["name"] + ".log"))
+    return out
+
+
 def shrunk_config(c):
+    if c == 3 and SECTOR_LOG:
+        return with_log_factors(synth.config(3, count_override=max(1, 256 // SHRINK)))
     if SHRINK <= 1:
         return synth.config(c)
     if c == 3:
@@ -388,10 +404,10 @@ def run_ours(args):
         total_s = max_over_ranks(sum(step_ms) * 1e-3)
         ev = evals_of(probs)
         fused_avg_s = statistics.fmean(fused_ms) * 1e-3
-        alg = ALG_FP64_PER_EVAL[c]
+        alg = ALG_FP64_PER_EVAL[c] + (ALG_FP64_SECTOR_LOG_EXTRA if c == 3 and SECTOR_LOG else 0)
         achieved = alg * ev / fused_avg_s
         sms, means, errs = batch.results()
-        rec = {"workload": workload_name(c) + (f" [SHRUNK x1/{SHRINK} for profiling: not a bench value]" if SHRINK > 1 else ""), "value": aggregate([ev * steps] * world, total_s), "unit": UNIT,
+        rec = {"workload": workload_name(c) + (" + log factors (lu log U + lf log F)^p [variant, not a BASELINE config]" if c == 3 and SECTOR_LOG else "") + (f" [SHRUNK x1/{SHRINK} for profiling: not a bench value]" if SHRINK > 1 else ""), "value": aggregate([ev * steps] * world, total_s), "unit": UNIT,
                "ms_per_step": total_s / steps * 1e3, "ms_per_step_best": min(step_ms), "steps": steps, "warmup": warmup,
                "evals_per_step_per_gpu": ev, "fused_kernel_ms": fused_avg_s * 1e3,
                "fused_kernel_share_of_step": fused_avg_s * 1e3 * steps / sum(step_ms),
@@ -535,6 +551,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--genz-table", action="store_true",
                     help="run the Genz protocol of the paper's Table 1 / Table 2 through qmc_integrate instead of the throughput bench")
+    ap.add_argument("--sector-log", action="store_true",
+                    help="configs[3] with the log factors of an eps-expansion term on every sector (use with --main 3 --main-only)")
     ap.add_argument("--shrink", type=int, default=1,
                     help="profiling only: run 1/S of every config's work (fewer sectors / a smaller prime n)")
     ap.add_argument("--main", type=int, default=MAIN_CONFIG, choices=[0, 1, 2, 3, 4],
@@ -542,8 +560,9 @@ def main():
     ap.add_argument("--others", type=lambda v: [int(x) for x in v.split(",") if x != ""], default=None,
                     help="comma-separated subset of configs 0,2,3,4 to time besides configs[1] (default: all)")
     args = ap.parse_args()
-    global SHRINK
+    global SHRINK, SECTOR_LOG
     SHRINK = max(1, args.shrink)
+    SECTOR_LOG = bool(args.sector_log)
     if args.impl == "reference":
         if args.steps > 40:
             args.steps = 40                                 # bounded: a step is ~1 s of host time
