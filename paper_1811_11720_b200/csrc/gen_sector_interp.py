@@ -5,104 +5,109 @@
 Why PTX: the interpreter dispatches one byte-coded step at a time on the coordinates x[q][j], which must
 stay in registers (shared memory cannot feed the FP64 pipe: 128 B/clk/SM against 2 fp64 warp
 instructions/clk/SM).  Register operands can only be selected by control flow, and nvcc lowers a C++
-`switch` to a tree of compare-and-branch pairs (5 dependent branches per step, which made the kernel
-latency bound).  PTX `brx.idx` gives one indexed branch per step; every case ends with its own dispatch
-(threaded code); step codes are fetched three steps ahead and the next coefficient one monomial ahead, so the
-branch target of the next step is known when a case is entered and its jump-table lookup overlaps the G fp64
-instructions of the step.  The program is followed by >= 3 readable padding bytes.  Measured dead ends (kept out):
-two rotating copies of the case table (no register moves, but twice the code) and fused two-variable steps (a third
-fewer dispatches, three times the cases) were both slower: the L0 instruction cache holds about 6 KB.
+`switch` to a tree of compare-and-branch pairs.  PTX `brx.idx` gives one indexed branch per step; every case
+ends with its own dispatch (threaded code); step codes are fetched two steps ahead, so the index of the next
+branch is known when a case is entered and its jump-table lookup overlaps the G fp64 instructions of the step.
 
-Step codes (qmc_sector.cuh): 0 = no-op, 1 = end of U, 2 = end of program, 3 = dense linear form
-(sum += sum_j c_j x_j with DP coefficients from the stream), 4 + 4*j + 2*FIRST + LAST:
-    FIRST & LAST : sum  = fma(coef, x_j, sum)
-    FIRST        : mon  = coef * x_j
-    LAST         : sum  = fma(mon, x_j, sum)
-    otherwise    : mon *= x_j
+The machine (qmc_sector.cuh has the device-side compiler that targets it): per point two accumulators, S (the value of
+the polynomial) and A (the value of the current group).  A polynomial is a sum of groups
+    x^P * (own + sum_k c_k x_k)          P a monomial (the shared prefix), own / c_k coefficients
+found by factoring the most frequent variable out of the monomial set repeatedly (a greedy multivariate Horner
+form: 30.6 steps instead of 44.4 for the flat monomial-by-monomial evaluation on the seeded sectors of configs[3]).
+Step kinds, one fp64 instruction per point each:
+    SC j : S = fma(A, x_j, S)            closes a group (last prefix variable)
+    SL j : S = fma(cf, x_j, S)           a degree-1 monomial of the polynomial
+    AL j : A = fma(cf, x_j, A)           a further leaf of the group
+    ALI j: A = fma(cf, x_j, cf2)         first leaf of a group (cf2 = own), or cf * x_j for a plain monomial (cf2 = 0)
+    AM j : A = A * x_j                   a prefix variable that is not the last
+Step code = 3 + 5 j + kind; 0 = no-op, 1 = end of a polynomial that is not the last (parks S in the thread's next
+shared-memory column and restarts it with the next polynomial's constant term), 2 = end of program.  SL / AL / ALI and
+the end-of-polynomial step read one 16-byte coefficient slot {cf, cf2} each, in program order.
+
+What was measured on a B200 (one interpreter in isolation, G = 8, 6 coordinates, 12 warps per SM):
+an indexed branch costs about 60 cycles that warps of one scheduler do not overlap well, so a step of 8 fp64
+instructions per warp leaves the FP64 pipe at 35-45 %; the cases must stay resident in the ~6 KB L0 instruction
+cache (48 cases of a three-accumulator Horner machine ran 50 % slower per step than 24, different programs on
+co-resident CTAs 45 % slower than one program per SM -- hence one CTA per SM for this family); a tree of direct
+branches on precomputed predicates was 20 % slower than brx.idx; moving the coefficient with or ahead of its use
+made no difference.
 """
 import os
 
-VARIANTS = [(4, 8), (6, 8), (8, 8), (16, 4)]      # (DP, G) instantiated by qmc_fused_f3.cu
+VARIANTS = [(4, 8, 384), (6, 8, 384), (8, 8, 256), (16, 4, 256)]      # (DP, G, threads per CTA) instantiated by qmc_fused_f3.cu
+KINDS = 5
+SC, SL, AL, ALI, AM = range(KINDS)
 
 
-def gen(dp, g):
-    # operand numbering: sum[q] = %q, U[q] = %(g+q), x[q][j] = %(2g + q*dp + j), then c0f, steps address, coefs address
+def gen(dp, g, nt):
+    # operand numbering: S[q] = %q, x[q][j] = %(g + q*dp + j), then steps address, coefficient address, park address
     s = lambda q: f"%{q}"
-    u = lambda q: f"%{g + q}"
-    x = lambda q, j: f"%{2 * g + q * dp + j}"
-    c0f, steps, coefs = (f"%{2 * g + g * dp + i}" for i in range(3))
+    x = lambda q, j: f"%{g + q * dp + j}"
+    steps, coefs, upark = (f"%{g + g * dp + i}" for i in range(3))
     L = []
     a = L.append
     a("{")
-    a(".reg .f64 " + ", ".join(f"m{q}" for q in range(g)) + ", cf, cfn, " + ", ".join(f"l{j}" for j in range(1, dp)) + ";")
-    a(".reg .u32 pc, pk, tgt, c0, c1;")
-    labels = ["T0_NOP", "T0_ENDU", "LEND", "T0_LIN"] + [f"T0_S{j}_{k}" for j in range(dp) for k in range(4)]
-    a("ts0: .branchtargets " + ", ".join(labels) + ";")
-    for q in range(g):
-        a(f"mov.f64 m{q}, 0d0000000000000000;")
+    a(".reg .f64 " + ", ".join(f"A{q}" for q in range(g)) + ", cfn, cf2n;")
+    a(".reg .u32 pc, pk, pp, tgt, c0;")
+    labels = ["T_NOP", "T_ENDU", "T_END"] + [f"T_{j}_{k}" for j in range(dp) for k in range(KINDS)]
+    a("ts: .branchtargets " + ", ".join(labels) + ";")
     a(f"mov.u32 pc, {steps};")
     a(f"mov.u32 pk, {coefs};")
-    a("ld.shared.f64 cfn, [pk];")
+    a(f"mov.u32 pp, {upark};")
+    for q in range(g):
+        a(f"mov.f64 A{q}, 0d0000000000000000;")
+    a("ld.shared.v2.f64 {cfn, cf2n}, [pk];")
     a("ld.shared.u8 tgt, [pc];")
     a("ld.shared.u8 c0, [pc+1];")
-    a("ld.shared.u8 c1, [pc+2];")
-    a("brx.idx.uni tgt, ts0;")
-    # on entry to the case of step i: c0 = code[i+1] (arrived), c1 = code[i+2] (in flight); the target of step i+1 is known
-    # at entry, so its jump-table lookup overlaps the fp64 work of step i
-    fetch = ["mov.u32 tgt, c0;", "mov.u32 c0, c1;", "ld.shared.u8 c1, [pc+3];", "add.u32 pc, pc, 1;"]
-    leave = "brx.idx.uni tgt, ts0;"
-    coef = ["mov.f64 cf, cfn;", "ld.shared.f64 cfn, [pk+8];", "add.u32 pk, pk, 8;"]
-    a("T0_NOP:")
+    leave = "brx.idx.uni tgt, ts;"
+    a(leave)
+    # on entry to the case of step i: c0 = code[i+1] has arrived; the branch index of step i+1 is known at entry
+    fetch = ["mov.u32 tgt, c0;", "ld.shared.u8 c0, [pc+2];", "add.u32 pc, pc, 1;"]
+    reload = ["ld.shared.v2.f64 {cfn, cf2n}, [pk+16];", "add.u32 pk, pk, 16;"]
+    a("T_NOP:")
     L.extend(fetch)
     a(leave)
-    a("T0_ENDU:")
+    a("T_ENDU:")
     L.extend(fetch)
     for q in range(g):
-        a(f"mov.f64 {u(q)}, {s(q)};")
-        a(f"mov.f64 {s(q)}, {c0f};")
-    a(leave)
-    # dense linear form: DP coefficients from the stream (the first one is the prefetched cfn)
-    a("T0_LIN:")
-    L.extend(fetch)
-    a("mov.f64 cf, cfn;")
-    for j in range(1, dp):
-        a(f"ld.shared.f64 l{j}, [pk+{8 * j}];")
-    a(f"ld.shared.f64 cfn, [pk+{8 * dp}];")
-    a(f"add.u32 pk, pk, {8 * dp};")
-    for j in range(dp):
-        for q in range(g):
-            a(f"fma.rn.f64 {s(q)}, {'cf' if j == 0 else f'l{j}'}, {x(q, j)}, {s(q)};")
+        a(f"st.shared.f64 [pp+{8 * nt * q}], {s(q)};")
+        a(f"mov.f64 {s(q)}, cfn;")
+    a(f"add.u32 pp, pp, {8 * nt * g};")
+    L.extend(reload)
     a(leave)
     for j in range(dp):
-        for k in range(4):
-            first, last = k >> 1, k & 1
-            a(f"T0_S{j}_{k}:")
+        for k in range(KINDS):
+            a(f"T_{j}_{k}:")
             L.extend(fetch)
-            if first:
-                L.extend(coef)
             for q in range(g):
-                if first and last:
-                    a(f"fma.rn.f64 {s(q)}, cf, {x(q, j)}, {s(q)};")
-                elif first:
-                    a(f"mul.rn.f64 m{q}, cf, {x(q, j)};")
-                elif last:
-                    a(f"fma.rn.f64 {s(q)}, m{q}, {x(q, j)}, {s(q)};")
+                X = x(q, j)
+                if k == SC:
+                    a(f"fma.rn.f64 {s(q)}, A{q}, {X}, {s(q)};")
+                elif k == SL:
+                    a(f"fma.rn.f64 {s(q)}, cfn, {X}, {s(q)};")
+                elif k == AL:
+                    a(f"fma.rn.f64 A{q}, cfn, {X}, A{q};")
+                elif k == ALI:
+                    a(f"fma.rn.f64 A{q}, cfn, {X}, cf2n;")
                 else:
-                    a(f"mul.rn.f64 m{q}, m{q}, {x(q, j)};")
+                    a(f"mul.rn.f64 A{q}, A{q}, {X};")
+            if k in (SL, AL, ALI):
+                L.extend(reload)                      # after the last use of the slot: no register moves
             a(leave)
-    a("LEND:")
+    a("T_END:")
     a("}")
     body = "\n".join(f'        "{line}\\n\\t"' for line in L)
-    outs = ", ".join([f'"+d"(sum[{q}])' for q in range(g)] + [f'"+d"(U[{q}])' for q in range(g)])
-    ins = ", ".join([f'"d"(x[{q}][{j}])' for q in range(g) for j in range(dp)] + ['"d"(c0f)', '"r"(steps_addr)', '"r"(coefs_addr)'])
+    outs = ", ".join(f'"+d"(sum[{q}])' for q in range(g))
+    ins = ", ".join([f'"d"(x[{q}][{j}])' for q in range(g) for j in range(dp)] +
+                    ['"r"(steps_addr)', '"r"(coefs_addr)', '"r"(park_addr)'])
     return f"""
-template <> __device__ __forceinline__ void sector_interp<{dp}, {g}>(const double (&x)[{g}][{dp}], unsigned steps_addr,
-                                                                  unsigned coefs_addr, double c0f, double (&U)[{g}],
-                                                                  double (&sum)[{g}]) {{
+template <> __device__ __forceinline__ void sector_interp<{dp}, {g}, {nt}>(const double (&x)[{g}][{dp}], unsigned steps_addr,
+                                                                        unsigned coefs_addr, unsigned park_addr, double (&sum)[{g}]) {{
     asm volatile(
 {body}
         : {outs}
-        : {ins});
+        : {ins}
+        : "memory");
 }}
 """
 
@@ -111,12 +116,13 @@ def main():
     here = os.path.dirname(os.path.abspath(__file__))
     out = ["// GENERATED by gen_sector_interp.py -- do not edit.  Threaded-code interpreter of the sector family",
            "// (inline PTX, one brx.idx.uni per step); included by qmc_sector.cuh inside namespace qmc.",
-           "// sum[] must hold U's constant term on entry; on return U[q] = U(x_q), sum[q] = F(x_q).",
-           "template <int DP, int G> __device__ __forceinline__ void sector_interp(const double (&x)[G][DP], unsigned steps_addr,",
-           "                                                                       unsigned coefs_addr, double c0f, double (&U)[G],",
-           "                                                                       double (&sum)[G]);"]
-    for dp, g in VARIANTS:
-        out.append(gen(dp, g))
+           "// sum[] must hold the first polynomial's constant term on entry; polynomial p < last is parked at",
+           "// park_addr + 8 NT (G p + q) (shared memory, the thread's own column); on return sum[q] = the last polynomial at x_q.",
+           "template <int DP, int G, int NT> __device__ __forceinline__ void sector_interp(const double (&x)[G][DP], unsigned steps_addr,",
+           "                                                                               unsigned coefs_addr, unsigned park_addr,",
+           "                                                                               double (&sum)[G]);"]
+    for dp, g, nt in VARIANTS:
+        out.append(gen(dp, g, nt))
     with open(os.path.join(here, "qmc_sector_interp.inc"), "w") as f:
         f.write("\n".join(out))
 

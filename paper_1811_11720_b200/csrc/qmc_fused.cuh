@@ -34,14 +34,14 @@ template <> struct FamTraits<kKernelFamilyGenzMisc> { static constexpr int NC = 
 
 // Shared-memory image of the problem a CTA is working on.  The double arrays at the front are the
 // operands of the inner loop; they are read with ld.shared at sbase + compile-time offsets.
-template <int DP, int G> struct alignas(16) SmemCtx {
+template <int DP, int G, int NT = kThreads> struct alignas(16) SmemCtx {
     double delta[(DP * G > kDeltaCache) ? DP * G : kDeltaCache];   // [group][j][q] shifts (1/2 in padded slots): all groups of
                                    // the problem when they fit, else only the current group
     double fam[DP * 2];            // [j] = (fam_a, fam_b)
     double fit[DP * 10];           // [j] = (a4, a5, a6, 2 a5, 3 a6, -, a0, a2 (a0-1), a1, a3 (a1-1))  fit map of Eq. 19
     double kor[16];                // transform tables (DevProblem::kor)
     unsigned long long step[DP], back[DP], z[DP];
-    double red[2][kWarps][G * 2];  // double-buffered by group parity
+    double red[2][NT / 32][G * 2]; // double-buffered by group parity
     DevProblem prob;
     double fam0;
     long long tile;                // popped tile index
@@ -292,11 +292,12 @@ template <int FAMILY, int DP, int G, bool WIDE, int TR, int FIT> struct ClosedEv
 };
 
 // ---- one tile: residue walk (S1), G shifts per index (EV::eval = S2-S6), tile reduction (S7) ----
-template <class EV, int DP, int G, bool WIDE>
-__device__ __forceinline__ void run_tile(SmemCtx<DP, G>& sm, unsigned sbase, const typename EV::Extra& ex, long long tile_local,
+template <class EV, int DP, int G, bool WIDE, int NT = kThreads>
+__device__ __forceinline__ void run_tile(SmemCtx<DP, G, NT>& sm, unsigned sbase, const typename EV::Extra& ex, long long tile_local,
                                          bool changed, double* __restrict__ partials) {
     typedef typename Res<WIDE>::T RT;
     constexpr int NC = EV::NC;
+    constexpr int kThreads = NT, kWarps = NT / 32;           // threads of this kernel variant (shadow the closed-form default)
     // residue strides live in registers while they are few; otherwise they are re-read from shared memory
     constexpr bool STEP_IN_REGS = DP * (WIDE ? 2 : 1) <= 16;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -308,7 +309,7 @@ __device__ __forceinline__ void run_tile(SmemCtx<DP, G>& sm, unsigned sbase, con
     cx.fit_mode = pb.has_fit ? 1 + sm.fit_full : 0;
     cx.sel = (pb.tr_kind != TR_KORR && cx.fit_mode <= 1) ? pb.tr_kind * 2 + cx.fit_mode : -1;
     cx.fam_kind = pb.family; cx.fam_pow = pb.dim + 1;
-    typedef SmemCtx<DP, G> Ctx;
+    typedef SmemCtx<DP, G, NT> Ctx;
     typedef SmemOff<DP, G> Off;
     static_assert(offsetof(Ctx, fam) == Off::fam && offsetof(Ctx, fit) == Off::fit && offsetof(Ctx, kor) == Off::kor &&
                   offsetof(Ctx, step) == Off::step, "SmemOff must mirror SmemCtx");
@@ -400,20 +401,20 @@ __device__ __forceinline__ void run_tile(SmemCtx<DP, G>& sm, unsigned sbase, con
 }
 
 // the same tile loop as a real (not inlined) call: used for the correctness paths so that their register needs stay theirs
-template <class EV, int DP, int G, bool WIDE>
-__device__ __noinline__ void run_tile_call(SmemCtx<DP, G>& sm, unsigned sbase, const typename EV::Extra& ex, long long tile_local,
+template <class EV, int DP, int G, bool WIDE, int NT = kThreads>
+__device__ __noinline__ void run_tile_call(SmemCtx<DP, G, NT>& sm, unsigned sbase, const typename EV::Extra& ex, long long tile_local,
                                            bool changed, double* __restrict__ partials) {
-    run_tile<EV, DP, G, WIDE>(sm, sbase, ex, tile_local, changed, partials);
+    run_tile<EV, DP, G, WIDE, NT>(sm, sbase, ex, tile_local, changed, partials);
 }
 
 // ---- S0: per-slot constants of a problem, derived from the caller's arrays ------------------------
-// z mod n, the residue stride between a thread's points (kThreads z_j mod n), the rewind of a full walk, the family
+// z mod n, the residue stride between a thread's points (threads z_j mod n), the rewind of a full walk, the family
 // constants and the cubic-map constants of dimension slot j.  Slots j >= dim get the padding values (file header).
 struct SlotConst {
     unsigned long long z, step, back;
     double fa, fb, f[9];
 };
-__device__ __forceinline__ SlotConst derive_slot(const DevProblem& pb, int j) {
+__device__ __forceinline__ SlotConst derive_slot(const DevProblem& pb, int j, int threads = kThreads) {
     SlotConst s;
     s.z = 0; s.step = 0; s.back = 0; s.fa = 0.0; s.fb = 0.0;
     s.f[0] = 1.0; s.f[1] = s.f[2] = s.f[3] = s.f[4] = 0.0;
@@ -422,8 +423,8 @@ __device__ __forceinline__ SlotConst derive_slot(const DevProblem& pb, int j) {
     const unsigned long long n = pb.n;
     if (j < d) {
         s.z = pb.z[j] % n;
-        s.step = mulmod_u64((unsigned long long)kThreads % n, s.z, n);
-        s.back = mulmod_u64(((unsigned long long)pb.steps * kThreads) % n, s.z, n);
+        s.step = mulmod_u64((unsigned long long)threads % n, s.z, n);
+        s.back = mulmod_u64(((unsigned long long)pb.steps * threads) % n, s.z, n);
         const double* p = pb.params;
         if (pb.family == QMC_FAMILY_GENZ_OSC) { s.fa = p[1 + j]; }
         else if (pb.family == QMC_FAMILY_GENZ_PRODPEAK) { const double c = p[j]; s.fa = __ddiv_rn(1.0, __dmul_rn(c, c)); s.fb = p[d + j]; }
@@ -465,9 +466,10 @@ __device__ __forceinline__ double derive_fam0(const DevProblem& pb) {
 // shared-memory image of the problem (changed = true): closed-form families derive the slot constants
 // themselves (S0), the sector family reads what prepare_kernel left in DevAux.
 // `cur` = problem index loaded (-1: none), `iter` = tiles this CTA has taken (single mode).
-template <int DP, int G, bool SECTOR>
-__device__ __forceinline__ bool next_tile(SmemCtx<DP, G>& sm, const FusedLaunch& L, int& cur, int& iter, long long& tile_local,
+template <int DP, int G, bool SECTOR, int NT = kThreads>
+__device__ __forceinline__ bool next_tile(SmemCtx<DP, G, NT>& sm, const FusedLaunch& L, int& cur, int& iter, long long& tile_local,
                                           bool& changed) {
+    constexpr int kThreads = NT;
     const int tid = threadIdx.x;
     changed = false;
     __syncthreads();                                        // everyone is done with the previous tile

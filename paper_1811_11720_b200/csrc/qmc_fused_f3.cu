@@ -4,15 +4,21 @@
 
 namespace qmc {
 
+// one CTA per SM, dynamic shared memory (the parked weights and U of 256 / 384 threads exceed the static 48 KB)
 template <int DP, bool WIDE> static cudaError_t launch_one(int grid, cudaStream_t st, const FusedLaunch& a) {
-    fused_sector_kernel<DP, SectorGroup<DP>::value, WIDE><<<grid, kThreads, 0, st>>>(a);
+    constexpr int G = SectorGroup<DP>::value, NT = SectorThreads<DP>::value;
+    constexpr size_t smem = sizeof(SectorShared<DP, G, NT>);
+    cudaError_t e = cudaFuncSetAttribute(fused_sector_kernel<DP, G, WIDE, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    fused_sector_kernel<DP, G, WIDE, NT><<<grid, NT, smem, st>>>(a);
     return cudaGetLastError();
 }
 template <int DP, bool WIDE> static int occ_one() {
+    constexpr int G = SectorGroup<DP>::value, NT = SectorThreads<DP>::value;
+    constexpr size_t smem = sizeof(SectorShared<DP, G, NT>);
     int nb = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fused_sector_kernel<DP, SectorGroup<DP>::value, WIDE>, kThreads, 0) !=
-        cudaSuccess)
-        return -1;
+    if (cudaFuncSetAttribute(fused_sector_kernel<DP, G, WIDE, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, fused_sector_kernel<DP, G, WIDE, NT>, NT, smem) != cudaSuccess) return -1;
     return nb;
 }
 
@@ -36,6 +42,5 @@ int occupancy_fused_f3(int dp, bool wide) {
     QMC_F3_TABLE(occ_one)
     return -1;
 }
-int group_fused_f3(int dp) { return dp <= 8 ? SectorGroup<8>::value : SectorGroup<16>::value; }
 
 }  // namespace qmc

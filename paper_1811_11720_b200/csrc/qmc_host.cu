@@ -195,7 +195,7 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
         if (p.family == QMC_FAMILY_SECTOR) {
             const int nmono = (p.n_params - 4 - p.dim) / (1 + p.dim);
             d.aux_off = (int)prog_off;
-            d.aux_len = sector_coef_slots(nmono) + 2 * nmono + 1;       // coefs + 16 one-byte steps per monomial + end-of-U / padding
+            d.aux_len = sector_slot_words(nmono) + 2 * nmono + 1;       // coefficient slots + 16 one-byte steps per monomial + end steps / padding
             prog_off += (size_t)d.aux_len;
         }
         d.means_off = means_off;
@@ -219,6 +219,7 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
     // in proportion to their cost; a tile is at least one index per thread and at most kMaxSteps (bounds the fp64 chains)
     for (auto& v : plan->variants) {
         const int resident = kPlanSMs * (v.family == QMC_FAMILY_SECTOR ? min_blocks_sector(v.dp) : min_blocks_closed(v.dp, v.wide));
+        const int threads = v.family == QMC_FAMILY_SECTOR ? sector_threads(v.dp) : kThreads;   // CTA size of the variant's kernel
         const int env = tiles_target();
         // one problem: equal tiles, 2 per resident CTA (the queue evens out SM speed differences over a long kernel) -- or
         // exactly 1 when the whole kernel is short (< kShortEvalsPerCta evaluations per CTA: per-tile overhead and the
@@ -236,11 +237,11 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
             const double cost = (double)d.n * d.m * (12.0 * d.dim + 0.5 * d.n_params + 40.0);
             const double want = std::max(1.0, std::floor(target * cost / total_cost));
             unsigned long long tile_len = (unsigned long long)std::ceil((double)d.n / want);
-            tile_len = std::min<unsigned long long>(std::max<unsigned long long>(tile_len, kThreads), (unsigned long long)kMaxSteps * kThreads);
+            tile_len = std::min<unsigned long long>(std::max<unsigned long long>(tile_len, threads), (unsigned long long)kMaxSteps * threads);
             const unsigned long long tiles = (d.n + tile_len - 1) / tile_len;
             if (tiles > 0x7fffffffull) return QMC_ERR_N;
             d.tile_len = (long long)tile_len;
-            d.steps = (int)((tile_len + kThreads - 1) / kThreads);
+            d.steps = (int)((tile_len + threads - 1) / threads);
             d.tiles = (int)tiles;
         }
     }

@@ -21,12 +21,16 @@ constexpr int kWavesBatch = 8;         // ... and when it serves a batch of uneq
 // resident CTAs per SM each fused kernel is register-budgeted for (its __launch_bounds__ minimum)
 constexpr int min_blocks_closed(int dp, bool wide) { return (dp <= 8 || (dp <= 12 && !wide)) ? 4 : (dp <= 16 ? (wide ? 2 : 3) : 2); }
 constexpr int sector_group(int dp) { return dp <= 8 ? 8 : 4; }                       // shifts per group, sector family
-constexpr int min_blocks_sector(int dp) { return dp <= 6 ? 3 : 2; }
+// The sector kernels run ONE CTA per SM, as large as the registers allow (x[G][DP] lives in registers): every warp of an SM then
+// interprets the same program, whose cases stay in the L0 instruction cache.
+__host__ __device__ constexpr int sector_threads(int dp) { return dp <= 6 ? 384 : 256; }
+constexpr int min_blocks_sector(int) { return 1; }
 constexpr int kDeltaCache = 768;       // doubles of shared memory per CTA that cache the shifts of all groups of a problem
-constexpr int kMaxSectorOps = 1024;    // interpreter program length limit per polynomial
-constexpr int kMaxSectorMono = 64;
-constexpr int kSectorLinSlots = 32;    // extra coefficient slots of a sector program: one dense linear form (<= 16 entries) per polynomial
-__host__ __device__ constexpr int sector_coef_slots(int nmono) { return nmono + kSectorLinSlots; }   // coefficient region of a program, in doubles
+constexpr int kMaxSectorMono = 64;     // monomials per polynomial
+constexpr int kMaxSectorOps = 2 * kMaxSectorMono * 16 + 64;   // step bytes of a program: <= one per unit of degree (<= 16 per monomial) + end steps, padding
+// coefficient region of a program in 8-byte words: one 16-byte slot {cf, cf2} per non-constant monomial, one for the end of U,
+// one of read-ahead
+__host__ __device__ constexpr int sector_slot_words(int nmono) { return 2 * (nmono + 2); }
 
 // kernel family of a public family id: the four remaining Genz functions share one fused kernel (runtime sub-kind)
 constexpr int kKernelFamilyGenzMisc = 4;

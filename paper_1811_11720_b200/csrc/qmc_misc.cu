@@ -17,7 +17,7 @@ __global__ void __launch_bounds__(32) prepare_kernel(const DevProblem* __restric
     DevAux& a = aux[blockIdx.x];
     const int j = threadIdx.x;
     if (j < QMC_MAX_DIM) {
-        const SlotConst s = derive_slot(pb, j);
+        const SlotConst s = derive_slot(pb, j, sector_threads(sector_dim_slots(pb.dim)));
         a.z[j] = s.z; a.step[j] = s.step; a.back[j] = s.back; a.fam_a[j] = s.fa; a.fam_b[j] = s.fb;
 #pragma unroll
         for (int i = 0; i < 9; ++i) a.fit[i][j] = s.f[i];

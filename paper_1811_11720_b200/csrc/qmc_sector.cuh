@@ -4,73 +4,202 @@
 //
 // A C ABI cannot carry compiled functors (the paper compiles every sector with nvcc),
 // so the parameter block is compiled ON THE DEVICE (prepare_sector) into a tiny straight-line
-// program that the fused kernel interprets with warp-uniform control flow.  One program step is
-// one fp64 instruction per point:
-//     step = one byte: 4 + 4*(variable j) + 2*FIRST + LAST     (0 = no-op, 1 = end of U, 2 = end of program)
-//     FIRST & LAST : sum  = fma(coef, x_j, sum)        (degree-1 monomial; coef = next coefficient)
-//     FIRST        : mon  = coef * x_j
-//     LAST         : sum  = fma(mon, x_j, sum)
-//     otherwise    : mon *= x_j
-// so a polynomial costs sum_t deg(t) fp64 instructions per point, with no separate additions.
-// Steps are dispatched by one indexed branch each (PTX brx.idx, threaded code: every case fetches
-// the next step and the next coefficient before its own fp64 work); the decode cost of a step is
-// shared by the G points a thread evaluates together, which is why this family runs G = 8 shifts
-// per lattice index where the registers allow it.  U and F are one instruction stream (the
-// end-of-U step parks the sum and restarts it with F's constant).
+// program that the fused kernel interprets with warp-uniform control flow.  The target machine has
+// two accumulators per point, S (the polynomial) and A (the current group), and five step kinds of
+// one fp64 instruction per point each (gen_sector_interp.py):
+//     SC j : S = fma(A, x_j, S)        SL j : S = fma(cf, x_j, S)       AL j : A = fma(cf, x_j, A)
+//     ALI j: A = fma(cf, x_j, cf2)     AM j : A = A * x_j
+// A polynomial is compiled into a greedy multivariate Horner form: the variable that occurs in most
+// monomials is factored out, recursively, which yields groups  x^P (own + sum_k c_k x_k)  sharing
+// the prefix monomial x^P:
+//     ALI k_0 (cf = c_k0, cf2 = own), AL k_i ..., AM p_1 ... AM p_(D-1), SC p_D        D = deg P
+// (a monomial nobody shares a prefix with is ALI, AM ..., SC: deg steps; degree 1: SL).  On the 256 seeded
+// sectors of configs[3] this is 30.6 steps per point for U and F together where the monomial-by-monomial
+// evaluation of round 1 took 44.4 (48.0 with its dense linear forms).
+// Steps are dispatched by one indexed branch each (PTX brx.idx, threaded code); the decode cost of
+// a step is shared by the G points a thread evaluates together, and the CTA is as large as the SM
+// holds (one CTA per SM) so that every warp of an SM runs the same program: the cases a program
+// touches must stay in the 6 KB L0 instruction cache.
 #pragma once
 #include "qmc_fused.cuh"
 
 namespace qmc {
 
-constexpr int kSecMaxCoef = 192;     // coefficient stream of a program: non-constant monomials of U and F + two dense linear forms
+constexpr int kSecMaxSlots = sector_slot_words(2 * kMaxSectorMono) / 2;   // 16-byte coefficient slots of a program: one per monomial + end-of-polynomial + read-ahead
 constexpr int kSecMaxWords = kMaxSectorOps / 4;
+constexpr int kSecKinds = 5;
+constexpr int kSecParkRows = 16;                       // rows of G... doubles per thread parked in shared memory: weights [0, 8), U [8, 16)
 
-// step codes (one byte each): 0 = no-op, 1 = end of U, 2 = end of program, 3 = dense linear form (sum += sum_j c_j x_j over
-// all DP slots, DP coefficients from the stream: the degree-1 monomials of a polynomial in ONE step), 4 + 4*j + 2*FIRST + LAST
-enum : int { SEC_NOP = 0, SEC_ENDU = 1, SEC_END = 2, SEC_LIN = 3, SEC_BASE = 4 };
+// step codes (one byte each): 0 = no-op, 1 = end of a polynomial that is not the last, 2 = end of program, 3 + 5 j + kind
+enum : int { SEC_NOP = 0, SEC_ENDP = 1, SEC_END = 2, SEC_BASE = 3 };
+enum : int { SEC_SC = 0, SEC_SL = 1, SEC_AL = 2, SEC_ALI = 3, SEC_AM = 4 };
 
-struct alignas(16) SectorSmem {
-    double coefs[kSecMaxCoef];       // coefficients of the non-constant monomials, in step order
-    unsigned int words[kSecMaxWords];// step bytes: U's steps, SEC_ENDU, F's steps, SEC_END (copied word-wise)
-    double c0[2];                    // constant terms of U and F
+template <int NT> struct alignas(16) SectorSmem {
+    double slots[kSecMaxSlots * 2];  // {cf, cf2} per coefficient-consuming step, in program order
+    unsigned int words[kSecMaxWords];// step bytes: U's steps, SEC_ENDP, F's steps, SEC_END (copied word-wise)
+    double c0u;                      // constant term of U (F's travels in the slot of the end-of-polynomial step)
     unsigned long long nu_packed;    // nu_j in 4 bits each
     int a, b;                        // powers of U and F
     double lg[2];                    // lu, lf of the log factor
     int logp, pad_;                  // its power p (0 = no log factor)
-    double wpark[16 * kThreads];     // [q][thread]: the G weights of a thread, parked while the interpreter runs (registers);
-                                     // with a log factor afterwards U in [0, 8), F in [8, 16) for sector_log_factors
+    double park[kSecParkRows * NT];  // [row][thread]: rows [0, 8) the G weights of a thread while the interpreter runs (with a log
+                                     // factor afterwards F), rows [8, 16) U as the interpreter parks it
 };
 struct SectorOff {                   // byte offsets of the fields above (read with ld.shared in the inner loop)
-    static constexpr unsigned coefs = 0, words = kSecMaxCoef * 8, c0 = words + kSecMaxWords * 4, nu = c0 + 16, ab = nu + 8, lg = ab + 8, logp = lg + 16, wpark = logp + 8;
+    static constexpr unsigned slots = 0, words = kSecMaxSlots * 16, c0u = words + kSecMaxWords * 4, nu = c0u + 8, ab = nu + 8, lg = ab + 8,
+                              logp = lg + 16, park = logp + 8;
+};
+#define QMC_SECTOR_OFF_CHECK(NT)                                                                                                      \
+    static_assert(offsetof(SectorSmem<NT>, words) == SectorOff::words && offsetof(SectorSmem<NT>, c0u) == SectorOff::c0u &&           \
+                  offsetof(SectorSmem<NT>, nu_packed) == SectorOff::nu && offsetof(SectorSmem<NT>, a) == SectorOff::ab &&             \
+                  offsetof(SectorSmem<NT>, lg) == SectorOff::lg && offsetof(SectorSmem<NT>, logp) == SectorOff::logp &&               \
+                  offsetof(SectorSmem<NT>, park) == SectorOff::park, "SectorOff must mirror SectorSmem");
+QMC_SECTOR_OFF_CHECK(256) QMC_SECTOR_OFF_CHECK(384)
+#undef QMC_SECTOR_OFF_CHECK
+
+__host__ __device__ inline int sector_dim_slots(int dim) { return dim <= 4 ? 4 : (dim <= 6 ? 6 : (dim <= 8 ? 8 : (dim <= 16 ? 16 : -1))); }
+
+// ---- device-side compiler: params -> program (one thread per problem; runs once per call) ---------------------------
+// Program area of a problem (8-byte words at prog_area + aux_off): sector_slot_words(nmono) words of coefficient slots,
+// then the step bytes.  DevAux: sec_nops[0] = number of 32-bit step words, sec_ncoef[0] = number of slots.
+struct SecEmit {                     // output cursor of the compiler
+    double* slots;
+    unsigned char* ops;
+    int nslots, nops, max_slots, max_ops, status;
+    __device__ void op(int kind, int j) {
+        if (nops >= max_ops) { status = QMC_ERR_PARAMS; return; }
+        ops[nops++] = (unsigned char)(SEC_BASE + kSecKinds * j + kind);
+    }
+    __device__ void slot(double cf, double cf2) {
+        if (nslots >= max_slots) { status = QMC_ERR_PARAMS; return; }
+        slots[2 * nslots] = cf; slots[2 * nslots + 1] = cf2; ++nslots;
+    }
 };
 
-static_assert(offsetof(SectorSmem, words) == SectorOff::words && offsetof(SectorSmem, c0) == SectorOff::c0 &&
-              offsetof(SectorSmem, nu_packed) == SectorOff::nu && offsetof(SectorSmem, a) == SectorOff::ab &&
-              offsetof(SectorSmem, lg) == SectorOff::lg && offsetof(SectorSmem, logp) == SectorOff::logp &&
-              offsetof(SectorSmem, wpark) == SectorOff::wpark, "SectorOff must mirror SectorSmem");
-
-// ---- device-side compiler: params -> program (one thread; a few hundred steps at most) ---------
-// program area of a problem (8-byte words at prog_area + aux_off): coefs[nU + nF] (upper bound),
-// then the step bytes.  DevAux: sec_nops[0] = number of 32-bit step words, sec_ncoef[0] = number
-// of coefficients.
-__host__ __device__ inline int sector_dim_slots(int dim) { return dim <= 4 ? 4 : (dim <= 6 ? 6 : (dim <= 8 ? 8 : (dim <= 16 ? 16 : -1))); }
+// One polynomial: `cnt` monomials, coefficients c[t], exponents e[t*d + j] (validated by the caller: integers 0..8, degree <= 16).
+// Greedy Horner form.  A work item is a set of monomials (a range of idx[]) that share the prefix monomial they were reached
+// by; rem[t][j] are the exponents still to be factored out, left[t] their sum.  From an item the variable that occurs in most of
+// its monomials is factored out: the monomials that contain it form a child (processed as an item of its own unless it is a
+// single finished monomial, a "leaf"), the others stay.  When the item is used up its group is emitted: prefix, the coefficient
+// of the prefix monomial itself (own) and the leaves.  Returns the constant term.
+__device__ inline double compile_polynomial(const double* c, const double* e, int cnt, int d, SecEmit& out) {
+    unsigned char rem[kMaxSectorMono][16];
+    unsigned char left[kMaxSectorMono];
+    short idx[kMaxSectorMono];
+    // work items: ranges of idx with the prefix they share (exponents) and the coefficient of the prefix monomial; items on the
+    // stack are disjoint ranges with at least one unfinished monomial each, so there are never more than cnt of them
+    short it_b[kMaxSectorMono + 1], it_e[kMaxSectorMono + 1];
+    double it_own[kMaxSectorMono + 1];
+    unsigned char it_prefix[kMaxSectorMono + 1][16];
+    double c0 = 0.0;
+    int m = 0;
+    for (int t = 0; t < cnt; ++t) {
+        int deg = 0;
+        for (int j = 0; j < d; ++j) { const int v = (int)e[t * d + j]; rem[t][j] = (unsigned char)v; deg += v; }
+        for (int j = d; j < 16; ++j) rem[t][j] = 0;
+        left[t] = (unsigned char)deg;
+        if (deg == 0) c0 += c[t]; else idx[m++] = (short)t;
+    }
+    int top = 0;
+    it_b[0] = 0; it_e[0] = (short)m; it_own[0] = 0.0;
+    for (int j = 0; j < 16; ++j) it_prefix[0][j] = 0;
+    top = 1;
+    bool root = true;
+    while (top > 0) {
+        --top;
+        const int b = it_b[top], en = it_e[top];
+        const double own = it_own[top];
+        unsigned char prefix[16];
+        int pdeg = 0;
+        for (int j = 0; j < 16; ++j) { prefix[j] = it_prefix[top][j]; pdeg += prefix[j]; }
+        const bool is_root = root;
+        root = false;
+        double leaf_c[16];
+        int leaf_mask = 0;
+        int cur = b;
+        while (cur < en) {
+            // the variable that occurs in most of the remaining monomials (lowest index on ties)
+            int best = 0, best_cnt = -1;
+            for (int j = 0; j < d; ++j) {
+                int n = 0;
+                for (int i = cur; i < en; ++i) n += rem[idx[i]][j] > 0;
+                if (n > best_cnt) { best_cnt = n; best = j; }
+            }
+            // partition: monomials containing x_best to the front, the finished ones among them first
+            int mid = cur;
+            for (int i = cur; i < en; ++i)
+                if (rem[idx[i]][best] > 0) { const short t = idx[i]; idx[i] = idx[mid]; idx[mid] = t; ++mid; }
+            double child_own = 0.0;
+            int fin = cur;
+            for (int i = cur; i < mid; ++i) {
+                const short t = idx[i];
+                --rem[t][best]; --left[t];
+                if (left[t] == 0) { child_own += c[t]; idx[i] = idx[fin]; idx[fin] = t; ++fin; }
+            }
+            if (fin == mid) {                                  // nothing below: a leaf of this item
+                leaf_c[best] = (leaf_mask >> best & 1) ? leaf_c[best] + child_own : child_own;
+                leaf_mask |= 1 << best;
+            } else {                                           // a child item: prefix * x_best
+                it_b[top] = (short)fin; it_e[top] = (short)mid; it_own[top] = child_own;
+                for (int j = 0; j < 16; ++j) it_prefix[top][j] = prefix[j];
+                ++it_prefix[top][best];
+                ++top;
+            }
+            cur = mid;
+        }
+        // emit the group of this item
+        if (is_root) {
+            for (int k = 0; k < d; ++k)
+                if (leaf_mask >> k & 1) { out.op(SEC_SL, k); out.slot(leaf_c[k], 0.0); }
+            continue;
+        }
+        int last = 0;
+        for (int j = 0; j < d; ++j) if (prefix[j]) last = j;
+        if (leaf_mask) {
+            bool first = true;
+            for (int k = 0; k < d; ++k)
+                if (leaf_mask >> k & 1) {
+                    out.op(first ? SEC_ALI : SEC_AL, k);
+                    out.slot(leaf_c[k], first ? own : 0.0);
+                    first = false;
+                }
+            for (int j = 0; j < d; ++j)
+                for (int r = 0; r < prefix[j] - (j == last ? 1 : 0); ++r) out.op(SEC_AM, j);
+            out.op(SEC_SC, last);
+        } else if (own != 0.0) {
+            if (pdeg == 1) { out.op(SEC_SL, last); out.slot(own, 0.0); }
+            else {
+                int firstv = 0;
+                for (int j = d - 1; j >= 0; --j) if (prefix[j]) firstv = j;
+                out.op(SEC_ALI, firstv); out.slot(own, 0.0);
+                for (int j = 0; j < d; ++j) {
+                    const int reps = prefix[j] - (j == firstv ? 1 : 0) - (j == last ? 1 : 0);
+                    for (int r = 0; r < reps; ++r) out.op(SEC_AM, j);
+                }
+                out.op(SEC_SC, last);
+            }
+        }
+    }
+    return c0;
+}
 
 __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned long long* prog_area) {
     if (threadIdx.x != 0) return;
     const int d = pb.dim;
-    const int dp = sector_dim_slots(d);
     const double* p = pb.params;
-    int status = 0;
+    const int nmono_total = (pb.n_params - 4 - d) / (1 + d);
+    double* slots = reinterpret_cast<double*>(prog_area + pb.aux_off);
+    unsigned char* ops = reinterpret_cast<unsigned char*>(prog_area + pb.aux_off + sector_slot_words(nmono_total));
     // A rejected parameter block must still leave a program the interpreter can run to its end (the problem's
     // results are then replaced by NaN in the finalize stage): end-of-U, end, read-ahead padding.
-    {
-        const int slots = sector_coef_slots((pb.n_params - 4 - d) / (1 + d));
-        unsigned char* stub = reinterpret_cast<unsigned char*>(prog_area + pb.aux_off + slots);
-        stub[0] = (unsigned char)SEC_ENDU; stub[1] = (unsigned char)SEC_END;
-        for (int i = 2; i < 8; ++i) stub[i] = (unsigned char)SEC_NOP;
-        a.sec_nops[0] = 2; a.sec_nops[1] = 0; a.sec_ncoef[0] = 0; a.sec_ncoef[1] = 0;
+    auto stub = [&]() {
+        ops[0] = (unsigned char)SEC_ENDP; ops[1] = (unsigned char)SEC_END;
+        for (int i = 2; i < 8; ++i) ops[i] = (unsigned char)SEC_NOP;
+        slots[0] = 1.0; slots[1] = 0.0;
+        a.sec_nops[0] = 2; a.sec_nops[1] = 0; a.sec_ncoef[0] = 1; a.sec_ncoef[1] = 0;
         a.sec_c0[0] = a.sec_c0[1] = 1.0;
-    }
+    };
+    stub();
     const double av = p[0], bv = p[1], nUv = p[2], nFv = p[3];
     if (!(av >= 0.0 && av <= 8.0 && bv >= 0.0 && bv <= 8.0 && nUv >= 1.0 && nUv <= kMaxSectorMono && nFv >= 1.0 &&
           nFv <= kMaxSectorMono) ||
@@ -86,75 +215,53 @@ __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned 
         a.sec_log[0] = p[n_base]; a.sec_log[1] = p[n_base + 1]; a.sec_logp = (int)pw;
     } else if (pb.n_params != n_base) { a.status = QMC_ERR_PARAMS; return; }
     a.sec_a = (int)av; a.sec_b = (int)bv;
+    int status = 0;
     for (int j = 0; j < d; ++j) {
         const double v = p[4 + j];
         if (!(v >= 0.0 && v <= 8.0) || v != floor(v)) status = QMC_ERR_PARAMS;
         a.nu[j] = (unsigned char)(int)v;
     }
-    double* coefs = reinterpret_cast<double*>(prog_area + pb.aux_off);
-    const int max_coef = sector_coef_slots((pb.n_params - 4 - d) / (1 + d));   // the same upper bound as the host plan and the kernel
-    unsigned char* ops = reinterpret_cast<unsigned char*>(prog_area + pb.aux_off + max_coef);
-    const int max_ops = min((pb.aux_len - max_coef) * 8, kMaxSectorOps) - 8;   // room for SEC_ENDU, SEC_END and 3+ bytes of read-ahead padding
-    int nops = 0, ncoef = 0;
-    const double* base = p + 4 + d;
-    for (int pol = 0; pol < 2; ++pol) {
-        const double* c = base;
-        const double* e = base + cnt[pol];
-        double c0 = 0.0;
-        // the degree-1 monomials of the polynomial become one dense linear-form step when there are at least two
-        int nlin = 0;
-        for (int t = 0; t < cnt[pol]; ++t) {
-            int deg = 0;
-            for (int j = 0; j < d; ++j) deg += (int)e[t * d + j];
-            nlin += (deg == 1);
-        }
-        const bool lin = nlin >= 2 && ncoef + dp < kSecMaxCoef - 1 && nops + 1 <= max_ops;
-        if (lin) {
-            for (int j = 0; j < dp; ++j) coefs[ncoef + j] = 0.0;
+    // exponents: integers 0..8, total degree of a monomial <= 16 (include/qmc_lattice.h)
+    {
+        const double* base = p + 4 + d;
+        for (int pol = 0; pol < 2 && !status; ++pol) {
+            const double* e = base + cnt[pol];
             for (int t = 0; t < cnt[pol]; ++t) {
-                int deg = 0, var = 0;
-                for (int j = 0; j < d; ++j) { const int ej = (int)e[t * d + j]; deg += ej; if (ej) var = j; }
-                if (deg == 1) coefs[ncoef + var] += c[t];
-            }
-            ncoef += dp;
-            ops[nops++] = (unsigned char)SEC_LIN;
-        }
-        for (int t = 0; t < cnt[pol]; ++t) {
-            int deg = 0;
-            for (int j = 0; j < d; ++j) {
-                const double v = e[t * d + j];
-                if (!(v >= 0.0 && v <= 8.0) || v != floor(v)) { status = QMC_ERR_PARAMS; continue; }
-                deg += (int)v;
-            }
-            if (deg > 16 || status) { status = QMC_ERR_PARAMS; continue; }
-            if (deg == 0) { c0 += c[t]; continue; }
-            if (deg == 1 && lin) continue;
-            if (ncoef >= kSecMaxCoef - 1 || nops + deg > max_ops) { status = QMC_ERR_PARAMS; continue; }
-            coefs[ncoef++] = c[t];
-            int seen = 0;
-            for (int j = 0; j < d; ++j) {
-                const int ej = (int)e[t * d + j];
-                for (int r = 0; r < ej; ++r) {
-                    const int first = (seen == 0), last = (seen == deg - 1);
-                    ops[nops++] = (unsigned char)(SEC_BASE + j * 4 + first * 2 + last);
-                    ++seen;
+                int deg = 0;
+                for (int j = 0; j < d; ++j) {
+                    const double v = e[t * d + j];
+                    if (!(v >= 0.0 && v <= 8.0) || v != floor(v)) { status = QMC_ERR_PARAMS; break; }
+                    deg += (int)v;
                 }
+                if (deg > 16) status = QMC_ERR_PARAMS;
             }
+            base += cnt[pol] * (1 + d);
         }
-        a.sec_c0[pol] = c0;
-        if (!status) ops[nops++] = (unsigned char)(pol == 0 ? SEC_ENDU : SEC_END);
-        base += cnt[pol] * (1 + d);
     }
-    if (!status) while (nops & 3) ops[nops++] = (unsigned char)SEC_NOP;
-    if (!status) {
-        a.sec_nops[0] = nops / 4;
-        a.sec_ncoef[0] = ncoef;
-    } else {                                           // restore the stub (the loop above may have overwritten it)
-        ops[0] = (unsigned char)SEC_ENDU; ops[1] = (unsigned char)SEC_END;
-        for (int i = 2; i < 8; ++i) ops[i] = (unsigned char)SEC_NOP;
-        a.sec_c0[0] = a.sec_c0[1] = 1.0;
-    }
-    a.status = status;
+    if (status) { a.status = status; return; }
+    SecEmit out;
+    out.slots = slots; out.ops = ops; out.nslots = 0; out.nops = 0; out.status = 0;
+    out.max_slots = sector_slot_words(nmono_total) / 2 - 1;                              // one slot of read-ahead
+    out.max_ops = min((pb.aux_len - sector_slot_words(nmono_total)) * 8, kMaxSectorOps) - 8;   // room for the two end steps and the read-ahead padding
+    const double* base = p + 4 + d;
+    const double c0u = compile_polynomial(base, base + cnt[0], cnt[0], d, out);
+    base += cnt[0] * (1 + d);
+    // end of U: its step takes F's constant term from the slot stream -- the slot is filled after F is compiled
+    const int endp_slot = out.nslots;
+    out.ops[out.nops++] = (unsigned char)SEC_ENDP;          // max_ops keeps room for the end steps
+    out.slot(0.0, 0.0);
+    const double c0f = compile_polynomial(base, base + cnt[1], cnt[1], d, out);
+    if (out.status) { stub(); a.status = out.status; return; }
+    slots[2 * endp_slot] = c0f;
+    out.ops[out.nops++] = (unsigned char)SEC_END;
+    out.ops[out.nops++] = (unsigned char)SEC_NOP;       // the interpreter reads two step codes ahead
+    out.ops[out.nops++] = (unsigned char)SEC_NOP;
+    while (out.nops & 3) out.ops[out.nops++] = (unsigned char)SEC_NOP;
+    slots[2 * out.nslots] = 0.0; slots[2 * out.nslots + 1] = 0.0;                          // read-ahead slot
+    a.sec_c0[0] = c0u; a.sec_c0[1] = c0f;
+    a.sec_nops[0] = out.nops / 4;
+    a.sec_ncoef[0] = out.nslots + 1;
+    a.status = 0;
 }
 
 // ---- interpreter: U and F for G points (threaded code in inline PTX, see gen_sector_interp.py) ------
@@ -219,14 +326,15 @@ static __device__ __forceinline__ double log_normal_positive(double x) {
     return __fma_rn(ed, kLogC[12], __fma_rn(ed, kLogC[13], lm));   // log 2 = hi + lo
 }
 
-// Once per lattice index: the caller parks U[q] at park + 8 kThreads q and F[q] at park + 8 kThreads (8 + q) (its own
-// column of SectorSmem::wpark) and reads the factors back from the U slots.
+// Once per lattice index: F[q] sits in park row q and U[q] in row 8 + q (the thread's own column of SectorSmem::park);
+// the factors are written over the F rows.
+template <int NT>
 static __device__ __forceinline__ void sector_log_factors(unsigned park, int g, double lu, double lf, int p) {
 #pragma unroll 1
     for (int q = 0; q < g; q += 2) {                     // g is 4 or 8: two points = four independent logarithms per pass
-        const unsigned at = park + 8u * kThreads * q;
-        const double U0 = lds_f64(at), F0 = lds_f64(at + 64u * kThreads);
-        const double U1 = lds_f64(at + 8u * kThreads), F1 = lds_f64(at + 72u * kThreads);
+        const unsigned at = park + 8u * NT * q;
+        const double F0 = lds_f64(at), U0 = lds_f64(at + 64u * NT);
+        const double F1 = lds_f64(at + 8u * NT), U1 = lds_f64(at + 72u * NT);
         double a0 = log_normal_positive(U0), b0 = log_normal_positive(F0), a1 = log_normal_positive(U1), b1 = log_normal_positive(F1);
         if (!(log_arg_is_normal_positive(U0) && log_arg_is_normal_positive(F0) && log_arg_is_normal_positive(U1) &&
               log_arg_is_normal_positive(F1))) {
@@ -236,7 +344,7 @@ static __device__ __forceinline__ void sector_log_factors(unsigned park, int g, 
         double r0 = L0, r1 = L1;
         for (int e = 1; e < p; ++e) { r0 = __dmul_rn(r0, L0); r1 = __dmul_rn(r1, L1); }
         sts_f64(at, r0);
-        sts_f64(at + 8u * kThreads, r1);
+        sts_f64(at + 8u * NT, r1);
     }
 }
 
@@ -244,10 +352,10 @@ static __device__ __forceinline__ void sector_log_factors(unsigned park, int g, 
 // tile loop.  SLOW = false: Korobov-3 without fit map, the paper's default for loop integrals, as the only
 // inlined tile loop of the kernel (a smaller kernel body measurably helps the interpreter: DESIGN.md section 5); SLOW = true:
 // the generic coordinate block (any transform, any fit mode at run time), reached through a real call (run_tile_call).
-template <int DP, int G, bool WIDE, bool SLOW> struct SectorEval {
+template <int DP, int G, bool WIDE, bool SLOW, int NT> struct SectorEval {
     static constexpr int NC = 1;
     typedef unsigned Extra;                                  // shared address of the CTA's SectorSmem
-    static __device__ __forceinline__ void eval(const typename Res<WIDE>::T (&r)[DP], const SmemCtx<DP, G>&, const unsigned& exbase,
+    static __device__ __forceinline__ void eval(const typename Res<WIDE>::T (&r)[DP], const SmemCtx<DP, G, NT>&, const unsigned& exbase,
                                                 const EvalCtx& cx, double (&acc)[G][1]) {
         double x[G][DP], num[G];
         if (!SLOW) {
@@ -255,18 +363,19 @@ template <int DP, int G, bool WIDE, bool SLOW> struct SectorEval {
         } else {
             sector_coords<DP, G, WIDE, TR_KORR, FIT_RT>(r, cx, x, num);
         }
-        // the weights are not needed until the interpreter is done: park them in shared memory ([q][thread], conflict free)
-        const unsigned park = exbase + SectorOff::wpark + 8u * threadIdx.x;
+        // the weights are not needed until the interpreter is done: park them in shared memory ([row][thread], conflict free)
+        const unsigned park = exbase + SectorOff::park + 8u * threadIdx.x;
 #pragma unroll
-        for (int q = 0; q < G; ++q) sts_f64(park + 8u * kThreads * q, num[q]);
-        double c0u, c0f;
-        lds_f64x2(exbase + SectorOff::c0, c0u, c0f);
-        double U[G], F[G];
+        for (int q = 0; q < G; ++q) sts_f64(park + 8u * NT * q, num[q]);
+        double F[G];
+        {
+            const double c0u = lds_f64(exbase + SectorOff::c0u);
 #pragma unroll
-        for (int q = 0; q < G; ++q) { U[q] = 0.0; F[q] = c0u; }
-        sector_interp<DP, G>(x, exbase + SectorOff::words, exbase + SectorOff::coefs, c0f, U, F);
+            for (int q = 0; q < G; ++q) F[q] = c0u;
+        }
+        sector_interp<DP, G, NT>(x, exbase + SectorOff::words, exbase + SectorOff::slots, park + 64u * NT, F);   // U -> rows 8 ..
 #pragma unroll
-        for (int q = 0; q < G; ++q) num[q] = lds_f64(park + 8u * kThreads * q);
+        for (int q = 0; q < G; ++q) num[q] = lds_f64(park + 8u * NT * q);
         // num = W prod_j x_j^nu_j U^a, den = F^b   (small integer powers by repeated multiplication)
         const unsigned long long nup = lds_u64(exbase + SectorOff::nu);
         const unsigned long long ab = lds_u64(exbase + SectorOff::ab);
@@ -284,18 +393,23 @@ template <int DP, int G, bool WIDE, bool SLOW> struct SectorEval {
         if (lp) {
             const double lu = lds_f64(exbase + SectorOff::lg), lf = lds_f64(exbase + SectorOff::lg + 8u);
 #pragma unroll
-            for (int q = 0; q < G; ++q) { sts_f64(park + 8u * kThreads * q, U[q]); sts_f64(park + 8u * kThreads * (8 + q), F[q]); }
-            sector_log_factors(park, G, lu, lf, lp);
+            for (int q = 0; q < G; ++q) sts_f64(park + 8u * NT * q, F[q]);
+            sector_log_factors<NT>(park, G, lu, lf, lp);
 #pragma unroll
-            for (int q = 0; q < G; ++q) num[q] *= lds_f64(park + 8u * kThreads * q);
+            for (int q = 0; q < G; ++q) num[q] *= lds_f64(park + 8u * NT * q);
         }
         double den[G];
 #pragma unroll
         for (int q = 0; q < G; ++q) den[q] = 1.0;
-#pragma unroll 1
-        for (int e = 0; e < pa; ++e)
+        if (pa) {
+            double U[G];
 #pragma unroll
-            for (int q = 0; q < G; ++q) num[q] *= U[q];
+            for (int q = 0; q < G; ++q) U[q] = lds_f64(park + 8u * NT * (8 + q));
+#pragma unroll 1
+            for (int e = 0; e < pa; ++e)
+#pragma unroll
+                for (int q = 0; q < G; ++q) num[q] *= U[q];
+        }
 #pragma unroll 1
         for (int e = 0; e < pb; ++e)
 #pragma unroll
@@ -305,34 +419,41 @@ template <int DP, int G, bool WIDE, bool SLOW> struct SectorEval {
     }
 };
 
-// shifts per group and resident CTAs per SM by dimension-slot count (x[G][DP] lives in registers)
+// shifts per group and threads per CTA by dimension-slot count (x[G][DP] lives in registers; one CTA per SM)
 template <int DP> struct SectorGroup { static constexpr int value = sector_group(DP); };
-template <int DP, int G> struct SectorMinBlocks { static constexpr int value = min_blocks_sector(DP); };
+template <int DP> struct SectorThreads { static constexpr int value = sector_threads(DP); };
 
-template <int DP, int G, bool WIDE>
-__global__ void __launch_bounds__(kThreads, SectorMinBlocks<DP, G>::value) fused_sector_kernel(const __grid_constant__ FusedLaunch L) {
+template <int DP, int G, int NT> struct SectorShared {
+    SmemCtx<DP, G, NT> sm;
+    SectorSmem<NT> ex;
+};
+
+template <int DP, int G, bool WIDE, int NT>
+__global__ void __launch_bounds__(NT, 1) fused_sector_kernel(const __grid_constant__ FusedLaunch L) {
     const DevAux* __restrict__ aux = L.aux;
     const unsigned long long* __restrict__ prog_area = L.prog;
     double* __restrict__ partials = L.partials;
-    __shared__ SmemCtx<DP, G> sm;
-    __shared__ SectorSmem ex;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    SectorShared<DP, G, NT>& sh = *reinterpret_cast<SectorShared<DP, G, NT>*>(smem_raw);
+    SmemCtx<DP, G, NT>& sm = sh.sm;
+    SectorSmem<NT>& ex = sh.ex;
     const unsigned sbase = (unsigned)__cvta_generic_to_shared(&sm), exbase = (unsigned)__cvta_generic_to_shared(&ex);
     int cur = -1, iter = 0;
     long long tile_local = 0;
     bool changed;
-    while (next_tile<DP, G, true>(sm, L, cur, iter, tile_local, changed)) {
+    while (next_tile<DP, G, true, NT>(sm, L, cur, iter, tile_local, changed)) {
         if (changed) {
             const int tid = threadIdx.x;
             const DevAux& a = aux[cur];
             const DevProblem& pb = sm.prob;
-            const int ncoef = a.sec_ncoef[0], nwords = a.sec_nops[0];
-            const int max_coef = sector_coef_slots((pb.n_params - 4 - pb.dim) / (1 + pb.dim));
-            const double* coefs = reinterpret_cast<const double*>(prog_area + pb.aux_off);
-            const unsigned int* words = reinterpret_cast<const unsigned int*>(prog_area + pb.aux_off + max_coef);
-            for (int i = tid; i <= ncoef && i < kSecMaxCoef; i += kThreads) ex.coefs[i] = i < ncoef ? coefs[i] : 0.0;
-            for (int i = tid; i < nwords; i += kThreads) ex.words[i] = words[i];
+            const int nslots = a.sec_ncoef[0], nwords = a.sec_nops[0];
+            const int nmono_total = (pb.n_params - 4 - pb.dim) / (1 + pb.dim);
+            const double* slots = reinterpret_cast<const double*>(prog_area + pb.aux_off);
+            const unsigned int* words = reinterpret_cast<const unsigned int*>(prog_area + pb.aux_off + sector_slot_words(nmono_total));
+            for (int i = tid; i < 2 * nslots && i < 2 * kSecMaxSlots; i += NT) ex.slots[i] = slots[i];
+            for (int i = tid; i < nwords && i < kSecMaxWords; i += NT) ex.words[i] = words[i];
             if (tid == 32) {
-                ex.c0[0] = a.sec_c0[0]; ex.c0[1] = a.sec_c0[1];
+                ex.c0u = a.sec_c0[0];
                 ex.a = a.sec_a; ex.b = a.sec_b;
                 ex.lg[0] = a.sec_log[0]; ex.lg[1] = a.sec_log[1]; ex.logp = a.sec_logp; ex.pad_ = 0;
                 unsigned long long nup = 0;
@@ -342,8 +463,8 @@ __global__ void __launch_bounds__(kThreads, SectorMinBlocks<DP, G>::value) fused
             __syncthreads();
         }
         const bool fast = !sm.prob.has_fit && sm.prob.tr_kind == TR_KOR3;
-        if (fast) run_tile<SectorEval<DP, G, WIDE, false>, DP, G, WIDE>(sm, sbase, exbase, tile_local, changed, partials);
-        else run_tile_call<SectorEval<DP, G, WIDE, true>, DP, G, WIDE>(sm, sbase, exbase, tile_local, changed, partials);
+        if (fast) run_tile<SectorEval<DP, G, WIDE, false, NT>, DP, G, WIDE, NT>(sm, sbase, exbase, tile_local, changed, partials);
+        else run_tile_call<SectorEval<DP, G, WIDE, true, NT>, DP, G, WIDE, NT>(sm, sbase, exbase, tile_local, changed, partials);
     }
 }
 

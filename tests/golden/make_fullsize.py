@@ -6,12 +6,14 @@ of the method).  No value comes from the CUDA path.  Doubles are stored as C99 h
     python tests/golden/make_fullsize.py [2] [3] [4]        (hours of CPU time in total on 8 cores)
 
 configs[2]: all 32 per-shift means (re, im), estimate and error (Eq. 2-3).
-configs[3]: the sectors listed in SECTOR_SAMPLE (outputs the oracle can compute one by one).
+configs[3]: all 256 sectors (SECTOR_SAMPLE), one record each.
 configs[4]: projection histogram (n_fit lattice, first shift; Eq. 20, reading C-8),
             the oracle's cubic fit of it, and the 20 per-shift means with that fit map applied.
 """
+import hashlib
 import json
 import os
+import subprocess
 import sys
 import time
 
@@ -24,7 +26,7 @@ import oracle  # noqa: E402
 from paper_1811_11720_b200 import synth  # noqa: E402
 
 OUT = os.path.join(os.path.dirname(os.path.abspath(__file__)), "fullsize_oracle.json")
-SECTOR_SAMPLE = [0, 1, 17, 50, 77, 101, 128, 163, 200, 222, 254, 255]
+SECTOR_SAMPLE = list(range(256))        # every sector of configs[3] (about 25 minutes of oracle time on 8 cores)
 
 
 def hexlist(a):
@@ -47,12 +49,27 @@ def config4_problem():
     return dict(p, fit_coeffs=fit), H, fit
 
 
+def provenance():
+    """Which oracle wrote the file: sha256 of oracle/qmc_oracle.cpp and the commit it was run from (informative; the
+    binding check is tests/test_oracle_pins.py::test_fullsize_goldens_are_what_the_live_oracle_computes)."""
+    with open(os.path.join(ROOT, "oracle", "qmc_oracle.cpp"), "rb") as f:
+        sha = hashlib.sha256(f.read()).hexdigest()
+    try:
+        head = subprocess.run(["git", "-C", ROOT, "rev-parse", "HEAD"], capture_output=True, text=True, check=True).stdout.strip()
+        dirty = bool(subprocess.run(["git", "-C", ROOT, "status", "--porcelain", "--", "oracle"], capture_output=True,
+                                    text=True, check=True).stdout.strip())
+    except Exception:
+        head, dirty = "unknown", False
+    return {"oracle_sha256": sha, "git_head": head, "oracle_dirty": dirty}
+
+
 def main(argv):
     which = [int(a) for a in argv] or [2, 3, 4]
     table = {}
     if os.path.exists(OUT):
         with open(OUT) as f:
             table = json.load(f)
+    prov = table.setdefault("provenance", {})
     for c in which:
         print(f"config {c} ...", flush=True)
         if c == 3:
@@ -66,6 +83,7 @@ def main(argv):
             table["4"] = rec
         else:
             table[str(c)] = record(synth.config(c)[0])
+        prov[str(c)] = provenance()
         with open(OUT, "w") as f:
             json.dump(table, f, indent=0, sort_keys=True)
         print(f"config {c} done", flush=True)

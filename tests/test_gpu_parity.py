@@ -387,15 +387,17 @@ def test_config2_full_size_vs_stored_oracle():
     _check_full(synth.config(2)[0], g["2"])
 
 
-def test_config3_full_size_sampled_sectors():
-    """the full 256-sector batch in bench.py's launch configuration; sectors the oracle computed one by one"""
+def test_config3_full_size_all_sectors():
+    """the full 256-sector batch in bench.py's launch configuration: EVERY sector against the oracle's stored full-size record"""
     g = _golden()
     if "3" not in g:
         pytest.skip("config 3 not in golden file")
     probs = synth.config(3)
+    assert sorted(int(k) for k in g["3"]["sectors"]) == list(range(len(probs))), "the golden file must hold every sector of configs[3]"
     sms, means, errs = run_gpu(probs)
     for key, rec in g["3"]["sectors"].items():
         i = int(key)
+        assert rec["n"] == probs[i]["n"] and rec["m"] == probs[i]["m"] and rec["dim"] == probs[i]["dim"]
         sm_or, mean_or, err_or = _golden_arrays(rec, 1)
         assert_means(sms[i], sm_or, probs[i]["name"] + " (full size)")
         assert_err(errs[i, :1], err_or, sm_or, probs[i]["name"])

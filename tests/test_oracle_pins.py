@@ -538,3 +538,26 @@ def test_fit_recovers_exact_cubic():
     H2 = np.zeros((1, B)); H2[0, 0] = 1.0
     out2 = oracle.fit_cubic(H2)
     assert out2[0, 4] == 1.0 and out2[0, 5] == 0.0
+
+
+# ------------------------------------------------------------------------------------------------
+# stored full-size records (tests/golden/fullsize_oracle.json) must be what the committed oracle computes
+# ------------------------------------------------------------------------------------------------
+def test_fullsize_goldens_are_what_the_live_oracle_computes():
+    """Recomputes one stored record (sector 17 of configs[3] at full size, a few seconds of oracle time) with the live
+    oracle and requires BIT identity, so that a golden file that lags an oracle change cannot go unnoticed (a stored mean
+    is a whole-lattice sum: a cheaper partial check does not exist)."""
+    import json
+    path = os.path.join(GOLD, "fullsize_oracle.json")
+    with open(path) as f:
+        g = json.load(f)
+    assert sorted(int(k) for k in g["3"]["sectors"]) == list(range(256))
+    for key in ("2", "3", "4"):
+        assert len(g["provenance"][key]["oracle_sha256"]) == 64          # which oracle source wrote the record
+    rec = g["3"]["sectors"]["17"]
+    p = synth.config(3)[17]
+    assert rec["n"] == p["n"] and rec["m"] == p["m"] and rec["dim"] == p["dim"] and rec["name"] == p["name"]
+    sm, mean, err = oracle.integrate(p)
+    assert [float(v).hex() for v in np.asarray(sm).ravel()] == rec["shift_means"]
+    assert [float(v).hex() for v in np.asarray(mean).ravel()] == rec["mean"]
+    assert [float(v).hex() for v in np.asarray(err).ravel()] == rec["err"]
