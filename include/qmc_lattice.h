@@ -15,8 +15,12 @@
  * Conventions
  *  - every function returns a qmc_status (0 = OK, negative = error); on an argument error no output
  *    is written and nothing is launched;
- *  - the caller owns every buffer; the library keeps no global state, allocates nothing that
- *    outlives a call and may be called from several host threads on different streams;
+ *  - the caller owns every buffer passed in; the library may be called from several host threads on different
+ *    streams and devices.  What it keeps between calls is (i) PER HOST THREAD: the text of the last CUDA error, the
+ *    launch count and the profiling events of the measurement helpers, and the staging arena (one pinned host block,
+ *    one device block, grown on demand) of the synchronous HOST-pointer entries -- all released by
+ *    qmc_release_thread_resources() and at thread exit; (ii) per device ordinal: cached immutable attributes (SM count,
+ *    resident CTAs of each kernel).  The stream-ordered entries allocate nothing and read no environment variables;
  *  - "HOST" / "DEVICE" beside a pointer says which address space it must point to;
  *  - there is no CPU fallback: without a CUDA device every compute entry returns QMC_ERR_CUDA.
  *
@@ -39,8 +43,10 @@
  *      QMC_FAMILY_SECTOR        [a, b, nU, nF, nu_1..nu_d, cU_1..cU_nU, eU_{1,1}..eU_{nU,d},
  *                                cF_1..cF_nF, eF_{1,1}..eF_{nF,d}]
  *                               f = prod x_j^nu_j * U(x)^a / F(x)^b, U = sum_t cU_t prod_j x_j^eU_{t,j}
- *                               (sector-decomposed shape); limits: 0 <= a,b <= 8, nu_j <= 8,
- *                               nU,nF in 1..64, exponents <= 8, total degree of a monomial <= 16.
+ *                               (sector-decomposed shape); limits: dim <= QMC_MAX_SECTOR_DIM = 16 (the coordinates
+ *                               of G points live in registers), 0 <= a,b <= 8, nu_j <= 8, nU,nF in 1..64,
+ *                               exponents <= 8, total degree of a monomial <= 16 -- every block within these limits is
+ *                               accepted (the interpreter program holds up to 128 monomials of degree 16).
  *                               Optional trailing block [lu, lf, p] (n_params = the above + 3):
  *                               f * (lu log U + lf log F)^p, p an integer in 1..4 -- the shape of the order-eps^p
  *                               term of U^(a + lu eps) / F^(b - lf eps) in the eps-expansion of a sector;
@@ -61,7 +67,7 @@ extern "C" {
 typedef enum {
     QMC_OK = 0,
     QMC_ERR_NULL = -1,       /* a required pointer is NULL */
-    QMC_ERR_DIM = -2,        /* dim outside 1..QMC_MAX_DIM */
+    QMC_ERR_DIM = -2,        /* dim outside 1..QMC_MAX_DIM (1..QMC_MAX_SECTOR_DIM for QMC_FAMILY_SECTOR) */
     QMC_ERR_N = -3,          /* n outside 2 .. 2^53-1 (double(r) must be exact), or count/bins invalid */
     QMC_ERR_Z = -4,          /* z_j outside [1, n-1] or not coprime to n */
     QMC_ERR_SHIFT = -5,      /* a shift outside [0,1) or not finite */
@@ -86,7 +92,7 @@ enum { QMC_FAMILY_GENZ_OSC = 0, QMC_FAMILY_GENZ_PRODPEAK = 1, QMC_FAMILY_CEXP_PO
 enum { QMC_TRANSFORM_NONE = 0, QMC_TRANSFORM_BAKER = 1, QMC_TRANSFORM_KOROBOV = 100, QMC_TRANSFORM_SIDI = 200,
        QMC_TRANSFORM_KOROBOV_ASYM = 1000 };
 
-enum { QMC_MAX_DIM = 32, QMC_MAX_M = 4096 };
+enum { QMC_MAX_DIM = 32, QMC_MAX_M = 4096, QMC_MAX_SECTOR_DIM = 16 /* QMC_FAMILY_SECTOR only */ };
 
 /* One integration problem.  In qmc_lattice_integrate_batch / qmc_lattice_project the four data
  * pointers are DEVICE pointers; the struct array itself is HOST memory. */
@@ -120,8 +126,10 @@ int qmc_lattice_integrate_ex(int family, const double* params, int n_params, int
                              double* out_shift_means /*HOST or NULL*/);
 
 /* Stream-ordered batched call: `count` problems of arbitrary, unequal cost in ONE persistent-grid
- * launch (device-side tile queue; the paper's host-side work queue is P:L388-L402) followed by one
- * finalize launch.  Never synchronises.  problems: HOST array whose data pointers are DEVICE
+ * launch per kernel variant (device-side tile queue; the paper's host-side work queue is P:L388-L402) followed by
+ * one finalize launch.  Never waits for the device: a call for one closed-form problem is kernel launches (and at most
+ * one 8-byte memset) only and can be captured in a CUDA graph; a batch call also issues one cudaMemcpyAsync of its launch
+ * plan (KBs) from pageable host memory, which the runtime stages before the call returns.  problems: HOST array whose data pointers are DEVICE
  * pointers (only the struct fields are validated here; the pointed-to values are the caller's
  * responsibility -- use qmc_validate_problem_host before uploading).
  *   out_means, out_errs : DEVICE, count*2 doubles: [p*2 + c], c = 0 (re) / 1 (im, 0 for real families)
@@ -137,6 +145,29 @@ int qmc_lattice_integrate_batch(int count, const qmc_problem* problems /*HOST*/,
 
 /* Bytes of workspace qmc_lattice_integrate_batch / qmc_lattice_project need (0 on invalid input). */
 size_t qmc_workspace_bytes(int count, const qmc_problem* problems /*HOST*/);
+
+/* Launch-plan options for tests and tuning (zero-initialise for the library's plan): the same calls with an options
+ * struct.  tiles_target > 0: that many tiles per kernel variant instead of the planned count (S9; results are
+ * bit-identical only for equal tilings); force_wide != 0: the 64-bit-residue kernels even for n < 2^31 (they are
+ * otherwise reached only by n >= 2^31; results are bit-identical to the 32-bit kernels). */
+typedef struct { int tiles_target; int force_wide; } qmc_plan_options;
+int qmc_lattice_integrate_batch_opts(int count, const qmc_problem* problems /*HOST*/, double* out_means /*DEVICE*/,
+                                     double* out_errs /*DEVICE*/, double* out_shift_means /*DEVICE or NULL*/,
+                                     void* workspace /*DEVICE*/, size_t workspace_bytes, void* cuda_stream,
+                                     const qmc_plan_options* opts /*HOST or NULL*/);
+size_t qmc_workspace_bytes_opts(int count, const qmc_problem* problems /*HOST*/, const qmc_plan_options* opts /*HOST or NULL*/);
+
+/* Synchronous batched call, HOST pointers everywhere (problems[i].params / z / shifts / fit_coeffs included): full value
+ * validation of every problem, ONE host-to-device copy of all inputs from the calling thread's pinned staging block, the
+ * batched hot path on the default stream of the current device, one device-to-host copy of the results, synchronise.
+ *   out_means, out_errs : HOST, count*2 doubles [p*2 + c]
+ *   out_shift_means     : HOST or NULL, count * 2*max_m doubles [p*(2 max_m) + s*ncomp + c], max_m = largest m of the batch
+ * Returns QMC_ERR_NONFINITE (results still written) if a result is NaN/Inf. */
+int qmc_lattice_integrate_batch_host(int count, const qmc_problem* problems /*HOST, HOST data pointers*/,
+                                     double* out_means /*HOST*/, double* out_errs /*HOST*/, double* out_shift_means /*HOST or NULL*/);
+
+/* Releases what the calling host thread holds (profiling events, staging arena); also done at thread exit. */
+int qmc_release_thread_resources(void);
 
 /* Full value validation of one problem whose data pointers are HOST pointers. */
 int qmc_validate_problem_host(const qmc_problem* p /*HOST, HOST data pointers*/);
@@ -175,13 +206,14 @@ int qmc_finalize_means(const double* shift_means /*DEVICE*/, int m, int ncomp, d
                        double* out_err /*DEVICE*/, void* cuda_stream);
 
 /* The paper's `integrate` iteration (section 3.3.1; fields P:L887-L920; result P:L988-L995) around the
- * fused hot path: sample min_m shifted copies of the smallest ladder lattice with n >= min_n; if the error goal
+ * fused hot path (synchronous; device memory is allocated for the duration of the call only): sample min_m shifted copies of the smallest ladder lattice with n >= min_n; if the error goal
  *     err <= max(epsabs, epsrel * |E|)                                  (per component for complex)
  * is not met, DISCARD the result and take a larger lattice; stop when the goal is met or `maxeval`
  * evaluations have been spent; when the ladder is exhausted keep the largest lattice and add shifts
  * (Monte Carlo scaling) up to max_m.  The paper does not say how the next lattice is chosen (DESIGN.md reading
  * C-14): the smallest ladder n >= n * max(2, err / goal) (assumes >= 1/n error scaling), limited to what `maxeval` still
- * allows.  All pointers HOST; synchronous; allocates device memory for the duration of the call only.
+ * allows; a lattice is only tried if min_m samples of it fit the remaining budget (otherwise shifts are added to the current
+ * lattice while they fit), so only the first lattice can take `evaluations` past maxeval.  All pointers HOST.
  *   ladder_n[i] ascending, ladder_z[i*dim + j] the generating vector of lattice i (an INPUT: P:L940-L942)
  *   shifts[max_m][dim]: the first m rows are used for a lattice sampled with m shifts
  *   errormode: 0 = all components, 1 = largest component (ignored for real families)
@@ -222,6 +254,16 @@ int qmc_profile_last_fused_ms(double* out_ms /*HOST*/);
  * k indices per tile of problem 0.  Any pointer may be NULL. */
 int qmc_plan_info(int count, const qmc_problem* problems /*HOST*/, long long* out_tiles, int* out_ctas,
                   long long* out_tile_len0);
+
+/* Inspection: the interpreter program the device-side compiler makes of a QMC_FAMILY_SECTOR parameter block (all pointers
+ * HOST; synchronous).  out_steps: n_steps one-byte step codes (0 no-op, 1 end of U, 2 end, 3 + 5 j + kind with kind
+ * 0 SC: S = fma(A, x_j, S), 1 SL: S = fma(cf, x_j, S), 2 AL: A = fma(cf, x_j, A), 3 ALI: A = fma(cf, x_j, cf2), 4 AM: A = A x_j);
+ * out_slots: n_slots pairs {cf, cf2}, one per SL / AL / ALI / end-of-U step in program order (the end-of-U slot holds F's
+ * constant term) plus one of read-ahead; out_c0: constant terms of U and F.  out_steps / out_slots may be NULL (counts only);
+ * QMC_ERR_WORKSPACE if a capacity is too small. */
+int qmc_sector_compile(const double* params /*HOST*/, int n_params, int dim, unsigned char* out_steps /*HOST or NULL*/,
+                       int steps_cap, int* out_n_steps /*HOST*/, double* out_slots /*HOST or NULL*/, int slots_cap,
+                       int* out_n_slots /*HOST*/, double* out_c0 /*HOST [2]*/);
 
 int qmc_num_components(int family);          /* 1 or 2; <0 on unknown family */
 const char* qmc_status_string(int status);

@@ -20,6 +20,8 @@ EXPORTS = [
     "qmc_lattice_points", "qmc_finalize_means", "qmc_fp64_peak_probe", "qmc_last_launch_count", "qmc_plan_info",
     "qmc_profile_enable", "qmc_profile_last_fused_ms",
     "qmc_num_components", "qmc_status_string", "qmc_last_cuda_error", "qmc_integrate", "qmc_fit_polysingular",
+    "qmc_lattice_integrate_batch_opts", "qmc_workspace_bytes_opts", "qmc_lattice_integrate_batch_host",
+    "qmc_release_thread_resources", "qmc_sector_compile",
 ]
 
 QMC_OK = 0
@@ -41,6 +43,10 @@ class qmc_problem(C.Structure):
     _fields_ = [("family", C.c_int), ("dim", C.c_int), ("m", C.c_int), ("transform", C.c_int), ("n", C.c_uint64),
                 ("params", C.c_void_p), ("n_params", C.c_int), ("z", C.c_void_p), ("shifts", C.c_void_p),
                 ("fit_coeffs", C.c_void_p)]
+
+
+class qmc_plan_options(C.Structure):
+    _fields_ = [("tiles_target", C.c_int), ("force_wide", C.c_int)]
 
 
 class qmc_result(C.Structure):
@@ -66,6 +72,13 @@ def lib():
         L.qmc_lattice_integrate_batch.argtypes = [C.c_int, pp, vp, vp, vp, vp, C.c_size_t, vp]
         L.qmc_workspace_bytes.argtypes = [C.c_int, pp]
         L.qmc_workspace_bytes.restype = C.c_size_t
+        po = C.POINTER(qmc_plan_options)
+        L.qmc_lattice_integrate_batch_opts.argtypes = [C.c_int, pp, vp, vp, vp, vp, C.c_size_t, vp, po]
+        L.qmc_workspace_bytes_opts.argtypes = [C.c_int, pp, po]
+        L.qmc_workspace_bytes_opts.restype = C.c_size_t
+        L.qmc_lattice_integrate_batch_host.argtypes = [C.c_int, pp, dp, dp, dp]
+        L.qmc_sector_compile.argtypes = [dp, C.c_int, C.c_int, C.POINTER(C.c_ubyte), C.c_int, C.POINTER(C.c_int), dp, C.c_int,
+                                         C.POINTER(C.c_int), dp]
         L.qmc_validate_problem_host.argtypes = [pp]
         L.qmc_lattice_project.argtypes = [pp, C.c_int, vp, vp, C.c_size_t, vp]
         L.qmc_project_workspace_bytes.argtypes = [pp, C.c_int]
@@ -132,6 +145,45 @@ def qmc_lattice_integrate_ex(p: dict):
     return sm, mean[:nc].copy(), err[:nc].copy()
 
 
+def qmc_lattice_integrate_batch_host(problems):
+    """Synchronous HOST-pointer batch (one H2D copy of all inputs, one D2H copy of all results) ->
+    (shift_means list of (m, ncomp), means (count, 2), errs (count, 2))."""
+    count = len(problems)
+    arr = (qmc_problem * count)()
+    keep = []
+    for i, p in enumerate(problems):
+        params, shifts, fit = _f64(p["params"]), _f64(p["shifts"]), _f64(p.get("fit_coeffs"))
+        z = np.ascontiguousarray(p["z"], dtype=np.uint64)
+        keep += [params, shifts, fit, z]
+        arr[i] = qmc_problem(p["family"], p["dim"], p["m"], p["transform"], p["n"], params.ctypes.data, len(params), z.ctypes.data,
+                             shifts.ctypes.data, None if fit is None else fit.ctypes.data)
+    max_m = max(p["m"] for p in problems)
+    means, errs, sm = np.zeros((count, 2)), np.zeros((count, 2)), np.zeros((count, 2 * max_m))
+    _check(lib().qmc_lattice_integrate_batch_host(count, arr, _d(means), _d(errs), _d(sm)), "qmc_lattice_integrate_batch_host")
+    out = []
+    for i, p in enumerate(problems):
+        nc = qmc_num_components(p["family"])
+        out.append(sm[i, : p["m"] * nc].reshape(p["m"], nc).copy())
+    return out, means, errs
+
+
+def qmc_sector_compile(params, dim):
+    """The interpreter program of a sector parameter block, compiled on the device -> (steps uint8[], slots (n, 2), c0 (2,))."""
+    params = _f64(params)
+    nst, nsl, c0 = C.c_int(), C.c_int(), np.zeros(2)
+    _check(lib().qmc_sector_compile(_d(params), len(params), int(dim), None, 0, C.byref(nst), None, 0, C.byref(nsl), _d(c0)),
+           "qmc_sector_compile")
+    steps = np.zeros(nst.value, dtype=np.uint8)
+    slots = np.zeros((nsl.value, 2))
+    _check(lib().qmc_sector_compile(_d(params), len(params), int(dim), steps.ctypes.data_as(C.POINTER(C.c_ubyte)), len(steps),
+                                    C.byref(nst), _d(slots), len(slots), C.byref(nsl), _d(c0)), "qmc_sector_compile")
+    return steps, slots, c0
+
+
+def qmc_release_thread_resources():
+    _check(lib().qmc_release_thread_resources(), "qmc_release_thread_resources")
+
+
 def qmc_integrate(family, params, dim, transform, ladder_n, ladder_z, shifts, min_n=8191, min_m=32, epsrel=0.01, epsabs=1e-7,
                   maxeval=1000000, errormode=0, fit_coeffs=None):
     """The paper's `integrate` iteration (defaults: PAPER.md L887-L905) -> (dict result, status); status is QMC_OK when the
@@ -181,8 +233,9 @@ class DeviceBatch:
     (count, 2*max_m).
     """
 
-    def __init__(self, problems, device="cuda:0"):
+    def __init__(self, problems, device="cuda:0", tiles_target=0, force_wide=False):
         import torch
+        self.opts = qmc_plan_options(int(tiles_target), 1 if force_wide else 0)
         self.torch = torch
         self.device = torch.device(device)
         self.problems = problems
@@ -201,7 +254,7 @@ class DeviceBatch:
                                  None if t_fit is None else t_fit.data_ptr())
         self.arr = arr
         self.max_m = max(p["m"] for p in problems)
-        self.ws_bytes = int(lib().qmc_workspace_bytes(self.count, arr))
+        self.ws_bytes = int(lib().qmc_workspace_bytes_opts(self.count, arr, C.byref(self.opts)))
         if self.ws_bytes == 0:
             st = lib().qmc_plan_info(self.count, arr, None, None, None)
             raise QmcError(st if st != 0 else -11, "qmc_workspace_bytes")
@@ -220,8 +273,8 @@ class DeviceBatch:
     def integrate(self, stream=None):
         """qmc_lattice_integrate_batch on `stream` (default: torch's current stream); returns launch count."""
         s = self.torch.cuda.current_stream(self.device).cuda_stream if stream is None else stream
-        _check(lib().qmc_lattice_integrate_batch(self.count, self.arr, self.means.data_ptr(), self.errs.data_ptr(),
-                                                 self.shift_means.data_ptr(), self.ws_ptr, self.ws_bytes, s),
+        _check(lib().qmc_lattice_integrate_batch_opts(self.count, self.arr, self.means.data_ptr(), self.errs.data_ptr(),
+                                                      self.shift_means.data_ptr(), self.ws_ptr, self.ws_bytes, s, C.byref(self.opts)),
                "qmc_lattice_integrate_batch")
         return int(lib().qmc_last_launch_count())
 

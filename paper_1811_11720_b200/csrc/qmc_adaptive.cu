@@ -8,9 +8,16 @@
 
 #include <cuda_runtime.h>
 
-#include "../../include/qmc_lattice.h"
+#include "qmc_kernels.h"
 
 namespace {
+
+// CUDA failures are recorded for qmc_last_cuda_error() (qmc_host.cu)
+#define ADAPT_CUDA(call)                                                        \
+    do {                                                                        \
+        cudaError_t e_ = (call);                                                \
+        if (e_ != cudaSuccess) return qmc::report_cuda_error(e_, #call);        \
+    } while (0)
 
 struct DeviceBlock {              // one stream-ordered allocation, freed when the call returns
     char* p = nullptr;
@@ -68,8 +75,7 @@ extern "C" int qmc_integrate(int family, const double* params, int n_params, int
                  b_out = 256;
     DeviceBlock blk;
     blk.st = st;
-    if (cudaMallocAsync(reinterpret_cast<void**>(&blk.p), b_params + b_z + b_sh + b_fit + 2 * b_sm + b_out + ws_bytes, st) != cudaSuccess)
-        return QMC_ERR_CUDA;
+    ADAPT_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&blk.p), b_params + b_z + b_sh + b_fit + 2 * b_sm + b_out + ws_bytes, st));
     char* d_params = blk.p;
     char* d_z = d_params + b_params;
     char* d_sh = d_z + b_z;
@@ -78,11 +84,10 @@ extern "C" int qmc_integrate(int family, const double* params, int n_params, int
     double* d_sm_new = reinterpret_cast<double*>(reinterpret_cast<char*>(d_sm) + b_sm);   // means of an extension
     double* d_out = reinterpret_cast<double*>(reinterpret_cast<char*>(d_sm_new) + b_sm);  // mean(2), err(2)
     char* d_ws = reinterpret_cast<char*>(d_out) + b_out;
-    if (cudaMemcpyAsync(d_params, params, (size_t)n_params * 8, cudaMemcpyHostToDevice, st) != cudaSuccess ||
-        cudaMemcpyAsync(d_z, ladder_z, (size_t)n_lattices * dim * 8, cudaMemcpyHostToDevice, st) != cudaSuccess ||
-        cudaMemcpyAsync(d_sh, shifts, (size_t)max_m * dim * 8, cudaMemcpyHostToDevice, st) != cudaSuccess ||
-        (fit_coeffs && cudaMemcpyAsync(d_fit, fit_coeffs, (size_t)dim * 6 * 8, cudaMemcpyHostToDevice, st) != cudaSuccess))
-        return QMC_ERR_CUDA;
+    ADAPT_CUDA(cudaMemcpyAsync(d_params, params, (size_t)n_params * 8, cudaMemcpyHostToDevice, st));
+    ADAPT_CUDA(cudaMemcpyAsync(d_z, ladder_z, (size_t)n_lattices * dim * 8, cudaMemcpyHostToDevice, st));
+    ADAPT_CUDA(cudaMemcpyAsync(d_sh, shifts, (size_t)max_m * dim * 8, cudaMemcpyHostToDevice, st));
+    if (fit_coeffs) ADAPT_CUDA(cudaMemcpyAsync(d_fit, fit_coeffs, (size_t)dim * 6 * 8, cudaMemcpyHostToDevice, st));
 
     qmc_problem dp = hp;
     dp.params = reinterpret_cast<const double*>(d_params);
@@ -104,14 +109,12 @@ extern "C" int qmc_integrate(int family, const double* params, int n_params, int
         int rc = qmc_lattice_integrate_batch(1, &dp, d_out, d_out + 2, sm_dst, d_ws, ws_bytes, st);
         if (rc != QMC_OK) return rc;
         if (m_have > 0) {                                                // extension: append the new means, redo Eq. 2-3 over all
-            if (cudaMemcpyAsync(d_sm + (size_t)m_have * nc, d_sm_new, (size_t)m_add * nc * 8, cudaMemcpyDeviceToDevice, st) != cudaSuccess)
-                return QMC_ERR_CUDA;
+            ADAPT_CUDA(cudaMemcpyAsync(d_sm + (size_t)m_have * nc, d_sm_new, (size_t)m_add * nc * 8, cudaMemcpyDeviceToDevice, st));
             rc = qmc_finalize_means(d_sm, m, nc, d_out, d_out + 2, st);
             if (rc != QMC_OK) return rc;
         }
-        if (cudaMemcpyAsync(host_out, d_out, sizeof(host_out), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
-            cudaStreamSynchronize(st) != cudaSuccess)
-            return QMC_ERR_CUDA;
+        ADAPT_CUDA(cudaMemcpyAsync(host_out, d_out, sizeof(host_out), cudaMemcpyDeviceToHost, st));
+        ADAPT_CUDA(cudaStreamSynchronize(st));
         out->iterations += 1;
         out->evaluations += (uint64_t)m_add * ladder_n[li];
         out->n = ladder_n[li];
@@ -123,17 +126,23 @@ extern "C" int qmc_integrate(int family, const double* params, int n_params, int
         if (goal_met(out->integral, out->error, nc, epsrel, epsabs, errormode, &ratio)) return QMC_OK;
         if (out->evaluations >= maxeval) return QMC_ERR_MAXEVAL;
         const uint64_t budget = maxeval - out->evaluations;
+        bool enlarged = false;
         if (li + 1 < n_lattices) {
-            // larger lattice: smallest ladder n >= n * max(2, err/goal), limited by what maxeval still allows
+            // larger lattice: smallest ladder n >= n * max(2, err/goal), limited by what maxeval still allows: a lattice
+            // whose min_m samples do not fit the remaining budget is not tried
             const double want = (double)ladder_n[li] * std::fmax(2.0, std::isfinite(ratio) ? ratio : 2.0);
             int nx = li + 1;
             while (nx + 1 < n_lattices && (double)ladder_n[nx] < want) ++nx;
-            while (nx > li + 1 && (uint64_t)min_m * ladder_n[nx] > budget) --nx;
-            li = nx;
-            m = min_m;
-            m_have = 0;                                                  // earlier results are discarded
-        } else {
-            // ladder exhausted: add shifts on the largest lattice, Monte Carlo scaling err ~ m^-1/2
+            while (nx > li && (uint64_t)min_m * ladder_n[nx] > budget) --nx;
+            if (nx > li) {
+                li = nx;
+                m = min_m;
+                m_have = 0;                                              // earlier results are discarded
+                enlarged = true;
+            }
+        }
+        if (!enlarged) {
+            // ladder exhausted (or no larger lattice affordable): add shifts on the current lattice, Monte Carlo scaling err ~ m^-1/2
             if (m >= max_m) return QMC_ERR_MAXEVAL;
             double grow = std::isfinite(ratio) ? ratio * ratio : 2.0;
             long long m_next = (long long)std::ceil((double)m * std::fmin(std::fmax(grow, 1.25), 4.0));

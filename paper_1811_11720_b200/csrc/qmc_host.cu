@@ -15,14 +15,35 @@
 namespace qmc {
 namespace {
 
-thread_local std::string g_last_error;
-thread_local int g_last_launches = 0;
-thread_local bool g_profile = false;                 // qmc_profile_enable
-thread_local cudaEvent_t g_ev0 = nullptr, g_ev1 = nullptr;
-thread_local bool g_ev_valid = false;
+// Per-thread measurement and staging state (include/qmc_lattice.h, "Conventions"): the text of the last CUDA error, the launch
+// count of the last batch call, the profiling events (created on first use for the device that is current then) and the
+// staging arena of the synchronous HOST-pointer entries.  Everything is released by qmc_release_thread_resources() and by
+// the destructor at thread exit.
+struct ThreadState {
+    std::string last_error;
+    int last_launches = 0;
+    bool profile = false;                            // qmc_profile_enable
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    int ev_device = -1;
+    bool ev_valid = false;
+    // staging arena of the HOST-pointer entries: pinned host block + device block, grown on demand, bound to one device
+    char* pinned = nullptr;
+    char* device = nullptr;
+    size_t pinned_bytes = 0, device_bytes = 0;
+    int arena_device = -1;
+    void release() {
+        if (ev0) { cudaEventDestroy(ev0); cudaEventDestroy(ev1); ev0 = ev1 = nullptr; }
+        ev_valid = false; ev_device = -1;
+        if (pinned) { cudaFreeHost(pinned); pinned = nullptr; pinned_bytes = 0; }
+        if (device) { cudaFree(device); device = nullptr; device_bytes = 0; }
+        arena_device = -1;
+    }
+    ~ThreadState() { release(); }                    // errors (context already gone at process exit) are ignored
+};
+thread_local ThreadState g_ts;
 
 int cuda_fail(cudaError_t e, const char* where) {
-    g_last_error = std::string(where) + ": " + cudaGetErrorString(e);
+    g_ts.last_error = std::string(where) + ": " + cudaGetErrorString(e);
     return QMC_ERR_CUDA;
 }
 }  // namespace
@@ -49,11 +70,12 @@ int dim_slots(int family, int dim, bool wide) {
     if (wide) return dim <= 8 ? 8 : (dim <= 16 ? 16 : 32);
     return dim <= 4 ? 4 : (dim <= 6 ? 6 : (dim <= 8 ? 8 : (dim <= 12 ? 12 : (dim <= 16 ? 16 : 32))));
 }
-bool force_wide();
-bool is_wide(unsigned long long n) { return n >= (1ull << 31) || force_wide(); }
+bool is_wide(unsigned long long n, const qmc_plan_options& o) { return n >= (1ull << 31) || o.force_wide != 0; }
 // residue width of the kernel variant: 64-bit for n >= 2^31, and for the 32-slot closed-form kernels (dim > 16), which
 // exist only with wide residues
-bool variant_wide(int family, int dim, unsigned long long n) { return is_wide(n) || (family != QMC_FAMILY_SECTOR && dim > 16); }
+bool variant_wide(int family, int dim, unsigned long long n, const qmc_plan_options& o) {
+    return is_wide(n, o) || (family != QMC_FAMILY_SECTOR && dim > 16);
+}
 
 // transform id -> tile-loop kind, symmetric Korobov weight r (0 if none) and the generic-transform code
 // gen = GEN_* | r0 << 4 | r1 << 8 (Table A.2)
@@ -114,21 +136,6 @@ int validate_struct(const qmc_problem& p, bool need_two_shifts) {
     return QMC_OK;
 }
 
-int tiles_target() {
-    static const int v = [] {
-        const char* e = std::getenv("QMC_TILES_TARGET");
-        const int t = e ? std::atoi(e) : 0;
-        return t > 0 ? t : 0;
-    }();
-    return v;
-}
-
-// test knob: run small lattices through the 64-bit-residue kernels (they are otherwise reached only for n >= 2^31)
-bool force_wide() {
-    const char* e = std::getenv("QMC_FORCE_WIDE");
-    return e && e[0] == '1';
-}
-
 // ---- launch plan: tiles, kernel variants, workspace layout (pure function of the problem structs) ----
 struct Variant {
     int family, dp;                  // kernel family (kernel_family(public id)), dimension slots
@@ -147,7 +154,9 @@ struct Plan {
     long long total_tiles = 0;
 };
 
-int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan* plan) {
+const qmc_plan_options kDefaultOptions = {0, 0};
+
+int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan* plan, const qmc_plan_options& opt = kDefaultOptions) {
     if (count < 1 || !problems) return count < 1 ? QMC_ERR_N : QMC_ERR_NULL;
     plan->dev.resize(count);
     long long means_off = 0;
@@ -167,7 +176,7 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
         d.n_params = p.n_params;
         d.out_index = i;
         d.wconst = 1.0;
-        const int npad = dim_slots(p.family, p.dim, variant_wide(p.family, p.dim, p.n)) - p.dim;   // padded dimension slots sit at u = 1/2 (qmc_fused.cuh)
+        const int npad = dim_slots(p.family, p.dim, variant_wide(p.family, p.dim, p.n, opt)) - p.dim;   // padded dimension slots sit at u = 1/2 (qmc_fused.cuh)
         if (d.kor_r > 0) {
             // Eq. 15: c_r = (2r+1) C(2r,r); centred antiderivative coefficients of Eq. 14 (see qmc_device.cuh)
             const int r = d.kor_r;
@@ -206,7 +215,7 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
     // kernel variants
     for (int i = 0; i < count; ++i) {
         const DevProblem& d = plan->dev[i];
-        const bool wide = variant_wide(d.family, d.dim, d.n);
+        const bool wide = variant_wide(d.family, d.dim, d.n, opt);
         const int dp = dim_slots(d.family, d.dim, wide);
         Variant* v = nullptr;
         for (auto& c : plan->variants)
@@ -220,7 +229,7 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
     for (auto& v : plan->variants) {
         const int resident = kPlanSMs * (v.family == QMC_FAMILY_SECTOR ? min_blocks_sector(v.dp) : min_blocks_closed(v.dp, v.wide));
         const int threads = v.family == QMC_FAMILY_SECTOR ? sector_threads(v.dp) : kThreads;   // CTA size of the variant's kernel
-        const int env = tiles_target();
+        const int env = opt.tiles_target > 0 ? opt.tiles_target : 0;
         // one problem: equal tiles, 2 per resident CTA (the queue evens out SM speed differences over a long kernel) -- or
         // exactly 1 when the whole kernel is short (< kShortEvalsPerCta evaluations per CTA: per-tile overhead and the
         // queue reset matter more than balance); a batch of unequal problems: 8 per resident CTA
@@ -276,14 +285,21 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
     return QMC_OK;
 }
 
+// Immutable device attributes, cached per device ordinal (written once with the same value by whichever thread asks first).
+constexpr int kMaxDevices = 64;
+int current_device() {
+    int dev = 0;
+    return cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < kMaxDevices ? dev : -1;
+}
 int sm_count() {
-    static const int v = [] {
-        int dev = 0, n = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess) return 0;
-        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
-        return n;
-    }();
-    return v;
+    static int cache[kMaxDevices];
+    const int dev = current_device();
+    if (dev < 0) return 0;
+    if (cache[dev] > 0) return cache[dev];
+    int n = 0;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
+    cache[dev] = n;
+    return n;
 }
 
 // closed-form families: the kernel variants live in four parts per family (qmc_fused_closed.inc); try each
@@ -315,8 +331,10 @@ int occupancy_closed(int family, int dp, bool wide) {
 #undef QMC_TRY_PARTS
 
 int occupancy(int family, int dp, bool wide) {
-    static int cache[5][33][2];
-    int& c = cache[family][dp][wide ? 1 : 0];
+    static int cache[kMaxDevices][5][33][2];
+    const int dev = current_device();
+    if (dev < 0) return -1;
+    int& c = cache[dev][family][dp][wide ? 1 : 0];
     if (c > 0) return c;
     int v = -1;
     switch (family) {
@@ -327,12 +345,40 @@ int occupancy(int family, int dp, bool wide) {
     return v;
 }
 
+// the thread's staging arena (pinned host + device), grown on demand; bound to the device that is current
+int arena_reserve(size_t pinned_bytes, size_t device_bytes) {
+    ThreadState& t = g_ts;
+    const int dev = current_device();
+    if (dev < 0) return cuda_fail(cudaErrorNoDevice, "no CUDA device");
+    if (t.arena_device != dev && (t.pinned || t.device)) {
+        if (t.pinned) { cudaFreeHost(t.pinned); t.pinned = nullptr; t.pinned_bytes = 0; }
+        if (t.device) { cudaFree(t.device); t.device = nullptr; t.device_bytes = 0; }
+    }
+    t.arena_device = dev;
+    if (pinned_bytes > t.pinned_bytes) {
+        if (t.pinned) { cudaFreeHost(t.pinned); t.pinned = nullptr; t.pinned_bytes = 0; }
+        const size_t want = std::max<size_t>(pinned_bytes + pinned_bytes / 2, 1 << 16);
+        cudaError_t e = cudaMallocHost(reinterpret_cast<void**>(&t.pinned), want);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaMallocHost (staging arena)");
+        t.pinned_bytes = want;
+    }
+    if (device_bytes > t.device_bytes) {
+        if (t.device) { cudaFree(t.device); t.device = nullptr; t.device_bytes = 0; }
+        const size_t want = std::max<size_t>(device_bytes + device_bytes / 2, 1 << 20);
+        cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&t.device), want);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaMalloc (staging arena)");
+        t.device_bytes = want;
+    }
+    return QMC_OK;
+}
+
 int run_batch(int count, const qmc_problem* problems, double* out_means, double* out_errs, double* out_shift_means,
-              void* workspace, size_t workspace_bytes, cudaStream_t st) {
-    g_last_launches = 0;
+              void* workspace, size_t workspace_bytes, cudaStream_t st, const qmc_plan_options& opt = kDefaultOptions,
+              char* pinned_blob = nullptr) {
+    g_ts.last_launches = 0;
     if (!out_means || !out_errs) return QMC_ERR_NULL;
     Plan plan;
-    const int pst = make_plan(count, problems, true, &plan);
+    const int pst = make_plan(count, problems, true, &plan, opt);
     if (pst != QMC_OK) return pst;
     if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || workspace_bytes < plan.total) return QMC_ERR_WORKSPACE;
     const int sms = sm_count();
@@ -357,11 +403,16 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
     std::vector<VariantQueue> queues(plan.variants.size());
     if (!single) {
         // host image of [queue heads (zero) | probs | plist | prefix]: one upload resets the queues too
+        // (the synchronous HOST-pointer entries pass a pinned staging block; the stream-ordered entry copies from pageable memory,
+        // which the runtime stages before cudaMemcpyAsync returns -- the call does not wait for the device)
         const size_t blob_bytes = plan.off_aux - plan.off_counters;
-        std::vector<char> blob(blob_bytes, 0);
-        std::memcpy(blob.data() + (plan.off_probs - plan.off_counters), plan.dev.data(), (size_t)count * sizeof(DevProblem));
-        int* plist = reinterpret_cast<int*>(blob.data() + (plan.off_plist - plan.off_counters));
-        long long* prefix = reinterpret_cast<long long*>(blob.data() + (plan.off_prefix - plan.off_counters));
+        std::vector<char> pageable;
+        char* blob = pinned_blob;
+        if (!blob) { pageable.assign(blob_bytes, 0); blob = pageable.data(); }
+        else std::memset(blob, 0, blob_bytes);
+        std::memcpy(blob + (plan.off_probs - plan.off_counters), plan.dev.data(), (size_t)count * sizeof(DevProblem));
+        int* plist = reinterpret_cast<int*>(blob + (plan.off_plist - plan.off_counters));
+        long long* prefix = reinterpret_cast<long long*>(blob + (plan.off_prefix - plan.off_counters));
         size_t pl = 0, pf = 0;
         int vi = 0;
         for (auto& v : plan.variants) {
@@ -376,10 +427,10 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
             prefix[pf++] = acc;
             ++vi;
         }
-        QMC_CUDA(cudaMemcpyAsync(ws + plan.off_counters, blob.data(), blob_bytes, cudaMemcpyHostToDevice, st));
+        QMC_CUDA(cudaMemcpyAsync(ws + plan.off_counters, blob, blob_bytes, cudaMemcpyHostToDevice, st));
         if (any_sector) {                                   // S0 for the sector family: tables + device-side program compiler
             QMC_CUDA(launch_prepare(count, st, dprobs, daux, dprog));
-            ++g_last_launches;
+            ++g_ts.last_launches;
         }
     } else {
         std::memset(&queues[0], 0, sizeof(VariantQueue));
@@ -391,10 +442,12 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
             QMC_CUDA(cudaMemsetAsync(queues[0].counter, 0, sizeof(unsigned long long), st));
         }
     }
-    g_ev_valid = false;
-    if (g_profile) {
-        if (!g_ev0) { QMC_CUDA(cudaEventCreate(&g_ev0)); QMC_CUDA(cudaEventCreate(&g_ev1)); }
-        QMC_CUDA(cudaEventRecord(g_ev0, st));
+    g_ts.ev_valid = false;
+    if (g_ts.profile) {
+        const int dev = current_device();
+        if (g_ts.ev0 && g_ts.ev_device != dev) { cudaEventDestroy(g_ts.ev0); cudaEventDestroy(g_ts.ev1); g_ts.ev0 = g_ts.ev1 = nullptr; }
+        if (!g_ts.ev0) { QMC_CUDA(cudaEventCreate(&g_ts.ev0)); QMC_CUDA(cudaEventCreate(&g_ts.ev1)); g_ts.ev_device = dev; }
+        QMC_CUDA(cudaEventRecord(g_ts.ev0, st));
     }
     for (size_t vi = 0; vi < plan.variants.size(); ++vi) {
         const Variant& v = plan.variants[vi];
@@ -410,11 +463,11 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
             case 3: e = launch_fused_f3(v.dp, v.wide, grid, st, a); break;
         }
         if (e != cudaSuccess) return cuda_fail(e, "fused kernel launch");
-        ++g_last_launches;
+        ++g_ts.last_launches;
     }
-    if (g_profile) { QMC_CUDA(cudaEventRecord(g_ev1, st)); g_ev_valid = true; }
+    if (g_ts.profile) { QMC_CUDA(cudaEventRecord(g_ts.ev1, st)); g_ts.ev_valid = true; }
     QMC_CUDA(launch_finalize(count, st, base, dmeans, out_means, out_errs, out_shift_means, 2 * plan.max_m));
-    ++g_last_launches;
+    ++g_ts.last_launches;
     return QMC_OK;
 }
 
@@ -521,26 +574,32 @@ const char* qmc_status_string(int status) {
     return "unknown status";
 }
 
-const char* qmc_last_cuda_error(void) { return g_last_error.c_str(); }
-int qmc_last_launch_count(void) { return g_last_launches; }
+const char* qmc_last_cuda_error(void) { return g_ts.last_error.c_str(); }
+int qmc_last_launch_count(void) { return g_ts.last_launches; }
 
-int qmc_profile_enable(int on) { g_profile = on != 0; return QMC_OK; }
+int qmc_profile_enable(int on) { g_ts.profile = on != 0; return QMC_OK; }
+
+int qmc_release_thread_resources(void) {
+    g_ts.release();
+    return QMC_OK;
+}
 
 int qmc_profile_last_fused_ms(double* out_ms) {
     if (!out_ms) return QMC_ERR_NULL;
-    if (!g_ev_valid) return QMC_ERR_N;
-    QMC_CUDA(cudaEventSynchronize(g_ev1));
+    if (!g_ts.ev_valid) return QMC_ERR_N;
+    QMC_CUDA(cudaEventSynchronize(g_ts.ev1));
     float ms = 0.f;
-    QMC_CUDA(cudaEventElapsedTime(&ms, g_ev0, g_ev1));
+    QMC_CUDA(cudaEventElapsedTime(&ms, g_ts.ev0, g_ts.ev1));
     *out_ms = (double)ms;
     return QMC_OK;
 }
 
-size_t qmc_workspace_bytes(int count, const qmc_problem* problems) {
+size_t qmc_workspace_bytes_opts(int count, const qmc_problem* problems, const qmc_plan_options* opts) {
     Plan plan;
-    if (make_plan(count, problems, true, &plan) != QMC_OK) return 0;
+    if (make_plan(count, problems, true, &plan, opts ? *opts : kDefaultOptions) != QMC_OK) return 0;
     return plan.total;
 }
+size_t qmc_workspace_bytes(int count, const qmc_problem* problems) { return qmc_workspace_bytes_opts(count, problems, nullptr); }
 
 int qmc_plan_info(int count, const qmc_problem* problems, long long* out_tiles, int* out_ctas, long long* out_tile_len0) {
     Plan plan;
@@ -565,10 +624,85 @@ int qmc_validate_problem_host(const qmc_problem* p) {
     return validate_values(*p);
 }
 
+int qmc_lattice_integrate_batch_opts(int count, const qmc_problem* problems, double* out_means, double* out_errs,
+                                     double* out_shift_means, void* workspace, size_t workspace_bytes, void* cuda_stream,
+                                     const qmc_plan_options* opts) {
+    return run_batch(count, problems, out_means, out_errs, out_shift_means, workspace, workspace_bytes,
+                     static_cast<cudaStream_t>(cuda_stream), opts ? *opts : kDefaultOptions);
+}
 int qmc_lattice_integrate_batch(int count, const qmc_problem* problems, double* out_means, double* out_errs,
                                 double* out_shift_means, void* workspace, size_t workspace_bytes, void* cuda_stream) {
-    return run_batch(count, problems, out_means, out_errs, out_shift_means, workspace, workspace_bytes,
-                     static_cast<cudaStream_t>(cuda_stream));
+    return qmc_lattice_integrate_batch_opts(count, problems, out_means, out_errs, out_shift_means, workspace, workspace_bytes,
+                                            cuda_stream, nullptr);
+}
+
+// Synchronous HOST-pointer batch: every input of every problem travels in ONE host-to-device copy from the thread's pinned
+// staging block, the results come back in one device-to-host copy; device memory comes from the thread's arena.
+int qmc_lattice_integrate_batch_host(int count, const qmc_problem* problems, double* out_means, double* out_errs,
+                                     double* out_shift_means) {
+    if (count < 1) return QMC_ERR_N;
+    if (!problems || !out_means || !out_errs) return QMC_ERR_NULL;
+    int max_m = 0;
+    size_t in_bytes = 0;
+    for (int i = 0; i < count; ++i) {
+        const int vst = validate_values(problems[i]);
+        if (vst != QMC_OK) return vst;
+        const qmc_problem& p = problems[i];
+        max_m = std::max(max_m, p.m);
+        in_bytes += align_up((size_t)p.n_params * 8, 256) + align_up((size_t)p.dim * 8, 256) + align_up((size_t)p.m * p.dim * 8, 256) +
+                    (p.fit_coeffs ? align_up((size_t)p.dim * 6 * 8, 256) : 0);
+    }
+    const size_t out_doubles = (size_t)count * (4 + 2 * (size_t)max_m);     // means (2), errs (2), shift means (2 max_m) per problem
+    const size_t out_bytes = align_up(out_doubles * 8, 256);
+    // device problem structs first (pointers into the arena's device block), then the plan
+    std::vector<qmc_problem> dp(problems, problems + count);
+    Plan plan;
+    const int pst = make_plan(count, problems, true, &plan);
+    if (pst != QMC_OK) return pst;
+    const size_t blob_bytes = align_up(plan.off_aux - plan.off_counters, 256);
+    const int ast = arena_reserve(in_bytes + blob_bytes + out_bytes, in_bytes + out_bytes + plan.total + 256);
+    if (ast != QMC_OK) return ast;
+    char* h_in = g_ts.pinned;                         // [inputs | plan blob | results]
+    char* h_blob = h_in + in_bytes;
+    char* h_out = h_blob + blob_bytes;
+    char* d_in = g_ts.device;
+    double* d_out = reinterpret_cast<double*>(d_in + in_bytes);
+    char* d_ws = reinterpret_cast<char*>(d_out) + out_bytes;
+    size_t off = 0;
+    for (int i = 0; i < count; ++i) {
+        const qmc_problem& p = problems[i];
+        auto put = [&](const void* src, size_t bytes) {
+            std::memcpy(h_in + off, src, bytes);
+            const char* dev = d_in + off;
+            off += align_up(bytes, 256);
+            return dev;
+        };
+        dp[i].params = reinterpret_cast<const double*>(put(p.params, (size_t)p.n_params * 8));
+        dp[i].z = reinterpret_cast<const uint64_t*>(put(p.z, (size_t)p.dim * 8));
+        dp[i].shifts = reinterpret_cast<const double*>(put(p.shifts, (size_t)p.m * p.dim * 8));
+        dp[i].fit_coeffs = p.fit_coeffs ? reinterpret_cast<const double*>(put(p.fit_coeffs, (size_t)p.dim * 6 * 8)) : nullptr;
+    }
+    cudaStream_t st = 0;
+    double* d_means = d_out;
+    double* d_errs = d_out + (size_t)count * 2;
+    double* d_sm = d_out + (size_t)count * 4;
+    QMC_CUDA(cudaMemcpyAsync(d_in, h_in, in_bytes, cudaMemcpyHostToDevice, st));
+    const int status = run_batch(count, dp.data(), d_means, d_errs, d_sm, d_ws, plan.total, st, kDefaultOptions, h_blob);
+    if (status != QMC_OK) { cudaStreamSynchronize(st); return status; }
+    QMC_CUDA(cudaMemcpyAsync(h_out, d_out, out_doubles * 8, cudaMemcpyDeviceToHost, st));
+    QMC_CUDA(cudaStreamSynchronize(st));
+    const double* r = reinterpret_cast<const double*>(h_out);
+    bool finite = true;
+    for (int i = 0; i < count; ++i) {
+        const int nc = ncomp_of(problems[i].family);
+        for (int c = 0; c < 2; ++c) {
+            out_means[(size_t)i * 2 + c] = r[(size_t)i * 2 + c];
+            out_errs[(size_t)i * 2 + c] = r[(size_t)count * 2 + (size_t)i * 2 + c];
+            if (c < nc) finite = finite && std::isfinite(out_means[(size_t)i * 2 + c]) && std::isfinite(out_errs[(size_t)i * 2 + c]);
+        }
+    }
+    if (out_shift_means) std::memcpy(out_shift_means, r + (size_t)count * 4, (size_t)count * 2 * max_m * 8);
+    return finite ? QMC_OK : QMC_ERR_NONFINITE;
 }
 
 int qmc_lattice_integrate_ex(int family, const double* params, int n_params, int dim, uint64_t n, const uint64_t* z,
@@ -578,60 +712,72 @@ int qmc_lattice_integrate_ex(int family, const double* params, int n_params, int
     qmc_problem hp;
     hp.family = family; hp.dim = dim; hp.m = m; hp.transform = transform; hp.n = n;
     hp.params = params; hp.n_params = n_params; hp.z = z; hp.shifts = shifts; hp.fit_coeffs = fit_coeffs;
-    const int vst = validate_values(hp);
+    const int vst = validate_values(hp);                       // before the arrays below are sized from m
     if (vst != QMC_OK) return vst;
+    double means[2], errs[2];
+    std::vector<double> sm(out_shift_means ? (size_t)2 * m : 0);
+    const int st = qmc_lattice_integrate_batch_host(1, &hp, means, errs, out_shift_means ? sm.data() : nullptr);
+    if (st != QMC_OK && st != QMC_ERR_NONFINITE) return st;
     const int nc = ncomp_of(family);
-    // one stream-ordered allocation: [params | z | shifts | fit | out_means(2) | out_errs(2) | shift_means(2m) | workspace]
-    const size_t b_params = align_up((size_t)n_params * 8, 256), b_z = align_up((size_t)dim * 8, 256),
-                 b_sh = align_up((size_t)m * dim * 8, 256), b_fit = align_up((size_t)dim * 6 * 8, 256),
-                 b_out = align_up((size_t)(4 + 2 * m) * 8, 256);
-    qmc_problem dp = hp;
+    for (int c = 0; c < nc; ++c) { out_mean[c] = means[c]; out_err[c] = errs[c]; }
+    if (out_shift_means)
+        for (int i = 0; i < m * nc; ++i) out_shift_means[i] = sm[i];
+    return st;
+}
+
+// Inspection: the interpreter program the device-side compiler makes of a sector parameter block (qmc_sector.cuh).
+int qmc_sector_compile(const double* params, int n_params, int dim, unsigned char* out_steps, int steps_cap, int* out_n_steps,
+                       double* out_slots, int slots_cap, int* out_n_slots, double* out_c0) {
+    if (!params || !out_n_steps || !out_n_slots || !out_c0) return QMC_ERR_NULL;
+    if (dim < 1 || dim > 16) return QMC_ERR_DIM;
+    // a one-point problem around the block: only the struct-level checks and the program matter here
+    const uint64_t z1[16] = {1, 1, 1, 1, 1, 1, 1, 1, 1, 1, 1, 1, 1, 1, 1, 1};
+    std::vector<double> sh((size_t)2 * dim, 0.25);
+    qmc_problem hp;
+    hp.family = QMC_FAMILY_SECTOR; hp.dim = dim; hp.m = 2; hp.transform = QMC_TRANSFORM_NONE; hp.n = 2;
+    hp.params = params; hp.n_params = n_params; hp.z = z1; hp.shifts = sh.data(); hp.fit_coeffs = nullptr;
     Plan plan;
     const int pst = make_plan(1, &hp, true, &plan);
     if (pst != QMC_OK) return pst;
-    const size_t total = b_params + b_z + b_sh + b_fit + b_out + plan.total;
+    const size_t b_params = align_up((size_t)n_params * 8, 256), b_z = 256;
+    const size_t blob_bytes = align_up(plan.off_aux - plan.off_counters, 256);
+    const size_t prog_bytes = plan.prog_words * 8, back_bytes = align_up(sizeof(DevAux) + prog_bytes, 256);
+    const int ast = arena_reserve(b_params + b_z + blob_bytes + back_bytes, b_params + b_z + plan.total + 256);
+    if (ast != QMC_OK) return ast;
+    char* h = g_ts.pinned;
+    char* d = g_ts.device;
+    std::memcpy(h, params, (size_t)n_params * 8);
+    std::memcpy(h + b_params, z1, (size_t)dim * 8);
     cudaStream_t st = 0;
-    char* buf = nullptr;
-    QMC_CUDA(cudaMallocAsync(reinterpret_cast<void**>(&buf), total, st));
-    char* d_params = buf;
-    char* d_z = d_params + b_params;
-    char* d_sh = d_z + b_z;
-    char* d_fit = d_sh + b_sh;
-    double* d_out = reinterpret_cast<double*>(d_fit + b_fit);
-    char* d_ws = reinterpret_cast<char*>(d_out) + b_out;
-    int status = QMC_OK;
-    cudaError_t e;
-    std::vector<double> host_out((size_t)4 + 2 * m);
-    // the inputs travel in ONE host-to-device copy: [params | z | shifts | fit] packed with the device layout
-    const size_t b_in = b_params + b_z + b_sh + (fit_coeffs ? (size_t)dim * 6 * 8 : 0);
-    std::vector<char> host_in(b_in);
-    std::memcpy(host_in.data(), params, (size_t)n_params * 8);
-    std::memcpy(host_in.data() + b_params, z, (size_t)dim * 8);
-    std::memcpy(host_in.data() + b_params + b_z, shifts, (size_t)m * dim * 8);
-    if (fit_coeffs) std::memcpy(host_in.data() + b_params + b_z + b_sh, fit_coeffs, (size_t)dim * 6 * 8);
-    do {
-        if ((e = cudaMemcpyAsync(buf, host_in.data(), b_in, cudaMemcpyHostToDevice, st)) != cudaSuccess) break;
-        dp.params = reinterpret_cast<const double*>(d_params);
-        dp.z = reinterpret_cast<const uint64_t*>(d_z);
-        dp.shifts = reinterpret_cast<const double*>(d_sh);
-        dp.fit_coeffs = fit_coeffs ? reinterpret_cast<const double*>(d_fit) : nullptr;
-        status = run_batch(1, &dp, d_out, d_out + 2, d_out + 4, d_ws, plan.total, st);
-        if (status != QMC_OK) { e = cudaSuccess; break; }
-        if ((e = cudaMemcpyAsync(host_out.data(), d_out, (size_t)(4 + 2 * m) * 8, cudaMemcpyDeviceToHost, st)) != cudaSuccess) break;
-        e = cudaStreamSynchronize(st);
-    } while (0);
-    cudaFreeAsync(buf, st);
-    if (e != cudaSuccess) return cuda_fail(e, "qmc_lattice_integrate");
-    if (status != QMC_OK) return status;
-    bool finite = true;
-    for (int c = 0; c < nc; ++c) {
-        out_mean[c] = host_out[c];
-        out_err[c] = host_out[2 + c];
-        finite = finite && std::isfinite(out_mean[c]) && std::isfinite(out_err[c]);
-    }
-    if (out_shift_means)
-        for (int i = 0; i < m * nc; ++i) out_shift_means[i] = host_out[4 + i];
-    return finite ? QMC_OK : QMC_ERR_NONFINITE;
+    QMC_CUDA(cudaMemcpyAsync(d, h, b_params + b_z, cudaMemcpyHostToDevice, st));
+    DevProblem dv = plan.dev[0];
+    dv.params = reinterpret_cast<const double*>(d);
+    dv.z = reinterpret_cast<const unsigned long long*>(d + b_params);
+    dv.shifts = reinterpret_cast<const double*>(d);            // never read by the prepare kernel
+    char* ws = d + b_params + b_z;
+    char* h_blob = h + b_params + b_z;
+    std::memset(h_blob, 0, blob_bytes);
+    std::memcpy(h_blob + (plan.off_probs - plan.off_counters), &dv, sizeof(DevProblem));
+    QMC_CUDA(cudaMemcpyAsync(ws + plan.off_counters, h_blob, plan.off_aux - plan.off_counters, cudaMemcpyHostToDevice, st));
+    QMC_CUDA(launch_prepare(1, st, reinterpret_cast<const DevProblem*>(ws + plan.off_probs), reinterpret_cast<DevAux*>(ws + plan.off_aux),
+                            reinterpret_cast<unsigned long long*>(ws + plan.off_prog)));
+    char* h_back = h_blob + blob_bytes;
+    QMC_CUDA(cudaMemcpyAsync(h_back, ws + plan.off_aux, sizeof(DevAux), cudaMemcpyDeviceToHost, st));
+    QMC_CUDA(cudaMemcpyAsync(h_back + sizeof(DevAux), ws + plan.off_prog, prog_bytes, cudaMemcpyDeviceToHost, st));
+    QMC_CUDA(cudaStreamSynchronize(st));
+    DevAux aux;
+    std::memcpy(&aux, h_back, sizeof(DevAux));
+    if (aux.status != 0) return aux.status;
+    const int nmono = (n_params - 4 - dim) / (1 + dim);
+    const double* slots = reinterpret_cast<const double*>(h_back + sizeof(DevAux));
+    const unsigned char* steps = reinterpret_cast<const unsigned char*>(h_back + sizeof(DevAux)) + (size_t)sector_slot_words(nmono) * 8;
+    const int n_steps = aux.sec_nops[0] * 4, n_slots = aux.sec_ncoef[0];
+    *out_n_steps = n_steps;
+    *out_n_slots = n_slots;
+    out_c0[0] = aux.sec_c0[0]; out_c0[1] = aux.sec_c0[1];
+    if (out_steps) { if (steps_cap < n_steps) return QMC_ERR_WORKSPACE; std::memcpy(out_steps, steps, (size_t)n_steps); }
+    if (out_slots) { if (slots_cap < n_slots) return QMC_ERR_WORKSPACE; std::memcpy(out_slots, slots, (size_t)n_slots * 16); }
+    return QMC_OK;
 }
 
 int qmc_lattice_integrate(int family, const double* params, int dim, uint64_t n, const uint64_t* z, const double* shifts,

@@ -117,9 +117,14 @@ __global__ void __launch_bounds__(kThreads) points_kernel(PointsArgs a) {
 }
 
 // ---------------------------------------------------------------------------------------------
-// FP64 peak probe: 8 independent DFMA chains per thread, 2048 threads per SM
+// FP64 peak probe: 8 independent DFMA chains per thread, 2048 threads per SM.  The multiplier and the addend are
+// compile-time constants, so that each DFMA reads ONE 64-bit vector-register operand pair besides its accumulator (the
+// constant multiplier comes from a uniform register): with three distinct vector-register operands per DFMA (round 1's
+// probe took a and b as kernel arguments, which ptxas loaded into vector registers) the register file, not the FP64
+// pipe, limits the rate -- 17.07 instead of 18.38 Tinst/s on the same B200 at 1965 MHz (nominal 148 x 64 x 1.965 = 18.61).
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256, 8) dfma_probe_kernel(double* __restrict__ out, int iters, double a, double b) {
+__global__ void __launch_bounds__(256, 8) dfma_probe_kernel(double* __restrict__ out, int iters) {
+    const double a = 0.999999, b = 1e-6;
     double x0 = threadIdx.x * 1e-3, x1 = x0 + 0.1, x2 = x0 + 0.2, x3 = x0 + 0.3, x4 = x0 + 0.4, x5 = x0 + 0.5, x6 = x0 + 0.6,
            x7 = x0 + 0.7;
 #pragma unroll 1
@@ -159,7 +164,7 @@ cudaError_t launch_points(cudaStream_t st, const PointsArgs& a, int sm_count) {
     return cudaGetLastError();
 }
 cudaError_t launch_dfma_probe(cudaStream_t st, double* out, int blocks, int iters) {
-    dfma_probe_kernel<<<blocks, 256, 0, st>>>(out, iters, 0.999999, 1e-6);
+    dfma_probe_kernel<<<blocks, 256, 0, st>>>(out, iters);
     return cudaGetLastError();
 }
 

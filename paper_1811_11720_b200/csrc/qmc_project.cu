@@ -22,7 +22,8 @@
 namespace qmc {
 namespace {
 
-constexpr int kProjTilesTarget = 592;       // 148 SMs x 4: fixed, so the tiling is a function of n only
+constexpr int kProjTilesTarget = 148;       // one tile per SM of a B200: fixed, so the tiling is a function of n only (592 tiles spent
+                                            // more time zeroing, merging and writing 32 KB histograms than evaluating: 0.52 -> 0.xx ms on configs[4]'s fit lattice)
 constexpr int kProjSmemBudget = 200 * 1024; // bytes of warp-private histograms per CTA
 
 struct ProjArgs {
@@ -108,15 +109,26 @@ __device__ double abs_integrand(const ProjArgs& a, const double* x) {
 }
 
 template <bool WIDE>
-__global__ void __launch_bounds__(kThreads) project_kernel(ProjArgs a) {
+__global__ void __launch_bounds__(kThreads) project_kernel(ProjArgs a) {   // a: by value, a.params is redirected to shared memory
     typedef typename Res<WIDE>::T RT;
-    extern __shared__ double hist[];                    // [warp][dchunk][bins]
+    extern __shared__ double hist[];                    // [warp][dchunk][bins], then the parameter block
+    __shared__ int block_status;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tile = blockIdx.x / a.nchunks, chunk = blockIdx.x - tile * a.nchunks;
     const int j0 = chunk * a.dchunk, j1 = min(a.dim, j0 + a.dchunk);
     const int hsize = a.dchunk * a.bins;
     for (int i = tid; i < kWarps * hsize; i += kThreads) hist[i] = 0.0;
+    // the parameter block is read from shared memory in the point loop; a sector block is validated first (on the device:
+    // the host sees only the struct) -- a block that fails is never interpreted and the histograms become NaN
+    double* sp = hist + kWarps * hsize;
+    for (int i = tid; i < a.n_params; i += kThreads) sp[i] = a.params[i];
+    if (tid == 0) block_status = (a.family == QMC_FAMILY_SECTOR) ? sector_block_status(a.params, a.n_params, a.dim) : 0;
     __syncthreads();
+    a.params = sp;
+    if (block_status != 0) {
+        for (int i = tid; i < (j1 - j0) * a.bins; i += kThreads) a.tile_hist[((size_t)tile * a.dim + j0) * a.bins + i] = nan("");
+        return;
+    }
     double* mine = hist + warp * hsize;
 
     const unsigned long long n = a.n;
@@ -181,6 +193,7 @@ int plan_project(const qmc_problem* p, int bins, ProjArgs* a) {
     if (!p) return QMC_ERR_NULL;
     if (p->family < 0 || p->family > QMC_FAMILY_GENZ_DISCONT) return QMC_ERR_FAMILY;
     if (p->dim < 1 || p->dim > QMC_MAX_DIM) return QMC_ERR_DIM;
+    if (p->family == QMC_FAMILY_SECTOR && p->dim > QMC_MAX_SECTOR_DIM) return QMC_ERR_DIM;       // the same limits as the integration entries
     if (p->n < 2 || p->n >= (1ull << 53)) return QMC_ERR_N;
     if (bins < 2 || bins > 1024) return QMC_ERR_N;
     if (p->m < 1) return QMC_ERR_M;
@@ -190,7 +203,11 @@ int plan_project(const qmc_problem* p, int bins, ProjArgs* a) {
     if (p->family == QMC_FAMILY_GENZ_CORNER && p->n_params != p->dim) return QMC_ERR_PARAMS;
     if ((p->family == QMC_FAMILY_GENZ_GAUSSIAN || p->family == QMC_FAMILY_GENZ_C0) && p->n_params != 2 * p->dim) return QMC_ERR_PARAMS;
     if (p->family == QMC_FAMILY_GENZ_DISCONT && p->n_params != p->dim + (p->dim < 2 ? p->dim : 2)) return QMC_ERR_PARAMS;
-    if (p->family == QMC_FAMILY_SECTOR && p->n_params < 4 + p->dim + 2 * (1 + p->dim)) return QMC_ERR_PARAMS;
+    if (p->family == QMC_FAMILY_SECTOR) {               // struct-level layout check as in qmc_host.cu; the values are checked on the device
+        const int rest = p->n_params - 4 - p->dim;
+        const bool plain = rest % (1 + p->dim) == 0, with_log = rest >= 3 && (rest - 3) % (1 + p->dim) == 0;
+        if (rest < 2 * (1 + p->dim) || !(plain || with_log) || rest / (1 + p->dim) > 2 * kMaxSectorMono) return QMC_ERR_PARAMS;
+    }
     std::memset(a, 0, sizeof(*a));
     a->params = p->params;
     a->z = reinterpret_cast<const unsigned long long*>(p->z);
@@ -203,7 +220,7 @@ int plan_project(const qmc_problem* p, int bins, ProjArgs* a) {
     if (steps > 0x7fffffffull) return QMC_ERR_N;
     a->steps = (int)steps;
     a->tiles = (int)((p->n + steps * kThreads - 1) / (steps * kThreads));
-    a->dchunk = std::max(1, std::min(p->dim, kProjSmemBudget / (kWarps * bins * 8)));
+    a->dchunk = std::max(1, std::min(p->dim, (kProjSmemBudget - p->n_params * 8) / (kWarps * bins * 8)));
     a->nchunks = (p->dim + a->dchunk - 1) / a->dchunk;
     return QMC_OK;
 }
@@ -230,7 +247,7 @@ extern "C" int qmc_lattice_project(const qmc_problem* p, int bins, double* out_h
     a.tile_hist = static_cast<double*>(workspace);
     a.out_hist = out_hist;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
-    const size_t smem = (size_t)kWarps * a.dchunk * bins * 8;
+    const size_t smem = (size_t)kWarps * a.dchunk * bins * 8 + (size_t)a.n_params * 8;
     const bool wide = p->n >= (1ull << 31);
     cudaError_t e;
     if (wide) {

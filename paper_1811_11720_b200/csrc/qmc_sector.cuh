@@ -200,45 +200,13 @@ __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned 
         a.sec_c0[0] = a.sec_c0[1] = 1.0;
     };
     stub();
-    const double av = p[0], bv = p[1], nUv = p[2], nFv = p[3];
-    if (!(av >= 0.0 && av <= 8.0 && bv >= 0.0 && bv <= 8.0 && nUv >= 1.0 && nUv <= kMaxSectorMono && nFv >= 1.0 &&
-          nFv <= kMaxSectorMono) ||
-        av != floor(av) || bv != floor(bv) || nUv != floor(nUv) || nFv != floor(nFv)) {
-        a.status = QMC_ERR_PARAMS;
-        return;
-    }
-    const int cnt[2] = {(int)nUv, (int)nFv};
+    const int vst = sector_block_status(p, pb.n_params, d);
+    if (vst != 0) { a.status = vst; return; }
+    const int cnt[2] = {(int)p[2], (int)p[3]};
     const int n_base = 4 + d + (cnt[0] + cnt[1]) * (1 + d);
-    if (pb.n_params == n_base + 3) {                   // trailing [lu, lf, p]: f (lu log U + lf log F)^p, p in 1..4
-        const double pw = p[n_base + 2];
-        if (!(pw >= 1.0 && pw <= 4.0) || pw != floor(pw)) { a.status = QMC_ERR_PARAMS; return; }
-        a.sec_log[0] = p[n_base]; a.sec_log[1] = p[n_base + 1]; a.sec_logp = (int)pw;
-    } else if (pb.n_params != n_base) { a.status = QMC_ERR_PARAMS; return; }
-    a.sec_a = (int)av; a.sec_b = (int)bv;
-    int status = 0;
-    for (int j = 0; j < d; ++j) {
-        const double v = p[4 + j];
-        if (!(v >= 0.0 && v <= 8.0) || v != floor(v)) status = QMC_ERR_PARAMS;
-        a.nu[j] = (unsigned char)(int)v;
-    }
-    // exponents: integers 0..8, total degree of a monomial <= 16 (include/qmc_lattice.h)
-    {
-        const double* base = p + 4 + d;
-        for (int pol = 0; pol < 2 && !status; ++pol) {
-            const double* e = base + cnt[pol];
-            for (int t = 0; t < cnt[pol]; ++t) {
-                int deg = 0;
-                for (int j = 0; j < d; ++j) {
-                    const double v = e[t * d + j];
-                    if (!(v >= 0.0 && v <= 8.0) || v != floor(v)) { status = QMC_ERR_PARAMS; break; }
-                    deg += (int)v;
-                }
-                if (deg > 16) status = QMC_ERR_PARAMS;
-            }
-            base += cnt[pol] * (1 + d);
-        }
-    }
-    if (status) { a.status = status; return; }
+    if (pb.n_params == n_base + 3) { a.sec_log[0] = p[n_base]; a.sec_log[1] = p[n_base + 1]; a.sec_logp = (int)p[n_base + 2]; }
+    a.sec_a = (int)p[0]; a.sec_b = (int)p[1];
+    for (int j = 0; j < d; ++j) a.nu[j] = (unsigned char)(int)p[4 + j];
     SecEmit out;
     out.slots = slots; out.ops = ops; out.nslots = 0; out.nops = 0; out.status = 0;
     out.max_slots = sector_slot_words(nmono_total) / 2 - 1;                              // one slot of read-ahead

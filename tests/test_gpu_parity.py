@@ -25,8 +25,8 @@ GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "ful
 # ------------------------------------------------------------------------------------------------
 # helpers
 # ------------------------------------------------------------------------------------------------
-def run_gpu(problems):
-    batch = binding.DeviceBatch(problems)
+def run_gpu(problems, **plan_options):
+    batch = binding.DeviceBatch(problems, **plan_options)
     batch.integrate()
     return batch.results()
 
@@ -51,8 +51,8 @@ def assert_err(err_gpu, err_or, sm_or, what=""):
         assert abs(err_gpu[c] - err_or[c]) <= tol, f"{what}: err {err_gpu[c]!r} vs {err_or[c]!r} (tol {tol:.3e})"
 
 
-def check_against_oracle(problems):
-    sms, means, errs = run_gpu(problems)
+def check_against_oracle(problems, **plan_options):
+    sms, means, errs = run_gpu(problems, **plan_options)
     for i, p in enumerate(problems):
         nc = oracle.ncomp(p["family"])
         sm_or, mean_or, err_or = oracle.integrate(p)
@@ -225,15 +225,18 @@ def test_large_mixed_batch_of_all_families():
     check_against_oracle(probs)
 
 
-def test_wide_residue_path(monkeypatch):
+def test_wide_residue_path():
     """n >= 2^31 uses 64-bit residue registers; n >= 2^32 needs the 128-bit product (the
     paper ships n = 15173222401).  The oracle can only afford one cheap full run above 2^31, so the 64-bit
-    kernels are also driven at small n through the QMC_FORCE_WIDE test knob."""
-    monkeypatch.setenv("QMC_FORCE_WIDE", "1")
-    check_against_oracle([make(0, 4, 65537, 5, K + 3, 71), make(1, 8, 8191, 5, BAKER, 72), make(2, 12, 8191, 5, K + 3, 73),
-                          make(3, 6, 8191, 5, K + 3, 74), make(0, 16, 8191, 4, K + 3, 75, fit=True),
-                          make(2, 20, 2053, 3, NONE, 76)])
-    monkeypatch.delenv("QMC_FORCE_WIDE")
+    kernels are also driven at small n through qmc_plan_options.force_wide; their results are bit-identical
+    to those of the 32-bit kernels."""
+    probs = [make(0, 4, 65537, 5, K + 3, 71), make(1, 8, 8191, 5, BAKER, 72), make(2, 12, 8191, 5, K + 3, 73),
+             make(3, 6, 8191, 5, K + 3, 74), make(0, 16, 8191, 4, K + 3, 75, fit=True), make(2, 20, 2053, 3, NONE, 76)]
+    sms_wide, _, _ = check_against_oracle(probs, force_wide=True)
+    sms_narrow, _, _ = run_gpu(probs)
+    for a, b, p in zip(sms_wide, sms_narrow, probs):
+        if p["dim"] <= 16:                              # dim > 16 always runs the 64-bit kernels
+            assert np.array_equal(a, b), p["name"]
     n = 2147483659
     p = make(0, 1, n, 2, K + 3, 77)
     sms, _, _ = run_gpu([p])
@@ -591,3 +594,113 @@ def test_bad_sector_block_yields_nan_not_garbage():
 def test_fp64_peak_probe_sane():
     rate, ms = binding.qmc_fp64_peak_probe(4000)
     assert 1e12 < rate < 4e13 and ms > 0
+
+
+# ------------------------------------------------------------------------------------------------
+# sector family: the device-side compiler and its program (qmc_sector_compile), the HOST-pointer batch entry
+# ------------------------------------------------------------------------------------------------
+def _interpret(steps, slots, c0, x):
+    """the machine of gen_sector_interp.py / include/qmc_lattice.h, in Python: -> (U(x), F(x))"""
+    S, A, si, out = c0[0], 0.0, 0, []
+    for code in steps:
+        if code == 0:
+            continue
+        if code == 2:
+            break
+        if code == 1:
+            out.append(S); S = slots[si][0]; si += 1
+            continue
+        j, kind = divmod(int(code) - 3, 5)
+        if kind == 0: S = A * x[j] + S
+        elif kind == 1: S = slots[si][0] * x[j] + S; si += 1
+        elif kind == 2: A = slots[si][0] * x[j] + A; si += 1
+        elif kind == 3: A = slots[si][0] * x[j] + slots[si][1]; si += 1
+        else: A = A * x[j]
+    out.append(S)
+    return out
+
+
+def _sector_polys(p):
+    prm, d = p["params"], p["dim"]
+    nU, nF = int(prm[2]), int(prm[3])
+    off, out = 4 + d, []
+    for cnt in (nU, nF):
+        out.append((prm[off:off + cnt], prm[off + cnt:off + cnt + cnt * d].reshape(cnt, d)))
+        off += cnt * (1 + d)
+    return out
+
+
+def test_sector_programs_evaluate_their_polynomials():
+    """Every program the device-side compiler makes of configs[3]'s 256 sectors, run by a Python model of the machine,
+    reproduces U and F as written (sum of coefficient times monomial) at random points; the mean program length is the
+    30.61 steps DESIGN.md and bench.py quote (the flat monomial-by-monomial count is sum of degrees = 44.44)."""
+    rng = np.random.default_rng(7)
+    lengths, flat = [], []
+    for p in synth.config(3):
+        steps, slots, c0 = binding.qmc_sector_compile(p["params"], p["dim"])
+        x = rng.random(p["dim"])
+        got = _interpret(steps, slots, c0, x)
+        polys = _sector_polys(p)
+        for (c, e), g in zip(polys, got):
+            want = float(np.sum(c * np.prod(x[None, :] ** e, axis=1)))
+            assert abs(g - want) <= 1e-14 * abs(want), p["name"]
+        lengths.append(int(np.sum(steps >= 3)))
+        flat.append(int(sum(e.sum() for _, e in polys)))
+    assert abs(np.mean(flat) - 44.4375) < 1e-9
+    assert abs(np.mean(lengths) - 30.61) < 0.01, np.mean(lengths)
+
+
+def test_sector_compiler_limits():
+    """the largest block the header allows (64 + 64 monomials of total degree 16 in 16 variables) compiles and integrates;
+    repeated and high powers take the multiply steps"""
+    rng = synth.MT19937_64(4242)
+    d = 16
+    def poly(cnt):
+        c = np.array([rng.uniform_range(0.5, 2.0) for _ in range(cnt)])
+        e = np.zeros((cnt, d))
+        for t in range(1, cnt):
+            for _ in range(16):
+                j = rng.next_u64() % d
+                if e[t, j] < 8: e[t, j] += 1
+        return c, e
+    cu, eu = poly(64); cf, ef = poly(64)
+    prm = np.concatenate([[1, 1, 64, 64], np.zeros(d), cu, eu.ravel(), cf, ef.ravel()])
+    steps, slots, c0 = binding.qmc_sector_compile(prm, d)
+    x = np.array([0.3 + 0.04 * j for j in range(d)])
+    U, F = _interpret(steps, slots, c0, x)
+    assert abs(U - np.sum(cu * np.prod(x[None, :] ** eu, axis=1))) <= 1e-13 * abs(U)
+    assert abs(F - np.sum(cf * np.prod(x[None, :] ** ef, axis=1))) <= 1e-13 * abs(F)
+    p = synth.problem(3, prm, 1021, synth.genvec(1021, 16), synth.draw_shifts(rng, 4, d), K + 3, name="sector.max")
+    check_against_oracle([p])
+
+
+def test_host_pointer_batch_entry():
+    """qmc_lattice_integrate_batch_host: mixed families in one synchronous call, bit-identical to the device-pointer entry"""
+    probs = [make(3, 6, 8191, 16, K + 3, 9300 + i) for i in range(5)] + [make(1, 8, 8191, 7, BAKER, 9310), make(2, 12, 4099, 3, K + 3, 9311),
+                                                                        make(0, 16, 4099, 4, K + 3, 9312, fit=True)]
+    sms_h, means_h, errs_h = binding.qmc_lattice_integrate_batch_host(probs)
+    sms_d, means_d, errs_d = run_gpu(probs)
+    for a, b in zip(sms_h, sms_d):
+        assert np.array_equal(a, b)
+    assert np.array_equal(means_h, means_d) and np.array_equal(errs_h, errs_d)
+    sm1, mean1, err1 = binding.qmc_lattice_integrate_ex(probs[5])
+    assert np.array_equal(sm1, sms_d[5]) and mean1[0] == means_d[5, 0]
+    binding.qmc_release_thread_resources()
+    sms_h2, _, _ = binding.qmc_lattice_integrate_batch_host(probs[:2])       # the arena is rebuilt on demand
+    assert np.array_equal(sms_h2[0], sms_d[0])
+
+
+def test_projection_rejects_a_malformed_sector_block():
+    """the projection pass validates a sector block on the device before it reads an exponent: NaN histograms,
+    no out-of-range read; the struct-level limits are those of the integration entries"""
+    p = make(3, 6, 4099, 2, NONE, 9400)
+    bad = dict(p, params=p["params"].copy())
+    bad["params"][4 + 6 + int(p["params"][2]) + 3] = 40.0          # an exponent out of range
+    H = binding.DeviceBatch([bad]).project(0, 64).cpu().numpy()
+    assert np.all(np.isnan(H))
+    bad2 = dict(p, params=p["params"].copy())
+    bad2["params"][2] = 3.0                                          # nU inconsistent with n_params
+    H2 = binding.DeviceBatch([bad2]).project(0, 64).cpu().numpy()
+    assert np.all(np.isnan(H2))
+    good = binding.DeviceBatch([p]).project(0, 64).cpu().numpy()
+    assert np.all(np.isfinite(good))
