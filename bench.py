@@ -7,12 +7,15 @@ fp64 lattice-point integrand evaluations per second, and the fraction of the FP6
 
 A "step" is one pass of the whole hot path (prepare, fused persistent kernel,
 finalize) over one batch of synthetic input through the C ABI (qmc_lattice_integrate_batch).  The headline
-workload is BASELINE.json configs[1]; configs[0], [2], [3], [4] are timed too and reported under "others".
-Inputs are seeded and synthetic (paper_1811_11720_b200.synth).
+workload is the largest single-GPU configuration, BASELINE.json configs[4] (2.15e10 evaluations per step); configs[1],
+[2], [3] carry the same roofline record under "roofline_all" (configs[0] is the small parity case) and every config is
+timed under "others".  Inputs are seeded and synthetic (paper_1811_11720_b200.synth).
 
 Multi-GPU: the path has no exchange step: every rank integrates its own
 independent problems (same shapes, rank-specific seeds); weak scaling; the only communication is the
-MAX-reduction of the measured time.  `--impl reference` times the CPU oracle (oracle/) on the host cores.
+MAX-reduction of the measured time.  `python bench.py --gpus N` starts its own N ranks (torch.distributed.run,
+127.0.0.1) when it is not already running under torchrun.  `--impl reference` times the CPU oracle (oracle/) on the
+host cores, on a stated sub-range of the same workload's lattice indices.
 """
 from __future__ import annotations
 
@@ -34,26 +37,30 @@ from paper_1811_11720_b200 import synth  # noqa: E402
 
 METRIC = "fp64 lattice-point integrand evaluations per second"
 UNIT = "evals/s"
-MAIN_CONFIG = 1
+MAIN_CONFIG = 4
+ORACLE_SAMPLE_DIV = 64          # the oracle legs run about 1/64 of the workload's evaluations (oracle_sample)
 
 # Algorithmic FP64-pipe instructions per integrand evaluation (thread level; FMA, MUL, ADD each count 1), derived in
 # DESIGN.md section 5 from the method itself.  Per dimension: coordinate (1 FMA) + wrap/centre (1 ADD) = 2; transform: none 0,
 # baker 1, Korobov-3 7 (c^2, 1/4 - c^2, weight product, 3-term Horner, phi); cubic fit map 6; integrand term: oscillatory 1,
 # product peak 3, complex exp*poly 3.  Per evaluation: Korobov weight 3 (+1 with the fit Jacobian); cos 14 / sincos 21
 # (executed counts of the libdevice fast paths); reciprocal 5; accumulate 1 per component (+1 for the complex amplitude).
-# Sector family: sum of monomial degrees of U and F (mean 44.44 over the 256 seeded sectors) + prefactor (mean 3.04) +
-# powers (a: mean 1.51, b-1: mean 1.50) + weight*numerator 1.  These are the numerators of roofline.achieved; the EXECUTED
-# counts are in profiles/.
+# Sector family: steps of the greedy Horner programs of U and F (mean 30.61 over the 256 seeded sectors, one fp64 instruction per
+# point each: tests/test_gpu_parity.py::test_sector_programs_evaluate_their_polynomials; the monomial-by-monomial count of
+# round 1 was 44.44) + prefactor (mean 3.04) + powers (a: mean 1.51, b: mean 1.50) + weight*numerator 1.  These are the
+# numerators of roofline.achieved (the USEFUL fraction); EXECUTED_FP64_PER_EVAL below gives the issue fraction.
 ALG_FP64_PER_EVAL = {
     0: 4 * (2 + 7 + 1) + 3 + 14 + 1,                                  # 58   d=4 osc, Korobov-3
     1: 8 * (2 + 1 + 3) + 5 + 1,                                       # 54   d=8 product peak, baker
     2: 12 * (2 + 7 + 3) + 3 + 21 + 1 + 2,                             # 171  d=12 complex, Korobov-3
-    3: 6 * (2 + 7) + 3 + 44.44 + 3.04 + 1.51 + 1.50 + 1 + 5 + 1,      # 114.5 d=6 sector, Korobov-3
+    3: 6 * (2 + 7) + 3 + 30.61 + 3.04 + 1.51 + 1.50 + 1 + 5 + 1,      # 100.7 d=6 sector, Korobov-3
     4: 16 * (2 + 7 + 6 + 1) + 4 + 14 + 1,                             # 275  d=16 osc, Korobov-3 + cubic map
 }
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused kernel at full size, from the committed
-# `ncu --set full` capture profiles/r08_fused_full.md (configs[3], [4] were captured at 1/8 size: no full-size figure)
-PROFILED_DRAM_BYTES_PER_LAUNCH = {1: 70400, 2: 122368}
+# thread-level FP64-pipe instructions per evaluation the fused kernels EXECUTE (ncu smsp__inst_executed_pipe_fp64 x 32 / evaluations;
+# profiles/r2_dram_full.md): the conversion of the residues, padded slots and the interpreter's bookkeeping on top of the above
+EXECUTED_FP64_PER_EVAL = {1: 56.05, 2: 171.4, 3: 100.4, 4: 278.25}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused kernel at FULL size (ncu, profiles/r2_dram_full.md)
+PROFILED_DRAM_BYTES_PER_LAUNCH = {1: 70400, 2: 244992, 3: 1202176, 4: 215808}
 FP64_LANES_PER_SM = 64                        # B200 (sm_100): 64 FP64 FMA lanes per SM -> nominal peak
 
 
@@ -73,6 +80,7 @@ def evals_of(problems):
 SHRINK = 1        # --shrink S (profiling runs only): 1/S of the work of every config, same kernels and tile shapes
 
 
+EXTRA_SHIFT_FACTOR = 4  # time-to-target: up to 4 m shifts on the largest lattice
 SECTOR_LOG = False    # --sector-log: configs[3]'s sectors with the log factors of an eps-expansion term (reading C-15)
 # per evaluation on top of configs[3]: 2 logarithms (26 FP64 each: DESIGN.md section 9) + combination 3 + power (mean p - 1 = 1) + product 1
 ALG_FP64_SECTOR_LOG_EXTRA = 2 * 26 + 3 + 1 + 1
@@ -216,19 +224,18 @@ def config4_with_device_fit(binding, probs):
 
 
 def e2e_host_api(binding, probs, reps):
-    """The same metric through the synchronous HOST-pointer C-ABI call (qmc_lattice_integrate_ex): device
-    allocation, host->device copies of the inputs, the kernels, the device->host copy of the results and the
-    synchronisation are all inside the timed region (host wall clock around a blocking call)."""
+    """The same metric through the synchronous HOST-pointer C-ABI call (qmc_lattice_integrate_batch_host; one problem or a
+    whole batch in ONE call): validation, the host->device copy of all inputs from pinned staging memory, the kernels, the
+    device->host copy of the results and the synchronisation are all inside the timed region (host wall clock around a
+    blocking call)."""
     h2d = d2h = 0
     for p in probs:
         h2d += p["params"].nbytes + p["z"].nbytes + p["shifts"].nbytes + (0 if p.get("fit_coeffs") is None else p["fit_coeffs"].nbytes)
-        d2h += (4 + 2 * p["m"]) * 8
-    for p in probs[:2]:
-        binding.qmc_lattice_integrate_ex(p)                 # warm-up (module load, pools)
+    d2h = len(probs) * (4 + 2 * max(p["m"] for p in probs)) * 8
+    binding.qmc_lattice_integrate_batch_host(probs)         # warm-up (module load, staging arena)
     t0 = time.perf_counter()
     for _ in range(reps):
-        for p in probs:
-            binding.qmc_lattice_integrate_ex(p)
+        binding.qmc_lattice_integrate_batch_host(probs)
     dt = (time.perf_counter() - t0) / reps
     return dt, h2d, d2h
 
@@ -311,17 +318,21 @@ def time_to_target(binding, c, probs, epsrel=1e-8):
     error of 1e-8 on the committed lattice ladder, shifts and parameters of configs[c]; earlier lattices are discarded (L357)."""
     p = probs[0]
     ln, lz = synth.ladder(p["dim"], p["n"])
+    # the config's m shifts first, then seeded extra shifts up to 4 m for the shift-extension leg of the iteration (the ladder
+    # ends at the config's own n; PAPER.md L355)
+    rng = synth.MT19937_64(synth.CONFIG_SEED + 900 + c)
+    shifts = np.concatenate([p["shifts"], synth.draw_shifts(rng, EXTRA_SHIFT_FACTOR * p["m"] - p["m"], p["dim"])])
     kw = dict(min_n=1000, min_m=p["m"], epsrel=epsrel, epsabs=0.0, maxeval=2 ** 62, fit_coeffs=p.get("fit_coeffs"))
     binding.qmc_integrate(p["family"], p["params"], p["dim"], p["transform"], ln[:1], lz[:1], p["shifts"], **kw)   # warm-up
     t0 = time.perf_counter()
-    res, st = binding.qmc_integrate(p["family"], p["params"], p["dim"], p["transform"], ln, lz, p["shifts"], **kw)
+    res, st = binding.qmc_integrate(p["family"], p["params"], p["dim"], p["transform"], ln, lz, shifts, **kw)
     dt = time.perf_counter() - t0
     exact = closed_form(c, p["params"])
     est = complex(*res["integral"]) if len(res["integral"]) == 2 else complex(res["integral"][0])
     return {"workload": workload_name(c), "target_rel_err": epsrel, "reached": st == 0, "seconds": dt, "n": res["n"], "m": res["m"],
             "iterations": res["iterations"], "evaluations": res["evaluations"],
             "estimated_rel_err": float(max(res["error"]) / abs(est)), "true_rel_err": abs(est - exact) / abs(exact),
-            "ladder": [int(v) for v in ln]}
+            "max_m": int(shifts.shape[0]), "ladder": [int(v) for v in ln]}
 
 
 def time_to_target_batch(binding, probs, epsrel=1e-8):
@@ -406,17 +417,22 @@ def run_ours(args):
         fused_avg_s = statistics.fmean(fused_ms) * 1e-3
         alg = ALG_FP64_PER_EVAL[c] + (ALG_FP64_SECTOR_LOG_EXTRA if c == 3 and SECTOR_LOG else 0)
         achieved = alg * ev / fused_avg_s
+        executed = EXECUTED_FP64_PER_EVAL.get(c) if not (c == 3 and SECTOR_LOG) else None
         sms, means, errs = batch.results()
-        rec = {"workload": workload_name(c) + (" + log factors (lu log U + lf log F)^p [variant, not a BASELINE config]" if c == 3 and SECTOR_LOG else "") + (f" [SHRUNK x1/{SHRINK} for profiling: not a bench value]" if SHRINK > 1 else ""), "value": aggregate([ev * steps] * world, total_s), "unit": UNIT,
+        rec = {"workload": bench_config(c)["workload"], "value": aggregate([ev * steps] * world, total_s), "unit": UNIT,
                "ms_per_step": total_s / steps * 1e3, "ms_per_step_best": min(step_ms), "steps": steps, "warmup": warmup,
                "evals_per_step_per_gpu": ev, "fused_kernel_ms": fused_avg_s * 1e3,
                "fused_kernel_share_of_step": fused_avg_s * 1e3 * steps / sum(step_ms),
                "gpu_launches_per_step": launches, "plan": batch.plan_info(),
                "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": peak_rate / 1e12, "unit": "Tinst/s (thread-level FP64 instructions)",
-                            "frac": achieved / peak_rate, "traffic": PROFILED_DRAM_BYTES_PER_LAUNCH.get(c) if SHRINK == 1 else None,
-                            "traffic_unit": "bytes per launch (ncu, profiles/r08_fused_full.md); the path is ALU bound, inputs are KBs",
-                            "alg_fp64_inst_per_eval": alg,
-                            "peak_source": "qmc_fp64_peak_probe (DFMA chains) measured in this run",
+                            "frac": achieved / peak_rate,
+                            "frac_is": "USEFUL fraction: algorithmic FP64 instructions per evaluation x evaluations / fused-kernel time / peak",
+                            "issue_frac": None if executed is None else executed * ev / fused_avg_s / peak_rate,
+                            "issue_frac_is": "EXECUTED FP64-pipe instructions per evaluation (ncu, profiles/) x evaluations / fused-kernel time / peak",
+                            "traffic": PROFILED_DRAM_BYTES_PER_LAUNCH.get(c) if SHRINK == 1 and not SECTOR_LOG else None,
+                            "traffic_unit": "dram bytes per launch of the fused kernel at full size (ncu, profiles/r2_dram_full.md); the path is ALU bound, inputs are KBs",
+                            "alg_fp64_inst_per_eval": alg, "executed_fp64_inst_per_eval": executed,
+                            "peak_source": "qmc_fp64_peak_probe measured in this run (DFMA chains with one register multiplicand: FP64-pipe bound, not register-file bound)",
                             "peak_nominal": sm_count * FP64_LANES_PER_SM * 1.965e9 / 1e12},
                "result_mean": [float(v) for v in means[0]], "result_err": [float(v) for v in errs[0]]}
         return rec, probs, (w0, w1)
@@ -426,12 +442,40 @@ def run_ours(args):
     windows.append(w)
     others = []
     if not args.main_only:
-        for c, (k, wu) in {0: (50, 5), 1: (50, 5), 2: (5, 3), 3: (3, 3), 4: (2, 3)}.items():
+        for c, (k, wu) in {0: (50, 5), 1: (50, 5), 2: (10, 3), 3: (5, 3), 4: (3, 3)}.items():
             if c == args.main or (args.others is not None and c not in args.others):
                 continue
             rec, _, w = measure(c, k, wu)
             windows.append(w)
             others.append(rec)
+    # the roofline record of every config of the target (configs[1..4]) at top level
+    roofline_all = {}
+    for rec_c, rec in [(args.main, main)] + [(int(r["workload"].split("]")[0].split("[")[1]), r) for r in others]:
+        if rec_c >= 1:
+            roofline_all[f"configs[{rec_c}]"] = dict(rec["roofline"], fused_kernel_ms=rec["fused_kernel_ms"], ms_per_step=rec["ms_per_step"],
+                                                     evals_per_s=rec["value"], workload=rec["workload"])
+
+    # S10, the projection pass of configs[4] (n_fit lattice, one shift, 256 bins, all 16 dimensions): device time of the two kernels
+    projection = None
+    if rank == 0 and world == 1 and not args.main_only:
+        p4 = rank_problems(4, 0)[0]
+        proj = dict(p4, n=synth.CONFIG4_NFIT, z=synth.genvec(synth.CONFIG4_NFIT, p4["dim"]), transform=synth.TRANSFORM_NONE)
+        pb = binding.DeviceBatch([proj], device=device)
+        for _ in range(3):
+            pb.project(0, synth.PROJECTION_BINS)
+        tms = []
+        for _ in range(10):
+            flush()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            pb.project(0, synth.PROJECTION_BINS, sync=False)
+            e1.record()
+            e1.synchronize()
+            tms.append(e0.elapsed_time(e1))
+        pms = statistics.median(tms)
+        projection = {"workload": f"projection pass of configs[4]: n_fit={synth.CONFIG4_NFIT}, d=16, 1 shift, {synth.PROJECTION_BINS} bins, transform none",
+                      "ms": pms, "evals_per_s": synth.CONFIG4_NFIT / (pms * 1e-3), "histogram_updates_per_s": synth.CONFIG4_NFIT * 16 / (pms * 1e-3),
+                      "note": "project_kernel + project_merge_kernel; shared-memory bound (warp-private histograms, lane-ordered merge), 0.2 % of a configs[4] step"}
 
     # the same step replayed from a CUDA graph (single-problem calls are capturable): launch overhead of small problems
     graphs = []
@@ -468,7 +512,7 @@ def run_ours(args):
 
     # end-to-end through the HOST-pointer entry (rank-local; max over ranks)
     barrier()
-    e2e_reps = max(5, min(args.steps, 50))
+    e2e_reps = max(3, min(args.steps, 50 if main["ms_per_step"] < 10 else 5))
     e2e_s, h2d, d2h = e2e_host_api(binding, main_probs, e2e_reps)
     e2e_s = max_over_ranks(e2e_s)
     sampler.stop()
@@ -477,21 +521,22 @@ def run_ours(args):
     out = {"metric": METRIC, "value": main["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": main["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f64", "data": "synthetic",
-           "config": {"workload": main["workload"], "evals_per_step_per_gpu": main["evals_per_step_per_gpu"],
-                      "l2": "256 MiB buffer written between timed iterations (inputs are KB-sized and stay resident)",
-                      "parallelism": f"replicas x{world} (independent problems per rank, no data-path collective)",
-                      "plan": main["plan"]},
+           "config": bench_config(args.main),
+           "run": {"l2": "256 MiB buffer written between timed iterations (inputs are KB-sized and stay resident)",
+                   "parallelism": f"replicas x{world} (independent problems per rank, no data-path collective)",
+                   "plan": main["plan"], "timed_region_s": main["ms_per_step"] * args.steps * 1e-3},
            "e2e": {"value": aggregate([main["evals_per_step_per_gpu"]] * world, e2e_s), "unit": UNIT, "h2d_bytes_per_step": h2d,
-                   "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3,
-                   "api": "qmc_lattice_integrate_ex (HOST pointers; alloc + H2D + kernels + D2H + sync inside the timed call)"},
+                   "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3, "reps": e2e_reps,
+                   "api": "qmc_lattice_integrate_batch_host (HOST pointers; validation + H2D from pinned staging + kernels + D2H + sync inside the timed call)"},
            "gpu_launches": main["gpu_launches_per_step"] * args.steps,
-           "roofline": main["roofline"], "fused_kernel_ms": main["fused_kernel_ms"],
+           "roofline": main["roofline"], "roofline_all": roofline_all, "projection_pass": projection,
+           "fused_kernel_ms": main["fused_kernel_ms"],
            "fused_kernel_share_of_step": main["fused_kernel_share_of_step"],
            "fp64_peak_probe": {"thread_inst_per_s": peak_rate, "ms": peak_ms, "sm_count": sm_count,
                                "implied_clock_mhz_at_64_lanes": peak_rate / (sm_count * FP64_LANES_PER_SM) / 1e6},
            "clocks": clocks, "others": others, "time_to_rel_err_1e-8": ttt, "cuda_graph": graphs}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        out["cpu_baseline"] = cpu_baseline(args.main, reps=3)
+        out["cpu_baseline"] = cpu_baseline(args.main)
     if rank == 0:
         print(json.dumps(out))
     if dist is not None:
@@ -501,53 +546,146 @@ def run_ours(args):
 # ----------------------------------------------------------------------------------------------------
 # CPU oracle arm (reported baseline; never tuned)
 # ----------------------------------------------------------------------------------------------------
-def cpu_baseline(c, reps):
-    import oracle
+def oracle_problems(c):
+    """the headline workload for the oracle legs; configs[4] takes the fit map the ORACLE derives from its own projection pass"""
     probs = shrunk_config(c)
+    if c == 4:
+        import oracle
+        p = probs[0]
+        proj = dict(p, n=synth.CONFIG4_NFIT, z=synth.genvec(synth.CONFIG4_NFIT, p["dim"]), transform=synth.TRANSFORM_NONE)
+        probs = [dict(p, fit_coeffs=oracle.fit_cubic(oracle.project(proj, synth.PROJECTION_BINS)))]
+    return probs
+
+
+ORACLE_MIN_INDICES = 128 * 65536     # the oracle parallelises over 2^16-index chunks: a sample keeps every host core busy
+
+
+def oracle_sample(probs, div):
+    """The bounded sample of a workload, about 1/div of its evaluations: for a batch of at least div problems every div-th
+    problem on its whole lattice; otherwise lattice indices [0, k_end) of every problem, all shifts, with
+    k_end = min(n, max(ceil(n / div), 128 * 2^16)).  -> list of (problem, k_end)"""
+    if len(probs) >= div:
+        return [(p, p["n"]) for p in probs[::div]]
+    return [(p, min(p["n"], max(-(-p["n"] // div), ORACLE_MIN_INDICES))) for p in probs]
+
+
+def oracle_sample_pass(probs, div):
+    """the oracle as it stands on the bounded sample -> evaluations done"""
+    import oracle
+    done = 0
+    for p, k_end in oracle_sample(probs, div):
+        oracle.shift_sums(p, 0, k_end)
+        done += k_end * p["m"]
+    return float(done)
+
+
+def sample_text(c, div, done):
+    probs = shrunk_config(c)
+    smp = oracle_sample(probs, div)
+    what = (f"every {div}-th problem ({len(smp)} of {len(probs)}) on its whole lattice" if len(probs) >= div
+            else f"lattice indices [0, {smp[0][1]}) of n = {probs[0]['n']}")
+    return (f"{what}, all shifts, of {workload_name(c)}: {done:.3g} of {evals_of(probs):.3g} evaluations per pass; "
+            "throughput = evaluations done / wall time; OpenMP over 2^16-index chunks")
+
+
+def cpu_baseline(c, budget_s=12.0):
+    """The oracle timed on the host cores on a bounded sample of the SAME workload (about 10-30 s), plus the per-core figure of
+    SURVEY 8(d): the same code with OMP_NUM_THREADS=1 on a 1/4096 sub-range, in a child process (the OpenMP runtime reads the
+    variable once)."""
+    import oracle
+    import subprocess
+    probs = oracle_problems(c)
+    passes, done, t0 = 0, 0.0, time.perf_counter()
+    while True:
+        done += oracle_sample_pass(probs, ORACLE_SAMPLE_DIV)
+        passes += 1
+        dt = time.perf_counter() - t0
+        if dt >= budget_s or passes >= 3:
+            break
+    rec = {"value": done / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+           "sample": sample_text(c, ORACLE_SAMPLE_DIV, done / passes) + f"; {passes} pass(es), {dt:.1f} s", "seconds": dt}
+    try:
+        env = dict(os.environ, OMP_NUM_THREADS="1")
+        out = subprocess.run([sys.executable, os.path.abspath(__file__), "--oracle-per-core", str(c)] +
+                             (["--sector-log"] if SECTOR_LOG else []) + (["--shrink", str(SHRINK)] if SHRINK > 1 else []),
+                             env=env, capture_output=True, text=True, timeout=600, check=True).stdout.strip().splitlines()[-1]
+        rec["per_core"] = json.loads(out)
+    except Exception as e:                                   # the per-core figure is an extra; never fail the bench line for it
+        rec["per_core"] = {"unavailable": repr(e)[:200]}
+    return rec
+
+
+def run_oracle_per_core(c):
+    import oracle
+    probs = oracle_problems(c)
+    p = probs[0]                                             # one problem, 4 chunks of 2^16 indices
+    k_end = min(p["n"], 4 * 65536)
     t0 = time.perf_counter()
-    for _ in range(reps):
-        for p in probs:
-            oracle.integrate(p)
-    dt = (time.perf_counter() - t0) / reps
-    return {"value": evals_of(probs) / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-            "sample": f"the full {workload_name(c)} ({evals_of(probs):.3g} evaluations), {reps} repetitions, OpenMP over 2^16-index chunks",
-            "seconds_per_pass": dt}
+    oracle.shift_sums(p, 0, k_end)
+    dt = time.perf_counter() - t0
+    done = float(k_end * p["m"])
+    print(json.dumps({"value": done / dt, "unit": UNIT, "cores": oracle.num_threads(), "seconds": dt,
+                      "sample": f"lattice indices [0, {k_end}) of the first problem of {workload_name(c)}, all shifts ({done:.3g} evaluations); OMP_NUM_THREADS=1"}))
+
+
+def bench_config(c):
+    """the `config` object both arms print: it names the workload and nothing that differs between the arms"""
+    return {"workload": workload_name(c) + (" + log factors (lu log U + lf log F)^p [variant, not a BASELINE config]" if c == 3 and SECTOR_LOG else "")
+            + (f" [SHRUNK x1/{SHRINK} for profiling: not a bench value]" if SHRINK > 1 else ""),
+            "evals_per_step_per_gpu": evals_of(shrunk_config(c))}
 
 
 def run_reference(args):
+    """The reference arm of this tier = the CPU oracle as it stands, on this arm's workload, metric and unit.  A step is one
+    bounded sample of the workload (sample_text); the number of steps is cut so that the run ends within a few minutes."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     import oracle
-    probs = synth.config(MAIN_CONFIG)
-    ev = evals_of(probs)
+    c = args.main
+    probs = oracle_problems(c)
     for _ in range(min(args.warmup, 1)):
-        oracle.integrate(probs[0])
-    times = []
-    for _ in range(args.steps):
+        oracle.shift_sums(probs[0], 0, min(probs[0]["n"], 8 * 65536))
+    times, done, steps = [], 0.0, args.steps
+    i = 0
+    while i < steps:
         t0 = time.perf_counter()
-        for p in probs:
-            oracle.integrate(p)
+        done += oracle_sample_pass(probs, ORACLE_SAMPLE_DIV)
         times.append(time.perf_counter() - t0)
+        i += 1
+        if i == 1:
+            steps = max(1, min(steps, int(150.0 / max(times[0], 1e-3))))     # bounded: the whole run stays within minutes
     total = sum(times)
-    value = ev * args.steps / total
-    sample = f"each step = the full {workload_name(MAIN_CONFIG)} ({ev:.3g} evaluations) on the host cores"
+    value = done / total
+    sample = sample_text(c, ORACLE_SAMPLE_DIV, done / len(times)) + f"; {len(times)} step(s) of one pass each"
     print(json.dumps({"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-                      "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": total / args.steps * 1e3,
+                      "steps": len(times), "warmup": min(args.warmup, 1), "ms_per_step": total / len(times) * 1e3,
                       "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                      "config": {"workload": workload_name(MAIN_CONFIG), "evals_per_step_per_gpu": ev},
+                      "config": bench_config(c),
                       "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
                       "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
                       "gpu_launches": 0}))
 
 
+def spawn_ranks(args):
+    """`python bench.py --gpus N` outside torchrun: start N ranks of this script on this node (127.0.0.1) and pass the line on"""
+    import socket
+    import subprocess
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
-    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--main-only", action="store_true", help="time configs[1] only (skip the 'others' list)")
+    ap.add_argument("--main-only", action="store_true", help="time the headline config only (skip 'others', time-to-target, graphs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--genz-table", action="store_true",
                     help="run the Genz protocol of the paper's Table 1 / Table 2 through qmc_integrate instead of the throughput bench")
@@ -556,16 +694,23 @@ def main():
     ap.add_argument("--shrink", type=int, default=1,
                     help="profiling only: run 1/S of every config's work (fewer sectors / a smaller prime n)")
     ap.add_argument("--main", type=int, default=MAIN_CONFIG, choices=[0, 1, 2, 3, 4],
-                    help="config reported as the headline line (default configs[1]; others are for profiling runs)")
+                    help="config reported as the headline line (default configs[4], the largest single-GPU configuration)")
     ap.add_argument("--others", type=lambda v: [int(x) for x in v.split(",") if x != ""], default=None,
-                    help="comma-separated subset of configs 0,2,3,4 to time besides configs[1] (default: all)")
+                    help="comma-separated subset of the configs to time besides the headline (default: all)")
+    ap.add_argument("--oracle-per-core", type=int, default=None, help=argparse.SUPPRESS)   # child process of cpu_baseline
     args = ap.parse_args()
     global SHRINK, SECTOR_LOG
     SHRINK = max(1, args.shrink)
     SECTOR_LOG = bool(args.sector_log)
+    if args.oracle_per_core is not None:
+        run_oracle_per_core(args.oracle_per_core)
+        return
+    world = int(os.environ.get("WORLD_SIZE", "0"))
+    if world == 0 and args.gpus > 1:
+        spawn_ranks(args)                                    # does not return
+    if world > 0 and world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}")
     if args.impl == "reference":
-        if args.steps > 40:
-            args.steps = 40                                 # bounded: a step is ~1 s of host time
         run_reference(args)
     else:
         if args.warmup < 3:

@@ -302,7 +302,7 @@ class DeviceBatch:
             out.append(sm[i, : p["m"] * nc].reshape(p["m"], nc).copy())
         return out, means, errs
 
-    def project(self, index=0, bins=256, stream=None):
+    def project(self, index=0, bins=256, stream=None, sync=True):
         """qmc_lattice_project for problem `index` -> torch tensor (dim, bins) on the device."""
         torch = self.torch
         p = self.problems[index]
@@ -315,7 +315,10 @@ class DeviceBatch:
         hist = torch.zeros(p["dim"], bins, dtype=torch.float64, device=self.device)
         s = torch.cuda.current_stream(self.device).cuda_stream if stream is None else stream
         _check(lib().qmc_lattice_project(one, int(bins), hist.data_ptr(), ptr, need, s), "qmc_lattice_project")
-        torch.cuda.synchronize(self.device)
+        if sync:
+            torch.cuda.synchronize(self.device)
+        else:
+            self._keep_ws = (ws, hist)                      # stream-ordered: keep the buffers alive until the caller synchronises
         return hist
 
 

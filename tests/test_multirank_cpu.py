@@ -73,3 +73,42 @@ def test_rank0_gets_exactly_the_seeded_config():
     c = bench.rank_problems(2, 3)[0]
     assert c["shifts"].shape == b["shifts"].shape and not np.array_equal(c["shifts"], b["shifts"])
     assert np.all((c["shifts"] >= 0) & (c["shifts"] < 1))
+
+
+def test_gpus_flag_spawns_its_own_ranks(monkeypatch):
+    """`python bench.py --gpus N` outside torchrun starts N ranks of itself on 127.0.0.1 (--gpus was ignored
+    without torchrun); under torchrun a mismatching --gpus is an error."""
+    import subprocess
+    import sys
+    import bench
+    seen = {}
+    monkeypatch.setattr(subprocess, "call", lambda cmd: seen.setdefault("cmd", cmd) and 0)
+    monkeypatch.delenv("WORLD_SIZE", raising=False)
+    monkeypatch.setattr(sys, "argv", ["bench.py", "--gpus", "4", "--steps", "2", "--warmup", "3"])
+    with pytest.raises(SystemExit) as ex:
+        bench.main()
+    assert ex.value.code == 0
+    cmd = seen["cmd"]
+    assert cmd[1:4] == ["-m", "torch.distributed.run", "--nnodes=1"] and "--nproc-per-node=4" in cmd
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1"
+    assert cmd[-6:] == ["--gpus", "4", "--steps", "2", "--warmup", "3"] and cmd[-7].endswith("bench.py")
+    monkeypatch.setenv("WORLD_SIZE", "2")
+    with pytest.raises(SystemExit) as ex:
+        bench.main()
+    assert "WORLD_SIZE" in str(ex.value.code)
+
+
+def test_oracle_sample_keeps_the_cores_busy_and_is_bounded():
+    """the bounded sample of the oracle legs: about 1/64 of the evaluations, never fewer than 128 chunks of 2^16 indices per
+    problem unless the lattice is smaller, whole problems for a batch"""
+    import bench
+    from paper_1811_11720_b200 import synth
+    for c in (1, 2, 3, 4):
+        probs = synth.config(c)
+        smp = bench.oracle_sample(probs, bench.ORACLE_SAMPLE_DIV)
+        done = sum(k * p["m"] for p, k in smp)
+        assert done <= bench.evals_of(probs)
+        if c == 3:
+            assert len(smp) == 4 and all(k == p["n"] for p, k in smp)
+        else:
+            assert smp[0][1] == min(probs[0]["n"], max(-(-probs[0]["n"] // 64), 128 * 65536))
