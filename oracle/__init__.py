@@ -67,7 +67,7 @@ def num_threads() -> int:
 
 
 def ncomp(family: int) -> int:
-    return 2 if family == 2 else 1
+    return 2 if family in (2, 8) else 1
 
 
 def lattice_points(n, z, shift, k0, count):
@@ -101,7 +101,7 @@ def integrand(family, params, x):
     st = lib().oracle_integrand(int(family), _d(params), len(params), len(x), _d(x), _d(out))
     if st:
         raise ValueError(f"oracle_integrand status {st}")
-    return complex(out[0], out[1]) if family == 2 else float(out[0])
+    return complex(out[0], out[1]) if family in (2, 8) else float(out[0])
 
 
 def shift_sums(p, k_begin=0, k_end=None):

@@ -35,6 +35,7 @@
 //
 // Build: g++ -O2 -std=c++17 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/build.py).
 #include <cmath>
+#include <complex>
 #include <cstdint>
 #include <cstring>
 #include <vector>
@@ -46,8 +47,9 @@ namespace {
 
 typedef unsigned __int128 u128;
 
-enum { FAM_OSC = 0, FAM_PRODPEAK = 1, FAM_CEXP = 2, FAM_SECTOR = 3, FAM_CORNER = 4, FAM_GAUSS = 5, FAM_C0 = 6, FAM_DISC = 7 };
-const int FAM_LAST = FAM_DISC;
+enum { FAM_OSC = 0, FAM_PRODPEAK = 1, FAM_CEXP = 2, FAM_SECTOR = 3, FAM_CORNER = 4, FAM_GAUSS = 5, FAM_C0 = 6, FAM_DISC = 7,
+       FAM_CSECTOR = 8 };
+const int FAM_LAST = FAM_CSECTOR;
 // transform ids: Table A.2.  Korobov<r> = 100 + r; Sidi<r> = 200 + r; Korobov<r0,r1> = 1000 + 16 r0 + r1.
 enum { TR_NONE = 0, TR_BAKER = 1, TR_KOROBOV = 100, TR_SIDI = 200, TR_KOROBOV_ASYM = 1000 };
 const int MAX_DIM = 64;
@@ -184,8 +186,45 @@ double sparse_poly(const double* c, const double* e, int count, int dim, const d
 //  5 Genz Gaussian     f = exp(-sum c_j^2 (x_j - w_j)^2)        [c, w]
 //  6 Genz C^0          f = exp(-sum c_j |x_j - w_j|)            [c, w]
 //  7 Genz discontinuous f = 0 if x_1 > w_1 or x_2 > w_2, else exp(sum c_j x_j)   [c, w_1, w_2]
+//  8 complex sector    f = prod x_j^nu_j * U(x)^a / F(x)^b with COMPLEX coefficients: the shape of a sector after the
+//    contour deformation x_j -> x_j - i lambda_j x_j (1 - x_j) dF/dx_j that handles integrable singularities: every
+//    factor of the deformed integrand (U, F, the Jacobian) is a polynomial in the real x with complex coefficients
+//    (reading C-16).  Layout [a, b, nU, nF, nu_1..nu_d, Re cU (nU), Im cU (nU), eU (nU x d), Re cF (nF),
+//    Im cF (nF), eF (nF x d)] and the optional trailing [lu, lf, p]: f * (lu Log U + lf Log F)^p with the principal
+//    branch Log z = log |z| + i arg z, arg in (-pi, pi].
+typedef std::complex<double> cplx;
+
+inline cplx cpow_int(cplx b, int e) { cplx r(1.0, 0.0); for (int i = 0; i < e; ++i) r *= b; return r; }
+
+// sum_t (cre_t + i cim_t) prod_j x_j^e_tj
+inline cplx sparse_cpoly(const double* cre, const double* cim, const double* e, int cnt, int dim, const double* x) {
+    cplx s(0.0, 0.0);
+    for (int t = 0; t < cnt; ++t) {
+        double mon = 1.0;
+        for (int j = 0; j < dim; ++j) mon *= ipow(x[j], (int)e[t * dim + j]);
+        s += cplx(cre[t], cim[t]) * mon;
+    }
+    return s;
+}
+
 inline void integrand(int fam, const double* p, int n_params, int dim, const double* x, double* re, double* im) {
     *im = 0.0;
+    if (fam == FAM_CSECTOR) {
+        int a = (int)p[0], b = (int)p[1], nU = (int)p[2], nF = (int)p[3];
+        const double* nu = p + 4;
+        const double* cUr = nu + dim; const double* cUi = cUr + nU; const double* eU = cUi + nU;
+        const double* cFr = eU + (size_t)nU * dim; const double* cFi = cFr + nF; const double* eF = cFi + nF;
+        double pre = 1.0;
+        for (int j = 0; j < dim; ++j) pre *= ipow(x[j], (int)nu[j]);
+        const cplx U = sparse_cpoly(cUr, cUi, eU, nU, dim, x), F = sparse_cpoly(cFr, cFi, eF, nF, dim, x);
+        cplx f = pre * cpow_int(U, a) / cpow_int(F, b);
+        if (n_params == 4 + dim + (nU + nF) * (2 + dim) + 3) {           // trailing [lu, lf, p], principal branch
+            const double* t = p + n_params - 3;
+            f *= cpow_int(t[0] * std::log(U) + t[1] * std::log(F), (int)t[2]);
+        }
+        *re = f.real(); *im = f.imag();
+        return;
+    }
     if (fam == FAM_OSC) {
         double ph = 2.0 * M_PI * p[0];
         for (int j = 0; j < dim; ++j) ph += p[1 + j] * x[j];
@@ -231,7 +270,7 @@ inline void integrand(int fam, const double* p, int n_params, int dim, const dou
     }
 }
 
-inline int ncomp_of(int fam) { return fam == FAM_CEXP ? 2 : 1; }
+inline int ncomp_of(int fam) { return (fam == FAM_CEXP || fam == FAM_CSECTOR) ? 2 : 1; }
 
 int expected_params(int fam, const double* p, int n_params, int dim) {
     if (fam == FAM_OSC) return 1 + dim;
@@ -239,6 +278,14 @@ int expected_params(int fam, const double* p, int n_params, int dim) {
     if (fam == FAM_SECTOR) {
         int nU = (int)p[2], nF = (int)p[3], base = 4 + dim + (nU + nF) * (1 + dim);
         if (n_params == base + 3) {                                        // trailing [lu, lf, p], p a small positive integer
+            const double pw = p[base + 2];
+            return (pw >= 1.0 && pw <= 4.0 && pw == std::floor(pw)) ? n_params : -1;
+        }
+        return base;
+    }
+    if (fam == FAM_CSECTOR) {
+        int nU = (int)p[2], nF = (int)p[3], base = 4 + dim + (nU + nF) * (2 + dim);
+        if (n_params == base + 3) {
             const double pw = p[base + 2];
             return (pw >= 1.0 && pw <= 4.0 && pw == std::floor(pw)) ? n_params : -1;
         }

@@ -183,6 +183,29 @@ def sector_log(rng, d, **kw):
     return np.concatenate([prm, np.array([lu, lf, float(pw)])])
 
 
+FAMILY_SECTOR_COMPLEX = 8
+
+
+def sector_complex(rng, d, lam=0.5, log_block=False, **kw):
+    """Complex sector integrand (family 8): the shape of a sector after contour deformation -- polynomials in the real x with
+    complex coefficients (reading C-16).  The real sector recipe gives exponents and real parts; then, in layout
+    order, Im cU_t = Re cU_t * U[-lam, lam) and Im cF_t = -Re cF_t * U[0.1 lam, lam): Im F < 0 on the whole cube (the
+    Feynman prescription F - i delta after deformation), so F has no zero.  Layout
+    [a, b, nU, nF, nu_j, Re cU, Im cU, eU, Re cF, Im cF, eF] (+ [lu, lf, p])."""
+    prm = sector(rng, d, **kw)
+    nU, nF = int(prm[2]), int(prm[3])
+    off = 4 + d
+    cU, eU = prm[off:off + nU], prm[off + nU:off + nU + nU * d]
+    off += nU * (1 + d)
+    cF, eF = prm[off:off + nF], prm[off + nF:off + nF + nF * d]
+    iU = np.array([c * rng.uniform_range(-lam, lam) for c in cU])
+    iF = np.array([-c * rng.uniform_range(0.1 * lam, lam) for c in cF])
+    out = np.concatenate([prm[:4 + d], cU, iU, eU, cF, iF, eF])
+    if log_block:
+        out = np.concatenate([out, [rng.uniform_range(0.5, 2.0), rng.uniform_range(-3.0, -1.0), float(1 + rng.next_u64() % 3)]])
+    return out
+
+
 def problem(family, params, n, z, shifts, transform, fit_coeffs=None, name=""):
     shifts = np.ascontiguousarray(shifts, dtype=np.float64)
     return {"name": name, "family": int(family), "params": np.ascontiguousarray(params, dtype=np.float64),

@@ -561,3 +561,128 @@ def test_fullsize_goldens_are_what_the_live_oracle_computes():
     assert [float(v).hex() for v in np.asarray(sm).ravel()] == rec["shift_means"]
     assert [float(v).hex() for v in np.asarray(mean).ravel()] == rec["mean"]
     assert [float(v).hex() for v in np.asarray(err).ravel()] == rec["err"]
+
+
+# ------------------------------------------------------------------------------------------------
+# family 8: sector polynomials with COMPLEX coefficients (contour-deformed shape; reading C-16)
+# ------------------------------------------------------------------------------------------------
+def csector(a, b, nu, U, F, log_block=None):
+    """U, F: lists of (complex coefficient, exponent tuple) -> parameter block of family 8"""
+    d = len(nu)
+    out = [float(a), float(b), float(len(U)), float(len(F))] + [float(v) for v in nu]
+    for poly in (U, F):
+        out += [complex(c).real for c, _ in poly] + [complex(c).imag for c, _ in poly]
+        for _, e in poly:
+            assert len(e) == d
+            out += [float(v) for v in e]
+    if log_block is not None:
+        out += [float(v) for v in log_block]
+    return np.array(out)
+
+
+def gl_integral(prm, d, order=40):
+    """tensor Gauss-Legendre of the oracle's integrand over the unit cube (d <= 2)"""
+    xs, ws = np.polynomial.legendre.leggauss(order)
+    xs, ws = 0.5 * (xs + 1.0), 0.5 * ws
+    tot = 0.0 + 0.0j
+    if d == 1:
+        for x, w in zip(xs, ws):
+            tot += w * oracle.integrand(8, prm, [x])
+    else:
+        for x0, w0 in zip(xs, ws):
+            for x1, w1 in zip(xs, ws):
+                tot += w0 * w1 * oracle.integrand(8, prm, [x0, x1])
+    return tot
+
+
+def test_complex_sector_one_dimensional_closed_forms():
+    """int_0^1 1/(1+ix) = pi/4 - i ln2/2;  int 1/(1+ix)^2 = (1-i)/2;  int x/(1+ix)^2 = (1-ln2)/2 - i (pi/4 - 1/2);
+    int (1+ix)^2 = 2/3 + i  -- which coefficient is the imaginary part, the powers a and b, the prefactor x^nu, the division"""
+    one = [(1.0, (0,))]
+    lin = [(1.0, (0,)), (1j, (1,))]
+    ln2 = math.log(2.0)
+    cases = [(csector(0, 1, [0], one, lin), math.pi / 4 - 0.5j * ln2),
+             (csector(0, 2, [0], one, lin), 0.5 - 0.5j),
+             (csector(0, 2, [1], one, lin), 0.5 * (1.0 - ln2) - 1j * (math.pi / 4 - 0.5)),
+             (csector(2, 0, [0], lin, one), 2.0 / 3.0 + 1j),
+             (csector(1, 1, [0], [(2.0 - 1j, (0,))], [(0.5j, (0,))]), (2.0 - 1j) / 0.5j)]     # constants: complex division alone
+    for prm, exact in cases:
+        got = gl_integral(prm, 1)
+        assert abs(got - exact) <= 1e-13 * abs(exact), (got, exact)
+
+
+def test_complex_sector_two_dimensional_product():
+    """F = (1 + i x0)(1 + i x1) = 1 + i x0 + i x1 - x0 x1 (a negative real and two imaginary coefficients):
+    int int 1/F = (pi/4 - i ln2/2)^2;  with a = 1, U = 1 + i x0: int int U/F = pi/4 - i ln2/2"""
+    F = [(1.0, (0, 0)), (1j, (1, 0)), (1j, (0, 1)), (-1.0, (1, 1))]
+    v = math.pi / 4 - 0.5j * math.log(2.0)
+    assert abs(gl_integral(csector(0, 1, [0, 0], [(1.0, (0, 0))], F), 2) - v * v) <= 1e-13
+    assert abs(gl_integral(csector(1, 1, [0, 0], [(1.0, (0, 0)), (1j, (1, 0))], F), 2) - v) <= 1e-13
+
+
+@pytest.mark.parametrize("lam", [0.0, 0.3, 1.0, 2.5])
+def test_complex_sector_cauchy_invariance_under_contour_deformation(lam):
+    """The deformation z = x - i lam x (1 - x) dF/dx of int_0^1 dx / (c + x)^2 and of int int dx0 dx1 / (c + x0 + x1)^2 (x0
+    deformed): every factor becomes a polynomial in the real x with complex coefficients (reading C-16), and by Cauchy's
+    theorem the integral keeps its value 1/c - 1/(1+c), ln((c+1)^2 / (c (c+2))) for every lam."""
+    c = 0.7
+    U1 = [(1.0 - 1j * lam, (0,)), (2j * lam, (1,))]                          # Jacobian 1 - i lam (1 - 2x)
+    F1 = [(c, (0,)), (1.0 - 1j * lam, (1,)), (1j * lam, (2,))]               # c + z
+    got = gl_integral(csector(1, 2, [0], U1, F1), 1, order=60)
+    assert abs(got - (1.0 / c - 1.0 / (1.0 + c))) <= 1e-12
+    U2 = [(1.0 - 1j * lam, (0, 0)), (2j * lam, (1, 0))]
+    F2 = [(c, (0, 0)), (1.0 - 1j * lam, (1, 0)), (1j * lam, (2, 0)), (1.0, (0, 1))]
+    got2 = gl_integral(csector(1, 2, [0, 0], U2, F2), 2, order=60)
+    assert abs(got2 - math.log((c + 1.0) ** 2 / (c * (c + 2.0)))) <= 1e-12
+
+
+def test_complex_sector_log_factor_takes_the_principal_branch():
+    """int_0^1 Log(1 + i x) dx and int_0^1 Log(-1 - i x) dx from the antiderivative (z Log z - z)/z' with arg in (-pi, pi]
+    (the second path lies in the third quadrant: arg -> -pi, not +pi); a squared logarithm against scipy quadrature"""
+    import cmath
+    one = [(1.0, (0,))]
+    G = lambda z: z * cmath.log(z) - z
+    prm = csector(0, 0, [0], [(1.0, (0,)), (1j, (1,))], one, log_block=[1.0, 0.0, 1])
+    assert abs(gl_integral(prm, 1, order=60) - (G(1 + 1j) - G(1 + 0j)) / 1j) <= 1e-13
+    prm = csector(0, 0, [0], one, [(-1.0, (0,)), (-1j, (1,))], log_block=[0.0, 1.0, 1])
+    exact = (G(-1 - 1j) - (-1.0) * complex(0.0, -math.pi) - 1.0) / (-1j)       # G(-1 - i0+) = (-1)(-i pi) + 1
+    got = gl_integral(prm, 1, order=200)
+    assert abs(got - exact) <= 1e-9 * abs(exact), (got, exact)                 # the integrand has a log kink at the end point
+    assert got.imag < -2.0                                                     # arg near -pi: the other branch would give > +2
+    prm = csector(1, 1, [0], [(1.0, (0,)), (0.5j, (1,))], [(2.0, (0,)), (-1j, (1,))], log_block=[0.7, -1.3, 2])
+    f = lambda x: (1 + 0.5j * x) / (2 - 1j * x) * (0.7 * cmath.log(1 + 0.5j * x) - 1.3 * cmath.log(2 - 1j * x)) ** 2
+    re = scipy.integrate.quad(lambda x: f(x).real, 0, 1, epsabs=1e-14, epsrel=1e-14)[0]
+    im = scipy.integrate.quad(lambda x: f(x).imag, 0, 1, epsabs=1e-14, epsrel=1e-14)[0]
+    assert abs(gl_integral(prm, 1) - complex(re, im)) <= 1e-13
+
+
+def test_complex_sector_with_real_coefficients_is_the_real_sector():
+    """imaginary parts zero: the value is that of family 3 for the same polynomials (and the imaginary part vanishes)"""
+    rng = synth.MT19937_64(8801)
+    for d in (2, 4, 6):
+        prm3 = synth.sector(rng, d)
+        nU, nF = int(prm3[2]), int(prm3[3])
+        off = 4 + d
+        cU, eU = prm3[off:off + nU], prm3[off + nU:off + nU + nU * d]
+        off += nU * (1 + d)
+        cF, eF = prm3[off:off + nF], prm3[off + nF:off + nF + nF * d]
+        prm8 = np.concatenate([prm3[:4 + d], cU, np.zeros(nU), eU, cF, np.zeros(nF), eF])
+        for _ in range(20):
+            x = np.array([rng.uniform() for _ in range(d)])
+            v3, v8 = oracle.integrand(3, prm3, x), oracle.integrand(8, prm8, x)
+            assert abs(v8.real - v3) <= 4e-16 * abs(v3) and v8.imag == 0.0
+
+
+def test_complex_sector_whole_rule():
+    """Eq. 2-3 with family 8: the lam-deformed one-dimensional integral through the lattice rule (Korobov 3, baker, none)
+    lands on 1/c - 1/(1+c) inside its error bars; both components get an error estimate"""
+    c, lam = 0.7, 0.8
+    prm = csector(1, 2, [0], [(1.0 - 1j * lam, (0,)), (2j * lam, (1,))], [(c, (0,)), (1.0 - 1j * lam, (1,)), (1j * lam, (2,))])
+    rng = synth.MT19937_64(8802)
+    exact = 1.0 / c - 1.0 / (1.0 + c)
+    for tr in (K3, synth.TRANSFORM_BAKER):
+        p = synth.problem(8, prm, 65537, [1], synth.draw_shifts(rng, 16, 1), tr)
+        sm, mean, err = oracle.integrate(p)
+        assert sm.shape == (16, 2) and err.shape == (2,)
+        assert abs(mean[0] - exact) <= 6 * err[0] + 1e-12 and abs(mean[1]) <= 6 * err[1] + 1e-12
+        assert abs(mean[0] - exact) < 1e-7
