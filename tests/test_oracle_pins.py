@@ -670,7 +670,7 @@ def test_complex_sector_with_real_coefficients_is_the_real_sector():
         for _ in range(20):
             x = np.array([rng.uniform() for _ in range(d)])
             v3, v8 = oracle.integrand(3, prm3, x), oracle.integrand(8, prm8, x)
-            assert abs(v8.real - v3) <= 4e-16 * abs(v3) and v8.imag == 0.0
+            assert abs(v8.real - v3) <= 2e-15 * abs(v3) and v8.imag == 0.0      # complex division rounds differently by ulps
 
 
 def test_complex_sector_whole_rule():
