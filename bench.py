@@ -240,6 +240,42 @@ def e2e_host_api(binding, probs, reps):
     return dt, h2d, d2h
 
 
+def variant_workloads():
+    """-> [(label, problems, algorithmic FP64 instructions per evaluation, timed steps)]: workloads outside BASELINE.json's configs
+    that exercise the generic tile loop (every transform of Table A.2 other than none / baker / Korobov-3, pole-term fit, P:L1054-L1060,
+    Eq. 19) and the complex sector family (reading C-16), on the shapes of configs[2], [4] (at n / 8) and [3]."""
+    K, S, KA = synth.TRANSFORM_KOROBOV, synth.TRANSFORM_SIDI, synth.TRANSFORM_KOROBOV_ASYM
+    out = []
+    p2 = synth.config(2)[0]
+    d = p2["dim"]
+    fam2 = 3 * d + 21 + 1 + 2                           # integrand terms, sincos, accumulate, amplitude (as configs[2])
+    for name, tr, per_coord, per_point in [("Korobov r=1", K + 1, 2 + 5, 1), ("Korobov r=2", K + 2, 2 + 6, 2),
+                                           ("Korobov (5,3)", KA + 16 * 5 + 3, 2 + 21.5, 1), ("Sidi r=3", S + 3, 2 + 38, 1)]:
+        out.append((f"configs[2] shape (d=12 complex exp*poly, n={p2['n']}, m={p2['m']}) with {name} [variant]",
+                    [dict(p2, transform=tr, name=f"cfg2.{name}")], d * per_coord + per_point + fam2, 5))
+    from paper_1811_11720_b200 import cbc
+    n4 = synth.CONFIG_SHAPES[4][1] // 8
+    while not cbc.is_prime(n4):
+        n4 -= 1
+    p4 = synth.config(4, n_override=n4)[0]
+    rng = synth.MT19937_64(synth.CONFIG_SEED + 4040)
+    fit = np.array([[1.001 + 0.5 * rng.uniform(), -0.001 - 0.5 * rng.uniform(), 0.25 * rng.uniform(), 0.25 * rng.uniform(),
+                     0.45 + 0.3 * rng.uniform(), 0.2 * rng.uniform() - 0.05] for _ in range(p4["dim"])])
+    # pole terms: two reciprocals (5 + 1 each), k q, y e, a e q: 2 x (6 + 1 + 1 + 2) = 20 on top of the cubic map's 6
+    out.append((f"configs[4] shape at n/8 (d=16 oscillatory, n={n4}, m={p4['m']}) with the complete fit function of Eq. 19 (pole terms) [variant]",
+                [dict(p4, fit_coeffs=fit, name="cfg4.polefit")], 16 * (2 + 7 + 6 + 20 + 1) + 4 + 14 + 1, 3))
+    probs = []
+    for i in range(256):
+        rng = synth.MT19937_64(synth.SECTOR_SEED + 20000 + i)
+        prm = synth.sector_complex(rng, 6)
+        q = synth.config(3, count_override=1)[0]
+        probs.append(dict(q, family=synth.FAMILY_SECTOR_COMPLEX, params=prm, shifts=synth.draw_shifts(rng, q["m"], 6), name=f"csector{i}"))
+    # coordinates 6 x 9 + weight 3; complex Horner programs 2 x 30.6; prefactor 3; U^a 1.5 x 4; F^b 2.5 x 4; division 13; accumulate 2
+    out.append(("configs[3] shape (256 sectors, d=6, n=4194301, m=16) with complex coefficients: family 8, contour-deformed shape [variant]",
+                probs, 6 * 9 + 3 + 2 * 30.6 + 3 + 6 + 10 + 13 + 2, 3))
+    return out
+
+
 def closed_form(c, prm):
     """exact integrals of the closed-form configs (Genz families 1, 2: PAPER.md L709-L713; complex exp*poly): analysis only"""
     d = synth.CONFIG_SHAPES[c][0]
@@ -406,6 +442,12 @@ def run_ours(args):
         probs = rank_problems(c, rank)
         if c == 4:
             probs = config4_with_device_fit(binding, probs)
+        alg = ALG_FP64_PER_EVAL[c] + (ALG_FP64_SECTOR_LOG_EXTRA if c == 3 and SECTOR_LOG else 0)
+        executed = EXECUTED_FP64_PER_EVAL.get(c) if not (c == 3 and SECTOR_LOG) else None
+        traffic = PROFILED_DRAM_BYTES_PER_LAUNCH.get(c) if SHRINK == 1 and not SECTOR_LOG else None
+        return measure_probs(bench_config(c)["workload"], probs, alg, executed, traffic, steps, warmup)
+
+    def measure_probs(label, probs, alg, executed, traffic, steps, warmup):
         batch = binding.DeviceBatch(probs, device=device)
         barrier()
         w0 = time.perf_counter()
@@ -415,11 +457,9 @@ def run_ours(args):
         total_s = max_over_ranks(sum(step_ms) * 1e-3)
         ev = evals_of(probs)
         fused_avg_s = statistics.fmean(fused_ms) * 1e-3
-        alg = ALG_FP64_PER_EVAL[c] + (ALG_FP64_SECTOR_LOG_EXTRA if c == 3 and SECTOR_LOG else 0)
         achieved = alg * ev / fused_avg_s
-        executed = EXECUTED_FP64_PER_EVAL.get(c) if not (c == 3 and SECTOR_LOG) else None
         sms, means, errs = batch.results()
-        rec = {"workload": bench_config(c)["workload"], "value": aggregate([ev * steps] * world, total_s), "unit": UNIT,
+        rec = {"workload": label, "value": aggregate([ev * steps] * world, total_s), "unit": UNIT,
                "ms_per_step": total_s / steps * 1e3, "ms_per_step_best": min(step_ms), "steps": steps, "warmup": warmup,
                "evals_per_step_per_gpu": ev, "fused_kernel_ms": fused_avg_s * 1e3,
                "fused_kernel_share_of_step": fused_avg_s * 1e3 * steps / sum(step_ms),
@@ -429,7 +469,7 @@ def run_ours(args):
                             "frac_is": "USEFUL fraction: algorithmic FP64 instructions per evaluation x evaluations / fused-kernel time / peak",
                             "issue_frac": None if executed is None else executed * ev / fused_avg_s / peak_rate,
                             "issue_frac_is": "EXECUTED FP64-pipe instructions per evaluation (ncu, profiles/) x evaluations / fused-kernel time / peak",
-                            "traffic": PROFILED_DRAM_BYTES_PER_LAUNCH.get(c) if SHRINK == 1 and not SECTOR_LOG else None,
+                            "traffic": traffic,
                             "traffic_unit": "dram bytes per launch of the fused kernel at full size (ncu, profiles/r2_dram_full.md); the path is ALU bound, inputs are KBs",
                             "alg_fp64_inst_per_eval": alg, "executed_fp64_inst_per_eval": executed,
                             "peak_source": "qmc_fp64_peak_probe measured in this run (DFMA chains with one register multiplicand: FP64-pipe bound, not register-file bound)",
@@ -448,6 +488,15 @@ def run_ours(args):
             rec, _, w = measure(c, k, wu)
             windows.append(w)
             others.append(rec)
+    # variants beyond the BASELINE configs: the generic transforms and the pole-term fit on configs[2]'s / [4]'s shape, the
+    # complex sector family on configs[3]'s shape.  alg counts: DESIGN.md section 5 ("variants").
+    variants = []
+    if rank == 0 and world == 1 and not args.main_only and (args.others is None or 9 in args.others):
+        for label, probs, alg, k in variant_workloads():
+            rec, _, w = measure_probs(label, probs, alg, None, None, k, 3)
+            windows.append(w)
+            variants.append(rec)
+
     # the roofline record of every config of the target (configs[1..4]) at top level
     roofline_all = {}
     for rec_c, rec in [(args.main, main)] + [(int(r["workload"].split("]")[0].split("[")[1]), r) for r in others]:
@@ -534,7 +583,7 @@ def run_ours(args):
            "fused_kernel_share_of_step": main["fused_kernel_share_of_step"],
            "fp64_peak_probe": {"thread_inst_per_s": peak_rate, "ms": peak_ms, "sm_count": sm_count,
                                "implied_clock_mhz_at_64_lanes": peak_rate / (sm_count * FP64_LANES_PER_SM) / 1e6},
-           "clocks": clocks, "others": others, "time_to_rel_err_1e-8": ttt, "cuda_graph": graphs}
+           "clocks": clocks, "others": others, "variants": variants, "time_to_rel_err_1e-8": ttt, "cuda_graph": graphs}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(args.main)
     if rank == 0:

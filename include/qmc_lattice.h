@@ -53,6 +53,15 @@
  *                               U, F > 0 is the caller's responsibility (a non-positive value gives NaN results).
  *                               Entry points that take n_params accept it; qmc_lattice_integrate, which derives
  *                               n_params from (family, dim, params), reads the block without it.
+ *      QMC_FAMILY_SECTOR_COMPLEX [a, b, nU, nF, nu_1..nu_d, Re cU_1..nU, Im cU_1..nU, eU_{1,1}..eU_{nU,d},
+ *                                 Re cF_1..nF, Im cF_1..nF, eF_{1,1}..eF_{nF,d}]     (complex results)
+ *                               the same f with COMPLEX coefficients on the real cube: the shape of a sector after the
+ *                               contour deformation x_j -> x_j - i lambda_j x_j (1 - x_j) dF/dx_j that handles integrable
+ *                               singularities -- U, F and the Jacobian of the deformed integrand are polynomials
+ *                               in the real x with complex coefficients (reading C-16).  Same limits as
+ *                               QMC_FAMILY_SECTOR; F(x) != 0 on the cube is the caller's responsibility.  Optional
+ *                               trailing [lu, lf, p]: f * (lu Log U + lf Log F)^p with the principal branch
+ *                               Log z = log|z| + i arg z, arg in (-pi, pi].
  */
 #ifndef QMC_LATTICE_H
 #define QMC_LATTICE_H
@@ -83,7 +92,9 @@ typedef enum {
 
 enum { QMC_FAMILY_GENZ_OSC = 0, QMC_FAMILY_GENZ_PRODPEAK = 1, QMC_FAMILY_CEXP_POLY = 2, QMC_FAMILY_SECTOR = 3,
        /* the remaining functions of Genz' test suite: */
-       QMC_FAMILY_GENZ_CORNER = 4, QMC_FAMILY_GENZ_GAUSSIAN = 5, QMC_FAMILY_GENZ_C0 = 6, QMC_FAMILY_GENZ_DISCONT = 7 };
+       QMC_FAMILY_GENZ_CORNER = 4, QMC_FAMILY_GENZ_GAUSSIAN = 5, QMC_FAMILY_GENZ_C0 = 6, QMC_FAMILY_GENZ_DISCONT = 7,
+       /* sector polynomials with complex coefficients (complex results): */
+       QMC_FAMILY_SECTOR_COMPLEX = 8 };
 
 /* Periodizing transforms, Table A.2: none; baker Eq. 17;
  * Korobov with symmetric weight r, Eq. 15: QMC_TRANSFORM_KOROBOV + r, r = 1..6;

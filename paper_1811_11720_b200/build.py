@@ -15,7 +15,8 @@ OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libqmc_lattice.so")
 # (source, extra nvcc defines, object name): the closed-form fused kernels are one source compiled per (family, part)
 SOURCES = [("qmc_host.cu", [], "qmc_host.o"), ("qmc_adaptive.cu", [], "qmc_adaptive.o"), ("qmc_fit.cu", [], "qmc_fit.o"),
-           ("qmc_misc.cu", [], "qmc_misc.o"), ("qmc_project.cu", [], "qmc_project.o"), ("qmc_fused_f3.cu", [], "qmc_fused_f3.o")]
+           ("qmc_misc.cu", [], "qmc_misc.o"), ("qmc_project.cu", [], "qmc_project.o"), ("qmc_fused_f3.cu", [], "qmc_fused_f3.o"),
+           ("qmc_fused_f8.cu", [], "qmc_fused_f8.o")]
 SOURCES += [("qmc_fused_closed.cu", [f"-DQMC_FAM={f}", f"-DQMC_PART={q}"], f"qmc_fused_closed_f{f}_p{q}.o")
             for q in (3, 2, 1, 0) for f in (2, 4, 1, 0)]       # the slowest parts first
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]

@@ -20,6 +20,9 @@ Step kinds, one fp64 instruction per point each:
     AL j : A = fma(cf, x_j, A)           a further leaf of the group
     ALI j: A = fma(cf, x_j, cf2)         first leaf of a group (cf2 = own), or cf * x_j for a plain monomial (cf2 = 0)
     AM j : A = A * x_j                   a prefix variable that is not the last
+The complex family (sector polynomials with complex coefficients on real coordinates, reading C-16) runs the same five kinds
+on paired accumulators (S_re, S_im), (A_re, A_im): two fp64 instructions per point and step, coefficient slots of 32 bytes
+{cf_re, cf_im, cf2_re, cf2_im}.
 Step code = 3 + 5 j + kind; 0 = no-op, 1 = end of a polynomial that is not the last (parks S in the thread's next
 shared-memory column and restarts it with the next polynomial's constant term), 2 = end of program.  SL / AL / ALI and
 the end-of-polynomial step read one 16-byte coefficient slot {cf, cf2} each, in program order.
@@ -34,20 +37,29 @@ made no difference.
 """
 import os
 
-VARIANTS = [(4, 8, 384), (6, 8, 384), (8, 8, 256), (16, 4, 256)]      # (DP, G, threads per CTA) instantiated by qmc_fused_f3.cu
+# (DP, G, threads per CTA, complex) instantiated by qmc_fused_f3.cu (real sectors) and qmc_fused_f8.cu (complex sectors)
+VARIANTS = [(4, 8, 384, False), (6, 8, 384, False), (8, 8, 256, False), (16, 4, 256, False),
+            (4, 4, 384, True), (6, 4, 384, True), (8, 4, 384, True), (16, 2, 384, True)]
 KINDS = 5
 SC, SL, AL, ALI, AM = range(KINDS)
 
 
-def gen(dp, g, nt):
-    # operand numbering: S[q] = %q, x[q][j] = %(g + q*dp + j), then steps address, coefficient address, park address
-    s = lambda q: f"%{q}"
-    x = lambda q, j: f"%{g + q * dp + j}"
-    steps, coefs, upark = (f"%{g + g * dp + i}" for i in range(3))
+def gen(dp, g, nt, cplx):
+    # operand numbering: S[q] = %q (complex: S_re[q] = %q, S_im[q] = %(g+q)), x[q][j] next, then steps address,
+    # coefficient address, park address
+    ns = 2 * g if cplx else g
+    sr = lambda q: f"%{q}"
+    si = lambda q: f"%{g + q}"
+    x = lambda q, j: f"%{ns + q * dp + j}"
+    steps, coefs, upark = (f"%{ns + g * dp + i}" for i in range(3))
+    slot = 32 if cplx else 16
     L = []
     a = L.append
     a("{")
-    a(".reg .f64 " + ", ".join(f"A{q}" for q in range(g)) + ", cfn, cf2n;")
+    if cplx:
+        a(".reg .f64 " + ", ".join(f"A{q}, B{q}" for q in range(g)) + ", cfn, cfni, cf2n, cf2ni;")      # B = Im A
+    else:
+        a(".reg .f64 " + ", ".join(f"A{q}" for q in range(g)) + ", cfn, cf2n;")
     a(".reg .u32 pc, pk, pp, tgt, c0;")
     labels = ["T_NOP", "T_ENDU", "T_END"] + [f"T_{j}_{k}" for j in range(dp) for k in range(KINDS)]
     a("ts: .branchtargets " + ", ".join(labels) + ";")
@@ -56,23 +68,36 @@ def gen(dp, g, nt):
     a(f"mov.u32 pp, {upark};")
     for q in range(g):
         a(f"mov.f64 A{q}, 0d0000000000000000;")
-    a("ld.shared.v2.f64 {cfn, cf2n}, [pk];")
+        if cplx:
+            a(f"mov.f64 B{q}, 0d0000000000000000;")
+
+    def load_slot(off):
+        if cplx:
+            return [f"ld.shared.v2.f64 {{cfn, cfni}}, [pk+{off}];", f"ld.shared.v2.f64 {{cf2n, cf2ni}}, [pk+{off + 16}];"]
+        return [f"ld.shared.v2.f64 {{cfn, cf2n}}, [pk+{off}];"]
+    L.extend(load_slot(0))
     a("ld.shared.u8 tgt, [pc];")
     a("ld.shared.u8 c0, [pc+1];")
     leave = "brx.idx.uni tgt, ts;"
     a(leave)
     # on entry to the case of step i: c0 = code[i+1] has arrived; the branch index of step i+1 is known at entry
     fetch = ["mov.u32 tgt, c0;", "ld.shared.u8 c0, [pc+2];", "add.u32 pc, pc, 1;"]
-    reload = ["ld.shared.v2.f64 {cfn, cf2n}, [pk+16];", "add.u32 pk, pk, 16;"]
+    reload = load_slot(slot) + [f"add.u32 pk, pk, {slot};"]
     a("T_NOP:")
     L.extend(fetch)
     a(leave)
     a("T_ENDU:")
     L.extend(fetch)
     for q in range(g):
-        a(f"st.shared.f64 [pp+{8 * nt * q}], {s(q)};")
-        a(f"mov.f64 {s(q)}, cfn;")
-    a(f"add.u32 pp, pp, {8 * nt * g};")
+        if cplx:
+            a(f"st.shared.f64 [pp+{8 * nt * (2 * q)}], {sr(q)};")
+            a(f"st.shared.f64 [pp+{8 * nt * (2 * q + 1)}], {si(q)};")
+            a(f"mov.f64 {sr(q)}, cfn;")
+            a(f"mov.f64 {si(q)}, cfni;")
+        else:
+            a(f"st.shared.f64 [pp+{8 * nt * q}], {sr(q)};")
+            a(f"mov.f64 {sr(q)}, cfn;")
+    a(f"add.u32 pp, pp, {8 * nt * ns};")
     L.extend(reload)
     a(leave)
     for j in range(dp):
@@ -82,24 +107,41 @@ def gen(dp, g, nt):
             for q in range(g):
                 X = x(q, j)
                 if k == SC:
-                    a(f"fma.rn.f64 {s(q)}, A{q}, {X}, {s(q)};")
+                    a(f"fma.rn.f64 {sr(q)}, A{q}, {X}, {sr(q)};")
+                    if cplx: a(f"fma.rn.f64 {si(q)}, B{q}, {X}, {si(q)};")
                 elif k == SL:
-                    a(f"fma.rn.f64 {s(q)}, cfn, {X}, {s(q)};")
+                    a(f"fma.rn.f64 {sr(q)}, cfn, {X}, {sr(q)};")
+                    if cplx: a(f"fma.rn.f64 {si(q)}, cfni, {X}, {si(q)};")
                 elif k == AL:
                     a(f"fma.rn.f64 A{q}, cfn, {X}, A{q};")
+                    if cplx: a(f"fma.rn.f64 B{q}, cfni, {X}, B{q};")
                 elif k == ALI:
                     a(f"fma.rn.f64 A{q}, cfn, {X}, cf2n;")
+                    if cplx: a(f"fma.rn.f64 B{q}, cfni, {X}, cf2ni;")
                 else:
                     a(f"mul.rn.f64 A{q}, A{q}, {X};")
+                    if cplx: a(f"mul.rn.f64 B{q}, B{q}, {X};")
             if k in (SL, AL, ALI):
                 L.extend(reload)                      # after the last use of the slot: no register moves
             a(leave)
     a("T_END:")
     a("}")
     body = "\n".join(f'        "{line}\\n\\t"' for line in L)
-    outs = ", ".join(f'"+d"(sum[{q}])' for q in range(g))
+    outs = ", ".join([f'"+d"(sum[{q}])' for q in range(g)] + ([f'"+d"(sum_im[{q}])' for q in range(g)] if cplx else []))
     ins = ", ".join([f'"d"(x[{q}][{j}])' for q in range(g) for j in range(dp)] +
                     ['"r"(steps_addr)', '"r"(coefs_addr)', '"r"(park_addr)'])
+    if cplx:
+        return f"""
+template <> __device__ __forceinline__ void csector_interp<{dp}, {g}, {nt}>(const double (&x)[{g}][{dp}], unsigned steps_addr,
+                                                                         unsigned coefs_addr, unsigned park_addr, double (&sum)[{g}],
+                                                                         double (&sum_im)[{g}]) {{
+    asm volatile(
+{body}
+        : {outs}
+        : {ins}
+        : "memory");
+}}
+"""
     return f"""
 template <> __device__ __forceinline__ void sector_interp<{dp}, {g}, {nt}>(const double (&x)[{g}][{dp}], unsigned steps_addr,
                                                                         unsigned coefs_addr, unsigned park_addr, double (&sum)[{g}]) {{
@@ -121,10 +163,17 @@ def main():
            "template <int DP, int G, int NT> __device__ __forceinline__ void sector_interp(const double (&x)[G][DP], unsigned steps_addr,",
            "                                                                               unsigned coefs_addr, unsigned park_addr,",
            "                                                                               double (&sum)[G]);"]
-    for dp, g, nt in VARIANTS:
-        out.append(gen(dp, g, nt))
+    out += ["// complex family: sum / sum_im hold the first polynomial's constant term (re, im) on entry; polynomial p < last is parked at",
+            "// park_addr + 8 NT (2 G p + 2 q + c), c = 0 (re), 1 (im); on return (sum[q], sum_im[q]) = the last polynomial at x_q.",
+            "template <int DP, int G, int NT> __device__ __forceinline__ void csector_interp(const double (&x)[G][DP], unsigned steps_addr,",
+            "                                                                                unsigned coefs_addr, unsigned park_addr,",
+            "                                                                                double (&sum)[G], double (&sum_im)[G]);"]
+    real = [v for v in VARIANTS if not v[3]]
+    cplx = [v for v in VARIANTS if v[3]]
     with open(os.path.join(here, "qmc_sector_interp.inc"), "w") as f:
-        f.write("\n".join(out))
+        f.write("\n".join(out[:7] + [gen(*v) for v in real]))
+    with open(os.path.join(here, "qmc_csector_interp.inc"), "w") as f:
+        f.write("\n".join(out[:2] + out[7:] + [gen(*v) for v in cplx]))
 
 
 if __name__ == "__main__":

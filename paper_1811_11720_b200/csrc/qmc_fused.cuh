@@ -169,6 +169,103 @@ __device__ __forceinline__ void fit_poles(double y, double a0, double k2, double
     dp = __fma_rn(a0 * e0, q0, __fma_rn(a1 * e1, q1, dp));
 }
 
+// x^e for 0 <= e <= 7 without a loop or a branch (e is warp-uniform): squarings and selected multipliers
+__device__ __forceinline__ double ipow_upto7(double x, int e) {
+    const double x2 = x * x, x4 = x2 * x2;
+    double r = (e & 1) ? x : 1.0;
+    r *= (e & 2) ? x2 : 1.0;
+    r *= (e & 4) ? x4 : 1.0;
+    return r;
+}
+
+// The generic tile loop's S3-S4 for ONE dimension and the G shifts of the group: the transform kind and the fit mode are decided
+// once per dimension (warp-uniform branches), the G coordinates inside each branch are straight-line code, so that their
+// dependency chains overlap (a DFMA result takes ~35 cycles; decided per coordinate, as in round 1, the chains ran one after the
+// other and the generic loop reached 17-19 % of the FP64 peak).  Symmetric Korobov weights carry P = prod (1/4 - c^2) and are
+// raised to the power r once per point (point_weight); the others multiply their weight into P directly.
+template <int G>
+__device__ __forceinline__ void generic_coord_group(const double (&t)[G], unsigned kor_addr, int gen, const FitC& fc, double (&x)[G],
+                                                    double (&P)[G], double (&D)[G]) {
+    const int kind = gen & 15, r0 = (gen >> 4) & 15, r1 = (gen >> 8) & 15;
+    if (kind == GEN_NONE) {
+#pragma unroll
+        for (int q = 0; q < G; ++q) x[q] = wrap_u(t[q]);
+    } else if (kind == GEN_BAKER) {
+#pragma unroll
+        for (int q = 0; q < G; ++q) x[q] = 1.0 - fabs(baker_w(t[q]));
+    } else if (kind == GEN_KOROBOV_SYM) {
+        // g_r(s) by a fixed six-step Horner scheme: the table is zero above degree r, and fma(0, s, k) = k exactly
+        double k[7];
+#pragma unroll
+        for (int i = 0; i < 7; ++i) k[i] = lds_f64(kor_addr + 8u * i);
+#pragma unroll
+        for (int q = 0; q < G; ++q) {
+            const double c = centre_c(t[q]);
+            const double s = c * c;
+            P[q] *= (0.25 - s);
+            double g = k[6];
+#pragma unroll
+            for (int i = 5; i >= 0; --i) g = __fma_rn(g, s, k[i]);
+            x[q] = __fma_rn(c, g, 0.5);
+        }
+    } else if (kind == GEN_KOROBOV_ASYM) {
+#pragma unroll
+        for (int q = 0; q < G; ++q) {
+            const double u = wrap_u(t[q]);
+            const double um = 1.0 - u;
+            const bool low = u <= 0.5;
+            const double v = low ? u : um;
+            const unsigned tab = kor_addr + (low ? 0u : 64u);
+            double k[7];
+#pragma unroll
+            for (int i = 0; i < 7; ++i) k[i] = lds_f64(tab + 8u * i);
+            double h = k[6];
+#pragma unroll
+            for (int i = 5; i >= 0; --i) h = __fma_rn(h, v, k[i]);
+            const double ph = ipow_upto7(v, (low ? r0 : r1) + 1) * h;
+            P[q] *= ipow_upto7(u, r0) * ipow_upto7(um, r1);
+            x[q] = low ? ph : 1.0 - ph;
+        }
+    } else {                                                  // Sidi: I_n = ((n-1) I_(n-2) - sin^(n-1) cos) / n from I_0 = pi u, I_1 = 1 - cos
+        const bool even = (r0 & 1) == 0;
+        const double K = lds_f64(kor_addr);
+#pragma unroll
+        for (int q = 0; q < G; ++q) {
+            const double u = wrap_u(t[q]);
+            double sn, cs;
+            sincospi(u, &sn, &cs);
+            const double s2 = sn * sn;
+            double I = even ? 3.141592653589793238462643383279 * u : 1.0 - cs;
+            double sp = even ? sn : s2;                       // sin^(n-1) of the first step (n = 2 or 3)
+            // at most three steps (r <= 6): n = 2, 4, 6 or 3, 5; the divisions by n are multiplications by the constants 1/n
+            const double n0 = even ? 2.0 : 3.0;
+#pragma unroll
+            for (int st = 0; st < 3; ++st) {
+                const double n = n0 + 2.0 * st;
+                const double inv = (st == 0) ? (even ? 0.5 : 1.0 / 3.0) : (st == 1 ? (even ? 0.25 : 0.2) : 1.0 / 6.0);
+                const double In = __fma_rn(n - 1.0, I, -(sp * cs)) * inv;
+                const bool on = n <= (double)r0;
+                I = on ? In : I;
+                sp *= s2;
+            }
+            P[q] *= ipow_upto7(sn, r0);
+            x[q] = K * I;
+        }
+    }
+    if (fc.mode) {                                            // S4: fit map of Eq. 19
+#pragma unroll
+        for (int q = 0; q < G; ++q) {
+            const double y = x[q];
+            const double h = __fma_rn(y, __fma_rn(y, fc.f2, fc.f1), fc.f0);
+            double dp = __fma_rn(y, __fma_rn(y, fc.f4, fc.f3), fc.f0);
+            double xx = y * h;
+            if (fc.mode == 2) fit_poles(y, fc.a0, fc.k2, fc.a1, fc.k3, xx, dp);
+            D[q] *= dp;
+            x[q] = xx;
+        }
+    }
+}
+
 // Returns x_j; multiplies P by u(1-u) (Korobov) and D by p'(y) (fit).
 template <int TR, int FIT>
 __device__ __forceinline__ double point_coord(double rd, double inv_n, double delta, const FitC& fc, unsigned kor_addr,
@@ -208,7 +305,7 @@ __device__ __forceinline__ double point_coord(double rd, double inv_n, double de
 template <int TR, int FIT> __device__ __forceinline__ double point_weight(double P, double D, double wconst, int kor_r) {
     double W = 1.0;
     if (TR == TR_KOR3) W = wconst * (P * P * P);
-    else if (TR == TR_KORR) W = wconst * P;                  // generic transforms carry the full weight product
+    else if (TR == TR_KORR) W = wconst * (((kor_r & 15) == GEN_KOROBOV_SYM) ? ipow_small(P, (kor_r >> 4) & 15) : P);   // symmetric Korobov: P = prod (1/4 - c^2)
     if (FIT) W = (TR == TR_KOR3 || TR == TR_KORR) ? W * D : D;
     return W;
 }
@@ -262,15 +359,24 @@ __device__ __forceinline__ void eval_point_group(const typename Res<WIDE>::T (&r
         double fa, fb, dl[G];
         FitC fc;
         load_slot<DP, G, FIT>(cx.sbase, cx.delta, j, cx.fit_mode, fa, fb, fc, dl);
+        if constexpr (TR == TR_KORR) {                        // generic tile loop: kind and fit mode decided once per dimension
+            double t[G], xg[G];
 #pragma unroll
-        for (int q = 0; q < G; ++q) {
-            if (FAMILY == QMC_FAMILY_GENZ_PRODPEAK && TR == TR_BAKER && !FIT) {
-                // x - w_j = (1 - w_j) - |w| with the slot constant fb = 1 - w_j (derive_slot): the baker map folds into the factor
-                const double dd = fb - fabs(baker_w(coord_t(rd, cx.inv_n, dl[q])));
-                s0[q] *= __fma_rn(dd, dd, fa);
-            } else {
-                const double x = point_coord<TR, FIT>(rd, cx.inv_n, dl[q], fc, cx.sbase + SmemOff<DP, G>::kor, cx.kor_r, P[q], D[q]);
-                fam_dim<FAMILY>(s0[q], s1[q], x, fa, fb, cx.fam_kind);
+            for (int q = 0; q < G; ++q) t[q] = coord_t(rd, cx.inv_n, dl[q]);
+            generic_coord_group<G>(t, cx.sbase + SmemOff<DP, G>::kor, cx.kor_r, fc, xg, P, D);
+#pragma unroll
+            for (int q = 0; q < G; ++q) fam_dim<FAMILY>(s0[q], s1[q], xg[q], fa, fb, cx.fam_kind);
+        } else {
+#pragma unroll
+            for (int q = 0; q < G; ++q) {
+                if (FAMILY == QMC_FAMILY_GENZ_PRODPEAK && TR == TR_BAKER && !FIT) {
+                    // x - w_j = (1 - w_j) - |w| with the slot constant fb = 1 - w_j (derive_slot): the baker map folds into the factor
+                    const double dd = fb - fabs(baker_w(coord_t(rd, cx.inv_n, dl[q])));
+                    s0[q] *= __fma_rn(dd, dd, fa);
+                } else {
+                    const double x = point_coord<TR, FIT>(rd, cx.inv_n, dl[q], fc, cx.sbase + SmemOff<DP, G>::kor, cx.kor_r, P[q], D[q]);
+                    fam_dim<FAMILY>(s0[q], s1[q], x, fa, fb, cx.fam_kind);
+                }
             }
         }
     }

@@ -59,14 +59,14 @@ namespace {
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 int ncomp_of(int family) {
-    if (family == QMC_FAMILY_CEXP_POLY) return 2;
+    if (family == QMC_FAMILY_CEXP_POLY || family == QMC_FAMILY_SECTOR_COMPLEX) return 2;
     if (family >= 0 && family <= QMC_FAMILY_GENZ_DISCONT) return 1;
     return -1;
 }
 
 // dimension slots of the kernel variant that serves (family, dim, residue width); slots beyond dim are padded
 int dim_slots(int family, int dim, bool wide) {
-    if (family == QMC_FAMILY_SECTOR) return dim <= 4 ? 4 : (dim <= 6 ? 6 : (dim <= 8 ? 8 : (dim <= 16 ? 16 : -1)));   // = sector_dim_slots (qmc_sector.cuh)
+    if (is_sector_family(family)) return dim <= 4 ? 4 : (dim <= 6 ? 6 : (dim <= 8 ? 8 : (dim <= 16 ? 16 : -1)));   // = sector_dim_slots (qmc_sector.cuh)
     if (wide) return dim <= 8 ? 8 : (dim <= 16 ? 16 : 32);
     return dim <= 4 ? 4 : (dim <= 6 ? 6 : (dim <= 8 ? 8 : (dim <= 12 ? 12 : (dim <= 16 ? 16 : 32))));
 }
@@ -74,7 +74,7 @@ bool is_wide(unsigned long long n, const qmc_plan_options& o) { return n >= (1ul
 // residue width of the kernel variant: 64-bit for n >= 2^31, and for the 32-slot closed-form kernels (dim > 16), which
 // exist only with wide residues
 bool variant_wide(int family, int dim, unsigned long long n, const qmc_plan_options& o) {
-    return is_wide(n, o) || (family != QMC_FAMILY_SECTOR && dim > 16);
+    return is_wide(n, o) || (!is_sector_family(family) && dim > 16);
 }
 
 // transform id -> tile-loop kind, symmetric Korobov weight r (0 if none) and the generic-transform code
@@ -128,10 +128,10 @@ int validate_struct(const qmc_problem& p, bool need_two_shifts) {
     if (p.family == QMC_FAMILY_GENZ_CORNER && p.n_params != p.dim) return QMC_ERR_PARAMS;
     if ((p.family == QMC_FAMILY_GENZ_GAUSSIAN || p.family == QMC_FAMILY_GENZ_C0) && p.n_params != 2 * p.dim) return QMC_ERR_PARAMS;
     if (p.family == QMC_FAMILY_GENZ_DISCONT && p.n_params != p.dim + std::min(p.dim, 2)) return QMC_ERR_PARAMS;
-    if (p.family == QMC_FAMILY_SECTOR) {
-        const int rest = p.n_params - 4 - p.dim;
-        const bool plain = rest % (1 + p.dim) == 0, with_log = rest >= 3 && (rest - 3) % (1 + p.dim) == 0;   // optional trailing [lu, lf, p]
-        if (rest < 2 * (1 + p.dim) || !(plain || with_log) || rest / (1 + p.dim) > 2 * kMaxSectorMono) return QMC_ERR_PARAMS;
+    if (is_sector_family(p.family)) {
+        const int rest = p.n_params - 4 - p.dim, rec = sector_mono_stride(p.family, p.dim);
+        const bool plain = rest % rec == 0, with_log = rest >= 3 && (rest - 3) % rec == 0;   // optional trailing [lu, lf, p]
+        if (rest < 2 * rec || !(plain || with_log) || rest / rec > 2 * kMaxSectorMono) return QMC_ERR_PARAMS;
     }
     return QMC_OK;
 }
@@ -201,10 +201,10 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
             d.kor[0] = K / 3.141592653589793238462643383279;
             for (int j = 0; j < p.dim; ++j) d.wconst *= K;
         }
-        if (p.family == QMC_FAMILY_SECTOR) {
-            const int nmono = (p.n_params - 4 - p.dim) / (1 + p.dim);
+        if (is_sector_family(p.family)) {
+            const int nmono = (p.n_params - 4 - p.dim) / sector_mono_stride(p.family, p.dim);
             d.aux_off = (int)prog_off;
-            d.aux_len = sector_slot_words(nmono) + 2 * nmono + 1;       // coefficient slots + 16 one-byte steps per monomial + end steps / padding
+            d.aux_len = sector_slot_words(nmono, p.family == QMC_FAMILY_SECTOR_COMPLEX) + 2 * nmono + 1;   // coefficient slots + 16 one-byte steps per monomial + end steps / padding
             prog_off += (size_t)d.aux_len;
         }
         d.means_off = means_off;
@@ -227,8 +227,9 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
     // tiling (S9): per kernel variant aim at kWaves x (resident CTAs of a B200) tiles, shared among the variant's problems
     // in proportion to their cost; a tile is at least one index per thread and at most kMaxSteps (bounds the fp64 chains)
     for (auto& v : plan->variants) {
-        const int resident = kPlanSMs * (v.family == QMC_FAMILY_SECTOR ? min_blocks_sector(v.dp) : min_blocks_closed(v.dp, v.wide));
-        const int threads = v.family == QMC_FAMILY_SECTOR ? sector_threads(v.dp) : kThreads;   // CTA size of the variant's kernel
+        const bool sector_variant = v.family == QMC_FAMILY_SECTOR || v.family == kKernelFamilyCSector;
+        const int resident = kPlanSMs * (sector_variant ? min_blocks_sector(v.dp) : min_blocks_closed(v.dp, v.wide));
+        const int threads = v.family == QMC_FAMILY_SECTOR ? sector_threads(v.dp) : (v.family == kKernelFamilyCSector ? kCSectorThreads : kThreads);   // CTA size of the variant's kernel
         const int env = opt.tiles_target > 0 ? opt.tiles_target : 0;
         // one problem: equal tiles, 2 per resident CTA (the queue evens out SM speed differences over a long kernel) -- or
         // exactly 1 when the whole kernel is short (< kShortEvalsPerCta evaluations per CTA: per-tile overhead and the
@@ -331,7 +332,7 @@ int occupancy_closed(int family, int dp, bool wide) {
 #undef QMC_TRY_PARTS
 
 int occupancy(int family, int dp, bool wide) {
-    static int cache[kMaxDevices][5][33][2];
+    static int cache[kMaxDevices][kKernelFamilies][33][2];
     const int dev = current_device();
     if (dev < 0) return -1;
     int& c = cache[dev][family][dp][wide ? 1 : 0];
@@ -340,6 +341,7 @@ int occupancy(int family, int dp, bool wide) {
     switch (family) {
         case 0: case 1: case 2: case 4: v = occupancy_closed(family, dp, wide); break;
         case 3: v = occupancy_fused_f3(dp, wide); break;
+        case kKernelFamilyCSector: v = occupancy_fused_f8(dp, wide); break;
     }
     if (v > 0) c = v;
     return v;
@@ -391,7 +393,7 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
     double* dmeans = reinterpret_cast<double*>(ws + plan.off_means);
     double* dpart = reinterpret_cast<double*>(ws + plan.off_partials);
     bool any_sector = false;
-    for (const DevProblem& d : plan.dev) any_sector = any_sector || d.family == QMC_FAMILY_SECTOR;
+    for (const DevProblem& d : plan.dev) any_sector = any_sector || is_sector_family(d.family);
     // single mode: one closed-form problem travels in the kernel parameter; nothing is uploaded, reset or prepared
     const bool single = count == 1 && !any_sector;
     FusedLaunch base;
@@ -461,6 +463,7 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
         switch (v.family) {
             case 0: case 1: case 2: case 4: e = launch_closed(v.family, v.dp, v.wide, grid, st, a); break;
             case 3: e = launch_fused_f3(v.dp, v.wide, grid, st, a); break;
+            case kKernelFamilyCSector: e = launch_fused_f8(v.dp, v.wide, grid, st, a); break;
         }
         if (e != cudaSuccess) return cuda_fail(e, "fused kernel launch");
         ++g_ts.last_launches;
@@ -491,12 +494,12 @@ int validate_values(const qmc_problem& p) {
     if (p.family == QMC_FAMILY_GENZ_PRODPEAK)
         for (int j = 0; j < p.dim; ++j)
             if (p.params[j] == 0.0) return QMC_ERR_PARAMS;
-    if (p.family == QMC_FAMILY_SECTOR) {
+    if (is_sector_family(p.family)) {
         const double* q = p.params;
         for (int k = 0; k < 4; ++k)
             if (q[k] != std::floor(q[k]) || q[k] < 0.0) return QMC_ERR_PARAMS;
         if (q[0] > 8 || q[1] > 8 || q[2] < 1 || q[3] < 1 || q[2] > kMaxSectorMono || q[3] > kMaxSectorMono) return QMC_ERR_PARAMS;
-        const int base = 4 + p.dim + ((int)q[2] + (int)q[3]) * (1 + p.dim);
+        const int base = 4 + p.dim + ((int)q[2] + (int)q[3]) * sector_mono_stride(p.family, p.dim);
         if (p.n_params == base + 3) {                                            // log factor: p an integer in 1..4
             if (!(q[base + 2] >= 1.0 && q[base + 2] <= 4.0) || q[base + 2] != std::floor(q[base + 2])) return QMC_ERR_PARAMS;
         } else if (p.n_params != base) return QMC_ERR_PARAMS;
@@ -536,10 +539,10 @@ int family_param_count(int family, const double* params, int dim) {
     if (family == QMC_FAMILY_GENZ_CORNER) return dim;
     if (family == QMC_FAMILY_GENZ_GAUSSIAN || family == QMC_FAMILY_GENZ_C0) return 2 * dim;
     if (family == QMC_FAMILY_GENZ_DISCONT) return dim + std::min(dim, 2);
-    if (family == QMC_FAMILY_SECTOR && params) {
+    if (is_sector_family(family) && params) {
         const double nU = params[2], nF = params[3];
         if (!(nU >= 1 && nU <= kMaxSectorMono && nF >= 1 && nF <= kMaxSectorMono)) return -1;
-        return 4 + dim + ((int)nU + (int)nF) * (1 + dim);
+        return 4 + dim + ((int)nU + (int)nF) * sector_mono_stride(family, dim);
     }
     return -1;
 }

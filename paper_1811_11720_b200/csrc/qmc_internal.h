@@ -21,6 +21,8 @@ constexpr int kWavesBatch = 8;         // ... and when it serves a batch of uneq
 // resident CTAs per SM each fused kernel is register-budgeted for (its __launch_bounds__ minimum)
 constexpr int min_blocks_closed(int dp, bool wide) { return (dp <= 8 || (dp <= 12 && !wide)) ? 4 : (dp <= 16 ? (wide ? 2 : 3) : 2); }
 constexpr int sector_group(int dp) { return dp <= 8 ? 8 : 4; }                       // shifts per group, sector family
+constexpr int csector_group(int dp) { return dp <= 8 ? 4 : 2; }                      // complex sector family: paired accumulators
+constexpr int kCSectorThreads = 384;
 // The sector kernels run ONE CTA per SM, as large as the registers allow (x[G][DP] lives in registers): every warp of an SM then
 // interprets the same program, whose cases stay in the L0 instruction cache.
 __host__ __device__ constexpr int sector_threads(int dp) { return dp <= 6 ? 384 : 256; }
@@ -30,11 +32,20 @@ constexpr int kMaxSectorMono = 64;     // monomials per polynomial
 constexpr int kMaxSectorOps = 2 * kMaxSectorMono * 16 + 64;   // step bytes of a program: <= one per unit of degree (<= 16 per monomial) + end steps, padding
 // coefficient region of a program in 8-byte words: one 16-byte slot {cf, cf2} per non-constant monomial, one for the end of U,
 // one of read-ahead
-__host__ __device__ constexpr int sector_slot_words(int nmono) { return 2 * (nmono + 2); }
+// (complex family: 32-byte slots {cf_re, cf_im, cf2_re, cf2_im})
+__host__ __device__ constexpr int sector_slot_words(int nmono, bool cplx = false) { return (cplx ? 4 : 2) * (nmono + 2); }
 
-// kernel family of a public family id: the four remaining Genz functions share one fused kernel (runtime sub-kind)
+// kernel family of a public family id: the four remaining Genz functions share one fused kernel (runtime sub-kind); the complex
+// sector family has its own
 constexpr int kKernelFamilyGenzMisc = 4;
-__host__ __device__ constexpr int kernel_family(int family) { return family <= QMC_FAMILY_SECTOR ? family : kKernelFamilyGenzMisc; }
+constexpr int kKernelFamilyCSector = 5;
+constexpr int kKernelFamilies = 6;
+__host__ __device__ constexpr int kernel_family(int family) {
+    return family <= QMC_FAMILY_SECTOR ? family : (family == QMC_FAMILY_SECTOR_COMPLEX ? kKernelFamilyCSector : kKernelFamilyGenzMisc);
+}
+__host__ __device__ constexpr bool is_sector_family(int family) { return family == QMC_FAMILY_SECTOR || family == QMC_FAMILY_SECTOR_COMPLEX; }
+// monomial record of a sector block: coefficient (re [, im]) + dim exponents
+__host__ __device__ constexpr int sector_mono_stride(int family, int dim) { return (family == QMC_FAMILY_SECTOR_COMPLEX ? 2 : 1) + dim; }
 
 // transform kinds after host-side decoding
 enum : int { TR_NONE = 0, TR_BAKER = 1, TR_KOR3 = 2, TR_KORR = 3 };   // TR_KORR = the generic tile loop, see GEN_*
@@ -81,7 +92,8 @@ struct alignas(16) DevAux {
     double fam_b[QMC_MAX_DIM];
     double fit[9][QMC_MAX_DIM];            // a4, a5, a6, 2*a5, 3*a6 of the cubic part; a0, a2 (a0-1), a1, a3 (a1-1) of the poles
     double fam0;                           // OSC: 2 pi u0
-    double sec_c0[2];                      // sector: constant terms of U and F
+    double sec_c0[2];                      // sector: constant terms of U and F (real parts)
+    double sec_c0i[2];                     // complex sector: their imaginary parts
     double sec_log[2];                     // sector: lu, lf of the optional log factor (lu log U + lf log F)^p
     int sec_a, sec_b;                      // sector: powers of U and F
     int sec_logp, sec_pad_;                // sector: p of the log factor, 0 = none

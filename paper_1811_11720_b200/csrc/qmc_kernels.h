@@ -37,5 +37,7 @@ QMC_DECLARE_FAMILY(0) QMC_DECLARE_FAMILY(1) QMC_DECLARE_FAMILY(2) QMC_DECLARE_FA
 #undef QMC_DECLARE_PART
 cudaError_t launch_fused_f3(int dp, bool wide, int grid, cudaStream_t st, const FusedLaunch& a);
 int occupancy_fused_f3(int dp, bool wide);
+cudaError_t launch_fused_f8(int dp, bool wide, int grid, cudaStream_t st, const FusedLaunch& a);   // complex sector family
+int occupancy_fused_f8(int dp, bool wide);
 
 }  // namespace qmc

@@ -13,11 +13,11 @@ namespace qmc {
 __global__ void __launch_bounds__(32) prepare_kernel(const DevProblem* __restrict__ probs, DevAux* __restrict__ aux,
                                                      unsigned long long* __restrict__ prog_area) {
     const DevProblem pb = probs[blockIdx.x];
-    if (pb.family != QMC_FAMILY_SECTOR) return;             // closed-form families derive their tables inside the fused kernel
+    if (!is_sector_family(pb.family)) return;               // closed-form families derive their tables inside the fused kernel
     DevAux& a = aux[blockIdx.x];
     const int j = threadIdx.x;
     if (j < QMC_MAX_DIM) {
-        const SlotConst s = derive_slot(pb, j, sector_threads(sector_dim_slots(pb.dim)));
+        const SlotConst s = derive_slot(pb, j, pb.family == QMC_FAMILY_SECTOR ? sector_threads(sector_dim_slots(pb.dim)) : kCSectorThreads);
         a.z[j] = s.z; a.step[j] = s.step; a.back[j] = s.back; a.fam_a[j] = s.fa; a.fam_b[j] = s.fb;
 #pragma unroll
         for (int i = 0; i < 9; ++i) a.fit[i][j] = s.f[i];
@@ -30,9 +30,9 @@ __global__ void __launch_bounds__(32) prepare_kernel(const DevProblem* __restric
         a.sec_a = a.sec_b = 0;
         a.sec_logp = 0; a.sec_log[0] = a.sec_log[1] = 0.0;
         a.sec_nops[0] = a.sec_nops[1] = a.sec_ncoef[0] = a.sec_ncoef[1] = 0;
-        a.sec_c0[0] = a.sec_c0[1] = 0.0;
+        a.sec_c0[0] = a.sec_c0[1] = 0.0; a.sec_c0i[0] = a.sec_c0i[1] = 0.0;
     }
-    if (pb.family == QMC_FAMILY_SECTOR) {
+    {
         __syncwarp();
         prepare_sector(pb, a, prog_area);
     }
@@ -62,7 +62,7 @@ __global__ void __launch_bounds__(kFinalizeThreads) finalize_kernel(const __grid
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nc = pb.ncomp, m = pb.m, tiles = pb.tiles, npairs = m * nc;
     double* means = means_ws + pb.means_off;
-    const bool bad = pb.family == QMC_FAMILY_SECTOR && L.aux[blockIdx.x].status != 0;
+    const bool bad = is_sector_family(pb.family) && L.aux[blockIdx.x].status != 0;
     for (int pair = warp; pair < npairs; pair += kFinalizeThreads / 32) {
         const double* src = partials + pb.partial_off + (long long)pair * tiles;
         CompSum cs;

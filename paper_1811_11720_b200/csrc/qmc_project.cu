@@ -86,6 +86,31 @@ __device__ double abs_integrand(const ProjArgs& a, const double* x) {
     double pre = 1.0;
     for (int j = 0; j < d; ++j) pre *= ipow_small(x[j], (int)p[4 + j]);
     const double* base = p + 4 + d;
+    if (a.family == QMC_FAMILY_SECTOR_COMPLEX) {                             // |f| = pre |U|^a / |F|^b (|Log| factor: modulus of the power)
+        double re[2], im[2];
+        const int cnt2[2] = {nU, nF};
+        for (int w = 0; w < 2; ++w) {
+            const double* cr = base;
+            const double* ci = base + cnt2[w];
+            const double* e = base + 2 * cnt2[w];
+            double sr = 0.0, si = 0.0;
+            for (int t = 0; t < cnt2[w]; ++t) {
+                double mon = 1.0;
+                for (int j = 0; j < d; ++j) mon *= ipow_small(x[j], (int)e[t * d + j]);
+                sr = __fma_rn(cr[t], mon, sr); si = __fma_rn(ci[t], mon, si);
+            }
+            re[w] = sr; im[w] = si;
+            base += cnt2[w] * (2 + d);
+        }
+        const double mu = sqrt(re[0] * re[0] + im[0] * im[0]), mf = sqrt(re[1] * re[1] + im[1] * im[1]);
+        double f = pre * ipow_small(mu, pa) / ipow_small(mf, pb);
+        if (a.n_params == 4 + d + (nU + nF) * (2 + d) + 3) {
+            const double* t = p + a.n_params - 3;
+            const double Lr = t[0] * log(mu) + t[1] * log(mf), Li = t[0] * atan2(im[0], re[0]) + t[1] * atan2(im[1], re[1]);
+            f *= ipow_small(sqrt(Lr * Lr + Li * Li), (int)t[2]);
+        }
+        return fabs(f);
+    }
     double poly[2];
     const int cnt[2] = {nU, nF};
     for (int w = 0; w < 2; ++w) {
@@ -122,7 +147,7 @@ __global__ void __launch_bounds__(kThreads) project_kernel(ProjArgs a) {   // a:
     // the host sees only the struct) -- a block that fails is never interpreted and the histograms become NaN
     double* sp = hist + kWarps * hsize;
     for (int i = tid; i < a.n_params; i += kThreads) sp[i] = a.params[i];
-    if (tid == 0) block_status = (a.family == QMC_FAMILY_SECTOR) ? sector_block_status(a.params, a.n_params, a.dim) : 0;
+    if (tid == 0) block_status = is_sector_family(a.family) ? sector_block_status(a.params, a.n_params, a.dim, a.family == QMC_FAMILY_SECTOR_COMPLEX) : 0;
     __syncthreads();
     a.params = sp;
     if (block_status != 0) {
@@ -191,9 +216,9 @@ __global__ void __launch_bounds__(256) project_merge_kernel(ProjArgs a) {
 
 int plan_project(const qmc_problem* p, int bins, ProjArgs* a) {
     if (!p) return QMC_ERR_NULL;
-    if (p->family < 0 || p->family > QMC_FAMILY_GENZ_DISCONT) return QMC_ERR_FAMILY;
+    if (p->family < 0 || p->family > QMC_FAMILY_SECTOR_COMPLEX) return QMC_ERR_FAMILY;
     if (p->dim < 1 || p->dim > QMC_MAX_DIM) return QMC_ERR_DIM;
-    if (p->family == QMC_FAMILY_SECTOR && p->dim > QMC_MAX_SECTOR_DIM) return QMC_ERR_DIM;       // the same limits as the integration entries
+    if (is_sector_family(p->family) && p->dim > QMC_MAX_SECTOR_DIM) return QMC_ERR_DIM;          // the same limits as the integration entries
     if (p->n < 2 || p->n >= (1ull << 53)) return QMC_ERR_N;
     if (bins < 2 || bins > 1024) return QMC_ERR_N;
     if (p->m < 1) return QMC_ERR_M;
@@ -203,10 +228,10 @@ int plan_project(const qmc_problem* p, int bins, ProjArgs* a) {
     if (p->family == QMC_FAMILY_GENZ_CORNER && p->n_params != p->dim) return QMC_ERR_PARAMS;
     if ((p->family == QMC_FAMILY_GENZ_GAUSSIAN || p->family == QMC_FAMILY_GENZ_C0) && p->n_params != 2 * p->dim) return QMC_ERR_PARAMS;
     if (p->family == QMC_FAMILY_GENZ_DISCONT && p->n_params != p->dim + (p->dim < 2 ? p->dim : 2)) return QMC_ERR_PARAMS;
-    if (p->family == QMC_FAMILY_SECTOR) {               // struct-level layout check as in qmc_host.cu; the values are checked on the device
-        const int rest = p->n_params - 4 - p->dim;
-        const bool plain = rest % (1 + p->dim) == 0, with_log = rest >= 3 && (rest - 3) % (1 + p->dim) == 0;
-        if (rest < 2 * (1 + p->dim) || !(plain || with_log) || rest / (1 + p->dim) > 2 * kMaxSectorMono) return QMC_ERR_PARAMS;
+    if (is_sector_family(p->family)) {                  // struct-level layout check as in qmc_host.cu; the values are checked on the device
+        const int rest = p->n_params - 4 - p->dim, rec = sector_mono_stride(p->family, p->dim);
+        const bool plain = rest % rec == 0, with_log = rest >= 3 && (rest - 3) % rec == 0;
+        if (rest < 2 * rec || !(plain || with_log) || rest / rec > 2 * kMaxSectorMono) return QMC_ERR_PARAMS;
     }
     std::memset(a, 0, sizeof(*a));
     a->params = p->params;

@@ -25,7 +25,7 @@
 
 namespace qmc {
 
-constexpr int kSecMaxSlots = sector_slot_words(2 * kMaxSectorMono) / 2;   // 16-byte coefficient slots of a program: one per monomial + end-of-polynomial + read-ahead
+constexpr int kSecMaxSlots = sector_slot_words(2 * kMaxSectorMono) / 2;   // coefficient slots of a program: one per monomial + end-of-polynomial + read-ahead
 constexpr int kSecMaxWords = kMaxSectorOps / 4;
 constexpr int kSecKinds = 5;
 constexpr int kSecParkRows = 16;                       // rows of G... doubles per thread parked in shared memory: weights [0, 8), U [8, 16)
@@ -35,18 +35,18 @@ enum : int { SEC_NOP = 0, SEC_ENDP = 1, SEC_END = 2, SEC_BASE = 3 };
 enum : int { SEC_SC = 0, SEC_SL = 1, SEC_AL = 2, SEC_ALI = 3, SEC_AM = 4 };
 
 template <int NT> struct alignas(16) SectorSmem {
-    double slots[kSecMaxSlots * 2];  // {cf, cf2} per coefficient-consuming step, in program order
+    double slots[kSecMaxSlots * 4];  // {cf, cf2} per coefficient-consuming step, in program order (complex family: {cf_re, cf_im, cf2_re, cf2_im})
     unsigned int words[kSecMaxWords];// step bytes: U's steps, SEC_ENDP, F's steps, SEC_END (copied word-wise)
-    double c0u;                      // constant term of U (F's travels in the slot of the end-of-polynomial step)
+    double c0u, c0u_im;              // constant term of U (F's travels in the slot of the end-of-polynomial step)
     unsigned long long nu_packed;    // nu_j in 4 bits each
     int a, b;                        // powers of U and F
     double lg[2];                    // lu, lf of the log factor
     int logp, pad_;                  // its power p (0 = no log factor)
     double park[kSecParkRows * NT];  // [row][thread]: rows [0, 8) the G weights of a thread while the interpreter runs (with a log
-                                     // factor afterwards F), rows [8, 16) U as the interpreter parks it
+                                     // factor afterwards F), rows [8, 16) U as the interpreter parks it (complex: (re, im) pairs)
 };
 struct SectorOff {                   // byte offsets of the fields above (read with ld.shared in the inner loop)
-    static constexpr unsigned slots = 0, words = kSecMaxSlots * 16, c0u = words + kSecMaxWords * 4, nu = c0u + 8, ab = nu + 8, lg = ab + 8,
+    static constexpr unsigned slots = 0, words = kSecMaxSlots * 32, c0u = words + kSecMaxWords * 4, nu = c0u + 16, ab = nu + 8, lg = ab + 8,
                               logp = lg + 16, park = logp + 8;
 };
 #define QMC_SECTOR_OFF_CHECK(NT)                                                                                                      \
@@ -66,13 +66,16 @@ struct SecEmit {                     // output cursor of the compiler
     double* slots;
     unsigned char* ops;
     int nslots, nops, max_slots, max_ops, status;
+    bool cplx;                       // 32-byte slots {cf_re, cf_im, cf2_re, cf2_im}
     __device__ void op(int kind, int j) {
         if (nops >= max_ops) { status = QMC_ERR_PARAMS; return; }
         ops[nops++] = (unsigned char)(SEC_BASE + kSecKinds * j + kind);
     }
-    __device__ void slot(double cf, double cf2) {
+    __device__ void slot(double cf, double cfi, double cf2, double cf2i) {
         if (nslots >= max_slots) { status = QMC_ERR_PARAMS; return; }
-        slots[2 * nslots] = cf; slots[2 * nslots + 1] = cf2; ++nslots;
+        if (cplx) { slots[4 * nslots] = cf; slots[4 * nslots + 1] = cfi; slots[4 * nslots + 2] = cf2; slots[4 * nslots + 3] = cf2i; }
+        else { slots[2 * nslots] = cf; slots[2 * nslots + 1] = cf2; }
+        ++nslots;
     }
 };
 
@@ -82,39 +85,41 @@ struct SecEmit {                     // output cursor of the compiler
 // its monomials is factored out: the monomials that contain it form a child (processed as an item of its own unless it is a
 // single finished monomial, a "leaf"), the others stay.  When the item is used up its group is emitted: prefix, the coefficient
 // of the prefix monomial itself (own) and the leaves.  Returns the constant term.
-__device__ inline double compile_polynomial(const double* c, const double* e, int cnt, int d, SecEmit& out) {
+// ci: imaginary parts of the coefficients (complex family) or nullptr; the constant term is returned through c0_re / c0_im.
+__device__ inline void compile_polynomial(const double* c, const double* ci, const double* e, int cnt, int d, SecEmit& out,
+                                          double* c0_re, double* c0_im) {
     unsigned char rem[kMaxSectorMono][16];
     unsigned char left[kMaxSectorMono];
     short idx[kMaxSectorMono];
     // work items: ranges of idx with the prefix they share (exponents) and the coefficient of the prefix monomial; items on the
     // stack are disjoint ranges with at least one unfinished monomial each, so there are never more than cnt of them
     short it_b[kMaxSectorMono + 1], it_e[kMaxSectorMono + 1];
-    double it_own[kMaxSectorMono + 1];
+    double it_own[kMaxSectorMono + 1], it_owni[kMaxSectorMono + 1];
     unsigned char it_prefix[kMaxSectorMono + 1][16];
-    double c0 = 0.0;
+    double c0 = 0.0, c0i = 0.0;
     int m = 0;
     for (int t = 0; t < cnt; ++t) {
         int deg = 0;
         for (int j = 0; j < d; ++j) { const int v = (int)e[t * d + j]; rem[t][j] = (unsigned char)v; deg += v; }
         for (int j = d; j < 16; ++j) rem[t][j] = 0;
         left[t] = (unsigned char)deg;
-        if (deg == 0) c0 += c[t]; else idx[m++] = (short)t;
+        if (deg == 0) { c0 += c[t]; if (ci) c0i += ci[t]; } else idx[m++] = (short)t;
     }
     int top = 0;
-    it_b[0] = 0; it_e[0] = (short)m; it_own[0] = 0.0;
+    it_b[0] = 0; it_e[0] = (short)m; it_own[0] = 0.0; it_owni[0] = 0.0;
     for (int j = 0; j < 16; ++j) it_prefix[0][j] = 0;
     top = 1;
     bool root = true;
     while (top > 0) {
         --top;
         const int b = it_b[top], en = it_e[top];
-        const double own = it_own[top];
+        const double own = it_own[top], owni = it_owni[top];
         unsigned char prefix[16];
         int pdeg = 0;
         for (int j = 0; j < 16; ++j) { prefix[j] = it_prefix[top][j]; pdeg += prefix[j]; }
         const bool is_root = root;
         root = false;
-        double leaf_c[16];
+        double leaf_c[16], leaf_ci[16];
         int leaf_mask = 0;
         int cur = b;
         while (cur < en) {
@@ -129,18 +134,19 @@ __device__ inline double compile_polynomial(const double* c, const double* e, in
             int mid = cur;
             for (int i = cur; i < en; ++i)
                 if (rem[idx[i]][best] > 0) { const short t = idx[i]; idx[i] = idx[mid]; idx[mid] = t; ++mid; }
-            double child_own = 0.0;
+            double child_own = 0.0, child_owni = 0.0;
             int fin = cur;
             for (int i = cur; i < mid; ++i) {
                 const short t = idx[i];
                 --rem[t][best]; --left[t];
-                if (left[t] == 0) { child_own += c[t]; idx[i] = idx[fin]; idx[fin] = t; ++fin; }
+                if (left[t] == 0) { child_own += c[t]; if (ci) child_owni += ci[t]; idx[i] = idx[fin]; idx[fin] = t; ++fin; }
             }
             if (fin == mid) {                                  // nothing below: a leaf of this item
                 leaf_c[best] = (leaf_mask >> best & 1) ? leaf_c[best] + child_own : child_own;
+                leaf_ci[best] = (leaf_mask >> best & 1) ? leaf_ci[best] + child_owni : child_owni;
                 leaf_mask |= 1 << best;
             } else {                                           // a child item: prefix * x_best
-                it_b[top] = (short)fin; it_e[top] = (short)mid; it_own[top] = child_own;
+                it_b[top] = (short)fin; it_e[top] = (short)mid; it_own[top] = child_own; it_owni[top] = child_owni;
                 for (int j = 0; j < 16; ++j) it_prefix[top][j] = prefix[j];
                 ++it_prefix[top][best];
                 ++top;
@@ -150,7 +156,7 @@ __device__ inline double compile_polynomial(const double* c, const double* e, in
         // emit the group of this item
         if (is_root) {
             for (int k = 0; k < d; ++k)
-                if (leaf_mask >> k & 1) { out.op(SEC_SL, k); out.slot(leaf_c[k], 0.0); }
+                if (leaf_mask >> k & 1) { out.op(SEC_SL, k); out.slot(leaf_c[k], leaf_ci[k], 0.0, 0.0); }
             continue;
         }
         int last = 0;
@@ -160,18 +166,18 @@ __device__ inline double compile_polynomial(const double* c, const double* e, in
             for (int k = 0; k < d; ++k)
                 if (leaf_mask >> k & 1) {
                     out.op(first ? SEC_ALI : SEC_AL, k);
-                    out.slot(leaf_c[k], first ? own : 0.0);
+                    out.slot(leaf_c[k], leaf_ci[k], first ? own : 0.0, first ? owni : 0.0);
                     first = false;
                 }
             for (int j = 0; j < d; ++j)
                 for (int r = 0; r < prefix[j] - (j == last ? 1 : 0); ++r) out.op(SEC_AM, j);
             out.op(SEC_SC, last);
-        } else if (own != 0.0) {
-            if (pdeg == 1) { out.op(SEC_SL, last); out.slot(own, 0.0); }
+        } else if (own != 0.0 || owni != 0.0) {
+            if (pdeg == 1) { out.op(SEC_SL, last); out.slot(own, owni, 0.0, 0.0); }
             else {
                 int firstv = 0;
                 for (int j = d - 1; j >= 0; --j) if (prefix[j]) firstv = j;
-                out.op(SEC_ALI, firstv); out.slot(own, 0.0);
+                out.op(SEC_ALI, firstv); out.slot(own, owni, 0.0, 0.0);
                 for (int j = 0; j < d; ++j) {
                     const int reps = prefix[j] - (j == firstv ? 1 : 0) - (j == last ? 1 : 0);
                     for (int r = 0; r < reps; ++r) out.op(SEC_AM, j);
@@ -180,53 +186,57 @@ __device__ inline double compile_polynomial(const double* c, const double* e, in
             }
         }
     }
-    return c0;
+    *c0_re = c0; *c0_im = c0i;
 }
 
 __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned long long* prog_area) {
     if (threadIdx.x != 0) return;
     const int d = pb.dim;
+    const bool cplx = pb.family == QMC_FAMILY_SECTOR_COMPLEX;
+    const int rec = sector_mono_stride(pb.family, d), sw = cplx ? 4 : 2;                 // monomial record, doubles per slot
     const double* p = pb.params;
-    const int nmono_total = (pb.n_params - 4 - d) / (1 + d);
+    const int nmono_total = (pb.n_params - 4 - d) / rec;
     double* slots = reinterpret_cast<double*>(prog_area + pb.aux_off);
-    unsigned char* ops = reinterpret_cast<unsigned char*>(prog_area + pb.aux_off + sector_slot_words(nmono_total));
+    unsigned char* ops = reinterpret_cast<unsigned char*>(prog_area + pb.aux_off + sector_slot_words(nmono_total, cplx));
     // A rejected parameter block must still leave a program the interpreter can run to its end (the problem's
     // results are then replaced by NaN in the finalize stage): end-of-U, end, read-ahead padding.
     auto stub = [&]() {
         ops[0] = (unsigned char)SEC_ENDP; ops[1] = (unsigned char)SEC_END;
         for (int i = 2; i < 8; ++i) ops[i] = (unsigned char)SEC_NOP;
-        slots[0] = 1.0; slots[1] = 0.0;
-        a.sec_nops[0] = 2; a.sec_nops[1] = 0; a.sec_ncoef[0] = 1; a.sec_ncoef[1] = 0;
-        a.sec_c0[0] = a.sec_c0[1] = 1.0;
+        for (int i = 0; i < 2 * sw; ++i) slots[i] = (i == 0) ? 1.0 : 0.0;
+        a.sec_nops[0] = 2; a.sec_nops[1] = 0; a.sec_ncoef[0] = 2; a.sec_ncoef[1] = 0;
+        a.sec_c0[0] = a.sec_c0[1] = 1.0; a.sec_c0i[0] = a.sec_c0i[1] = 0.0;
     };
     stub();
-    const int vst = sector_block_status(p, pb.n_params, d);
+    const int vst = sector_block_status(p, pb.n_params, d, cplx);
     if (vst != 0) { a.status = vst; return; }
     const int cnt[2] = {(int)p[2], (int)p[3]};
-    const int n_base = 4 + d + (cnt[0] + cnt[1]) * (1 + d);
+    const int n_base = 4 + d + (cnt[0] + cnt[1]) * rec;
     if (pb.n_params == n_base + 3) { a.sec_log[0] = p[n_base]; a.sec_log[1] = p[n_base + 1]; a.sec_logp = (int)p[n_base + 2]; }
     a.sec_a = (int)p[0]; a.sec_b = (int)p[1];
     for (int j = 0; j < d; ++j) a.nu[j] = (unsigned char)(int)p[4 + j];
     SecEmit out;
-    out.slots = slots; out.ops = ops; out.nslots = 0; out.nops = 0; out.status = 0;
-    out.max_slots = sector_slot_words(nmono_total) / 2 - 1;                              // one slot of read-ahead
-    out.max_ops = min((pb.aux_len - sector_slot_words(nmono_total)) * 8, kMaxSectorOps) - 8;   // room for the two end steps and the read-ahead padding
-    const double* base = p + 4 + d;
-    const double c0u = compile_polynomial(base, base + cnt[0], cnt[0], d, out);
-    base += cnt[0] * (1 + d);
+    out.slots = slots; out.ops = ops; out.nslots = 0; out.nops = 0; out.status = 0; out.cplx = cplx;
+    out.max_slots = sector_slot_words(nmono_total, cplx) / sw - 1;                       // one slot of read-ahead
+    out.max_ops = min((pb.aux_len - sector_slot_words(nmono_total, cplx)) * 8, kMaxSectorOps) - 8;   // room for the two end steps and the read-ahead padding
+    const double* base = p + 4 + d;                    // polynomial: Re c (cnt) [, Im c (cnt)], exponents (cnt x d)
+    double c0u, c0ui, c0f, c0fi;
+    compile_polynomial(base, cplx ? base + cnt[0] : nullptr, base + (cplx ? 2 : 1) * cnt[0], cnt[0], d, out, &c0u, &c0ui);
+    base += cnt[0] * rec;
     // end of U: its step takes F's constant term from the slot stream -- the slot is filled after F is compiled
     const int endp_slot = out.nslots;
     out.ops[out.nops++] = (unsigned char)SEC_ENDP;          // max_ops keeps room for the end steps
-    out.slot(0.0, 0.0);
-    const double c0f = compile_polynomial(base, base + cnt[1], cnt[1], d, out);
+    out.slot(0.0, 0.0, 0.0, 0.0);
+    compile_polynomial(base, cplx ? base + cnt[1] : nullptr, base + (cplx ? 2 : 1) * cnt[1], cnt[1], d, out, &c0f, &c0fi);
     if (out.status) { stub(); a.status = out.status; return; }
-    slots[2 * endp_slot] = c0f;
+    slots[sw * endp_slot] = c0f;
+    if (cplx) slots[sw * endp_slot + 1] = c0fi;
     out.ops[out.nops++] = (unsigned char)SEC_END;
     out.ops[out.nops++] = (unsigned char)SEC_NOP;       // the interpreter reads two step codes ahead
     out.ops[out.nops++] = (unsigned char)SEC_NOP;
     while (out.nops & 3) out.ops[out.nops++] = (unsigned char)SEC_NOP;
-    slots[2 * out.nslots] = 0.0; slots[2 * out.nslots + 1] = 0.0;                          // read-ahead slot
-    a.sec_c0[0] = c0u; a.sec_c0[1] = c0f;
+    for (int i = 0; i < sw; ++i) slots[sw * out.nslots + i] = 0.0;                         // read-ahead slot
+    a.sec_c0[0] = c0u; a.sec_c0[1] = c0f; a.sec_c0i[0] = c0ui; a.sec_c0i[1] = c0fi;
     a.sec_nops[0] = out.nops / 4;
     a.sec_ncoef[0] = out.nslots + 1;
     a.status = 0;
@@ -234,6 +244,7 @@ __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned 
 
 // ---- interpreter: U and F for G points (threaded code in inline PTX, see gen_sector_interp.py) ------
 #include "qmc_sector_interp.inc"
+#include "qmc_csector_interp.inc"
 
 // S2-S4 for the G points of one lattice index: x[q][j] and the weight W[q] (Eq. 12, Eq. 18)
 template <int DP, int G, bool WIDE, int TR, int FIT>
@@ -248,9 +259,18 @@ __device__ __forceinline__ void sector_coords(const typename Res<WIDE>::T (&r)[D
         double fa, fb, dl[G];
         FitC fc;
         load_slot<DP, G, FIT>(cx.sbase, cx.delta, j, cx.fit_mode, fa, fb, fc, dl);
+        if constexpr (TR == TR_KORR) {                        // generic tile loop: kind and fit mode decided once per dimension
+            double t[G], xg[G];
 #pragma unroll
-        for (int q = 0; q < G; ++q)
-            x[q][j] = point_coord<TR, FIT>(rd, cx.inv_n, dl[q], fc, cx.sbase + SmemOff<DP, G>::kor, cx.kor_r, P[q], D[q]);
+            for (int q = 0; q < G; ++q) t[q] = coord_t(rd, cx.inv_n, dl[q]);
+            generic_coord_group<G>(t, cx.sbase + SmemOff<DP, G>::kor, cx.kor_r, fc, xg, P, D);
+#pragma unroll
+            for (int q = 0; q < G; ++q) x[q][j] = xg[q];
+        } else {
+#pragma unroll
+            for (int q = 0; q < G; ++q)
+                x[q][j] = point_coord<TR, FIT>(rd, cx.inv_n, dl[q], fc, cx.sbase + SmemOff<DP, G>::kor, cx.kor_r, P[q], D[q]);
+        }
     }
 #pragma unroll
     for (int q = 0; q < G; ++q) W[q] = point_weight<TR, FIT>(P[q], D[q], cx.wconst, cx.kor_r);
@@ -387,16 +407,103 @@ template <int DP, int G, bool WIDE, bool SLOW, int NT> struct SectorEval {
     }
 };
 
+// The complex sector family (reading C-16): U, F complex-valued polynomials of the real coordinates; f = W prod x^nu U^a / F^b
+// in complex arithmetic, two accumulators per shift.  The interpreter parks U as (re, im) row pairs from row 8 on.
+template <int DP, int G, bool WIDE, bool SLOW, int NT> struct CSectorEval {
+    static constexpr int NC = 2;
+    typedef unsigned Extra;
+    static __device__ __forceinline__ void eval(const typename Res<WIDE>::T (&r)[DP], const SmemCtx<DP, G, NT>&, const unsigned& exbase,
+                                                const EvalCtx& cx, double (&acc)[G][2]) {
+        double x[G][DP], w[G];
+        if (!SLOW) {
+            sector_coords<DP, G, WIDE, TR_KOR3, 0>(r, cx, x, w);
+        } else {
+            sector_coords<DP, G, WIDE, TR_KORR, FIT_RT>(r, cx, x, w);
+        }
+        const unsigned park = exbase + SectorOff::park + 8u * threadIdx.x;
+#pragma unroll
+        for (int q = 0; q < G; ++q) sts_f64(park + 8u * NT * q, w[q]);
+        double Fr[G], Fi[G];
+        {
+            double c0r, c0i;
+            lds_f64x2(exbase + SectorOff::c0u, c0r, c0i);
+#pragma unroll
+            for (int q = 0; q < G; ++q) { Fr[q] = c0r; Fi[q] = c0i; }
+        }
+        csector_interp<DP, G, NT>(x, exbase + SectorOff::words, exbase + SectorOff::slots, park + 64u * NT, Fr, Fi);
+#pragma unroll
+        for (int q = 0; q < G; ++q) w[q] = lds_f64(park + 8u * NT * q);
+        const unsigned long long nup = lds_u64(exbase + SectorOff::nu);
+        const unsigned long long ab = lds_u64(exbase + SectorOff::ab);
+        const int pa = (int)(unsigned)ab, pb = (int)(ab >> 32);
+#pragma unroll
+        for (int j = 0; j < DP; ++j) {
+            const int nu = (int)((nup >> (4 * j)) & 15ull);
+#pragma unroll 1
+            for (int e = 0; e < nu; ++e)
+#pragma unroll
+                for (int q = 0; q < G; ++q) w[q] *= x[q][j];
+        }
+        double nr[G], ni[G], Ur[G], Ui[G];
+#pragma unroll
+        for (int q = 0; q < G; ++q) {
+            nr[q] = w[q]; ni[q] = 0.0;
+            Ur[q] = lds_f64(park + 8u * NT * (8 + 2 * q)); Ui[q] = lds_f64(park + 8u * NT * (9 + 2 * q));
+        }
+#pragma unroll 1
+        for (int e = 0; e < pa; ++e)
+#pragma unroll
+            for (int q = 0; q < G; ++q) {
+                const double t = __fma_rn(nr[q], Ur[q], -(ni[q] * Ui[q]));
+                ni[q] = __fma_rn(nr[q], Ui[q], ni[q] * Ur[q]);
+                nr[q] = t;
+            }
+        // optional log factor (lu Log U + lf Log F)^p, principal branch: a cold, warp-uniform branch
+        const int lp = (int)(unsigned)lds_u64(exbase + SectorOff::logp);
+        if (lp) {
+            const double lu = lds_f64(exbase + SectorOff::lg), lf = lds_f64(exbase + SectorOff::lg + 8u);
+#pragma unroll 1
+            for (int q = 0; q < G; ++q) {
+                const double Lr = __fma_rn(lu, 0.5 * log(__fma_rn(Ur[q], Ur[q], Ui[q] * Ui[q])), lf * (0.5 * log(__fma_rn(Fr[q], Fr[q], Fi[q] * Fi[q]))));
+                const double Li = __fma_rn(lu, atan2(Ui[q], Ur[q]), lf * atan2(Fi[q], Fr[q]));
+                double pr = Lr, pi = Li;
+                for (int e = 1; e < lp; ++e) { const double t = pr * Lr - pi * Li; pi = pr * Li + pi * Lr; pr = t; }
+                const double t = nr[q] * pr - ni[q] * pi;
+                ni[q] = nr[q] * pi + ni[q] * pr;
+                nr[q] = t;
+            }
+        }
+        double dr[G], di[G];
+#pragma unroll
+        for (int q = 0; q < G; ++q) { dr[q] = 1.0; di[q] = 0.0; }
+#pragma unroll 1
+        for (int e = 0; e < pb; ++e)
+#pragma unroll
+            for (int q = 0; q < G; ++q) {
+                const double t = __fma_rn(dr[q], Fr[q], -(di[q] * Fi[q]));
+                di[q] = __fma_rn(dr[q], Fi[q], di[q] * Fr[q]);
+                dr[q] = t;
+            }
+        // n / d = n conj(d) / |d|^2
+#pragma unroll
+        for (int q = 0; q < G; ++q) {
+            const double inv = rcp_nr(__fma_rn(dr[q], dr[q], di[q] * di[q]));
+            acc[q][0] = __fma_rn(__fma_rn(nr[q], dr[q], ni[q] * di[q]), inv, acc[q][0]);
+            acc[q][1] = __fma_rn(__fma_rn(ni[q], dr[q], -(nr[q] * di[q])), inv, acc[q][1]);
+        }
+    }
+};
+
 // shifts per group and threads per CTA by dimension-slot count (x[G][DP] lives in registers; one CTA per SM)
-template <int DP> struct SectorGroup { static constexpr int value = sector_group(DP); };
-template <int DP> struct SectorThreads { static constexpr int value = sector_threads(DP); };
+template <int DP, bool CPLX> struct SectorGroup { static constexpr int value = CPLX ? csector_group(DP) : sector_group(DP); };
+template <int DP, bool CPLX> struct SectorThreads { static constexpr int value = CPLX ? kCSectorThreads : sector_threads(DP); };
 
 template <int DP, int G, int NT> struct SectorShared {
     SmemCtx<DP, G, NT> sm;
     SectorSmem<NT> ex;
 };
 
-template <int DP, int G, bool WIDE, int NT>
+template <int DP, int G, bool WIDE, int NT, bool CPLX>
 __global__ void __launch_bounds__(NT, 1) fused_sector_kernel(const __grid_constant__ FusedLaunch L) {
     const DevAux* __restrict__ aux = L.aux;
     const unsigned long long* __restrict__ prog_area = L.prog;
@@ -414,14 +521,15 @@ __global__ void __launch_bounds__(NT, 1) fused_sector_kernel(const __grid_consta
             const int tid = threadIdx.x;
             const DevAux& a = aux[cur];
             const DevProblem& pb = sm.prob;
+            constexpr int SW = CPLX ? 4 : 2;                 // doubles per coefficient slot
             const int nslots = a.sec_ncoef[0], nwords = a.sec_nops[0];
-            const int nmono_total = (pb.n_params - 4 - pb.dim) / (1 + pb.dim);
+            const int nmono_total = (pb.n_params - 4 - pb.dim) / sector_mono_stride(pb.family, pb.dim);
             const double* slots = reinterpret_cast<const double*>(prog_area + pb.aux_off);
-            const unsigned int* words = reinterpret_cast<const unsigned int*>(prog_area + pb.aux_off + sector_slot_words(nmono_total));
-            for (int i = tid; i < 2 * nslots && i < 2 * kSecMaxSlots; i += NT) ex.slots[i] = slots[i];
+            const unsigned int* words = reinterpret_cast<const unsigned int*>(prog_area + pb.aux_off + sector_slot_words(nmono_total, CPLX));
+            for (int i = tid; i < SW * nslots && i < 4 * kSecMaxSlots; i += NT) ex.slots[i] = slots[i];
             for (int i = tid; i < nwords && i < kSecMaxWords; i += NT) ex.words[i] = words[i];
             if (tid == 32) {
-                ex.c0u = a.sec_c0[0];
+                ex.c0u = a.sec_c0[0]; ex.c0u_im = a.sec_c0i[0];
                 ex.a = a.sec_a; ex.b = a.sec_b;
                 ex.lg[0] = a.sec_log[0]; ex.lg[1] = a.sec_log[1]; ex.logp = a.sec_logp; ex.pad_ = 0;
                 unsigned long long nup = 0;
@@ -431,8 +539,13 @@ __global__ void __launch_bounds__(NT, 1) fused_sector_kernel(const __grid_consta
             __syncthreads();
         }
         const bool fast = !sm.prob.has_fit && sm.prob.tr_kind == TR_KOR3;
-        if (fast) run_tile<SectorEval<DP, G, WIDE, false, NT>, DP, G, WIDE, NT>(sm, sbase, exbase, tile_local, changed, partials);
-        else run_tile_call<SectorEval<DP, G, WIDE, true, NT>, DP, G, WIDE, NT>(sm, sbase, exbase, tile_local, changed, partials);
+        if constexpr (CPLX) {
+            if (fast) run_tile<CSectorEval<DP, G, WIDE, false, NT>, DP, G, WIDE, NT>(sm, sbase, exbase, tile_local, changed, partials);
+            else run_tile_call<CSectorEval<DP, G, WIDE, true, NT>, DP, G, WIDE, NT>(sm, sbase, exbase, tile_local, changed, partials);
+        } else {
+            if (fast) run_tile<SectorEval<DP, G, WIDE, false, NT>, DP, G, WIDE, NT>(sm, sbase, exbase, tile_local, changed, partials);
+            else run_tile_call<SectorEval<DP, G, WIDE, true, NT>, DP, G, WIDE, NT>(sm, sbase, exbase, tile_local, changed, partials);
+        }
     }
 }
 

@@ -78,6 +78,8 @@ def make(fam, d, n, m, tr, seed, fit=False, z=None, a_hi=1.0):
         prm = synth.genz_prodpeak(rng, d)
     elif fam == 2:
         prm = synth.cexp_poly(rng, d)
+    elif fam == 8:
+        prm = synth.sector_complex(rng, d)                   # complex sector polynomials (reading C-16)
     elif fam >= 4:
         prm = synth.genz_protocol(rng, fam, d)               # Genz families 3-6 at the paper's difficulties
     else:
@@ -704,3 +706,71 @@ def test_projection_rejects_a_malformed_sector_block():
     assert np.all(np.isnan(H2))
     good = binding.DeviceBatch([p]).project(0, 64).cpu().numpy()
     assert np.all(np.isfinite(good))
+
+
+# ------------------------------------------------------------------------------------------------
+# family 8: sector polynomials with complex coefficients (contour-deformed shape, reading C-16)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("d", [1, 2, 3, 4, 5, 6, 7, 8, 11, 16])
+def test_complex_sector_all_slot_counts(d):
+    """every dimension-slot variant of the complex sector kernels (4 / 6 / 8 / 16 slots; groups of 4 or 2 shifts), m not a
+    multiple of the group, against the oracle at 1e-13 of the modulus"""
+    check_against_oracle([make(8, d, 8191, 7, K + 3, 9500 + d), make(8, d, 4099, 2, K + 3, 9520 + d)])
+
+
+@pytest.mark.parametrize("tr,fit", [(NONE, False), (BAKER, False), (K + 1, False), (K + 3, True), (K + 3, "full"), (SIDI + 2, False),
+                                    (KA + 16 * 2 + 1, True)])
+def test_complex_sector_transforms_and_fit(tr, fit):
+    check_against_oracle([make(8, 6, 8191, 9, tr, 9540 + tr % 89, fit=fit), make(8, 3, 8191, 5, tr, 9560 + tr % 89, fit=fit)])
+
+
+def test_complex_sector_log_factors_and_mixed_batch():
+    """principal-branch log factors (p = 1..3) and a batch mixing both sector families with closed-form ones"""
+    rng = synth.MT19937_64(9580)
+    probs = []
+    for i, d in enumerate((2, 4, 6, 6, 8)):
+        prm = synth.sector_complex(rng, d, log_block=True)
+        probs.append(synth.problem(8, prm, 8191, synth.korobov_form_vector(8191, d, 2731), synth.draw_shifts(rng, 6, d), K + 3,
+                                   name=f"csector.log.d{d}"))
+    probs += [make(3, 6, 8191, 16, K + 3, 9590), make(8, 6, 8191, 16, K + 3, 9591), make(2, 12, 4099, 4, K + 3, 9592),
+              make(1, 8, 4099, 5, BAKER, 9593)]
+    check_against_oracle(probs)
+
+
+def test_complex_sector_contour_deformation_value():
+    """the Cauchy pin of the oracle, end to end on the GPU: the deformed one- and two-dimensional integrals keep their real
+    values for every lambda"""
+    c = 0.7
+    rng = synth.MT19937_64(9600)
+    def block(a, b, nu, U, F):
+        d = len(nu)
+        out = [float(a), float(b), float(len(U)), float(len(F))] + [float(v) for v in nu]
+        for poly in (U, F):
+            out += [complex(cc).real for cc, _ in poly] + [complex(cc).imag for cc, _ in poly]
+            for _, e in poly:
+                out += [float(v) for v in e]
+        return np.array(out)
+    for lam in (0.0, 0.6, 2.0):
+        prm = block(1, 2, [0, 0], [(1.0 - 1j * lam, (0, 0)), (2j * lam, (1, 0))],
+                    [(c, (0, 0)), (1.0 - 1j * lam, (1, 0)), (1j * lam, (2, 0)), (1.0, (0, 1))])
+        p = synth.problem(8, prm, 1048573, synth.genvec(1048573, 8)[:2], synth.draw_shifts(rng, 8, 2), K + 3, name=f"cauchy.lam{lam}")
+        sms, means, errs = check_against_oracle([p])
+        exact = np.log((c + 1.0) ** 2 / (c * (c + 2.0)))
+        assert abs(means[0, 0] - exact) < 1e-9 and abs(means[0, 1]) < 1e-9
+
+
+def test_complex_sector_projection_and_adaptive():
+    """projection histogram of |f| (modulus) against the oracle; qmc_integrate with both error modes ends on the oracle's (n, m)"""
+    p = make(8, 5, 8191, 2, NONE, 9610)
+    H_or = oracle.project(p, 128)
+    H = binding.DeviceBatch([p]).project(0, 128).cpu().numpy()
+    assert np.all(np.abs(H - H_or) <= 1e-12 * np.maximum(np.abs(H_or), 1e-300))
+    q = make(8, 4, 8191, 8, K + 3, 9611)
+    ln, lz = synth.ladder(4, 65521)
+    for errormode in (0, 1):
+        res, st = binding.qmc_integrate(8, q["params"], 4, K + 3, ln, lz, q["shifts"], min_n=1000, min_m=8, epsrel=1e-6, epsabs=0.0,
+                                        maxeval=10 ** 9, errormode=errormode)
+        i = list(ln).index(res["n"])
+        ref = synth.problem(8, q["params"], res["n"], lz[i], q["shifts"][:res["m"]], K + 3)
+        sm_or, mean_or, err_or = oracle.integrate(ref)
+        assert np.all(np.abs(res["integral"] - mean_or) <= 1e-13 * np.hypot(*mean_or))
