@@ -42,6 +42,8 @@ def lib():
         L.oracle_integrate.argtypes = [C.c_int, dp, C.c_int, C.c_int, C.c_uint64, up, dp, C.c_int, C.c_int, dp, dp, dp, dp]
         L.oracle_project.argtypes = [C.c_int, dp, C.c_int, C.c_int, C.c_uint64, up, dp, C.c_int, dp]
         L.oracle_fit_cubic.argtypes = [dp, C.c_int, C.c_int, dp]
+        L.oracle_cdf_samples.argtypes = [C.c_int, dp, C.c_int, C.c_int, C.c_uint64, up, dp, C.c_int, dp, dp]
+        L.oracle_fit_cubic_cdf.argtypes = [dp, dp, C.c_int, C.c_uint64, dp]
         _lib = L
     return _lib
 
@@ -156,4 +158,24 @@ def fit_cubic(hist):
     d, bins = H.shape
     out = np.zeros((d, 6))
     lib().oracle_fit_cubic(_d(H), d, bins, _d(out))
+    return out
+
+
+def cdf_samples(p, step=10, shift=None):
+    """The paper's sort-based CDF sampling (PAPER.md L226-L231, L958-L960) -> (x (dim, K), cdf (dim, K)), K = n // step."""
+    params, z = _f64(p["params"]), _u64(p["z"])
+    shift = _f64(p["shifts"][0] if shift is None else shift)
+    K = p["n"] // step
+    xs, cdf = np.zeros((p["dim"], K)), np.zeros((p["dim"], K))
+    st = lib().oracle_cdf_samples(p["family"], _d(params), len(params), p["dim"], p["n"], _u(z), _d(shift), int(step), _d(xs), _d(cdf))
+    if st:
+        raise ValueError(f"oracle_cdf_samples status {st}")
+    return xs, cdf
+
+
+def fit_cubic_cdf(xs, cdf):
+    xs, cdf = _f64(xs), _f64(cdf)
+    d, K = xs.shape
+    out = np.zeros((d, 6))
+    lib().oracle_fit_cubic_cdf(_d(xs), _d(cdf), d, K, _d(out))
     return out

@@ -34,6 +34,7 @@
 // oracle).
 //
 // Build: g++ -O2 -std=c++17 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/build.py).
+#include <algorithm>
 #include <cmath>
 #include <complex>
 #include <cstdint>
@@ -445,6 +446,71 @@ int oracle_project(int fam, const double* params, int n_params, int dim, uint64_
         }
     }
     for (size_t q = 0; q < H.size(); ++q) out_hist[q] = H[q].value();
+    return 0;
+}
+
+// O9b (the paper's own CDF sampling; reading C-8b): the integrand is sampled on the n points of one
+// shifted lattice (transform None, weight 1); per dimension j the samples are sorted by x_j ("after sorting by value"), the
+// running sum of |f| over the sorted samples divided by the total is the empirical CDF of Eq. 20 at the sorted coordinates, and
+// every `step`-th sorted point is kept (fitstepsize, default 10): kept point t = 1..K, K = floor(n / step), is the sorted sample
+// with 0-based rank t * step - 1.  out_x, out_cdf: [dim][K].  Equal coordinates keep their index order (stable sort).
+int oracle_cdf_samples(int fam, const double* params, int n_params, int dim, uint64_t n, const uint64_t* z, const double* shift,
+                       int step, double* out_x, double* out_cdf) {
+    if (fam < 0 || fam > FAM_LAST) return -8;
+    if (dim < 1 || dim > MAX_DIM) return -2;
+    if (step < 1 || (uint64_t)step > n) return -3;
+    if (expected_params(fam, params, n_params, dim) != n_params) return -9;
+    const double inv_n = 1.0 / (double)n;
+    const uint64_t K = n / (uint64_t)step;
+    std::vector<double> xs((size_t)dim * n), v(n);
+    double x[MAX_DIM];
+    for (uint64_t k = 0; k < n; ++k) {
+        for (int j = 0; j < dim; ++j) { x[j] = coordinate(residue(k, z[j], n), inv_n, shift[j]); xs[(size_t)j * n + k] = x[j]; }
+        double re, im; integrand(fam, params, n_params, dim, x, &re, &im);
+        v[k] = ncomp_of(fam) == 2 ? std::hypot(re, im) : std::fabs(re);
+    }
+    Comp tot; for (uint64_t k = 0; k < n; ++k) tot.add(v[k]);
+    const double total = tot.value();
+    std::vector<uint64_t> order(n);
+    for (int j = 0; j < dim; ++j) {
+        const double* xj = xs.data() + (size_t)j * n;
+        for (uint64_t k = 0; k < n; ++k) order[k] = k;
+        std::stable_sort(order.begin(), order.end(), [xj](uint64_t a, uint64_t b) { return xj[a] < xj[b]; });
+        Comp run;
+        uint64_t t = 0;
+        for (uint64_t i = 0; i < n; ++i) {
+            run.add(v[order[i]]);
+            if ((i + 1) % (uint64_t)step == 0 && t < K) {
+                out_x[(size_t)j * K + t] = xj[order[i]];
+                out_cdf[(size_t)j * K + t] = run.value() / total;
+                ++t;
+            }
+        }
+    }
+    return 0;
+}
+
+// Cubic fit of the inverse CDF from sampled pairs (c_t, x_t) (reading C-8b): minimise sum_t (p(c_t) - x_t)^2 over (a4, a5) with
+// p(c) = c^3 + a4 (c - c^3) + a5 (c^2 - c^3); identity if min p' on [0,1] <= 0.05 or the system is singular.
+int oracle_fit_cubic_cdf(const double* xs, const double* cdf, int dim, uint64_t count, double* fit_coeffs) {
+    for (int j = 0; j < dim; ++j) {
+        double A11 = 0, A12 = 0, A22 = 0, B1 = 0, B2 = 0;
+        for (uint64_t t = 0; t < count; ++t) {
+            const double c = cdf[(size_t)j * count + t], e = xs[(size_t)j * count + t];
+            const double c3 = c * c * c, g1 = c - c3, g2 = c * c - c3, r = e - c3;
+            A11 += g1 * g1; A12 += g1 * g2; A22 += g2 * g2; B1 += g1 * r; B2 += g2 * r;
+        }
+        double a4 = 1.0, a5 = 0.0;
+        const double det = A11 * A22 - A12 * A12;
+        if (std::fabs(det) > 1e-300) {
+            const double c4 = (B1 * A22 - B2 * A12) / det, c5 = (A11 * B2 - A12 * B1) / det, c6 = 1.0 - c4 - c5;
+            double mn = std::fmin(c4, c4 + 2.0 * c5 + 3.0 * c6);
+            if (c6 != 0.0) { const double yv = -c5 / (3.0 * c6); if (yv > 0.0 && yv < 1.0) mn = std::fmin(mn, c4 + yv * (2.0 * c5 + 3.0 * c6 * yv)); }
+            if (mn > 0.05) { a4 = c4; a5 = c5; }
+        }
+        double* o = fit_coeffs + 6 * j;
+        o[0] = 1.001; o[1] = -0.001; o[2] = 0.0; o[3] = 0.0; o[4] = a4; o[5] = a5;
+    }
     return 0;
 }
 

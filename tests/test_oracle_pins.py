@@ -686,3 +686,63 @@ def test_complex_sector_whole_rule():
         assert sm.shape == (16, 2) and err.shape == (2,)
         assert abs(mean[0] - exact) <= 6 * err[0] + 1e-12 and abs(mean[1]) <= 6 * err[1] + 1e-12
         assert abs(mean[0] - exact) < 1e-7
+
+
+# ------------------------------------------------------------------------------------------------
+# O9b: the paper's sort-based CDF sampling (reading C-8b)
+# ------------------------------------------------------------------------------------------------
+def test_cdf_samples_constant_integrand():
+    """f = 1 (product of (1 + 0 x)): the empirical CDF at the t-th kept point is exactly t * step / n and the kept
+    coordinates are the (t * step)-th smallest of the lattice's coordinates, whatever the dimension"""
+    n, step, d = 1021, 10, 3
+    rng = synth.MT19937_64(77001)
+    p = synth.problem(2, np.zeros(2 * d), n, synth.korobov_form_vector(n, d, 341), synth.draw_shifts(rng, 1, d), synth.TRANSFORM_NONE)
+    xs, cdf = oracle.cdf_samples(p, step)
+    K = n // step
+    assert xs.shape == (d, K)
+    _, u = oracle.lattice_points(n, p["z"], p["shifts"][0], 0, n)
+    for j in range(d):
+        srt = np.sort(u[:, j])
+        assert np.array_equal(xs[j], srt[step - 1::step][:K])
+        np.testing.assert_allclose(cdf[j], (np.arange(1, K + 1) * step) / n, rtol=1e-15)
+
+
+def test_cdf_samples_follow_the_marginal_cdf_in_closed_form():
+    """product peak: the marginal CDF of dimension j is (atan(c (x - w)) + atan(c w)) / (atan(c (1 - w)) + atan(c w)); the
+    sampled CDF must follow it to O(1/n) + the lattice's integration error; coordinates ascending, CDF non-decreasing, ends near 1"""
+    n, step, d = 65537, 10, 4
+    rng = synth.MT19937_64(77002)
+    prm = synth.genz_prodpeak(rng, d)
+    p = synth.problem(1, prm, n, synth.genvec(n, 4), synth.draw_shifts(rng, 1, d), synth.TRANSFORM_NONE)
+    xs, cdf = oracle.cdf_samples(p, step)
+    c, w = prm[:d], prm[d:]
+    for j in range(d):
+        assert np.all(np.diff(xs[j]) > 0) and np.all(np.diff(cdf[j]) >= 0)
+        exact = (np.arctan(c[j] * (xs[j] - w[j])) + np.arctan(c[j] * w[j])) / (np.arctan(c[j] * (1 - w[j])) + np.arctan(c[j] * w[j]))
+        assert np.max(np.abs(cdf[j] - exact)) < 2e-3
+        assert 1.0 - cdf[j][-1] < 2.0 * step / n * 30
+
+
+def test_cdf_samples_one_dimension_by_hand():
+    """n = 11, z = 1, shift 0.05, f = 1 + 2 x (complex exp * poly family with a = 0, b = 2: |f| = 1 + 2x), step = 3: the three
+    kept points and their cumulative sums written out with exact rationals"""
+    n, step = 11, 3
+    p = synth.problem(2, np.array([0.0, 2.0]), n, [1], np.array([[0.05]]), synth.TRANSFORM_NONE)
+    xs, cdf = oracle.cdf_samples(p, step)
+    x_all = sorted(Fraction(k, n) + Fraction(1, 20) for k in range(n))           # no wrap: 10/11 + 0.05 < 1
+    f_all = [1 + 2 * x for x in x_all]
+    tot = sum(f_all)
+    for t in range(1, n // step + 1):
+        i = t * step - 1
+        assert abs(xs[0, t - 1] - float(x_all[i])) <= 2e-16
+        assert abs(cdf[0, t - 1] - float(sum(f_all[:i + 1]) / tot)) <= 1e-15
+
+
+def test_cubic_fit_from_cdf_samples_recovers_an_exact_cubic():
+    """pairs (c, x) with x = p(c) for a cubic p of the family: the least squares returns its (a4, a5)"""
+    a4, a5 = 0.55, 0.35
+    c = np.linspace(0.001, 0.999, 500)
+    x = c * (a4 + c * (a5 + c * (1 - a4 - a5)))
+    out = oracle.fit_cubic_cdf(np.stack([x, x]), np.stack([c, c]))
+    assert np.allclose(out[:, 4], a4, atol=1e-12) and np.allclose(out[:, 5], a5, atol=1e-12)
+    assert np.all(out[:, 2] == 0) and np.all(out[:, 3] == 0)
