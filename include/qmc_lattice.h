@@ -203,6 +203,27 @@ int qmc_fit_cubic(const double* hist /*HOST [dim][bins]*/, int dim, int bins, do
  * increasing on [0,1].  bins in 8..1024.  hist, fit_coeffs: HOST.  The result is valid input for every compute entry. */
 int qmc_fit_polysingular(const double* hist /*HOST [dim][bins]*/, int dim, int bins, double* fit_coeffs /*HOST [dim][6]*/);
 
+/* The paper's own CDF sampling for the fit (`evaluate`; fitstepsize; DESIGN.md reading
+ * C-8b): |f| on the n points of the lattice shifted by the first shift of p (transform None, weight 1); per dimension j the
+ * samples sorted by x_j, the running sum of |f| over the sorted samples divided by the total, every fitstepsize-th sorted sample
+ * kept: for t = 1..K, K = n / fitstepsize (qmc_cdf_sample_count),
+ *   out_x[j*K + t-1]   = the (t * fitstepsize)-th smallest coordinate x_j of the lattice,
+ *   out_cdf[j*K + t-1] = sum of |f| over the t * fitstepsize samples with the smallest x_j / sum over all samples.
+ * No sort is performed: in one dimension the sorted order of a shifted rank-1 lattice is the cyclic order of its residues, so
+ * every sample is scattered to its rank.  Stream-ordered, deterministic.  p: HOST struct with DEVICE data pointers (p->m >= 1;
+ * transform and fit_coeffs ignored).  out_x, out_cdf: DEVICE, dim*K doubles.  A sector block that fails the device-side
+ * validation gives NaN outputs. */
+int qmc_lattice_cdf_samples(const qmc_problem* p /*HOST*/, int fitstepsize, double* out_x /*DEVICE*/, double* out_cdf /*DEVICE*/,
+                            void* workspace /*DEVICE*/, size_t workspace_bytes, void* cuda_stream);
+size_t qmc_cdf_workspace_bytes(const qmc_problem* p /*HOST*/, int fitstepsize);
+long long qmc_cdf_sample_count(uint64_t n, int fitstepsize);        /* K; 0 if fitstepsize is outside 1..n */
+
+/* Host-side fits from those samples: pairs (CDF_t, x_t), p(CDF_t) ~ x_t.  with_poles = 0: cubic sub-family, closed-form least
+ * squares (identity map if not safely monotone); 1: the complete fit function of Eq. 19 by the bounded Levenberg-Marquardt of
+ * qmc_fit_polysingular.  x, cdf: HOST [dim][count]; count >= 8. */
+int qmc_fit_from_cdf(const double* x /*HOST*/, const double* cdf /*HOST*/, int dim, long long count, int with_poles,
+                     double* fit_coeffs /*HOST [dim][6]*/);
+
 /* Inspection: residues r = (k z_j) mod n and coordinates u = {r/n + shift_j} for k = k0..k0+count-1,
  * produced by the same device code the fused kernel uses (Eq. 2; fp64 realisation:
  * u = wrap(fma(double(r), 1/double(n), shift_j)), reading C-2).

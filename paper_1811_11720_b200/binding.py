@@ -21,7 +21,8 @@ EXPORTS = [
     "qmc_profile_enable", "qmc_profile_last_fused_ms",
     "qmc_num_components", "qmc_status_string", "qmc_last_cuda_error", "qmc_integrate", "qmc_fit_polysingular",
     "qmc_lattice_integrate_batch_opts", "qmc_workspace_bytes_opts", "qmc_lattice_integrate_batch_host",
-    "qmc_release_thread_resources", "qmc_sector_compile",
+    "qmc_release_thread_resources", "qmc_sector_compile", "qmc_lattice_cdf_samples", "qmc_cdf_workspace_bytes",
+    "qmc_cdf_sample_count", "qmc_fit_from_cdf",
 ]
 
 QMC_OK = 0
@@ -84,6 +85,12 @@ def lib():
         L.qmc_project_workspace_bytes.argtypes = [pp, C.c_int]
         L.qmc_project_workspace_bytes.restype = C.c_size_t
         L.qmc_fit_cubic.argtypes = [dp, C.c_int, C.c_int, dp]
+        L.qmc_lattice_cdf_samples.argtypes = [pp, C.c_int, vp, vp, vp, C.c_size_t, vp]
+        L.qmc_cdf_workspace_bytes.argtypes = [pp, C.c_int]
+        L.qmc_cdf_workspace_bytes.restype = C.c_size_t
+        L.qmc_cdf_sample_count.argtypes = [C.c_uint64, C.c_int]
+        L.qmc_cdf_sample_count.restype = C.c_longlong
+        L.qmc_fit_from_cdf.argtypes = [dp, dp, C.c_int, C.c_longlong, C.c_int, dp]
         L.qmc_fit_polysingular.argtypes = [dp, C.c_int, C.c_int, dp]
         L.qmc_lattice_points.argtypes = [C.c_uint64, C.c_int, up, dp, C.c_uint64, C.c_uint64, vp, vp, vp]
         L.qmc_finalize_means.argtypes = [vp, C.c_int, C.c_int, vp, vp, vp]
@@ -216,6 +223,15 @@ def qmc_fit_cubic(hist):
     return out
 
 
+def qmc_fit_from_cdf(x, cdf, with_poles=False):
+    """Fit of Eq. 19 (cubic sub-family, or complete with pole terms) to the sort-based CDF samples -> (dim, 6)."""
+    X, Cd = _f64(x), _f64(cdf)
+    d, K = X.shape
+    out = np.zeros((d, 6))
+    _check(lib().qmc_fit_from_cdf(_d(X), _d(Cd), d, K, 1 if with_poles else 0, _d(out)), "qmc_fit_from_cdf")
+    return out
+
+
 def qmc_fit_polysingular(hist):
     """Bounded Levenberg-Marquardt fit of the complete fit function of Eq. 19 -> (dim, 6) coefficients a_0..a_5."""
     H = _f64(hist)
@@ -301,6 +317,27 @@ class DeviceBatch:
             nc = qmc_num_components(p["family"])
             out.append(sm[i, : p["m"] * nc].reshape(p["m"], nc).copy())
         return out, means, errs
+
+    def cdf_samples(self, index=0, fitstepsize=10, stream=None, sync=True):
+        """qmc_lattice_cdf_samples for problem `index` -> torch tensors (x (dim, K), cdf (dim, K)) on the device."""
+        torch = self.torch
+        p = self.problems[index]
+        one = (qmc_problem * 1)(self.arr[index])
+        K = int(lib().qmc_cdf_sample_count(p["n"], int(fitstepsize)))
+        need = int(lib().qmc_cdf_workspace_bytes(one, int(fitstepsize)))
+        if K == 0 or need == 0:
+            raise QmcError(-3, "qmc_cdf_workspace_bytes")
+        ws = torch.empty(need + 256, dtype=torch.uint8, device=self.device)
+        ptr = ws.data_ptr() + ((-ws.data_ptr()) % 256)
+        xs = torch.zeros(p["dim"], K, dtype=torch.float64, device=self.device)
+        cdf = torch.zeros(p["dim"], K, dtype=torch.float64, device=self.device)
+        s = torch.cuda.current_stream(self.device).cuda_stream if stream is None else stream
+        _check(lib().qmc_lattice_cdf_samples(one, int(fitstepsize), xs.data_ptr(), cdf.data_ptr(), ptr, need, s), "qmc_lattice_cdf_samples")
+        if sync:
+            torch.cuda.synchronize(self.device)
+        else:
+            self._keep_ws = (ws, xs, cdf)
+        return xs, cdf
 
     def project(self, index=0, bins=256, stream=None, sync=True):
         """qmc_lattice_project for problem `index` -> torch tensor (dim, bins) on the device."""

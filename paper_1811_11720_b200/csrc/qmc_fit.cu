@@ -72,6 +72,72 @@ bool solve6(long double A[6][6], long double* b) {               // Gaussian eli
     return true;
 }
 
+// Bounded Levenberg-Marquardt fit of Eq. 19 to pairs (c_i, e_i): p(c_i) ~ e_i.  o: in, the cubic solution (a4, a5 used as the
+// start); out, the full parameter set if it is a strictly better valid fit.
+void fit_full_pairs(const std::vector<long double>& c, const std::vector<long double>& e, double* o) {
+    long double a[6] = {1.1L, -0.1L, 0.0L, 0.0L, o[4], o[5]};
+    // two starts: the cubic solution with dormant poles, and the same with small active poles (the gradient of a0, a1 vanishes
+    // while a2 = a3 = 0)
+    long double best[6], best_cost = cost(a, c, e);
+    for (int k = 0; k < 6; ++k) best[k] = a[k];
+    for (int start = 0; start < 2; ++start) {
+        long double th[6] = {1.1L, -0.1L, start ? 0.05L : 0.0L, start ? 0.05L : 0.0L, o[4], o[5]};
+        long double cur = cost(th, c, e), lambda = 1e-3L;
+        for (int it = 0; it < 400; ++it) {
+            long double JTJ[6][6] = {}, JTr[6] = {};
+            for (size_t b = 0; b < c.size(); ++b) {
+                long double g[6];
+                const long double r = Model::eval(th, c[b], g) - e[b];
+                for (int p = 0; p < 6; ++p) { JTr[p] += g[p] * r; for (int q = 0; q < 6; ++q) JTJ[p][q] += g[p] * g[q]; }
+            }
+            long double A[6][6], rhs[6];
+            for (int p = 0; p < 6; ++p) {
+                rhs[p] = -JTr[p];
+                for (int q = 0; q < 6; ++q) A[p][q] = JTJ[p][q];
+                A[p][p] += lambda * std::max(JTJ[p][p], 1e-12L);
+            }
+            if (!solve6(A, rhs)) { lambda *= 10.0L; continue; }
+            long double trial[6];
+            for (int p = 0; p < 6; ++p) trial[p] = th[p] + rhs[p];
+            project(trial);
+            const long double tc = cost(trial, c, e);
+            if (tc < cur) {
+                const long double gain = (cur - tc) / std::max(cur, 1e-300L);
+                for (int p = 0; p < 6; ++p) th[p] = trial[p];
+                cur = tc;
+                lambda = std::max(lambda / 3.0L, 1e-12L);
+                if (gain < 1e-12L) break;
+            } else {
+                lambda *= 4.0L;
+                if (lambda > 1e12L) break;
+            }
+        }
+        if (cur < best_cost && Model::increasing(th)) { best_cost = cur; for (int k = 0; k < 6; ++k) best[k] = th[k]; }
+    }
+    // keep the cubic result unless the full function is a strictly better, valid fit
+    const long double cubic[6] = {1.1L, -0.1L, 0.0L, 0.0L, o[4], o[5]};
+    if (best_cost < cost(cubic, c, e) && Model::increasing(best) && (best[2] > 0.0L || best[3] > 0.0L))
+        for (int k = 0; k < 6; ++k) o[k] = (double)best[k];
+}
+
+// Closed-form least squares for the cubic sub-family on pairs (c_i, e_i) (as qmc_fit_cubic): identity if not safely monotone.
+void fit_cubic_pairs(const std::vector<long double>& cs, const std::vector<long double>& es, double* o) {
+    long double s11 = 0, s12 = 0, s22 = 0, t1 = 0, t2 = 0;
+    for (size_t i = 0; i < cs.size(); ++i) {
+        const long double c = cs[i], c3 = c * c * c, g1 = c - c3, g2 = c * c - c3, rhs = es[i] - c3;
+        s11 += g1 * g1; s12 += g1 * g2; s22 += g2 * g2; t1 += g1 * rhs; t2 += g2 * rhs;
+    }
+    double a4 = 1.0, a5 = 0.0;
+    const long double det = s11 * s22 - s12 * s12;
+    if (fabsl(det) > 1e-300L) {
+        const double c4 = (double)((t1 * s22 - t2 * s12) / det), c5 = (double)((s11 * t2 - s12 * t1) / det), c6 = 1.0 - c4 - c5;
+        double mn = std::fmin(c4, c4 + 2.0 * c5 + 3.0 * c6);
+        if (c6 != 0.0) { const double yv = -c5 / (3.0 * c6); if (yv > 0.0 && yv < 1.0) mn = std::fmin(mn, c4 + yv * (2.0 * c5 + 3.0 * c6 * yv)); }
+        if (mn > 0.05) { a4 = c4; a5 = c5; }
+    }
+    o[0] = 1.001; o[1] = -0.001; o[2] = 0.0; o[3] = 0.0; o[4] = a4; o[5] = a5;
+}
+
 }  // namespace
 
 extern "C" int qmc_fit_polysingular(const double* hist, int dim, int bins, double* fit_coeffs) {
@@ -89,50 +155,29 @@ extern "C" int qmc_fit_polysingular(const double* hist, int dim, int bins, doubl
         std::vector<long double> c, e;                             // CDF values at the bin edges: p(c_b) = e_b (Eq. 18-20)
         long double run = 0.0L;
         for (int b = 1; b < bins; ++b) { run += h[b - 1]; c.push_back(run / total); e.push_back((long double)b / bins); }
-        double* o = fit_coeffs + 6 * j;
-        long double a[6] = {1.1L, -0.1L, 0.0L, 0.0L, o[4], o[5]};
-        // two starts: the cubic solution with dormant poles, and the same with small active poles (the gradient of a0, a1 vanishes
-        // while a2 = a3 = 0)
-        long double best[6], best_cost = cost(a, c, e);
-        for (int k = 0; k < 6; ++k) best[k] = a[k];
-        for (int start = 0; start < 2; ++start) {
-            long double th[6] = {1.1L, -0.1L, start ? 0.05L : 0.0L, start ? 0.05L : 0.0L, o[4], o[5]};
-            long double cur = cost(th, c, e), lambda = 1e-3L;
-            for (int it = 0; it < 400; ++it) {
-                long double JTJ[6][6] = {}, JTr[6] = {};
-                for (size_t b = 0; b < c.size(); ++b) {
-                    long double g[6];
-                    const long double r = Model::eval(th, c[b], g) - e[b];
-                    for (int p = 0; p < 6; ++p) { JTr[p] += g[p] * r; for (int q = 0; q < 6; ++q) JTJ[p][q] += g[p] * g[q]; }
-                }
-                long double A[6][6], rhs[6];
-                for (int p = 0; p < 6; ++p) {
-                    rhs[p] = -JTr[p];
-                    for (int q = 0; q < 6; ++q) A[p][q] = JTJ[p][q];
-                    A[p][p] += lambda * std::max(JTJ[p][p], 1e-12L);
-                }
-                if (!solve6(A, rhs)) { lambda *= 10.0L; continue; }
-                long double trial[6];
-                for (int p = 0; p < 6; ++p) trial[p] = th[p] + rhs[p];
-                project(trial);
-                const long double tc = cost(trial, c, e);
-                if (tc < cur) {
-                    const long double gain = (cur - tc) / std::max(cur, 1e-300L);
-                    for (int p = 0; p < 6; ++p) th[p] = trial[p];
-                    cur = tc;
-                    lambda = std::max(lambda / 3.0L, 1e-12L);
-                    if (gain < 1e-12L) break;
-                } else {
-                    lambda *= 4.0L;
-                    if (lambda > 1e12L) break;
-                }
-            }
-            if (cur < best_cost && Model::increasing(th)) { best_cost = cur; for (int k = 0; k < 6; ++k) best[k] = th[k]; }
+        fit_full_pairs(c, e, fit_coeffs + 6 * j);
+    }
+    return QMC_OK;
+}
+
+
+// The same two fits from the paper's sort-based CDF samples (qmc_lattice_cdf_samples): pairs
+// (CDF_t, x_t), p(CDF_t) ~ x_t.  x, cdf: HOST [dim][count].  with_poles = 0: cubic sub-family in closed form; 1: Eq. 19 complete.
+extern "C" int qmc_fit_from_cdf(const double* x, const double* cdf, int dim, long long count, int with_poles, double* fit_coeffs) {
+    if (!x || !cdf || !fit_coeffs) return QMC_ERR_NULL;
+    if (dim < 1 || dim > QMC_MAX_DIM) return QMC_ERR_DIM;
+    if (count < 8) return QMC_ERR_N;
+    for (int j = 0; j < dim; ++j) {
+        std::vector<long double> c((size_t)count), e((size_t)count);
+        bool ok = true;
+        for (long long t = 0; t < count; ++t) {
+            c[t] = cdf[(size_t)j * count + t]; e[t] = x[(size_t)j * count + t];
+            ok = ok && std::isfinite((double)c[t]) && std::isfinite((double)e[t]);
         }
-        // keep the cubic result unless the full function is a strictly better, valid fit
-        const long double cubic[6] = {1.1L, -0.1L, 0.0L, 0.0L, o[4], o[5]};
-        if (best_cost < cost(cubic, c, e) && Model::increasing(best) && (best[2] > 0.0L || best[3] > 0.0L))
-            for (int k = 0; k < 6; ++k) o[k] = (double)best[k];
+        double* o = fit_coeffs + 6 * j;
+        if (!ok) { o[0] = 1.001; o[1] = -0.001; o[2] = 0.0; o[3] = 0.0; o[4] = 1.0; o[5] = 0.0; continue; }   // identity map
+        fit_cubic_pairs(c, e, o);
+        if (with_poles) fit_full_pairs(c, e, o);
     }
     return QMC_OK;
 }

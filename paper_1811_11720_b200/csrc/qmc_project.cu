@@ -214,6 +214,121 @@ __global__ void __launch_bounds__(256) project_merge_kernel(ProjArgs a) {
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// S10b: the paper's own CDF sampling (all samples sorted per dimension, every fitstepsize-th
+// kept; reading C-8b) WITHOUT a sort.  In dimension j the coordinate of lattice index k is x = wrap(fma(r, 1/n, Delta_j)),
+// r = k z_j mod n, and both branches of the wrap are increasing in r: sorted by x the samples come in the cyclic residue
+// order r0, r0+1, ..., n-1, 0, ..., r0-1 with r0 the first residue that wraps.  The rank of sample k is therefore
+// (r - r0) mod n: the samples are SCATTERED to their ranks, summed in buckets of `step` consecutive ranks and scanned.
+// Fixed shapes (a function of n and step only): deterministic, no floating-point atomics.
+//   cdf_eval_kernel     v[k] = |f(x_k)|
+//   cdf_scatter_kernel  vs[j][rank_j(k)] = v[k]
+//   cdf_scan_kernel     one CTA per dimension: bucket sums, block scan, total; writes x_t and CDF_t, t = 1..K
+// ---------------------------------------------------------------------------------------------
+struct CdfArgs {
+    ProjArgs pa;                 // params, z, shift, n, inv_n, family, dim, n_params (bins unused)
+    int step;                    // fitstepsize
+    long long K;                 // kept points per dimension = n / step
+    double* v;                   // [n]
+    double* vs;                  // [dim][n]
+    unsigned long long* r0;      // [dim] first residue whose coordinate wraps (n if none)
+    double* out_x;               // [dim][K]
+    double* out_cdf;             // [dim][K]
+    int* status;                 // device flag: sector block invalid -> outputs NaN
+};
+
+// first residue r with fma(r, 1/n, delta) >= 1 (the sum is non-decreasing in r), n if there is none
+__device__ unsigned long long first_wrapping_residue(unsigned long long n, double inv_n, double delta) {
+    unsigned long long lo = 0, hi = n;                       // answer in [lo, hi]
+    while (lo < hi) {
+        const unsigned long long mid = lo + (hi - lo) / 2;
+        if (ge_one(coord_t((double)mid, inv_n, delta))) hi = mid; else lo = mid + 1;
+    }
+    return lo;
+}
+
+__global__ void __launch_bounds__(256) cdf_eval_kernel(CdfArgs c) {
+    extern __shared__ double sp[];                           // the parameter block
+    __shared__ int block_status;
+    ProjArgs a = c.pa;
+    for (int i = threadIdx.x; i < a.n_params; i += blockDim.x) sp[i] = a.params[i];
+    if (threadIdx.x == 0) block_status = is_sector_family(a.family) ? sector_block_status(a.params, a.n_params, a.dim, a.family == QMC_FAMILY_SECTOR_COMPLEX) : 0;
+    __syncthreads();
+    if (block_status != 0) { if (blockIdx.x == 0 && threadIdx.x == 0) *c.status = block_status; return; }
+    if (blockIdx.x == 0 && threadIdx.x < a.dim) c.r0[threadIdx.x] = first_wrapping_residue(a.n, a.inv_n, a.shift[threadIdx.x]);
+    a.params = sp;
+    const unsigned long long n = a.n, stride = (unsigned long long)gridDim.x * blockDim.x;
+    double x[QMC_MAX_DIM];
+    for (unsigned long long k = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += stride) {
+        for (int j = 0; j < a.dim; ++j) x[j] = wrap_u(coord_t((double)mulmod_u64(k, a.z[j] % n, n), a.inv_n, a.shift[j]));
+        c.v[k] = abs_integrand(a, x);
+    }
+}
+
+__global__ void __launch_bounds__(256) cdf_scatter_kernel(CdfArgs c) {
+    const unsigned long long n = c.pa.n, stride = (unsigned long long)gridDim.x * blockDim.x;
+    const int j = blockIdx.y;
+    const unsigned long long z = c.pa.z[j] % n, r0 = c.r0[j];
+    double* vs = c.vs + (size_t)j * n;
+    for (unsigned long long k = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += stride) {
+        const unsigned long long r = mulmod_u64(k, z, n);
+        vs[r >= r0 ? r - r0 : r + (n - r0)] = c.v[k];
+    }
+}
+
+constexpr int kCdfScanThreads = 1024;
+__global__ void __launch_bounds__(kCdfScanThreads) cdf_scan_kernel(CdfArgs c) {
+    __shared__ double part[kCdfScanThreads];
+    const int j = blockIdx.x, tid = threadIdx.x;
+    const unsigned long long n = c.pa.n;
+    const long long K = c.K;
+    const int step = c.step;
+    double* ox = c.out_x + (size_t)j * K;
+    double* oc = c.out_cdf + (size_t)j * K;
+    if (*c.status != 0) {
+        for (long long t = tid; t < K; t += kCdfScanThreads) { ox[t] = nan(""); oc[t] = nan(""); }
+        return;
+    }
+    const double* vs = c.vs + (size_t)j * n;
+    // thread `tid` owns the kept points t in [t0, t1): a contiguous chunk, the same split for every dimension
+    const long long per = (K + kCdfScanThreads - 1) / kCdfScanThreads;
+    const long long t0 = min(K, (long long)tid * per), t1 = min(K, t0 + per);
+    double local = 0.0;
+    for (long long t = t0; t < t1; ++t) {
+        double b = 0.0;
+        for (int i = 0; i < step; ++i) b += vs[(size_t)t * step + i];
+        local += b;
+    }
+    // samples beyond the last kept point (fewer than step of them) belong to the total only: the last thread adds them
+    double tail = 0.0;
+    if (tid == kCdfScanThreads - 1)
+        for (unsigned long long i = (unsigned long long)K * step; i < n; ++i) tail += vs[i];
+    part[tid] = local;
+    __syncthreads();
+    // inclusive block scan (Hillis-Steele, fixed shape)
+    for (int off = 1; off < kCdfScanThreads; off <<= 1) {
+        const double add = tid >= off ? part[tid - off] : 0.0;
+        __syncthreads();
+        part[tid] += add;
+        __syncthreads();
+    }
+    __shared__ double total;
+    if (tid == kCdfScanThreads - 1) total = part[tid] + tail;
+    __syncthreads();
+    double run = part[tid] - local;                           // exclusive prefix of this thread's chunk
+    const unsigned long long r0 = c.r0[j];
+    const double delta = c.pa.shift[j];
+    for (long long t = t0; t < t1; ++t) {
+        double b = 0.0;
+        for (int i = 0; i < step; ++i) b += vs[(size_t)t * step + i];
+        run += b;
+        const unsigned long long rank = (unsigned long long)t * step + (step - 1);
+        const unsigned long long r = rank < n - r0 ? r0 + rank : rank - (n - r0);
+        ox[t] = wrap_u(coord_t((double)r, c.pa.inv_n, delta));
+        oc[t] = __ddiv_rn(run, total);
+    }
+}
+
 int plan_project(const qmc_problem* p, int bins, ProjArgs* a) {
     if (!p) return QMC_ERR_NULL;
     if (p->family < 0 || p->family > QMC_FAMILY_SECTOR_COMPLEX) return QMC_ERR_FAMILY;
@@ -289,5 +404,69 @@ extern "C" int qmc_lattice_project(const qmc_problem* p, int bins, double* out_h
         e = cudaGetLastError();
     }
     if (e != cudaSuccess) return report_cuda_error(e, "qmc_lattice_project");
+    return QMC_OK;
+}
+
+
+// ---- sort-based CDF sampling (S10b) -----------------------------------------------------------------
+namespace {
+size_t cdf_layout(const qmc_problem* p, long long K, size_t* off_vs, size_t* off_r0, size_t* off_status) {
+    size_t o = 0;
+    o = ((size_t)p->n * 8 + 255) / 256 * 256;                // v
+    *off_vs = o; o += ((size_t)p->dim * p->n * 8 + 255) / 256 * 256;
+    *off_r0 = o; o += 256;
+    *off_status = o; o += 256;
+    (void)K;
+    return o;
+}
+}  // namespace
+
+extern "C" long long qmc_cdf_sample_count(uint64_t n, int fitstepsize) {
+    if (fitstepsize < 1 || (uint64_t)fitstepsize > n) return 0;
+    return (long long)(n / (uint64_t)fitstepsize);
+}
+
+extern "C" size_t qmc_cdf_workspace_bytes(const qmc_problem* p, int fitstepsize) {
+    qmc::ProjArgs a;
+    if (qmc::plan_project(p, 2, &a) != QMC_OK || qmc_cdf_sample_count(p->n, fitstepsize) == 0) return 0;
+    size_t o1, o2, o3;
+    return cdf_layout(p, 0, &o1, &o2, &o3);
+}
+
+extern "C" int qmc_lattice_cdf_samples(const qmc_problem* p, int fitstepsize, double* out_x, double* out_cdf, void* workspace,
+                                       size_t workspace_bytes, void* cuda_stream) {
+    qmc::ProjArgs a;
+    const int st = qmc::plan_project(p, 2, &a);
+    if (st != QMC_OK) return st;
+    const long long K = qmc_cdf_sample_count(p->n, fitstepsize);
+    if (K < 1) return QMC_ERR_N;
+    if (!out_x || !out_cdf) return QMC_ERR_NULL;
+    size_t off_vs, off_r0, off_status;
+    const size_t need = cdf_layout(p, K, &off_vs, &off_r0, &off_status);
+    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || workspace_bytes < need) return QMC_ERR_WORKSPACE;
+    char* ws = static_cast<char*>(workspace);
+    qmc::CdfArgs c;
+    c.pa = a; c.step = fitstepsize; c.K = K;
+    c.v = reinterpret_cast<double*>(ws);
+    c.vs = reinterpret_cast<double*>(ws + off_vs);
+    c.r0 = reinterpret_cast<unsigned long long*>(ws + off_r0);
+    c.status = reinterpret_cast<int*>(ws + off_status);
+    c.out_x = out_x; c.out_cdf = out_cdf;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    cudaError_t e = cudaMemsetAsync(c.status, 0, sizeof(int), stream);
+    const int blocks = (int)std::min<unsigned long long>((p->n + 255) / 256, 148ull * 8);
+    if (e == cudaSuccess) {
+        qmc::cdf_eval_kernel<<<blocks, 256, (size_t)a.n_params * 8, stream>>>(c);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) {
+        qmc::cdf_scatter_kernel<<<dim3(blocks, p->dim), 256, 0, stream>>>(c);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) {
+        qmc::cdf_scan_kernel<<<p->dim, qmc::kCdfScanThreads, 0, stream>>>(c);
+        e = cudaGetLastError();
+    }
+    if (e != cudaSuccess) return qmc::report_cuda_error(e, "qmc_lattice_cdf_samples");
     return QMC_OK;
 }

@@ -70,7 +70,7 @@ def test_validate_problem_host_accepts_all_configs():
     (lambda p: p.update(transform=207), -7),                 # Sidi weight outside 1..6
     (lambda p: p.update(transform=1000 + 16 * 0 + 3), -7),   # asymmetric Korobov weights outside 1..6
     (lambda p: p.update(transform=1000 + 16 * 3 + 7), -7),
-    (lambda p: p.update(family=8), -8),
+    (lambda p: p.update(family=9), -8),
     (lambda p: p.update(family=7), -9),                      # a valid family now, but the block has the wrong length
     (lambda p: p.update(params=p["params"][:-1]), -9),
     (lambda p: p.update(fit_coeffs=synth.cubic_fit_coeffs(4, a4=-0.2, a5=0.3)), -10),

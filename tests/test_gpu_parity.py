@@ -774,3 +774,51 @@ def test_complex_sector_projection_and_adaptive():
         ref = synth.problem(8, q["params"], res["n"], lz[i], q["shifts"][:res["m"]], K + 3)
         sm_or, mean_or, err_or = oracle.integrate(ref)
         assert np.all(np.abs(res["integral"] - mean_or) <= 1e-13 * np.hypot(*mean_or))
+
+
+# ------------------------------------------------------------------------------------------------
+# S10b: the paper's sort-based CDF sampling without a sort (reading C-8b)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("fam,d,n,step", [(0, 16, 65537, 10), (1, 8, 65537, 10), (2, 12, 16381, 7), (3, 6, 16381, 10), (8, 6, 8191, 10),
+                                          (4, 5, 8191, 3), (5, 8, 8191, 1), (1, 2, 127, 5), (7, 5, 1021, 1021), (0, 32, 4099, 10),
+                                          (1, 3, 1048573, 10)])
+def test_cdf_samples_match_the_oracle_sort(fam, d, n, step):
+    """kept coordinates bit-exact (the lattice's cyclic residue order IS the sorted order), CDF values at 1e-12, twice the same bits"""
+    p = make(fam, d, n, 2, NONE, 9700 + fam + d)
+    x_or, c_or = oracle.cdf_samples(p, step)
+    batch = binding.DeviceBatch([p])
+    x, c = batch.cdf_samples(0, step)
+    x, c = x.cpu().numpy(), c.cpu().numpy()
+    assert x.shape == x_or.shape == (d, n // step)
+    assert x.tobytes() == x_or.tobytes()
+    assert np.all(np.abs(c - c_or) <= 1e-12 * c_or)
+    x2, c2 = batch.cdf_samples(0, step)
+    assert c2.cpu().numpy().tobytes() == c.tobytes()
+
+
+def test_cdf_samples_shift_edge_cases():
+    """shift 0 (nothing wraps), a shift just below 1 (almost everything wraps) and the paper's n = 55 lattice of Fig. 1"""
+    for n, z, sh in [(55, [1, 34], [0.0, 0.999999]), (1021, [1, 374], [1e-300, 0.5]), (8191, [1, 2731], [0.25, 1.0 - 2.0 ** -53])]:
+        p = synth.problem(1, np.array([2.0, 3.0, 0.3, 0.6]), n, z, np.array([sh, sh]), NONE)
+        x_or, c_or = oracle.cdf_samples(p, 5)
+        x, c = binding.DeviceBatch([p]).cdf_samples(0, 5)
+        assert x.cpu().numpy().tobytes() == x_or.tobytes()
+        assert np.all(np.abs(c.cpu().numpy() - c_or) <= 1e-12 * c_or)
+
+
+def test_fit_from_cdf_samples():
+    """cubic fit from the sampled pairs against the oracle's (same closed form on the same pairs), and the projection -> fit ->
+    integration chain with the sort-based samples: the error estimate of a boundary-peaked integrand drops"""
+    p = make(1, 4, 65537, 8, K + 3, 9750)
+    proj = dict(p, transform=NONE)
+    x, c = binding.DeviceBatch([proj]).cdf_samples(0, 10)
+    x, c = x.cpu().numpy(), c.cpu().numpy()
+    fit = binding.qmc_fit_from_cdf(x, c)
+    fit_or = oracle.fit_cubic_cdf(x, c)
+    assert np.allclose(fit, fit_or, rtol=0, atol=1e-10)
+    full = binding.qmc_fit_from_cdf(x, c, with_poles=True)
+    assert binding.qmc_validate_problem_host(dict(p, fit_coeffs=full)) == 0
+    _, _, err0 = run_gpu([p])
+    _, _, err1 = run_gpu([dict(p, fit_coeffs=full)])
+    assert err1[0, 0] < err0[0, 0]
+    check_against_oracle([dict(p, fit_coeffs=full, name="cdf-fit")])
