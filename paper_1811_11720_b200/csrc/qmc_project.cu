@@ -7,11 +7,12 @@
 // transform None, weight 1, first shift only, all n lattice points.
 //
 // Determinism: a tile is a fixed range of lattice indices; inside a tile every warp owns a private
-// shared-memory histogram and adds its points in a fixed order (index step by step; within a step
-// the lanes that hit the same bin are summed in lane order by the lowest lane, found with
-// __match_any_sync -- no floating-point atomics anywhere).  Warp histograms are merged in warp
-// order, tile histograms in tile order (compensated) by project_merge_kernel.  The result does not
-// depend on the grid size, the SM count or the scheduling order.
+// shared-memory histogram.  Per step the 32 lanes evaluate their points and stage (x, |f|) in shared
+// memory; then lane L adds the 32 staged points, in lane order, to the histogram row of dimension L:
+// rows are private to a lane, so there is no conflict to resolve and no floating-point atomic (round 1
+// resolved same-bin lanes with __match_any_sync and a vote loop per dimension: 10 times slower).  Warp
+// histograms are merged in warp order, tile histograms in tile order (compensated) by
+// project_merge_kernel.  The result does not depend on the grid size, the SM count or the scheduling order.
 #include <algorithm>
 #include <cmath>
 #include <cstring>
@@ -22,8 +23,7 @@
 namespace qmc {
 namespace {
 
-constexpr int kProjTilesTarget = 148;       // one tile per SM of a B200: fixed, so the tiling is a function of n only (592 tiles spent
-                                            // more time zeroing, merging and writing 32 KB histograms than evaluating: 0.52 -> 0.xx ms on configs[4]'s fit lattice)
+constexpr int kProjTilesTarget = 148;       // one tile per SM of a B200: fixed, so the tiling is a function of n only
 constexpr int kProjSmemBudget = 200 * 1024; // bytes of warp-private histograms per CTA
 
 struct ProjArgs {
@@ -155,6 +155,7 @@ __global__ void __launch_bounds__(kThreads) project_kernel(ProjArgs a) {   // a:
         return;
     }
     double* mine = hist + warp * hsize;
+    double* stage = sp + ((a.n_params + 1) & ~1) + (size_t)warp * 32 * (QMC_MAX_DIM + 1);   // [point of the warp][x_0 .. x_(dim-1), |f|]
 
     const unsigned long long n = a.n;
     const unsigned long long tile_len = (unsigned long long)a.steps * kThreads;
@@ -168,31 +169,35 @@ __global__ void __launch_bounds__(kThreads) project_kernel(ProjArgs a) {   // a:
         step[j] = (RT)mulmod_u64((unsigned long long)kThreads % n, z, n);
     }
     unsigned long long k = k0 + tid;
+    const int row = QMC_MAX_DIM + 1;
     for (int i = 0; i < a.steps; ++i, k += kThreads) {
+        // every lane evaluates its point and stages (x, |f|); a dead lane (beyond the lattice) stages |f| = -1
         const bool live = k < kend;
-        double v = 0.0;
+        double v = -1.0;
         if (live) {
             for (int j = 0; j < a.dim; ++j) x[j] = wrap_u(coord_t(Res<WIDE>::to_double(r[j]), a.inv_n, a.shift[j]));
             v = abs_integrand(a, x);
+            for (int j = j0; j < j1; ++j) stage[lane * row + j] = x[j];
         }
-        for (int j = j0; j < j1; ++j) {
-            int b = -1 - lane;                                        // dead lanes: unique keys, never added
-            if (live) {
-                b = (int)floor((double)a.bins * x[j]);
-                if (b >= a.bins) b = a.bins - 1;
+        stage[lane * row + QMC_MAX_DIM] = v;
+        __syncwarp();
+        // lane L < (j1 - j0) owns dimension j0 + L of the warp's private histogram and adds the 32 points in lane order: no two
+        // lanes touch the same row, so there is nothing to resolve and the order of the additions is fixed
+        const int j = j0 + lane;
+        if (j < j1) {
+            double* hrow = mine + (size_t)lane * a.bins;
+            const double fb = (double)a.bins;
+#pragma unroll 4
+            for (int p = 0; p < 32; ++p) {
+                const double pv = stage[p * row + QMC_MAX_DIM];
+                if (pv >= 0.0) {
+                    int b = (int)floor(fb * stage[p * row + j]);
+                    if (b >= a.bins) b = a.bins - 1;
+                    hrow[b] += pv;
+                }
             }
-            unsigned peers = __match_any_sync(0xffffffffu, b);
-            const bool leader = (__ffs(peers) - 1) == lane;
-            double sum = v;
-            unsigned rem = peers & (peers - 1);                       // peers above the leader, lane order
-            while (__any_sync(0xffffffffu, leader && rem != 0u)) {
-                const int src = (leader && rem) ? (__ffs(rem) - 1) : lane;
-                const double pv = __shfl_sync(0xffffffffu, v, src);
-                if (leader && rem) { sum += pv; rem &= rem - 1; }
-            }
-            if (live && leader) mine[(j - j0) * a.bins + b] += sum;    // bins of one step are distinct per leader
-            __syncwarp();
         }
+        __syncwarp();
         for (int j = 0; j < a.dim; ++j) r[j] = add_mod<RT>(r[j], step[j], (RT)n);
     }
     __syncthreads();
@@ -360,7 +365,7 @@ int plan_project(const qmc_problem* p, int bins, ProjArgs* a) {
     if (steps > 0x7fffffffull) return QMC_ERR_N;
     a->steps = (int)steps;
     a->tiles = (int)((p->n + steps * kThreads - 1) / (steps * kThreads));
-    a->dchunk = std::max(1, std::min(p->dim, (kProjSmemBudget - p->n_params * 8) / (kWarps * bins * 8)));
+    a->dchunk = std::max(1, std::min(std::min(p->dim, 32), (kProjSmemBudget - p->n_params * 8 - kWarps * 32 * (QMC_MAX_DIM + 1) * 8) / (kWarps * bins * 8)));   // <= 32: one lane per dimension of the chunk
     a->nchunks = (p->dim + a->dchunk - 1) / a->dchunk;
     return QMC_OK;
 }
@@ -387,7 +392,7 @@ extern "C" int qmc_lattice_project(const qmc_problem* p, int bins, double* out_h
     a.tile_hist = static_cast<double*>(workspace);
     a.out_hist = out_hist;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
-    const size_t smem = (size_t)kWarps * a.dchunk * bins * 8 + (size_t)a.n_params * 8;
+    const size_t smem = (size_t)kWarps * a.dchunk * bins * 8 + (size_t)((a.n_params + 1) & ~1) * 8 + (size_t)kWarps * 32 * (QMC_MAX_DIM + 1) * 8;   // histograms, parameter block, staging
     const bool wide = p->n >= (1ull << 31);
     cudaError_t e;
     if (wide) {
