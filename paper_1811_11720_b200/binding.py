@@ -174,6 +174,32 @@ def qmc_lattice_integrate_batch_host(problems):
     return out, means, errs
 
 
+class HostBatch:
+    """Problems marshalled once for repeated synchronous HOST-pointer calls (qmc_lattice_integrate_batch_host): the numpy
+    arrays stay where they are, `integrate()` is the C call and nothing else."""
+
+    def __init__(self, problems):
+        self.problems = problems
+        self.count = len(problems)
+        self.arr = (qmc_problem * self.count)()
+        self._keep = []
+        for i, p in enumerate(problems):
+            params, shifts, fit = _f64(p["params"]), _f64(p["shifts"]), _f64(p.get("fit_coeffs"))
+            z = np.ascontiguousarray(p["z"], dtype=np.uint64)
+            self._keep += [params, shifts, fit, z]
+            self.arr[i] = qmc_problem(p["family"], p["dim"], p["m"], p["transform"], p["n"], params.ctypes.data, len(params),
+                                      z.ctypes.data, shifts.ctypes.data, None if fit is None else fit.ctypes.data)
+        self.max_m = max(p["m"] for p in problems)
+        self.means, self.errs = np.zeros((self.count, 2)), np.zeros((self.count, 2))
+        self.shift_means = np.zeros((self.count, 2 * self.max_m))
+        self._args = (self.count, self.arr, _d(self.means), _d(self.errs), _d(self.shift_means))
+        self._fn = lib().qmc_lattice_integrate_batch_host
+
+    def integrate(self):
+        _check(self._fn(*self._args), "qmc_lattice_integrate_batch_host")
+        return self.means, self.errs
+
+
 def qmc_sector_compile(params, dim):
     """The interpreter program of a sector parameter block, compiled on the device -> (steps uint8[], slots (n, 2), c0 (2,))."""
     params = _f64(params)

@@ -140,21 +140,44 @@ void fit_cubic_pairs(const std::vector<long double>& cs, const std::vector<long 
 
 }  // namespace
 
+// ---- variance-reduction fit from histograms (reading C-8): the CDF at the inner bin edges gives the pairs (c_b, e_b = b / bins)
+namespace {
+bool histogram_pairs(const double* h, int bins, std::vector<long double>* c, std::vector<long double>* e) {
+    long double total = 0.0L;
+    for (int b = 0; b < bins; ++b) {
+        if (!std::isfinite(h[b]) || h[b] < 0.0) return false;
+        total += h[b];
+    }
+    if (!(total > 0.0L)) return false;
+    c->clear(); e->clear();
+    long double run = 0.0L;
+    for (int b = 1; b < bins; ++b) { run += h[b - 1]; c->push_back(run / total); e->push_back((long double)b / (long double)bins); }
+    return true;
+}
+}  // namespace
+
+extern "C" int qmc_fit_cubic(const double* hist, int dim, int bins, double* fit_coeffs) {
+    if (!hist || !fit_coeffs) return QMC_ERR_NULL;
+    if (dim < 1 || dim > QMC_MAX_DIM) return QMC_ERR_DIM;
+    if (bins < 2 || bins > 1024) return QMC_ERR_N;
+    std::vector<long double> c, e;
+    for (int j = 0; j < dim; ++j) {
+        double* o = fit_coeffs + 6 * j;
+        if (histogram_pairs(hist + (size_t)j * bins, bins, &c, &e)) fit_cubic_pairs(c, e, o);
+        else { o[0] = 1.001; o[1] = -0.001; o[2] = 0.0; o[3] = 0.0; o[4] = 1.0; o[5] = 0.0; }   // identity map (bounds of P:L231 for the unused poles)
+    }
+    return QMC_OK;
+}
+
 extern "C" int qmc_fit_polysingular(const double* hist, int dim, int bins, double* fit_coeffs) {
     if (!hist || !fit_coeffs) return QMC_ERR_NULL;
     if (dim < 1 || dim > QMC_MAX_DIM) return QMC_ERR_DIM;
     if (bins < 8 || bins > 1024) return QMC_ERR_N;
     const int st = qmc_fit_cubic(hist, dim, bins, fit_coeffs);   // starting point and fall-back (identity if that fails too)
     if (st != QMC_OK) return st;
+    std::vector<long double> c, e;                                 // CDF values at the bin edges: p(c_b) = e_b (Eq. 18-20)
     for (int j = 0; j < dim; ++j) {
-        const double* h = hist + (size_t)j * bins;
-        long double total = 0.0L;
-        bool ok = true;
-        for (int b = 0; b < bins; ++b) { ok = ok && std::isfinite(h[b]) && h[b] >= 0.0; total += h[b]; }
-        if (!ok || !(total > 0.0L)) continue;
-        std::vector<long double> c, e;                             // CDF values at the bin edges: p(c_b) = e_b (Eq. 18-20)
-        long double run = 0.0L;
-        for (int b = 1; b < bins; ++b) { run += h[b - 1]; c.push_back(run / total); e.push_back((long double)b / bins); }
+        if (!histogram_pairs(hist + (size_t)j * bins, bins, &c, &e)) continue;
         fit_full_pairs(c, e, fit_coeffs + 6 * j);
     }
     return QMC_OK;

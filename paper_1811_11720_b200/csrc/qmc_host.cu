@@ -107,10 +107,12 @@ bool decode_transform(int transform, int* kind, int* r, int* gen = nullptr) {
     return ok;
 }
 
+// C(a, b) for the small arguments of the transform tables (a <= 12): exact integer Pascal recurrence
 double binom(int a, int b) {
-    double v = 1.0;
-    for (int i = 1; i <= b; ++i) v = v * (double)(a - b + i) / (double)i;
-    return v;
+    unsigned long long row[16] = {1};
+    for (int n = 1; n <= a; ++n)
+        for (int k = n; k >= 1; --k) row[k] += row[k - 1];
+    return (b < 0 || b > a) ? 0.0 : (double)row[b];
 }
 
 // struct-level validation (no dereference of the data pointers)
@@ -376,12 +378,15 @@ int arena_reserve(size_t pinned_bytes, size_t device_bytes) {
 
 int run_batch(int count, const qmc_problem* problems, double* out_means, double* out_errs, double* out_shift_means,
               void* workspace, size_t workspace_bytes, cudaStream_t st, const qmc_plan_options& opt = kDefaultOptions,
-              char* pinned_blob = nullptr) {
+              char* pinned_blob = nullptr, Plan* prebuilt = nullptr) {
     g_ts.last_launches = 0;
     if (!out_means || !out_errs) return QMC_ERR_NULL;
-    Plan plan;
-    const int pst = make_plan(count, problems, true, &plan, opt);
-    if (pst != QMC_OK) return pst;
+    Plan local_plan;
+    Plan& plan = prebuilt ? *prebuilt : local_plan;          // the HOST-pointer entry plans once and patches the data pointers
+    if (!prebuilt) {
+        const int pst = make_plan(count, problems, true, &local_plan, opt);
+        if (pst != QMC_OK) return pst;
+    }
     if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || workspace_bytes < plan.total) return QMC_ERR_WORKSPACE;
     const int sms = sm_count();
     if (sms <= 0) return cuda_fail(cudaErrorNoDevice, "no CUDA device");
@@ -657,8 +662,6 @@ int qmc_lattice_integrate_batch_host(int count, const qmc_problem* problems, dou
     }
     const size_t out_doubles = (size_t)count * (4 + 2 * (size_t)max_m);     // means (2), errs (2), shift means (2 max_m) per problem
     const size_t out_bytes = align_up(out_doubles * 8, 256);
-    // device problem structs first (pointers into the arena's device block), then the plan
-    std::vector<qmc_problem> dp(problems, problems + count);
     Plan plan;
     const int pst = make_plan(count, problems, true, &plan);
     if (pst != QMC_OK) return pst;
@@ -680,17 +683,18 @@ int qmc_lattice_integrate_batch_host(int count, const qmc_problem* problems, dou
             off += align_up(bytes, 256);
             return dev;
         };
-        dp[i].params = reinterpret_cast<const double*>(put(p.params, (size_t)p.n_params * 8));
-        dp[i].z = reinterpret_cast<const uint64_t*>(put(p.z, (size_t)p.dim * 8));
-        dp[i].shifts = reinterpret_cast<const double*>(put(p.shifts, (size_t)p.m * p.dim * 8));
-        dp[i].fit_coeffs = p.fit_coeffs ? reinterpret_cast<const double*>(put(p.fit_coeffs, (size_t)p.dim * 6 * 8)) : nullptr;
+        DevProblem& d = plan.dev[i];                         // planned from the HOST structs: redirect the data pointers to the device copies
+        d.params = reinterpret_cast<const double*>(put(p.params, (size_t)p.n_params * 8));
+        d.z = reinterpret_cast<const unsigned long long*>(put(p.z, (size_t)p.dim * 8));
+        d.shifts = reinterpret_cast<const double*>(put(p.shifts, (size_t)p.m * p.dim * 8));
+        d.fit = p.fit_coeffs ? reinterpret_cast<const double*>(put(p.fit_coeffs, (size_t)p.dim * 6 * 8)) : nullptr;
     }
     cudaStream_t st = 0;
     double* d_means = d_out;
     double* d_errs = d_out + (size_t)count * 2;
     double* d_sm = d_out + (size_t)count * 4;
     QMC_CUDA(cudaMemcpyAsync(d_in, h_in, in_bytes, cudaMemcpyHostToDevice, st));
-    const int status = run_batch(count, dp.data(), d_means, d_errs, d_sm, d_ws, plan.total, st, kDefaultOptions, h_blob);
+    const int status = run_batch(count, problems, d_means, d_errs, d_sm, d_ws, plan.total, st, kDefaultOptions, h_blob, &plan);
     if (status != QMC_OK) { cudaStreamSynchronize(st); return status; }
     QMC_CUDA(cudaMemcpyAsync(h_out, d_out, out_doubles * 8, cudaMemcpyDeviceToHost, st));
     QMC_CUDA(cudaStreamSynchronize(st));
@@ -857,40 +861,4 @@ int qmc_fp64_peak_probe(int iters, double* out_rate, double* out_ms, void* cuda_
 
 }  // extern "C"
 
-// ---- variance-reduction fit: host-side closed-form least squares (reading C-8) ----------
-extern "C" int qmc_fit_cubic(const double* hist, int dim, int bins, double* fit_coeffs) {
-    if (!hist || !fit_coeffs) return QMC_ERR_NULL;
-    if (dim < 1 || dim > QMC_MAX_DIM) return QMC_ERR_DIM;
-    if (bins < 2 || bins > 1024) return QMC_ERR_N;
-    for (int j = 0; j < dim; ++j) {
-        const double* h = hist + (size_t)j * bins;
-        long double total = 0.0L;
-        bool ok = true;
-        for (int b = 0; b < bins; ++b) { ok = ok && std::isfinite(h[b]) && h[b] >= 0.0; total += h[b]; }
-        double a4 = 1.0, a5 = 0.0;                              // identity map unless a safe fit exists
-        if (ok && total > 0.0L) {
-            // p(c) = c^3 + a4 (c - c^3) + a5 (c^2 - c^3) must reproduce the bin edges e_b at the CDF values c_b
-            long double s11 = 0, s12 = 0, s22 = 0, t1 = 0, t2 = 0, run = 0;
-            for (int b = 1; b < bins; ++b) {
-                run += h[b - 1];
-                const long double c = run / total, e = (long double)b / (long double)bins;
-                const long double c3 = c * c * c, g1 = c - c3, g2 = c * c - c3, rhs = e - c3;
-                s11 += g1 * g1; s12 += g1 * g2; s22 += g2 * g2; t1 += g1 * rhs; t2 += g2 * rhs;
-            }
-            const long double det = s11 * s22 - s12 * s12;
-            if (fabsl(det) > 1e-300L) {
-                const double c4 = (double)((t1 * s22 - t2 * s12) / det), c5 = (double)((s11 * t2 - s12 * t1) / det);
-                const double c6 = 1.0 - c4 - c5;
-                double mn = std::fmin(c4, c4 + 2.0 * c5 + 3.0 * c6);     // p' at the end points
-                if (c6 != 0.0) {
-                    const double yv = -c5 / (3.0 * c6);                   // interior extremum of p'
-                    if (yv > 0.0 && yv < 1.0) mn = std::fmin(mn, c4 + yv * (2.0 * c5 + 3.0 * c6 * yv));
-                }
-                if (mn > 0.05) { a4 = c4; a5 = c5; }
-            }
-        }
-        double* o = fit_coeffs + 6 * j;
-        o[0] = 1.001; o[1] = -0.001; o[2] = 0.0; o[3] = 0.0; o[4] = a4; o[5] = a5;   // bounds of P:L231 for the unused poles
-    }
-    return QMC_OK;
-}
+// (the host-side fits are in qmc_fit.cu)

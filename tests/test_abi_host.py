@@ -243,3 +243,64 @@ def test_fit_polysingular_recovers_a_map_with_poles():
     flat = binding.qmc_fit_polysingular(np.ones((2, 64)))
     np.testing.assert_allclose(flat[:, 4:], [[1.0, 0.0]] * 2, atol=1e-12)
     assert np.all(flat[:, 2:4] == 0.0)
+
+
+def test_fit_from_cdf_pairs_on_the_host():
+    """qmc_fit_from_cdf (host code): the cubic from sampled pairs equals the oracle's on the same pairs and recovers an exact
+    cubic; with_poles recovers a map with a pole term; argument errors"""
+    a4, a5 = 0.55, 0.35
+    c = np.linspace(0.0005, 0.9995, 2000)
+    x = c * (a4 + c * (a5 + c * (1 - a4 - a5)))
+    got = binding.qmc_fit_from_cdf(np.stack([x, x]), np.stack([c, c]))
+    ref = oracle.fit_cubic_cdf(np.stack([x, x]), np.stack([c, c]))
+    np.testing.assert_allclose(got, ref, rtol=0, atol=1e-10)
+    assert abs(got[0, 4] - a4) < 1e-10 and abs(got[0, 5] - a5) < 1e-10
+    a = np.array([1.05, -0.2, 0.3, 0.0, 0.4, 0.2])                     # Eq. 19 with one pole term
+    a6 = 1 - a[2] - a[3] - a[4] - a[5]
+    xp = a[2] * c * (a[0] - 1) / (a[0] - c) + c * (a[4] + c * (a[5] + c * a6))
+    full = binding.qmc_fit_from_cdf(xp[None, :], c[None, :], with_poles=True)
+    model = full[0, 2] * c * (full[0, 0] - 1) / (full[0, 0] - c) + full[0, 3] * c * (full[0, 1] - 1) / (full[0, 1] - c) + \
+        c * (full[0, 4] + c * (full[0, 5] + c * (1 - full[0, 2:].sum())))
+    assert np.max(np.abs(model - xp)) < 1e-6 and full[0, 2] > 0.05
+    L = binding.lib()
+    out = np.zeros(6)
+    assert L.qmc_fit_from_cdf(None, None, 1, 100, 0, binding._d(out)) == -1
+    assert L.qmc_fit_from_cdf(binding._d(x), binding._d(c), 1, 4, 0, binding._d(out)) == -3
+    assert L.qmc_cdf_sample_count(1048573, 10) == 104857 and L.qmc_cdf_sample_count(100, 0) == 0 and L.qmc_cdf_sample_count(100, 101) == 0
+
+
+def test_host_pointer_batch_rejects_before_touching_the_device(L):
+    """qmc_lattice_integrate_batch_host validates every problem (values included) before it stages or launches anything"""
+    p = _cfg0()
+    def call(probs):
+        arr = (binding.qmc_problem * len(probs))()
+        keep = []
+        for i, q in enumerate(probs):
+            prm, sh, z = np.ascontiguousarray(q["params"]), np.ascontiguousarray(q["shifts"]), np.ascontiguousarray(q["z"], dtype=np.uint64)
+            keep += [prm, sh, z]
+            arr[i] = binding.qmc_problem(q["family"], q["dim"], q["m"], q["transform"], q["n"], prm.ctypes.data, len(prm), z.ctypes.data,
+                                         sh.ctypes.data, None)
+        means, errs = np.zeros((len(probs), 2)), np.zeros((len(probs), 2))
+        return L.qmc_lattice_integrate_batch_host(len(probs), arr, binding._d(means), binding._d(errs), None)
+    bad_shift = dict(p, shifts=p["shifts"].copy())
+    bad_shift["shifts"][1, 0] = 1.0
+    assert call([p, bad_shift]) == -5
+    assert call([dict(p, z=np.array([2, 4, 6, 65537 - 1], dtype=np.uint64) * 0 + 65537)]) == -4
+    assert L.qmc_lattice_integrate_batch_host(0, None, None, None, None) == -3
+    assert L.qmc_lattice_integrate_batch_host(1, None, None, None, None) == -1
+
+
+def test_sector_family_limits_in_the_struct_checks(L):
+    """dim <= QMC_MAX_SECTOR_DIM for both sector families; the complex family has (2 + d) doubles per monomial"""
+    rng = synth.MT19937_64(3)
+    d = 6
+    prm = synth.sector_complex(rng, d)
+    sh = synth.draw_shifts(rng, 4, d)
+    ok = synth.problem(8, prm, 8191, synth.korobov_form_vector(8191, d, 2731), sh, K3)
+    assert binding.qmc_validate_problem_host(ok) == 0
+    assert binding.qmc_validate_problem_host(dict(ok, params=prm[:-1])) == -9
+    assert binding.qmc_validate_problem_host(dict(ok, family=3)) == -9                 # the real family reads (1 + d) per monomial
+    d17 = 17
+    big = synth.problem(3, np.concatenate([[1, 1, 1, 1], np.zeros(d17), [1.0], np.zeros(d17), [1.0], np.zeros(d17)]), 8191,
+                        synth.korobov_form_vector(8191, d17, 2731), synth.draw_shifts(rng, 2, d17), K3)
+    assert binding.qmc_validate_problem_host(big) == -2
