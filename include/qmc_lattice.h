@@ -297,6 +297,44 @@ int qmc_sector_compile(const double* params /*HOST*/, int n_params, int dim, uns
                        int steps_cap, int* out_n_steps /*HOST*/, double* out_slots /*HOST or NULL*/, int slots_cap,
                        int* out_n_slots /*HOST*/, double* out_c0 /*HOST [2]*/);
 
+/* ---- modules of specialised sector kernels ------------------------------------------------------------------------------
+ * The paper's integrands are compiled functions (every sector is C++ source compiled for the GPU before the
+ * integration starts).  A C ABI carries parameter blocks instead, which the default kernels interpret step by step; a MODULE
+ * gives the compiled route back: qmc_sector_module_create translates every QMC_FAMILY_SECTOR problem of a batch into
+ * straight-line sm_100a code -- the same operations in the same order as the interpreting kernel, so both return the same bits --
+ * inside copies of the fused kernel (up to `sectors_per_kernel` sectors per kernel, 0 = 32; at most 63 kernels per batch),
+ * assembled on the HOST with the CUDA toolkit's nvJitLink (opened at run time; QMC_ERR_CUDA with the assembler's text in
+ * qmc_last_cuda_error if that fails), kernels in parallel on the host's cores.  It needs no GPU.  Used of each problem:
+ * family, dim, n_params and params (HOST pointer; read during the call only); everything else is ignored, so one module
+ * serves any lattice, shift set and sample count of the same integrands.  Problems of other families, and sector blocks the
+ * validation rejects, simply stay on the default kernels.  The caller owns the module and destroys it (also unloads it from
+ * every device it ran on); a module may be used from several host threads and on several devices.
+ *
+ * qmc_lattice_integrate_batch_module is qmc_lattice_integrate_batch (same arguments, stream-ordered; the workspace size comes
+ * from qmc_sector_module_workspace_bytes: every kernel of the module has a tile queue of its own) with
+ * the module's kernels for the problems that have code there AND run the default tile loop (transform Korobov r = 3, no fit map,
+ * n < 2^31); the rest of the batch takes the default kernels in the same call.  `problems` must be the batch the module was
+ * built from, in its order (count / family / dim / n_params are checked: QMC_ERR_N / QMC_ERR_PARAMS; the VALUES of params
+ * are the caller's promise -- polynomials are read from the module, nu / a / b / log factors too).  The first launch on a
+ * device loads the images there (a synchronous driver call). */
+typedef struct qmc_sector_module qmc_sector_module;
+int qmc_sector_module_create(int count, const qmc_problem* problems /*HOST, HOST params*/, int sectors_per_kernel,
+                             qmc_sector_module** out /*HOST*/);
+void qmc_sector_module_destroy(qmc_sector_module* module);
+/* what was built: specialised problems, kernels, host milliseconds of the create call, bytes of device code, host threads used
+ * (any pointer may be NULL) */
+int qmc_sector_module_info(const qmc_sector_module* module, int* n_specialised, int* n_kernels, double* build_ms, size_t* image_bytes,
+                           int* host_threads);
+/* kernel `kernel`'s device image (an ELF for cuobjdump -sass) and the assembler's report (registers, spills); sizes through
+ * *image_bytes with image = NULL; QMC_ERR_WORKSPACE if image_cap is too small */
+int qmc_sector_module_image(const qmc_sector_module* module, int kernel, void* image /*HOST or NULL*/, size_t image_cap,
+                            size_t* image_bytes /*HOST or NULL*/, char* log /*HOST or NULL*/, size_t log_cap);
+size_t qmc_sector_module_workspace_bytes(const qmc_sector_module* module, int count, const qmc_problem* problems /*HOST*/);  /* 0 on invalid input */
+int qmc_lattice_integrate_batch_module(qmc_sector_module* module, int count, const qmc_problem* problems /*HOST*/,
+                                       double* out_means /*DEVICE*/, double* out_errs /*DEVICE*/,
+                                       double* out_shift_means /*DEVICE or NULL*/, void* workspace /*DEVICE*/,
+                                       size_t workspace_bytes, void* cuda_stream);
+
 int qmc_num_components(int family);          /* 1 or 2; <0 on unknown family */
 const char* qmc_status_string(int status);
 const char* qmc_last_cuda_error(void);       /* thread-local text of the last CUDA error ("" if none) */

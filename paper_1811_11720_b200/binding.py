@@ -22,7 +22,8 @@ EXPORTS = [
     "qmc_num_components", "qmc_status_string", "qmc_last_cuda_error", "qmc_integrate", "qmc_fit_polysingular",
     "qmc_lattice_integrate_batch_opts", "qmc_workspace_bytes_opts", "qmc_lattice_integrate_batch_host",
     "qmc_release_thread_resources", "qmc_sector_compile", "qmc_lattice_cdf_samples", "qmc_cdf_workspace_bytes",
-    "qmc_cdf_sample_count", "qmc_fit_from_cdf",
+    "qmc_cdf_sample_count", "qmc_fit_from_cdf", "qmc_sector_module_create", "qmc_sector_module_destroy", "qmc_sector_module_info",
+    "qmc_sector_module_image", "qmc_lattice_integrate_batch_module", "qmc_sector_module_workspace_bytes",
 ]
 
 QMC_OK = 0
@@ -80,6 +81,14 @@ def lib():
         L.qmc_lattice_integrate_batch_host.argtypes = [C.c_int, pp, dp, dp, dp]
         L.qmc_sector_compile.argtypes = [dp, C.c_int, C.c_int, C.POINTER(C.c_ubyte), C.c_int, C.POINTER(C.c_int), dp, C.c_int,
                                          C.POINTER(C.c_int), dp]
+        L.qmc_sector_module_create.argtypes = [C.c_int, pp, C.c_int, C.POINTER(vp)]
+        L.qmc_sector_module_destroy.argtypes = [vp]
+        L.qmc_sector_module_destroy.restype = None
+        L.qmc_sector_module_info.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int), dp, C.POINTER(C.c_size_t), C.POINTER(C.c_int)]
+        L.qmc_sector_module_image.argtypes = [vp, C.c_int, vp, C.c_size_t, C.POINTER(C.c_size_t), C.c_char_p, C.c_size_t]
+        L.qmc_sector_module_workspace_bytes.argtypes = [vp, C.c_int, pp]
+        L.qmc_sector_module_workspace_bytes.restype = C.c_size_t
+        L.qmc_lattice_integrate_batch_module.argtypes = [vp, C.c_int, pp, vp, vp, vp, vp, C.c_size_t, vp]
         L.qmc_validate_problem_host.argtypes = [pp]
         L.qmc_lattice_project.argtypes = [pp, C.c_int, vp, vp, C.c_size_t, vp]
         L.qmc_project_workspace_bytes.argtypes = [pp, C.c_int]
@@ -213,6 +222,51 @@ def qmc_sector_compile(params, dim):
     return steps, slots, c0
 
 
+class SectorModule:
+    """qmc_sector_module_create: the real sectors of `problems` as straight-line sm_100a code (built on the host, no GPU needed).
+    DeviceBatch(problems, module=...) runs them; `info` tells what was built."""
+
+    def __init__(self, problems, sectors_per_kernel=0):
+        count = len(problems)
+        arr = (qmc_problem * count)()
+        keep = []
+        for i, p in enumerate(problems):
+            params = _f64(p["params"])
+            keep.append(params)
+            arr[i] = qmc_problem(p["family"], p["dim"], p.get("m", 0), p.get("transform", 0), p.get("n", 0), params.ctypes.data,
+                                 len(params), None, None, None)
+        self.count = count
+        self.handle = C.c_void_p()
+        _check(lib().qmc_sector_module_create(count, arr, int(sectors_per_kernel), C.byref(self.handle)), "qmc_sector_module_create")
+
+    @property
+    def info(self):
+        ns, nk, ms, nb, th = C.c_int(), C.c_int(), C.c_double(), C.c_size_t(), C.c_int()
+        _check(lib().qmc_sector_module_info(self.handle, C.byref(ns), C.byref(nk), C.byref(ms), C.byref(nb), C.byref(th)),
+               "qmc_sector_module_info")
+        return {"specialised": ns.value, "kernels": nk.value, "build_ms": ms.value, "image_bytes": nb.value, "host_threads": th.value}
+
+    def image(self, kernel=0):
+        """(device image bytes, assembler report) of one kernel"""
+        nb = C.c_size_t()
+        log = C.create_string_buffer(1 << 16)
+        _check(lib().qmc_sector_module_image(self.handle, int(kernel), None, 0, C.byref(nb), log, len(log)), "qmc_sector_module_image")
+        buf = C.create_string_buffer(nb.value)
+        _check(lib().qmc_sector_module_image(self.handle, int(kernel), buf, nb.value, None, None, 0), "qmc_sector_module_image")
+        return buf.raw, log.value.decode(errors="replace")
+
+    def close(self):
+        if self.handle:
+            lib().qmc_sector_module_destroy(self.handle)
+            self.handle = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
 def qmc_release_thread_resources():
     _check(lib().qmc_release_thread_resources(), "qmc_release_thread_resources")
 
@@ -275,8 +329,9 @@ class DeviceBatch:
     (count, 2*max_m).
     """
 
-    def __init__(self, problems, device="cuda:0", tiles_target=0, force_wide=False):
+    def __init__(self, problems, device="cuda:0", tiles_target=0, force_wide=False, module=None):
         import torch
+        self.module = module                               # a SectorModule built from the same problems, or None
         self.opts = qmc_plan_options(int(tiles_target), 1 if force_wide else 0)
         self.torch = torch
         self.device = torch.device(device)
@@ -297,6 +352,8 @@ class DeviceBatch:
         self.arr = arr
         self.max_m = max(p["m"] for p in problems)
         self.ws_bytes = int(lib().qmc_workspace_bytes_opts(self.count, arr, C.byref(self.opts)))
+        if module is not None:
+            self.ws_bytes = max(self.ws_bytes, int(lib().qmc_sector_module_workspace_bytes(module.handle, self.count, arr)))
         if self.ws_bytes == 0:
             st = lib().qmc_plan_info(self.count, arr, None, None, None)
             raise QmcError(st if st != 0 else -11, "qmc_workspace_bytes")
@@ -315,6 +372,11 @@ class DeviceBatch:
     def integrate(self, stream=None):
         """qmc_lattice_integrate_batch on `stream` (default: torch's current stream); returns launch count."""
         s = self.torch.cuda.current_stream(self.device).cuda_stream if stream is None else stream
+        if self.module is not None:
+            _check(lib().qmc_lattice_integrate_batch_module(self.module.handle, self.count, self.arr, self.means.data_ptr(),
+                                                            self.errs.data_ptr(), self.shift_means.data_ptr(), self.ws_ptr,
+                                                            self.ws_bytes, s), "qmc_lattice_integrate_batch_module")
+            return int(lib().qmc_last_launch_count())
         _check(lib().qmc_lattice_integrate_batch_opts(self.count, self.arr, self.means.data_ptr(), self.errs.data_ptr(),
                                                       self.shift_means.data_ptr(), self.ws_ptr, self.ws_bytes, s, C.byref(self.opts)),
                "qmc_lattice_integrate_batch")

@@ -154,6 +154,24 @@ template <> __device__ __forceinline__ void sector_interp<{dp}, {g}, {nt}>(const
 """
 
 
+def gen_site(dp, g):
+    """The place where a specialised kernel evaluates its sector (qmc_spec.cu splices straight-line PTX over the marker)."""
+    ops = ([f'"=d"(num[{q}])' for q in range(g)] + [f'"=d"(den[{q}])' for q in range(g)] + [f'"=d"(F[{q}])' for q in range(g)])
+    ins = ([f'"d"(x[{q}][{j}])' for q in range(g) for j in range(dp)] + [f'"d"(W[{q}])' for q in range(g)] + ['"r"(sel)', '"r"(park_addr)'])
+    n = len(ops) + len(ins)
+    text = "@@QMC_SITE " + " ".join(f"%{i}" for i in range(n)) + ";"
+    return f"""
+template <> __device__ __forceinline__ void sector_poly_site<{dp}, {g}>(const double (&x)[{g}][{dp}], const double (&W)[{g}], unsigned sel,
+                                                                     unsigned park_addr, double (&num)[{g}], double (&den)[{g}],
+                                                                     double (&F)[{g}]) {{
+    asm volatile("{text}"
+        : {", ".join(ops)}
+        : {", ".join(ins)}
+        : "memory");
+}}
+"""
+
+
 def main():
     here = os.path.dirname(os.path.abspath(__file__))
     out = ["// GENERATED by gen_sector_interp.py -- do not edit.  Threaded-code interpreter of the sector family",
@@ -174,6 +192,14 @@ def main():
         f.write("\n".join(out[:7] + [gen(*v) for v in real]))
     with open(os.path.join(here, "qmc_csector_interp.inc"), "w") as f:
         f.write("\n".join(out[:2] + out[7:] + [gen(*v) for v in cplx]))
+    site = ["// GENERATED by gen_sector_interp.py -- do not edit.  The marker a specialised sector kernel carries where the code of its",
+            "// sectors goes (qmc_spec_template.cu is compiled to PTX only; qmc_spec.cu replaces the marker line, whose operands are,",
+            "// in this order: num[G], den[G], F[G] (outputs), x[G][DP], W[G], the case selector, the thread's park address).",
+            "template <int DP, int G> __device__ __forceinline__ void sector_poly_site(const double (&x)[G][DP], const double (&W)[G], unsigned sel,",
+            "                                                                          unsigned park_addr, double (&num)[G], double (&den)[G],",
+            "                                                                          double (&F)[G]);"]
+    with open(os.path.join(here, "qmc_sector_site.inc"), "w") as f:
+        f.write("\n".join(site + [gen_site(dp, g) for dp, g, _, c in VARIANTS if not c]))
 
 
 if __name__ == "__main__":

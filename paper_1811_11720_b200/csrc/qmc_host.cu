@@ -11,6 +11,7 @@
 
 #include "qmc_fused.cuh"
 #include "qmc_kernels.h"
+#include "qmc_spec.h"
 
 namespace qmc {
 namespace {
@@ -140,10 +141,11 @@ int validate_struct(const qmc_problem& p, bool need_two_shifts) {
 
 // ---- launch plan: tiles, kernel variants, workspace layout (pure function of the problem structs) ----
 struct Variant {
-    int family, dp;                  // kernel family (kernel_family(public id)), dimension slots
+    int family, dp;                  // kernel family (kernel_family(public id), or kKernelFamilySpec), dimension slots
     bool wide;
     std::vector<int> plist;          // problem indices, queue order (most expensive tiles first)
     long long total_tiles = 0;
+    int spec_kernel = -1;            // kKernelFamilySpec: the module's kernel
 };
 
 struct Plan {
@@ -158,8 +160,15 @@ struct Plan {
 
 const qmc_plan_options kDefaultOptions = {0, 0};
 
-int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan* plan, const qmc_plan_options& opt = kDefaultOptions) {
+int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan* plan, const qmc_plan_options& opt = kDefaultOptions,
+              const qmc_sector_module* module = nullptr) {
     if (count < 1 || !problems) return count < 1 ? QMC_ERR_N : QMC_ERR_NULL;
+    if (module) {                                        // the batch the module was built from, in its order
+        if (spec_problem_count(module) != count) return QMC_ERR_N;
+        const SpecProblem* sp = spec_problems(module);
+        for (int i = 0; i < count; ++i)
+            if (sp[i].family != problems[i].family || sp[i].dim != problems[i].dim || sp[i].n_params != problems[i].n_params) return QMC_ERR_PARAMS;
+    }
     plan->dev.resize(count);
     long long means_off = 0;
     size_t prog_off = 0;
@@ -219,19 +228,27 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
         const DevProblem& d = plan->dev[i];
         const bool wide = variant_wide(d.family, d.dim, d.n, opt);
         const int dp = dim_slots(d.family, d.dim, wide);
+        // a specialised kernel holds the sector's code and serves the default tile loop only (Korobov-3, no fit map, narrow residues)
+        int kfam = kernel_family(d.family), spec_kernel = -1;
+        if (module && d.family == QMC_FAMILY_SECTOR && !wide && d.tr_kind == TR_KOR3 && !d.has_fit && spec_problems(module)[i].kernel >= 0) {
+            kfam = kKernelFamilySpec;
+            spec_kernel = spec_problems(module)[i].kernel;
+            plan->dev[i].spec_case = spec_problems(module)[i].kase;
+        }
         Variant* v = nullptr;
         for (auto& c : plan->variants)
-            if (c.family == kernel_family(d.family) && c.dp == dp && c.wide == wide) v = &c;
-        if (!v) { plan->variants.push_back(Variant{kernel_family(d.family), dp, wide, {}, 0}); v = &plan->variants.back(); }
+            if (c.family == kfam && c.dp == dp && c.wide == wide && c.spec_kernel == spec_kernel) v = &c;
+        if (!v) { plan->variants.push_back(Variant{kfam, dp, wide, {}, 0, spec_kernel}); v = &plan->variants.back(); }
         v->plist.push_back(i);
     }
     if (plan->variants.size() > 64) return QMC_ERR_WORKSPACE;
     // tiling (S9): per kernel variant aim at kWaves x (resident CTAs of a B200) tiles, shared among the variant's problems
     // in proportion to their cost; a tile is at least one index per thread and at most kMaxSteps (bounds the fp64 chains)
     for (auto& v : plan->variants) {
-        const bool sector_variant = v.family == QMC_FAMILY_SECTOR || v.family == kKernelFamilyCSector;
+        const bool sector_variant = v.family == QMC_FAMILY_SECTOR || v.family == kKernelFamilyCSector || v.family == kKernelFamilySpec;
         const int resident = kPlanSMs * (sector_variant ? min_blocks_sector(v.dp) : min_blocks_closed(v.dp, v.wide));
-        const int threads = v.family == QMC_FAMILY_SECTOR ? sector_threads(v.dp) : (v.family == kKernelFamilyCSector ? kCSectorThreads : kThreads);   // CTA size of the variant's kernel
+        const int threads = (v.family == QMC_FAMILY_SECTOR || v.family == kKernelFamilySpec) ? sector_threads(v.dp)
+                                                                                              : (v.family == kKernelFamilyCSector ? kCSectorThreads : kThreads);   // CTA size of the variant's kernel
         const int env = opt.tiles_target > 0 ? opt.tiles_target : 0;
         // one problem: equal tiles, 2 per resident CTA (the queue evens out SM speed differences over a long kernel) -- or
         // exactly 1 when the whole kernel is short (< kShortEvalsPerCta evaluations per CTA: per-tile overhead and the
@@ -279,7 +296,7 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
     plan->off_counters = o; o = align_up(o + 64 * sizeof(unsigned long long), 256);
     plan->off_probs = o; o = align_up(o + (size_t)count * sizeof(DevProblem), 256);
     plan->off_plist = o; o = align_up(o + (size_t)count * sizeof(int), 256);
-    plan->off_prefix = o; o = align_up(o + ((size_t)count + plan->variants.size()) * sizeof(long long), 256);
+    plan->off_prefix = o; o = align_up(o + ((size_t)count + 64) * sizeof(long long), 256);   // <= 64 variants: the size does not depend on the routing
     plan->off_aux = o; o = align_up(o + (size_t)count * sizeof(DevAux), 256);
     plan->off_prog = o; o = align_up(o + plan->prog_words * 8, 256);
     plan->off_means = o; o = align_up(o + plan->means_doubles * 8, 256);
@@ -378,13 +395,13 @@ int arena_reserve(size_t pinned_bytes, size_t device_bytes) {
 
 int run_batch(int count, const qmc_problem* problems, double* out_means, double* out_errs, double* out_shift_means,
               void* workspace, size_t workspace_bytes, cudaStream_t st, const qmc_plan_options& opt = kDefaultOptions,
-              char* pinned_blob = nullptr, Plan* prebuilt = nullptr) {
+              char* pinned_blob = nullptr, Plan* prebuilt = nullptr, qmc_sector_module* module = nullptr) {
     g_ts.last_launches = 0;
     if (!out_means || !out_errs) return QMC_ERR_NULL;
     Plan local_plan;
     Plan& plan = prebuilt ? *prebuilt : local_plan;          // the HOST-pointer entry plans once and patches the data pointers
     if (!prebuilt) {
-        const int pst = make_plan(count, problems, true, &local_plan, opt);
+        const int pst = make_plan(count, problems, true, &local_plan, opt, module);
         if (pst != QMC_OK) return pst;
     }
     if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) || workspace_bytes < plan.total) return QMC_ERR_WORKSPACE;
@@ -458,12 +475,19 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
     }
     for (size_t vi = 0; vi < plan.variants.size(); ++vi) {
         const Variant& v = plan.variants[vi];
-        const int occ = occupancy(v.family, v.dp, v.wide);
+        const int occ = v.family == kKernelFamilySpec ? spec_occupancy(module, v.spec_kernel) : occupancy(v.family, v.dp, v.wide);
+        if (occ <= 0 && v.family == kKernelFamilySpec) return QMC_ERR_CUDA;      // the loader left the text
         if (occ <= 0) return cuda_fail(cudaErrorInvalidDeviceFunction, "occupancy query (is the sm_100a image loadable on this device?)");
         const long long cap = (long long)sms * occ;
         const int grid = (int)std::min<long long>(cap, v.total_tiles);
         FusedLaunch a = base;
         a.vq = queues[vi];
+        if (v.family == kKernelFamilySpec) {
+            const int rc = spec_launch(module, v.spec_kernel, grid, st, a);
+            if (rc != QMC_OK) return rc;
+            ++g_ts.last_launches;
+            continue;
+        }
         cudaError_t e = cudaErrorInvalidValue;
         switch (v.family) {
             case 0: case 1: case 2: case 4: e = launch_closed(v.family, v.dp, v.wide, grid, st, a); break;
@@ -608,6 +632,11 @@ size_t qmc_workspace_bytes_opts(int count, const qmc_problem* problems, const qm
     return plan.total;
 }
 size_t qmc_workspace_bytes(int count, const qmc_problem* problems) { return qmc_workspace_bytes_opts(count, problems, nullptr); }
+size_t qmc_sector_module_workspace_bytes(const qmc_sector_module* module, int count, const qmc_problem* problems) {
+    Plan plan;
+    if (!module || make_plan(count, problems, true, &plan, kDefaultOptions, module) != QMC_OK) return 0;
+    return plan.total;
+}
 
 int qmc_plan_info(int count, const qmc_problem* problems, long long* out_tiles, int* out_ctas, long long* out_tile_len0) {
     Plan plan;
@@ -637,6 +666,13 @@ int qmc_lattice_integrate_batch_opts(int count, const qmc_problem* problems, dou
                                      const qmc_plan_options* opts) {
     return run_batch(count, problems, out_means, out_errs, out_shift_means, workspace, workspace_bytes,
                      static_cast<cudaStream_t>(cuda_stream), opts ? *opts : kDefaultOptions);
+}
+int qmc_lattice_integrate_batch_module(qmc_sector_module* module, int count, const qmc_problem* problems, double* out_means,
+                                       double* out_errs, double* out_shift_means, void* workspace, size_t workspace_bytes,
+                                       void* cuda_stream) {
+    if (!module) return QMC_ERR_NULL;
+    return run_batch(count, problems, out_means, out_errs, out_shift_means, workspace, workspace_bytes,
+                     static_cast<cudaStream_t>(cuda_stream), kDefaultOptions, nullptr, nullptr, module);
 }
 int qmc_lattice_integrate_batch(int count, const qmc_problem* problems, double* out_means, double* out_errs,
                                 double* out_shift_means, void* workspace, size_t workspace_bytes, void* cuda_stream) {

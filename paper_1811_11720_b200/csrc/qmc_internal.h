@@ -81,6 +81,7 @@ struct alignas(16) DevProblem {
     int aux_len;
     int out_index;             // index of the problem in the caller's arrays
     int gen;                   // the transform for the generic tile loop: GEN_* | r0 << 4 | r1 << 8
+    int spec_case;             // specialised sector kernel (qmc_spec.cu): the problem's case in its kernel; else 0
 };
 
 // Per-problem tables derived on the device by prepare_kernel (one record per problem).

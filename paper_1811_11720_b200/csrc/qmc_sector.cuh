@@ -22,17 +22,14 @@
 // touches must stay in the 6 KB L0 instruction cache.
 #pragma once
 #include "qmc_fused.cuh"
+#include "qmc_sector_compile.h"
 
 namespace qmc {
 
 constexpr int kSecMaxSlots = sector_slot_words(2 * kMaxSectorMono) / 2;   // coefficient slots of a program: one per monomial + end-of-polynomial + read-ahead
 constexpr int kSecMaxWords = kMaxSectorOps / 4;
-constexpr int kSecKinds = 5;
 constexpr int kSecParkRows = 16;                       // rows of G... doubles per thread parked in shared memory: weights [0, 8), U [8, 16)
 
-// step codes (one byte each): 0 = no-op, 1 = end of a polynomial that is not the last, 2 = end of program, 3 + 5 j + kind
-enum : int { SEC_NOP = 0, SEC_ENDP = 1, SEC_END = 2, SEC_BASE = 3 };
-enum : int { SEC_SC = 0, SEC_SL = 1, SEC_AL = 2, SEC_ALI = 3, SEC_AM = 4 };
 
 template <int NT> struct alignas(16) SectorSmem {
     double slots[kSecMaxSlots * 4];  // {cf, cf2} per coefficient-consuming step, in program order (complex family: {cf_re, cf_im, cf2_re, cf2_im})
@@ -41,13 +38,13 @@ template <int NT> struct alignas(16) SectorSmem {
     unsigned long long nu_packed;    // nu_j in 4 bits each
     int a, b;                        // powers of U and F
     double lg[2];                    // lu, lf of the log factor
-    int logp, pad_;                  // its power p (0 = no log factor)
+    int logp, sel;                   // its power p (0 = no log factor); specialised kernels: the problem's case selector
     double park[kSecParkRows * NT];  // [row][thread]: rows [0, 8) the G weights of a thread while the interpreter runs (with a log
                                      // factor afterwards F), rows [8, 16) U as the interpreter parks it (complex: (re, im) pairs)
 };
 struct SectorOff {                   // byte offsets of the fields above (read with ld.shared in the inner loop)
     static constexpr unsigned slots = 0, words = kSecMaxSlots * 32, c0u = words + kSecMaxWords * 4, nu = c0u + 16, ab = nu + 8, lg = ab + 8,
-                              logp = lg + 16, park = logp + 8;
+                              logp = lg + 16, sel = logp + 4, park = logp + 8;
 };
 #define QMC_SECTOR_OFF_CHECK(NT)                                                                                                      \
     static_assert(offsetof(SectorSmem<NT>, words) == SectorOff::words && offsetof(SectorSmem<NT>, c0u) == SectorOff::c0u &&           \
@@ -58,136 +55,6 @@ QMC_SECTOR_OFF_CHECK(256) QMC_SECTOR_OFF_CHECK(384)
 #undef QMC_SECTOR_OFF_CHECK
 
 __host__ __device__ inline int sector_dim_slots(int dim) { return dim <= 4 ? 4 : (dim <= 6 ? 6 : (dim <= 8 ? 8 : (dim <= 16 ? 16 : -1))); }
-
-// ---- device-side compiler: params -> program (one thread per problem; runs once per call) ---------------------------
-// Program area of a problem (8-byte words at prog_area + aux_off): sector_slot_words(nmono) words of coefficient slots,
-// then the step bytes.  DevAux: sec_nops[0] = number of 32-bit step words, sec_ncoef[0] = number of slots.
-struct SecEmit {                     // output cursor of the compiler
-    double* slots;
-    unsigned char* ops;
-    int nslots, nops, max_slots, max_ops, status;
-    bool cplx;                       // 32-byte slots {cf_re, cf_im, cf2_re, cf2_im}
-    __device__ void op(int kind, int j) {
-        if (nops >= max_ops) { status = QMC_ERR_PARAMS; return; }
-        ops[nops++] = (unsigned char)(SEC_BASE + kSecKinds * j + kind);
-    }
-    __device__ void slot(double cf, double cfi, double cf2, double cf2i) {
-        if (nslots >= max_slots) { status = QMC_ERR_PARAMS; return; }
-        if (cplx) { slots[4 * nslots] = cf; slots[4 * nslots + 1] = cfi; slots[4 * nslots + 2] = cf2; slots[4 * nslots + 3] = cf2i; }
-        else { slots[2 * nslots] = cf; slots[2 * nslots + 1] = cf2; }
-        ++nslots;
-    }
-};
-
-// One polynomial: `cnt` monomials, coefficients c[t], exponents e[t*d + j] (validated by the caller: integers 0..8, degree <= 16).
-// Greedy Horner form.  A work item is a set of monomials (a range of idx[]) that share the prefix monomial they were reached
-// by; rem[t][j] are the exponents still to be factored out, left[t] their sum.  From an item the variable that occurs in most of
-// its monomials is factored out: the monomials that contain it form a child (processed as an item of its own unless it is a
-// single finished monomial, a "leaf"), the others stay.  When the item is used up its group is emitted: prefix, the coefficient
-// of the prefix monomial itself (own) and the leaves.  Returns the constant term.
-// ci: imaginary parts of the coefficients (complex family) or nullptr; the constant term is returned through c0_re / c0_im.
-__device__ inline void compile_polynomial(const double* c, const double* ci, const double* e, int cnt, int d, SecEmit& out,
-                                          double* c0_re, double* c0_im) {
-    unsigned char rem[kMaxSectorMono][16];
-    unsigned char left[kMaxSectorMono];
-    short idx[kMaxSectorMono];
-    // work items: ranges of idx with the prefix they share (exponents) and the coefficient of the prefix monomial; items on the
-    // stack are disjoint ranges with at least one unfinished monomial each, so there are never more than cnt of them
-    short it_b[kMaxSectorMono + 1], it_e[kMaxSectorMono + 1];
-    double it_own[kMaxSectorMono + 1], it_owni[kMaxSectorMono + 1];
-    unsigned char it_prefix[kMaxSectorMono + 1][16];
-    double c0 = 0.0, c0i = 0.0;
-    int m = 0;
-    for (int t = 0; t < cnt; ++t) {
-        int deg = 0;
-        for (int j = 0; j < d; ++j) { const int v = (int)e[t * d + j]; rem[t][j] = (unsigned char)v; deg += v; }
-        for (int j = d; j < 16; ++j) rem[t][j] = 0;
-        left[t] = (unsigned char)deg;
-        if (deg == 0) { c0 += c[t]; if (ci) c0i += ci[t]; } else idx[m++] = (short)t;
-    }
-    int top = 0;
-    it_b[0] = 0; it_e[0] = (short)m; it_own[0] = 0.0; it_owni[0] = 0.0;
-    for (int j = 0; j < 16; ++j) it_prefix[0][j] = 0;
-    top = 1;
-    bool root = true;
-    while (top > 0) {
-        --top;
-        const int b = it_b[top], en = it_e[top];
-        const double own = it_own[top], owni = it_owni[top];
-        unsigned char prefix[16];
-        int pdeg = 0;
-        for (int j = 0; j < 16; ++j) { prefix[j] = it_prefix[top][j]; pdeg += prefix[j]; }
-        const bool is_root = root;
-        root = false;
-        double leaf_c[16], leaf_ci[16];
-        int leaf_mask = 0;
-        int cur = b;
-        while (cur < en) {
-            // the variable that occurs in most of the remaining monomials (lowest index on ties)
-            int best = 0, best_cnt = -1;
-            for (int j = 0; j < d; ++j) {
-                int n = 0;
-                for (int i = cur; i < en; ++i) n += rem[idx[i]][j] > 0;
-                if (n > best_cnt) { best_cnt = n; best = j; }
-            }
-            // partition: monomials containing x_best to the front, the finished ones among them first
-            int mid = cur;
-            for (int i = cur; i < en; ++i)
-                if (rem[idx[i]][best] > 0) { const short t = idx[i]; idx[i] = idx[mid]; idx[mid] = t; ++mid; }
-            double child_own = 0.0, child_owni = 0.0;
-            int fin = cur;
-            for (int i = cur; i < mid; ++i) {
-                const short t = idx[i];
-                --rem[t][best]; --left[t];
-                if (left[t] == 0) { child_own += c[t]; if (ci) child_owni += ci[t]; idx[i] = idx[fin]; idx[fin] = t; ++fin; }
-            }
-            if (fin == mid) {                                  // nothing below: a leaf of this item
-                leaf_c[best] = (leaf_mask >> best & 1) ? leaf_c[best] + child_own : child_own;
-                leaf_ci[best] = (leaf_mask >> best & 1) ? leaf_ci[best] + child_owni : child_owni;
-                leaf_mask |= 1 << best;
-            } else {                                           // a child item: prefix * x_best
-                it_b[top] = (short)fin; it_e[top] = (short)mid; it_own[top] = child_own; it_owni[top] = child_owni;
-                for (int j = 0; j < 16; ++j) it_prefix[top][j] = prefix[j];
-                ++it_prefix[top][best];
-                ++top;
-            }
-            cur = mid;
-        }
-        // emit the group of this item
-        if (is_root) {
-            for (int k = 0; k < d; ++k)
-                if (leaf_mask >> k & 1) { out.op(SEC_SL, k); out.slot(leaf_c[k], leaf_ci[k], 0.0, 0.0); }
-            continue;
-        }
-        int last = 0;
-        for (int j = 0; j < d; ++j) if (prefix[j]) last = j;
-        if (leaf_mask) {
-            bool first = true;
-            for (int k = 0; k < d; ++k)
-                if (leaf_mask >> k & 1) {
-                    out.op(first ? SEC_ALI : SEC_AL, k);
-                    out.slot(leaf_c[k], leaf_ci[k], first ? own : 0.0, first ? owni : 0.0);
-                    first = false;
-                }
-            for (int j = 0; j < d; ++j)
-                for (int r = 0; r < prefix[j] - (j == last ? 1 : 0); ++r) out.op(SEC_AM, j);
-            out.op(SEC_SC, last);
-        } else if (own != 0.0 || owni != 0.0) {
-            if (pdeg == 1) { out.op(SEC_SL, last); out.slot(own, owni, 0.0, 0.0); }
-            else {
-                int firstv = 0;
-                for (int j = d - 1; j >= 0; --j) if (prefix[j]) firstv = j;
-                out.op(SEC_ALI, firstv); out.slot(own, owni, 0.0, 0.0);
-                for (int j = 0; j < d; ++j) {
-                    const int reps = prefix[j] - (j == firstv ? 1 : 0) - (j == last ? 1 : 0);
-                    for (int r = 0; r < reps; ++r) out.op(SEC_AM, j);
-                }
-                out.op(SEC_SC, last);
-            }
-        }
-    }
-    *c0_re = c0; *c0_im = c0i;
-}
 
 __device__ inline void prepare_sector(const DevProblem& pb, DevAux& a, unsigned long long* prog_area) {
     if (threadIdx.x != 0) return;
@@ -376,16 +243,6 @@ template <int DP, int G, bool WIDE, bool SLOW, int NT> struct SectorEval {
 #pragma unroll
                 for (int q = 0; q < G; ++q) num[q] *= x[q][j];
         }
-        // optional log factor (lu log U + lf log F)^p of an eps-expansion term: a cold, warp-uniform branch
-        const int lp = (int)(unsigned)lds_u64(exbase + SectorOff::logp);
-        if (lp) {
-            const double lu = lds_f64(exbase + SectorOff::lg), lf = lds_f64(exbase + SectorOff::lg + 8u);
-#pragma unroll
-            for (int q = 0; q < G; ++q) sts_f64(park + 8u * NT * q, F[q]);
-            sector_log_factors<NT>(park, G, lu, lf, lp);
-#pragma unroll
-            for (int q = 0; q < G; ++q) num[q] *= lds_f64(park + 8u * NT * q);
-        }
         double den[G];
 #pragma unroll
         for (int q = 0; q < G; ++q) den[q] = 1.0;
@@ -397,6 +254,16 @@ template <int DP, int G, bool WIDE, bool SLOW, int NT> struct SectorEval {
             for (int e = 0; e < pa; ++e)
 #pragma unroll
                 for (int q = 0; q < G; ++q) num[q] *= U[q];
+        }
+        // optional log factor (lu log U + lf log F)^p of an eps-expansion term: a cold, warp-uniform branch (after U^a: the order of the specialised kernels)
+        const int lp = (int)(unsigned)lds_u64(exbase + SectorOff::logp);
+        if (lp) {
+            const double lu = lds_f64(exbase + SectorOff::lg), lf = lds_f64(exbase + SectorOff::lg + 8u);
+#pragma unroll
+            for (int q = 0; q < G; ++q) sts_f64(park + 8u * NT * q, F[q]);
+            sector_log_factors<NT>(park, G, lu, lf, lp);
+#pragma unroll
+            for (int q = 0; q < G; ++q) num[q] *= lds_f64(park + 8u * NT * q);
         }
 #pragma unroll 1
         for (int e = 0; e < pb; ++e)
@@ -531,7 +398,7 @@ __global__ void __launch_bounds__(NT, 1) fused_sector_kernel(const __grid_consta
             if (tid == 32) {
                 ex.c0u = a.sec_c0[0]; ex.c0u_im = a.sec_c0i[0];
                 ex.a = a.sec_a; ex.b = a.sec_b;
-                ex.lg[0] = a.sec_log[0]; ex.lg[1] = a.sec_log[1]; ex.logp = a.sec_logp; ex.pad_ = 0;
+                ex.lg[0] = a.sec_log[0]; ex.lg[1] = a.sec_log[1]; ex.logp = a.sec_logp; ex.sel = 0;
                 unsigned long long nup = 0;
                 for (int j = 0; j < 16; ++j) nup |= (unsigned long long)(a.nu[j] & 15) << (4 * j);
                 ex.nu_packed = nup;
