@@ -352,8 +352,11 @@ class DeviceBatch:
         self.arr = arr
         self.max_m = max(p["m"] for p in problems)
         self.ws_bytes = int(lib().qmc_workspace_bytes_opts(self.count, arr, C.byref(self.opts)))
-        if module is not None:
-            self.ws_bytes = max(self.ws_bytes, int(lib().qmc_sector_module_workspace_bytes(module.handle, self.count, arr)))
+        if module is not None and self.ws_bytes:
+            with_module = int(lib().qmc_sector_module_workspace_bytes(module.handle, self.count, arr))
+            if with_module == 0:
+                raise QmcError(-10, "qmc_sector_module_workspace_bytes (the module was built from another batch)")
+            self.ws_bytes = max(self.ws_bytes, with_module)
         if self.ws_bytes == 0:
             st = lib().qmc_plan_info(self.count, arr, None, None, None)
             raise QmcError(st if st != 0 else -11, "qmc_workspace_bytes")

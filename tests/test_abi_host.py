@@ -304,3 +304,129 @@ def test_sector_family_limits_in_the_struct_checks(L):
     big = synth.problem(3, np.concatenate([[1, 1, 1, 1], np.zeros(d17), [1.0], np.zeros(d17), [1.0], np.zeros(d17)]), 8191,
                         synth.korobov_form_vector(8191, d17, 2731), synth.draw_shifts(rng, 2, d17), K3)
     assert binding.qmc_validate_problem_host(big) == -2
+
+
+# ---- modules of specialised sector kernels: built on the host, no GPU needed (compiled integrands) ----
+def _sector_problem(d, seed, n=4099, m=4, family=3):
+    rng = synth.MT19937_64(seed)
+    prm = synth.sector(rng, d) if family == 3 else synth.sector_complex(rng, d)
+    return synth.problem(family, prm, n, synth.korobov_form_vector(n, d, 1 + n // 3), synth.draw_shifts(rng, m, d),
+                         synth.TRANSFORM_KOROBOV + 3, name=f"sector.d{d}.{seed}")
+
+
+def test_sector_module_builds_without_a_gpu():
+    """every dimension-slot kind is assembled for sm_100a; kernels hold at most `sectors_per_kernel` sectors of one kind"""
+    probs = [_sector_problem(d, 500 + d) for d in (2, 4, 5, 6, 6, 6, 7, 8, 11, 16)]
+    mod = binding.SectorModule(probs, sectors_per_kernel=2)
+    info = mod.info
+    assert info["specialised"] == 10
+    assert info["kernels"] == 1 + 2 + 1 + 1                  # slots 4: d = 2, 4; 6: d = 5, 6, 6, 6 (2 kernels); 8: d = 7, 8; 16: d = 11, 16
+    assert info["build_ms"] > 0 and info["image_bytes"] > 10000 and 1 <= info["host_threads"] <= info["kernels"]
+    for k in range(info["kernels"]):
+        image, log = mod.image(k)
+        assert image[:4] == b"\x7fELF"
+        assert "registers" in log and "qmc_spec_dp" in log
+    with pytest.raises(binding.QmcError):
+        mod.image(info["kernels"])
+    mod.close()
+    mod.close()                                              # idempotent
+
+
+def test_sector_module_code_is_the_compiled_program():
+    """the device code of one sector: no indexed branch per step -- one per evaluation -- and as many FP64 instructions in the
+    case as the Horner program has steps (x G points), plus the tail's multiplications"""
+    import shutil
+    import subprocess
+    import tempfile
+    if shutil.which("cuobjdump") is None:
+        pytest.skip("cuobjdump not on PATH")
+    p = _sector_problem(6, 777)
+    mod = binding.SectorModule([p])
+    image, _ = mod.image(0)
+    with tempfile.NamedTemporaryFile(suffix=".cubin") as f:
+        f.write(image)
+        f.flush()
+        sass = subprocess.run(["cuobjdump", "-sass", f.name], capture_output=True, text=True, check=True).stdout
+    assert "sm_100" in sass
+    assert sass.count("BRX") == 0                            # one sector: no selector, and no indexed branch per step either
+    three = binding.SectorModule([p, _sector_problem(6, 778), _sector_problem(6, 779)])
+    with tempfile.NamedTemporaryFile(suffix=".cubin") as f:
+        f.write(three.image(0)[0])
+        f.flush()
+        assert subprocess.run(["cuobjdump", "-sass", f.name], capture_output=True, text=True, check=True).stdout.count("BRX") == 1
+    ref = binding.SectorModule([dict(p, family=0, params=np.ones(7))])       # a batch with nothing to specialise: no kernels
+    assert ref.info["kernels"] == 0 and ref.info["specialised"] == 0
+    # count the polynomial's operations from the parameter block with the oracle-side model of the Horner form: every monomial
+    # of degree D costs between 1 and D steps, so the case holds at least (monomials - constants) and at most sum(D) steps per point
+    prm = p["params"]
+    nU, nF = int(prm[2]), int(prm[3])
+    off, lo, hi = 4 + 6, 0, 0
+    for cnt in (nU, nF):
+        e = prm[off + cnt:off + cnt + cnt * 6].reshape(cnt, 6)
+        deg = e.sum(axis=1)
+        lo += int((deg > 0).sum())
+        hi += int(deg.sum())
+        off += cnt * 7
+    fp64 = sass.count("DFMA") + sass.count("DMUL")
+    base = binding.SectorModule([dict(p, params=_one_monomial_block(6))])
+    img0, _ = base.image(0)
+    with tempfile.NamedTemporaryFile(suffix=".cubin") as f:
+        f.write(img0)
+        f.flush()
+        sass0 = subprocess.run(["cuobjdump", "-sass", f.name], capture_output=True, text=True, check=True).stdout
+    extra = fp64 - (sass0.count("DFMA") + sass0.count("DMUL"))
+    assert 8 * (lo - 2) <= extra <= 8 * (hi + 16), (extra, lo, hi)
+
+
+def _one_monomial_block(d):
+    """U = 1 + x_0, F = 1 + x_0, a = b = 1, nu = 0: the smallest valid sector"""
+    e = [0.0] * d
+    e1 = [1.0] + [0.0] * (d - 1)
+    return np.array([1.0, 1.0, 2.0, 2.0] + [0.0] * d + [1.0, 1.0] + e + e1 + [1.0, 1.0] + e + e1)
+
+
+def test_sector_module_skips_what_it_cannot_compile(L):
+    """other families, the complex sector family and blocks the validation rejects stay on the default kernels"""
+    good = _sector_problem(6, 900)
+    bad = _sector_problem(6, 901)
+    prm = bad["params"].copy()
+    prm[4 + 6 + int(prm[2]) + 2] = 9.0                       # an exponent outside 0..8
+    bad = dict(bad, params=prm)
+    osc = synth.config(0)[0]
+    cplx = _sector_problem(5, 902, family=8)
+    mod = binding.SectorModule([good, bad, osc, cplx, good])
+    assert mod.info["specialised"] == 2 and mod.info["kernels"] == 1
+    # argument checks
+    out = C.c_void_p()
+    arr = (binding.qmc_problem * 1)()
+    assert L.qmc_sector_module_create(0, arr, 0, C.byref(out)) == -3          # QMC_ERR_N
+    assert L.qmc_sector_module_create(1, None, 0, C.byref(out)) == -1         # QMC_ERR_NULL
+    assert L.qmc_sector_module_create(1, arr, 0, None) == -1
+    assert L.qmc_sector_module_create(1, arr, 5000, C.byref(out)) == -3
+    assert L.qmc_sector_module_info(None, None, None, None, None, None) == -1
+    L.qmc_sector_module_destroy(None)                        # a no-op
+
+
+def test_sector_module_is_bound_to_its_batch(L):
+    """the workspace query (and with it the launch) refuses a batch that is not the one the module was built from"""
+    probs = [_sector_problem(6, 950 + i) for i in range(3)]
+    mod = binding.SectorModule(probs)
+
+    def ws(batch):
+        arr = (binding.qmc_problem * len(batch))()
+        keep = []
+        for i, p in enumerate(batch):
+            z = np.ascontiguousarray(p["z"], dtype=np.uint64)
+            keep += [z, p["params"], p["shifts"]]
+            arr[i] = binding.qmc_problem(p["family"], p["dim"], p["m"], p["transform"], p["n"], p["params"].ctypes.data, len(p["params"]),
+                                         z.ctypes.data, p["shifts"].ctypes.data, None)
+        return L.qmc_sector_module_workspace_bytes(mod.handle, len(batch), arr), L.qmc_workspace_bytes(len(batch), arr)
+
+    with_module, default = ws(probs)
+    assert with_module > 0 and default > 0
+    assert ws(probs[:2])[0] == 0                             # another count
+    assert ws([probs[0], _sector_problem(5, 960), probs[2]])[0] == 0          # another dimension
+    assert ws([probs[0], dict(probs[1], family=0, params=np.ones(7)), probs[2]])[0] == 0
+    # another lattice, other shifts, another transform: the same module (the transform only changes the routing)
+    relattice = [dict(_sector_problem(6, 950 + i, n=65537, m=9), transform=synth.TRANSFORM_BAKER) for i in range(3)]
+    assert ws(relattice)[0] > 0

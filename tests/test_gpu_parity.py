@@ -822,3 +822,88 @@ def test_fit_from_cdf_samples():
     _, _, err1 = run_gpu([dict(p, fit_coeffs=full)])
     assert err1[0, 0] < err0[0, 0]
     check_against_oracle([dict(p, fit_coeffs=full, name="cdf-fit")])
+
+
+# ------------------------------------------------------------------------------------------------
+# specialised sector kernels (qmc_sector_module_*): the sectors of a batch as compiled straight-line code,
+# PAPER.md L427-L438 (the paper compiles every integrand); the interpreting kernel is the default
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("d", [1, 2, 3, 4, 5, 6, 7, 8, 9, 12, 16])
+def test_module_means_against_the_oracle(d):
+    """every dimension-slot kind (4, 6, 8, 16), ragged tile tails, several sectors per kernel and one per kernel"""
+    probs = [make(3, d, n, 5, K + 3, 9800 + 7 * d + i) for i, n in enumerate([127, 1021, 8191, 65537])]
+    for per_kernel in (0, 1):
+        mod = binding.SectorModule(probs, per_kernel)
+        assert mod.info["specialised"] == 4 and mod.info["kernels"] == (4 if per_kernel else 1)
+        check_against_oracle(probs, module=mod)
+        mod.close()
+
+
+@pytest.mark.parametrize("d", [3, 6, 8, 13])
+def test_module_returns_the_bits_of_the_interpreting_kernel(d):
+    """one problem per call: both routes tile alike, evaluate the same operations in the same order and must agree in every bit
+    (with and without a log factor, whose U goes through shared memory on both routes)"""
+    for p in (make(3, d, 262147, 9, K + 3, 9850 + d), make_log(d, 65537, 6, K + 3, 9860 + d, pw=2)):
+        mod = binding.SectorModule([p])
+        a = run_gpu([p])
+        b = run_gpu([p], module=mod)
+        assert a[0][0].tobytes() == b[0][0].tobytes() and a[1].tobytes() == b[1].tobytes() and a[2].tobytes() == b[2].tobytes()
+
+
+def test_module_mixed_batch_routes_only_what_it_covers():
+    """closed-form families, complex sectors, other transforms, fit maps and a rejected block stay on the default kernels in the
+    same call; a and b = 0, nu up to 8 and log factors run specialised"""
+    probs = [make(3, 6, 8191, 5, K + 3, 9900), make(0, 5, 4099, 4, K + 3, 9901), make(8, 4, 4099, 4, K + 3, 9902),
+             make(3, 6, 8191, 5, BAKER, 9903), make(3, 4, 8191, 5, K + 3, 9904, fit=True), make(3, 6, 8191, 5, K + 2, 9905),
+             make_log(6, 8191, 5, K + 3, 9906, pw=3), make_log(8, 4099, 4, K + 3, 9907, pw=4), make(3, 16, 4099, 4, K + 3, 9908)]
+    zero_powers = make(3, 5, 8191, 5, K + 3, 9909)
+    prm = zero_powers["params"].copy()
+    prm[0] = prm[1] = 0.0                                    # a = b = 0: the integrand is the monomial alone
+    prm[4:9] = [8.0, 0.0, 3.0, 1.0, 0.0]
+    probs.append(dict(zero_powers, params=prm, name="a=b=0"))
+    bad = make(3, 6, 8191, 5, K + 3, 9910)
+    prm = bad["params"].copy()
+    prm[4 + 6 + int(prm[2])] = 2.5                           # a fractional exponent in U
+    bad = dict(bad, params=prm, name="bad")
+    mod = binding.SectorModule(probs + [bad])
+    assert mod.info["specialised"] == 8                      # every real sector but the rejected one (routing is decided per call)
+    sms, means, errs = run_gpu(probs + [bad], module=mod)
+    assert np.isnan(means[-1, 0]) and np.isnan(errs[-1, 0])
+    ref = run_gpu(probs + [bad])
+    assert np.isnan(ref[1][-1, 0])
+    for i, p in enumerate(probs):
+        sm_or, mean_or, err_or = oracle.integrate(p)
+        assert_means(sms[i], sm_or, p["name"])
+        assert_err(errs[i, :sm_or.shape[1]], err_or, sm_or, p["name"])
+
+
+def test_module_serves_other_lattices_and_rejects_other_batches():
+    """the module depends on the integrands only: new n, z, shifts and m reuse it; a batch of another shape is refused"""
+    probs = [make(3, 6, 4099, 4, K + 3, 9950 + i) for i in range(5)]
+    mod = binding.SectorModule(probs)
+    other = [dict(make(3, 6, 65537, 7, K + 3, 9950 + i), name=f"relattice{i}") for i in range(5)]
+    for a, b in zip(probs, other):
+        assert np.array_equal(a["params"], b["params"])
+    check_against_oracle(other, module=mod)
+    with pytest.raises(binding.QmcError):
+        binding.DeviceBatch(probs[:4], module=mod)           # count differs: the workspace query fails
+    swapped = [probs[0], make(3, 5, 4099, 4, K + 3, 9960)] + probs[2:]
+    with pytest.raises(binding.QmcError):
+        binding.DeviceBatch(swapped, module=mod)
+
+
+def test_module_config3_full_size():
+    """BASELINE.json configs[3] at full size through the specialised kernels, bench.py's second launch configuration for that
+    workload: EVERY sector against the oracle's stored full-size record"""
+    g = _golden()
+    probs = synth.config(3)
+    mod = binding.SectorModule(probs)
+    assert mod.info["specialised"] == 256 and mod.info["kernels"] == 8
+    batch = binding.DeviceBatch(probs, module=mod)
+    assert batch.integrate() == 1 + 8 + 1                    # prepare, one launch per kernel of the module, finalize
+    sms, means, errs = batch.results()
+    for key, rec in g["3"]["sectors"].items():
+        i = int(key)
+        sm_or, mean_or, err_or = _golden_arrays(rec, 1)
+        assert_means(sms[i], sm_or, probs[i]["name"] + " (full size, specialised)")
+        assert_err(errs[i, :1], err_or, sm_or, probs[i]["name"])
