@@ -58,9 +58,9 @@ ALG_FP64_PER_EVAL = {
 }
 # thread-level FP64-pipe instructions per evaluation the fused kernels EXECUTE (ncu smsp__inst_executed_pipe_fp64 x 32 / evaluations;
 # profiles/r2_dram_full.md): the conversion of the residues, padded slots and the interpreter's bookkeeping on top of the above
-EXECUTED_FP64_PER_EVAL = {1: 56.05, 2: 171.4, 3: 100.4, 4: 278.25}
+EXECUTED_FP64_PER_EVAL = {1: 56.05, 2: 171.4, 3: 100.4, "3s": 100.44, 4: 278.25}     # "3s": configs[3] through the specialised kernels (profiles/r2_spec_full.md)
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused kernel at FULL size (ncu, profiles/r2_dram_full.md)
-PROFILED_DRAM_BYTES_PER_LAUNCH = {1: 70400, 2: 244992, 3: 1202176, 4: 215808}
+PROFILED_DRAM_BYTES_PER_LAUNCH = {1: 70400, 2: 244992, 3: 1202176, "3s": 376896, 4: 215808}   # "3s": mean of the 8 launches of a step
 FP64_LANES_PER_SM = 64                        # B200 (sm_100): 64 FP64 FMA lanes per SM -> nominal peak
 
 
@@ -223,7 +223,7 @@ def config4_with_device_fit(binding, probs):
     return [dict(p, fit_coeffs=binding.qmc_fit_cubic(H))]
 
 
-def e2e_host_api(binding, probs, reps):
+def e2e_host_api(binding, probs, reps, module=None):
     """The same metric through the synchronous HOST-pointer C-ABI call (qmc_lattice_integrate_batch_host; one problem or a
     whole batch in ONE call): validation, the host->device copy of all inputs from pinned staging memory, the kernels, the
     device->host copy of the results and the synchronisation are all inside the timed region (host wall clock around a
@@ -232,7 +232,7 @@ def e2e_host_api(binding, probs, reps):
     for p in probs:
         h2d += p["params"].nbytes + p["z"].nbytes + p["shifts"].nbytes + (0 if p.get("fit_coeffs") is None else p["fit_coeffs"].nbytes)
     d2h = len(probs) * (4 + 2 * max(p["m"] for p in probs)) * 8
-    hb = binding.HostBatch(probs)                           # argument structs built once; the timed call is the C entry
+    hb = binding.HostBatch(probs, module=module)            # argument structs built once; the timed call is the C entry
     hb.integrate()                                          # warm-up (module load, staging arena)
     t0 = time.perf_counter()
     for _ in range(reps):
@@ -439,17 +439,30 @@ def run_ours(args):
     peak_rate, peak_ms = binding.qmc_fp64_peak_probe(60000)
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
 
-    def measure(c, steps, warmup):
+    def measure(c, steps, warmup, specialised=False):
+        """specialised (configs[3] only): the sectors as compiled straight-line code (qmc_sector_module_create, PAPER.md L427-L438:
+        the paper compiles its integrands before integrating); the module is built once, outside the timed steps, and its
+        build time is reported beside the line"""
         probs = rank_problems(c, rank)
         if c == 4:
             probs = config4_with_device_fit(binding, probs)
         alg = ALG_FP64_PER_EVAL[c] + (ALG_FP64_SECTOR_LOG_EXTRA if c == 3 and SECTOR_LOG else 0)
-        executed = EXECUTED_FP64_PER_EVAL.get(c) if not (c == 3 and SECTOR_LOG) else None
-        traffic = PROFILED_DRAM_BYTES_PER_LAUNCH.get(c) if SHRINK == 1 and not SECTOR_LOG else None
-        return measure_probs(bench_config(c)["workload"], probs, alg, executed, traffic, steps, warmup)
+        key = "3s" if specialised else c
+        executed = EXECUTED_FP64_PER_EVAL.get(key) if not (c == 3 and SECTOR_LOG) else None
+        traffic = PROFILED_DRAM_BYTES_PER_LAUNCH.get(key) if SHRINK == 1 and not SECTOR_LOG else None
+        label = bench_config(c)["workload"]
+        if c == 3:
+            label += " [specialised kernels: qmc_sector_module]" if specialised else " [interpreting kernel: the default entry]"
+        module = binding.SectorModule(probs) if specialised else None
+        rec, probs, w = measure_probs(label, probs, alg, executed, traffic, steps, warmup, module)
+        if module is not None:
+            info = module.info
+            rec["sector_module"] = dict(info, note="built once per batch of integrands on the host (Horner compile -> PTX -> nvJitLink, "
+                                        "kernels in parallel), outside the timed steps; reused for every lattice, shift set and sample count")
+        return rec, probs, w
 
-    def measure_probs(label, probs, alg, executed, traffic, steps, warmup):
-        batch = binding.DeviceBatch(probs, device=device)
+    def measure_probs(label, probs, alg, executed, traffic, steps, warmup, module=None):
+        batch = binding.DeviceBatch(probs, device=device, module=module)
         barrier()
         w0 = time.perf_counter()
         step_ms, fused_ms, launches = time_steps(torch, binding, batch, steps, warmup, flush)
@@ -479,16 +492,20 @@ def run_ours(args):
         return rec, probs, (w0, w1)
 
     windows = []
-    main, main_probs, w = measure(args.main, args.steps, args.warmup)
+    main, main_probs, w = measure(args.main, args.steps, args.warmup, specialised=args.main == 3 and not args.interpret)
     windows.append(w)
     others = []
+    interpreted3 = None
     if not args.main_only:
         for c, (k, wu) in {0: (50, 5), 1: (50, 5), 2: (10, 3), 3: (5, 3), 4: (3, 3)}.items():
             if c == args.main or (args.others is not None and c not in args.others):
                 continue
-            rec, _, w = measure(c, k, wu)
+            rec, _, w = measure(c, k, wu, specialised=c == 3 and not args.interpret)
             windows.append(w)
             others.append(rec)
+            if c == 3 and not args.interpret:                # the same workload through the default entry, beside it
+                interpreted3, _, w = measure(3, k, wu)
+                windows.append(w)
     # variants beyond the BASELINE configs: the generic transforms and the pole-term fit on configs[2]'s / [4]'s shape, the
     # complex sector family on configs[3]'s shape.  alg counts: DESIGN.md section 5 ("variants").
     variants = []
@@ -504,6 +521,12 @@ def run_ours(args):
         if rec_c >= 1:
             roofline_all[f"configs[{rec_c}]"] = dict(rec["roofline"], fused_kernel_ms=rec["fused_kernel_ms"], ms_per_step=rec["ms_per_step"],
                                                      evals_per_s=rec["value"], workload=rec["workload"])
+            if "sector_module" in rec:
+                roofline_all[f"configs[{rec_c}]"]["sector_module"] = rec["sector_module"]
+    if interpreted3 is not None:
+        r = interpreted3
+        roofline_all["configs[3] interpreted"] = dict(r["roofline"], fused_kernel_ms=r["fused_kernel_ms"], ms_per_step=r["ms_per_step"],
+                                                      evals_per_s=r["value"], workload=r["workload"])
 
     # S10, the projection pass of configs[4] (n_fit lattice, one shift, 256 bins, all 16 dimensions): device time of the two kernels
     projection = None
@@ -563,7 +586,8 @@ def run_ours(args):
     # end-to-end through the HOST-pointer entry (rank-local; max over ranks)
     barrier()
     e2e_reps = max(3, min(args.steps, 50 if main["ms_per_step"] < 10 else 5))
-    e2e_s, h2d, d2h = e2e_host_api(binding, main_probs, e2e_reps)
+    main_module = binding.SectorModule(main_probs) if "sector_module" in main else None   # configs[3]: the route of the headline line
+    e2e_s, h2d, d2h = e2e_host_api(binding, main_probs, e2e_reps, main_module)
     e2e_s = max_over_ranks(e2e_s)
     sampler.stop()
     clocks = sampler.summary(windows)
@@ -577,7 +601,7 @@ def run_ours(args):
                    "plan": main["plan"], "timed_region_s": main["ms_per_step"] * args.steps * 1e-3},
            "e2e": {"value": aggregate([main["evals_per_step_per_gpu"]] * world, e2e_s), "unit": UNIT, "h2d_bytes_per_step": h2d,
                    "d2h_bytes_per_step": d2h, "ms_per_step": e2e_s * 1e3, "reps": e2e_reps,
-                   "api": "qmc_lattice_integrate_batch_host (HOST pointers; validation + H2D from pinned staging + kernels + D2H + sync inside the timed call)"},
+                   "api": ("qmc_lattice_integrate_batch_host_module" if main_module is not None else "qmc_lattice_integrate_batch_host") + " (HOST pointers; validation + H2D from pinned staging + kernels + D2H + sync inside the timed call)"},
            "gpu_launches": main["gpu_launches_per_step"] * args.steps,
            "roofline": main["roofline"], "roofline_all": roofline_all, "projection_pass": projection,
            "fused_kernel_ms": main["fused_kernel_ms"],
@@ -737,6 +761,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--main-only", action="store_true", help="time the headline config only (skip 'others', time-to-target, graphs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--interpret", action="store_true",
+                    help="configs[3]: time the interpreting kernel only (no module of specialised sector kernels is built)")
     ap.add_argument("--genz-table", action="store_true",
                     help="run the Genz protocol of the paper's Table 1 / Table 2 through qmc_integrate instead of the throughput bench")
     ap.add_argument("--sector-log", action="store_true",

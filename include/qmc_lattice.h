@@ -329,6 +329,10 @@ int qmc_sector_module_info(const qmc_sector_module* module, int* n_specialised, 
  * *image_bytes with image = NULL; QMC_ERR_WORKSPACE if image_cap is too small */
 int qmc_sector_module_image(const qmc_sector_module* module, int kernel, void* image /*HOST or NULL*/, size_t image_cap,
                             size_t* image_bytes /*HOST or NULL*/, char* log /*HOST or NULL*/, size_t log_cap);
+/* qmc_lattice_integrate_batch_host (synchronous, HOST data pointers) with a module; module = NULL is that entry itself */
+int qmc_lattice_integrate_batch_host_module(qmc_sector_module* module /*or NULL*/, int count,
+                                            const qmc_problem* problems /*HOST, HOST data pointers*/, double* out_means /*HOST*/,
+                                            double* out_errs /*HOST*/, double* out_shift_means /*HOST or NULL*/);
 size_t qmc_sector_module_workspace_bytes(const qmc_sector_module* module, int count, const qmc_problem* problems /*HOST*/);  /* 0 on invalid input */
 int qmc_lattice_integrate_batch_module(qmc_sector_module* module, int count, const qmc_problem* problems /*HOST*/,
                                        double* out_means /*DEVICE*/, double* out_errs /*DEVICE*/,

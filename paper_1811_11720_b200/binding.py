@@ -24,6 +24,7 @@ EXPORTS = [
     "qmc_release_thread_resources", "qmc_sector_compile", "qmc_lattice_cdf_samples", "qmc_cdf_workspace_bytes",
     "qmc_cdf_sample_count", "qmc_fit_from_cdf", "qmc_sector_module_create", "qmc_sector_module_destroy", "qmc_sector_module_info",
     "qmc_sector_module_image", "qmc_lattice_integrate_batch_module", "qmc_sector_module_workspace_bytes",
+    "qmc_lattice_integrate_batch_host_module",
 ]
 
 QMC_OK = 0
@@ -86,6 +87,7 @@ def lib():
         L.qmc_sector_module_destroy.restype = None
         L.qmc_sector_module_info.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int), dp, C.POINTER(C.c_size_t), C.POINTER(C.c_int)]
         L.qmc_sector_module_image.argtypes = [vp, C.c_int, vp, C.c_size_t, C.POINTER(C.c_size_t), C.c_char_p, C.c_size_t]
+        L.qmc_lattice_integrate_batch_host_module.argtypes = [vp, C.c_int, pp, dp, dp, dp]
         L.qmc_sector_module_workspace_bytes.argtypes = [vp, C.c_int, pp]
         L.qmc_sector_module_workspace_bytes.restype = C.c_size_t
         L.qmc_lattice_integrate_batch_module.argtypes = [vp, C.c_int, pp, vp, vp, vp, vp, C.c_size_t, vp]
@@ -187,8 +189,9 @@ class HostBatch:
     """Problems marshalled once for repeated synchronous HOST-pointer calls (qmc_lattice_integrate_batch_host): the numpy
     arrays stay where they are, `integrate()` is the C call and nothing else."""
 
-    def __init__(self, problems):
+    def __init__(self, problems, module=None):
         self.problems = problems
+        self.module = module                               # a SectorModule built from the same problems, or None
         self.count = len(problems)
         self.arr = (qmc_problem * self.count)()
         self._keep = []
@@ -203,6 +206,9 @@ class HostBatch:
         self.shift_means = np.zeros((self.count, 2 * self.max_m))
         self._args = (self.count, self.arr, _d(self.means), _d(self.errs), _d(self.shift_means))
         self._fn = lib().qmc_lattice_integrate_batch_host
+        if module is not None:
+            self._args = (module.handle,) + self._args
+            self._fn = lib().qmc_lattice_integrate_batch_host_module
 
     def integrate(self):
         _check(self._fn(*self._args), "qmc_lattice_integrate_batch_host")

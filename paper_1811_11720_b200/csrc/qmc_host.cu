@@ -684,6 +684,11 @@ int qmc_lattice_integrate_batch(int count, const qmc_problem* problems, double* 
 // staging block, the results come back in one device-to-host copy; device memory comes from the thread's arena.
 int qmc_lattice_integrate_batch_host(int count, const qmc_problem* problems, double* out_means, double* out_errs,
                                      double* out_shift_means) {
+    return qmc_lattice_integrate_batch_host_module(nullptr, count, problems, out_means, out_errs, out_shift_means);
+}
+
+int qmc_lattice_integrate_batch_host_module(qmc_sector_module* module, int count, const qmc_problem* problems, double* out_means,
+                                            double* out_errs, double* out_shift_means) {
     if (count < 1) return QMC_ERR_N;
     if (!problems || !out_means || !out_errs) return QMC_ERR_NULL;
     int max_m = 0;
@@ -699,7 +704,7 @@ int qmc_lattice_integrate_batch_host(int count, const qmc_problem* problems, dou
     const size_t out_doubles = (size_t)count * (4 + 2 * (size_t)max_m);     // means (2), errs (2), shift means (2 max_m) per problem
     const size_t out_bytes = align_up(out_doubles * 8, 256);
     Plan plan;
-    const int pst = make_plan(count, problems, true, &plan);
+    const int pst = make_plan(count, problems, true, &plan, kDefaultOptions, module);
     if (pst != QMC_OK) return pst;
     const size_t blob_bytes = align_up(plan.off_aux - plan.off_counters, 256);
     const int ast = arena_reserve(in_bytes + blob_bytes + out_bytes, in_bytes + out_bytes + plan.total + 256);
@@ -730,7 +735,7 @@ int qmc_lattice_integrate_batch_host(int count, const qmc_problem* problems, dou
     double* d_errs = d_out + (size_t)count * 2;
     double* d_sm = d_out + (size_t)count * 4;
     QMC_CUDA(cudaMemcpyAsync(d_in, h_in, in_bytes, cudaMemcpyHostToDevice, st));
-    const int status = run_batch(count, problems, d_means, d_errs, d_sm, d_ws, plan.total, st, kDefaultOptions, h_blob, &plan);
+    const int status = run_batch(count, problems, d_means, d_errs, d_sm, d_ws, plan.total, st, kDefaultOptions, h_blob, &plan, module);
     if (status != QMC_OK) { cudaStreamSynchronize(st); return status; }
     QMC_CUDA(cudaMemcpyAsync(h_out, d_out, out_doubles * 8, cudaMemcpyDeviceToHost, st));
     QMC_CUDA(cudaStreamSynchronize(st));
