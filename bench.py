@@ -514,6 +514,12 @@ def run_ours(args):
             rec, _, w = measure_probs(label, probs, alg, None, None, k, 3)
             windows.append(w)
             variants.append(rec)
+            if probs[0]["family"] == synth.FAMILY_SECTOR_COMPLEX and not args.interpret:       # the same batch as compiled code
+                module = binding.SectorModule(probs)
+                rec, _, w = measure_probs(label + " [specialised kernels: qmc_sector_module]", probs, alg, None, None, k, 3, module)
+                rec["sector_module"] = module.info
+                windows.append(w)
+                variants.append(rec)
 
     # the roofline record of every config of the target (configs[1..4]) at top level
     roofline_all = {}

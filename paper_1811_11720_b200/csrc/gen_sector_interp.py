@@ -172,6 +172,24 @@ template <> __device__ __forceinline__ void sector_poly_site<{dp}, {g}>(const do
 """
 
 
+def gen_csite(dp, g):
+    """complex family: outputs n = W prod x^nu U^a, d = F^b, F and U as (re, im) pairs"""
+    names = ["nr", "ni", "dr", "di", "Fr", "Fi", "Ur", "Ui"]
+    ops = [f'"=d"({nm}[{q}])' for nm in names for q in range(g)]
+    ins = ([f'"d"(x[{q}][{j}])' for q in range(g) for j in range(dp)] + [f'"d"(W[{q}])' for q in range(g)] + ['"r"(sel)'])
+    text = "@@QMC_SITE " + " ".join(f"%{i}" for i in range(len(ops) + len(ins))) + ";"
+    args = ", ".join(f"double (&{nm})[{g}]" for nm in names)
+    return f"""
+template <> __device__ __forceinline__ void csector_poly_site<{dp}, {g}>(const double (&x)[{g}][{dp}], const double (&W)[{g}], unsigned sel,
+                                                                      {args}) {{
+    asm volatile("{text}"
+        : {", ".join(ops)}
+        : {", ".join(ins)}
+        : "memory");
+}}
+"""
+
+
 def main():
     here = os.path.dirname(os.path.abspath(__file__))
     out = ["// GENERATED by gen_sector_interp.py -- do not edit.  Threaded-code interpreter of the sector family",
@@ -200,6 +218,11 @@ def main():
             "                                                                          double (&F)[G]);"]
     with open(os.path.join(here, "qmc_sector_site.inc"), "w") as f:
         f.write("\n".join(site + [gen_site(dp, g) for dp, g, _, c in VARIANTS if not c]))
+        f.write("\n".join(["", "// complex family: operands nr[G], ni[G], dr[G], di[G], Fr[G], Fi[G], Ur[G], Ui[G] (outputs), x[G][DP], W[G], the case selector",
+                           "template <int DP, int G> __device__ __forceinline__ void csector_poly_site(const double (&x)[G][DP], const double (&W)[G], unsigned sel,",
+                           "                                                                           double (&nr)[G], double (&ni)[G], double (&dr)[G], double (&di)[G],",
+                           "                                                                           double (&Fr)[G], double (&Fi)[G], double (&Ur)[G], double (&Ui)[G]);"]
+                          + [gen_csite(dp, g) for dp, g, _, c in VARIANTS if c]))
 
 
 if __name__ == "__main__":

@@ -230,7 +230,7 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
         const int dp = dim_slots(d.family, d.dim, wide);
         // a specialised kernel holds the sector's code and serves the default tile loop only (Korobov-3, no fit map, narrow residues)
         int kfam = kernel_family(d.family), spec_kernel = -1;
-        if (module && d.family == QMC_FAMILY_SECTOR && !wide && d.tr_kind == TR_KOR3 && !d.has_fit && spec_problems(module)[i].kernel >= 0) {
+        if (module && is_sector_family(d.family) && !wide && d.tr_kind == TR_KOR3 && !d.has_fit && spec_problems(module)[i].kernel >= 0) {
             kfam = kKernelFamilySpec;
             spec_kernel = spec_problems(module)[i].kernel;
             plan->dev[i].spec_case = spec_problems(module)[i].kase;
@@ -247,8 +247,8 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
     for (auto& v : plan->variants) {
         const bool sector_variant = v.family == QMC_FAMILY_SECTOR || v.family == kKernelFamilyCSector || v.family == kKernelFamilySpec;
         const int resident = kPlanSMs * (sector_variant ? min_blocks_sector(v.dp) : min_blocks_closed(v.dp, v.wide));
-        const int threads = (v.family == QMC_FAMILY_SECTOR || v.family == kKernelFamilySpec) ? sector_threads(v.dp)
-                                                                                              : (v.family == kKernelFamilyCSector ? kCSectorThreads : kThreads);   // CTA size of the variant's kernel
+        const int threads = v.family == kKernelFamilySpec ? spec_kernel_threads(module, v.spec_kernel)
+                            : (v.family == QMC_FAMILY_SECTOR ? sector_threads(v.dp) : (v.family == kKernelFamilyCSector ? kCSectorThreads : kThreads));   // CTA size of the variant's kernel
         const int env = opt.tiles_target > 0 ? opt.tiles_target : 0;
         // one problem: equal tiles, 2 per resident CTA (the queue evens out SM speed differences over a long kernel) -- or
         // exactly 1 when the whole kernel is short (< kShortEvalsPerCta evaluations per CTA: per-tile overhead and the

@@ -34,22 +34,29 @@ namespace qmc {
 namespace {
 
 // ---- the kernel template ---------------------------------------------------------------------------------------------
-struct SlotKind { int dp, g, threads; const char* entry; size_t smem; };
-const SlotKind kSlotKinds[4] = {{4, 8, 384, "qmc_spec_dp4", sizeof(SectorShared<4, 8, 384>)},
-                                {6, 8, 384, "qmc_spec_dp6", sizeof(SectorShared<6, 8, 384>)},
-                                {8, 8, 256, "qmc_spec_dp8", sizeof(SectorShared<8, 8, 256>)},
-                                {16, 4, 256, "qmc_spec_dp16", sizeof(SectorShared<16, 4, 256>)}};
-static_assert(sector_group(4) == 8 && sector_group(16) == 4 && sector_threads(6) == 384 && sector_threads(8) == 256,
+struct SlotKind { int dp, g, threads; bool cplx; const char* entry; size_t smem; };
+constexpr int kSlotKindCount = 8;
+const SlotKind kSlotKinds[kSlotKindCount] = {{4, 8, 384, false, "qmc_spec_dp4", sizeof(SectorShared<4, 8, 384>)},
+                                             {6, 8, 384, false, "qmc_spec_dp6", sizeof(SectorShared<6, 8, 384>)},
+                                             {8, 8, 256, false, "qmc_spec_dp8", sizeof(SectorShared<8, 8, 256>)},
+                                             {16, 4, 256, false, "qmc_spec_dp16", sizeof(SectorShared<16, 4, 256>)},
+                                             {4, 4, 384, true, "qmc_cspec_dp4", sizeof(SectorShared<4, 4, 384>)},
+                                             {6, 4, 384, true, "qmc_cspec_dp6", sizeof(SectorShared<6, 4, 384>)},
+                                             {8, 4, 384, true, "qmc_cspec_dp8", sizeof(SectorShared<8, 4, 384>)},
+                                             {16, 2, 384, true, "qmc_cspec_dp16", sizeof(SectorShared<16, 2, 384>)}};
+static_assert(sector_group(4) == 8 && sector_group(16) == 4 && sector_threads(6) == 384 && sector_threads(8) == 256 &&
+                  csector_group(8) == 4 && csector_group(16) == 2 && kCSectorThreads == 384,
               "kSlotKinds must mirror the interpreting kernels' shapes (qmc_spec_template.cu has the same numbers)");
-int slot_kind_of(int dp) { return dp == 4 ? 0 : (dp == 6 ? 1 : (dp == 8 ? 2 : (dp == 16 ? 3 : -1))); }
+int slot_kind_of(int dp, bool cplx) { return (cplx ? 4 : 0) + (dp == 4 ? 0 : (dp == 6 ? 1 : (dp == 8 ? 2 : (dp == 16 ? 3 : -100)))); }
 
 struct EntryText {
     std::string before, after;               // the entry's PTX around the marker line
-    std::vector<std::string> operands;       // the marker's operands: num[G], den[G], F[G], x[G][DP], W[G], sel, park
+    std::vector<std::string> operands;       // the marker's operands: num[G], den[G], F[G], x[G][DP], W[G], sel, park (complex:
+                                             // nr, ni, dr, di, Fr, Fi, Ur, Ui [G] each, x[G][DP], W[G], sel)
 };
 struct Template {
     std::string header;                      // .version / .target / module-scope declarations
-    EntryText entry[4];
+    EntryText entry[kSlotKindCount];
     bool ok = false;
 };
 
@@ -60,9 +67,9 @@ const Template& kernel_template() {
         const std::string key = ".visible .entry ";
         std::vector<size_t> starts;
         for (size_t at = text.find(key); at != std::string::npos; at = text.find(key, at + 1)) starts.push_back(at);
-        if (starts.size() != 4) return r;
+        if (starts.size() != (size_t)kSlotKindCount) return r;
         r.header = text.substr(0, starts[0]);
-        for (int k = 0; k < 4; ++k) {
+        for (int k = 0; k < kSlotKindCount; ++k) {
             const size_t name_at = text.find(key + kSlotKinds[k].entry + "(");
             if (name_at == std::string::npos) return r;
             size_t end = text.size();
@@ -83,7 +90,7 @@ const Template& kernel_template() {
                 p = q;
             }
             const int g = kSlotKinds[k].g, dp = kSlotKinds[k].dp;
-            if ((int)r.entry[k].operands.size() != 3 * g + g * dp + g + 2) return r;
+            if ((int)r.entry[k].operands.size() != (kSlotKinds[k].cplx ? 8 * g + g * dp + g + 1 : 3 * g + g * dp + g + 2)) return r;
         }
         r.ok = true;
         return r;
@@ -94,18 +101,19 @@ const Template& kernel_template() {
 // ---- one sector on the host: the program of compile_polynomial, per polynomial ------------------------------------------
 struct HostPoly {
     std::vector<unsigned char> ops;
-    std::vector<double> slots;               // {cf, cf2} per coefficient-consuming step
-    double c0 = 0.0;
+    std::vector<double> slots;               // {cf, cf2} per coefficient-consuming step (complex: {cf_re, cf_im, cf2_re, cf2_im})
+    double c0 = 0.0, c0i = 0.0;
 };
 struct HostSector {
     HostPoly U, F;
     int a = 0, b = 0, nu[16] = {0}, logp = 0;
 };
 
-bool compile_sector_host(const double* p, int n_params, int d, HostSector* out) {
-    if (sector_block_status(p, n_params, d, false) != 0) return false;
+bool compile_sector_host(const double* p, int n_params, int d, bool cplx, HostSector* out) {
+    if (sector_block_status(p, n_params, d, cplx) != 0) return false;
     const int cnt[2] = {(int)p[2], (int)p[3]};
-    const int n_base = 4 + d + (cnt[0] + cnt[1]) * (1 + d);
+    const int rec = (cplx ? 2 : 1) + d, sw = cplx ? 4 : 2;
+    const int n_base = 4 + d + (cnt[0] + cnt[1]) * rec;
     out->a = (int)p[0]; out->b = (int)p[1];
     for (int j = 0; j < d; ++j) out->nu[j] = (int)p[4 + j];
     out->logp = n_params == n_base + 3 ? (int)p[n_base + 2] : 0;
@@ -114,16 +122,15 @@ bool compile_sector_host(const double* p, int n_params, int d, HostSector* out) 
     for (int k = 0; k < 2; ++k) {
         HostPoly& hp = *pol[k];
         hp.ops.assign(16 * cnt[k] + 8, 0);
-        hp.slots.assign(2 * (cnt[k] + 2), 0.0);
+        hp.slots.assign(sw * (cnt[k] + 2), 0.0);
         SecEmit em;
-        em.slots = hp.slots.data(); em.ops = hp.ops.data(); em.nslots = 0; em.nops = 0; em.status = 0; em.cplx = false;
+        em.slots = hp.slots.data(); em.ops = hp.ops.data(); em.nslots = 0; em.nops = 0; em.status = 0; em.cplx = cplx;
         em.max_slots = cnt[k] + 1; em.max_ops = 16 * cnt[k];
-        double c0i;
-        compile_polynomial(base, nullptr, base + cnt[k], cnt[k], d, em, &hp.c0, &c0i);
+        compile_polynomial(base, cplx ? base + cnt[k] : nullptr, base + (cplx ? 2 : 1) * cnt[k], cnt[k], d, em, &hp.c0, &hp.c0i);
         if (em.status) return false;
         hp.ops.resize(em.nops);
-        hp.slots.resize(2 * em.nslots);
-        base += cnt[k] * (1 + d);
+        hp.slots.resize(sw * em.nslots);
+        base += cnt[k] * rec;
     }
     return true;
 }
@@ -203,6 +210,88 @@ int emit_case(const HostSector& hs, int d, const SlotKind& sk, const std::vector
                 out.line("st.shared.f64 [%s+%d], %s;", park, 8 * sk.threads * (8 + q), val[0][q].c_str());
             }
         }
+    }
+    return nt;
+}
+
+// Complex family: the same programs on paired accumulators (two fp64 instructions per step and point); the products with U and F
+// are CSectorEval's complex multiplications, t = fma(a, c, -(b d)), fma(a, d, b c), except that the first one, (w, 0) U and
+// (1, 0) F, is written as what it evaluates to for finite values (w Ur, w Ui and F itself).
+int emit_case_complex(const HostSector& hs, int d, const SlotKind& sk, const std::vector<std::string>& o, Text& out) {
+    const int G = sk.g, DP = sk.dp;
+    auto outp = [&](int which, int q) { return o[which * G + q].c_str(); };    // nr, ni, dr, di, Fr, Fi, Ur, Ui
+    auto x = [&](int q, int j) { return o[8 * G + q * DP + j].c_str(); };
+    auto W = [&](int q) { return o[8 * G + G * DP + q].c_str(); };
+    int nt = 0;
+    auto fresh = [&]() { return "t" + std::to_string(++nt); };
+    auto op3 = [&](const char* ins, const std::string& a, const std::string& b, const std::string& c) {
+        const std::string t = fresh();
+        out.line("%s %s, %s, %s, %s;", ins, t.c_str(), a.c_str(), b.c_str(), c.c_str());
+        return t;
+    };
+    auto mul = [&](const std::string& a, const std::string& b) {
+        const std::string t = fresh();
+        out.line("mul.rn.f64 %s, %s, %s;", t.c_str(), a.c_str(), b.c_str());
+        return t;
+    };
+    auto neg = [&](const std::string& a) {
+        const std::string t = fresh();
+        out.line("neg.f64 %s, %s;", t.c_str(), a.c_str());
+        return t;
+    };
+    std::vector<std::string> vr[2], vi[2];                  // U, F at the G points
+    const HostPoly* pol[2] = {&hs.U, &hs.F};
+    for (int k = 0; k < 2; ++k) {
+        const HostPoly& hp = *pol[k];
+        std::vector<std::string> Sr(G, imm(hp.c0)), Si(G, imm(hp.c0i)), Ar(G, imm(0.0)), Ai(G, imm(0.0));
+        int si = 0;
+        for (unsigned char code : hp.ops) {
+            const int j = (code - SEC_BASE) / kSecKinds, kind = (code - SEC_BASE) % kSecKinds;
+            std::string cr, ci, c2r, c2i;
+            if (kind == SEC_SL || kind == SEC_AL || kind == SEC_ALI) {
+                cr = imm(hp.slots[4 * si]); ci = imm(hp.slots[4 * si + 1]); c2r = imm(hp.slots[4 * si + 2]); c2i = imm(hp.slots[4 * si + 3]);
+                ++si;
+            }
+            for (int q = 0; q < G; ++q) {
+                const std::string X = x(q, j);
+                switch (kind) {
+                    case SEC_SC: Sr[q] = op3("fma.rn.f64", Ar[q], X, Sr[q]); Si[q] = op3("fma.rn.f64", Ai[q], X, Si[q]); break;
+                    case SEC_SL: Sr[q] = op3("fma.rn.f64", cr, X, Sr[q]); Si[q] = op3("fma.rn.f64", ci, X, Si[q]); break;
+                    case SEC_AL: Ar[q] = op3("fma.rn.f64", cr, X, Ar[q]); Ai[q] = op3("fma.rn.f64", ci, X, Ai[q]); break;
+                    case SEC_ALI: Ar[q] = op3("fma.rn.f64", cr, X, c2r); Ai[q] = op3("fma.rn.f64", ci, X, c2i); break;
+                    default: Ar[q] = mul(Ar[q], X); Ai[q] = mul(Ai[q], X); break;
+                }
+            }
+        }
+        vr[k] = Sr; vi[k] = Si;
+    }
+    auto in_register = [&](const std::string& v) {           // a polynomial without steps is a constant: through a register
+        if (v[0] != '0') return v;
+        const std::string t = fresh();
+        out.line("mov.f64 %s, %s;", t.c_str(), v.c_str());
+        return t;
+    };
+    for (int q = 0; q < G; ++q) {
+        const std::string Ur = in_register(vr[0][q]), Ui = in_register(vi[0][q]), Fr = in_register(vr[1][q]), Fi = in_register(vi[1][q]);
+        std::string w = W(q);
+        for (int j = 0; j < d; ++j)
+            for (int e = 0; e < hs.nu[j]; ++e) w = mul(w, x(q, j));
+        std::string nr = w, ni = imm(0.0);
+        for (int e = 0; e < hs.a; ++e) {
+            if (e == 0) { nr = mul(w, Ur); ni = mul(w, Ui); continue; }
+            const std::string t = op3("fma.rn.f64", nr, Ur, neg(mul(ni, Ui)));
+            ni = op3("fma.rn.f64", nr, Ui, mul(ni, Ur));
+            nr = t;
+        }
+        std::string dr = imm(1.0), di = imm(0.0);
+        for (int e = 0; e < hs.b; ++e) {
+            if (e == 0) { dr = Fr; di = Fi; continue; }
+            const std::string t = op3("fma.rn.f64", dr, Fr, neg(mul(di, Fi)));
+            di = op3("fma.rn.f64", dr, Fi, mul(di, Fr));
+            dr = t;
+        }
+        const std::string* vals[8] = {&nr, &ni, &dr, &di, &Fr, &Fi, &Ur, &Ui};
+        for (int k = 0; k < 8; ++k) out.line("mov.f64 %s, %s;", outp(k, q), vals[k]->c_str());
     }
     return nt;
 }
@@ -374,6 +463,7 @@ const std::vector<Loaded>* loaded_on_current_device(qmc_sector_module* mod) {
 int spec_problem_count(const qmc_sector_module* mod) { return (int)mod->problems.size(); }
 const SpecProblem* spec_problems(const qmc_sector_module* mod) { return mod->problems.data(); }
 int spec_kernel_dp(const qmc_sector_module* mod, int kernel) { return kSlotKinds[mod->kernels[kernel].kind].dp; }
+int spec_kernel_threads(const qmc_sector_module* mod, int kernel) { return kSlotKinds[mod->kernels[kernel].kind].threads; }
 
 int spec_occupancy(qmc_sector_module* mod, int kernel) {
     const std::vector<Loaded>* l = loaded_on_current_device(mod);
@@ -407,17 +497,18 @@ int qmc_sector_module_create(int count, const qmc_problem* problems, int sectors
     qmc_sector_module* mod = new qmc_sector_module;
     mod->problems.resize(count);
     std::vector<HostSector> sectors(count);
-    std::vector<int> by_kind[4];
+    std::vector<int> by_kind[kSlotKindCount];
     for (int i = 0; i < count; ++i) {
         const qmc_problem& p = problems[i];
         SpecProblem& sp = mod->problems[i];
         sp.family = p.family; sp.dim = p.dim; sp.n_params = p.n_params; sp.kernel = -1; sp.kase = 0;
-        if (p.family != QMC_FAMILY_SECTOR || !p.params || p.dim < 1 || p.dim > QMC_MAX_SECTOR_DIM) continue;
-        const int kind = slot_kind_of(sector_dim_slots(p.dim));
-        if (kind < 0 || !compile_sector_host(p.params, p.n_params, p.dim, &sectors[i])) continue;   // the interpreting kernel reports a bad block
+        if (!is_sector_family(p.family) || !p.params || p.dim < 1 || p.dim > QMC_MAX_SECTOR_DIM) continue;
+        const bool cplx = p.family == QMC_FAMILY_SECTOR_COMPLEX;
+        const int kind = slot_kind_of(sector_dim_slots(p.dim), cplx);
+        if (kind < 0 || !compile_sector_host(p.params, p.n_params, p.dim, cplx, &sectors[i])) continue;   // the interpreting kernel reports a bad block
         by_kind[kind].push_back(i);
     }
-    for (int kind = 0; kind < 4; ++kind)
+    for (int kind = 0; kind < kSlotKindCount; ++kind)
         for (size_t b = 0; b < by_kind[kind].size(); b += (size_t)sectors_per_kernel) {
             Kernel k;
             k.kind = kind;
@@ -440,7 +531,8 @@ int qmc_sector_module_create(int count, const qmc_problem* problems, int sectors
             int max_t = 0;
             for (size_t c = 0; c < k.problems.size(); ++c) {
                 code.line("QMC_CASE_%zu:", c);
-                max_t = std::max(max_t, emit_case(sectors[k.problems[c]], problems[k.problems[c]].dim, sk, et.operands, code));
+                max_t = std::max(max_t, sk.cplx ? emit_case_complex(sectors[k.problems[c]], problems[k.problems[c]].dim, sk, et.operands, code)
+                                                : emit_case(sectors[k.problems[c]], problems[k.problems[c]].dim, sk, et.operands, code));
                 code.line("bra.uni QMC_SITE_DONE;");
             }
             std::string ptx;
@@ -449,7 +541,7 @@ int qmc_sector_module_create(int count, const qmc_problem* problems, int sectors
             ptx += et.before;
             ptx += "{\n.reg .f64 t<" + std::to_string(max_t + 1) + ">;\nqmc_cases: .branchtargets ";
             for (size_t c = 0; c < k.problems.size(); ++c) ptx += (c ? ", QMC_CASE_" : "QMC_CASE_") + std::to_string(c);
-            ptx += ";\nbrx.idx.uni " + et.operands[et.operands.size() - 2] + ", qmc_cases;\n";
+            ptx += ";\nbrx.idx.uni " + et.operands[et.operands.size() - (sk.cplx ? 1 : 2)] + ", qmc_cases;\n";
             ptx += code.s;
             ptx += "QMC_SITE_DONE:\n}";
             ptx += et.after;

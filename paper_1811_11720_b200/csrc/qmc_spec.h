@@ -18,6 +18,7 @@ struct SpecProblem {              // one record per problem the module was built
 int spec_problem_count(const qmc_sector_module* mod);
 const SpecProblem* spec_problems(const qmc_sector_module* mod);
 int spec_kernel_dp(const qmc_sector_module* mod, int kernel);
+int spec_kernel_threads(const qmc_sector_module* mod, int kernel);
 // both load the module on the current device on first use; occupancy <= 0 and a launch error are CUDA failures whose text is
 // left with report_cuda_error
 int spec_occupancy(qmc_sector_module* mod, int kernel);

@@ -42,7 +42,42 @@ template <int DP, int G, int NT> struct SectorEvalSpec {
     }
 };
 
-template <int DP, int G, int NT> __device__ __forceinline__ void spec_kernel_body(const FusedLaunch& L) {
+// complex sector family (reading C-16): the site returns n = W prod x^nu U^a, d = F^b and the values of F, U; the log factor
+// and the division are CSectorEval's
+template <int DP, int G, int NT> struct CSectorEvalSpec {
+    static constexpr int NC = 2;
+    typedef unsigned Extra;
+    static __device__ __forceinline__ void eval(const typename Res<false>::T (&r)[DP], const SmemCtx<DP, G, NT>&, const unsigned& exbase,
+                                                const EvalCtx& cx, double (&acc)[G][2]) {
+        double x[G][DP], W[G];
+        sector_coords<DP, G, false, TR_KOR3, 0>(r, cx, x, W);
+        const unsigned sel = (unsigned)(lds_u64(exbase + SectorOff::logp) >> 32);
+        double nr[G], ni[G], dr[G], di[G], Fr[G], Fi[G], Ur[G], Ui[G];
+        csector_poly_site<DP, G>(x, W, sel, nr, ni, dr, di, Fr, Fi, Ur, Ui);
+        const int lp = (int)(unsigned)lds_u64(exbase + SectorOff::logp);
+        if (lp) {                                             // (lu Log U + lf Log F)^p, principal branch: a cold, warp-uniform branch
+            const double lu = lds_f64(exbase + SectorOff::lg), lf = lds_f64(exbase + SectorOff::lg + 8u);
+#pragma unroll 1
+            for (int q = 0; q < G; ++q) {
+                const double Lr = __fma_rn(lu, 0.5 * log(__fma_rn(Ur[q], Ur[q], Ui[q] * Ui[q])), lf * (0.5 * log(__fma_rn(Fr[q], Fr[q], Fi[q] * Fi[q]))));
+                const double Li = __fma_rn(lu, atan2(Ui[q], Ur[q]), lf * atan2(Fi[q], Fr[q]));
+                double pr = Lr, pi = Li;
+                for (int e = 1; e < lp; ++e) { const double t = pr * Lr - pi * Li; pi = pr * Li + pi * Lr; pr = t; }
+                const double t = nr[q] * pr - ni[q] * pi;
+                ni[q] = nr[q] * pi + ni[q] * pr;
+                nr[q] = t;
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < G; ++q) {                         // n / d = n conj(d) / |d|^2
+            const double inv = rcp_nr(__fma_rn(dr[q], dr[q], di[q] * di[q]));
+            acc[q][0] = __fma_rn(__fma_rn(nr[q], dr[q], ni[q] * di[q]), inv, acc[q][0]);
+            acc[q][1] = __fma_rn(__fma_rn(ni[q], dr[q], -(nr[q] * di[q])), inv, acc[q][1]);
+        }
+    }
+};
+
+template <int DP, int G, int NT, bool CPLX> __device__ __forceinline__ void spec_kernel_body(const FusedLaunch& L) {
     const DevAux* __restrict__ aux = L.aux;
     double* __restrict__ partials = L.partials;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -61,14 +96,21 @@ template <int DP, int G, int NT> __device__ __forceinline__ void spec_kernel_bod
             }
             __syncthreads();
         }
-        run_tile<SectorEvalSpec<DP, G, NT>, DP, G, false, NT>(sm, sbase, exbase, tile_local, changed, partials);
+        if constexpr (CPLX) run_tile<CSectorEvalSpec<DP, G, NT>, DP, G, false, NT>(sm, sbase, exbase, tile_local, changed, partials);
+        else run_tile<SectorEvalSpec<DP, G, NT>, DP, G, false, NT>(sm, sbase, exbase, tile_local, changed, partials);
     }
 }
 
 }  // namespace qmc
 
-// one entry point per dimension-slot count; the names are looked up in the assembled module
-extern "C" __global__ void __launch_bounds__(384, 1) qmc_spec_dp4(const __grid_constant__ qmc::FusedLaunch L) { qmc::spec_kernel_body<4, 8, 384>(L); }
-extern "C" __global__ void __launch_bounds__(384, 1) qmc_spec_dp6(const __grid_constant__ qmc::FusedLaunch L) { qmc::spec_kernel_body<6, 8, 384>(L); }
-extern "C" __global__ void __launch_bounds__(256, 1) qmc_spec_dp8(const __grid_constant__ qmc::FusedLaunch L) { qmc::spec_kernel_body<8, 8, 256>(L); }
-extern "C" __global__ void __launch_bounds__(256, 1) qmc_spec_dp16(const __grid_constant__ qmc::FusedLaunch L) { qmc::spec_kernel_body<16, 4, 256>(L); }
+// one entry point per family and dimension-slot count; the names are looked up in the assembled module
+#define QMC_SPEC_ENTRY(NAME, DP, G, NT, CPLX) \
+    extern "C" __global__ void __launch_bounds__(NT, 1) NAME(const __grid_constant__ qmc::FusedLaunch L) { qmc::spec_kernel_body<DP, G, NT, CPLX>(L); }
+QMC_SPEC_ENTRY(qmc_spec_dp4, 4, 8, 384, false)
+QMC_SPEC_ENTRY(qmc_spec_dp6, 6, 8, 384, false)
+QMC_SPEC_ENTRY(qmc_spec_dp8, 8, 8, 256, false)
+QMC_SPEC_ENTRY(qmc_spec_dp16, 16, 4, 256, false)
+QMC_SPEC_ENTRY(qmc_cspec_dp4, 4, 4, 384, true)
+QMC_SPEC_ENTRY(qmc_cspec_dp6, 6, 4, 384, true)
+QMC_SPEC_ENTRY(qmc_cspec_dp8, 8, 4, 384, true)
+QMC_SPEC_ENTRY(qmc_cspec_dp16, 16, 2, 384, true)

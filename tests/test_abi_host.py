@@ -386,7 +386,7 @@ def _one_monomial_block(d):
 
 
 def test_sector_module_skips_what_it_cannot_compile(L):
-    """other families, the complex sector family and blocks the validation rejects stay on the default kernels"""
+    """other families and blocks the validation rejects stay on the default kernels; complex sectors get kernels of their own"""
     good = _sector_problem(6, 900)
     bad = _sector_problem(6, 901)
     prm = bad["params"].copy()
@@ -395,7 +395,8 @@ def test_sector_module_skips_what_it_cannot_compile(L):
     osc = synth.config(0)[0]
     cplx = _sector_problem(5, 902, family=8)
     mod = binding.SectorModule([good, bad, osc, cplx, good])
-    assert mod.info["specialised"] == 2 and mod.info["kernels"] == 1
+    assert mod.info["specialised"] == 3 and mod.info["kernels"] == 2
+    assert "qmc_cspec_dp6" in mod.image(1)[1] and "qmc_spec_dp6" in mod.image(0)[1]
     # argument checks
     out = C.c_void_p()
     arr = (binding.qmc_problem * 1)()

@@ -850,9 +850,26 @@ def test_module_returns_the_bits_of_the_interpreting_kernel(d):
         assert a[0][0].tobytes() == b[0][0].tobytes() and a[1].tobytes() == b[1].tobytes() and a[2].tobytes() == b[2].tobytes()
 
 
+@pytest.mark.parametrize("d", [1, 3, 4, 5, 6, 8, 9, 16])
+def test_module_complex_sectors(d):
+    """family 8 (reading C-16) through specialised kernels: oracle parity on every slot kind, with log factors (principal branch),
+    and the bits of the interpreting kernel where the arithmetic is written with explicit roundings (no log factor)"""
+    probs = [make(8, d, n, 5, K + 3, 9970 + 5 * d + i) for i, n in enumerate([127, 1021, 8191])]
+    rng = synth.MT19937_64(9990 + d)
+    logp = synth.problem(8, synth.sector_complex(rng, d, log_block=True), 4099, synth.korobov_form_vector(4099, d, 1 + 4099 // 3),
+                         synth.draw_shifts(rng, 4, d), K + 3, name=f"csector.log.d{d}")
+    mod = binding.SectorModule(probs + [logp])
+    assert mod.info["specialised"] == 4 and mod.info["kernels"] == 1
+    check_against_oracle(probs + [logp], module=mod)
+    one = make(8, d, 65537, 6, K + 3, 9980 + d)
+    a = run_gpu([one])
+    b = run_gpu([one], module=binding.SectorModule([one]))
+    assert a[0][0].tobytes() == b[0][0].tobytes() and a[1].tobytes() == b[1].tobytes() and a[2].tobytes() == b[2].tobytes()
+
+
 def test_module_mixed_batch_routes_only_what_it_covers():
-    """closed-form families, complex sectors, other transforms, fit maps and a rejected block stay on the default kernels in the
-    same call; a and b = 0, nu up to 8 and log factors run specialised"""
+    """closed-form families, other transforms, fit maps and a rejected block stay on the default kernels in the same call;
+    a and b = 0, nu up to 8, log factors and complex sectors run specialised"""
     probs = [make(3, 6, 8191, 5, K + 3, 9900), make(0, 5, 4099, 4, K + 3, 9901), make(8, 4, 4099, 4, K + 3, 9902),
              make(3, 6, 8191, 5, BAKER, 9903), make(3, 4, 8191, 5, K + 3, 9904, fit=True), make(3, 6, 8191, 5, K + 2, 9905),
              make_log(6, 8191, 5, K + 3, 9906, pw=3), make_log(8, 4099, 4, K + 3, 9907, pw=4), make(3, 16, 4099, 4, K + 3, 9908)]
@@ -866,7 +883,7 @@ def test_module_mixed_batch_routes_only_what_it_covers():
     prm[4 + 6 + int(prm[2])] = 2.5                           # a fractional exponent in U
     bad = dict(bad, params=prm, name="bad")
     mod = binding.SectorModule(probs + [bad])
-    assert mod.info["specialised"] == 8                      # every real sector but the rejected one (routing is decided per call)
+    assert mod.info["specialised"] == 9                      # every sector but the rejected one (routing is decided per call)
     sms, means, errs = run_gpu(probs + [bad], module=mod)
     assert np.isnan(means[-1, 0]) and np.isnan(errs[-1, 0])
     ref = run_gpu(probs + [bad])
