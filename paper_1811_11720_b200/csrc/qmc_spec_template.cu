@@ -5,7 +5,7 @@
 // is the other route: it is compiled to PTX ONLY (build.py: nvcc -ptx) and embedded in the library as text; at run time
 // qmc_sector_module_create (qmc_spec.cu) replaces the marker line of sector_poly_site with the straight-line code of the
 // sectors of a batch -- coefficients as immediates, exponents unrolled, the Horner form of compile_polynomial -- and
-// assembles the result for sm_100a (nvPTXCompiler).  Everything but the hole is the code of the interpreting kernel: tile
+// assembles the result for sm_100a (nvJitLink).  Everything but the hole is the code of the interpreting kernel: tile
 // queue, lattice points, transform, reductions (qmc_fused.cuh).
 //
 // Only the default tile loop exists here (Korobov-3, no fit map, n < 2^31: the paper's setting for loop integrals);
