@@ -280,7 +280,7 @@ __device__ __forceinline__ double point_coord(double rd, double inv_n, double de
         } else if (TR == TR_KOR3) {
             const double c = centre_c(t);
             const double s = c * c;
-            P = __dmul_rn(P, __fma_rn(-c, c, 0.25));          // u (1-u) = 1/4 - c^2, one rounding (explicit: every kernel that inlines this takes the same form)
+            P = __dmul_rn(P, __dadd_rn(0.25, -s));            // u (1-u) = 1/4 - c^2 (explicit roundings: every kernel that inlines this takes the same form)
             double g = __fma_rn(-20.0, s, 21.0);              // g_3(s) = 35/16 - 35/4 s + 21 s^2 - 20 s^3
             g = __fma_rn(g, s, -8.75);
             g = __fma_rn(g, s, 2.1875);
