@@ -170,7 +170,8 @@ size_t qmc_workspace_bytes_opts(int count, const qmc_problem* problems /*HOST*/,
 
 /* Synchronous batched call, HOST pointers everywhere (problems[i].params / z / shifts / fit_coeffs included): full value
  * validation of every problem, ONE host-to-device copy of all inputs from the calling thread's pinned staging block, the
- * batched hot path on the default stream of the current device, one device-to-host copy of the results, synchronise.
+ * batched hot path on the default stream of the current device -- its last kernel writes the results into the same (mapped)
+ * staging block -- synchronise, copy out of the staging block.
  *   out_means, out_errs : HOST, count*2 doubles [p*2 + c]
  *   out_shift_means     : HOST or NULL, count * 2*max_m doubles [p*(2 max_m) + s*ncomp + c], max_m = largest m of the batch
  * Returns QMC_ERR_NONFINITE (results still written) if a result is NaN/Inf. */

@@ -379,7 +379,7 @@ int arena_reserve(size_t pinned_bytes, size_t device_bytes) {
     if (pinned_bytes > t.pinned_bytes) {
         if (t.pinned) { cudaFreeHost(t.pinned); t.pinned = nullptr; t.pinned_bytes = 0; }
         const size_t want = std::max<size_t>(pinned_bytes + pinned_bytes / 2, 1 << 16);
-        cudaError_t e = cudaMallocHost(reinterpret_cast<void**>(&t.pinned), want);
+        cudaError_t e = cudaHostAlloc(reinterpret_cast<void**>(&t.pinned), want, cudaHostAllocMapped | cudaHostAllocPortable);   // the results are written here by the device
         if (e != cudaSuccess) return cuda_fail(e, "cudaMallocHost (staging arena)");
         t.pinned_bytes = want;
     }
@@ -707,14 +707,16 @@ int qmc_lattice_integrate_batch_host_module(qmc_sector_module* module, int count
     const int pst = make_plan(count, problems, true, &plan, kDefaultOptions, module);
     if (pst != QMC_OK) return pst;
     const size_t blob_bytes = align_up(plan.off_aux - plan.off_counters, 256);
-    const int ast = arena_reserve(in_bytes + blob_bytes + out_bytes, in_bytes + out_bytes + plan.total + 256);
+    const int ast = arena_reserve(in_bytes + blob_bytes + out_bytes, in_bytes + plan.total + 256);
     if (ast != QMC_OK) return ast;
     char* h_in = g_ts.pinned;                         // [inputs | plan blob | results]
     char* h_blob = h_in + in_bytes;
     char* h_out = h_blob + blob_bytes;
     char* d_in = g_ts.device;
-    double* d_out = reinterpret_cast<double*>(d_in + in_bytes);
-    char* d_ws = reinterpret_cast<char*>(d_out) + out_bytes;
+    // the finalize kernel writes the results (a few KB) straight into the mapped staging block: no device-to-host copy to wait for
+    double* d_out = nullptr;
+    QMC_CUDA(cudaHostGetDevicePointer(reinterpret_cast<void**>(&d_out), h_out, 0));
+    char* d_ws = d_in + in_bytes;
     size_t off = 0;
     for (int i = 0; i < count; ++i) {
         const qmc_problem& p = problems[i];
@@ -737,7 +739,6 @@ int qmc_lattice_integrate_batch_host_module(qmc_sector_module* module, int count
     QMC_CUDA(cudaMemcpyAsync(d_in, h_in, in_bytes, cudaMemcpyHostToDevice, st));
     const int status = run_batch(count, problems, d_means, d_errs, d_sm, d_ws, plan.total, st, kDefaultOptions, h_blob, &plan, module);
     if (status != QMC_OK) { cudaStreamSynchronize(st); return status; }
-    QMC_CUDA(cudaMemcpyAsync(h_out, d_out, out_doubles * 8, cudaMemcpyDeviceToHost, st));
     QMC_CUDA(cudaStreamSynchronize(st));
     const double* r = reinterpret_cast<const double*>(h_out);
     bool finite = true;
