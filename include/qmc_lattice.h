@@ -340,6 +340,25 @@ int qmc_lattice_integrate_batch_module(qmc_sector_module* module, int count, con
                                        double* out_shift_means /*DEVICE or NULL*/, void* workspace /*DEVICE*/,
                                        size_t workspace_bytes, void* cuda_stream);
 
+/* ---- an entry that allocates nothing --------------------------------------------------------------------------------------
+ * For callers that cannot allocate device memory around a call (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid it): qmc_lattice_integrate_batch with the workspace in a device array that is part of the library image,
+ * QMC_STATIC_SCRATCH_BYTES (4 MiB) per GPU that loads the library, held until the process exits.  Arguments, kernels and results
+ * are those of qmc_lattice_integrate_batch (problems HOST structs with DEVICE data pointers, outputs DEVICE, stream-ordered, no
+ * synchronisation); the call itself issues no cudaMalloc / cudaFree / allocating library routine.
+ *   Limit: qmc_workspace_bytes(count, problems) <= qmc_static_scratch_bytes(); a larger batch is rejected with QMC_ERR_WORKSPACE
+ *   before anything is launched, and qmc_last_cuda_error() then says how many bytes the batch needs (configs[4] of the bench
+ *   needs 0.15 MB, the 256-sector batch of configs[3] 1.3 MB).
+ *   Sharing: every call on a device uses the same array, and the array keeps the last call's contents.  Nothing has to be
+ *   cleared by the caller -- a call resets its tile queues itself and writes every partial sum before it reads it -- but two
+ *   calls whose kernels OVERLAP on the GPU (different streams without an ordering between them, or two host threads on one
+ *   device) race on it: order them, or use qmc_lattice_integrate_batch with separate workspaces. */
+#define QMC_STATIC_SCRATCH_BYTES 4194304
+size_t qmc_static_scratch_bytes(void);
+int qmc_lattice_integrate_batch_static(int count, const qmc_problem* problems /*HOST*/, double* out_means /*DEVICE*/,
+                                       double* out_errs /*DEVICE*/, double* out_shift_means /*DEVICE or NULL*/,
+                                       void* cuda_stream);
+
 int qmc_num_components(int family);          /* 1 or 2; <0 on unknown family */
 const char* qmc_status_string(int status);
 const char* qmc_last_cuda_error(void);       /* thread-local text of the last CUDA error ("" if none) */

@@ -24,7 +24,7 @@ EXPORTS = [
     "qmc_release_thread_resources", "qmc_sector_compile", "qmc_lattice_cdf_samples", "qmc_cdf_workspace_bytes",
     "qmc_cdf_sample_count", "qmc_fit_from_cdf", "qmc_sector_module_create", "qmc_sector_module_destroy", "qmc_sector_module_info",
     "qmc_sector_module_image", "qmc_lattice_integrate_batch_module", "qmc_sector_module_workspace_bytes",
-    "qmc_lattice_integrate_batch_host_module",
+    "qmc_lattice_integrate_batch_host_module", "qmc_static_scratch_bytes", "qmc_lattice_integrate_batch_static",
 ]
 
 QMC_OK = 0
@@ -88,6 +88,8 @@ def lib():
         L.qmc_sector_module_info.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int), dp, C.POINTER(C.c_size_t), C.POINTER(C.c_int)]
         L.qmc_sector_module_image.argtypes = [vp, C.c_int, vp, C.c_size_t, C.POINTER(C.c_size_t), C.c_char_p, C.c_size_t]
         L.qmc_lattice_integrate_batch_host_module.argtypes = [vp, C.c_int, pp, dp, dp, dp]
+        L.qmc_static_scratch_bytes.restype = C.c_size_t
+        L.qmc_lattice_integrate_batch_static.argtypes = [C.c_int, pp, vp, vp, vp, vp]
         L.qmc_sector_module_workspace_bytes.argtypes = [vp, C.c_int, pp]
         L.qmc_sector_module_workspace_bytes.restype = C.c_size_t
         L.qmc_lattice_integrate_batch_module.argtypes = [vp, C.c_int, pp, vp, vp, vp, vp, C.c_size_t, vp]
@@ -389,6 +391,14 @@ class DeviceBatch:
         _check(lib().qmc_lattice_integrate_batch_opts(self.count, self.arr, self.means.data_ptr(), self.errs.data_ptr(),
                                                       self.shift_means.data_ptr(), self.ws_ptr, self.ws_bytes, s, C.byref(self.opts)),
                "qmc_lattice_integrate_batch")
+        return int(lib().qmc_last_launch_count())
+
+    def integrate_static(self, stream=None):
+        """qmc_lattice_integrate_batch_static: the same call with the library's static scratch array as workspace (nothing is
+        allocated; batches whose workspace exceeds qmc_static_scratch_bytes() are rejected); returns launch count."""
+        s = self.torch.cuda.current_stream(self.device).cuda_stream if stream is None else stream
+        _check(lib().qmc_lattice_integrate_batch_static(self.count, self.arr, self.means.data_ptr(), self.errs.data_ptr(),
+                                                        self.shift_means.data_ptr(), s), "qmc_lattice_integrate_batch_static")
         return int(lib().qmc_last_launch_count())
 
     def capture(self):
