@@ -266,6 +266,31 @@ int qmc_integrate(int family, const double* params /*HOST*/, int n_params, int d
                   uint64_t min_n, int min_m, int max_m, double epsrel, double epsabs, uint64_t maxeval, int errormode,
                   qmc_result* out /*HOST*/);
 
+/* The same iteration for MANY integrands at once (the batched counterpart of qmc_integrate; all pointers HOST, synchronous, default
+ * stream of the current device).  Every integrand follows qmc_integrate's rules on its own -- first lattice, enlargement by the
+ * error ratio, shift extension at the end of the ladder, maxeval per integrand -- but the lattice evaluations of one round, each
+ * integrand on its own current lattice and shift range, share ONE batched launch of the fused kernels, and a round costs one
+ * device-to-host copy and one synchronisation for all integrands.  With `module` (built from these integrands in this order:
+ * qmc_sector_module_create reads family, dim, n_params, params of a qmc_problem) the sectors run as compiled code; NULL = the
+ * default kernels.
+ *   integrands[p]    : family, dim, transform, n_params, params (HOST), fit_coeffs (HOST [dim][6] or NULL)
+ *   ladder_z, shifts : [n_lattices][ladder_dim] and [max_m][ladder_dim], ladder_dim >= every dim; an integrand of dimension d uses
+ *                      the first d components of each (generating vectors built component by component are nested this way)
+ *   out[p], out_status[p] : the result qmc_integrate would return for integrand p and its status (QMC_OK, QMC_ERR_MAXEVAL,
+ *                      QMC_ERR_NONFINITE)
+ * Returns QMC_OK if every integrand met its goal, else QMC_ERR_NONFINITE if one produced a non-finite value, else
+ * QMC_ERR_MAXEVAL; argument and validation errors (nothing launched, out untouched) as qmc_integrate. */
+typedef struct {
+    int family, dim, transform, n_params;
+    const double* params;      /* HOST */
+    const double* fit_coeffs;  /* HOST [dim][6] or NULL */
+} qmc_integrand;
+typedef struct qmc_sector_module qmc_sector_module;
+int qmc_integrate_batch(int count, const qmc_integrand* integrands /*HOST*/, qmc_sector_module* module /*or NULL*/, int n_lattices,
+                        const uint64_t* ladder_n /*HOST*/, const uint64_t* ladder_z /*HOST*/, int ladder_dim,
+                        const double* shifts /*HOST*/, uint64_t min_n, int min_m, int max_m, double epsrel, double epsabs,
+                        uint64_t maxeval, int errormode, qmc_result* out /*HOST [count]*/, int* out_status /*HOST [count]*/);
+
 /* Measurement helper: runs a DFMA-chain kernel (8 independent chains per thread, full occupancy)
  * for `iters` iterations on `cuda_stream`, synchronises, and returns the sustained thread-level
  * FP64 instruction rate in instructions/second through *out_rate (HOST) and the kernel time in ms
@@ -318,7 +343,6 @@ int qmc_sector_compile(const double* params /*HOST*/, int n_params, int dim, uns
  * built from, in its order (count / family / dim / n_params are checked: QMC_ERR_N / QMC_ERR_PARAMS; the VALUES of params
  * are the caller's promise -- polynomials are read from the module, nu / a / b / log factors too).  The first launch on a
  * device loads the images there (a synchronous driver call). */
-typedef struct qmc_sector_module qmc_sector_module;
 int qmc_sector_module_create(int count, const qmc_problem* problems /*HOST, HOST params*/, int sectors_per_kernel,
                              qmc_sector_module** out /*HOST*/);
 void qmc_sector_module_destroy(qmc_sector_module* module);

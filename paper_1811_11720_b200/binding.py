@@ -25,6 +25,7 @@ EXPORTS = [
     "qmc_cdf_sample_count", "qmc_fit_from_cdf", "qmc_sector_module_create", "qmc_sector_module_destroy", "qmc_sector_module_info",
     "qmc_sector_module_image", "qmc_lattice_integrate_batch_module", "qmc_sector_module_workspace_bytes",
     "qmc_lattice_integrate_batch_host_module", "qmc_static_scratch_bytes", "qmc_lattice_integrate_batch_static",
+    "qmc_integrate_batch",
 ]
 
 QMC_OK = 0
@@ -50,6 +51,11 @@ class qmc_problem(C.Structure):
 
 class qmc_plan_options(C.Structure):
     _fields_ = [("tiles_target", C.c_int), ("force_wide", C.c_int)]
+
+
+class qmc_integrand(C.Structure):
+    _fields_ = [("family", C.c_int), ("dim", C.c_int), ("transform", C.c_int), ("n_params", C.c_int), ("params", C.c_void_p),
+                ("fit_coeffs", C.c_void_p)]
 
 
 class qmc_result(C.Structure):
@@ -88,6 +94,8 @@ def lib():
         L.qmc_sector_module_info.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int), dp, C.POINTER(C.c_size_t), C.POINTER(C.c_int)]
         L.qmc_sector_module_image.argtypes = [vp, C.c_int, vp, C.c_size_t, C.POINTER(C.c_size_t), C.c_char_p, C.c_size_t]
         L.qmc_lattice_integrate_batch_host_module.argtypes = [vp, C.c_int, pp, dp, dp, dp]
+        L.qmc_integrate_batch.argtypes = [C.c_int, C.POINTER(qmc_integrand), vp, C.c_int, up, up, C.c_int, dp, C.c_uint64, C.c_int, C.c_int,
+                                          C.c_double, C.c_double, C.c_uint64, C.c_int, C.POINTER(qmc_result), C.POINTER(C.c_int)]
         L.qmc_static_scratch_bytes.restype = C.c_size_t
         L.qmc_lattice_integrate_batch_static.argtypes = [C.c_int, pp, vp, vp, vp, vp]
         L.qmc_sector_module_workspace_bytes.argtypes = [vp, C.c_int, pp]
@@ -293,6 +301,38 @@ def qmc_integrate(family, params, dim, transform, ladder_n, ladder_z, shifts, mi
                                     int(maxeval), int(errormode), C.byref(res)), "qmc_integrate", allow=(QMC_ERR_MAXEVAL,))
     return {"integral": np.array(res.integral[:nc]), "error": np.array(res.error[:nc]), "n": int(res.n), "m": int(res.m),
             "iterations": int(res.iterations), "evaluations": int(res.evaluations)}, st
+
+
+def qmc_integrate_batch(integrands, ladder_n, ladder_z, shifts, module=None, min_n=8191, min_m=32, epsrel=0.01, epsabs=1e-7,
+                        maxeval=1000000, errormode=0):
+    """qmc_integrate for many integrands at once (dicts with family, params, dim, transform[, fit_coeffs]); the lattice evaluations
+    of a round share one batched launch -> (list of result dicts, list of statuses, overall status)."""
+    count = len(integrands)
+    arr = (qmc_integrand * count)()
+    keep = []
+    for i, g in enumerate(integrands):
+        params, fit = _f64(g["params"]), _f64(g.get("fit_coeffs"))
+        keep += [params, fit]
+        arr[i] = qmc_integrand(int(g["family"]), int(g["dim"]), int(g["transform"]), len(params), params.ctypes.data,
+                               None if fit is None else fit.ctypes.data)
+    ln = np.ascontiguousarray(ladder_n, dtype=np.uint64)
+    lz = np.ascontiguousarray(ladder_z, dtype=np.uint64)
+    shifts = _f64(shifts)
+    ladder_dim = int(shifts.shape[1])
+    assert lz.shape == (len(ln), ladder_dim)
+    res = (qmc_result * count)()
+    sts = (C.c_int * count)()
+    st = _check(lib().qmc_integrate_batch(count, arr, None if module is None else module.handle, len(ln), _u(ln), _u(lz), ladder_dim,
+                                          _d(shifts), int(min_n), int(min_m), int(shifts.shape[0]), float(epsrel), float(epsabs),
+                                          int(maxeval), int(errormode), res, sts), "qmc_integrate_batch",
+                allow=(QMC_ERR_MAXEVAL, QMC_ERR_NONFINITE))
+    out = []
+    for i, g in enumerate(integrands):
+        nc = max(qmc_num_components(g["family"]), 1)
+        r = res[i]
+        out.append({"integral": np.array(r.integral[:nc]), "error": np.array(r.error[:nc]), "n": int(r.n), "m": int(r.m),
+                    "iterations": int(r.iterations), "evaluations": int(r.evaluations)})
+    return out, [int(v) for v in sts], st
 
 
 def qmc_validate_problem_host(p: dict) -> int:

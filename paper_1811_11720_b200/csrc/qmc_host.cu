@@ -161,13 +161,19 @@ struct Plan {
 const qmc_plan_options kDefaultOptions = {0, 0};
 
 int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan* plan, const qmc_plan_options& opt = kDefaultOptions,
-              const qmc_sector_module* module = nullptr) {
+              const qmc_sector_module* module = nullptr, const int* module_index = nullptr) {
     if (count < 1 || !problems) return count < 1 ? QMC_ERR_N : QMC_ERR_NULL;
-    if (module) {                                        // the batch the module was built from, in its order
-        if (spec_problem_count(module) != count) return QMC_ERR_N;
+    // the batch the module was built from, in its order -- or (internal callers: the batched iteration) any selection of its
+    // problems, problems[i] being problem module_index[i] of the module's batch
+    auto in_module = [&](int i) { return module_index ? module_index[i] : i; };
+    if (module) {
+        if (!module_index && spec_problem_count(module) != count) return QMC_ERR_N;
         const SpecProblem* sp = spec_problems(module);
-        for (int i = 0; i < count; ++i)
-            if (sp[i].family != problems[i].family || sp[i].dim != problems[i].dim || sp[i].n_params != problems[i].n_params) return QMC_ERR_PARAMS;
+        for (int i = 0; i < count; ++i) {
+            const int k = in_module(i);
+            if (k < 0 || k >= spec_problem_count(module)) return QMC_ERR_N;
+            if (sp[k].family != problems[i].family || sp[k].dim != problems[i].dim || sp[k].n_params != problems[i].n_params) return QMC_ERR_PARAMS;
+        }
     }
     plan->dev.resize(count);
     long long means_off = 0;
@@ -230,10 +236,10 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
         const int dp = dim_slots(d.family, d.dim, wide);
         // a specialised kernel holds the sector's code and serves the default tile loop only (Korobov-3, no fit map, narrow residues)
         int kfam = kernel_family(d.family), spec_kernel = -1;
-        if (module && is_sector_family(d.family) && !wide && d.tr_kind == TR_KOR3 && !d.has_fit && spec_problems(module)[i].kernel >= 0) {
+        if (module && is_sector_family(d.family) && !wide && d.tr_kind == TR_KOR3 && !d.has_fit && spec_problems(module)[in_module(i)].kernel >= 0) {
             kfam = kKernelFamilySpec;
-            spec_kernel = spec_problems(module)[i].kernel;
-            plan->dev[i].spec_case = spec_problems(module)[i].kase;
+            spec_kernel = spec_problems(module)[in_module(i)].kernel;
+            plan->dev[i].spec_case = spec_problems(module)[in_module(i)].kase;
         }
         Variant* v = nullptr;
         for (auto& c : plan->variants)
@@ -395,7 +401,7 @@ int arena_reserve(size_t pinned_bytes, size_t device_bytes) {
 
 int run_batch(int count, const qmc_problem* problems, double* out_means, double* out_errs, double* out_shift_means,
               void* workspace, size_t workspace_bytes, cudaStream_t st, const qmc_plan_options& opt = kDefaultOptions,
-              char* pinned_blob = nullptr, Plan* prebuilt = nullptr, qmc_sector_module* module = nullptr) {
+              char* pinned_blob = nullptr, Plan* prebuilt = nullptr, qmc_sector_module* module = nullptr, int sm_stride = 0) {
     g_ts.last_launches = 0;
     if (!out_means || !out_errs) return QMC_ERR_NULL;
     Plan local_plan;
@@ -498,11 +504,35 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
         ++g_ts.last_launches;
     }
     if (g_ts.profile) { QMC_CUDA(cudaEventRecord(g_ts.ev1, st)); g_ts.ev_valid = true; }
-    QMC_CUDA(launch_finalize(count, st, base, dmeans, out_means, out_errs, out_shift_means, 2 * plan.max_m));
+    QMC_CUDA(launch_finalize(count, st, base, dmeans, out_means, out_errs, out_shift_means, sm_stride > 0 ? sm_stride : 2 * plan.max_m));
     ++g_ts.last_launches;
     return QMC_OK;
 }
 
+}  // namespace
+
+// Internal (qmc_kernels.h; the batched iteration of qmc_adaptive.cu): a batch call whose problems are a selection of a module's
+// batch (module_index, may be null without a module) and whose results land in caller-chosen rows: problem i writes
+// out_means / out_errs [out_row[i] * 2 + c] and out_shift_means [out_row[i] * sm_stride + s * ncomp + c].
+size_t routed_workspace_bytes(int count, const qmc_problem* problems, const qmc_sector_module* module, const int* module_index) {
+    Plan plan;
+    if (make_plan(count, problems, false, &plan, kDefaultOptions, module, module_index) != QMC_OK) return 0;
+    return plan.total;
+}
+int run_batch_routed(int count, const qmc_problem* problems, double* out_means, double* out_errs, double* out_shift_means,
+                     void* workspace, size_t workspace_bytes, cudaStream_t st, qmc_sector_module* module, const int* module_index,
+                     const int* out_row, int sm_stride) {
+    Plan plan;
+    const int pst = make_plan(count, problems, true, &plan, kDefaultOptions, module, module_index);
+    if (pst != QMC_OK) return pst;
+    int max_m = 0;
+    for (int i = 0; i < count; ++i) { plan.dev[i].out_index = out_row[i]; max_m = std::max(max_m, plan.dev[i].m * plan.dev[i].ncomp); }
+    if (sm_stride < max_m) return QMC_ERR_M;
+    return run_batch(count, problems, out_means, out_errs, out_shift_means, workspace, workspace_bytes, st, kDefaultOptions, nullptr, &plan,
+                     module, sm_stride);
+}
+
+namespace {
 // ---- full value validation of host-resident data --------------------------------------------------
 unsigned long long gcd_u64(unsigned long long a, unsigned long long b) {
     while (b) { const unsigned long long t = a % b; a = b; b = t; }

@@ -20,6 +20,12 @@ struct PointsArgs {
 // records a CUDA error for qmc_last_cuda_error() and returns QMC_ERR_CUDA (qmc_host.cu)
 int report_cuda_error(cudaError_t e, const char* where);
 
+// a batch call for internal callers (qmc_host.cu): problems may be a selection of a module's batch, results go to chosen rows
+size_t routed_workspace_bytes(int count, const qmc_problem* problems, const qmc_sector_module* module, const int* module_index);
+int run_batch_routed(int count, const qmc_problem* problems, double* out_means, double* out_errs, double* out_shift_means,
+                     void* workspace, size_t workspace_bytes, cudaStream_t st, qmc_sector_module* module, const int* module_index,
+                     const int* out_row, int sm_stride);
+
 cudaError_t launch_prepare(int count, cudaStream_t st, const DevProblem* probs, DevAux* aux, unsigned long long* prog_area);
 cudaError_t launch_finalize(int count, cudaStream_t st, const FusedLaunch& a, double* means_ws, double* out_means, double* out_errs,
                             double* out_shift_means, int stride);

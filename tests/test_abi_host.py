@@ -431,3 +431,37 @@ def test_sector_module_is_bound_to_its_batch(L):
     # another lattice, other shifts, another transform: the same module (the transform only changes the routing)
     relattice = [dict(_sector_problem(6, 950 + i, n=65537, m=9), transform=synth.TRANSFORM_BAKER) for i in range(3)]
     assert ws(relattice)[0] > 0
+
+
+def test_integrate_batch_rejects_before_touching_the_device():
+    """qmc_integrate_batch validates every integrand on every lattice on the host; these calls return before any CUDA call"""
+    rng = synth.MT19937_64(31)
+    good = dict(family=3, dim=4, transform=synth.TRANSFORM_KOROBOV + 3, params=synth.sector(rng, 4))
+    ln, lz = synth.ladder(6, 4093)
+    shifts = synth.draw_shifts(rng, 8, 6)
+    kw = dict(min_n=1000, min_m=4, epsrel=1e-6, epsabs=0.0, maxeval=10**6)
+
+    def status(integrands, ln=ln, lz=lz, shifts=shifts, **over):
+        try:
+            binding.qmc_integrate_batch(integrands, ln, lz, shifts, **dict(kw, **over))
+        except binding.QmcError as e:
+            return e.status
+        return 0
+
+    assert status([dict(good, dim=7)]) == -2                           # wider than the ladder
+    assert status([dict(good, family=9)]) == -8
+    assert status([dict(good, transform=77)]) == -7
+    assert status([dict(good, params=good["params"][:-1])]) == -9
+    bad_shift = shifts.copy()
+    bad_shift[2, 3] = -0.25
+    assert status([good], shifts=bad_shift) == -5
+    bad_z = lz.copy()
+    bad_z[1, 2] = 0
+    assert status([good], lz=bad_z) == -4
+    assert status([good], ln=ln[::-1].copy(), lz=lz[::-1].copy()) == -3          # the ladder must ascend
+    assert status([good], min_m=1) == -6
+    assert status([good], epsrel=-1.0) == -9
+    # a shift of a component the integrand does not use is not its problem
+    unused = shifts.copy()
+    unused[2, 5] = 7.0
+    assert status([dict(good, dim=7)], shifts=unused) == -2

@@ -126,3 +126,97 @@ def test_argument_errors():
     with pytest.raises(binding.QmcError) as e:
         binding.qmc_integrate(0, p["params"], 4, K + 3, ln, bad, p["shifts"], min_m=10)
     assert e.value.status == -4
+
+
+# ------------------------------------------------------------------------------------------------
+# qmc_integrate_batch: the same iteration for many integrands, one batched launch per round
+# ------------------------------------------------------------------------------------------------
+def _mixed_integrands():
+    rng = synth.MT19937_64(5151)
+    out = [dict(family=0, dim=4, transform=K + 3, params=synth.genz_osc(rng, 4))]
+    for _ in range(3):
+        out.append(dict(family=3, dim=6, transform=K + 3, params=synth.sector(rng, 6)))
+    out.append(dict(family=8, dim=3, transform=K + 3, params=synth.sector_complex(rng, 3)))
+    out.append(dict(family=2, dim=6, transform=K + 3, params=synth.cexp_poly(rng, 6)))
+    out.append(dict(family=3, dim=5, transform=synth.TRANSFORM_BAKER, params=synth.sector(rng, 5)))
+    out.append(dict(family=1, dim=2, transform=K + 2, params=synth.genz_prodpeak(rng, 2)))
+    return out
+
+
+def _check_batch_against_oracle_and_single(integrands, results, statuses, ln, lz, shifts, **kw):
+    for g, res, st in zip(integrands, results, statuses):
+        d = g["dim"]
+        i = int(np.where(ln == res["n"])[0][0])
+        q = synth.problem(g["family"], g["params"], res["n"], lz[i, :d], shifts[:res["m"], :d], g["transform"], g.get("fit_coeffs"))
+        sm_or, mean_or, err_or = oracle.integrate(q)
+        nc = len(mean_or)
+        scale = np.max(np.abs(sm_or)) if nc == 1 else np.max(np.hypot(sm_or[:, 0], sm_or[:, 1]))
+        assert np.all(np.abs(res["integral"] - mean_or) <= 1e-13 * scale), g
+        assert np.all(np.abs(res["error"] - err_or) <= 1e-12 * err_or + 1e-13 * scale), g
+        # the sequential driver on the same inputs takes the same decisions
+        one, st1 = binding.qmc_integrate(g["family"], g["params"], d, g["transform"], ln, np.ascontiguousarray(lz[:, :d]),
+                                         np.ascontiguousarray(shifts[:, :d]), fit_coeffs=g.get("fit_coeffs"), **kw)
+        assert (one["n"], one["m"], one["iterations"], one["evaluations"], st1) == (res["n"], res["m"], res["iterations"], res["evaluations"], st), g
+        assert np.all(np.abs(res["integral"] - one["integral"]) <= 1e-13 * scale)
+
+
+@pytest.mark.parametrize("with_module", [False, True])
+def test_batch_iteration_mixed_integrands(with_module):
+    """integrands of different families, dimensions and transforms climb the ladder at their own pace in shared launches; with a
+    module the sectors it covers run as compiled code (the others stay on the default kernels in the same launch)"""
+    integrands = _mixed_integrands()
+    ln, lz = synth.ladder(6, 262139)
+    shifts = synth.draw_shifts(synth.MT19937_64(99), 12, 6)
+    module = binding.SectorModule(integrands) if with_module else None
+    if module is not None:
+        assert module.info["specialised"] == 5
+    kw = dict(min_n=1000, min_m=8, epsrel=2e-7, epsabs=0.0, maxeval=10**8)
+    results, statuses, overall = binding.qmc_integrate_batch(integrands, ln, lz, shifts, module=module, **kw)
+    assert len({r["n"] for r in results}) >= 2                 # they do not all stop on the same lattice
+    assert overall == (0 if all(s == 0 for s in statuses) else binding.QMC_ERR_MAXEVAL)
+    _check_batch_against_oracle_and_single(integrands, results, statuses, ln, lz, shifts, **kw)
+
+
+def test_batch_iteration_extends_shifts_and_respects_maxeval():
+    """a one-lattice ladder: every integrand adds shifts until its own goal or the shift supply ends; a tight maxeval stops others"""
+    rng = synth.MT19937_64(6161)
+    integrands = [dict(family=0, dim=4, transform=synth.TRANSFORM_NONE, params=synth.genz_osc(rng, 4)) for _ in range(3)]
+    integrands += [dict(family=3, dim=4, transform=synth.TRANSFORM_BAKER, params=synth.sector(rng, 4)) for _ in range(2)]
+    ln, lz = synth.ladder(4, 1021)
+    shifts = synth.draw_shifts(synth.MT19937_64(98), 64, 4)
+    first, _, _ = binding.qmc_integrate_batch(integrands, ln, lz, shifts[:4], min_n=1, min_m=4, epsrel=0.0, epsabs=0.0, maxeval=1)
+    rel = sorted(float(r["error"][0] / abs(r["integral"][0])) for r in first)
+    kw = dict(min_n=1, min_m=4, epsrel=rel[2] / 2.5, epsabs=0.0, maxeval=10**8)      # the median: some extend, some need less
+    results, statuses, overall = binding.qmc_integrate_batch(integrands, ln, lz, shifts, **kw)
+    assert any(r["m"] > 4 for r in results) and all(r["n"] == 1021 for r in results)
+    assert len({r["m"] for r in results}) >= 2
+    assert all(r["evaluations"] == 1021 * r["m"] for r in results)
+    _check_batch_against_oracle_and_single(integrands, results, statuses, ln, lz, shifts, **kw)
+    kw = dict(min_n=1, min_m=4, epsrel=1e-12, epsabs=0.0, maxeval=20000)
+    results, statuses, overall = binding.qmc_integrate_batch(integrands, ln, lz, shifts, **kw)
+    assert overall == binding.QMC_ERR_MAXEVAL and all(s == binding.QMC_ERR_MAXEVAL for s in statuses)
+    assert all(r["evaluations"] <= 20000 + 1021 * 2 for r in results)
+    _check_batch_against_oracle_and_single(integrands, results, statuses, ln, lz, shifts, **kw)
+
+
+def test_batch_iteration_rejects_bad_arguments():
+    integrands = _mixed_integrands()[:2]
+    ln, lz = synth.ladder(6, 65521)
+    shifts = synth.draw_shifts(synth.MT19937_64(97), 8, 6)
+    kw = dict(min_n=1000, min_m=8, epsrel=1e-6, epsabs=0.0, maxeval=10**7)
+    with pytest.raises(binding.QmcError):                      # an integrand wider than the ladder
+        binding.qmc_integrate_batch([dict(integrands[0], dim=7, params=np.ones(8))], ln, lz, shifts, **kw)
+    with pytest.raises(binding.QmcError):                      # a shift outside [0, 1)
+        bad = shifts.copy()
+        bad[3, 1] = 1.0
+        binding.qmc_integrate_batch(integrands, ln, lz, bad, **kw)
+    with pytest.raises(binding.QmcError):                      # a module built from another batch
+        binding.qmc_integrate_batch(integrands, ln, lz, shifts, module=binding.SectorModule(_mixed_integrands()[2:4]), **kw)
+    # U = 1e308 with a = 2 overflows: that integrand alone ends with QMC_ERR_NONFINITE, the others are unaffected
+    nonfinite = dict(family=3, dim=2, transform=K + 3, params=np.array([2.0, 1.0, 1.0, 1.0, 0.0, 0.0, 1e308, 0.0, 0.0, 1.0, 0.0, 0.0]))
+    alone, st_alone, _ = binding.qmc_integrate_batch(integrands, ln, lz, shifts, **kw)
+    results, statuses, overall = binding.qmc_integrate_batch(integrands + [nonfinite], ln, lz, shifts, **kw)
+    assert statuses[2] == binding.QMC_ERR_NONFINITE and overall == binding.QMC_ERR_NONFINITE and statuses[:2] == st_alone
+    assert results[2]["iterations"] == 1
+    for r, q in zip(results[:2], alone):
+        assert (r["n"], r["m"]) == (q["n"], q["m"]) and np.all(np.abs(r["integral"] - q["integral"]) <= 1e-13 * np.abs(q["integral"]))
