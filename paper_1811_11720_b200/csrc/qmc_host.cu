@@ -272,7 +272,16 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
             const double cost = (double)d.n * d.m * (12.0 * d.dim + 0.5 * d.n_params + 40.0);
             const double want = std::max(1.0, std::floor(target * cost / total_cost));
             unsigned long long tile_len = (unsigned long long)std::ceil((double)d.n / want);
-            tile_len = std::min<unsigned long long>(std::max<unsigned long long>(tile_len, threads), (unsigned long long)kMaxSteps * threads);
+            const unsigned long long max_len = (unsigned long long)kMaxSteps * threads;
+            if (tile_len > max_len && v.plist.size() == 1 && env == 0) {
+                // a lattice too long for `target` tiles of at most kMaxSteps indices per thread: more tiles, in whole waves --
+                // a multiple of the resident CTAs, all of equal length, so that the last wave is as full as the others
+                // (configs[4]: 8436 tiles = 19 waves of 444 instead of 8192 = 18.45)
+                unsigned long long tiles_min = (d.n + max_len - 1) / max_len;
+                tiles_min = (tiles_min + resident - 1) / resident * resident;
+                tile_len = (d.n + tiles_min - 1) / tiles_min;
+            }
+            tile_len = std::min<unsigned long long>(std::max<unsigned long long>(tile_len, threads), max_len);
             const unsigned long long tiles = (d.n + tile_len - 1) / tile_len;
             if (tiles > 0x7fffffffull) return QMC_ERR_N;
             d.tile_len = (long long)tile_len;
