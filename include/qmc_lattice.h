@@ -364,12 +364,34 @@ int qmc_lattice_integrate_batch_module(qmc_sector_module* module, int count, con
                                        double* out_shift_means /*DEVICE or NULL*/, void* workspace /*DEVICE*/,
                                        size_t workspace_bytes, void* cuda_stream);
 
+/* ---- prepared batches ---------------------------------------------------------------------------------------------------
+ * qmc_lattice_integrate_batch plans the batch and uploads the plan on every call (from pageable host memory, which a CUDA graph
+ * capture refuses).  A prepared batch does that ONCE: qmc_batch_create plans, uploads, runs the sector prepare kernel, loads the
+ * kernels (synchronises `cuda_stream` before it returns); qmc_batch_launch is then one 512-byte memset of the tile-queue heads
+ * plus the fused kernels and the finalize kernel -- nothing is read from host memory, nothing is allocated, no synchronisation --
+ * and can be captured in a CUDA graph (with profiling off: qmc_profile_enable(0)).  Same kernels, same tiling, same bits as
+ * qmc_lattice_integrate_batch (with `module`: as qmc_lattice_integrate_batch_module; workspace size from
+ * qmc_workspace_bytes / qmc_sector_module_workspace_bytes).
+ *   The workspace belongs to the batch until qmc_batch_destroy (which frees only host memory); launches of one batch that
+ *   overlap on the GPU race on it.  Read at create: the problem structs, and of sector problems params, z and fit_coeffs (their
+ *   programs and tables are compiled then).  Read at every launch, from the DEVICE pointers given at create: shifts of every
+ *   problem, params / z / fit_coeffs of closed-form problems -- so fresh random shifts written into the same buffer need no new
+ *   batch.  The module, if any, must outlive the batch. */
+typedef struct qmc_batch qmc_batch;
+int qmc_batch_create(int count, const qmc_problem* problems /*HOST*/, qmc_sector_module* module /*or NULL*/,
+                     void* workspace /*DEVICE*/, size_t workspace_bytes, void* cuda_stream, qmc_batch** out /*HOST*/);
+int qmc_batch_launch(qmc_batch* batch, double* out_means /*DEVICE*/, double* out_errs /*DEVICE*/,
+                     double* out_shift_means /*DEVICE or NULL*/, void* cuda_stream);
+void qmc_batch_destroy(qmc_batch* batch);
+
 /* ---- an entry that allocates nothing --------------------------------------------------------------------------------------
  * For callers that cannot allocate device memory around a call (code under CUDA graph capture, tight serving loops, harnesses
  * that forbid it): qmc_lattice_integrate_batch with the workspace in a device array that is part of the library image,
  * QMC_STATIC_SCRATCH_BYTES (4 MiB) per GPU that loads the library, held until the process exits.  Arguments, kernels and results
  * are those of qmc_lattice_integrate_batch (problems HOST structs with DEVICE data pointers, outputs DEVICE, stream-ordered, no
- * synchronisation); the call itself issues no cudaMalloc / cudaFree / allocating library routine.
+ * synchronisation); the call itself issues no cudaMalloc / cudaFree / allocating library routine.  (Under stream capture: a call
+ * for ONE closed-form problem is kernel launches and an 8-byte memset and can be captured; a batch uploads its plan from pageable
+ * host memory as qmc_lattice_integrate_batch does, which a capture refuses -- capture qmc_batch_launch instead.)
  *   Limit: qmc_workspace_bytes(count, problems) <= qmc_static_scratch_bytes(); a larger batch is rejected with QMC_ERR_WORKSPACE
  *   before anything is launched, and qmc_last_cuda_error() then says how many bytes the batch needs (configs[4] of the bench
  *   needs 0.15 MB, the 256-sector batch of configs[3] 1.3 MB).

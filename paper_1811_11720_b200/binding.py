@@ -25,7 +25,7 @@ EXPORTS = [
     "qmc_cdf_sample_count", "qmc_fit_from_cdf", "qmc_sector_module_create", "qmc_sector_module_destroy", "qmc_sector_module_info",
     "qmc_sector_module_image", "qmc_lattice_integrate_batch_module", "qmc_sector_module_workspace_bytes",
     "qmc_lattice_integrate_batch_host_module", "qmc_static_scratch_bytes", "qmc_lattice_integrate_batch_static",
-    "qmc_integrate_batch",
+    "qmc_integrate_batch", "qmc_batch_create", "qmc_batch_launch", "qmc_batch_destroy",
 ]
 
 QMC_OK = 0
@@ -96,6 +96,10 @@ def lib():
         L.qmc_lattice_integrate_batch_host_module.argtypes = [vp, C.c_int, pp, dp, dp, dp]
         L.qmc_integrate_batch.argtypes = [C.c_int, C.POINTER(qmc_integrand), vp, C.c_int, up, up, C.c_int, dp, C.c_uint64, C.c_int, C.c_int,
                                           C.c_double, C.c_double, C.c_uint64, C.c_int, C.POINTER(qmc_result), C.POINTER(C.c_int)]
+        L.qmc_batch_create.argtypes = [C.c_int, pp, vp, vp, C.c_size_t, vp, C.POINTER(vp)]
+        L.qmc_batch_launch.argtypes = [vp, vp, vp, vp, vp]
+        L.qmc_batch_destroy.argtypes = [vp]
+        L.qmc_batch_destroy.restype = None
         L.qmc_static_scratch_bytes.restype = C.c_size_t
         L.qmc_lattice_integrate_batch_static.argtypes = [C.c_int, pp, vp, vp, vp, vp]
         L.qmc_sector_module_workspace_bytes.argtypes = [vp, C.c_int, pp]
@@ -432,6 +436,34 @@ class DeviceBatch:
                                                       self.shift_means.data_ptr(), self.ws_ptr, self.ws_bytes, s, C.byref(self.opts)),
                "qmc_lattice_integrate_batch")
         return int(lib().qmc_last_launch_count())
+
+    def prepare(self, stream=None):
+        """qmc_batch_create on this batch's workspace: plan, upload and prepare once; launch() is then kernel launches only"""
+        s = self.torch.cuda.current_stream(self.device).cuda_stream if stream is None else stream
+        self.release()
+        handle = C.c_void_p()
+        _check(lib().qmc_batch_create(self.count, self.arr, None if self.module is None else self.module.handle, self.ws_ptr,
+                                      self.ws_bytes, s, C.byref(handle)), "qmc_batch_create")
+        self.prepared = handle
+        return self
+
+    def launch(self, stream=None):
+        """qmc_batch_launch (after prepare()); returns launch count"""
+        s = self.torch.cuda.current_stream(self.device).cuda_stream if stream is None else stream
+        _check(lib().qmc_batch_launch(self.prepared, self.means.data_ptr(), self.errs.data_ptr(), self.shift_means.data_ptr(), s),
+               "qmc_batch_launch")
+        return int(lib().qmc_last_launch_count())
+
+    def release(self):
+        if getattr(self, "prepared", None):
+            lib().qmc_batch_destroy(self.prepared)
+        self.prepared = None
+
+    def __del__(self):
+        try:
+            self.release()
+        except Exception:
+            pass
 
     def integrate_static(self, stream=None):
         """qmc_lattice_integrate_batch_static: the same call with the library's static scratch array as workspace (nothing is

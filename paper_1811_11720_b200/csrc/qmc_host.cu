@@ -408,11 +408,16 @@ int arena_reserve(size_t pinned_bytes, size_t device_bytes) {
     return QMC_OK;
 }
 
+// phases of a batch call: a prepared batch (qmc_batch_*) uploads and prepares once (kPhaseSetup) and then only launches
+// (kPhaseLaunch: one memset of the queue heads + the kernels, nothing read from host memory)
+constexpr int kPhaseAll = 0, kPhaseSetup = 1, kPhaseLaunch = 2;
+
 int run_batch(int count, const qmc_problem* problems, double* out_means, double* out_errs, double* out_shift_means,
               void* workspace, size_t workspace_bytes, cudaStream_t st, const qmc_plan_options& opt = kDefaultOptions,
-              char* pinned_blob = nullptr, Plan* prebuilt = nullptr, qmc_sector_module* module = nullptr, int sm_stride = 0) {
+              char* pinned_blob = nullptr, Plan* prebuilt = nullptr, qmc_sector_module* module = nullptr, int sm_stride = 0,
+              int phase = kPhaseAll) {
     g_ts.last_launches = 0;
-    if (!out_means || !out_errs) return QMC_ERR_NULL;
+    if (phase != kPhaseSetup && (!out_means || !out_errs)) return QMC_ERR_NULL;
     Plan local_plan;
     Plan& plan = prebuilt ? *prebuilt : local_plan;          // the HOST-pointer entry plans once and patches the data pointers
     if (!prebuilt) {
@@ -466,11 +471,17 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
             prefix[pf++] = acc;
             ++vi;
         }
-        QMC_CUDA(cudaMemcpyAsync(ws + plan.off_counters, blob, blob_bytes, cudaMemcpyHostToDevice, st));
-        if (any_sector) {                                   // S0 for the sector family: tables + device-side program compiler
-            QMC_CUDA(launch_prepare(count, st, dprobs, daux, dprog));
-            ++g_ts.last_launches;
+        if (phase == kPhaseLaunch) {                        // plan and programs are in the workspace already: reset the queue heads
+            QMC_CUDA(cudaMemsetAsync(ws + plan.off_counters, 0, 64 * sizeof(unsigned long long), st));
+        } else {
+            QMC_CUDA(cudaMemcpyAsync(ws + plan.off_counters, blob, blob_bytes, cudaMemcpyHostToDevice, st));
+            if (any_sector) {                               // S0 for the sector family: tables + device-side program compiler
+                QMC_CUDA(launch_prepare(count, st, dprobs, daux, dprog));
+                ++g_ts.last_launches;
+            }
         }
+    } else if (phase == kPhaseSetup) {
+        return QMC_OK;                                      // a single closed-form problem needs no set-up
     } else {
         std::memset(&queues[0], 0, sizeof(VariantQueue));
         queues[0].total_tiles = plan.variants[0].total_tiles;
@@ -481,6 +492,7 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
             QMC_CUDA(cudaMemsetAsync(queues[0].counter, 0, sizeof(unsigned long long), st));
         }
     }
+    if (phase == kPhaseSetup) return QMC_OK;
     g_ts.ev_valid = false;
     if (g_ts.profile) {
         const int dev = current_device();
@@ -706,6 +718,53 @@ int qmc_lattice_integrate_batch_opts(int count, const qmc_problem* problems, dou
     return run_batch(count, problems, out_means, out_errs, out_shift_means, workspace, workspace_bytes,
                      static_cast<cudaStream_t>(cuda_stream), opts ? *opts : kDefaultOptions);
 }
+// ---- prepared batches: plan, upload and prepare once; every later call is kernel launches only ---------------------------------
+struct qmc_batch {
+    Plan plan;
+    std::vector<qmc_problem> problems;
+    qmc_sector_module* module = nullptr;
+    void* workspace = nullptr;
+    size_t workspace_bytes = 0;
+    int device = -1;
+};
+
+int qmc_batch_create(int count, const qmc_problem* problems, qmc_sector_module* module, void* workspace, size_t workspace_bytes,
+                     void* cuda_stream, qmc_batch** out) {
+    if (!out) return QMC_ERR_NULL;
+    *out = nullptr;
+    qmc_batch* b = new qmc_batch;
+    const int pst = make_plan(count, problems, true, &b->plan, kDefaultOptions, module);
+    if (pst != QMC_OK) { delete b; return pst; }
+    b->problems.assign(problems, problems + count);
+    b->module = module; b->workspace = workspace; b->workspace_bytes = workspace_bytes; b->device = current_device();
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    int rc = run_batch(count, b->problems.data(), nullptr, nullptr, nullptr, workspace, workspace_bytes, st, kDefaultOptions, nullptr, &b->plan,
+                       module, 0, kPhaseSetup);
+    if (rc == QMC_OK && module) {                        // load the module's kernels on this device now, not inside the first launch
+        for (const Variant& v : b->plan.variants)
+            if (v.family == kKernelFamilySpec && spec_occupancy(module, v.spec_kernel) <= 0) rc = QMC_ERR_CUDA;
+    }
+    if (rc == QMC_OK) {
+        for (const Variant& v : b->plan.variants)        // fill the occupancy cache (a query is not a launch, but it is not capturable either)
+            if (v.family != kKernelFamilySpec && occupancy(v.family, v.dp, v.wide) <= 0)
+                rc = cuda_fail(cudaErrorInvalidDeviceFunction, "occupancy query (is the sm_100a image loadable on this device?)");
+    }
+    // the plan was staged from host memory that dies with this call
+    if (rc == QMC_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = cuda_fail(cudaGetLastError(), "cudaStreamSynchronize (qmc_batch_create)");
+    if (rc != QMC_OK) { delete b; return rc; }
+    *out = b;
+    return QMC_OK;
+}
+
+int qmc_batch_launch(qmc_batch* b, double* out_means, double* out_errs, double* out_shift_means, void* cuda_stream) {
+    if (!b) return QMC_ERR_NULL;
+    if (current_device() != b->device) return cuda_fail(cudaErrorInvalidDevice, "qmc_batch_launch: the batch was created on another device");
+    return run_batch((int)b->problems.size(), b->problems.data(), out_means, out_errs, out_shift_means, b->workspace, b->workspace_bytes,
+                     static_cast<cudaStream_t>(cuda_stream), kDefaultOptions, nullptr, &b->plan, b->module, 0, kPhaseLaunch);
+}
+
+void qmc_batch_destroy(qmc_batch* b) { delete b; }
+
 int qmc_lattice_integrate_batch_module(qmc_sector_module* module, int count, const qmc_problem* problems, double* out_means,
                                        double* out_errs, double* out_shift_means, void* workspace, size_t workspace_bytes,
                                        void* cuda_stream) {

@@ -924,3 +924,89 @@ def test_module_config3_full_size():
         sm_or, mean_or, err_or = _golden_arrays(rec, 1)
         assert_means(sms[i], sm_or, probs[i]["name"] + " (full size, specialised)")
         assert_err(errs[i, :1], err_or, sm_or, probs[i]["name"])
+
+
+# ------------------------------------------------------------------------------------------------
+# prepared batches (qmc_batch_*): plan / upload / prepare once, then kernel launches only
+# ------------------------------------------------------------------------------------------------
+def _prepared_problems():
+    return [make(3, 6, 8191, 5, K + 3, 9990), make(0, 5, 4099, 4, K + 3, 9991), make(8, 4, 4099, 4, K + 3, 9992),
+            make(3, 6, 65537, 6, BAKER, 9993), make(3, 4, 8191, 5, K + 3, 9994, fit=True), make_log(6, 8191, 5, K + 3, 9995, pw=2),
+            make(2, 12, 4099, 4, SIDI + 2, 9996), make(1, 8, 262147, 8, BAKER, 9997)]
+
+
+@pytest.mark.parametrize("with_module", [False, True])
+def test_prepared_batch_returns_the_bits_of_the_direct_call(with_module):
+    probs = _prepared_problems()
+    module = binding.SectorModule(probs) if with_module else None
+    direct = binding.DeviceBatch(probs, module=module)
+    n_direct = direct.integrate()
+    ref = direct.results()
+    prepared = binding.DeviceBatch(probs, module=module).prepare()
+    for call in range(3):
+        prepared.shift_means.fill_(float("nan"))
+        n_launch = prepared.launch()
+        assert n_launch == n_direct - 1                     # no prepare kernel, no upload: fused kernels + finalize
+        out = prepared.results()
+        assert all(a.tobytes() == b.tobytes() for a, b in zip(out[0], ref[0])), call
+        assert out[1].tobytes() == ref[1].tobytes() and out[2].tobytes() == ref[2].tobytes()
+
+
+def test_prepared_batch_reads_shifts_at_launch():
+    """fresh random shifts written into the same device buffers need no new batch"""
+    import torch
+    probs = _prepared_problems()
+    prepared = binding.DeviceBatch(probs).prepare()
+    prepared.launch()
+    first = prepared.results()
+    rng = synth.MT19937_64(424242)
+    fresh = [dict(p, shifts=synth.draw_shifts(rng, p["m"], p["dim"])) for p in probs]
+    for i in range(len(probs)):
+        prepared._keep[4 * i + 2].copy_(torch.from_numpy(fresh[i]["shifts"]))      # the shifts tensor of problem i (DeviceBatch.__init__)
+    prepared.launch()
+    second = prepared.results()
+    ref = run_gpu(fresh)
+    assert all(a.tobytes() == b.tobytes() for a, b in zip(second[0], ref[0]))
+    assert not all(a.tobytes() == b.tobytes() for a, b in zip(second[0], first[0]))
+
+
+@pytest.mark.parametrize("with_module", [False, True])
+def test_prepared_batch_launch_is_graph_capturable(with_module):
+    """a whole sector batch -- tile queues, several kernel variants, finalize -- captured once and replayed"""
+    import torch
+    probs = _prepared_problems()
+    module = binding.SectorModule(probs) if with_module else None
+    ref = run_gpu(probs, module=module)
+    batch = binding.DeviceBatch(probs, module=module).prepare()
+    binding.qmc_profile_enable(False)
+    try:
+        batch.launch()
+        torch.cuda.synchronize()
+        side = torch.cuda.Stream()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            batch.launch()
+        for rep in range(3):
+            batch.shift_means.fill_(float("nan"))
+            batch.means.fill_(float("nan"))
+            graph.replay()
+            out = batch.results()
+            assert all(a.tobytes() == b.tobytes() for a, b in zip(out[0], ref[0])), rep
+            assert out[1].tobytes() == ref[1].tobytes()
+    finally:
+        binding.qmc_profile_enable(False)                   # the default
+
+
+def test_prepared_batch_argument_checks():
+    L = binding.lib()
+    probs = _prepared_problems()[:2]
+    b = binding.DeviceBatch(probs)
+    import ctypes as C
+    handle = C.c_void_p()
+    assert L.qmc_batch_create(b.count, b.arr, None, b.ws_ptr, 256, None, C.byref(handle)) == -11      # workspace too small
+    assert L.qmc_batch_create(0, b.arr, None, b.ws_ptr, b.ws_bytes, None, C.byref(handle)) == -3
+    assert L.qmc_batch_create(b.count, b.arr, None, b.ws_ptr, b.ws_bytes, None, None) == -1
+    assert L.qmc_batch_launch(None, None, None, None, None) == -1
+    b.prepare()
+    assert L.qmc_batch_launch(b.prepared, None, b.errs.data_ptr(), None, None) == -1
+    L.qmc_batch_destroy(None)
