@@ -160,8 +160,10 @@ size_t qmc_workspace_bytes(int count, const qmc_problem* problems /*HOST*/);
 /* Launch-plan options for tests and tuning (zero-initialise for the library's plan): the same calls with an options
  * struct.  tiles_target > 0: that many tiles per kernel variant instead of the planned count (S9; results are
  * bit-identical only for equal tilings); force_wide != 0: the 64-bit-residue kernels even for n < 2^31 (they are
- * otherwise reached only by n >= 2^31; results are bit-identical to the 32-bit kernels). */
-typedef struct { int tiles_target; int force_wide; } qmc_plan_options;
+ * otherwise reached only by n >= 2^31; results are bit-identical to the 32-bit kernels); group = 4 or 8: shifts evaluated per
+ * lattice index by the product-peak kernels of <= 8 dimension slots (0: the plan chooses from m; other kernels ignore it; the
+ * per-shift results do not depend on it bit for bit). */
+typedef struct { int tiles_target; int force_wide; int group; } qmc_plan_options;
 int qmc_lattice_integrate_batch_opts(int count, const qmc_problem* problems /*HOST*/, double* out_means /*DEVICE*/,
                                      double* out_errs /*DEVICE*/, double* out_shift_means /*DEVICE or NULL*/,
                                      void* workspace /*DEVICE*/, size_t workspace_bytes, void* cuda_stream,

@@ -146,6 +146,7 @@ struct Variant {
     std::vector<int> plist;          // problem indices, queue order (most expensive tiles first)
     long long total_tiles = 0;
     int spec_kernel = -1;            // kKernelFamilySpec: the module's kernel
+    int group = kGroup;              // closed-form families: shifts per group of the kernel (4, or 8: pick_group)
 };
 
 struct Plan {
@@ -158,7 +159,23 @@ struct Plan {
     long long total_tiles = 0;
 };
 
-const qmc_plan_options kDefaultOptions = {0, 0};
+const qmc_plan_options kDefaultOptions = {0, 0, 0};
+
+// Shifts per group of a closed-form kernel.  The product-peak kernels of <= 8 dimension slots exist with 4 and with 8 shifts per
+// lattice index: 8 amortise the residue walk over twice the shifts and give every warp twice the independent chains (configs[1]:
+// 0.141 -> 0.130 ms), but a ragged last group evaluates idle slots, so the choice follows m: the fewer slots, an 8-group slot
+// counted as kGroup8Cost of a 4-group slot.  Measured for every family at 4 / 6 / 8 slots and m = 32: the other families (longer
+// per-point chains, more live registers at the same 128-register cap) lose 1-20 % with 8, and so does the product peak with a fit
+// map: they keep 4.
+constexpr double kGroup8Cost = 0.95;
+int pick_group(int kernel_fam, int dp, bool wide, int m, bool has_fit, const qmc_plan_options& opt) {
+    if (!closed_has_group8(kernel_fam, dp, wide)) return kGroup;
+    if (opt.group == kGroup || opt.group == kGroupWide) return opt.group;
+    if (has_fit) return kGroup;
+    const double slots4 = (double)((m + kGroup - 1) / kGroup * kGroup);
+    const double slots8 = (double)((m + kGroupWide - 1) / kGroupWide * kGroupWide) * kGroup8Cost;
+    return slots8 < slots4 ? kGroupWide : kGroup;
+}
 
 int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan* plan, const qmc_plan_options& opt = kDefaultOptions,
               const qmc_sector_module* module = nullptr, const int* module_index = nullptr) {
@@ -241,10 +258,11 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
             spec_kernel = spec_problems(module)[in_module(i)].kernel;
             plan->dev[i].spec_case = spec_problems(module)[in_module(i)].kase;
         }
+        const int group = pick_group(kfam, dp, wide, d.m, d.has_fit != 0, opt);
         Variant* v = nullptr;
         for (auto& c : plan->variants)
-            if (c.family == kfam && c.dp == dp && c.wide == wide && c.spec_kernel == spec_kernel) v = &c;
-        if (!v) { plan->variants.push_back(Variant{kfam, dp, wide, {}, 0, spec_kernel}); v = &plan->variants.back(); }
+            if (c.family == kfam && c.dp == dp && c.wide == wide && c.spec_kernel == spec_kernel && c.group == group) v = &c;
+        if (!v) { plan->variants.push_back(Variant{kfam, dp, wide, {}, 0, spec_kernel, group}); v = &plan->variants.back(); }
         v->plist.push_back(i);
     }
     if (plan->variants.size() > 64) return QMC_ERR_WORKSPACE;
@@ -337,7 +355,7 @@ int sm_count() {
     return n;
 }
 
-// closed-form families: the kernel variants live in four parts per family (qmc_fused_closed.inc); try each
+// closed-form families: the kernel variants live in four parts per family (+ one of the product peak with 8 shifts per group) (qmc_fused_closed.inc); try each
 #define QMC_TRY_PARTS(FAM, PREFIX, FAIL, ...)                                                             \
     {                                                                                                    \
         auto r0 = PREFIX##FAM##_0(__VA_ARGS__); if (r0 != FAIL) return r0;                               \
@@ -345,35 +363,39 @@ int sm_count() {
         auto r2 = PREFIX##FAM##_2(__VA_ARGS__); if (r2 != FAIL) return r2;                               \
         return PREFIX##FAM##_3(__VA_ARGS__);                                                             \
     }
-cudaError_t launch_closed(int family, int dp, bool wide, int grid, cudaStream_t st, const FusedLaunch& a) {
+cudaError_t launch_closed(int family, int dp, bool wide, int group, int grid, cudaStream_t st, const FusedLaunch& a) {
     switch (family) {
-        case 0: QMC_TRY_PARTS(0, launch_fused_part_, cudaErrorInvalidValue, dp, wide, grid, st, a)
-        case 1: QMC_TRY_PARTS(1, launch_fused_part_, cudaErrorInvalidValue, dp, wide, grid, st, a)
-        case 2: QMC_TRY_PARTS(2, launch_fused_part_, cudaErrorInvalidValue, dp, wide, grid, st, a)
-        case 4: QMC_TRY_PARTS(4, launch_fused_part_, cudaErrorInvalidValue, dp, wide, grid, st, a)
+        case 0: QMC_TRY_PARTS(0, launch_fused_part_, cudaErrorInvalidValue, dp, wide, group, grid, st, a)
+        case 1:
+            if (group == kGroupWide) return launch_fused_part_1_4(dp, wide, group, grid, st, a);
+            QMC_TRY_PARTS(1, launch_fused_part_, cudaErrorInvalidValue, dp, wide, group, grid, st, a)
+        case 2: QMC_TRY_PARTS(2, launch_fused_part_, cudaErrorInvalidValue, dp, wide, group, grid, st, a)
+        case 4: QMC_TRY_PARTS(4, launch_fused_part_, cudaErrorInvalidValue, dp, wide, group, grid, st, a)
     }
     return cudaErrorInvalidValue;
 }
-int occupancy_closed(int family, int dp, bool wide) {
+int occupancy_closed(int family, int dp, bool wide, int group) {
     switch (family) {
-        case 0: QMC_TRY_PARTS(0, occupancy_fused_part_, -1, dp, wide)
-        case 1: QMC_TRY_PARTS(1, occupancy_fused_part_, -1, dp, wide)
-        case 2: QMC_TRY_PARTS(2, occupancy_fused_part_, -1, dp, wide)
-        case 4: QMC_TRY_PARTS(4, occupancy_fused_part_, -1, dp, wide)
+        case 0: QMC_TRY_PARTS(0, occupancy_fused_part_, -1, dp, wide, group)
+        case 1:
+            if (group == kGroupWide) return occupancy_fused_part_1_4(dp, wide, group);
+            QMC_TRY_PARTS(1, occupancy_fused_part_, -1, dp, wide, group)
+        case 2: QMC_TRY_PARTS(2, occupancy_fused_part_, -1, dp, wide, group)
+        case 4: QMC_TRY_PARTS(4, occupancy_fused_part_, -1, dp, wide, group)
     }
     return -1;
 }
 #undef QMC_TRY_PARTS
 
-int occupancy(int family, int dp, bool wide) {
-    static int cache[kMaxDevices][kKernelFamilies][33][2];
+int occupancy(int family, int dp, bool wide, int group = kGroup) {
+    static int cache[kMaxDevices][kKernelFamilies][33][2][2];
     const int dev = current_device();
     if (dev < 0) return -1;
-    int& c = cache[dev][family][dp][wide ? 1 : 0];
+    int& c = cache[dev][family][dp][wide ? 1 : 0][group == kGroupWide ? 1 : 0];
     if (c > 0) return c;
     int v = -1;
     switch (family) {
-        case 0: case 1: case 2: case 4: v = occupancy_closed(family, dp, wide); break;
+        case 0: case 1: case 2: case 4: v = occupancy_closed(family, dp, wide, group); break;
         case 3: v = occupancy_fused_f3(dp, wide); break;
         case kKernelFamilyCSector: v = occupancy_fused_f8(dp, wide); break;
     }
@@ -486,7 +508,7 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
         std::memset(&queues[0], 0, sizeof(VariantQueue));
         queues[0].total_tiles = plan.variants[0].total_tiles;
         const Variant& v0 = plan.variants[0];
-        if (v0.total_tiles > (long long)sms * std::max(1, occupancy(v0.family, v0.dp, v0.wide))) {
+        if (v0.total_tiles > (long long)sms * std::max(1, occupancy(v0.family, v0.dp, v0.wide, v0.group))) {
             // more tiles than resident CTAs: dynamic queue (one 8-byte reset); otherwise every CTA owns one tile
             queues[0].counter = reinterpret_cast<unsigned long long*>(ws + plan.off_counters);
             QMC_CUDA(cudaMemsetAsync(queues[0].counter, 0, sizeof(unsigned long long), st));
@@ -502,7 +524,7 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
     }
     for (size_t vi = 0; vi < plan.variants.size(); ++vi) {
         const Variant& v = plan.variants[vi];
-        const int occ = v.family == kKernelFamilySpec ? spec_occupancy(module, v.spec_kernel) : occupancy(v.family, v.dp, v.wide);
+        const int occ = v.family == kKernelFamilySpec ? spec_occupancy(module, v.spec_kernel) : occupancy(v.family, v.dp, v.wide, v.group);
         if (occ <= 0 && v.family == kKernelFamilySpec) return QMC_ERR_CUDA;      // the loader left the text
         if (occ <= 0) return cuda_fail(cudaErrorInvalidDeviceFunction, "occupancy query (is the sm_100a image loadable on this device?)");
         const long long cap = (long long)sms * occ;
@@ -517,7 +539,7 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
         }
         cudaError_t e = cudaErrorInvalidValue;
         switch (v.family) {
-            case 0: case 1: case 2: case 4: e = launch_closed(v.family, v.dp, v.wide, grid, st, a); break;
+            case 0: case 1: case 2: case 4: e = launch_closed(v.family, v.dp, v.wide, v.group, grid, st, a); break;
             case 3: e = launch_fused_f3(v.dp, v.wide, grid, st, a); break;
             case kKernelFamilyCSector: e = launch_fused_f8(v.dp, v.wide, grid, st, a); break;
         }
@@ -699,7 +721,7 @@ int qmc_plan_info(int count, const qmc_problem* problems, long long* out_tiles, 
         int ctas = 0;
         const int sms = sm_count();
         for (auto& v : plan.variants) {
-            const int occ = sms > 0 ? occupancy(v.family, v.dp, v.wide) : 0;
+            const int occ = sms > 0 ? occupancy(v.family, v.dp, v.wide, v.group) : 0;
             ctas += (int)std::min<long long>((long long)sms * std::max(occ, 0), v.total_tiles);
         }
         *out_ctas = ctas;
@@ -746,7 +768,7 @@ int qmc_batch_create(int count, const qmc_problem* problems, qmc_sector_module* 
     }
     if (rc == QMC_OK) {
         for (const Variant& v : b->plan.variants)        // fill the occupancy cache (a query is not a launch, but it is not capturable either)
-            if (v.family != kKernelFamilySpec && occupancy(v.family, v.dp, v.wide) <= 0)
+            if (v.family != kKernelFamilySpec && occupancy(v.family, v.dp, v.wide, v.group) <= 0)
                 rc = cuda_fail(cudaErrorInvalidDeviceFunction, "occupancy query (is the sm_100a image loadable on this device?)");
     }
     // the plan was staged from host memory that dies with this call

@@ -11,6 +11,8 @@ namespace qmc {
 constexpr int kThreads = 128;          // threads per CTA of the fused kernels (4 warps)
 constexpr int kWarps = kThreads / 32;
 constexpr int kGroup = 4;             // shifts evaluated together per lattice index (register-resident)
+constexpr int kGroupWide = 8;          // ... the product-peak kernels of <= 8 dimension slots also exist with 8 (chosen by the plan from m)
+constexpr bool closed_has_group8(int kernel_family, int dp, bool wide) { return kernel_family == QMC_FAMILY_GENZ_PRODPEAK && dp <= 8 && !wide; }
 constexpr int kMaxSteps = 1024;        // max lattice indices per thread per tile (bounds the naive fp64 chain length)
 constexpr int kPlanSMs = 148;          // the tiling is planned for a B200 (a pure function of the problem structs: results
                                        // are bit-identical on any device, only the balance is tuned for 148 SMs)

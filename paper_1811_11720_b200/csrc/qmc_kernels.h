@@ -35,10 +35,11 @@ cudaError_t launch_dfma_probe(cudaStream_t st, double* out, int blocks, int iter
 
 // fused kernels: closed-form families 0-2 in parts (qmc_fused_closed.inc), the sector family in qmc_fused_f3.cu
 #define QMC_DECLARE_PART(FAM, PART)                                                                                         \
-    cudaError_t launch_fused_part_##FAM##_##PART(int dp, bool wide, int grid, cudaStream_t st, const FusedLaunch& a); \
-    int occupancy_fused_part_##FAM##_##PART(int dp, bool wide);
+    cudaError_t launch_fused_part_##FAM##_##PART(int dp, bool wide, int group, int grid, cudaStream_t st, const FusedLaunch& a); \
+    int occupancy_fused_part_##FAM##_##PART(int dp, bool wide, int group);
 #define QMC_DECLARE_FAMILY(FAM) QMC_DECLARE_PART(FAM, 0) QMC_DECLARE_PART(FAM, 1) QMC_DECLARE_PART(FAM, 2) QMC_DECLARE_PART(FAM, 3)
 QMC_DECLARE_FAMILY(0) QMC_DECLARE_FAMILY(1) QMC_DECLARE_FAMILY(2) QMC_DECLARE_FAMILY(4)
+QMC_DECLARE_PART(1, 4)     // product peak, <= 8 slots, 8 shifts per group
 #undef QMC_DECLARE_FAMILY
 #undef QMC_DECLARE_PART
 cudaError_t launch_fused_f3(int dp, bool wide, int grid, cudaStream_t st, const FusedLaunch& a);

@@ -1010,3 +1010,18 @@ def test_prepared_batch_argument_checks():
     b.prepare()
     assert L.qmc_batch_launch(b.prepared, None, b.errs.data_ptr(), None, None) == -1
     L.qmc_batch_destroy(None)
+
+
+@pytest.mark.parametrize("d", [1, 3, 4, 5, 6, 8])
+@pytest.mark.parametrize("m", [2, 5, 8, 11, 16, 32])
+def test_product_peak_group_of_8_shifts(d, m):
+    """the product-peak kernels of <= 8 slots exist with 4 and 8 shifts per lattice index (the plan chooses from m): per-shift
+    results are the same bits either way, ragged last groups included, and match the oracle"""
+    for tr in (BAKER, K + 3, NONE):
+        p = make(1, d, 8191, m, tr, 9700 + 10 * d + m)
+        a = run_gpu([p], group=4)
+        b = run_gpu([p], group=8)
+        c = run_gpu([p])
+        assert a[0][0].tobytes() == b[0][0].tobytes() == c[0][0].tobytes()
+        assert a[1].tobytes() == b[1].tobytes() and a[2].tobytes() == b[2].tobytes()
+    check_against_oracle([p], group=8)
