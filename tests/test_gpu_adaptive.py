@@ -220,3 +220,22 @@ def test_batch_iteration_rejects_bad_arguments():
     assert results[2]["iterations"] == 1
     for r, q in zip(results[:2], alone):
         assert (r["n"], r["m"]) == (q["n"], q["m"]) and np.all(np.abs(r["integral"] - q["integral"]) <= 1e-13 * np.abs(q["integral"]))
+
+
+def test_batch_iteration_with_fit_maps_and_wide_ladder():
+    """integrands with a fit map (cubic and with pole terms) next to plain ones, on a ladder and shifts of more dimensions than any of them"""
+    rng = synth.MT19937_64(7171)
+    cubic = np.array([[1.001, -0.001, 0.0, 0.0, 0.45 + 0.5 * rng.uniform(), 0.5 * rng.uniform() - 0.1] for _ in range(4)])
+    poles = np.array([[1.2 + 0.3 * rng.uniform(), -0.2 - 0.3 * rng.uniform(), 0.2 * rng.uniform(), 0.2 * rng.uniform(),
+                       0.45 + 0.3 * rng.uniform(), 0.2 * rng.uniform() - 0.05] for _ in range(5)])
+    integrands = [dict(family=1, dim=4, transform=K + 3, params=synth.genz_prodpeak(rng, 4), fit_coeffs=cubic),
+                  dict(family=3, dim=5, transform=K + 3, params=synth.sector(rng, 5), fit_coeffs=poles),
+                  dict(family=3, dim=5, transform=K + 3, params=synth.sector(rng, 5)),
+                  dict(family=0, dim=3, transform=synth.TRANSFORM_BAKER, params=synth.genz_osc(rng, 3))]
+    ln, lz = synth.ladder(8, 65521)
+    shifts = synth.draw_shifts(synth.MT19937_64(96), 10, 8)
+    module = binding.SectorModule(integrands)
+    kw = dict(min_n=1000, min_m=6, epsrel=1e-6, epsabs=0.0, maxeval=10**8)
+    for mod in (None, module):
+        results, statuses, overall = binding.qmc_integrate_batch(integrands, ln, lz, shifts, module=mod, **kw)
+        _check_batch_against_oracle_and_single(integrands, results, statuses, ln, lz, shifts, **kw)
