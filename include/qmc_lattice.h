@@ -162,8 +162,9 @@ size_t qmc_workspace_bytes(int count, const qmc_problem* problems /*HOST*/);
  * bit-identical only for equal tilings); force_wide != 0: the 64-bit-residue kernels even for n < 2^31 (they are
  * otherwise reached only by n >= 2^31; results are bit-identical to the 32-bit kernels); group = 4 or 8: shifts evaluated per
  * lattice index by the product-peak kernels of <= 8 dimension slots (0: the plan chooses from m; other kernels ignore it; the
- * per-shift results do not depend on it bit for bit). */
-typedef struct { int tiles_target; int force_wide; int group; } qmc_plan_options;
+ * per-shift results do not depend on it bit for bit); generic_call != 0: Korobov r != 3, Korobov (r0, r1) and Sidi run the
+ * generic loop inside the family's kernel even where a dedicated kernel exists (no fit map, n < 2^31, dim <= 16). */
+typedef struct { int tiles_target; int force_wide; int group; int generic_call; } qmc_plan_options;
 int qmc_lattice_integrate_batch_opts(int count, const qmc_problem* problems /*HOST*/, double* out_means /*DEVICE*/,
                                      double* out_errs /*DEVICE*/, double* out_shift_means /*DEVICE or NULL*/,
                                      void* workspace /*DEVICE*/, size_t workspace_bytes, void* cuda_stream,

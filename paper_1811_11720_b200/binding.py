@@ -50,7 +50,7 @@ class qmc_problem(C.Structure):
 
 
 class qmc_plan_options(C.Structure):
-    _fields_ = [("tiles_target", C.c_int), ("force_wide", C.c_int), ("group", C.c_int)]
+    _fields_ = [("tiles_target", C.c_int), ("force_wide", C.c_int), ("group", C.c_int), ("generic_call", C.c_int)]
 
 
 class qmc_integrand(C.Structure):
@@ -381,10 +381,10 @@ class DeviceBatch:
     (count, 2*max_m).
     """
 
-    def __init__(self, problems, device="cuda:0", tiles_target=0, force_wide=False, module=None, group=0):
+    def __init__(self, problems, device="cuda:0", tiles_target=0, force_wide=False, module=None, group=0, generic_call=False):
         import torch
         self.module = module                               # a SectorModule built from the same problems, or None
-        self.opts = qmc_plan_options(int(tiles_target), 1 if force_wide else 0, int(group))
+        self.opts = qmc_plan_options(int(tiles_target), 1 if force_wide else 0, int(group), 1 if generic_call else 0)
         self.torch = torch
         self.device = torch.device(device)
         self.problems = problems

@@ -178,37 +178,32 @@ __device__ __forceinline__ double ipow_upto7(double x, int e) {
     return r;
 }
 
-// The generic tile loop's S3-S4 for ONE dimension and the G shifts of the group: the transform kind and the fit mode are decided
-// once per dimension (warp-uniform branches), the G coordinates inside each branch are straight-line code, so that their
-// dependency chains overlap (a DFMA result takes ~35 cycles; decided per coordinate, as in round 1, the chains ran one after the
-// other and the generic loop reached 17-19 % of the FP64 peak).  Symmetric Korobov weights carry P = prod (1/4 - c^2) and are
-// raised to the power r once per point (point_weight); the others multiply their weight into P directly.
+// symmetric Korobov weight, any r <= 6: g_r(s) by a fixed six-step Horner scheme on the zero-padded table k (degree r; fma(0, s, k) = k
+// exactly, so the padded steps change nothing); P *= 1/4 - c^2, raised to the power r once per point (point_weight)
 template <int G>
-__device__ __forceinline__ void generic_coord_group(const double (&t)[G], unsigned kor_addr, int gen, const FitC& fc, double (&x)[G],
-                                                    double (&P)[G], double (&D)[G]) {
-    const int kind = gen & 15, r0 = (gen >> 4) & 15, r1 = (gen >> 8) & 15;
-    if (kind == GEN_NONE) {
+__device__ __forceinline__ void korobov_sym_points(const double (&t)[G], const double (&k)[7], double (&x)[G], double (&P)[G]) {
 #pragma unroll
-        for (int q = 0; q < G; ++q) x[q] = wrap_u(t[q]);
-    } else if (kind == GEN_BAKER) {
+    for (int q = 0; q < G; ++q) {
+        const double c = centre_c(t[q]);
+        const double s = c * c;
+        P[q] *= (0.25 - s);
+        double g = k[6];
 #pragma unroll
-        for (int q = 0; q < G; ++q) x[q] = 1.0 - fabs(baker_w(t[q]));
-    } else if (kind == GEN_KOROBOV_SYM) {
-        // g_r(s) by a fixed six-step Horner scheme: the table is zero above degree r, and fma(0, s, k) = k exactly
+        for (int i = 5; i >= 0; --i) g = __fma_rn(g, s, k[i]);
+        x[q] = __fma_rn(c, g, 0.5);
+    }
+}
+
+// The three weight transforms of the generic loop for the G shifts of a group, one dimension, straight-line each (see
+// generic_coord_group); r0, r1 are warp-uniform.  KIND is a GEN_* code.
+template <int G, int KIND>
+__device__ __forceinline__ void generic_kind_group(const double (&t)[G], unsigned kor_addr, int r0, int r1, double (&x)[G], double (&P)[G]) {
+    if constexpr (KIND == GEN_KOROBOV_SYM) {
         double k[7];
 #pragma unroll
         for (int i = 0; i < 7; ++i) k[i] = lds_f64(kor_addr + 8u * i);
-#pragma unroll
-        for (int q = 0; q < G; ++q) {
-            const double c = centre_c(t[q]);
-            const double s = c * c;
-            P[q] *= (0.25 - s);
-            double g = k[6];
-#pragma unroll
-            for (int i = 5; i >= 0; --i) g = __fma_rn(g, s, k[i]);
-            x[q] = __fma_rn(c, g, 0.5);
-        }
-    } else if (kind == GEN_KOROBOV_ASYM) {
+        korobov_sym_points<G>(t, k, x, P);
+    } else if constexpr (KIND == GEN_KOROBOV_ASYM) {
 #pragma unroll
         for (int q = 0; q < G; ++q) {
             const double u = wrap_u(t[q]);
@@ -251,6 +246,30 @@ __device__ __forceinline__ void generic_coord_group(const double (&t)[G], unsign
             P[q] *= ipow_upto7(sn, r0);
             x[q] = K * I;
         }
+    }
+}
+
+// The generic tile loop's S3-S4 for ONE dimension and the G shifts of the group: the transform kind and the fit mode are decided
+// once per dimension (warp-uniform branches), the G coordinates inside each branch are straight-line code, so that their
+// dependency chains overlap (a DFMA result takes ~35 cycles; decided per coordinate, as in round 1, the chains ran one after the
+// other and the generic loop reached 17-19 % of the FP64 peak).  Symmetric Korobov weights carry P = prod (1/4 - c^2) and are
+// raised to the power r once per point (point_weight); the others multiply their weight into P directly.
+template <int G>
+__device__ __forceinline__ void generic_coord_group(const double (&t)[G], unsigned kor_addr, int gen, const FitC& fc, double (&x)[G],
+                                                    double (&P)[G], double (&D)[G]) {
+    const int kind = gen & 15, r0 = (gen >> 4) & 15, r1 = (gen >> 8) & 15;
+    if (kind == GEN_NONE) {
+#pragma unroll
+        for (int q = 0; q < G; ++q) x[q] = wrap_u(t[q]);
+    } else if (kind == GEN_BAKER) {
+#pragma unroll
+        for (int q = 0; q < G; ++q) x[q] = 1.0 - fabs(baker_w(t[q]));
+    } else if (kind == GEN_KOROBOV_SYM) {
+        generic_kind_group<G, GEN_KOROBOV_SYM>(t, kor_addr, r0, r1, x, P);
+    } else if (kind == GEN_KOROBOV_ASYM) {
+        generic_kind_group<G, GEN_KOROBOV_ASYM>(t, kor_addr, r0, r1, x, P);
+    } else {
+        generic_kind_group<G, GEN_SIDI>(t, kor_addr, r0, r1, x, P);
     }
     if (fc.mode) {                                            // S4: fit map of Eq. 19
 #pragma unroll
@@ -305,8 +324,8 @@ __device__ __forceinline__ double point_coord(double rd, double inv_n, double de
 template <int TR, int FIT> __device__ __forceinline__ double point_weight(double P, double D, double wconst, int kor_r) {
     double W = 1.0;
     if (TR == TR_KOR3) W = wconst * (P * P * P);
-    else if (TR == TR_KORR) W = wconst * (((kor_r & 15) == GEN_KOROBOV_SYM) ? ipow_small(P, (kor_r >> 4) & 15) : P);   // symmetric Korobov: P = prod (1/4 - c^2)
-    if (FIT) W = (TR == TR_KOR3 || TR == TR_KORR) ? W * D : D;
+    else if (TR == TR_KORR || TR >= TR_GEN0) W = wconst * (((kor_r & 15) == GEN_KOROBOV_SYM) ? ipow_small(P, (kor_r >> 4) & 15) : P);   // symmetric Korobov: P = prod (1/4 - c^2)
+    if (FIT) W = (TR == TR_KOR3 || TR == TR_KORR || TR >= TR_GEN0) ? W * D : D;
     return W;
 }
 
@@ -353,8 +372,34 @@ __device__ __forceinline__ void eval_point_group(const typename Res<WIDE>::T (&r
     double s0[G], s1[G], P[G], D[G];
 #pragma unroll
     for (int q = 0; q < G; ++q) { fam_init<FAMILY>(s0[q], s1[q], cx.fam0); P[q] = 1.0; D[q] = 1.0; }
+    if constexpr (TR >= TR_GEN0) {
+        // dedicated generic kernels: the transform kind is a template parameter and there is no fit map, so the dimensions form one
+        // basic block like the specialised loops' (the orders r0, r1 stay run-time values)
+        static_assert(FIT == 0, "the dedicated generic kernels have no fit map");
+        constexpr int KIND = TR - TR_GEN0;
+        const int r0 = (cx.kor_r >> 4) & 15, r1 = (cx.kor_r >> 8) & 15;
+        const unsigned kor_addr = cx.sbase + SmemOff<DP, G>::kor;
+        double ksym[7];
+        if constexpr (KIND == GEN_KOROBOV_SYM) {
 #pragma unroll
-    for (int j = 0; j < DP; ++j) {
+            for (int i = 0; i < 7; ++i) ksym[i] = lds_f64(kor_addr + 8u * i);
+        }
+#pragma unroll
+        for (int j = 0; j < DP; ++j) {
+            const double rd = Res<WIDE>::to_double(r[j]);
+            double fa, fb, dl[G], t[G], xg[G];
+            FitC fc;
+            load_slot<DP, G, 0>(cx.sbase, cx.delta, j, 0, fa, fb, fc, dl);
+#pragma unroll
+            for (int q = 0; q < G; ++q) t[q] = coord_t(rd, cx.inv_n, dl[q]);
+            if constexpr (KIND == GEN_KOROBOV_SYM) korobov_sym_points<G>(t, ksym, xg, P);
+            else generic_kind_group<G, KIND>(t, kor_addr, r0, r1, xg, P);
+#pragma unroll
+            for (int q = 0; q < G; ++q) fam_dim<FAMILY>(s0[q], s1[q], xg[q], fa, fb, cx.fam_kind);
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < (TR >= TR_GEN0 ? 0 : DP); ++j) {
         const double rd = Res<WIDE>::to_double(r[j]);
         double fa, fb, dl[G];
         FitC fc;
@@ -380,7 +425,7 @@ __device__ __forceinline__ void eval_point_group(const typename Res<WIDE>::T (&r
             }
         }
     }
-    constexpr bool USEW = (TR == TR_KOR3 || TR == TR_KORR || FIT != 0);
+    constexpr bool USEW = (TR == TR_KOR3 || TR == TR_KORR || TR >= TR_GEN0 || FIT != 0);
 #pragma unroll
     for (int q = 0; q < G; ++q)
         fam_finish<FAMILY>(s0[q], s1[q], point_weight<TR, FIT>(P[q], D[q], cx.wconst, cx.kor_r), USEW, acc[q], cx.fam_kind, cx.fam_pow);
@@ -675,6 +720,22 @@ __global__ void __launch_bounds__(kThreads, MinBlocks<DP, WIDE>::value) fused_ke
             default: run_tile_call<ClosedEval<FAMILY, DP, G, WIDE, TR_KORR, FIT_RT>, DP, G, WIDE>(sm, sbase, ex, tile_local, changed, L.partials); break;
         }
     }
+}
+
+// The generic weight transforms without a fit map as kernels of their own (TRG = TR_GEN0 + GEN_* kind): inside fused_kernel the generic
+// loop is a call target that must live with the register cap of the specialised loops and decides the kind per dimension; here
+// the kind is fixed at compile time and the register budget is the kernel's own.  32-bit residues only; fit maps, n >= 2^31
+// and dim > 16 keep the generic loop of fused_kernel.
+template <int FAMILY, int DP, int G, int TRG>
+__global__ void __launch_bounds__(kThreads, min_blocks_generic(DP)) fused_generic_kernel(const __grid_constant__ FusedLaunch L) {
+    __shared__ SmemCtx<DP, G> sm;
+    const unsigned sbase = (unsigned)__cvta_generic_to_shared(&sm);
+    int cur = -1, iter = 0;
+    long long tile_local = 0;
+    bool changed;
+    NoExtra ex;
+    while (next_tile<DP, G, false>(sm, L, cur, iter, tile_local, changed))
+        run_tile<ClosedEval<FAMILY, DP, G, false, TRG, 0>, DP, G, false>(sm, sbase, ex, tile_local, changed, L.partials);
 }
 
 }  // namespace qmc

@@ -147,6 +147,7 @@ struct Variant {
     long long total_tiles = 0;
     int spec_kernel = -1;            // kKernelFamilySpec: the module's kernel
     int group = kGroup;              // closed-form families: shifts per group of the kernel (4, or 8: pick_group)
+    int gen_kind = -1;               // closed-form families: GEN_* kind of a dedicated generic kernel, or -1
 };
 
 struct Plan {
@@ -159,7 +160,7 @@ struct Plan {
     long long total_tiles = 0;
 };
 
-const qmc_plan_options kDefaultOptions = {0, 0, 0};
+const qmc_plan_options kDefaultOptions = {0, 0, 0, 0};
 
 // Shifts per group of a closed-form kernel.  The product-peak kernels of <= 8 dimension slots exist with 4 and with 8 shifts per
 // lattice index: 8 amortise the residue walk over twice the shifts and give every warp twice the independent chains (configs[1]:
@@ -259,10 +260,15 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
             plan->dev[i].spec_case = spec_problems(module)[in_module(i)].kase;
         }
         const int group = pick_group(kfam, dp, wide, d.m, d.has_fit != 0, opt);
+        // Korobov r != 3, Korobov (r0, r1) and Sidi without a fit map, 32-bit residues, <= 16 slots: the dedicated generic kernels
+        int gen_kind = -1;
+        const bool closed = kfam == 0 || kfam == 1 || kfam == 2 || kfam == kKernelFamilyGenzMisc;
+        if (closed && !wide && dp <= 16 && d.tr_kind == TR_KORR && !d.has_fit && (d.gen & 15) < kGenKinds && !opt.generic_call)
+            gen_kind = d.gen & 15;
         Variant* v = nullptr;
         for (auto& c : plan->variants)
-            if (c.family == kfam && c.dp == dp && c.wide == wide && c.spec_kernel == spec_kernel && c.group == group) v = &c;
-        if (!v) { plan->variants.push_back(Variant{kfam, dp, wide, {}, 0, spec_kernel, group}); v = &plan->variants.back(); }
+            if (c.family == kfam && c.dp == dp && c.wide == wide && c.spec_kernel == spec_kernel && c.group == group && c.gen_kind == gen_kind) v = &c;
+        if (!v) { plan->variants.push_back(Variant{kfam, dp, wide, {}, 0, spec_kernel, group, gen_kind}); v = &plan->variants.back(); }
         v->plist.push_back(i);
     }
     if (plan->variants.size() > 64) return QMC_ERR_WORKSPACE;
@@ -270,7 +276,7 @@ int make_plan(int count, const qmc_problem* problems, bool need_two_shifts, Plan
     // in proportion to their cost; a tile is at least one index per thread and at most kMaxSteps (bounds the fp64 chains)
     for (auto& v : plan->variants) {
         const bool sector_variant = v.family == QMC_FAMILY_SECTOR || v.family == kKernelFamilyCSector || v.family == kKernelFamilySpec;
-        const int resident = kPlanSMs * (sector_variant ? min_blocks_sector(v.dp) : min_blocks_closed(v.dp, v.wide));
+        const int resident = kPlanSMs * (sector_variant ? min_blocks_sector(v.dp) : (v.gen_kind >= 0 ? min_blocks_generic(v.dp) : min_blocks_closed(v.dp, v.wide)));
         const int threads = v.family == kKernelFamilySpec ? spec_kernel_threads(module, v.spec_kernel)
                             : (v.family == QMC_FAMILY_SECTOR ? sector_threads(v.dp) : (v.family == kKernelFamilyCSector ? kCSectorThreads : kThreads));   // CTA size of the variant's kernel
         const int env = opt.tiles_target > 0 ? opt.tiles_target : 0;
@@ -386,6 +392,41 @@ int occupancy_closed(int family, int dp, bool wide, int group) {
     return -1;
 }
 #undef QMC_TRY_PARTS
+
+#define QMC_GENERIC_KINDS(FAM, PREFIX, ...)                      \
+    switch (kind) {                                               \
+        case 0: return PREFIX##FAM##_0(__VA_ARGS__);              \
+    }                                                             \
+    break;
+cudaError_t launch_generic(int family, int kind, int dp, int grid, cudaStream_t st, const FusedLaunch& a) {
+    switch (family) {
+        case 0: QMC_GENERIC_KINDS(0, launch_fused_generic_, dp, grid, st, a)
+        case 1: QMC_GENERIC_KINDS(1, launch_fused_generic_, dp, grid, st, a)
+        case 2: QMC_GENERIC_KINDS(2, launch_fused_generic_, dp, grid, st, a)
+        case 4: QMC_GENERIC_KINDS(4, launch_fused_generic_, dp, grid, st, a)
+    }
+    return cudaErrorInvalidValue;
+}
+int occupancy_generic_uncached(int family, int kind, int dp) {
+    switch (family) {
+        case 0: QMC_GENERIC_KINDS(0, occupancy_fused_generic_, dp)
+        case 1: QMC_GENERIC_KINDS(1, occupancy_fused_generic_, dp)
+        case 2: QMC_GENERIC_KINDS(2, occupancy_fused_generic_, dp)
+        case 4: QMC_GENERIC_KINDS(4, occupancy_fused_generic_, dp)
+    }
+    return -1;
+}
+#undef QMC_GENERIC_KINDS
+int occupancy_generic(int family, int kind, int dp) {
+    static int cache[kMaxDevices][kKernelFamilies][kGenKinds][17];
+    const int dev = current_device();
+    if (dev < 0 || kind < 0 || kind >= kGenKinds || dp > 16) return -1;
+    int& c = cache[dev][family][kind][dp];
+    if (c > 0) return c;
+    const int v = occupancy_generic_uncached(family, kind, dp);
+    if (v > 0) c = v;
+    return v;
+}
 
 int occupancy(int family, int dp, bool wide, int group = kGroup) {
     static int cache[kMaxDevices][kKernelFamilies][33][2][2];
@@ -508,7 +549,7 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
         std::memset(&queues[0], 0, sizeof(VariantQueue));
         queues[0].total_tiles = plan.variants[0].total_tiles;
         const Variant& v0 = plan.variants[0];
-        if (v0.total_tiles > (long long)sms * std::max(1, occupancy(v0.family, v0.dp, v0.wide, v0.group))) {
+        if (v0.total_tiles > (long long)sms * std::max(1, (v0.gen_kind >= 0 ? occupancy_generic(v0.family, v0.gen_kind, v0.dp) : occupancy(v0.family, v0.dp, v0.wide, v0.group)))) {
             // more tiles than resident CTAs: dynamic queue (one 8-byte reset); otherwise every CTA owns one tile
             queues[0].counter = reinterpret_cast<unsigned long long*>(ws + plan.off_counters);
             QMC_CUDA(cudaMemsetAsync(queues[0].counter, 0, sizeof(unsigned long long), st));
@@ -524,7 +565,7 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
     }
     for (size_t vi = 0; vi < plan.variants.size(); ++vi) {
         const Variant& v = plan.variants[vi];
-        const int occ = v.family == kKernelFamilySpec ? spec_occupancy(module, v.spec_kernel) : occupancy(v.family, v.dp, v.wide, v.group);
+        const int occ = v.family == kKernelFamilySpec ? spec_occupancy(module, v.spec_kernel) : (v.gen_kind >= 0 ? occupancy_generic(v.family, v.gen_kind, v.dp) : occupancy(v.family, v.dp, v.wide, v.group));
         if (occ <= 0 && v.family == kKernelFamilySpec) return QMC_ERR_CUDA;      // the loader left the text
         if (occ <= 0) return cuda_fail(cudaErrorInvalidDeviceFunction, "occupancy query (is the sm_100a image loadable on this device?)");
         const long long cap = (long long)sms * occ;
@@ -539,7 +580,9 @@ int run_batch(int count, const qmc_problem* problems, double* out_means, double*
         }
         cudaError_t e = cudaErrorInvalidValue;
         switch (v.family) {
-            case 0: case 1: case 2: case 4: e = launch_closed(v.family, v.dp, v.wide, v.group, grid, st, a); break;
+            case 0: case 1: case 2: case 4:
+                e = v.gen_kind >= 0 ? launch_generic(v.family, v.gen_kind, v.dp, grid, st, a) : launch_closed(v.family, v.dp, v.wide, v.group, grid, st, a);
+                break;
             case 3: e = launch_fused_f3(v.dp, v.wide, grid, st, a); break;
             case kKernelFamilyCSector: e = launch_fused_f8(v.dp, v.wide, grid, st, a); break;
         }
@@ -721,7 +764,7 @@ int qmc_plan_info(int count, const qmc_problem* problems, long long* out_tiles, 
         int ctas = 0;
         const int sms = sm_count();
         for (auto& v : plan.variants) {
-            const int occ = sms > 0 ? occupancy(v.family, v.dp, v.wide, v.group) : 0;
+            const int occ = sms > 0 ? (v.gen_kind >= 0 ? occupancy_generic(v.family, v.gen_kind, v.dp) : occupancy(v.family, v.dp, v.wide, v.group)) : 0;
             ctas += (int)std::min<long long>((long long)sms * std::max(occ, 0), v.total_tiles);
         }
         *out_ctas = ctas;
@@ -768,7 +811,7 @@ int qmc_batch_create(int count, const qmc_problem* problems, qmc_sector_module* 
     }
     if (rc == QMC_OK) {
         for (const Variant& v : b->plan.variants)        // fill the occupancy cache (a query is not a launch, but it is not capturable either)
-            if (v.family != kKernelFamilySpec && occupancy(v.family, v.dp, v.wide, v.group) <= 0)
+            if (v.family != kKernelFamilySpec && (v.gen_kind >= 0 ? occupancy_generic(v.family, v.gen_kind, v.dp) : occupancy(v.family, v.dp, v.wide, v.group)) <= 0)
                 rc = cuda_fail(cudaErrorInvalidDeviceFunction, "occupancy query (is the sm_100a image loadable on this device?)");
     }
     // the plan was staged from host memory that dies with this call

@@ -51,6 +51,10 @@ __host__ __device__ constexpr int sector_mono_stride(int family, int dim) { retu
 
 // transform kinds after host-side decoding
 enum : int { TR_NONE = 0, TR_BAKER = 1, TR_KOR3 = 2, TR_KORR = 3 };   // TR_KORR = the generic tile loop, see GEN_*
+// template-only codes of the dedicated generic kernels (fused_generic_kernel): TR_GEN0 + GEN_* kind, kind < kGenKinds, no fit map
+enum : int { TR_GEN0 = 4 };
+constexpr int kGenKinds = 1;           // GEN_KOROBOV_SYM only: Korobov (r0, r1) and Sidi measured slower as one basic block
+constexpr int min_blocks_generic(int dp) { return dp <= 8 ? 4 : 3; }   // resident CTAs per SM of the dedicated generic kernels
 // The generic tile loop serves every transform (selected per coordinate by DevProblem::gen = kind | r0 << 4 | r1 << 8)
 // and every fit mode at run time; the specialised loops are none / baker / Korobov-3 x (no fit, cubic fit).
 enum : int { GEN_KOROBOV_SYM = 0, GEN_KOROBOV_ASYM = 1, GEN_SIDI = 2, GEN_NONE = 3, GEN_BAKER = 4 };

@@ -42,6 +42,14 @@ QMC_DECLARE_FAMILY(0) QMC_DECLARE_FAMILY(1) QMC_DECLARE_FAMILY(2) QMC_DECLARE_FA
 QMC_DECLARE_PART(1, 4)     // product peak, <= 8 slots, 8 shifts per group
 #undef QMC_DECLARE_FAMILY
 #undef QMC_DECLARE_PART
+// dedicated kernels of the generic weight transforms (qmc_fused_generic.cu): family x GEN_* kind
+#define QMC_DECLARE_GENERIC(FAM, KIND)                                                                              \
+    cudaError_t launch_fused_generic_##FAM##_##KIND(int dp, int grid, cudaStream_t st, const FusedLaunch& a);       \
+    int occupancy_fused_generic_##FAM##_##KIND(int dp);
+#define QMC_DECLARE_GENERIC_FAMILY(FAM) QMC_DECLARE_GENERIC(FAM, 0)
+QMC_DECLARE_GENERIC_FAMILY(0) QMC_DECLARE_GENERIC_FAMILY(1) QMC_DECLARE_GENERIC_FAMILY(2) QMC_DECLARE_GENERIC_FAMILY(4)
+#undef QMC_DECLARE_GENERIC_FAMILY
+#undef QMC_DECLARE_GENERIC
 cudaError_t launch_fused_f3(int dp, bool wide, int grid, cudaStream_t st, const FusedLaunch& a);
 int occupancy_fused_f3(int dp, bool wide);
 cudaError_t launch_fused_f8(int dp, bool wide, int grid, cudaStream_t st, const FusedLaunch& a);   // complex sector family

@@ -1025,3 +1025,16 @@ def test_product_peak_group_of_8_shifts(d, m):
         assert a[0][0].tobytes() == b[0][0].tobytes() == c[0][0].tobytes()
         assert a[1].tobytes() == b[1].tobytes() and a[2].tobytes() == b[2].tobytes()
     check_against_oracle([p], group=8)
+
+
+@pytest.mark.parametrize("fam", [0, 1, 2, 5])
+@pytest.mark.parametrize("d", [2, 4, 6, 8, 11, 16])
+def test_dedicated_korobov_kernels_and_the_generic_call_path(fam, d):
+    """Korobov r != 3 without a fit map runs in kernels of its own (the transform kind fixed at compile time); the generic loop
+    inside the family's kernel still serves it on request -- both against the oracle, every r, ragged tiles"""
+    probs = [make(fam, d, n, 5, K + r, 9600 + 7 * d + r) for r, n in ((1, 8191), (2, 127), (4, 65537), (5, 4099), (6, 1021))]
+    check_against_oracle(probs)
+    check_against_oracle(probs, generic_call=True)
+    a = run_gpu(probs)
+    b = run_gpu(probs)
+    assert all(x.tobytes() == y.tobytes() for x, y in zip(a[0], b[0]))
