@@ -179,3 +179,30 @@ def fit_cubic_cdf(xs, cdf):
     out = np.zeros((d, 6))
     lib().oracle_fit_cubic_cdf(_d(xs), _d(cdf), d, K, _d(out))
     return out
+
+
+def fit_polysingular_pairs(c, e, start45=(1.0, 0.0)):
+    """The complete fit function of Eq. 19 fitted to pairs (c_i, e_i), p(c_i) ~ e_i, by bounded non-linear least
+    squares with the parameter bounds of PAPER.md L231 (a0 >= 1.001, a1 <= -0.001, a2, a3 >= 0); a6 = 1 - a2 - a3 - a4 - a5 by
+    p(1) = 1.  The paper runs GSL's Levenberg-Marquardt; the oracle takes scipy.optimize.least_squares (trust-region reflective,
+    the library's bounded solver) from two starts -- dormant and small active poles, since the gradient in a0, a1 vanishes while
+    a2 = a3 = 0 -- and returns (best parameters a0..a5, sum of squared residuals).  The minimiser is not unique (a dormant pole's
+    position is free): what compares across implementations is the residual, not the parameters."""
+    from scipy.optimize import least_squares
+    c = np.asarray(c, dtype=np.float64)
+    e = np.asarray(e, dtype=np.float64)
+
+    def p_of(a, y):
+        a6 = 1.0 - a[2] - a[3] - a[4] - a[5]
+        return a[2] * y * (a[0] - 1.0) / (a[0] - y) + a[3] * y * (a[1] - 1.0) / (a[1] - y) + y * (a[4] + y * (a[5] + y * a6))
+
+    lo = [1.001, -np.inf, 0.0, 0.0, -np.inf, -np.inf]
+    hi = [np.inf, -0.001, np.inf, np.inf, np.inf, np.inf]
+    best, best_cost = None, np.inf
+    for a2 in (0.0, 0.05):
+        x0 = np.array([1.1, -0.1, a2, a2, start45[0], start45[1]])
+        sol = least_squares(lambda a: p_of(a, c) - e, x0, bounds=(lo, hi), method="trf", xtol=1e-15, ftol=1e-15, gtol=1e-15, max_nfev=4000)
+        cost = float(np.sum(sol.fun ** 2))
+        if cost < best_cost:
+            best, best_cost = sol.x.copy(), cost
+    return best, best_cost

@@ -465,3 +465,38 @@ def test_integrate_batch_rejects_before_touching_the_device():
     unused = shifts.copy()
     unused[2, 5] = 7.0
     assert status([dict(good, dim=7)], shifts=unused) == -2
+
+
+def _peak_cdf_pairs(a, w, count=400):
+    """marginal of the product peak 1 / (a^-2 + (x - w)^2) in closed form: pairs (CDF(x_t), x_t)"""
+    x = np.linspace(0.0025, 0.9975, count)
+    cdf = (np.arctan(a * (x - w)) + np.arctan(a * w)) / (np.arctan(a * (1 - w)) + np.arctan(a * w))
+    return cdf, x
+
+
+def test_polysingular_fit_against_the_library_solver():
+    """the bounded Levenberg-Marquardt of the product (qmc_fit.cu) against the oracle's fit of the same function with the same
+    bounds by scipy.optimize.least_squares: the same residual, and -- where both poles are active and the
+    minimum is unique -- the same parameters; on data generated from the model both reach a zero residual"""
+    def sse(a, c, e):
+        return float(sum((oracle.fit_map(a, y)[0] - t) ** 2 for y, t in zip(c, e)))
+
+    for truth in ([1.05, -0.4, 0.35, 0.0, 0.30, 0.25], [1.6, -0.03, 0.0, 0.45, 0.35, 0.10]):
+        c = np.linspace(0.002, 0.998, 400)
+        e = np.array([oracle.fit_map(np.array(truth), y)[0] for y in c])
+        a_or, cost_or = oracle.fit_polysingular_pairs(c, e)
+        assert cost_or < 1e-24                                # pins the oracle's model against the C++ oracle's fit_map
+        full = binding.qmc_fit_from_cdf(e[None, :], c[None, :], with_poles=True)[0]
+        assert sse(full, c, e) < 1e-24
+    for a, w in ((6.0, 0.4), (12.0, 0.03), (40.0, 0.7), (3.0, 0.9)):
+        c, e = _peak_cdf_pairs(a, w)
+        cub = binding.qmc_fit_from_cdf(e[None, :], c[None, :], with_poles=False)[0]
+        full = binding.qmc_fit_from_cdf(e[None, :], c[None, :], with_poles=True)[0]
+        a_or, cost_or = oracle.fit_polysingular_pairs(c, e, start45=(cub[4], cub[5]))
+        cost = sse(full, c, e)
+        assert cost <= cost_or * (1 + 1e-3) + 1e-18, (a, w, cost, cost_or)
+        assert cost_or <= cost * (1 + 1e-3) + 1e-18, (a, w, cost, cost_or)           # neither solver beats the other
+        assert cost < 1e-3 * sse(cub, c, e)                   # the poles matter for a peak
+        if full[2] > 1e-3 and full[3] > 1e-3:
+            np.testing.assert_allclose(full, a_or, rtol=1e-4, atol=1e-6)
+        assert binding.qmc_validate_problem_host(dict(_cfg0(), fit_coeffs=np.tile(full, (4, 1)))) == 0
