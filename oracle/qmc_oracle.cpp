@@ -30,8 +30,8 @@
 // the sector family at d<=3; x0*x1*x2 -> 1/8 (Fig. 2); log factors of the sector family by one-dimensional
 // closed forms and the eps-derivative identity; Eq. 3 on hand-made means; projection marginals in
 // closed form; fit recovers an exact cubic.
-// Parity unpinned: nothing in this file (the CBC tool and the Levenberg-Marquardt fit of the product are not part of the
-// oracle).
+// Parity unpinned: nothing in this file (the CBC tool is not part of the oracle; the bounded fit of Eq. 19 has its oracle
+// counterpart in oracle/__init__.py: fit_polysingular_pairs).
 //
 // Build: g++ -O2 -std=c++17 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/build.py).
 #include <algorithm>
