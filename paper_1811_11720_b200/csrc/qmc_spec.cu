@@ -169,27 +169,33 @@ int emit_case(const HostSector& hs, int d, const SlotKind& sk, const std::vector
     auto fresh = [&]() { return "t" + std::to_string(++nt); };
     std::vector<std::string> val[2];                       // U, F at the G points
     const HostPoly* pol[2] = {&hs.U, &hs.F};
-    for (int k = 0; k < 2; ++k) {
-        const HostPoly& hp = *pol[k];
-        std::vector<std::string> S(G, imm(hp.c0)), A(G, imm(0.0));
-        int si = 0;
-        for (unsigned char code : hp.ops) {
+    // U and F are independent: their steps are written out alternately, so that the assembler's scheduling window always holds
+    // two polynomials' worth of independent chains (each polynomial's own operations keep their order: the values do not change)
+    std::vector<std::string> S[2], A[2];
+    size_t at[2] = {0, 0};
+    int si[2] = {0, 0};
+    for (int k = 0; k < 2; ++k) { S[k].assign(G, imm(pol[k]->c0)); A[k].assign(G, imm(0.0)); }
+    while (at[0] < hs.U.ops.size() || at[1] < hs.F.ops.size()) {
+        for (int k = 0; k < 2; ++k) {
+            const HostPoly& hp = *pol[k];
+            if (at[k] >= hp.ops.size()) continue;
+            const unsigned char code = hp.ops[at[k]++];
             const int j = (code - SEC_BASE) / kSecKinds, kind = (code - SEC_BASE) % kSecKinds;
             std::string cf, cf2;
-            if (kind == SEC_SL || kind == SEC_AL || kind == SEC_ALI) { cf = imm(hp.slots[2 * si]); cf2 = imm(hp.slots[2 * si + 1]); ++si; }
+            if (kind == SEC_SL || kind == SEC_AL || kind == SEC_ALI) { cf = imm(hp.slots[2 * si[k]]); cf2 = imm(hp.slots[2 * si[k] + 1]); ++si[k]; }
             for (int q = 0; q < G; ++q) {
                 const std::string t = fresh();
                 switch (kind) {
-                    case SEC_SC: out.line("fma.rn.f64 %s, %s, %s, %s;", t.c_str(), A[q].c_str(), x(q, j), S[q].c_str()); S[q] = t; break;
-                    case SEC_SL: out.line("fma.rn.f64 %s, %s, %s, %s;", t.c_str(), cf.c_str(), x(q, j), S[q].c_str()); S[q] = t; break;
-                    case SEC_AL: out.line("fma.rn.f64 %s, %s, %s, %s;", t.c_str(), cf.c_str(), x(q, j), A[q].c_str()); A[q] = t; break;
-                    case SEC_ALI: out.line("fma.rn.f64 %s, %s, %s, %s;", t.c_str(), cf.c_str(), x(q, j), cf2.c_str()); A[q] = t; break;
-                    default: out.line("mul.rn.f64 %s, %s, %s;", t.c_str(), A[q].c_str(), x(q, j)); A[q] = t; break;
+                    case SEC_SC: out.line("fma.rn.f64 %s, %s, %s, %s;", t.c_str(), A[k][q].c_str(), x(q, j), S[k][q].c_str()); S[k][q] = t; break;
+                    case SEC_SL: out.line("fma.rn.f64 %s, %s, %s, %s;", t.c_str(), cf.c_str(), x(q, j), S[k][q].c_str()); S[k][q] = t; break;
+                    case SEC_AL: out.line("fma.rn.f64 %s, %s, %s, %s;", t.c_str(), cf.c_str(), x(q, j), A[k][q].c_str()); A[k][q] = t; break;
+                    case SEC_ALI: out.line("fma.rn.f64 %s, %s, %s, %s;", t.c_str(), cf.c_str(), x(q, j), cf2.c_str()); A[k][q] = t; break;
+                    default: out.line("mul.rn.f64 %s, %s, %s;", t.c_str(), A[k][q].c_str(), x(q, j)); A[k][q] = t; break;
                 }
             }
         }
-        val[k] = S;
     }
+    val[0] = S[0]; val[1] = S[1];
     // num = W prod_j x_j^nu_j U^a, den = F^b: the multiplications of the interpreting kernel, in its order
     for (int q = 0; q < G; ++q) {
         std::string n = W(q);
@@ -241,30 +247,35 @@ int emit_case_complex(const HostSector& hs, int d, const SlotKind& sk, const std
     };
     std::vector<std::string> vr[2], vi[2];                  // U, F at the G points
     const HostPoly* pol[2] = {&hs.U, &hs.F};
-    for (int k = 0; k < 2; ++k) {
-        const HostPoly& hp = *pol[k];
-        std::vector<std::string> Sr(G, imm(hp.c0)), Si(G, imm(hp.c0i)), Ar(G, imm(0.0)), Ai(G, imm(0.0));
-        int si = 0;
-        for (unsigned char code : hp.ops) {
+    // U and F alternately, step by step (see emit_case)
+    std::vector<std::string> Sr[2], Si[2], Ar[2], Ai[2];
+    size_t at[2] = {0, 0};
+    int si[2] = {0, 0};
+    for (int k = 0; k < 2; ++k) { Sr[k].assign(G, imm(pol[k]->c0)); Si[k].assign(G, imm(pol[k]->c0i)); Ar[k].assign(G, imm(0.0)); Ai[k].assign(G, imm(0.0)); }
+    while (at[0] < hs.U.ops.size() || at[1] < hs.F.ops.size()) {
+        for (int k = 0; k < 2; ++k) {
+            const HostPoly& hp = *pol[k];
+            if (at[k] >= hp.ops.size()) continue;
+            const unsigned char code = hp.ops[at[k]++];
             const int j = (code - SEC_BASE) / kSecKinds, kind = (code - SEC_BASE) % kSecKinds;
             std::string cr, ci, c2r, c2i;
             if (kind == SEC_SL || kind == SEC_AL || kind == SEC_ALI) {
-                cr = imm(hp.slots[4 * si]); ci = imm(hp.slots[4 * si + 1]); c2r = imm(hp.slots[4 * si + 2]); c2i = imm(hp.slots[4 * si + 3]);
-                ++si;
+                cr = imm(hp.slots[4 * si[k]]); ci = imm(hp.slots[4 * si[k] + 1]); c2r = imm(hp.slots[4 * si[k] + 2]); c2i = imm(hp.slots[4 * si[k] + 3]);
+                ++si[k];
             }
             for (int q = 0; q < G; ++q) {
                 const std::string X = x(q, j);
                 switch (kind) {
-                    case SEC_SC: Sr[q] = op3("fma.rn.f64", Ar[q], X, Sr[q]); Si[q] = op3("fma.rn.f64", Ai[q], X, Si[q]); break;
-                    case SEC_SL: Sr[q] = op3("fma.rn.f64", cr, X, Sr[q]); Si[q] = op3("fma.rn.f64", ci, X, Si[q]); break;
-                    case SEC_AL: Ar[q] = op3("fma.rn.f64", cr, X, Ar[q]); Ai[q] = op3("fma.rn.f64", ci, X, Ai[q]); break;
-                    case SEC_ALI: Ar[q] = op3("fma.rn.f64", cr, X, c2r); Ai[q] = op3("fma.rn.f64", ci, X, c2i); break;
-                    default: Ar[q] = mul(Ar[q], X); Ai[q] = mul(Ai[q], X); break;
+                    case SEC_SC: Sr[k][q] = op3("fma.rn.f64", Ar[k][q], X, Sr[k][q]); Si[k][q] = op3("fma.rn.f64", Ai[k][q], X, Si[k][q]); break;
+                    case SEC_SL: Sr[k][q] = op3("fma.rn.f64", cr, X, Sr[k][q]); Si[k][q] = op3("fma.rn.f64", ci, X, Si[k][q]); break;
+                    case SEC_AL: Ar[k][q] = op3("fma.rn.f64", cr, X, Ar[k][q]); Ai[k][q] = op3("fma.rn.f64", ci, X, Ai[k][q]); break;
+                    case SEC_ALI: Ar[k][q] = op3("fma.rn.f64", cr, X, c2r); Ai[k][q] = op3("fma.rn.f64", ci, X, c2i); break;
+                    default: Ar[k][q] = mul(Ar[k][q], X); Ai[k][q] = mul(Ai[k][q], X); break;
                 }
             }
         }
-        vr[k] = Sr; vi[k] = Si;
     }
+    for (int k = 0; k < 2; ++k) { vr[k] = Sr[k]; vi[k] = Si[k]; }
     auto in_register = [&](const std::string& v) {           // a polynomial without steps is a constant: through a register
         if (v[0] != '0') return v;
         const std::string t = fresh();
