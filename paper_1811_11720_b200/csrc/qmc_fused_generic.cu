@@ -1,5 +1,6 @@
 // Dedicated kernels of the generic weight transforms (fused_generic_kernel, qmc_fused.cuh); compiled once per
-// (-DQMC_FAM=0, 1, 2 or 4, -DQMC_KIND=0 symmetric Korobov r, 1 Korobov (r0, r1), 2 Sidi r) by build.py.
+// (-DQMC_FAM=0, 1, 2 or 4, -DQMC_KIND=<GEN_* kind>) by build.py.  Only kind 0, the symmetric Korobov weights, is built and
+// routed (kGenKinds): Korobov (r0, r1) and Sidi compile here too but ran slower than the generic loop.
 #ifndef QMC_FAM
 #error "compile with -DQMC_FAM=<family> -DQMC_KIND=<GEN_* kind> (see paper_1811_11720_b200/build.py)"
 #endif
