@@ -331,7 +331,8 @@ int qmc_sector_compile(const double* params /*HOST*/, int n_params, int dim, uns
  * integration starts).  A C ABI carries parameter blocks instead, which the default kernels interpret step by step; a MODULE
  * gives the compiled route back: qmc_sector_module_create translates every QMC_FAMILY_SECTOR problem of a batch into
  * straight-line sm_100a code -- the same operations in the same order as the interpreting kernel, so both return the same bits --
- * inside copies of the fused kernel (up to `sectors_per_kernel` sectors per kernel, 0 = 32; at most 63 kernels per batch),
+ * inside copies of the fused kernel (up to `sectors_per_kernel` sectors per kernel; 0 = 32, doubled until the batch needs at most
+ * 48 kernels; a batch call serves at most 64 kernel variants in all and returns QMC_ERR_WORKSPACE beyond),
  * assembled on the HOST with the CUDA toolkit's nvJitLink (opened at run time; QMC_ERR_CUDA with the assembler's text in
  * qmc_last_cuda_error if that fails), kernels in parallel on the host's cores.  It needs no GPU.  Used of each problem:
  * family, dim, n_params and params (HOST pointer; read during the call only); everything else is ignored, so one module

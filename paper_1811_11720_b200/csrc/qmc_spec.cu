@@ -501,7 +501,8 @@ int qmc_sector_module_create(int count, const qmc_problem* problems, int sectors
     *out = nullptr;
     if (count < 1) return QMC_ERR_N;
     if (sectors_per_kernel < 0 || sectors_per_kernel > 1024) return QMC_ERR_N;
-    if (sectors_per_kernel == 0) sectors_per_kernel = 32;
+    const bool auto_size = sectors_per_kernel == 0;
+    if (auto_size) sectors_per_kernel = 32;
     const Template& tpl = kernel_template();
     if (!tpl.ok) { report_cuda_error(cudaErrorUnknown, "the embedded kernel template has no usable marker"); return QMC_ERR_CUDA; }
     const auto t0 = std::chrono::steady_clock::now();
@@ -518,6 +519,13 @@ int qmc_sector_module_create(int count, const qmc_problem* problems, int sectors
         const int kind = slot_kind_of(sector_dim_slots(p.dim), cplx);
         if (kind < 0 || !compile_sector_host(p.params, p.n_params, p.dim, cplx, &sectors[i])) continue;   // the interpreting kernel reports a bad block
         by_kind[kind].push_back(i);
+    }
+    if (auto_size) {
+        // a batch call serves at most 64 kernel variants: with many sectors, more of them share a kernel (at most kMaxAutoKernels
+        // kernels, the rest of the variants is left to the batch's other families)
+        constexpr size_t kMaxAutoKernels = 48;
+        auto kernels_at = [&](size_t per) { size_t n = 0; for (auto& v : by_kind) n += (v.size() + per - 1) / per; return n; };
+        while (kernels_at((size_t)sectors_per_kernel) > kMaxAutoKernels && sectors_per_kernel < 1024) sectors_per_kernel *= 2;
     }
     for (int kind = 0; kind < kSlotKindCount; ++kind)
         for (size_t b = 0; b < by_kind[kind].size(); b += (size_t)sectors_per_kernel) {

@@ -500,3 +500,15 @@ def test_polysingular_fit_against_the_library_solver():
         if full[2] > 1e-3 and full[3] > 1e-3:
             np.testing.assert_allclose(full, a_or, rtol=1e-4, atol=1e-6)
         assert binding.qmc_validate_problem_host(dict(_cfg0(), fit_coeffs=np.tile(full, (4, 1)))) == 0
+
+
+def test_sector_module_sizes_its_kernels_for_large_batches():
+    """with sectors_per_kernel = 0 a large batch shares kernels so that a batch call's variant limit (64) is not hit"""
+    rng = synth.MT19937_64(1234)
+    blocks = [synth.sector(rng, 3, n_lo=2, n_span=2) for _ in range(40)]
+    probs = [synth.problem(3, blocks[i % 40], 1021, synth.korobov_form_vector(1021, 3, 341), synth.draw_shifts(rng, 2, 3),
+                           synth.TRANSFORM_KOROBOV + 3, name=f"s{i}") for i in range(1600)]
+    mod = binding.SectorModule(probs)
+    info = mod.info
+    assert info["specialised"] == 1600 and info["kernels"] <= 48 and info["kernels"] * 64 >= 1600
+    assert binding.SectorModule(probs[:100], sectors_per_kernel=25).info["kernels"] == 4
