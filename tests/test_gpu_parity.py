@@ -1038,3 +1038,21 @@ def test_dedicated_korobov_kernels_and_the_generic_call_path(fam, d):
     a = run_gpu(probs)
     b = run_gpu(probs)
     assert all(x.tobytes() == y.tobytes() for x, y in zip(a[0], b[0]))
+
+
+def test_prepared_batch_of_one_closed_form_problem_and_an_empty_module():
+    """the degenerate ends: one closed-form problem (its plan travels in the kernel parameter, nothing to set up) as a prepared
+    batch, and a module that found nothing to specialise (no kernels) in a batch call"""
+    p = make(1, 8, 262147, 8, BAKER, 9401)
+    ref = run_gpu([p])
+    one = binding.DeviceBatch([p]).prepare()
+    for _ in range(2):
+        assert one.launch() == 2                              # fused kernel + finalize
+        out = one.results()
+        assert out[0][0].tobytes() == ref[0][0].tobytes() and out[2].tobytes() == ref[2].tobytes()
+    probs = [p, make(0, 4, 4099, 4, K + 3, 9402)]
+    empty = binding.SectorModule(probs)
+    assert empty.info["kernels"] == 0 and empty.info["specialised"] == 0
+    a = run_gpu(probs)
+    b = run_gpu(probs, module=empty)
+    assert all(x.tobytes() == y.tobytes() for x, y in zip(a[0], b[0]))
