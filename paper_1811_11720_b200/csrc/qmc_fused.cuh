@@ -24,6 +24,10 @@
 
 #include "qmc_device.cuh"
 
+#ifndef QMC_PAIR_DIMS
+#define QMC_PAIR_DIMS 1
+#endif
+
 namespace qmc {
 
 template <int FAMILY> struct FamTraits;
@@ -366,6 +370,9 @@ struct EvalCtx {            // per-tile constants held in registers
     int fam_kind, fam_pow;  // kernel family 4: public family id and the corner-peak exponent d + 1
 };
 
+// resident CTAs per SM the register budget is sized for (128 / 168 / 255 registers per thread)
+template <int DP, bool WIDE> struct MinBlocks { static constexpr int value = min_blocks_closed(DP, WIDE); };
+
 template <int FAMILY, int DP, int G, bool WIDE, int TR, int FIT>
 __device__ __forceinline__ void eval_point_group(const typename Res<WIDE>::T (&r)[DP], const EvalCtx& cx,
                                                  double (&acc)[G][FamTraits<FAMILY>::NC]) {
@@ -398,8 +405,74 @@ __device__ __forceinline__ void eval_point_group(const typename Res<WIDE>::T (&r
             for (int q = 0; q < G; ++q) fam_dim<FAMILY>(s0[q], s1[q], xg[q], fa, fb, cx.fam_kind);
         }
     }
+    // Korobov-3 (no fit map / cubic fit map): two dimensions at a time, written stage by stage across the 2 G coordinates, so that
+    // the assembler's scheduling window holds twice the independent chains; every coordinate sees the same operations and the
+    // products over the dimensions keep their order, so the values are those of the one-dimension-at-a-time form bit for bit
+    // (only in the kernels with the 168-register budget, 16 slots: measured, configs[4] 419.4 -> 413.9 ms; at 12 slots and 128 registers
+    // configs[2] lost 1.5 % to the registers the second dimension holds)
+    constexpr bool PAIRED = QMC_PAIR_DIMS && TR == TR_KOR3 && (FIT == 0 || FIT == 1) && DP % 2 == 0 && !WIDE && MinBlocks<DP, WIDE>::value == 3;
+    if constexpr (PAIRED) {
 #pragma unroll
-    for (int j = 0; j < (TR >= TR_GEN0 ? 0 : DP); ++j) {
+        for (int j = 0; j < DP; j += 2) {
+            double fa[2], fb[2], dl[2][G], rd[2], c[2][G], sq[2][G], g[2][G], x[2][G];
+            FitC fc[2];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                rd[h] = Res<WIDE>::to_double(r[j + h]);
+                load_slot<DP, G, FIT>(cx.sbase, cx.delta, j + h, cx.fit_mode, fa[h], fb[h], fc[h], dl[h]);
+            }
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int q = 0; q < G; ++q) c[h][q] = centre_c(coord_t(rd[h], cx.inv_n, dl[h][q]));
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int q = 0; q < G; ++q) sq[h][q] = c[h][q] * c[h][q];
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int q = 0; q < G; ++q) g[h][q] = __fma_rn(-20.0, sq[h][q], 21.0);
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int q = 0; q < G; ++q) g[h][q] = __fma_rn(g[h][q], sq[h][q], -8.75);
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int q = 0; q < G; ++q) g[h][q] = __fma_rn(g[h][q], sq[h][q], 2.1875);
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int q = 0; q < G; ++q) x[h][q] = __fma_rn(c[h][q], g[h][q], 0.5);
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int q = 0; q < G; ++q) P[q] = __dmul_rn(P[q], __dadd_rn(0.25, -sq[h][q]));
+            if constexpr (FIT == 1) {
+                double dp[2][G];
+#pragma unroll
+                for (int h = 0; h < 2; ++h)
+#pragma unroll
+                    for (int q = 0; q < G; ++q) {
+                        const double y = x[h][q];
+                        const double hh = __fma_rn(y, __fma_rn(y, fc[h].f2, fc[h].f1), fc[h].f0);
+                        dp[h][q] = __fma_rn(y, __fma_rn(y, fc[h].f4, fc[h].f3), fc[h].f0);
+                        x[h][q] = y * hh;
+                    }
+#pragma unroll
+                for (int h = 0; h < 2; ++h)
+#pragma unroll
+                    for (int q = 0; q < G; ++q) D[q] *= dp[h][q];
+            }
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int q = 0; q < G; ++q) fam_dim<FAMILY>(s0[q], s1[q], x[h][q], fa[h], fb[h], cx.fam_kind);
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < ((TR >= TR_GEN0 || PAIRED) ? 0 : DP); ++j) {
         const double rd = Res<WIDE>::to_double(r[j]);
         double fa, fb, dl[G];
         FitC fc;
@@ -695,8 +768,6 @@ __device__ __forceinline__ bool next_tile(SmemCtx<DP, G, NT>& sm, const FusedLau
     return true;
 }
 
-// resident CTAs per SM the register budget is sized for (128 / 168 / 255 registers per thread)
-template <int DP, bool WIDE> struct MinBlocks { static constexpr int value = min_blocks_closed(DP, WIDE); };
 
 template <int FAMILY, int DP, int G, bool WIDE>
 __global__ void __launch_bounds__(kThreads, MinBlocks<DP, WIDE>::value) fused_kernel(const __grid_constant__ FusedLaunch L) {
