@@ -27,6 +27,9 @@
 #ifndef QMC_PAIR_DIMS
 #define QMC_PAIR_DIMS 1
 #endif
+#ifndef QMC_PAIR_ND
+#define QMC_PAIR_ND 2
+#endif
 
 namespace qmc {
 
@@ -412,47 +415,48 @@ __device__ __forceinline__ void eval_point_group(const typename Res<WIDE>::T (&r
     // configs[2] lost 1.5 % to the registers the second dimension holds)
     constexpr bool PAIRED = QMC_PAIR_DIMS && TR == TR_KOR3 && (FIT == 0 || FIT == 1) && DP % 2 == 0 && !WIDE && MinBlocks<DP, WIDE>::value == 3;
     if constexpr (PAIRED) {
+        constexpr int ND = QMC_PAIR_ND;
 #pragma unroll
-        for (int j = 0; j < DP; j += 2) {
-            double fa[2], fb[2], dl[2][G], rd[2], c[2][G], sq[2][G], g[2][G], x[2][G];
-            FitC fc[2];
+        for (int j = 0; j < DP; j += ND) {
+            double fa[ND], fb[ND], dl[ND][G], rd[ND], c[ND][G], sq[ND][G], g[ND][G], x[ND][G];
+            FitC fc[ND];
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
+            for (int h = 0; h < ND; ++h) {
                 rd[h] = Res<WIDE>::to_double(r[j + h]);
                 load_slot<DP, G, FIT>(cx.sbase, cx.delta, j + h, cx.fit_mode, fa[h], fb[h], fc[h], dl[h]);
             }
 #pragma unroll
-            for (int h = 0; h < 2; ++h)
+            for (int h = 0; h < ND; ++h)
 #pragma unroll
                 for (int q = 0; q < G; ++q) c[h][q] = centre_c(coord_t(rd[h], cx.inv_n, dl[h][q]));
 #pragma unroll
-            for (int h = 0; h < 2; ++h)
+            for (int h = 0; h < ND; ++h)
 #pragma unroll
                 for (int q = 0; q < G; ++q) sq[h][q] = c[h][q] * c[h][q];
 #pragma unroll
-            for (int h = 0; h < 2; ++h)
+            for (int h = 0; h < ND; ++h)
 #pragma unroll
                 for (int q = 0; q < G; ++q) g[h][q] = __fma_rn(-20.0, sq[h][q], 21.0);
 #pragma unroll
-            for (int h = 0; h < 2; ++h)
+            for (int h = 0; h < ND; ++h)
 #pragma unroll
                 for (int q = 0; q < G; ++q) g[h][q] = __fma_rn(g[h][q], sq[h][q], -8.75);
 #pragma unroll
-            for (int h = 0; h < 2; ++h)
+            for (int h = 0; h < ND; ++h)
 #pragma unroll
                 for (int q = 0; q < G; ++q) g[h][q] = __fma_rn(g[h][q], sq[h][q], 2.1875);
 #pragma unroll
-            for (int h = 0; h < 2; ++h)
+            for (int h = 0; h < ND; ++h)
 #pragma unroll
                 for (int q = 0; q < G; ++q) x[h][q] = __fma_rn(c[h][q], g[h][q], 0.5);
 #pragma unroll
-            for (int h = 0; h < 2; ++h)
+            for (int h = 0; h < ND; ++h)
 #pragma unroll
                 for (int q = 0; q < G; ++q) P[q] = __dmul_rn(P[q], __dadd_rn(0.25, -sq[h][q]));
             if constexpr (FIT == 1) {
-                double dp[2][G];
+                double dp[ND][G];
 #pragma unroll
-                for (int h = 0; h < 2; ++h)
+                for (int h = 0; h < ND; ++h)
 #pragma unroll
                     for (int q = 0; q < G; ++q) {
                         const double y = x[h][q];
@@ -461,12 +465,12 @@ __device__ __forceinline__ void eval_point_group(const typename Res<WIDE>::T (&r
                         x[h][q] = y * hh;
                     }
 #pragma unroll
-                for (int h = 0; h < 2; ++h)
+                for (int h = 0; h < ND; ++h)
 #pragma unroll
                     for (int q = 0; q < G; ++q) D[q] *= dp[h][q];
             }
 #pragma unroll
-            for (int h = 0; h < 2; ++h)
+            for (int h = 0; h < ND; ++h)
 #pragma unroll
                 for (int q = 0; q < G; ++q) fam_dim<FAMILY>(s0[q], s1[q], x[h][q], fa[h], fb[h], cx.fam_kind);
         }
