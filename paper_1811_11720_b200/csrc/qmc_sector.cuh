@@ -24,6 +24,10 @@
 #include "qmc_fused.cuh"
 #include "qmc_sector_compile.h"
 
+#ifndef QMC_SECTOR_PAIR_DIMS
+#define QMC_SECTOR_PAIR_DIMS 1
+#endif
+
 namespace qmc {
 
 constexpr int kSecMaxSlots = sector_slot_words(2 * kMaxSectorMono) / 2;   // coefficient slots of a program: one per monomial + end-of-polynomial + read-ahead
@@ -120,8 +124,50 @@ __device__ __forceinline__ void sector_coords(const typename Res<WIDE>::T (&r)[D
     double P[G], D[G];
 #pragma unroll
     for (int q = 0; q < G; ++q) { P[q] = 1.0; D[q] = 1.0; }
+    // Korobov-3 without a fit map: two dimensions per stage (see eval_point_group, PAIRED)
+    constexpr bool PAIRED = QMC_SECTOR_PAIR_DIMS && TR == TR_KOR3 && FIT == 0 && DP % 2 == 0;
+    if constexpr (PAIRED) {
 #pragma unroll
-    for (int j = 0; j < DP; ++j) {
+        for (int j = 0; j < DP; j += 2) {
+            double fa, fb, dl[2][G], rd[2], c[2][G], sq[2][G], g[2][G];
+            FitC fc;
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                rd[h] = Res<WIDE>::to_double(r[j + h]);
+                load_slot<DP, G, 0>(cx.sbase, cx.delta, j + h, 0, fa, fb, fc, dl[h]);
+            }
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int q = 0; q < G; ++q) c[h][q] = centre_c(coord_t(rd[h], cx.inv_n, dl[h][q]));
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int q = 0; q < G; ++q) sq[h][q] = c[h][q] * c[h][q];
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int q = 0; q < G; ++q) g[h][q] = __fma_rn(-20.0, sq[h][q], 21.0);
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int q = 0; q < G; ++q) g[h][q] = __fma_rn(g[h][q], sq[h][q], -8.75);
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int q = 0; q < G; ++q) g[h][q] = __fma_rn(g[h][q], sq[h][q], 2.1875);
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int q = 0; q < G; ++q) x[q][j + h] = __fma_rn(c[h][q], g[h][q], 0.5);
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int q = 0; q < G; ++q) P[q] = __dmul_rn(P[q], __dadd_rn(0.25, -sq[h][q]));
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < (PAIRED ? 0 : DP); ++j) {
         const double rd = Res<WIDE>::to_double(r[j]);
         double fa, fb, dl[G];
         FitC fc;
