@@ -58,9 +58,9 @@ ALG_FP64_PER_EVAL = {
 }
 # thread-level FP64-pipe instructions per evaluation the fused kernels EXECUTE (ncu smsp__inst_executed_pipe_fp64 x 32 / evaluations;
 # profiles/r2_dram_full.md): the conversion of the residues, padded slots and the interpreter's bookkeeping on top of the above
-EXECUTED_FP64_PER_EVAL = {1: 55.03, 2: 171.4, 3: 100.4, "3s": 100.44, 4: 279.29}     # "3s": configs[3] through the specialised kernels (profiles/r2_spec_full.md)
+EXECUTED_FP64_PER_EVAL = {1: 55.03, 2: 171.4, 3: 101.42, "3s": 100.44, 4: 279.29}     # "3s": configs[3] through the specialised kernels (profiles/r2_spec_full.md)
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused kernel at FULL size (ncu, profiles/r2_dram_full.md)
-PROFILED_DRAM_BYTES_PER_LAUNCH = {1: 70400, 2: 244992, 3: 1202176, "3s": 334368, 4: 300544}   # "3s": mean of the 8 launches of a step
+PROFILED_DRAM_BYTES_PER_LAUNCH = {1: 70400, 2: 244992, 3: 1072640, "3s": 328320, 4: 207872}   # "3s": mean of the 8 launches of a step
 FP64_LANES_PER_SM = 64                        # B200 (sm_100): 64 FP64 FMA lanes per SM -> nominal peak
 
 
