@@ -329,7 +329,8 @@ int qmc_sector_compile(const double* params /*HOST*/, int n_params, int dim, uns
 /* ---- modules of specialised sector kernels ------------------------------------------------------------------------------
  * The paper's integrands are compiled functions (every sector is C++ source compiled for the GPU before the
  * integration starts).  A C ABI carries parameter blocks instead, which the default kernels interpret step by step; a MODULE
- * gives the compiled route back: qmc_sector_module_create translates every QMC_FAMILY_SECTOR problem of a batch into
+ * gives the compiled route back: qmc_sector_module_create translates every QMC_FAMILY_SECTOR and QMC_FAMILY_SECTOR_COMPLEX
+ * problem of a batch into
  * straight-line sm_100a code -- the same operations in the same order as the interpreting kernel, so both return the same bits --
  * inside copies of the fused kernel (up to `sectors_per_kernel` sectors per kernel; 0 = 32, doubled until the batch needs at most
  * 48 kernels; a batch call serves at most 64 kernel variants in all and returns QMC_ERR_WORKSPACE beyond),
